@@ -1,0 +1,246 @@
+"""ctypes wrapper around oracle/marut_oracle.cpp -- TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  It never imports paper_2605_26388_b200 and shares no
+code with it; inputs come from the neutral `workloads` module.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "marut_oracle.cpp")
+_LIB = os.path.join(_HERE, "libmarut_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c++17", "-shared", "-fPIC", _SRC, "-o", _LIB]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _MechDesc(C.Structure):
+    _fields_ = [("n_species", C.c_int), ("n_reac", C.c_int), ("T_mid", C.c_double),
+                ("W", C.c_void_p), ("nasa", C.c_void_p), ("nu_r", C.c_void_p), ("nu_p", C.c_void_p),
+                ("A", C.c_void_p), ("b", C.c_void_p), ("Ea", C.c_void_p)]
+
+
+class _MeshDesc(C.Structure):
+    _fields_ = [("dim", C.c_int), ("N", C.c_int), ("n_elem", C.c_long), ("node_xyz", C.c_void_p),
+                ("n_iface", C.c_long), ("iface", C.c_void_p), ("n_mortar", C.c_long), ("mortar", C.c_void_p),
+                ("n_bface", C.c_long), ("bface", C.c_void_p), ("n_bc", C.c_int), ("bc_state", C.c_void_p),
+                ("physics", C.c_int), ("gamma", C.c_double), ("mu", C.c_double), ("Pr", C.c_double),
+                ("mech", C.c_void_p)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        L = _lib
+        dp, vp = C.POINTER(C.c_double), C.c_void_p
+        L.oracle_mesh_create.restype = vp
+        L.oracle_mesh_create.argtypes = [vp]
+        L.oracle_mesh_destroy.argtypes = [vp]
+        L.oracle_nvar.argtypes = [vp]
+        L.oracle_dx_min.restype = C.c_double
+        L.oracle_dx_min.argtypes = [vp]
+        L.oracle_max_dt.restype = C.c_double
+        L.oracle_max_dt.argtypes = [vp, vp, C.c_double, vp]
+        L.oracle_run.restype = C.c_double
+        L.oracle_run.argtypes = [vp, vp, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp]
+        L.oracle_rhs.argtypes = [vp, vp, vp, C.c_double]
+        L.oracle_rhs_inviscid.argtypes = [vp, vp, vp]
+        L.oracle_rhs_viscous.argtypes = [vp, vp, vp]
+        L.oracle_br1_gradient.argtypes = [vp, vp, vp]
+        L.oracle_chem_source.argtypes = [vp, vp, vp]
+        L.oracle_metrics.argtypes = [vp, vp, vp]
+        L.oracle_primitives.argtypes = [vp, vp, vp]
+        L.oracle_ssprk_stage.argtypes = [vp, C.c_int, C.c_double, C.c_double, vp, vp, vp]
+        L.oracle_ssprk3_scalar.restype = C.c_double
+        L.oracle_ssprk3_scalar.argtypes = [C.c_double] * 5
+        L.oracle_operators.argtypes = [C.c_int, vp, vp, vp]
+        L.oracle_mortar_matrices.argtypes = [C.c_int, vp, vp, vp, vp]
+        L.oracle_rusanov.argtypes = [C.c_int, C.c_double, vp, vp, vp, vp, vp]
+        L.oracle_viscous_flux.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, vp, vp, vp, vp]
+        L.oracle_k_forward.restype = C.c_double
+        L.oracle_k_forward.argtypes = [vp, C.c_int, C.c_double]
+        L.oracle_k_equilibrium.restype = C.c_double
+        L.oracle_k_equilibrium.argtypes = [vp, C.c_int, C.c_double]
+        L.oracle_production_rates.argtypes = [vp, C.c_double, vp, vp]
+        L.oracle_temperature.restype = C.c_double
+        L.oracle_temperature.argtypes = [vp, vp, C.c_double]
+        L.oracle_species_thermo.argtypes = [vp, C.c_int, C.c_double, vp]
+        L.oracle_num_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None and a.size else None
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+class MechHandle:
+    """keeps the numpy arrays behind an oracle_mech_desc alive"""
+
+    def __init__(self, mech):
+        self.keep = [_f64(mech.W), _f64(mech.nasa), _i32(mech.nu_r), _i32(mech.nu_p), _f64(mech.A), _f64(mech.b), _f64(mech.Ea)]
+        k = self.keep
+        self.desc = _MechDesc(len(k[0]), len(k[4]), float(mech.T_mid), _p(k[0]), _p(k[1]), _p(k[2]), _p(k[3]), _p(k[4]), _p(k[5]), _p(k[6]))
+        self.ns = len(k[0])
+
+    @property
+    def ptr(self):
+        return C.addressof(self.desc)
+
+    def k_forward(self, r, T):
+        return lib().oracle_k_forward(self.ptr, r, T)
+
+    def k_equilibrium(self, r, T):
+        return lib().oracle_k_equilibrium(self.ptr, r, T)
+
+    def production_rates(self, T, rho_s):
+        rho_s = _f64(rho_s)
+        om = np.zeros(self.ns)
+        lib().oracle_production_rates(self.ptr, T, _p(rho_s), _p(om))
+        return om
+
+    def temperature(self, rho_s, e_int):
+        rho_s = _f64(rho_s)
+        return lib().oracle_temperature(self.ptr, _p(rho_s), e_int)
+
+    def species_thermo(self, s, T):
+        out = np.zeros(5)
+        lib().oracle_species_thermo(self.ptr, s, T, _p(out))
+        return dict(cp_R=out[0], h_RT=out[1], s_R=out[2], e=out[3], cv=out[4])
+
+
+class OracleMesh:
+    def __init__(self, mesh):
+        L = lib()
+        self.mesh = mesh
+        self._keep = [_f64(mesh.node_xyz), _i32(mesh.iface), _i32(mesh.mortar), _i32(mesh.bface), _f64(mesh.bc_state)]
+        k = self._keep
+        self._mech = MechHandle(mesh.mech) if mesh.mech is not None else None
+        d = _MeshDesc(mesh.dim, mesh.N, mesh.n_elem, _p(k[0]), len(k[1]), _p(k[1]), len(k[2]), _p(k[2]),
+                      len(k[3]), _p(k[3]), len(k[4]), _p(k[4]), mesh.physics, mesh.gamma, mesh.mu, mesh.Pr,
+                      self._mech.ptr if self._mech else None)
+        self.h = L.oracle_mesh_create(C.addressof(d))
+        self.nvar = L.oracle_nvar(self.h)
+        self.shape = (mesh.n_elem, self.nvar, mesh.nn)
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            lib().oracle_mesh_destroy(self.h)
+            self.h = None
+
+    @property
+    def dx_min(self):
+        return lib().oracle_dx_min(self.h)
+
+    def metrics(self):
+        m = self.mesh
+        Ja = np.zeros((m.n_elem, m.nn, m.dim, m.dim))
+        J = np.zeros((m.n_elem, m.nn))
+        lib().oracle_metrics(self.h, _p(Ja), _p(J))
+        return Ja, J
+
+    def _call(self, fn, u, *extra):
+        u = _f64(u)
+        out = np.zeros(self.shape)
+        fn(self.h, _p(u), _p(out), *extra)
+        return out
+
+    def rhs(self, u, t=0.0):
+        return self._call(lib().oracle_rhs, u, t)
+
+    def rhs_inviscid(self, u):
+        return self._call(lib().oracle_rhs_inviscid, u)
+
+    def rhs_viscous(self, u):
+        return self._call(lib().oracle_rhs_viscous, u)
+
+    def chem_source(self, u):
+        return self._call(lib().oracle_chem_source, u)
+
+    def br1_gradient(self, u):
+        m = self.mesh
+        u = _f64(u)
+        S = np.zeros((m.n_elem, m.nn, m.dim + 2, m.dim))
+        lib().oracle_br1_gradient(self.h, _p(u), _p(S))
+        return S
+
+    def primitives(self, U):
+        U = _f64(U)
+        out = np.zeros(7)
+        lib().oracle_primitives(self.h, _p(U), _p(out))
+        return dict(rho=out[0], p=out[1], a=out[2], T=out[3], vel=out[4:7].copy())
+
+    def ssprk_stage(self, stage, dt, t_n, u_n, u_in):
+        u_n, u_in = _f64(u_n), _f64(u_in)
+        out = np.zeros(self.shape)
+        lib().oracle_ssprk_stage(self.h, stage, dt, t_n, _p(u_n), _p(u_in), _p(out))
+        return out
+
+    def max_dt(self, u, cfl, return_lambda=False):
+        u = _f64(u)
+        lam = C.c_double(0.0)
+        dt = lib().oracle_max_dt(self.h, _p(u), cfl, C.addressof(lam))
+        return (dt, lam.value) if return_lambda else dt
+
+    def run(self, u, nsteps, cfl=0.5, dt=0.0, t0=0.0):
+        """advance a copy of u by nsteps SSPRK3 steps; returns (u, t_end, min_rho, min_p)"""
+        u = _f64(u).copy()
+        mr, mp = C.c_double(0.0), C.c_double(0.0)
+        t = lib().oracle_run(self.h, _p(u), nsteps, cfl, dt, t0, C.addressof(mr), C.addressof(mp))
+        return u, t, mr.value, mp.value
+
+
+def operators(N):
+    n = N + 1
+    x, w, D = np.zeros(n), np.zeros(n), np.zeros((n, n))
+    lib().oracle_operators(N, _p(x), _p(w), _p(D))
+    return x, w, D
+
+
+def mortar_matrices(N):
+    n = N + 1
+    M = [np.zeros((n, n)) for _ in range(4)]
+    lib().oracle_mortar_matrices(N, *[_p(a) for a in M])
+    return M  # Pf_lo, Pf_up, Pr_lo, Pr_up
+
+
+def rusanov(dim, gamma, Um, Up, nv):
+    Um, Up, nv = _f64(Um), _f64(Up), _f64(nv)
+    Fs = np.zeros(dim + 2)
+    lam = C.c_double(0.0)
+    lib().oracle_rusanov(dim, gamma, _p(Um), _p(Up), _p(nv), _p(Fs), C.addressof(lam))
+    return Fs, lam.value
+
+
+def viscous_flux(dim, gamma, mu, Pr, U, S, nv):
+    U, S, nv = _f64(U), _f64(S), _f64(nv)
+    F = np.zeros(dim + 2)
+    lib().oracle_viscous_flux(dim, gamma, mu, Pr, _p(U), _p(S), _p(nv), _p(F))
+    return F
+
+
+def ssprk3_scalar(y0, lam, c2, t0, dt):
+    return lib().oracle_ssprk3_scalar(y0, lam, c2, t0, dt)
+
+
+def num_threads():
+    return lib().oracle_num_threads()

@@ -1,0 +1,897 @@
+// ============================================================================
+// oracle/marut_oracle.cpp  --  TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, fp64 CPU restatement of the hot path of MARUT (arxiv 2605.26388):
+// the semi-discrete spectral-DG right-hand side for compressible Euler /
+// Navier-Stokes (BR1) / reacting Euler with a finite-rate chemistry source, the
+// SSP-RK33 stage update and the CFL time step.  It follows the paper step by
+// step (citations are PAPER.md line numbers) and the readings listed in
+// DESIGN.md section 3.  No blocking, no fusion, no reordering.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+// reference legs may build, load or call this file.  It shares no code, header,
+// table or constant generator with paper_2605_26388_b200/ (the CUDA path).
+//
+// Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC  (see oracle/__init__.py)
+// -ffp-contract=off: no FMA contraction, so every operation below is a single
+// IEEE-754 double operation in the order written.
+//
+// Parity pins: every function below is pinned by tests/test_oracle_*.py to
+// closed forms / invariants / paper-printed values;
+// none is "parity unpinned".
+//
+// Layouts (all row-major, last index fastest):
+//   node_xyz [e][c][node]     node = i + n*(j + n*k), n = N+1
+//   u, du    [e][v][node]     v = rho_1..rho_ns, rho*u_1..rho*u_d, E
+//   iface    [f][5] = eL,fL,eR,fR,orient      face f = 2*l + side
+//   mortar   [m][6] = eC,fC,eF_lo,eF_up,fF,orient   (2-D only)
+//   bface    [b][3] = e,f,bc_id ;  bc_state [bc][nvar]
+// ============================================================================
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#include <algorithm>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+constexpr double R_UNIVERSAL = 8.31446261815324;   // J/(mol K)
+constexpr double P_REF = 101325.0;                 // Pa, standard-state pressure of K_c
+constexpr int MAXV = 16;                           // max variables per node
+constexpr int MAXS = 8;                            // max species
+
+enum Physics { EULER = 0, NAVIER_STOKES = 1, REACTING_EULER = 2 };
+
+// ---------------------------------------------------------------------------
+// O1. One-dimensional operators on Legendre-Gauss-Lobatto nodes.
+// ---------------------------------------------------------------------------
+// Legendre polynomial P_N(x) and its derivative by the three-term recurrence
+//   (k+1) P_{k+1} = (2k+1) x P_k - k P_{k-1},   P'_{k+1} = P'_{k-1} + (2k+1) P_k.
+static void legendre(int N, double x, double &P, double &dP) {
+  double Pm = 1.0, dPm = 0.0;          // P_0
+  if (N == 0) { P = Pm; dP = dPm; return; }
+  double Pc = x, dPc = 1.0;            // P_1
+  for (int k = 1; k < N; ++k) {
+    double Pn = ((2.0 * k + 1.0) * x * Pc - k * Pm) / (k + 1.0);
+    double dPn = dPm + (2.0 * k + 1.0) * Pc;
+    Pm = Pc; dPm = dPc; Pc = Pn; dPc = dPn;
+  }
+  P = Pc; dP = dPc;
+}
+
+struct Ops {
+  int N = 0, n = 0;
+  std::vector<double> x, w, D;         // D[i*n+j] = l_j'(x_i)
+};
+
+// LGL nodes: x_0=-1, x_N=+1 and the roots of P'_N; w_j = 2/(N(N+1) P_N(x_j)^2);
+// D by barycentric weights, diagonal = -(sum of the off-diagonals of the row).
+static Ops make_ops(int N) {
+  Ops o; o.N = N; o.n = N + 1;
+  const int n = o.n;
+  o.x.assign(n, 0.0); o.w.assign(n, 0.0); o.D.assign(n * n, 0.0);
+  o.x[0] = -1.0; o.x[N] = 1.0;
+  const double PI = 3.14159265358979323846;
+  for (int j = 1; j < N; ++j) {
+    double x = -std::cos(PI * j / N);            // Chebyshev-Lobatto starting guess
+    for (int it = 0; it < 100; ++it) {
+      double P, dP; legendre(N, x, P, dP);
+      // Legendre ODE: (1-x^2) P'' = 2 x P' - N(N+1) P
+      double d2P = (2.0 * x * dP - N * (N + 1.0) * P) / (1.0 - x * x);
+      double dx = dP / d2P;
+      x -= dx;
+      if (std::fabs(dx) < 1e-16) break;
+    }
+    o.x[j] = x;
+  }
+  for (int j = 0; j < n; ++j) {
+    double P, dP; legendre(N, o.x[j], P, dP);
+    o.w[j] = 2.0 / (N * (N + 1.0) * P * P);
+  }
+  std::vector<double> lam(n, 1.0);
+  for (int j = 0; j < n; ++j) {
+    double prod = 1.0;
+    for (int k = 0; k < n; ++k) if (k != j) prod *= (o.x[j] - o.x[k]);
+    lam[j] = 1.0 / prod;
+  }
+  for (int i = 0; i < n; ++i) {
+    double s = 0.0;
+    for (int j = 0; j < n; ++j) if (j != i) {
+      o.D[i * n + j] = (lam[j] / lam[i]) / (o.x[i] - o.x[j]);
+      s += o.D[i * n + j];
+    }
+    o.D[i * n + i] = -s;
+  }
+  return o;
+}
+
+// value of the j-th Lagrange polynomial on nodes x[] at point y (product form)
+static double lagrange(const std::vector<double> &x, int j, double y) {
+  double v = 1.0;
+  for (size_t k = 0; k < x.size(); ++k) if ((int)k != j) v *= (y - x[k]) / (x[j] - x[k]);
+  return v;
+}
+
+// Gauss-Legendre nodes/weights with m points: roots of P_m, w = 2/((1-x^2) P_m'(x)^2)
+static void gauss_legendre(int m, std::vector<double> &g, std::vector<double> &wg) {
+  g.assign(m, 0.0); wg.assign(m, 0.0);
+  const double PI = 3.14159265358979323846;
+  for (int q = 0; q < m; ++q) {
+    double x = -std::cos(PI * (q + 0.75) / (m + 0.5));
+    for (int it = 0; it < 100; ++it) {
+      double P, dP; legendre(m, x, P, dP);
+      double dx = P / dP; x -= dx;
+      if (std::fabs(dx) < 1e-16) break;
+    }
+    double P, dP; legendre(m, x, P, dP);
+    g[q] = x; wg[q] = 2.0 / ((1.0 - x * x) * dP * dP);
+  }
+}
+
+// ---------------------------------------------------------------------------
+// O7. 2:1 mortar projection matrices, reading R7.
+// Coarse face parameter z in [-1,1]; "lo" mortar covers [-1,0], "up" covers [0,1].
+//   P_fwd^lo[i][j] = l_j((x_i-1)/2),  P_fwd^up[i][j] = l_j((x_i+1)/2)
+//   P_rev^m = exact L2 projection of the piecewise (lo,up) data onto degree-N
+//   polynomials on the coarse face, via Legendre coefficients with (N+1)-point
+//   Gauss quadrature, evaluated at the LGL nodes.
+// ---------------------------------------------------------------------------
+static void make_mortar(const Ops &o, std::vector<double> Pf[2], std::vector<double> Pr[2]) {
+  const int n = o.n, N = o.N;
+  std::vector<double> g, wg; gauss_legendre(n, g, wg);
+  for (int m = 0; m < 2; ++m) {
+    const double shift = (m == 0) ? -1.0 : 1.0;
+    Pf[m].assign(n * n, 0.0); Pr[m].assign(n * n, 0.0);
+    for (int i = 0; i < n; ++i)
+      for (int j = 0; j < n; ++j) Pf[m][i * n + j] = lagrange(o.x, j, (o.x[i] + shift) / 2.0);
+    for (int i = 0; i < n; ++i)
+      for (int j = 0; j < n; ++j) {
+        double acc = 0.0;
+        for (int k = 0; k <= N; ++k) {
+          // q_k = (2k+1)/2 * 1/2 * int_{-1}^{1} l_j(eta) L_k((eta+shift)/2) d eta
+          double integ = 0.0;
+          for (int q = 0; q < n; ++q) {
+            double Lk, dLk; legendre(k, (g[q] + shift) / 2.0, Lk, dLk);
+            integ += wg[q] * lagrange(o.x, j, g[q]) * Lk;
+          }
+          double Lki, dLki; legendre(k, o.x[i], Lki, dLki);
+          acc += Lki * (2.0 * k + 1.0) / 2.0 * 0.5 * integ;
+        }
+        Pr[m][i * n + j] = acc;
+      }
+  }
+}
+
+// ---------------------------------------------------------------------------
+// O12. Thermochemistry; single temperature.
+// ---------------------------------------------------------------------------
+struct Mech {
+  int ns = 0, nr = 0;
+  double T_mid = 1000.0;
+  std::vector<double> W;        // [ns] kg/mol
+  std::vector<double> nasa;     // [ns][2][7] (low range, then high range)
+  std::vector<int> nu_r, nu_p;  // [nr][ns]  nu' (reactants), nu'' (products)
+  std::vector<double> A, b, Ea; // [nr]   k_f = A T^b exp(-Ea/T); A in cm^3-mol-s units, Ea in K
+};
+
+static const double *nasa_range(const Mech &m, int s, double T) {
+  return &m.nasa[(s * 2 + (T < m.T_mid ? 0 : 1)) * 7];
+}
+// NASA-7: cp/R = a1 + a2 T + a3 T^2 + a4 T^3 + a5 T^4
+static double cp_over_R(const Mech &m, int s, double T) {
+  const double *a = nasa_range(m, s, T);
+  return a[0] + a[1] * T + a[2] * T * T + a[3] * T * T * T + a[4] * T * T * T * T;
+}
+// h/(RT) = a1 + a2 T/2 + a3 T^2/3 + a4 T^3/4 + a5 T^4/5 + a6/T
+static double h_over_RT(const Mech &m, int s, double T) {
+  const double *a = nasa_range(m, s, T);
+  return a[0] + a[1] * T / 2.0 + a[2] * T * T / 3.0 + a[3] * T * T * T / 4.0 +
+         a[4] * T * T * T * T / 5.0 + a[5] / T;
+}
+// s/R = a1 ln T + a2 T + a3 T^2/2 + a4 T^3/3 + a5 T^4/4 + a7
+static double s_over_R(const Mech &m, int s, double T) {
+  const double *a = nasa_range(m, s, T);
+  return a[0] * std::log(T) + a[1] * T + a[2] * T * T / 2.0 + a[3] * T * T * T / 3.0 +
+         a[4] * T * T * T * T / 4.0 + a[6];
+}
+// specific internal energy e_s = h_s - R_s T (formation enthalpy inside h_s) [J/kg]
+static double e_species(const Mech &m, int s, double T) {
+  double Rs = R_UNIVERSAL / m.W[s];
+  return Rs * T * (h_over_RT(m, s, T) - 1.0);
+}
+static double cv_species(const Mech &m, int s, double T) {
+  double Rs = R_UNIVERSAL / m.W[s];
+  return Rs * (cp_over_R(m, s, T) - 1.0);
+}
+// Newton on f(T) = sum_s rho_s e_s(T) - e_int = 0, f' = sum_s rho_s cv_s(T)
+// (PAPER.md:288(i)); start 4000 K, stop |dT| <= 1e-13 T, cap 50 (R12).
+static double temperature_from_energy(const Mech &m, const double *rho_s, double e_int) {
+  double T = 4000.0;
+  for (int it = 0; it < 50; ++it) {
+    double f = -e_int, df = 0.0;
+    for (int s = 0; s < m.ns; ++s) { f += rho_s[s] * e_species(m, s, T); df += rho_s[s] * cv_species(m, s, T); }
+    double dT = f / df;
+    T -= dT;
+    if (std::fabs(dT) <= 1e-13 * T) break;
+  }
+  return T;
+}
+// forward rate constant, modified Arrhenius (eq. 6 with T_a = T)
+static double k_forward(const Mech &m, int r, double T) {
+  return m.A[r] * std::pow(T, m.b[r]) * std::exp(-m.Ea[r] / T);
+}
+// equilibrium constant in concentration units of mol/cm^3 (R12):
+//   K_c = exp(-sum_s dnu_s g_s/(R_u T)) * (p_ref/(R_u T) * 1e-6)^(sum_s dnu_s),
+//   g_s/(R_u T) = h_s/(R_u T) - s_s/R_u
+static double k_equilibrium(const Mech &m, int r, double T) {
+  double dG = 0.0; int dnu = 0;
+  for (int s = 0; s < m.ns; ++s) {
+    int d = m.nu_p[r * m.ns + s] - m.nu_r[r * m.ns + s];
+    if (d != 0) { dG += d * (h_over_RT(m, s, T) - s_over_R(m, s, T)); dnu += d; }
+  }
+  double c0 = P_REF / (R_UNIVERSAL * T) * 1.0e-6;   // mol/cm^3
+  double f = 1.0;
+  for (int k = 0; k < std::abs(dnu); ++k) f *= c0;
+  if (dnu < 0) f = 1.0 / f;
+  return std::exp(-dG) * f;
+}
+// net molar rate of reaction r (eq. 21), concentrations [X_s] = rho_s/W_s in mol/cm^3
+static double reaction_rate(const Mech &m, int r, double T, const double *X) {
+  double kf = k_forward(m, r, T);
+  double kb = kf / k_equilibrium(m, r, T);
+  double pf = 1.0, pb = 1.0;
+  for (int s = 0; s < m.ns; ++s) {
+    for (int k = 0; k < m.nu_r[r * m.ns + s]; ++k) pf *= X[s];
+    for (int k = 0; k < m.nu_p[r * m.ns + s]; ++k) pb *= X[s];
+  }
+  return kf * pf - kb * pb;
+}
+// species mass production rates (eq. 22), kg/(m^3 s)
+static void production_rates(const Mech &m, double T, const double *rho_s, double *omega) {
+  double X[MAXS];
+  for (int s = 0; s < m.ns; ++s) { X[s] = rho_s[s] / m.W[s] * 1.0e-6; omega[s] = 0.0; }
+  for (int r = 0; r < m.nr; ++r) {
+    double Rr = reaction_rate(m, r, T, X);
+    for (int s = 0; s < m.ns; ++s) omega[s] += (m.nu_p[r * m.ns + s] - m.nu_r[r * m.ns + s]) * Rr;
+  }
+  for (int s = 0; s < m.ns; ++s) omega[s] = m.W[s] * omega[s] * 1.0e6;
+}
+
+// ---------------------------------------------------------------------------
+// Mesh + geometry
+// ---------------------------------------------------------------------------
+struct Mesh {
+  int dim = 0, N = 0, n = 0, nn = 0, nvar = 0, ns = 1, physics = EULER;
+  long ne = 0;
+  Ops ops;
+  std::vector<double> xyz;      // [e][c][node]
+  std::vector<double> Ja;       // [e][node][l][c]  contravariant vectors J a^l
+  std::vector<double> J;        // [e][node]
+  std::vector<int> iface, mortar, bface;
+  std::vector<double> bc_state;
+  double gamma = 1.4, mu = 0.0, Pr = 0.72;
+  Mech mech;
+  std::vector<double> Pf[2], Pr_[2];
+  double dx_min = 0.0;
+};
+
+static inline int node_index(const Mesh &m, const int *ijk) {
+  int idx = 0;
+  for (int c = m.dim - 1; c >= 0; --c) idx = idx * m.n + ijk[c];
+  return idx;
+}
+static inline void node_ijk(const Mesh &m, int node, int *ijk) {
+  for (int c = 0; c < m.dim; ++c) { ijk[c] = node % m.n; node /= m.n; }
+}
+// derivative along reference direction l of a nodal field f[node] at node `node`
+static double dxi(const Mesh &m, const double *f, int node, int l) {
+  int ijk[3]; node_ijk(m, node, ijk);
+  const int il = ijk[l];
+  double s = 0.0;
+  for (int q = 0; q < m.n; ++q) {
+    ijk[l] = q;
+    s += m.ops.D[il * m.n + q] * f[node_index(m, ijk)];
+  }
+  return s;
+}
+// volume-node index of face node `a` (a = a0 + n*a1) of face f = 2*l + side:
+// the index along l is 0 (side 0) or N (side 1); the remaining directions, in
+// increasing order, take a0 (and a1).
+static int face_node(const Mesh &m, int f, int a) {
+  int l = f / 2, side = f % 2, ijk[3] = {0, 0, 0};
+  int t = 0;
+  for (int c = 0; c < m.dim; ++c) {
+    if (c == l) ijk[c] = side ? m.N : 0;
+    else { ijk[c] = (t == 0) ? (a % m.n) : (a / m.n); ++t; }
+  }
+  return node_index(m, ijk);
+}
+// partner face-node index under `orient` (2-D: 1 = reversed; 3-D: only 0)
+static int orient_map(const Mesh &m, int a, int orient) {
+  if (orient == 0) return a;
+  return m.N - a;     // 2-D flipped
+}
+
+// O2. Metric terms.
+//  2-D: Ja^1 = (y_eta, -x_eta), Ja^2 = (-y_xi, x_xi), J = x_xi y_eta - x_eta y_xi.
+//  3-D: conservative curl form (R2):
+//    (Ja^i)_n = d_{xi_k}[X_l d_{xi_j} X_m] - d_{xi_j}[X_l d_{xi_k} X_m],
+//    (i,j,k) cyclic, (n,m,l) cyclic;  J = X_xi . (X_eta x X_zeta).
+static void compute_metrics(Mesh &m) {
+  const int nn = m.nn, d = m.dim;
+  m.Ja.assign((size_t)m.ne * nn * d * d, 0.0);
+  m.J.assign((size_t)m.ne * nn, 0.0);
+#pragma omp parallel for schedule(static)
+  for (long e = 0; e < m.ne; ++e) {
+    const double *X[3] = {nullptr, nullptr, nullptr};
+    for (int c = 0; c < d; ++c) X[c] = &m.xyz[((size_t)e * d + c) * nn];
+    double *Ja = &m.Ja[(size_t)e * nn * d * d];
+    double *J = &m.J[(size_t)e * nn];
+    if (d == 2) {
+      for (int p = 0; p < nn; ++p) {
+        double x_xi = dxi(m, X[0], p, 0), x_eta = dxi(m, X[0], p, 1);
+        double y_xi = dxi(m, X[1], p, 0), y_eta = dxi(m, X[1], p, 1);
+        Ja[(p * 2 + 0) * 2 + 0] = y_eta;  Ja[(p * 2 + 0) * 2 + 1] = -x_eta;
+        Ja[(p * 2 + 1) * 2 + 0] = -y_xi;  Ja[(p * 2 + 1) * 2 + 1] = x_xi;
+        J[p] = x_xi * y_eta - x_eta * y_xi;
+      }
+    } else {
+      std::vector<double> dX(9 * nn);            // dX[(c*3+l)*nn+p] = d X_c / d xi_l
+      for (int c = 0; c < 3; ++c)
+        for (int l = 0; l < 3; ++l)
+          for (int p = 0; p < nn; ++p) dX[(c * 3 + l) * nn + p] = dxi(m, X[c], p, l);
+      for (int p = 0; p < nn; ++p) {
+        const double *g = &dX[0];
+        auto G = [&](int c, int l) { return g[(c * 3 + l) * nn + p]; };
+        J[p] = G(0, 0) * (G(1, 1) * G(2, 2) - G(1, 2) * G(2, 1)) -
+               G(0, 1) * (G(1, 0) * G(2, 2) - G(1, 2) * G(2, 0)) +
+               G(0, 2) * (G(1, 0) * G(2, 1) - G(1, 1) * G(2, 0));
+      }
+      std::vector<double> A(nn), B(nn);
+      for (int i = 0; i < 3; ++i) {
+        const int j = (i + 1) % 3, k = (i + 2) % 3;
+        for (int c = 0; c < 3; ++c) {            // Cartesian component n = c
+          const int mm = (c + 1) % 3, ll = (c + 2) % 3;
+          for (int p = 0; p < nn; ++p) {
+            A[p] = X[ll][p] * dX[(mm * 3 + j) * nn + p];   // X_l d_{xi_j} X_m
+            B[p] = X[ll][p] * dX[(mm * 3 + k) * nn + p];   // X_l d_{xi_k} X_m
+          }
+          for (int p = 0; p < nn; ++p)
+            Ja[(p * 3 + i) * 3 + c] = dxi(m, A.data(), p, k) - dxi(m, B.data(), p, j);
+        }
+      }
+    }
+  }
+  // O11: characteristic element size dx_e = 2 (min_i J_i)^(1/d); dx_min = min_e
+  double dxm = 1e300;
+  for (long e = 0; e < m.ne; ++e) {
+    double Jmin = 1e300;
+    for (int p = 0; p < nn; ++p) Jmin = std::min(Jmin, m.J[(size_t)e * nn + p]);
+    double dx = 2.0 * std::pow(Jmin, 1.0 / d);
+    dxm = std::min(dxm, dx);
+  }
+  m.dx_min = dxm;
+}
+
+// ---------------------------------------------------------------------------
+// O3. State -> primitives.
+// ---------------------------------------------------------------------------
+struct Prim {
+  double rho, vel[3], p, a, T;
+};
+static Prim primitives(const Mesh &m, const double *U) {
+  Prim q; q.vel[0] = q.vel[1] = q.vel[2] = 0.0;
+  const int ns = m.ns, d = m.dim;
+  double rho = 0.0;
+  for (int s = 0; s < ns; ++s) rho += U[s];
+  q.rho = rho;
+  double ke = 0.0;
+  for (int c = 0; c < d; ++c) { q.vel[c] = U[ns + c] / rho; ke += q.vel[c] * q.vel[c]; }
+  ke = 0.5 * rho * ke;
+  const double E = U[ns + d];
+  if (m.physics == REACTING_EULER) {
+    const Mech &k = m.mech;
+    q.T = temperature_from_energy(k, U, E - ke);
+    double R = 0.0, cp = 0.0;                       // mixture gas constant, frozen cp
+    for (int s = 0; s < ns; ++s) {
+      double Ys = U[s] / rho, Rs = R_UNIVERSAL / k.W[s];
+      R += Ys * Rs; cp += Ys * Rs * cp_over_R(k, s, q.T);
+    }
+    q.p = rho * R * q.T;                            // p = rho R T
+    double gf = cp / (cp - R);                      // frozen gamma (R12)
+    q.a = std::sqrt(gf * R * q.T);
+  } else {
+    q.p = (m.gamma - 1.0) * (E - ke);
+    q.a = std::sqrt(m.gamma * q.p / rho);
+    q.T = q.p / rho;                                // R = 1
+  }
+  return q;
+}
+// inviscid flux contracted with a (scaled) vector nv: F_inv(U) . nv
+static void flux_dot(const Mesh &m, const double *U, const Prim &q, const double *nv, double *F) {
+  const int ns = m.ns, d = m.dim;
+  double vn = 0.0;
+  for (int c = 0; c < d; ++c) vn += q.vel[c] * nv[c];
+  for (int s = 0; s < ns; ++s) F[s] = U[s] * vn;
+  for (int c = 0; c < d; ++c) F[ns + c] = U[ns + c] * vn + q.p * nv[c];
+  F[ns + d] = (U[ns + d] + q.p) * vn;
+}
+// O5. Local Lax-Friedrichs / Rusanov flux with scaled outward normal nv:
+//   F* = 1/2 (F(U-)+F(U+)).nv - 1/2 lambda |nv| (U+ - U-),
+//   lambda = max(|v-.nhat| + a-, |v+.nhat| + a+),  nhat = nv/|nv|.
+static void rusanov(const Mesh &m, const double *Um, const double *Up, const double *nv, double *Fs) {
+  const int d = m.dim, nv_ = m.nvar;
+  Prim qm = primitives(m, Um), qp = primitives(m, Up);
+  double nrm = 0.0;
+  for (int c = 0; c < d; ++c) nrm += nv[c] * nv[c];
+  nrm = std::sqrt(nrm);
+  double vnm = 0.0, vnp = 0.0;
+  for (int c = 0; c < d; ++c) { vnm += qm.vel[c] * (nv[c] / nrm); vnp += qp.vel[c] * (nv[c] / nrm); }
+  double lam = std::max(std::fabs(vnm) + qm.a, std::fabs(vnp) + qp.a);
+  double Fm[MAXV], Fp[MAXV];
+  flux_dot(m, Um, qm, nv, Fm); flux_dot(m, Up, qp, nv, Fp);
+  for (int v = 0; v < nv_; ++v) Fs[v] = 0.5 * (Fm[v] + Fp[v]) - 0.5 * lam * nrm * (Up[v] - Um[v]);
+}
+
+static inline void gather(const Mesh &m, const double *u, long e, int node, double *U) {
+  for (int v = 0; v < m.nvar; ++v) U[v] = u[((size_t)e * m.nvar + v) * m.nn + node];
+}
+// outward scaled normal of face f at volume node `node` of element e:  n_ref * Ja^{l_f}
+static inline void face_normal(const Mesh &m, long e, int f, int node, double *nv) {
+  const int l = f / 2; const double sgn = (f % 2) ? 1.0 : -1.0;
+  const double *Ja = &m.Ja[((size_t)e * m.nn + node) * m.dim * m.dim + l * m.dim];
+  for (int c = 0; c < m.dim; ++c) nv[c] = sgn * Ja[c];
+}
+
+// ---------------------------------------------------------------------------
+// O4 + O6. Inviscid residual: volume term (eq. 9) and surface lift (eq. 12).
+// ---------------------------------------------------------------------------
+static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
+  const int nn = m.nn, d = m.dim, nvar = m.nvar, n = m.n;
+  // --- volume: R_i = -(1/J_i) sum_l sum_m D_{i_l m} Ftilde^l_m,  Ftilde^l = Ja^l . F_inv
+#pragma omp parallel for schedule(static)
+  for (long e = 0; e < m.ne; ++e) {
+    std::vector<double> Ft((size_t)d * nvar * nn);      // [l][v][node]
+    for (int p = 0; p < nn; ++p) {
+      double U[MAXV], F[MAXV]; gather(m, u, e, p, U);
+      Prim q = primitives(m, U);
+      for (int l = 0; l < d; ++l) {
+        const double *Ja = &m.Ja[((size_t)e * nn + p) * d * d + l * d];
+        flux_dot(m, U, q, Ja, F);
+        for (int v = 0; v < nvar; ++v) Ft[((size_t)l * nvar + v) * nn + p] = F[v];
+      }
+    }
+    for (int v = 0; v < nvar; ++v)
+      for (int p = 0; p < nn; ++p) {
+        double s = 0.0;
+        for (int l = 0; l < d; ++l) s += dxi(m, &Ft[((size_t)l * nvar + v) * nn], p, l);
+        du[((size_t)e * nvar + v) * nn + p] = -s / m.J[(size_t)e * nn + p];
+      }
+  }
+  const int nf = (d == 2) ? n : n * n;                  // nodes per face
+  const double wb = m.ops.w[0];                         // LGL weight of the boundary index (w_0 = w_N)
+  auto lift = [&](long e, int node, const double *Fstar, const double *Fown) {
+    const double Jn = m.J[(size_t)e * nn + node];
+    for (int v = 0; v < nvar; ++v) du[((size_t)e * nvar + v) * nn + node] -= (Fstar[v] - Fown[v]) / (Jn * wb);
+  };
+  // --- conforming interfaces (O5/O6): one flux per face node with the L-side normal
+  for (size_t f = 0; f < m.iface.size() / 5; ++f) {
+    const int *I = &m.iface[f * 5];
+    const long eL = I[0], eR = I[2]; const int fL = I[1], fR = I[3], orient = I[4];
+    for (int a = 0; a < nf; ++a) {
+      const int pL = face_node(m, fL, a), pR = face_node(m, fR, orient_map(m, a, orient));
+      double Um[MAXV], Up[MAXV], nL[3], nR[3], Fs[MAXV], Fo[MAXV], mFs[MAXV];
+      gather(m, u, eL, pL, Um); gather(m, u, eR, pR, Up);
+      face_normal(m, eL, fL, pL, nL); face_normal(m, eR, fR, pR, nR);
+      rusanov(m, Um, Up, nL, Fs);
+      flux_dot(m, Um, primitives(m, Um), nL, Fo);   lift(eL, pL, Fs, Fo);
+      for (int v = 0; v < nvar; ++v) mFs[v] = -Fs[v];
+      flux_dot(m, Up, primitives(m, Up), nR, Fo);   lift(eR, pR, mFs, Fo);
+    }
+  }
+  // --- 2:1 mortars (O7), 2-D only
+  for (size_t q = 0; q < m.mortar.size() / 6; ++q) {
+    const int *M = &m.mortar[q * 6];
+    const long eC = M[0]; const int fC = M[1], fF = M[4];
+    std::vector<double> UC((size_t)n * nvar), FC((size_t)n * nvar, 0.0);
+    for (int j = 0; j < n; ++j) gather(m, u, eC, face_node(m, fC, j), &UC[(size_t)j * nvar]);
+    for (int s = 0; s < 2; ++s) {
+      const long eF = M[2 + s];
+      for (int a = 0; a < n; ++a) {
+        const int pF = face_node(m, fF, a);
+        double UF[MAXV], Ui[MAXV], nF[3], Fs[MAXV], Fo[MAXV];
+        gather(m, u, eF, pF, UF);
+        for (int v = 0; v < nvar; ++v) {            // coarse trace interpolated to the mortar
+          double acc = 0.0;
+          for (int j = 0; j < n; ++j) acc += m.Pf[s][a * n + j] * UC[(size_t)j * nvar + v];
+          Ui[v] = acc;
+        }
+        face_normal(m, eF, fF, pF, nF);
+        rusanov(m, UF, Ui, nF, Fs);                 // fine-side normal, fine-side quadrature
+        flux_dot(m, UF, primitives(m, UF), nF, Fo);  lift(eF, pF, Fs, Fo);
+        // coarse side: outward flux on the mortar is -F*; area ratio 2
+        for (int i = 0; i < n; ++i)
+          for (int v = 0; v < nvar; ++v) FC[(size_t)i * nvar + v] += m.Pr_[s][i * n + a] * (2.0 * (-Fs[v]));
+      }
+    }
+    for (int i = 0; i < n; ++i) {
+      const int pC = face_node(m, fC, i);
+      double nC[3], Fo[MAXV];
+      face_normal(m, eC, fC, pC, nC);
+      flux_dot(m, &UC[(size_t)i * nvar], primitives(m, &UC[(size_t)i * nvar]), nC, Fo);
+      lift(eC, pC, &FC[(size_t)i * nvar], Fo);
+    }
+  }
+  // --- boundary faces (O8): exterior state prescribed
+  for (size_t b = 0; b < m.bface.size() / 3; ++b) {
+    const long e = m.bface[b * 3]; const int f = m.bface[b * 3 + 1], bc = m.bface[b * 3 + 2];
+    for (int a = 0; a < nf; ++a) {
+      const int p = face_node(m, f, a);
+      double Um[MAXV], nv[3], Fs[MAXV], Fo[MAXV];
+      gather(m, u, e, p, Um); face_normal(m, e, f, p, nv);
+      rusanov(m, Um, &m.bc_state[(size_t)bc * nvar], nv, Fs);
+      flux_dot(m, Um, primitives(m, Um), nv, Fo);   lift(e, p, Fs, Fo);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------
+// O9. BR1 viscous residual; conforming faces only.
+// W = (rho, u_1..u_d, T), T = p/rho.  S[e][node][w][c] = d W_w / d x_c.
+// ---------------------------------------------------------------------------
+static void prim_gradient_vars(const Mesh &m, const double *U, double *W) {
+  Prim q = primitives(m, U);
+  W[0] = q.rho;
+  for (int c = 0; c < m.dim; ++c) W[1 + c] = q.vel[c];
+  W[1 + m.dim] = q.T;
+}
+// viscous flux F_v(U,S) contracted with vector nv (eq. 15, q = -k grad T)
+static void viscous_flux_dot(const Mesh &m, const double *U, const double *S, const double *nv, double *F) {
+  const int d = m.dim;
+  Prim q = primitives(m, U);
+  const double mu = m.mu, k = m.gamma * mu / (m.Pr * (m.gamma - 1.0));
+  // S[w*d + c]; velocity gradient dv[i][j] = d u_i / d x_j
+  double divu = 0.0;
+  for (int i = 0; i < d; ++i) divu += S[(1 + i) * d + i];
+  double tau[3][3];
+  for (int i = 0; i < d; ++i)
+    for (int j = 0; j < d; ++j) {
+      if (i == j) {
+        double others = divu - S[(1 + i) * d + i];
+        tau[i][j] = 4.0 / 3.0 * mu * S[(1 + i) * d + i] - 2.0 / 3.0 * mu * others;
+      } else tau[i][j] = mu * (S[(1 + i) * d + j] + S[(1 + j) * d + i]);
+    }
+  F[0] = 0.0;
+  double Fe = 0.0;
+  for (int j = 0; j < d; ++j) {            // direction j of the flux, contracted with nv[j]
+    double work = 0.0;
+    for (int i = 0; i < d; ++i) work += q.vel[i] * tau[i][j];
+    double qj = -k * S[(1 + d) * d + j];
+    Fe += (work - qj) * nv[j];
+  }
+  for (int i = 0; i < d; ++i) {
+    double s = 0.0;
+    for (int j = 0; j < d; ++j) s += tau[i][j] * nv[j];
+    F[1 + i] = s;
+  }
+  F[1 + d] = Fe;
+}
+static void br1_gradient(const Mesh &m, const double *u, std::vector<double> &S) {
+  const int nn = m.nn, d = m.dim, nw = d + 2, n = m.n;
+  S.assign((size_t)m.ne * nn * nw * d, 0.0);
+#pragma omp parallel for schedule(static)
+  for (long e = 0; e < m.ne; ++e) {
+    std::vector<double> W((size_t)nw * nn), G(nn);
+    for (int p = 0; p < nn; ++p) {
+      double U[MAXV], Wp[MAXV]; gather(m, u, e, p, U); prim_gradient_vars(m, U, Wp);
+      for (int w = 0; w < nw; ++w) W[(size_t)w * nn + p] = Wp[w];
+    }
+    for (int w = 0; w < nw; ++w)
+      for (int c = 0; c < d; ++c) {
+        // volume part: sum_l D_l( (Ja^l)_c W )
+        std::vector<double> acc(nn, 0.0);
+        for (int l = 0; l < d; ++l) {
+          for (int p = 0; p < nn; ++p) G[p] = m.Ja[((size_t)e * nn + p) * d * d + l * d + c] * W[(size_t)w * nn + p];
+          for (int p = 0; p < nn; ++p) acc[p] += dxi(m, G.data(), p, l);
+        }
+        for (int p = 0; p < nn; ++p) S[(((size_t)e * nn + p) * nw + w) * d + c] = acc[p];
+      }
+  }
+  const int nf = (d == 2) ? n : n * n;
+  const double wb = m.ops.w[0];
+  // surface part: + (1/w_b) (What - W) n_c with What = 1/2 (W- + W+) (eq. 13)
+  for (size_t f = 0; f < m.iface.size() / 5; ++f) {
+    const int *I = &m.iface[f * 5];
+    const long eL = I[0], eR = I[2]; const int fL = I[1], fR = I[3], orient = I[4];
+    for (int a = 0; a < nf; ++a) {
+      const int pL = face_node(m, fL, a), pR = face_node(m, fR, orient_map(m, a, orient));
+      double Um[MAXV], Up[MAXV], Wm[MAXV], Wp[MAXV], nL[3], nR[3];
+      gather(m, u, eL, pL, Um); gather(m, u, eR, pR, Up);
+      prim_gradient_vars(m, Um, Wm); prim_gradient_vars(m, Up, Wp);
+      face_normal(m, eL, fL, pL, nL); face_normal(m, eR, fR, pR, nR);
+      for (int w = 0; w < nw; ++w) {
+        double What = 0.5 * (Wm[w] + Wp[w]);
+        for (int c = 0; c < d; ++c) {
+          S[(((size_t)eL * nn + pL) * nw + w) * d + c] += (What - Wm[w]) * nL[c] / wb;
+          S[(((size_t)eR * nn + pR) * nw + w) * d + c] += (What - Wp[w]) * nR[c] / wb;
+        }
+      }
+    }
+  }
+  // rescale by the inverse Jacobian
+  for (long e = 0; e < m.ne; ++e)
+    for (int p = 0; p < nn; ++p)
+      for (int k = 0; k < nw * d; ++k) S[((size_t)e * nn + p) * nw * d + k] /= m.J[(size_t)e * nn + p];
+}
+static void rhs_viscous_add(const Mesh &m, const double *u, double *du) {
+  const int nn = m.nn, d = m.dim, nvar = m.nvar, nw = d + 2, n = m.n;
+  std::vector<double> S; br1_gradient(m, u, S);
+  // volume: + (1/J) sum_l D_l (Ja^l . F_v)
+#pragma omp parallel for schedule(static)
+  for (long e = 0; e < m.ne; ++e) {
+    std::vector<double> Ft((size_t)d * nvar * nn);
+    for (int p = 0; p < nn; ++p) {
+      double U[MAXV], F[MAXV]; gather(m, u, e, p, U);
+      for (int l = 0; l < d; ++l) {
+        const double *Ja = &m.Ja[((size_t)e * nn + p) * d * d + l * d];
+        viscous_flux_dot(m, U, &S[((size_t)e * nn + p) * nw * d], Ja, F);
+        for (int v = 0; v < nvar; ++v) Ft[((size_t)l * nvar + v) * nn + p] = F[v];
+      }
+    }
+    for (int v = 0; v < nvar; ++v)
+      for (int p = 0; p < nn; ++p) {
+        double s = 0.0;
+        for (int l = 0; l < d; ++l) s += dxi(m, &Ft[((size_t)l * nvar + v) * nn], p, l);
+        du[((size_t)e * nvar + v) * nn + p] += s / m.J[(size_t)e * nn + p];
+      }
+  }
+  // surface: + (1/(J w_b)) (F_v* - F_v) . n,  F_v* = 1/2 (F_v(U-,S-) + F_v(U+,S+)) (eq. 16)
+  const int nf = (d == 2) ? n : n * n;
+  const double wb = m.ops.w[0];
+  for (size_t f = 0; f < m.iface.size() / 5; ++f) {
+    const int *I = &m.iface[f * 5];
+    const long eL = I[0], eR = I[2]; const int fL = I[1], fR = I[3], orient = I[4];
+    for (int a = 0; a < nf; ++a) {
+      const int pL = face_node(m, fL, a), pR = face_node(m, fR, orient_map(m, a, orient));
+      double Um[MAXV], Up[MAXV], nL[3], nR[3], FmL[MAXV], FpL[MAXV], FpR[MAXV];
+      gather(m, u, eL, pL, Um); gather(m, u, eR, pR, Up);
+      face_normal(m, eL, fL, pL, nL); face_normal(m, eR, fR, pR, nR);
+      const double *Sm = &S[((size_t)eL * nn + pL) * nw * d], *Sp = &S[((size_t)eR * nn + pR) * nw * d];
+      viscous_flux_dot(m, Um, Sm, nL, FmL); viscous_flux_dot(m, Up, Sp, nL, FpL);
+      viscous_flux_dot(m, Up, Sp, nR, FpR);
+      const double JL = m.J[(size_t)eL * nn + pL], JR = m.J[(size_t)eR * nn + pR];
+      for (int v = 0; v < nvar; ++v) {
+        double Fstar = 0.5 * (FmL[v] + FpL[v]);        // single-valued, L-side normal
+        du[((size_t)eL * nvar + v) * nn + pL] += (Fstar - FmL[v]) / (JL * wb);
+        du[((size_t)eR * nvar + v) * nn + pR] += (-Fstar - FpR[v]) / (JR * wb);
+      }
+    }
+  }
+}
+// K7/a9: chemistry source added per node (eq. 20 without the E_v row)
+static void chem_source(const Mesh &m, const double *u, double *s, bool accumulate) {
+  const int nn = m.nn, nvar = m.nvar, ns = m.ns;
+#pragma omp parallel for schedule(static)
+  for (long e = 0; e < m.ne; ++e)
+    for (int p = 0; p < nn; ++p) {
+      double U[MAXV], om[MAXS]; gather(m, u, e, p, U);
+      Prim q = primitives(m, U);
+      production_rates(m.mech, q.T, U, om);
+      for (int v = 0; v < nvar; ++v) {
+        double val = (v < ns) ? om[v] : 0.0;
+        size_t idx = ((size_t)e * nvar + v) * nn + p;
+        if (accumulate) s[idx] += val; else s[idx] = val;
+      }
+    }
+}
+// the semi-discrete operator L(U,t); t unused (no time-dependent BC/source)
+static void rhs_full(const Mesh &m, const double *u, double *du) {
+  rhs_inviscid(m, u, du);
+  if (m.physics == NAVIER_STOKES) rhs_viscous_add(m, u, du);
+  if (m.physics == REACTING_EULER) chem_source(m, u, du, true);
+}
+// O11. time step: dt = min(dt_C, dt_D)
+static double max_dt(const Mesh &m, const double *u, double cfl, double *lam_out) {
+  double lam = 0.0, nu = 0.0;
+  for (long e = 0; e < m.ne; ++e)
+    for (int p = 0; p < m.nn; ++p) {
+      double U[MAXV]; gather(m, u, e, p, U);
+      Prim q = primitives(m, U);
+      double v2 = 0.0;
+      for (int c = 0; c < m.dim; ++c) v2 += q.vel[c] * q.vel[c];
+      lam = std::max(lam, std::sqrt(v2) + q.a);
+      if (m.physics == NAVIER_STOKES) nu = std::max(nu, m.mu / q.rho);
+    }
+  if (lam_out) *lam_out = lam;
+  const double P2 = 2.0 * m.N + 1.0;
+  double dt = cfl * m.dx_min / (P2 * lam);
+  if (m.physics == NAVIER_STOKES) {
+    double numax = nu * std::max(1.0, 1.0 / m.Pr);
+    dt = std::min(dt, cfl * m.dx_min * m.dx_min / (P2 * P2 * numax));
+  }
+  return dt;
+}
+
+}  // namespace
+
+// ============================================================================
+// C interface for the Python tests (ctypes).  All pointers are host pointers.
+// ============================================================================
+extern "C" {
+
+struct oracle_mech_desc {
+  int n_species, n_reac;
+  double T_mid;
+  const double *W, *nasa;
+  const int *nu_r, *nu_p;
+  const double *A, *b, *Ea;
+};
+struct oracle_mesh_desc {
+  int dim, N;
+  long n_elem;
+  const double *node_xyz;
+  long n_iface; const int *iface;
+  long n_mortar; const int *mortar;
+  long n_bface; const int *bface;
+  int n_bc; const double *bc_state;
+  int physics;
+  double gamma, mu, Pr;
+  const oracle_mech_desc *mech;
+};
+
+static Mech to_mech(const oracle_mech_desc *d) {
+  Mech k;
+  if (!d) return k;
+  k.ns = d->n_species; k.nr = d->n_reac; k.T_mid = d->T_mid;
+  k.W.assign(d->W, d->W + k.ns);
+  k.nasa.assign(d->nasa, d->nasa + (size_t)k.ns * 14);
+  k.nu_r.assign(d->nu_r, d->nu_r + (size_t)k.nr * k.ns);
+  k.nu_p.assign(d->nu_p, d->nu_p + (size_t)k.nr * k.ns);
+  k.A.assign(d->A, d->A + k.nr); k.b.assign(d->b, d->b + k.nr); k.Ea.assign(d->Ea, d->Ea + k.nr);
+  return k;
+}
+
+void oracle_operators(int N, double *x, double *w, double *D) {
+  Ops o = make_ops(N);
+  std::copy(o.x.begin(), o.x.end(), x); std::copy(o.w.begin(), o.w.end(), w);
+  std::copy(o.D.begin(), o.D.end(), D);
+}
+void oracle_mortar_matrices(int N, double *Pf_lo, double *Pf_up, double *Pr_lo, double *Pr_up) {
+  Ops o = make_ops(N); std::vector<double> Pf[2], Pr[2]; make_mortar(o, Pf, Pr);
+  std::copy(Pf[0].begin(), Pf[0].end(), Pf_lo); std::copy(Pf[1].begin(), Pf[1].end(), Pf_up);
+  std::copy(Pr[0].begin(), Pr[0].end(), Pr_lo); std::copy(Pr[1].begin(), Pr[1].end(), Pr_up);
+}
+
+void *oracle_mesh_create(const oracle_mesh_desc *d) {
+  Mesh *m = new Mesh;
+  m->dim = d->dim; m->N = d->N; m->n = d->N + 1; m->ne = d->n_elem;
+  m->nn = (d->dim == 2) ? m->n * m->n : m->n * m->n * m->n;
+  m->physics = d->physics; m->gamma = d->gamma; m->mu = d->mu; m->Pr = d->Pr;
+  m->mech = to_mech(d->mech);
+  m->ns = (m->physics == REACTING_EULER) ? m->mech.ns : 1;
+  m->nvar = m->ns + m->dim + 1;
+  m->ops = make_ops(m->N);
+  make_mortar(m->ops, m->Pf, m->Pr_);
+  m->xyz.assign(d->node_xyz, d->node_xyz + (size_t)m->ne * m->dim * m->nn);
+  if (d->n_iface) m->iface.assign(d->iface, d->iface + d->n_iface * 5);
+  if (d->n_mortar) m->mortar.assign(d->mortar, d->mortar + d->n_mortar * 6);
+  if (d->n_bface) m->bface.assign(d->bface, d->bface + d->n_bface * 3);
+  if (d->n_bc) m->bc_state.assign(d->bc_state, d->bc_state + (size_t)d->n_bc * m->nvar);
+  compute_metrics(*m);
+  return m;
+}
+void oracle_mesh_destroy(void *h) { delete (Mesh *)h; }
+int oracle_nvar(void *h) { return ((Mesh *)h)->nvar; }
+double oracle_dx_min(void *h) { return ((Mesh *)h)->dx_min; }
+// metrics out: Ja [e][node][l][c], J [e][node]
+void oracle_metrics(void *h, double *Ja, double *J) {
+  Mesh *m = (Mesh *)h;
+  std::copy(m->Ja.begin(), m->Ja.end(), Ja); std::copy(m->J.begin(), m->J.end(), J);
+}
+void oracle_rhs(void *h, const double *u, double *du, double /*t*/) { rhs_full(*(Mesh *)h, u, du); }
+void oracle_rhs_inviscid(void *h, const double *u, double *du) { rhs_inviscid(*(Mesh *)h, u, du); }
+void oracle_rhs_viscous(void *h, const double *u, double *du) {
+  Mesh *m = (Mesh *)h;
+  std::fill(du, du + (size_t)m->ne * m->nvar * m->nn, 0.0);
+  rhs_viscous_add(*m, u, du);
+}
+// S out: [e][node][w][c]
+void oracle_br1_gradient(void *h, const double *u, double *S) {
+  std::vector<double> s; br1_gradient(*(Mesh *)h, u, s); std::copy(s.begin(), s.end(), S);
+}
+void oracle_chem_source(void *h, const double *u, double *s) { chem_source(*(Mesh *)h, u, s, false); }
+// O10. one SSP-RK33 stage (Shu-Osher):
+//   u_out = a_s u_n + b_s (u_in + dt L(u_in, t_n + c_s dt)),
+//   (a,b,c) = (0,1,0), (3/4,1/4,1), (1/3,2/3,1/2)
+void oracle_ssprk_stage(void *h, int stage, double dt, double t_n, const double *u_n, const double *u_in,
+                        double *u_out) {
+  Mesh *m = (Mesh *)h;
+  static const double a[3] = {0.0, 3.0 / 4.0, 1.0 / 3.0}, b[3] = {1.0, 1.0 / 4.0, 2.0 / 3.0}, c[3] = {0.0, 1.0, 0.5};
+  const size_t len = (size_t)m->ne * m->nvar * m->nn;
+  std::vector<double> L(len);
+  (void)(t_n + c[stage] * dt);
+  rhs_full(*m, u_in, L.data());
+  for (size_t i = 0; i < len; ++i) u_out[i] = a[stage] * u_n[i] + b[stage] * (u_in[i] + dt * L[i]);
+}
+// generic SSPRK3 driver on a user ODE y' = lam*y + c2*t^2 (for the scalar pins of O10)
+double oracle_ssprk3_scalar(double y0, double lam, double c2, double t0, double dt) {
+  auto L = [&](double y, double t) { return lam * y + c2 * t * t; };
+  double y1 = y0 + dt * L(y0, t0);
+  double y2 = 0.75 * y0 + 0.25 * (y1 + dt * L(y1, t0 + dt));
+  return 1.0 / 3.0 * y0 + 2.0 / 3.0 * (y2 + dt * L(y2, t0 + 0.5 * dt));
+}
+double oracle_max_dt(void *h, const double *u, double cfl, double *lam_max) { return max_dt(*(Mesh *)h, u, cfl, lam_max); }
+// full SSPRK3 steps; if cfl > 0, dt is recomputed by max_dt each step, else fixed dt.
+// returns the final time; u is advanced in place.  min_rho/min_p report positivity.
+double oracle_run(void *h, double *u, int nsteps, double cfl, double dt_fixed, double t0, double *min_rho, double *min_p) {
+  Mesh *m = (Mesh *)h;
+  const size_t len = (size_t)m->ne * m->nvar * m->nn;
+  std::vector<double> u1(len), u2(len);
+  double t = t0, mr = 1e300, mp = 1e300;
+  for (int s = 0; s < nsteps; ++s) {
+    double dt = (cfl > 0.0) ? max_dt(*m, u, cfl, nullptr) : dt_fixed;
+    oracle_ssprk_stage(h, 0, dt, t, u, u, u1.data());
+    oracle_ssprk_stage(h, 1, dt, t, u, u1.data(), u2.data());
+    oracle_ssprk_stage(h, 2, dt, t, u, u2.data(), u);
+    t += dt;
+    for (long e = 0; e < m->ne; ++e)
+      for (int p = 0; p < m->nn; ++p) {
+        double U[MAXV]; gather(*m, u, e, p, U);
+        Prim q = primitives(*m, U);
+        double rmin = q.rho;
+        for (int k = 0; k < m->ns; ++k) rmin = std::min(rmin, U[k]);
+        mr = std::min(mr, rmin); mp = std::min(mp, q.p);
+      }
+  }
+  if (min_rho) *min_rho = mr;
+  if (min_p) *min_p = mp;
+  return t;
+}
+// --- pointwise pieces, exposed for the pins ---------------------------------
+void oracle_rusanov(int dim, double gamma, const double *Um, const double *Up, const double *nv, double *Fs, double *lam) {
+  Mesh m; m.dim = dim; m.ns = 1; m.nvar = dim + 2; m.gamma = gamma; m.physics = EULER;
+  rusanov(m, Um, Up, nv, Fs);
+  if (lam) {
+    Prim qm = primitives(m, Um), qp = primitives(m, Up);
+    double nrm = 0.0; for (int c = 0; c < dim; ++c) nrm += nv[c] * nv[c]; nrm = std::sqrt(nrm);
+    double a = 0.0, b = 0.0;
+    for (int c = 0; c < dim; ++c) { a += qm.vel[c] * (nv[c] / nrm); b += qp.vel[c] * (nv[c] / nrm); }
+    *lam = std::max(std::fabs(a) + qm.a, std::fabs(b) + qp.a);
+  }
+}
+void oracle_viscous_flux(int dim, double gamma, double mu, double Pr, const double *U, const double *S, const double *nv, double *F) {
+  Mesh m; m.dim = dim; m.ns = 1; m.nvar = dim + 2; m.gamma = gamma; m.mu = mu; m.Pr = Pr; m.physics = NAVIER_STOKES;
+  viscous_flux_dot(m, U, S, nv, F);
+}
+double oracle_k_forward(const oracle_mech_desc *d, int r, double T) { Mech k = to_mech(d); return k_forward(k, r, T); }
+double oracle_k_equilibrium(const oracle_mech_desc *d, int r, double T) { Mech k = to_mech(d); return k_equilibrium(k, r, T); }
+void oracle_production_rates(const oracle_mech_desc *d, double T, const double *rho_s, double *omega) {
+  Mech k = to_mech(d); production_rates(k, T, rho_s, omega);
+}
+double oracle_temperature(const oracle_mech_desc *d, const double *rho_s, double e_int) {
+  Mech k = to_mech(d); return temperature_from_energy(k, rho_s, e_int);
+}
+// thermo of one species: out = {cp/R, h/(RT), s/R, e [J/kg], cv [J/(kg K)]}
+void oracle_species_thermo(const oracle_mech_desc *d, int s, double T, double *out) {
+  Mech k = to_mech(d);
+  out[0] = cp_over_R(k, s, T); out[1] = h_over_RT(k, s, T); out[2] = s_over_R(k, s, T);
+  out[3] = e_species(k, s, T); out[4] = cv_species(k, s, T);
+}
+// primitives of a reacting/ideal state at one node: out = {rho, p, a, T, vel[0..2]}
+void oracle_primitives(void *h, const double *U, double *out) {
+  Prim q = primitives(*(Mesh *)h, U);
+  out[0] = q.rho; out[1] = q.p; out[2] = q.a; out[3] = q.T; out[4] = q.vel[0]; out[5] = q.vel[1]; out[6] = q.vel[2];
+}
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"
