@@ -804,13 +804,15 @@ void oracle_br1_gradient(void *h, const double *u, double *S) {
   std::vector<double> s; br1_gradient(*(Mesh *)h, u, s); std::copy(s.begin(), s.end(), S);
 }
 void oracle_chem_source(void *h, const double *u, double *s) { chem_source(*(Mesh *)h, u, s, false); }
-// O10. one SSP-RK33 stage (Shu-Osher):
+// O10. SSP-RK33 coefficients (Shu-Osher), shared by the two drivers below
+static const double SSP_A[3] = {0.0, 3.0 / 4.0, 1.0 / 3.0}, SSP_B[3] = {1.0, 1.0 / 4.0, 2.0 / 3.0}, SSP_C[3] = {0.0, 1.0, 0.5};
+// one SSP-RK33 stage:
 //   u_out = a_s u_n + b_s (u_in + dt L(u_in, t_n + c_s dt)),
 //   (a,b,c) = (0,1,0), (3/4,1/4,1), (1/3,2/3,1/2)
 void oracle_ssprk_stage(void *h, int stage, double dt, double t_n, const double *u_n, const double *u_in,
                         double *u_out) {
   Mesh *m = (Mesh *)h;
-  static const double a[3] = {0.0, 3.0 / 4.0, 1.0 / 3.0}, b[3] = {1.0, 1.0 / 4.0, 2.0 / 3.0}, c[3] = {0.0, 1.0, 0.5};
+  const double *a = SSP_A, *b = SSP_B, *c = SSP_C;
   const size_t len = (size_t)m->ne * m->nvar * m->nn;
   std::vector<double> L(len);
   (void)(t_n + c[stage] * dt);
@@ -820,9 +822,9 @@ void oracle_ssprk_stage(void *h, int stage, double dt, double t_n, const double 
 // generic SSPRK3 driver on a user ODE y' = lam*y + c2*t^2 (for the scalar pins of O10)
 double oracle_ssprk3_scalar(double y0, double lam, double c2, double t0, double dt) {
   auto L = [&](double y, double t) { return lam * y + c2 * t * t; };
-  double y1 = y0 + dt * L(y0, t0);
-  double y2 = 0.75 * y0 + 0.25 * (y1 + dt * L(y1, t0 + dt));
-  return 1.0 / 3.0 * y0 + 2.0 / 3.0 * (y2 + dt * L(y2, t0 + 0.5 * dt));
+  double y = y0;
+  for (int s = 0; s < 3; ++s) y = SSP_A[s] * y0 + SSP_B[s] * (y + dt * L(y, t0 + SSP_C[s] * dt));
+  return y;
 }
 double oracle_max_dt(void *h, const double *u, double cfl, double *lam_max) { return max_dt(*(Mesh *)h, u, cfl, lam_max); }
 // full SSPRK3 steps; if cfl > 0, dt is recomputed by max_dt each step, else fixed dt.
