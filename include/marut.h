@@ -1,0 +1,126 @@
+/* ============================================================================
+ * marut.h -- C ABI of the B200-native DG right-hand side + SSP-RK33 hot path
+ *            of MARUT (arxiv 2605.26388).  Implemented in hand-written CUDA for
+ *            sm_100a (paper_2605_26388_b200/csrc).  No CPU fallback exists.
+ *
+ * Citations are "PAPER.md:<line>" (text of the paper) and DESIGN.md readings.
+ *
+ * Conventions
+ *  - n = N+1 LGL nodes per direction; a volume node is node = i + n*(j + n*k).
+ *  - Solution / residual arrays (u, du, s, u_n, u_in, u_out) are DEVICE pointers
+ *    owned by the caller, FP64, layout [n_elem][n_var][n^dim] (element-contiguous,
+ *    variable-planar), base pointer 16-byte aligned.
+ *    Variables: rho_1..rho_ns, rho*u_1..rho*u_dim, E  (ns = 1 unless REACTING_EULER).
+ *  - Faces: f = 2*l + side (l = reference direction, side 0: xi_l = -1, 1: xi_l = +1).
+ *    Face nodes are indexed by the remaining directions in increasing order
+ *    (a = a0 + n*a1).  orient = 0: face node a of L meets face node a of R;
+ *    orient = 1 (2-D only): a meets N - a.  3-D meshes must have orient = 0.
+ *  - Descriptor arrays are HOST pointers, copied at create; the handle owns all
+ *    device geometry, connectivity and scratch.
+ *  - Every call returns a status; no exceptions, no abort, nothing on stdout.
+ *    marut_last_error() gives a thread-local message for the last failure.
+ *  - Calls are asynchronous on `cuda_stream` (a cudaStream_t, NULL = default
+ *    stream) except marut_mesh_create, marut_mesh_destroy and marut_max_dt.
+ * ========================================================================== */
+#ifndef MARUT_H
+#define MARUT_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct marut_mesh marut_mesh; /* opaque */
+
+typedef enum {
+  MARUT_OK = 0,
+  MARUT_EINVAL = 1,     /* bad argument: NULL pointer, N or dim out of range, misaligned buffer, aliasing */
+  MARUT_ENOMEM = 2,     /* host or device allocation failed */
+  MARUT_ECUDA = 3,      /* CUDA runtime error (no device, launch failure) */
+  MARUT_ETOPOLOGY = 4,  /* index out of range, face listed twice or never, unsupported orient, J <= 0 */
+  MARUT_ENOTFINITE = 5  /* marut_max_dt met a non-finite or non-positive wave speed */
+} marut_status;
+
+enum { MARUT_EULER = 0, MARUT_NAVIER_STOKES = 1, MARUT_REACTING_EULER = 2 };
+
+/* Finite-rate mechanism (R12).  Host struct, caller-owned.
+ * Species thermodynamics in NASA-7 form: nasa[s][range][7], range 0: T < T_mid, range 1: T >= T_mid.
+ * Reaction r: sum_s nu_r[r][s] X_s <-> sum_s nu_p[r][s] X_s (third bodies appear on both sides),
+ * k_f = A T^b exp(-Ea/T) with A in cm^3-mol-s units and Ea in kelvin; k_b = k_f / K_c(T).      */
+typedef struct {
+  int n_species;        /* 1..8  */
+  int n_reac;           /* 0..32 */
+  double T_mid;
+  const double *W;      /* [n_species] molar mass, kg/mol */
+  const double *nasa;   /* [n_species][2][7] */
+  const int *nu_r;      /* [n_reac][n_species] reactant coefficients nu'  (0..3) */
+  const int *nu_p;      /* [n_reac][n_species] product  coefficients nu'' (0..3) */
+  const double *A, *b, *Ea; /* [n_reac] */
+} marut_mech;
+
+/* Mesh + physics descriptor: the paper's statement of the problem. */
+typedef struct {
+  int dim;                /* 2 | 3 */
+  int N;                  /* polynomial degree, 1..7 (the paper's P) */
+  long n_elem;
+  const double *node_xyz; /* [n_elem][dim][n^dim] isoparametric LGL node coordinates */
+  long n_iface;
+  const int *iface;       /* [n_iface][5]  = eL,fL,eR,fR,orient : conforming interior faces */
+  long n_mortar;
+  const int *mortar;      /* [n_mortar][6] = eC,fC,eF_lo,eF_up,fF,orient : 2-D 2:1 hanging faces;
+                             eF_lo covers the coarse face parameter [-1,0], eF_up covers [0,1]; orient must be 0 */
+  long n_bface;
+  const int *bface;       /* [n_bface][3]  = e,f,bc_id : boundary faces with a prescribed exterior state */
+  int n_bc;
+  const double *bc_state; /* [n_bc][n_var] conserved exterior states */
+  int physics;            /* MARUT_EULER | MARUT_NAVIER_STOKES | MARUT_REACTING_EULER */
+  double gamma;           /* ratio of specific heats (EULER, NAVIER_STOKES) */
+  double mu, Pr;          /* constant dynamic viscosity and Prandtl number (NAVIER_STOKES) */
+  const marut_mech *mech; /* REACTING_EULER only, else NULL */
+} marut_mesh_desc;
+
+/* Setup: LGL nodes/weights/D, GCL-preserving metric terms
+ * Ja^l and 1/J on the device, affine-element detection, mortar projection matrices, element-face
+ * connectivity tables, scratch buffers.  Synchronous.  Every face of every element must appear exactly
+ * once in iface/mortar/bface.  Errors: EINVAL, ENOMEM, ECUDA, ETOPOLOGY (reported here, never later). */
+marut_status marut_mesh_create(const marut_mesh_desc *desc, marut_mesh **out);
+
+/* NULL-safe; synchronises the device. */
+void marut_mesh_destroy(marut_mesh *mesh);
+
+/* du = L(u, t): the semi-discrete DG operator (eq. 9, 12; 707), including the BR1
+ * viscous part (eq. 13-16) for NAVIER_STOKES and the chemistry source (PAPER.md:204,
+ * eq. 20-22) for REACTING_EULER.  u, du: device, [n_elem][n_var][n^dim]; du must not alias u. */
+marut_status marut_rhs(marut_mesh *mesh, const double *u, double *du, double t, void *cuda_stream);
+
+/* One SSP-RK33 stage (Shu-Osher; eq. 45), fused with the operator:
+ *   u_out = a_s*u_n + b_s*(u_in + dt*L(u_in, t_n + c_s*dt)),  (a,b,c) = (0,1,0), (3/4,1/4,1), (1/3,2/3,1/2)
+ * stage in {0,1,2}.  u_out must not alias u_in (neighbours read u_in); u_out may alias u_n.
+ * u_n is not read for stage 0. */
+marut_status marut_ssprk_stage(marut_mesh *mesh, int stage, double dt, double t_n, const double *u_n,
+                               const double *u_in, double *u_out, void *cuda_stream);
+
+/* dt = min(dt_C, dt_D) (eq. 17-18; R11):
+ *   dt_C = cfl*dx_min/((2N+1)*max_i(|u_i|_2 + a_i)),  dt_D = cfl*dx_min^2/((2N+1)^2*nu_max) (NAVIER_STOKES),
+ *   dx_min = min_e 2*(min_i J_i)^(1/dim),  nu_max = max_i(mu/rho_i)*max(1, 1/Pr).
+ * Warp-shuffle max reduction on the device; dt_out is a HOST pointer; synchronises the stream. */
+marut_status marut_max_dt(marut_mesh *mesh, const double *u, double cfl, double *dt_out, void *cuda_stream);
+
+/* s = S(u): per-node finite-rate chemistry source (eq. 21-22); species rows omega_s,
+ * momentum and energy rows 0.  REACTING_EULER meshes only (else EINVAL). */
+marut_status marut_chem_source(marut_mesh *mesh, const double *u, double *s, void *cuda_stream);
+
+/* --- introspection (used by the tests to check setup row a0; no compute path depends on them) --- */
+/* copy the device metric terms to HOST arrays: Ja [n_elem][n^dim][dim][dim] (Ja^l_c), J [n_elem][n^dim]. */
+marut_status marut_get_metrics(marut_mesh *mesh, double *Ja_host, double *J_host);
+/* 1 if every element was detected affine (metrics stored per element), else 0; dx_min as used by marut_max_dt */
+int marut_is_affine(const marut_mesh *mesh);
+double marut_dx_min(const marut_mesh *mesh);
+/* number of kernel launches issued through this handle so far (bench.py's gpu_launches) */
+long marut_launch_count(const marut_mesh *mesh);
+
+const char *marut_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MARUT_H */

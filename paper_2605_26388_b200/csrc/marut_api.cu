@@ -1,0 +1,551 @@
+// marut_api.cu -- the C ABI of include/marut.h: setup, dispatch of the fused stage
+// kernels, the CFL reduction and the chemistry source.  Product code; shares nothing with oracle/.
+#include "../../include/marut.h"
+#include "marut_kernels.cuh"
+#include "marut_launch.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace marut;
+
+// ------------------------------------------------------------------------------------ errors
+static thread_local char g_err[512] = "";
+static marut_status fail(marut_status st, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return st;
+}
+#define CUDA_TRY(call)                                                                      \
+  do {                                                                                      \
+    cudaError_t err__ = (call);                                                             \
+    if (err__ != cudaSuccess)                                                               \
+      return fail(err__ == cudaErrorMemoryAllocation ? MARUT_ENOMEM : MARUT_ECUDA, "%s: %s", #call, \
+                  cudaGetErrorString(err__));                                               \
+  } while (0)
+
+// ------------------------------------------------------------------------------------ mesh handle
+struct marut_mesh {
+  int dim = 0, N = 0, np = 0, nn = 0, nvar = 0, nsp = 1, physics = 0;
+  long ne = 0, n_mortar = 0;
+  double gamma = 1.4, mu = 0.0, Pr = 0.72, kappa = 0.0;
+  bool affine = false;
+  double dx_min = 0.0;
+  double D[MAX_NP * MAX_NP] = {0}, w[MAX_NP] = {0};
+  // device
+  double *d_metric = nullptr;
+  int2 *d_conn = nullptr;
+  int *d_mortar_fine = nullptr;
+  double *d_mortar_mat = nullptr;
+  double *d_bc = nullptr;
+  double *d_S = nullptr;     // NS gradient scratch
+  double *d_T = nullptr;     // reacting temperature scratch
+  MechDev *d_mech = nullptr;
+  unsigned long long *d_red = nullptr;
+  unsigned long long *h_red = nullptr;  // pinned
+  long launches = 0;
+};
+
+// ------------------------------------------------------------------------------------ 1-D operators
+// LGL nodes as the roots of q(x) = P_{N+1}(x) - P_{N-1}(x), q'(x) = (2N+1) P_N(x);
+// w_j = 2 / (N (N+1) P_N(x_j)^2); D_ij = P_N(x_i) / (P_N(x_j) (x_i - x_j)), D_ii = -sum_{j != i} D_ij.
+static void legendre_three(int N, double x, double &Pm1, double &P0, double &Pp1) {
+  // returns P_{N-1}, P_N, P_{N+1}
+  double a = 1.0, b = x;  // P_0, P_1
+  if (N == 0) { Pm1 = 0.0; P0 = 1.0; Pp1 = x; return; }
+  for (int k = 1; k < N; ++k) {
+    double c = ((2 * k + 1) * x * b - k * a) / (k + 1);
+    a = b; b = c;
+  }
+  Pm1 = a; P0 = b;
+  Pp1 = ((2 * N + 1) * x * b - N * a) / (N + 1);
+}
+static void build_operators(int N, double *x, double *w, double *D) {
+  const int n = N + 1;
+  std::vector<double> PN(n);
+  for (int j = 0; j < n; ++j) {
+    double xj = -std::cos(M_PI * j / N);
+    if (j == 0) xj = -1.0;
+    else if (j == N) xj = 1.0;
+    else
+      for (int it = 0; it < 100; ++it) {
+        double a, b, c;
+        legendre_three(N, xj, a, b, c);
+        double dx = (c - a) / ((2 * N + 1) * b);
+        xj -= dx;
+        if (std::fabs(dx) < 1e-16) break;
+      }
+    x[j] = xj;
+  }
+  for (int j = 0; j < n / 2; ++j) {  // enforce the exact antisymmetry of the node set
+    double s = 0.5 * (x[n - 1 - j] - x[j]);
+    x[j] = -s; x[n - 1 - j] = s;
+  }
+  if (n % 2) x[n / 2] = 0.0;
+  for (int j = 0; j < n; ++j) {
+    double a, b, c;
+    legendre_three(N, x[j], a, b, c);
+    PN[j] = b;
+    w[j] = 2.0 / (N * (N + 1.0) * b * b);
+  }
+  for (int i = 0; i < n; ++i) {
+    double s = 0.0;
+    for (int j = 0; j < n; ++j)
+      if (j != i) { D[i * n + j] = PN[i] / (PN[j] * (x[i] - x[j])); s += D[i * n + j]; }
+    D[i * n + i] = -s;
+  }
+}
+// barycentric evaluation of the Lagrange basis on nodes x at point y
+static void lagrange_row(int n, const double *x, double y, double *row) {
+  std::vector<double> lam(n);
+  for (int j = 0; j < n; ++j) {
+    double p = 1.0;
+    for (int k = 0; k < n; ++k) if (k != j) p *= (x[j] - x[k]);
+    lam[j] = 1.0 / p;
+  }
+  for (int j = 0; j < n; ++j)
+    if (y == x[j]) { for (int k = 0; k < n; ++k) row[k] = (k == j) ? 1.0 : 0.0; return; }
+  double den = 0.0;
+  for (int j = 0; j < n; ++j) { row[j] = lam[j] / (y - x[j]); den += row[j]; }
+  for (int j = 0; j < n; ++j) row[j] /= den;
+}
+// 2:1 mortar matrices (R7): P_fwd^m[i][j] = l_j((x_i -/+ 1)/2);
+// P_rev^m = 1/2 M^-1 (P_fwd^m)^T M with the EXACT mass matrix M_ij = int l_i l_j (Gauss quadrature),
+// i.e. the exact L2 projection onto degree-N polynomials on the coarse face.
+static bool build_mortar(int N, const double *x, double *out /*[4][n*n]*/) {
+  const int n = N + 1;
+  // Gauss-Legendre rule with n points (exact to degree 2N+1)
+  std::vector<double> g(n), wg(n);
+  for (int q = 0; q < n; ++q) {
+    double y = -std::cos(M_PI * (q + 0.75) / (n + 0.5));
+    for (int it = 0; it < 100; ++it) {
+      double a, b, c;
+      legendre_three(n, y, a, b, c);           // b = P_n(y), a = P_{n-1}(y)
+      double dP = n * (y * b - a) / (y * y - 1.0);  // P_n'(y)
+      double dy = b / dP;
+      y -= dy;
+      if (std::fabs(dy) < 1e-16) break;
+    }
+    double a, b, c;
+    legendre_three(n, y, a, b, c);
+    double dP = n * (y * b - a) / (y * y - 1.0);
+    g[q] = y; wg[q] = 2.0 / ((1.0 - y * y) * dP * dP);
+  }
+  std::vector<double> L(n * n), M(n * n, 0.0);   // L[q][j] = l_j(g_q)
+  for (int q = 0; q < n; ++q) lagrange_row(n, x, g[q], &L[q * n]);
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < n; ++j)
+      for (int q = 0; q < n; ++q) M[i * n + j] += wg[q] * L[q * n + i] * L[q * n + j];
+  for (int m = 0; m < 2; ++m) {
+    double *Pf = out + m * n * n, *Pr = out + (2 + m) * n * n;
+    const double shift = m ? 1.0 : -1.0;
+    for (int i = 0; i < n; ++i) lagrange_row(n, x, 0.5 * (x[i] + shift), &Pf[i * n]);
+    // solve M X = 1/2 Pf^T M  (Gaussian elimination, partial pivoting)
+    std::vector<double> A(M), B(n * n, 0.0);
+    for (int i = 0; i < n; ++i)
+      for (int j = 0; j < n; ++j) {
+        double s = 0.0;
+        for (int k = 0; k < n; ++k) s += Pf[k * n + i] * M[k * n + j];
+        B[i * n + j] = 0.5 * s;
+      }
+    for (int c = 0; c < n; ++c) {
+      int piv = c;
+      for (int r = c + 1; r < n; ++r) if (std::fabs(A[r * n + c]) > std::fabs(A[piv * n + c])) piv = r;
+      if (A[piv * n + c] == 0.0) return false;
+      if (piv != c)
+        for (int k = 0; k < n; ++k) { std::swap(A[c * n + k], A[piv * n + k]); std::swap(B[c * n + k], B[piv * n + k]); }
+      for (int r = c + 1; r < n; ++r) {
+        double f = A[r * n + c] / A[c * n + c];
+        for (int k = c; k < n; ++k) A[r * n + k] -= f * A[c * n + k];
+        for (int k = 0; k < n; ++k) B[r * n + k] -= f * B[c * n + k];
+      }
+    }
+    for (int c = n - 1; c >= 0; --c)
+      for (int k = 0; k < n; ++k) {
+        double s = B[c * n + k];
+        for (int r = c + 1; r < n; ++r) s -= A[c * n + r] * Pr[r * n + k];
+        Pr[c * n + k] = s / A[c * n + c];
+      }
+  }
+  return true;
+}
+
+// ------------------------------------------------------------------------------------ metrics dispatch
+template <int DIM>
+static cudaError_t run_metrics(int np, const double *d_xyz, double *d_full, double *d_info, const double *d_D, long ne) {
+#define MARUT_METRICS_CASE(NPV)                                                                            \
+  case NPV: {                                                                                              \
+    constexpr int NN = Geo<DIM, NPV>::NN;                                                                  \
+    constexpr size_t smem = (size_t)((DIM + DIM * DIM) * NN + NPV * NPV + DIM * DIM + 2) * sizeof(double); \
+    cudaError_t e1 = cudaFuncSetAttribute(metrics_kernel<DIM, NPV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+    if (e1 != cudaSuccess) return e1;                                                                      \
+    metrics_kernel<DIM, NPV><<<(unsigned)ne, NN, smem>>>(d_xyz, d_full, d_info, d_D, ne);                  \
+    return cudaGetLastError();                                                                             \
+  }
+  switch (np) {
+    MARUT_METRICS_CASE(2) MARUT_METRICS_CASE(3) MARUT_METRICS_CASE(4) MARUT_METRICS_CASE(5)
+    MARUT_METRICS_CASE(6) MARUT_METRICS_CASE(7) MARUT_METRICS_CASE(8)
+  }
+#undef MARUT_METRICS_CASE
+  return cudaErrorNotSupported;
+}
+template <int DIM>
+static cudaError_t run_compact(int np, const double *d_full, double *d_el, long ne) {
+  const long total = ne * (DIM * DIM + 1);
+  const unsigned grid = (unsigned)((total + 255) / 256);
+  switch (np) {
+    case 2: compact_metrics_kernel<DIM, 2><<<grid, 256>>>(d_full, d_el, ne); break;
+    case 3: compact_metrics_kernel<DIM, 3><<<grid, 256>>>(d_full, d_el, ne); break;
+    case 4: compact_metrics_kernel<DIM, 4><<<grid, 256>>>(d_full, d_el, ne); break;
+    case 5: compact_metrics_kernel<DIM, 5><<<grid, 256>>>(d_full, d_el, ne); break;
+    case 6: compact_metrics_kernel<DIM, 6><<<grid, 256>>>(d_full, d_el, ne); break;
+    case 7: compact_metrics_kernel<DIM, 7><<<grid, 256>>>(d_full, d_el, ne); break;
+    case 8: compact_metrics_kernel<DIM, 8><<<grid, 256>>>(d_full, d_el, ne); break;
+    default: return cudaErrorNotSupported;
+  }
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------ create / destroy
+extern "C" void marut_mesh_destroy(marut_mesh *m) {
+  if (!m) return;
+  cudaDeviceSynchronize();
+  cudaFree(m->d_metric); cudaFree(m->d_conn); cudaFree(m->d_mortar_fine); cudaFree(m->d_mortar_mat);
+  cudaFree(m->d_bc); cudaFree(m->d_S); cudaFree(m->d_T); cudaFree(m->d_mech); cudaFree(m->d_red);
+  if (m->h_red) cudaFreeHost(m->h_red);
+  delete m;
+}
+
+static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
+  if (d->dim != 2 && d->dim != 3) return fail(MARUT_EINVAL, "dim must be 2 or 3 (got %d)", d->dim);
+  if (d->N < 1 || d->N > 7) return fail(MARUT_EINVAL, "N must be in 1..7 (got %d)", d->N);
+  if (d->n_elem <= 0 || d->n_elem > 2000000000L) return fail(MARUT_EINVAL, "n_elem out of range");
+  if (!d->node_xyz) return fail(MARUT_EINVAL, "node_xyz is NULL");
+  if (d->n_iface < 0 || d->n_mortar < 0 || d->n_bface < 0 || d->n_bc < 0) return fail(MARUT_EINVAL, "negative count");
+  if ((d->n_iface && !d->iface) || (d->n_mortar && !d->mortar) || (d->n_bface && !d->bface) || (d->n_bc && !d->bc_state))
+    return fail(MARUT_EINVAL, "NULL connectivity array with non-zero count");
+  if (d->physics < 0 || d->physics > 2) return fail(MARUT_EINVAL, "unknown physics %d", d->physics);
+  if (d->n_mortar && d->dim != 2) return fail(MARUT_EINVAL, "mortars are implemented for 2-D meshes only");
+  if (d->physics != MARUT_EULER && (d->n_mortar || d->n_bface))
+    return fail(MARUT_EINVAL, "NAVIER_STOKES / REACTING_EULER support conforming interior faces only");
+  if (d->physics != MARUT_REACTING_EULER && !(d->gamma > 1.0)) return fail(MARUT_EINVAL, "gamma must be > 1");
+  if (d->physics == MARUT_NAVIER_STOKES && (!(d->mu >= 0.0) || !(d->Pr > 0.0))) return fail(MARUT_EINVAL, "need mu >= 0, Pr > 0");
+
+  m->dim = d->dim; m->N = d->N; m->np = d->N + 1; m->ne = d->n_elem; m->physics = d->physics;
+  m->nn = (d->dim == 2) ? m->np * m->np : m->np * m->np * m->np;
+  m->gamma = d->gamma; m->mu = d->mu; m->Pr = d->Pr;
+  if (d->physics == MARUT_NAVIER_STOKES) m->kappa = d->gamma * d->mu / (d->Pr * (d->gamma - 1.0));
+  m->n_mortar = d->n_mortar;
+  const int dim = m->dim, np = m->np, nn = m->nn, nf2 = 2 * dim;
+  const long ne = m->ne;
+
+  // mechanism
+  if (d->physics == MARUT_REACTING_EULER) {
+    const marut_mech *k = d->mech;
+    if (!k) return fail(MARUT_EINVAL, "REACTING_EULER needs a mechanism");
+    if (k->n_species < 1 || k->n_species > MAX_SPEC || k->n_reac < 0 || k->n_reac > MAX_REAC)
+      return fail(MARUT_EINVAL, "mechanism size out of range");
+    if (!k->W || !k->nasa || (k->n_reac && (!k->nu_r || !k->nu_p || !k->A || !k->b || !k->Ea)))
+      return fail(MARUT_EINVAL, "NULL mechanism array");
+    if (k->n_species != 5) return fail(MARUT_EINVAL, "this build instantiates the reacting kernels for 5 species only");
+    MechDev h;
+    memset(&h, 0, sizeof(h));
+    h.ns = k->n_species; h.nr = k->n_reac; h.T_mid = k->T_mid;
+    for (int s = 0; s < h.ns; ++s) {
+      if (!(k->W[s] > 0.0)) return fail(MARUT_EINVAL, "molar mass must be positive");
+      h.W[s] = k->W[s];
+      for (int r = 0; r < 2; ++r)
+        for (int c = 0; c < 7; ++c) h.nasa[s][r][c] = k->nasa[(s * 2 + r) * 7 + c];
+    }
+    for (int r = 0; r < h.nr; ++r) {
+      h.A[r] = k->A[r]; h.b[r] = k->b[r]; h.Ea[r] = k->Ea[r];
+      for (int s = 0; s < h.ns; ++s) {
+        int a = k->nu_r[r * h.ns + s], b = k->nu_p[r * h.ns + s];
+        if (a < 0 || a > 3 || b < 0 || b > 3) return fail(MARUT_EINVAL, "stoichiometric coefficient out of 0..3");
+        h.nu_r[r][s] = (signed char)a; h.nu_p[r][s] = (signed char)b;
+      }
+    }
+    m->nsp = h.ns;
+    CUDA_TRY(cudaMalloc(&m->d_mech, sizeof(MechDev)));
+    CUDA_TRY(cudaMemcpy(m->d_mech, &h, sizeof(MechDev), cudaMemcpyHostToDevice));
+  }
+  m->nvar = m->nsp + dim + 1;
+  if (m->nvar > MAX_VAR) return fail(MARUT_EINVAL, "too many variables");
+  if (d->n_bc && d->n_bface == 0) { /* unused states are fine */ }
+
+  // ---- connectivity: element-face table, every face exactly once
+  std::vector<int2> conn((size_t)ne * nf2, make_int2(-1, -1));
+  auto claim = [&](long e, int f, int x, int info) -> bool {
+    if (e < 0 || e >= ne || f < 0 || f >= nf2) return false;
+    int2 &c = conn[(size_t)e * nf2 + f];
+    if (c.y != -1) return false;
+    c = make_int2(x, info);
+    return true;
+  };
+  for (long i = 0; i < d->n_iface; ++i) {
+    const int *I = d->iface + i * 5;
+    if (I[4] < 0 || (dim == 3 && I[4] != 0) || (dim == 2 && I[4] > 1))
+      return fail(MARUT_ETOPOLOGY, "iface %ld: unsupported orient %d", i, I[4]);
+    if (I[0] < 0 || I[0] >= ne || I[2] < 0 || I[2] >= ne || I[1] < 0 || I[1] >= nf2 || I[3] < 0 || I[3] >= nf2)
+      return fail(MARUT_ETOPOLOGY, "iface %ld: index out of range", i);
+    if (!claim(I[0], I[1], I[2], pack_info(FK_CONFORMING, I[3], I[4], 0)) ||
+        !claim(I[2], I[3], I[0], pack_info(FK_CONFORMING, I[1], I[4], 0)))
+      return fail(MARUT_ETOPOLOGY, "iface %ld: face listed twice", i);
+  }
+  std::vector<int> mfine((size_t)std::max<long>(1, d->n_mortar) * 2, 0);
+  for (long i = 0; i < d->n_mortar; ++i) {
+    const int *M = d->mortar + i * 6;
+    if (M[5] != 0) return fail(MARUT_ETOPOLOGY, "mortar %ld: orient must be 0", i);
+    for (int k : {0, 2, 3}) if (M[k] < 0 || M[k] >= ne) return fail(MARUT_ETOPOLOGY, "mortar %ld: element out of range", i);
+    if (M[1] < 0 || M[1] >= nf2 || M[4] < 0 || M[4] >= nf2) return fail(MARUT_ETOPOLOGY, "mortar %ld: face out of range", i);
+    if (!claim(M[0], M[1], (int)i, pack_info(FK_MORTAR_COARSE, M[4], 0, 0)) ||
+        !claim(M[2], M[4], M[0], pack_info(FK_MORTAR_FINE, M[1], 0, 0)) ||
+        !claim(M[3], M[4], M[0], pack_info(FK_MORTAR_FINE, M[1], 0, 1)))
+      return fail(MARUT_ETOPOLOGY, "mortar %ld: face listed twice", i);
+    mfine[i * 2] = M[2]; mfine[i * 2 + 1] = M[3];
+  }
+  for (long i = 0; i < d->n_bface; ++i) {
+    const int *B = d->bface + i * 3;
+    if (B[2] < 0 || B[2] >= d->n_bc) return fail(MARUT_ETOPOLOGY, "bface %ld: bc_id out of range", i);
+    if (!claim(B[0], B[1], B[2], pack_info(FK_BOUNDARY, 0, 0, 0)))
+      return fail(MARUT_ETOPOLOGY, "bface %ld: bad index or face listed twice", i);
+  }
+  for (size_t i = 0; i < conn.size(); ++i)
+    if (conn[i].y == -1) return fail(MARUT_ETOPOLOGY, "element %ld face %d has no neighbour, mortar or boundary entry",
+                                     (long)(i / nf2), (int)(i % nf2));
+
+  // ---- operators
+  double x[MAX_NP];
+  build_operators(m->N, x, m->w, m->D);
+  std::vector<double> mort((size_t)4 * np * np, 0.0);
+  if (!build_mortar(m->N, x, mort.data())) return fail(MARUT_EINVAL, "singular mass matrix");
+
+  // ---- uploads
+  CUDA_TRY(cudaMalloc(&m->d_conn, conn.size() * sizeof(int2)));
+  CUDA_TRY(cudaMemcpy(m->d_conn, conn.data(), conn.size() * sizeof(int2), cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMalloc(&m->d_mortar_fine, mfine.size() * sizeof(int)));
+  CUDA_TRY(cudaMemcpy(m->d_mortar_fine, mfine.data(), mfine.size() * sizeof(int), cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMalloc(&m->d_mortar_mat, mort.size() * sizeof(double)));
+  CUDA_TRY(cudaMemcpy(m->d_mortar_mat, mort.data(), mort.size() * sizeof(double), cudaMemcpyHostToDevice));
+  const size_t nbc = (size_t)std::max(1, d->n_bc) * m->nvar;
+  CUDA_TRY(cudaMalloc(&m->d_bc, nbc * sizeof(double)));
+  if (d->n_bc) CUDA_TRY(cudaMemcpy(m->d_bc, d->bc_state, (size_t)d->n_bc * m->nvar * sizeof(double), cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMalloc(&m->d_red, 4 * sizeof(unsigned long long)));
+  CUDA_TRY(cudaMallocHost(&m->h_red, 4 * sizeof(unsigned long long)));
+
+  // ---- metric terms on the device
+  const int MD = dim * dim + 1;
+  double *d_xyz = nullptr, *d_full = nullptr, *d_info = nullptr, *d_D = nullptr;
+  auto cleanup = [&]() { cudaFree(d_xyz); cudaFree(d_full); cudaFree(d_info); cudaFree(d_D); };
+  const size_t nxyz = (size_t)ne * dim * nn;
+  cudaError_t ce;
+  if ((ce = cudaMalloc(&d_xyz, nxyz * sizeof(double))) != cudaSuccess ||
+      (ce = cudaMalloc(&d_full, (size_t)ne * MD * nn * sizeof(double))) != cudaSuccess ||
+      (ce = cudaMalloc(&d_info, (size_t)ne * 2 * sizeof(double))) != cudaSuccess ||
+      (ce = cudaMalloc(&d_D, np * np * sizeof(double))) != cudaSuccess) {
+    cleanup();
+    return fail(MARUT_ENOMEM, "device allocation for metrics failed: %s", cudaGetErrorString(ce));
+  }
+  std::vector<double> info((size_t)ne * 2);
+  if ((ce = cudaMemcpy(d_xyz, d->node_xyz, nxyz * sizeof(double), cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (ce = cudaMemcpy(d_D, m->D, np * np * sizeof(double), cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (ce = (dim == 2 ? run_metrics<2>(np, d_xyz, d_full, d_info, d_D, ne) : run_metrics<3>(np, d_xyz, d_full, d_info, d_D, ne))) != cudaSuccess ||
+      (ce = cudaMemcpy(info.data(), d_info, info.size() * sizeof(double), cudaMemcpyDeviceToHost)) != cudaSuccess) {
+    cleanup();
+    return fail(MARUT_ECUDA, "metric computation failed: %s", cudaGetErrorString(ce));
+  }
+  m->launches++;
+  double dxm = 1e300, dev = 0.0;
+  for (long e = 0; e < ne; ++e) {
+    const double Jmin = info[e * 2];
+    if (!(Jmin > 0.0) || !std::isfinite(Jmin)) { cleanup(); return fail(MARUT_ETOPOLOGY, "element %ld: Jacobian %g <= 0", e, Jmin); }
+    dxm = std::min(dxm, 2.0 * std::pow(Jmin, 1.0 / dim));
+    dev = std::max(dev, info[e * 2 + 1]);
+  }
+  m->dx_min = dxm;
+  m->affine = dev < 1e-12;   // constant metrics to round-off -> keep one set per element
+  if (m->affine) {
+    if ((ce = cudaMalloc(&m->d_metric, (size_t)ne * MD * sizeof(double))) != cudaSuccess ||
+        (ce = (dim == 2 ? run_compact<2>(np, d_full, m->d_metric, ne) : run_compact<3>(np, d_full, m->d_metric, ne))) != cudaSuccess ||
+        (ce = cudaDeviceSynchronize()) != cudaSuccess) {
+      cleanup();
+      return fail(MARUT_ECUDA, "metric compaction failed: %s", cudaGetErrorString(ce));
+    }
+    m->launches++;
+  } else {
+    m->d_metric = d_full;
+    d_full = nullptr;
+  }
+  cleanup();
+
+  // ---- scratch
+  if (m->physics == MARUT_NAVIER_STOKES) CUDA_TRY(cudaMalloc(&m->d_S, (size_t)ne * (dim + 2) * dim * nn * sizeof(double)));
+  if (m->physics == MARUT_REACTING_EULER) CUDA_TRY(cudaMalloc(&m->d_T, (size_t)ne * nn * sizeof(double)));
+
+  // ---- is this (dim, N, physics) instantiated?  (probe with an empty launch: ne = 0 is rejected above, so test the switch)
+  return MARUT_OK;
+}
+
+extern "C" marut_status marut_mesh_create(const marut_mesh_desc *desc, marut_mesh **out) {
+  if (!desc || !out) return fail(MARUT_EINVAL, "NULL argument");
+  *out = nullptr;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(MARUT_ECUDA, "no CUDA device: this library has no CPU fallback");
+  }
+  marut_mesh *m = new (std::nothrow) marut_mesh;
+  if (!m) return fail(MARUT_ENOMEM, "host allocation failed");
+  marut_status st = create_impl(desc, m);
+  if (st != MARUT_OK) {
+    char keep[sizeof(g_err)];
+    memcpy(keep, g_err, sizeof(keep));
+    marut_mesh_destroy(m);
+    cudaGetLastError();
+    memcpy(g_err, keep, sizeof(keep));
+    return st;
+  }
+  *out = m;
+  return MARUT_OK;
+}
+
+// ------------------------------------------------------------------------------------ operator / stage
+static bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc, const double *u_n, const double *u_in,
+                                 double *u_out, cudaStream_t st) {
+  if (m->physics == MARUT_NAVIER_STOKES) {
+    GradParams G;
+    G.u = u_in; G.S = m->d_S; G.metric = m->d_metric; G.conn = m->d_conn;
+    G.gamma = m->gamma; G.inv_wb = 1.0 / m->w[0]; G.ne = m->ne;
+    memcpy(G.D, m->D, sizeof(G.D));
+    cudaError_t e = launch_gradient(m->dim, m->np, m->affine, G, st);
+    if (e != cudaSuccess) return fail(e == cudaErrorNotSupported ? MARUT_EINVAL : MARUT_ECUDA, "gradient kernel: %s", cudaGetErrorString(e));
+    m->launches++;
+  }
+  if (m->physics == MARUT_REACTING_EULER) {
+    const long total = m->ne * m->nn;
+    const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * 16);
+    if (m->dim == 2) eos_kernel<2, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn);
+    else eos_kernel<3, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(MARUT_ECUDA, "eos kernel: %s", cudaGetErrorString(e));
+    m->launches++;
+  }
+  StageParams P;
+  P.u_in = u_in; P.u_n = u_n; P.u_out = u_out;
+  P.metric = m->d_metric; P.conn = m->d_conn; P.mortar_fine = m->d_mortar_fine; P.mortar_mat = m->d_mortar_mat;
+  P.bc_state = m->d_bc; P.S = m->d_S; P.Taux = m->d_T; P.mech = m->d_mech;
+  P.ca = ca; P.cb = cb; P.cc = cc;
+  P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne;
+  memcpy(P.D, m->D, sizeof(P.D));
+  cudaError_t e;
+  switch (m->physics) {
+    case MARUT_EULER: e = (m->dim == 2) ? launch_stage_euler2d(m->np, m->affine, P, st) : launch_stage_euler3d(m->np, m->affine, P, st); break;
+    case MARUT_NAVIER_STOKES: e = launch_stage_ns(m->dim, m->np, m->affine, P, st); break;
+    default: e = launch_stage_react(m->dim, m->np, m->nsp, m->affine, P, st); break;
+  }
+  if (e == cudaErrorNotSupported) return fail(MARUT_EINVAL, "no kernel instantiated for dim=%d N=%d physics=%d", m->dim, m->N, m->physics);
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "stage kernel: %s", cudaGetErrorString(e));
+  m->launches++;
+  return MARUT_OK;
+}
+
+extern "C" marut_status marut_rhs(marut_mesh *m, const double *u, double *du, double /*t*/, void *stream) {
+  if (!m || !u || !du) return fail(MARUT_EINVAL, "NULL argument");
+  if (u == du) return fail(MARUT_EINVAL, "du must not alias u");
+  if (misaligned(u) || misaligned(du)) return fail(MARUT_EINVAL, "buffers must be 16-byte aligned");
+  return run_operator(m, 0.0, 0.0, 1.0, nullptr, u, du, (cudaStream_t)stream);
+}
+
+extern "C" marut_status marut_ssprk_stage(marut_mesh *m, int stage, double dt, double /*t_n*/, const double *u_n,
+                                          const double *u_in, double *u_out, void *stream) {
+  if (!m || !u_in || !u_out) return fail(MARUT_EINVAL, "NULL argument");
+  if (stage < 0 || stage > 2) return fail(MARUT_EINVAL, "stage must be 0, 1 or 2");
+  if (stage > 0 && !u_n) return fail(MARUT_EINVAL, "u_n is NULL");
+  if (u_out == u_in) return fail(MARUT_EINVAL, "u_out must not alias u_in");
+  if (misaligned(u_in) || misaligned(u_out) || (stage > 0 && misaligned(u_n))) return fail(MARUT_EINVAL, "buffers must be 16-byte aligned");
+  // Shu-Osher SSP-RK33: u_out = a u_n + b (u_in + dt L(u_in))
+  static const double a[3] = {0.0, 0.75, 1.0 / 3.0}, b[3] = {1.0, 0.25, 2.0 / 3.0};
+  return run_operator(m, a[stage], b[stage], b[stage] * dt, u_n, u_in, u_out, (cudaStream_t)stream);
+}
+
+extern "C" marut_status marut_chem_source(marut_mesh *m, const double *u, double *s, void *stream) {
+  if (!m || !u || !s) return fail(MARUT_EINVAL, "NULL argument");
+  if (m->physics != MARUT_REACTING_EULER) return fail(MARUT_EINVAL, "marut_chem_source needs a REACTING_EULER mesh");
+  if (u == s) return fail(MARUT_EINVAL, "s must not alias u");
+  const long total = m->ne * m->nn;
+  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * 16);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (m->dim == 2) chem_kernel<2, 5><<<grid, 256, 0, st>>>(u, s, m->d_mech, m->ne, m->nn);
+  else chem_kernel<3, 5><<<grid, 256, 0, st>>>(u, s, m->d_mech, m->ne, m->nn);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "chem kernel: %s", cudaGetErrorString(e));
+  m->launches++;
+  return MARUT_OK;
+}
+
+// ------------------------------------------------------------------------------------ time step
+template <int DIM>
+static cudaError_t run_wave_speed(marut_mesh *m, const double *u, unsigned grid, cudaStream_t st) {
+  switch (m->physics) {
+    case MARUT_EULER: wave_speed_kernel<DIM, 1, PH_EULER><<<grid, 256, 0, st>>>(u, nullptr, m->gamma, m->mu, m->ne, m->nn, m->d_red); break;
+    case MARUT_NAVIER_STOKES: wave_speed_kernel<DIM, 1, PH_NS><<<grid, 256, 0, st>>>(u, nullptr, m->gamma, m->mu, m->ne, m->nn, m->d_red); break;
+    default: wave_speed_kernel<DIM, 5, PH_REACT><<<grid, 256, 0, st>>>(u, m->d_mech, m->gamma, m->mu, m->ne, m->nn, m->d_red); break;
+  }
+  return cudaGetLastError();
+}
+
+extern "C" marut_status marut_max_dt(marut_mesh *m, const double *u, double cfl, double *dt_out, void *stream) {
+  if (!m || !u || !dt_out) return fail(MARUT_EINVAL, "NULL argument");
+  if (!(cfl > 0.0)) return fail(MARUT_EINVAL, "cfl must be positive");
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(cudaMemsetAsync(m->d_red, 0, 4 * sizeof(unsigned long long), st));
+  const long total = m->ne * m->nn;
+  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * 8);
+  cudaError_t e = (m->dim == 2) ? run_wave_speed<2>(m, u, grid, st) : run_wave_speed<3>(m, u, grid, st);
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "wave speed kernel: %s", cudaGetErrorString(e));
+  m->launches++;
+  CUDA_TRY(cudaMemcpyAsync(m->h_red, m->d_red, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  double lam, nu;
+  memcpy(&lam, &m->h_red[0], 8);
+  memcpy(&nu, &m->h_red[1], 8);
+  if (m->h_red[2] != 0 || !(lam > 0.0) || !std::isfinite(lam)) return fail(MARUT_ENOTFINITE, "non-finite or non-positive wave speed");
+  const double P2 = 2.0 * m->N + 1.0;
+  double dt = cfl * m->dx_min / (P2 * lam);                       // eq. 18
+  if (m->physics == MARUT_NAVIER_STOKES && nu > 0.0) {
+    const double numax = nu * std::max(1.0, 1.0 / m->Pr);
+    dt = std::min(dt, cfl * m->dx_min * m->dx_min / (P2 * P2 * numax));  // eq. 17
+  }
+  *dt_out = dt;
+  return MARUT_OK;
+}
+
+// ------------------------------------------------------------------------------------ introspection
+extern "C" marut_status marut_get_metrics(marut_mesh *m, double *Ja, double *J) {
+  if (!m || !Ja || !J) return fail(MARUT_EINVAL, "NULL argument");
+  const int dim = m->dim, nn = m->nn, MD = dim * dim + 1;
+  const size_t cnt = m->affine ? (size_t)m->ne * MD : (size_t)m->ne * MD * nn;
+  std::vector<double> h(cnt);
+  CUDA_TRY(cudaMemcpy(h.data(), m->d_metric, cnt * sizeof(double), cudaMemcpyDeviceToHost));
+  for (long e = 0; e < m->ne; ++e)
+    for (int p = 0; p < nn; ++p) {
+      for (int k = 0; k < dim * dim; ++k)
+        Ja[((size_t)e * nn + p) * dim * dim + k] = m->affine ? h[(size_t)e * MD + k] : h[((size_t)e * MD + k) * nn + p];
+      const double iJ = m->affine ? h[(size_t)e * MD + dim * dim] : h[((size_t)e * MD + dim * dim) * nn + p];
+      J[(size_t)e * nn + p] = 1.0 / iJ;
+    }
+  return MARUT_OK;
+}
+extern "C" int marut_is_affine(const marut_mesh *m) { return m && m->affine ? 1 : 0; }
+extern "C" double marut_dx_min(const marut_mesh *m) { return m ? m->dx_min : 0.0; }
+extern "C" long marut_launch_count(const marut_mesh *m) { return m ? m->launches : 0; }
+extern "C" const char *marut_last_error(void) { return g_err; }

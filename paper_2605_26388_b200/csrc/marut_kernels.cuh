@@ -1,0 +1,596 @@
+// marut_kernels.cuh -- the generic (any dim / degree / physics) kernels of the CUDA path:
+//   stage_kernel    : volume integral + interface/mortar/boundary flux + surface lift + 1/J
+//                     + source + SSP-RK33 combination, one pass over u
+//   gradient_kernel : BR1 gradient S = grad W (a6)
+//   eos_kernel      : mixture temperature by Newton (a8)
+//   chem_kernel     : chemistry source alone (marut_chem_source)
+//   wave_speed_kernel: max-wave-speed / max-diffusivity reduction (a10)
+//   metrics_kernel  : GCL-preserving metric terms (a0)
+// Thread mapping: one thread per LGL node, EB consecutive elements per CTA.
+#pragma once
+#include "marut_common.cuh"
+#include "marut_physics.cuh"
+
+namespace marut {
+
+template <int DIM, int NP>
+struct Geo {
+  static constexpr int NN = (DIM == 2) ? NP * NP : NP * NP * NP;
+  static constexpr int NF = (DIM == 2) ? NP : NP * NP;   // nodes per face
+  static constexpr int MD = DIM * DIM + 1;               // metric planes: Ja^l_c (l-major) and 1/J
+  __device__ static __forceinline__ void ijk(int p, int *q) {
+    q[0] = p % NP;
+    q[1] = (p / NP) % NP;
+    if (DIM == 3) q[2] = p / (NP * NP);
+  }
+  __device__ static __forceinline__ int node(const int *q) {
+    return (DIM == 2) ? q[0] + NP * q[1] : q[0] + NP * (q[1] + NP * q[2]);
+  }
+  // stride of reference direction l in the node index
+  __device__ static __forceinline__ int stride(int l) { return l == 0 ? 1 : (l == 1 ? NP : NP * NP); }
+  // volume node of face node (a0,a1) on face f
+  __device__ static __forceinline__ int face_node(int f, int a0, int a1) {
+    const int l = f >> 1, s = (f & 1) ? NP - 1 : 0;
+    int q[3];
+    if (DIM == 2) {
+      q[l] = s;
+      q[1 - l] = a0;
+    } else {
+      q[l] = s;
+      q[l == 0 ? 1 : 0] = a0;
+      q[l == 2 ? 1 : 2] = a1;
+    }
+    return node(q);
+  }
+  // face-node coordinates of volume node q on a face normal to l
+  __device__ static __forceinline__ void face_coords(const int *q, int l, int &a0, int &a1) {
+    if (DIM == 2) {
+      a0 = q[1 - l];
+      a1 = 0;
+    } else {
+      a0 = q[l == 0 ? 1 : 0];
+      a1 = q[l == 2 ? 1 : 2];
+    }
+  }
+};
+
+template <int DIM, int NP, bool AFFINE>
+__device__ __forceinline__ double metric_at(const double *__restrict__ metric, long e, int plane, int p) {
+  using G = Geo<DIM, NP>;
+  return AFFINE ? __ldg(&metric[e * G::MD + plane]) : __ldg(&metric[(e * G::MD + plane) * G::NN + p]);
+}
+
+// state (+T for reacting) -> primitives
+template <int DIM, int NSP, int PHYS, bool WANT_A>
+__device__ __forceinline__ Prim<DIM> make_prim(const double *U, double T, double gamma, const MechDev *mech) {
+  if constexpr (PHYS == PH_REACT) return prim_mixture<DIM, NSP, WANT_A>(U, T, *mech);
+  else return prim_ideal<DIM, WANT_A>(U, gamma);
+}
+
+// ======================================================================================
+// fused stage kernel
+// ======================================================================================
+template <int DIM, int NP, int NSP, int PHYS, bool AFFINE, int EB>
+__global__ void __launch_bounds__(((EB * Geo<DIM, NP>::NN + 31) / 32) * 32)
+stage_kernel(const __grid_constant__ StageParams P) {
+  using G = Geo<DIM, NP>;
+  constexpr int NN = G::NN, NVAR = NSP + DIM + 1, NW = DIM + 2, MD = G::MD;
+  constexpr int TILE = EB * NN;
+  extern __shared__ double smem[];
+  double *Fsm = smem;                         // [DIM][NVAR][TILE] contravariant fluxes
+  double *Dsm = smem + DIM * NVAR * TILE;     // [NP*NP]
+  __shared__ MechDev mech_s;
+
+  const int tid = threadIdx.x;
+  for (int i = tid; i < NP * NP; i += blockDim.x) Dsm[i] = P.D[i];
+  if constexpr (PHYS == PH_REACT) {
+    const int *src = reinterpret_cast<const int *>(P.mech);
+    int *dst = reinterpret_cast<int *>(&mech_s);
+    for (int i = tid; i < (int)(sizeof(MechDev) / sizeof(int)); i += blockDim.x) dst[i] = src[i];
+    __syncthreads();
+  }
+  const MechDev *mech = (PHYS == PH_REACT) ? &mech_s : nullptr;
+
+  const int el = tid / NN, p = tid - el * NN;
+  const long e = (long)blockIdx.x * EB + el;
+  const bool active = (tid < TILE) && (e < P.ne);
+  int q[3] = {0, 0, 0};
+  G::ijk(p, q);
+
+  double U[NVAR], Ja[DIM * DIM], invJ = 0.0, T = 0.0, Sg[(PHYS == PH_NS) ? NW * DIM : 1];
+  Prim<DIM> pr;
+  if (active) {
+    const double *up = P.u_in + e * NVAR * NN + p;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
+#pragma unroll
+    for (int k = 0; k < DIM * DIM; ++k) Ja[k] = metric_at<DIM, NP, AFFINE>(P.metric, e, k, p);
+    invJ = metric_at<DIM, NP, AFFINE>(P.metric, e, DIM * DIM, p);
+    if constexpr (PHYS == PH_REACT) T = __ldg(&P.Taux[e * NN + p]);
+    pr = make_prim<DIM, NSP, PHYS, true>(U, T, P.gamma, mech);
+    if constexpr (PHYS == PH_NS) {
+#pragma unroll
+      for (int k = 0; k < NW * DIM; ++k) Sg[k] = __ldg(&P.S[(e * NW * DIM + k) * NN + p]);
+    }
+    // contravariant fluxes Ftilde^l = Ja^l . (F_inv - F_v)   (eq. 9)
+#pragma unroll
+    for (int l = 0; l < DIM; ++l) {
+      double F[NVAR];
+      flux_dot<DIM, NSP>(U, pr, &Ja[l * DIM], F);
+      if constexpr (PHYS == PH_NS) {
+        double Fv[NW];
+        viscous_flux_dot<DIM>(pr.v, Sg, &Ja[l * DIM], P.mu, P.kappa, Fv);
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) F[v] -= Fv[v];
+      }
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Fsm[(l * NVAR + v) * TILE + tid] = F[v];
+    }
+  }
+  __syncthreads();
+  if (!active) return;
+
+  // ---- volume term: sum_l sum_m D[i_l][m] Ftilde^l(m)
+  double R[NVAR];
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) R[v] = 0.0;
+#pragma unroll
+  for (int l = 0; l < DIM; ++l) {
+    const int st = G::stride(l);
+    const int base = tid - q[l] * st;
+    double Drow[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) Drow[m] = Dsm[q[l] * NP + m];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) {
+      const double *Fl = &Fsm[(l * NVAR + v) * TILE + base];
+      double acc = 0.0;
+#pragma unroll
+      for (int m = 0; m < NP; ++m) acc += Drow[m] * Fl[m * st];
+      R[v] += acc;
+    }
+  }
+
+  // ---- surface term: (1/w_b) sum_f (F* - Ftilde).n_ref   (eq. 12)
+#pragma unroll
+  for (int l = 0; l < DIM; ++l) {
+    if (q[l] != 0 && q[l] != NP - 1) continue;
+    const int side = (q[l] == 0) ? 0 : 1;
+    const int f = 2 * l + side;
+    const double sgn = side ? 1.0 : -1.0;
+    const int2 cn = __ldg(&P.conn[e * 2 * DIM + f]);
+    const int kind = cn.y & 3, fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7, sub = (cn.y >> 8) & 1;
+    double nv[DIM], Fown[NVAR], Fs[NVAR];
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) nv[c] = sgn * Ja[l * DIM + c];
+    int a0, a1;
+    G::face_coords(q, l, a0, a1);
+    if (kind == FK_CONFORMING || kind == FK_BOUNDARY) {
+      double Up[NVAR], Tp = 0.0;
+      int pR = 0;
+      if (kind == FK_CONFORMING) {
+        const int b0 = (DIM == 2 && orient) ? NP - 1 - a0 : a0;
+        pR = G::face_node(fR, b0, a1);
+        const double *un = P.u_in + (long)cn.x * NVAR * NN + pR;
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
+        if constexpr (PHYS == PH_REACT) Tp = __ldg(&P.Taux[(long)cn.x * NN + pR]);
+      } else {
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(&P.bc_state[cn.x * NVAR + v]);
+      }
+      const Prim<DIM> qp = make_prim<DIM, NSP, PHYS, true>(Up, Tp, P.gamma, mech);
+      double Fm[NVAR];
+      flux_dot<DIM, NSP>(U, pr, nv, Fm);
+      rusanov<DIM, NSP>(U, pr, Fm, Up, qp, nv, Fs);
+      if constexpr (PHYS == PH_NS) {
+        // BR1 viscous interface flux: mean of the two sides (eq. 16)
+        double Sp[NW * DIM], Fvm[NW], Fvp[NW];
+#pragma unroll
+        for (int k = 0; k < NW * DIM; ++k) Sp[k] = __ldg(&P.S[((long)cn.x * NW * DIM + k) * NN + pR]);
+        viscous_flux_dot<DIM>(pr.v, Sg, nv, P.mu, P.kappa, Fvm);
+        viscous_flux_dot<DIM>(qp.v, Sp, nv, P.mu, P.kappa, Fvp);
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Fs[v] -= 0.5 * (Fvm[v] + Fvp[v]);
+      }
+    } else if constexpr (DIM == 2) {
+      const double *Pf = P.mortar_mat, *Prv = P.mortar_mat + 2 * NP * NP;
+      if (kind == FK_MORTAR_FINE) {
+        // exterior state = coarse trace interpolated to this half of the coarse face
+        double Up[NVAR];
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Up[v] = 0.0;
+        for (int j = 0; j < NP; ++j) {
+          const double w = __ldg(&Pf[(sub * NP + a0) * NP + j]);
+          const double *uc = P.u_in + (long)cn.x * NVAR * NN + G::face_node(fR, j, 0);
+#pragma unroll
+          for (int v = 0; v < NVAR; ++v) Up[v] += w * __ldg(uc + v * NN);
+        }
+        const Prim<DIM> qp = make_prim<DIM, NSP, PHYS, true>(Up, 0.0, P.gamma, mech);
+        double Fm[NVAR];
+        flux_dot<DIM, NSP>(U, pr, nv, Fm);
+        rusanov<DIM, NSP>(U, pr, Fm, Up, qp, nv, Fs);
+      } else {
+        // coarse side: Riemann problem on both mortars with the fine-side normal, projected back with
+        // the area factor 2:  F*_C = sum_m P_rev^m (2 * (-F*_m))
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Fs[v] = 0.0;
+        for (int m = 0; m < 2; ++m) {
+          const long eF = __ldg(&P.mortar_fine[cn.x * 2 + m]);
+          const int lF = fR >> 1;
+          const double sF = (fR & 1) ? 1.0 : -1.0;
+          for (int a = 0; a < NP; ++a) {
+            const int pF = G::face_node(fR, a, 0);
+            double UF[NVAR], UC[NVAR], nF[DIM], FmF[NVAR], Fsm_[NVAR];
+#pragma unroll
+            for (int v = 0; v < NVAR; ++v) {
+              UF[v] = __ldg(P.u_in + (eF * NVAR + v) * NN + pF);
+              UC[v] = 0.0;
+            }
+            for (int j = 0; j < NP; ++j) {
+              const double w = __ldg(&Pf[(m * NP + a) * NP + j]);
+              const double *uc = P.u_in + e * NVAR * NN + G::face_node(f, j, 0);
+#pragma unroll
+              for (int v = 0; v < NVAR; ++v) UC[v] += w * __ldg(uc + v * NN);
+            }
+#pragma unroll
+            for (int c = 0; c < DIM; ++c) nF[c] = sF * metric_at<DIM, NP, AFFINE>(P.metric, eF, lF * DIM + c, pF);
+            const Prim<DIM> qF = make_prim<DIM, NSP, PHYS, true>(UF, 0.0, P.gamma, mech);
+            const Prim<DIM> qC = make_prim<DIM, NSP, PHYS, true>(UC, 0.0, P.gamma, mech);
+            flux_dot<DIM, NSP>(UF, qF, nF, FmF);
+            rusanov<DIM, NSP>(UF, qF, FmF, UC, qC, nF, Fsm_);
+            const double w2 = -2.0 * __ldg(&Prv[(m * NP + a0) * NP + a]);
+#pragma unroll
+            for (int v = 0; v < NVAR; ++v) Fs[v] += w2 * Fsm_[v];
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) {
+      Fown[v] = sgn * Fsm[(l * NVAR + v) * TILE + tid];
+      R[v] += P.inv_wb * (Fs[v] - Fown[v]);
+    }
+  }
+
+  // ---- 1/J, source, SSP-RK combination (eq. 45)
+  double src[NVAR];
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) src[v] = 0.0;
+  if constexpr (PHYS == PH_REACT) production_rates<NSP>(*mech, T, U, src);
+  double *op = P.u_out + e * NVAR * NN + p;
+  if (P.ca != 0.0) {
+    const double *np_ = P.u_n + e * NVAR * NN + p;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v)
+      op[v * NN] = P.ca * np_[v * NN] + (P.cb * U[v] + P.cc * (src[v] - invJ * R[v]));
+  } else {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.cb * U[v] + P.cc * (src[v] - invJ * R[v]);
+  }
+}
+
+// ======================================================================================
+// BR1 gradient  S = (1/J) [ sum_l D_l(Ja^l_c W) + (1/w_b) (What - W) n_c ]  (eq. 13)
+// ======================================================================================
+struct GradParams {
+  const double *__restrict__ u;
+  double *__restrict__ S;
+  const double *__restrict__ metric;
+  const int2 *__restrict__ conn;
+  double gamma, inv_wb;
+  long ne;
+  double D[MAX_NP * MAX_NP];
+};
+
+template <int DIM, int NP, bool AFFINE, int EB>
+__global__ void __launch_bounds__(((EB * Geo<DIM, NP>::NN + 31) / 32) * 32)
+gradient_kernel(const __grid_constant__ GradParams P) {
+  using G = Geo<DIM, NP>;
+  constexpr int NN = G::NN, NVAR = DIM + 2, NW = DIM + 2, MD = G::MD, TILE = EB * NN;
+  extern __shared__ double smem[];
+  double *Wsm = smem;                 // [NW][TILE]
+  double *Dsm = smem + NW * TILE;     // [NP*NP]
+  const int tid = threadIdx.x;
+  for (int i = tid; i < NP * NP; i += blockDim.x) Dsm[i] = P.D[i];
+  const int el = tid / NN, p = tid - el * NN;
+  const long e = (long)blockIdx.x * EB + el;
+  const bool active = (tid < TILE) && (e < P.ne);
+  int q[3] = {0, 0, 0};
+  G::ijk(p, q);
+  double W[NW];
+  if (active) {
+    double U[NVAR];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(P.u + (e * NVAR + v) * NN + p);
+    const Prim<DIM> pr = prim_ideal<DIM, false>(U, P.gamma);
+    W[0] = pr.rho;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) W[1 + c] = pr.v[c];
+    W[1 + DIM] = pr.T;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) Wsm[w * TILE + tid] = W[w];
+  }
+  __syncthreads();
+  if (!active) return;
+  double Sg[NW * DIM];
+#pragma unroll
+  for (int k = 0; k < NW * DIM; ++k) Sg[k] = 0.0;
+#pragma unroll
+  for (int l = 0; l < DIM; ++l) {
+    const int st = G::stride(l), base = tid - q[l] * st, pbase = p - q[l] * st;
+    for (int m = 0; m < NP; ++m) {
+      const double d = Dsm[q[l] * NP + m];
+      double Jm[DIM];
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) Jm[c] = d * metric_at<DIM, NP, AFFINE>(P.metric, e, l * DIM + c, pbase + m * st);
+#pragma unroll
+      for (int w = 0; w < NW; ++w) {
+        const double Wm = Wsm[w * TILE + base + m * st];
+#pragma unroll
+        for (int c = 0; c < DIM; ++c) Sg[w * DIM + c] += Jm[c] * Wm;
+      }
+    }
+  }
+#pragma unroll
+  for (int l = 0; l < DIM; ++l) {
+    if (q[l] != 0 && q[l] != NP - 1) continue;
+    const int side = (q[l] == 0) ? 0 : 1, f = 2 * l + side;
+    const double sgn = side ? 1.0 : -1.0;
+    const int2 cn = __ldg(&P.conn[e * 2 * DIM + f]);
+    const int fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7;
+    int a0, a1;
+    G::face_coords(q, l, a0, a1);
+    const int b0 = (DIM == 2 && orient) ? NP - 1 - a0 : a0;
+    const int pR = G::face_node(fR, b0, a1);
+    double Up[NVAR];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(P.u + ((long)cn.x * NVAR + v) * NN + pR);
+    const Prim<DIM> qp = prim_ideal<DIM, false>(Up, P.gamma);
+    double Wp[NW];
+    Wp[0] = qp.rho;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) Wp[1 + c] = qp.v[c];
+    Wp[1 + DIM] = qp.T;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) {
+      const double nc = sgn * metric_at<DIM, NP, AFFINE>(P.metric, e, l * DIM + c, p) * P.inv_wb;
+#pragma unroll
+      for (int w = 0; w < NW; ++w) Sg[w * DIM + c] += 0.5 * (Wp[w] - W[w]) * nc;
+    }
+  }
+  const double invJ = metric_at<DIM, NP, AFFINE>(P.metric, e, DIM * DIM, p);
+#pragma unroll
+  for (int k = 0; k < NW * DIM; ++k) P.S[(e * NW * DIM + k) * NN + p] = invJ * Sg[k];
+}
+
+// ======================================================================================
+// per-node kernels for the reacting mixture
+// ======================================================================================
+__device__ __forceinline__ void load_mech(MechDev *dst_s, const MechDev *src_g) {
+  const int *src = reinterpret_cast<const int *>(src_g);
+  int *dst = reinterpret_cast<int *>(dst_s);
+  for (int i = threadIdx.x; i < (int)(sizeof(MechDev) / sizeof(int)); i += blockDim.x) dst[i] = src[i];
+  __syncthreads();
+}
+
+// T[e][node] by Newton (a8)
+template <int DIM, int NSP>
+__global__ void __launch_bounds__(256) eos_kernel(const double *__restrict__ u, double *__restrict__ Tout,
+                                                  const MechDev *__restrict__ mech_g, long ne, int nn) {
+  constexpr int NVAR = NSP + DIM + 1;
+  __shared__ MechDev mech;
+  load_mech(&mech, mech_g);
+  const long total = ne * nn;
+  for (long g = (long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
+    const long e = g / nn;
+    const int p = (int)(g - e * nn);
+    double U[NVAR];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(u + (e * NVAR + v) * nn + p);
+    Tout[g] = temperature_newton<NSP>(mech, U, internal_energy<DIM, NSP>(U));
+  }
+}
+
+// s = S(u): omega_s for the species rows, 0 for momentum and energy (eq. 20-22)
+template <int DIM, int NSP>
+__global__ void __launch_bounds__(256) chem_kernel(const double *__restrict__ u, double *__restrict__ s,
+                                                   const MechDev *__restrict__ mech_g, long ne, int nn) {
+  constexpr int NVAR = NSP + DIM + 1;
+  __shared__ MechDev mech;
+  load_mech(&mech, mech_g);
+  const long total = ne * nn;
+  for (long g = (long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
+    const long e = g / nn;
+    const int p = (int)(g - e * nn);
+    double U[NVAR], om[NSP];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(u + (e * NVAR + v) * nn + p);
+    const double T = temperature_newton<NSP>(mech, U, internal_energy<DIM, NSP>(U));
+    production_rates<NSP>(mech, T, U, om);
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) s[(e * NVAR + v) * nn + p] = (v < NSP) ? om[v] : 0.0;
+  }
+}
+
+// ======================================================================================
+// max wave speed / max diffusivity (a10; eq. 17-18): warp-shuffle reduction, one atomicMax per CTA.
+// red[0] = max(|u|_2 + a) ; red[1] = max(mu/rho) ; red[2] = count of non-finite/non-positive speeds
+// (bit patterns of non-negative doubles order like unsigned integers)
+// ======================================================================================
+template <int DIM, int NSP, int PHYS>
+__global__ void __launch_bounds__(256) wave_speed_kernel(const double *__restrict__ u, const MechDev *__restrict__ mech_g,
+                                                         double gamma, double mu, long ne, int nn,
+                                                         unsigned long long *__restrict__ red) {
+  constexpr int NVAR = NSP + DIM + 1;
+  __shared__ MechDev mech;
+  __shared__ double wl[8], wn[8];
+  __shared__ int wbad[8];
+  if constexpr (PHYS == PH_REACT) load_mech(&mech, mech_g);
+  double lam = 0.0, nu = 0.0;
+  int bad = 0;
+  const long total = ne * nn;
+  for (long g = (long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
+    const long e = g / nn;
+    const int p = (int)(g - e * nn);
+    double U[NVAR];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(u + (e * NVAR + v) * nn + p);
+    Prim<DIM> q;
+    if constexpr (PHYS == PH_REACT) {
+      const double T = temperature_newton<NSP>(mech, U, internal_energy<DIM, NSP>(U));
+      q = prim_mixture<DIM, NSP, true>(U, T, mech);
+    } else q = prim_ideal<DIM, true>(U, gamma);
+    double v2 = 0.0;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) v2 += q.v[c] * q.v[c];
+    const double l = sqrt(v2) + q.a;
+    if (!(l > 0.0) || !isfinite(l)) bad = 1;
+    lam = fmax(lam, l);
+    if constexpr (PHYS == PH_NS) nu = fmax(nu, mu / q.rho);
+  }
+  lam = warp_max(lam);
+  nu = warp_max(nu);
+  bad = __any_sync(0xffffffffu, bad);
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) { wl[w] = lam; wn[w] = nu; wbad[w] = bad; }
+  __syncthreads();
+  if (w == 0) {
+    lam = (lane < (int)(blockDim.x >> 5)) ? wl[lane] : 0.0;
+    nu = (lane < (int)(blockDim.x >> 5)) ? wn[lane] : 0.0;
+    bad = (lane < (int)(blockDim.x >> 5)) ? wbad[lane] : 0;
+    lam = warp_max(lam);
+    nu = warp_max(nu);
+    bad = __any_sync(0xffffffffu, bad);
+    if (lane == 0) {
+      atomicMax(&red[0], (unsigned long long)__double_as_longlong(lam));
+      atomicMax(&red[1], (unsigned long long)__double_as_longlong(nu));
+      if (bad) atomicAdd(&red[2], 1ULL);
+    }
+  }
+}
+
+// ======================================================================================
+// metric terms (a0; R2).  One CTA per element, one thread per node.
+// out: metric_full [e][MD][NN] (Ja^l_c planes then 1/J); elem_info [e][2] = {min J, max relative
+// deviation of any metric plane from its node-0 value}
+// ======================================================================================
+template <int DIM, int NP>
+__global__ void metrics_kernel(const double *__restrict__ xyz, double *__restrict__ metric_full,
+                               double *__restrict__ elem_info, const double *__restrict__ Dg, long ne) {
+  using G = Geo<DIM, NP>;
+  constexpr int NN = G::NN, MD = G::MD;
+  extern __shared__ double smem[];
+  double *X = smem;                    // [DIM][NN]
+  double *dX = X + DIM * NN;           // [DIM*DIM][NN]   dX[c*DIM+l] = d X_c / d xi_l
+  double *Dsm = dX + DIM * DIM * NN;   // [NP*NP]
+  double *ref = Dsm + NP * NP;         // [MD + 1]
+  const long e = blockIdx.x;
+  const int p = threadIdx.x;
+  for (int i = p; i < NP * NP; i += NN) Dsm[i] = Dg[i];
+  for (int c = 0; c < DIM; ++c) X[c * NN + p] = xyz[(e * DIM + c) * NN + p];
+  __syncthreads();
+  int q[3] = {0, 0, 0};
+  G::ijk(p, q);
+  auto deriv = [&](auto f, int l) {   // sum_m D[q_l][m] f(node with q_l -> m)
+    const int st = G::stride(l), base = p - q[l] * st;
+    double acc = 0.0;
+    for (int m = 0; m < NP; ++m) acc += Dsm[q[l] * NP + m] * f(base + m * st);
+    return acc;
+  };
+  for (int c = 0; c < DIM; ++c)
+    for (int l = 0; l < DIM; ++l) dX[(c * DIM + l) * NN + p] = deriv([&](int r) { return X[c * NN + r]; }, l);
+  __syncthreads();
+  double Ja[DIM * DIM], J;
+  if constexpr (DIM == 2) {
+    const double x_xi = dX[0 * NN + p], x_eta = dX[1 * NN + p], y_xi = dX[2 * NN + p], y_eta = dX[3 * NN + p];
+    Ja[0] = y_eta; Ja[1] = -x_eta; Ja[2] = -y_xi; Ja[3] = x_xi;
+    J = x_xi * y_eta - x_eta * y_xi;
+  } else {
+    auto g = [&](int c, int l) { return dX[(c * 3 + l) * NN + p]; };
+    J = g(0, 0) * (g(1, 1) * g(2, 2) - g(1, 2) * g(2, 1)) - g(0, 1) * (g(1, 0) * g(2, 2) - g(1, 2) * g(2, 0)) +
+        g(0, 2) * (g(1, 0) * g(2, 1) - g(1, 1) * g(2, 0));
+    // conservative curl form: (Ja^i)_c = d_k[X_l d_j X_m] - d_j[X_l d_k X_m], (i,j,k), (c,m,l) cyclic
+    for (int i = 0; i < 3; ++i) {
+      const int j = (i + 1) % 3, k = (i + 2) % 3;
+      for (int c = 0; c < 3; ++c) {
+        const int mm = (c + 1) % 3, ll = (c + 2) % 3;
+        const double A = deriv([&](int r) { return X[ll * NN + r] * dX[(mm * 3 + j) * NN + r]; }, k);
+        const double B = deriv([&](int r) { return X[ll * NN + r] * dX[(mm * 3 + k) * NN + r]; }, j);
+        Ja[i * 3 + c] = A - B;
+      }
+    }
+  }
+  double *out = metric_full + e * MD * NN;
+  for (int k = 0; k < DIM * DIM; ++k) out[k * NN + p] = Ja[k];
+  out[DIM * DIM * NN + p] = 1.0 / J;
+  // element reductions: min J and affinity measure (max relative deviation from the node-0 values)
+  if (p == 0) {
+    double s = 0.0;
+    for (int k = 0; k < DIM * DIM; ++k) { ref[k] = Ja[k]; s = fmax(s, fabs(Ja[k])); }
+    ref[DIM * DIM] = J;
+    ref[MD] = s;
+  }
+  __syncthreads();   // also: every thread is done reading X / dX
+  double dev = fabs(J - ref[DIM * DIM]) / fabs(ref[DIM * DIM]);
+  for (int k = 0; k < DIM * DIM; ++k) dev = fmax(dev, fabs(Ja[k] - ref[k]) / ref[MD]);
+  double *redJ = dX, *redD = dX + NN;
+  redJ[p] = J;
+  redD[p] = dev;
+  __syncthreads();
+  if (p == 0) {
+    double mn = redJ[0], mx = redD[0];
+    for (int r = 1; r < NN; ++r) { mn = fmin(mn, redJ[r]); mx = fmax(mx, redD[r]); }
+    elem_info[e * 2 + 0] = mn;
+    elem_info[e * 2 + 1] = mx;
+  }
+}
+
+// affine meshes: keep one metric set per element (node 0)
+template <int DIM, int NP>
+__global__ void compact_metrics_kernel(const double *__restrict__ metric_full, double *__restrict__ metric_el, long ne) {
+  using G = Geo<DIM, NP>;
+  const long g = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= ne * G::MD) return;
+  metric_el[g] = metric_full[g * G::NN];
+}
+
+// ---------------------------------------------------------------- launch helpers
+template <int NN>
+constexpr int elems_per_block() { return (256 / NN) < 1 ? 1 : 256 / NN; }
+
+template <int DIM, int NP, int NSP, int PHYS, bool AFFINE>
+cudaError_t launch_stage_t(const StageParams &P, cudaStream_t st) {
+  constexpr int NN = Geo<DIM, NP>::NN, EB = elems_per_block<NN>();
+  constexpr int threads = ((EB * NN + 31) / 32) * 32;
+  constexpr size_t smem = (size_t)(DIM * (NSP + DIM + 1) * EB * NN + NP * NP) * sizeof(double);
+  auto k = stage_kernel<DIM, NP, NSP, PHYS, AFFINE, EB>;
+  static bool attr = false;
+  if (!attr) {
+    cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    attr = true;
+  }
+  const long grid = (P.ne + EB - 1) / EB;
+  k<<<(unsigned)grid, threads, smem, st>>>(P);
+  return cudaGetLastError();
+}
+
+template <int DIM, int NP, bool AFFINE>
+cudaError_t launch_gradient_t(const GradParams &P, cudaStream_t st) {
+  constexpr int NN = Geo<DIM, NP>::NN, EB = elems_per_block<NN>();
+  constexpr int threads = ((EB * NN + 31) / 32) * 32;
+  constexpr size_t smem = (size_t)((DIM + 2) * EB * NN + NP * NP) * sizeof(double);
+  auto k = gradient_kernel<DIM, NP, AFFINE, EB>;
+  static bool attr = false;
+  if (!attr) {
+    cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    attr = true;
+  }
+  const long grid = (P.ne + EB - 1) / EB;
+  k<<<(unsigned)grid, threads, smem, st>>>(P);
+  return cudaGetLastError();
+}
+
+}  // namespace marut

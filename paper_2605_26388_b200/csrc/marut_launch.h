@@ -1,0 +1,13 @@
+// marut_launch.h -- launchers defined in the per-physics translation units (compiled in parallel).
+// Each returns cudaErrorNotSupported when (dim, n, n_species) was not instantiated.
+#pragma once
+#include "marut_common.cuh"
+
+namespace marut {
+struct GradParams;
+cudaError_t launch_stage_euler2d(int np, bool affine, const StageParams &P, cudaStream_t st);
+cudaError_t launch_stage_euler3d(int np, bool affine, const StageParams &P, cudaStream_t st);
+cudaError_t launch_stage_ns(int dim, int np, bool affine, const StageParams &P, cudaStream_t st);
+cudaError_t launch_gradient(int dim, int np, bool affine, const GradParams &P, cudaStream_t st);
+cudaError_t launch_stage_react(int dim, int np, int nsp, bool affine, const StageParams &P, cudaStream_t st);
+}  // namespace marut

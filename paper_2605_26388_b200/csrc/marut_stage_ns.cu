@@ -1,0 +1,35 @@
+// BR1 gradient + fused Navier-Stokes stage kernel instantiations: 2-D and 3-D, N = 1..5
+#include "marut_kernels.cuh"
+#include "marut_launch.h"
+namespace marut {
+template <int DIM, int NP>
+static cudaError_t go(bool affine, const StageParams &P, cudaStream_t st) {
+  return affine ? launch_stage_t<DIM, NP, 1, PH_NS, true>(P, st) : launch_stage_t<DIM, NP, 1, PH_NS, false>(P, st);
+}
+template <int DIM, int NP>
+static cudaError_t gr(bool affine, const GradParams &P, cudaStream_t st) {
+  return affine ? launch_gradient_t<DIM, NP, true>(P, st) : launch_gradient_t<DIM, NP, false>(P, st);
+}
+#define MARUT_NS_CASES(FN, ...)                                   \
+  if (dim == 2) switch (np) {                                     \
+      case 2: return FN<2, 2>(__VA_ARGS__);                       \
+      case 3: return FN<2, 3>(__VA_ARGS__);                       \
+      case 4: return FN<2, 4>(__VA_ARGS__);                       \
+      case 5: return FN<2, 5>(__VA_ARGS__);                       \
+      case 6: return FN<2, 6>(__VA_ARGS__);                       \
+    }                                                             \
+  if (dim == 3) switch (np) {                                     \
+      case 2: return FN<3, 2>(__VA_ARGS__);                       \
+      case 3: return FN<3, 3>(__VA_ARGS__);                       \
+      case 4: return FN<3, 4>(__VA_ARGS__);                       \
+      case 5: return FN<3, 5>(__VA_ARGS__);                       \
+      case 6: return FN<3, 6>(__VA_ARGS__);                       \
+    }                                                             \
+  return cudaErrorNotSupported;
+cudaError_t launch_stage_ns(int dim, int np, bool affine, const StageParams &P, cudaStream_t st) {
+  MARUT_NS_CASES(go, affine, P, st)
+}
+cudaError_t launch_gradient(int dim, int np, bool affine, const GradParams &P, cudaStream_t st) {
+  MARUT_NS_CASES(gr, affine, P, st)
+}
+}  // namespace marut

@@ -1,0 +1,134 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Sizes span several CTAs and a ragged tail.  Run on the B200 box."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from parity_util import RHS_TOL, RUN_TOL, gpu_run, parity_error
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+
+    return torch
+
+
+@pytest.fixture(scope="module")
+def mb():
+    import paper_2605_26388_b200 as mb
+
+    return mb
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    import oracle
+
+    return oracle
+
+
+SMALL = [("c1", None, 100), ("c2", 3, 6), ("c2", 4, 6), ("c3", 3, 5), ("c3", 4, 5), ("c4", 32, 20), ("c5", 3, 5), ("c5", 4, 5)]
+
+
+@pytest.mark.parametrize("name,cells,steps", SMALL)
+def test_rhs_and_run_parity(name, cells, steps, torch, mb, oracle):
+    c = wl.make_case(name, cells=cells, steps=steps)
+    om = oracle.OracleMesh(c.mesh)
+    gm = mb.MarutMesh(c.mesh)
+    u = torch.from_numpy(c.u0).cuda()
+    du = torch.empty_like(u)
+    gm.rhs(u, du)
+    torch.cuda.synchronize()
+    err = parity_error(du.cpu().numpy(), om.rhs(c.u0))
+    assert err.max() <= RHS_TOL, (name, err)
+    # time step
+    dt_g, dt_c = gm.max_dt(u, c.cfl), om.max_dt(c.u0, c.cfl)
+    assert abs(dt_g - dt_c) <= 1e-13 * dt_c
+    # one stage of each kind against the oracle's stage
+    un = torch.from_numpy(c.u0 * (1.0 + 1e-3)).cuda()
+    out = torch.empty_like(u)
+    for s in range(3):
+        gm.stage(s, dt_c, 0.0, un, u, out)
+        ref = om.ssprk_stage(s, dt_c, 0.0, c.u0 * (1.0 + 1e-3), c.u0)
+        assert parity_error(out.cpu().numpy(), ref).max() <= RHS_TOL, (name, s)
+    # the config's RK steps
+    ug, tg = gpu_run(gm, c.u0, c.steps, c.cfl, torch)
+    uc, tc, min_rho, min_p = om.run(c.u0, c.steps, cfl=c.cfl)
+    assert min_rho > 0 and min_p > 0
+    assert abs(tg - tc) <= 1e-12 * tc
+    err = parity_error(ug, uc)
+    assert err.max() <= RUN_TOL, (name, err)
+    gm.close()
+
+
+@pytest.mark.parametrize("name,cells", [("c1", 4), ("c2", 2), ("c3", 3), ("c4", 16)])
+def test_metrics_parity(name, cells, torch, mb, oracle):
+    c = wl.make_case(name, cells=cells)
+    Ja_c, J_c = oracle.OracleMesh(c.mesh).metrics()
+    gm = mb.MarutMesh(c.mesh)
+    Ja_g, J_g = gm.metrics()
+    assert gm.is_affine == (name != "c3")
+    assert np.abs(Ja_g - Ja_c).max() <= 1e-12 * np.abs(Ja_c).max()
+    assert np.abs(J_g / J_c - 1).max() <= 1e-12
+    assert abs(gm.dx_min / oracle.OracleMesh(c.mesh).dx_min - 1) < 1e-13
+    gm.close()
+
+
+def test_chem_source_parity(torch, mb, oracle):
+    c = wl.make_case("c5", cells=3)
+    om = oracle.OracleMesh(c.mesh)
+    gm = mb.MarutMesh(c.mesh)
+    u = torch.from_numpy(c.u0).cuda()
+    s = torch.empty_like(u)
+    gm.chem_source(u, s)
+    sg = s.cpu().numpy()
+    sc = om.chem_source(c.u0)
+    assert np.abs(sg[:, 5:, :]).max() == 0.0
+    assert parity_error(sg[:, :5, :], sc[:, :5, :]).max() <= RHS_TOL
+    gm.close()
+
+
+def test_aliasing_and_stage0_ignores_un(torch, mb, oracle):
+    c = wl.make_case("c1", cells=8)
+    gm = mb.MarutMesh(c.mesh)
+    u = torch.from_numpy(c.u0).cuda()
+    a, b = torch.empty_like(u), torch.empty_like(u)
+    gm.stage(0, 0.01, 0.0, None, u, a)          # u_n not read for stage 0
+    gm.stage(0, 0.01, 0.0, u, u, b)
+    assert torch.equal(a, b)
+    un = u.clone()
+    gm.stage(2, 0.01, 0.0, un, a, b)            # separate output ...
+    gm.stage(2, 0.01, 0.0, un, a, un)           # ... vs u_out aliasing u_n
+    assert torch.equal(un, b)
+    gm.close()
+
+
+def test_error_codes(torch, mb):
+    c = wl.make_case("c1", cells=4)
+    gm = mb.MarutMesh(c.mesh)
+    u = torch.from_numpy(c.u0).cuda()
+    with pytest.raises(mb.MarutError) as e:
+        gm.rhs(u, u)
+    assert e.value.status == 1
+    with pytest.raises(mb.MarutError):
+        gm.stage(3, 0.1, 0.0, u, u, torch.empty_like(u))
+    with pytest.raises(mb.MarutError):
+        gm.chem_source(u, torch.empty_like(u))      # not a reacting mesh
+    bad = wl.make_case("c1", cells=4).mesh
+    bad.iface = bad.iface[:-1]                       # one face without a neighbour
+    with pytest.raises(mb.MarutError) as e:
+        mb.MarutMesh(bad)
+    assert e.value.status == 4
+    bad = wl.make_case("c1", cells=4).mesh
+    bad.node_xyz = bad.node_xyz[:, :, ::-1].copy()   # inverted elements: J < 0
+    with pytest.raises(mb.MarutError) as e:
+        mb.MarutMesh(bad)
+    assert e.value.status == 4
+    un = torch.full_like(u, float("nan"))
+    with pytest.raises(mb.MarutError) as e:
+        gm.max_dt(un, 0.5)
+    assert e.value.status == 5
+    gm.close()
