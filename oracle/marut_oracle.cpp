@@ -51,13 +51,14 @@ enum Physics { EULER = 0, NAVIER_STOKES = 1, REACTING_EULER = 2 };
 // ---------------------------------------------------------------------------
 // Legendre polynomial P_N(x) and its derivative by the three-term recurrence
 //   (k+1) P_{k+1} = (2k+1) x P_k - k P_{k-1},   P'_{k+1} = P'_{k-1} + (2k+1) P_k.
-static void legendre(int N, double x, double &P, double &dP) {
-  double Pm = 1.0, dPm = 0.0;          // P_0
+template <typename T>
+static void legendre(int N, T x, T &P, T &dP) {
+  T Pm = 1, dPm = 0;                   // P_0
   if (N == 0) { P = Pm; dP = dPm; return; }
-  double Pc = x, dPc = 1.0;            // P_1
+  T Pc = x, dPc = 1;                   // P_1
   for (int k = 1; k < N; ++k) {
-    double Pn = ((2.0 * k + 1.0) * x * Pc - k * Pm) / (k + 1.0);
-    double dPn = dPm + (2.0 * k + 1.0) * Pc;
+    T Pn = ((2 * k + 1) * x * Pc - k * Pm) / (k + 1);
+    T dPn = dPm + (2 * k + 1) * Pc;
     Pm = Pc; dPm = dPc; Pc = Pn; dPc = dPn;
   }
   P = Pc; dP = dPc;
@@ -70,42 +71,50 @@ struct Ops {
 
 // LGL nodes: x_0=-1, x_N=+1 and the roots of P'_N; w_j = 2/(N(N+1) P_N(x_j)^2);
 // D by barycentric weights, diagonal = -(sum of the off-diagonals of the row).
+// Evaluated in extended precision (long double) and rounded once, so that x, w and D are the
+// correctly rounded doubles of their exact values (independent of the formula used to get them).
 static Ops make_ops(int N) {
+  typedef long double LD;
   Ops o; o.N = N; o.n = N + 1;
   const int n = o.n;
-  o.x.assign(n, 0.0); o.w.assign(n, 0.0); o.D.assign(n * n, 0.0);
-  o.x[0] = -1.0; o.x[N] = 1.0;
-  const double PI = 3.14159265358979323846;
+  std::vector<LD> x(n), w(n), D((size_t)n * n, 0);
+  x[0] = -1; x[N] = 1;
+  const LD PI = 3.141592653589793238462643383279502884L;
   for (int j = 1; j < N; ++j) {
-    double x = -std::cos(PI * j / N);            // Chebyshev-Lobatto starting guess
+    LD xj = -cosl(PI * j / N);                   // Chebyshev-Lobatto starting guess
     for (int it = 0; it < 100; ++it) {
-      double P, dP; legendre(N, x, P, dP);
+      LD P, dP; legendre<LD>(N, xj, P, dP);
       // Legendre ODE: (1-x^2) P'' = 2 x P' - N(N+1) P
-      double d2P = (2.0 * x * dP - N * (N + 1.0) * P) / (1.0 - x * x);
-      double dx = dP / d2P;
-      x -= dx;
-      if (std::fabs(dx) < 1e-16) break;
+      LD d2P = (2 * xj * dP - N * (N + 1) * P) / (1 - xj * xj);
+      LD dx = dP / d2P;
+      xj -= dx;
+      if (fabsl(dx) < 1e-20L) break;
     }
-    o.x[j] = x;
+    x[j] = xj;
   }
+  if (N % 2 == 0) x[N / 2] = 0;                  // the middle node is exactly 0 by symmetry
   for (int j = 0; j < n; ++j) {
-    double P, dP; legendre(N, o.x[j], P, dP);
-    o.w[j] = 2.0 / (N * (N + 1.0) * P * P);
+    LD P, dP; legendre<LD>(N, x[j], P, dP);
+    w[j] = 2 / (N * (N + 1) * P * P);
   }
-  std::vector<double> lam(n, 1.0);
+  std::vector<LD> lam(n, 1);
   for (int j = 0; j < n; ++j) {
-    double prod = 1.0;
-    for (int k = 0; k < n; ++k) if (k != j) prod *= (o.x[j] - o.x[k]);
-    lam[j] = 1.0 / prod;
+    LD prod = 1;
+    for (int k = 0; k < n; ++k) if (k != j) prod *= (x[j] - x[k]);
+    lam[j] = 1 / prod;
   }
   for (int i = 0; i < n; ++i) {
-    double s = 0.0;
+    LD sum = 0;
     for (int j = 0; j < n; ++j) if (j != i) {
-      o.D[i * n + j] = (lam[j] / lam[i]) / (o.x[i] - o.x[j]);
-      s += o.D[i * n + j];
+      D[i * n + j] = (lam[j] / lam[i]) / (x[i] - x[j]);
+      sum += D[i * n + j];
     }
-    o.D[i * n + i] = -s;
+    D[i * n + i] = -sum;
   }
+  if (N % 2 == 0) D[(N / 2) * n + N / 2] = 0;    // antisymmetry of D about the centre: exact zero
+  o.x.resize(n); o.w.resize(n); o.D.resize((size_t)n * n);
+  for (int j = 0; j < n; ++j) { o.x[j] = (double)x[j]; o.w[j] = (double)w[j]; }
+  for (int k = 0; k < n * n; ++k) o.D[k] = (double)D[k];
   return o;
 }
 
@@ -123,11 +132,11 @@ static void gauss_legendre(int m, std::vector<double> &g, std::vector<double> &w
   for (int q = 0; q < m; ++q) {
     double x = -std::cos(PI * (q + 0.75) / (m + 0.5));
     for (int it = 0; it < 100; ++it) {
-      double P, dP; legendre(m, x, P, dP);
+      double P, dP; legendre<double>(m, x, P, dP);
       double dx = P / dP; x -= dx;
       if (std::fabs(dx) < 1e-16) break;
     }
-    double P, dP; legendre(m, x, P, dP);
+    double P, dP; legendre<double>(m, x, P, dP);
     g[q] = x; wg[q] = 2.0 / ((1.0 - x * x) * dP * dP);
   }
 }
@@ -155,10 +164,10 @@ static void make_mortar(const Ops &o, std::vector<double> Pf[2], std::vector<dou
           // q_k = (2k+1)/2 * 1/2 * int_{-1}^{1} l_j(eta) L_k((eta+shift)/2) d eta
           double integ = 0.0;
           for (int q = 0; q < n; ++q) {
-            double Lk, dLk; legendre(k, (g[q] + shift) / 2.0, Lk, dLk);
+            double Lk, dLk; legendre<double>(k, (g[q] + shift) / 2.0, Lk, dLk);
             integ += wg[q] * lagrange(o.x, j, g[q]) * Lk;
           }
-          double Lki, dLki; legendre(k, o.x[i], Lki, dLki);
+          double Lki, dLki; legendre<double>(k, o.x[i], Lki, dLki);
           acc += Lki * (2.0 * k + 1.0) / 2.0 * 0.5 * integ;
         }
         Pr[m][i * n + j] = acc;
@@ -327,8 +336,17 @@ static void compute_metrics(Mesh &m) {
   m.J.assign((size_t)m.ne * nn, 0.0);
 #pragma omp parallel for schedule(static)
   for (long e = 0; e < m.ne; ++e) {
+    // coordinates relative to the element's first node: derivatives and the curl form are
+    // translation invariant (D 1 = 0, and the curl of const * grad X_m vanishes because the
+    // tensor-product D's commute), so this is the same definition with round-off ~eps*h
+    // instead of ~eps*|X| (R2)
+    std::vector<double> Xs((size_t)d * nn);
     const double *X[3] = {nullptr, nullptr, nullptr};
-    for (int c = 0; c < d; ++c) X[c] = &m.xyz[((size_t)e * d + c) * nn];
+    for (int c = 0; c < d; ++c) {
+      const double *Xa = &m.xyz[((size_t)e * d + c) * nn];
+      for (int p = 0; p < nn; ++p) Xs[(size_t)c * nn + p] = Xa[p] - Xa[0];
+      X[c] = &Xs[(size_t)c * nn];
+    }
     double *Ja = &m.Ja[(size_t)e * nn * d * d];
     double *J = &m.J[(size_t)e * nn];
     if (d == 2) {
@@ -365,6 +383,25 @@ static void compute_metrics(Mesh &m) {
         }
       }
     }
+  }
+  // Affine elements (R2b; SURVEY 8(a) a0 "affine-element detection"): the mapping of an
+  // affine element has constant metric terms; what varies from node to node is only the round-off
+  // of the fp64 node coordinates (~eps*|X|/h).  An element whose metric terms all agree with their
+  // node-0 values to 1e-12 (relative to max_k |Ja_k|, resp. |J|) uses the node-0 values at every node.
+  for (long e = 0; e < m.ne; ++e) {
+    double *Ja = &m.Ja[(size_t)e * nn * d * d];
+    double *J = &m.J[(size_t)e * nn];
+    double scale = 0.0, dev = 0.0;
+    for (int k = 0; k < d * d; ++k) scale = std::max(scale, std::fabs(Ja[k]));
+    for (int p = 0; p < nn; ++p) {
+      dev = std::max(dev, std::fabs(J[p] - J[0]) / std::fabs(J[0]));
+      for (int k = 0; k < d * d; ++k) dev = std::max(dev, std::fabs(Ja[p * d * d + k] - Ja[k]) / scale);
+    }
+    if (dev < 1e-12)
+      for (int p = 1; p < nn; ++p) {
+        J[p] = J[0];
+        for (int k = 0; k < d * d; ++k) Ja[p * d * d + k] = Ja[k];
+      }
   }
   // O11: characteristic element size dx_e = 2 (min_i J_i)^(1/d); dx_min = min_e
   double dxm = 1e300;
@@ -478,19 +515,23 @@ static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
     const double Jn = m.J[(size_t)e * nn + node];
     for (int v = 0; v < nvar; ++v) du[((size_t)e * nvar + v) * nn + node] -= (Fstar[v] - Fown[v]) / (Jn * wb);
   };
-  // --- conforming interfaces (O5/O6): one flux per face node with the L-side normal
+  // --- conforming interfaces (O5/O6).  Eq. 12 is a per-node update in which F* takes
+  // the element's OWN contravariant vector Ja^{l_f} as its normal argument, so each side of a face
+  // evaluates F*(U-,U+; n_ref Ja^{l_f}) with its own metric terms (R5b).  In exact arithmetic
+  // the two evaluations are equal and opposite; in floating point this keeps the bracket (F* - Ftilde)
+  // free-stream preserving on each side even where the neighbours' normals differ by round-off.
   for (size_t f = 0; f < m.iface.size() / 5; ++f) {
     const int *I = &m.iface[f * 5];
     const long eL = I[0], eR = I[2]; const int fL = I[1], fR = I[3], orient = I[4];
     for (int a = 0; a < nf; ++a) {
       const int pL = face_node(m, fL, a), pR = face_node(m, fR, orient_map(m, a, orient));
-      double Um[MAXV], Up[MAXV], nL[3], nR[3], Fs[MAXV], Fo[MAXV], mFs[MAXV];
+      double Um[MAXV], Up[MAXV], nL[3], nR[3], Fs[MAXV], Fo[MAXV];
       gather(m, u, eL, pL, Um); gather(m, u, eR, pR, Up);
       face_normal(m, eL, fL, pL, nL); face_normal(m, eR, fR, pR, nR);
       rusanov(m, Um, Up, nL, Fs);
       flux_dot(m, Um, primitives(m, Um), nL, Fo);   lift(eL, pL, Fs, Fo);
-      for (int v = 0; v < nvar; ++v) mFs[v] = -Fs[v];
-      flux_dot(m, Up, primitives(m, Up), nR, Fo);   lift(eR, pR, mFs, Fo);
+      rusanov(m, Up, Um, nR, Fs);
+      flux_dot(m, Up, primitives(m, Up), nR, Fo);   lift(eR, pR, Fs, Fo);
     }
   }
   // --- 2:1 mortars (O7), 2-D only
@@ -657,17 +698,17 @@ static void rhs_viscous_add(const Mesh &m, const double *u, double *du) {
     const long eL = I[0], eR = I[2]; const int fL = I[1], fR = I[3], orient = I[4];
     for (int a = 0; a < nf; ++a) {
       const int pL = face_node(m, fL, a), pR = face_node(m, fR, orient_map(m, a, orient));
-      double Um[MAXV], Up[MAXV], nL[3], nR[3], FmL[MAXV], FpL[MAXV], FpR[MAXV];
+      double Um[MAXV], Up[MAXV], nL[3], nR[3], FmL[MAXV], FpL[MAXV], FmR[MAXV], FpR[MAXV];
       gather(m, u, eL, pL, Um); gather(m, u, eR, pR, Up);
       face_normal(m, eL, fL, pL, nL); face_normal(m, eR, fR, pR, nR);
       const double *Sm = &S[((size_t)eL * nn + pL) * nw * d], *Sp = &S[((size_t)eR * nn + pR) * nw * d];
       viscous_flux_dot(m, Um, Sm, nL, FmL); viscous_flux_dot(m, Up, Sp, nL, FpL);
-      viscous_flux_dot(m, Up, Sp, nR, FpR);
+      viscous_flux_dot(m, Um, Sm, nR, FmR); viscous_flux_dot(m, Up, Sp, nR, FpR);
       const double JL = m.J[(size_t)eL * nn + pL], JR = m.J[(size_t)eR * nn + pR];
       for (int v = 0; v < nvar; ++v) {
-        double Fstar = 0.5 * (FmL[v] + FpL[v]);        // single-valued, L-side normal
-        du[((size_t)eL * nvar + v) * nn + pL] += (Fstar - FmL[v]) / (JL * wb);
-        du[((size_t)eR * nvar + v) * nn + pR] += (-Fstar - FpR[v]) / (JR * wb);
+        // each side with its own outward normal (R5b)
+        du[((size_t)eL * nvar + v) * nn + pL] += (0.5 * (FmL[v] + FpL[v]) - FmL[v]) / (JL * wb);
+        du[((size_t)eR * nvar + v) * nn + pR] += (0.5 * (FpR[v] + FmR[v]) - FpR[v]) / (JR * wb);
       }
     }
   }

@@ -56,51 +56,55 @@ struct marut_mesh {
 // ------------------------------------------------------------------------------------ 1-D operators
 // LGL nodes as the roots of q(x) = P_{N+1}(x) - P_{N-1}(x), q'(x) = (2N+1) P_N(x);
 // w_j = 2 / (N (N+1) P_N(x_j)^2); D_ij = P_N(x_i) / (P_N(x_j) (x_i - x_j)), D_ii = -sum_{j != i} D_ij.
-static void legendre_three(int N, double x, double &Pm1, double &P0, double &Pp1) {
+// Evaluated in extended precision and rounded once: x, w, D are the correctly rounded doubles of
+// their exact values, so the setup is reproducible to the last bit across implementations.
+template <typename T>
+static void legendre_three(int N, T x, T &Pm1, T &P0, T &Pp1) {
   // returns P_{N-1}, P_N, P_{N+1}
-  double a = 1.0, b = x;  // P_0, P_1
-  if (N == 0) { Pm1 = 0.0; P0 = 1.0; Pp1 = x; return; }
+  T a = 1, b = x;  // P_0, P_1
+  if (N == 0) { Pm1 = 0; P0 = 1; Pp1 = x; return; }
   for (int k = 1; k < N; ++k) {
-    double c = ((2 * k + 1) * x * b - k * a) / (k + 1);
+    T c = ((2 * k + 1) * x * b - k * a) / (k + 1);
     a = b; b = c;
   }
   Pm1 = a; P0 = b;
   Pp1 = ((2 * N + 1) * x * b - N * a) / (N + 1);
 }
-static void build_operators(int N, double *x, double *w, double *D) {
+static void build_operators(int N, double *x_out, double *w_out, double *D_out) {
+  typedef long double LD;
   const int n = N + 1;
-  std::vector<double> PN(n);
+  std::vector<LD> x(n), w(n), PN(n), D((size_t)n * n, 0);
+  const LD PI = 3.141592653589793238462643383279502884L;
   for (int j = 0; j < n; ++j) {
-    double xj = -std::cos(M_PI * j / N);
-    if (j == 0) xj = -1.0;
-    else if (j == N) xj = 1.0;
+    LD xj = -cosl(PI * j / N);
+    if (j == 0) xj = -1;
+    else if (j == N) xj = 1;
     else
       for (int it = 0; it < 100; ++it) {
-        double a, b, c;
-        legendre_three(N, xj, a, b, c);
-        double dx = (c - a) / ((2 * N + 1) * b);
+        LD a, b, c;
+        legendre_three<LD>(N, xj, a, b, c);
+        LD dx = (c - a) / ((2 * N + 1) * b);
         xj -= dx;
-        if (std::fabs(dx) < 1e-16) break;
+        if (fabsl(dx) < 1e-20L) break;
       }
     x[j] = xj;
   }
-  for (int j = 0; j < n / 2; ++j) {  // enforce the exact antisymmetry of the node set
-    double s = 0.5 * (x[n - 1 - j] - x[j]);
-    x[j] = -s; x[n - 1 - j] = s;
-  }
-  if (n % 2) x[n / 2] = 0.0;
+  if (n % 2) x[n / 2] = 0;
   for (int j = 0; j < n; ++j) {
-    double a, b, c;
-    legendre_three(N, x[j], a, b, c);
+    LD a, b, c;
+    legendre_three<LD>(N, x[j], a, b, c);
     PN[j] = b;
-    w[j] = 2.0 / (N * (N + 1.0) * b * b);
+    w[j] = 2 / (N * (N + 1) * b * b);
   }
   for (int i = 0; i < n; ++i) {
-    double s = 0.0;
+    LD s = 0;
     for (int j = 0; j < n; ++j)
       if (j != i) { D[i * n + j] = PN[i] / (PN[j] * (x[i] - x[j])); s += D[i * n + j]; }
     D[i * n + i] = -s;
   }
+  if (n % 2) D[(n / 2) * n + n / 2] = 0;
+  for (int j = 0; j < n; ++j) { x_out[j] = (double)x[j]; w_out[j] = (double)w[j]; }
+  for (int k = 0; k < n * n; ++k) D_out[k] = (double)D[k];
 }
 // barycentric evaluation of the Lagrange basis on nodes x at point y
 static void lagrange_row(int n, const double *x, double y, double *row) {
@@ -127,14 +131,14 @@ static bool build_mortar(int N, const double *x, double *out /*[4][n*n]*/) {
     double y = -std::cos(M_PI * (q + 0.75) / (n + 0.5));
     for (int it = 0; it < 100; ++it) {
       double a, b, c;
-      legendre_three(n, y, a, b, c);           // b = P_n(y), a = P_{n-1}(y)
+      legendre_three<double>(n, y, a, b, c);           // b = P_n(y), a = P_{n-1}(y)
       double dP = n * (y * b - a) / (y * y - 1.0);  // P_n'(y)
       double dy = b / dP;
       y -= dy;
       if (std::fabs(dy) < 1e-16) break;
     }
     double a, b, c;
-    legendre_three(n, y, a, b, c);
+    legendre_three<double>(n, y, a, b, c);
     double dP = n * (y * b - a) / (y * y - 1.0);
     g[q] = y; wg[q] = 2.0 / ((1.0 - y * y) * dP * dP);
   }

@@ -488,14 +488,20 @@ __global__ void metrics_kernel(const double *__restrict__ xyz, double *__restric
   const long e = blockIdx.x;
   const int p = threadIdx.x;
   for (int i = p; i < NP * NP; i += NN) Dsm[i] = Dg[i];
-  for (int c = 0; c < DIM; ++c) X[c * NN + p] = xyz[(e * DIM + c) * NN + p];
+  // coordinates relative to the element's first node (translation invariance of D and of the curl
+  // form; round-off ~eps*h instead of ~eps*|X|; R2)
+  for (int c = 0; c < DIM; ++c) X[c * NN + p] = xyz[(e * DIM + c) * NN + p] - xyz[(e * DIM + c) * NN];
   __syncthreads();
   int q[3] = {0, 0, 0};
   G::ijk(p, q);
-  auto deriv = [&](auto f, int l) {   // sum_m D[q_l][m] f(node with q_l -> m)
+  // Every operation below is a single correctly rounded FP64 operation in a fixed order
+  // (__dmul_rn / __dadd_rn are never contracted into FMAs): with the 1-D operators rounded from
+  // extended precision the metric terms are reproducible to the last bit, which matters because
+  // low-Mach flows amplify metric round-off by p0/(rho u^2) through the discrete GCL residual.
+  auto deriv = [&](auto f, int l) {   // sum_m D[q_l][m] f(node with q_l -> m), m ascending
     const int st = G::stride(l), base = p - q[l] * st;
     double acc = 0.0;
-    for (int m = 0; m < NP; ++m) acc += Dsm[q[l] * NP + m] * f(base + m * st);
+    for (int m = 0; m < NP; ++m) acc = __dadd_rn(acc, __dmul_rn(Dsm[q[l] * NP + m], f(base + m * st)));
     return acc;
   };
   for (int c = 0; c < DIM; ++c)
@@ -505,25 +511,25 @@ __global__ void metrics_kernel(const double *__restrict__ xyz, double *__restric
   if constexpr (DIM == 2) {
     const double x_xi = dX[0 * NN + p], x_eta = dX[1 * NN + p], y_xi = dX[2 * NN + p], y_eta = dX[3 * NN + p];
     Ja[0] = y_eta; Ja[1] = -x_eta; Ja[2] = -y_xi; Ja[3] = x_xi;
-    J = x_xi * y_eta - x_eta * y_xi;
+    J = __dsub_rn(__dmul_rn(x_xi, y_eta), __dmul_rn(x_eta, y_xi));
   } else {
     auto g = [&](int c, int l) { return dX[(c * 3 + l) * NN + p]; };
-    J = g(0, 0) * (g(1, 1) * g(2, 2) - g(1, 2) * g(2, 1)) - g(0, 1) * (g(1, 0) * g(2, 2) - g(1, 2) * g(2, 0)) +
-        g(0, 2) * (g(1, 0) * g(2, 1) - g(1, 1) * g(2, 0));
+    auto det2 = [&](double a, double b, double c, double d) { return __dsub_rn(__dmul_rn(a, b), __dmul_rn(c, d)); };
+    const double t1 = __dmul_rn(g(0, 0), det2(g(1, 1), g(2, 2), g(1, 2), g(2, 1)));
+    const double t2 = __dmul_rn(g(0, 1), det2(g(1, 0), g(2, 2), g(1, 2), g(2, 0)));
+    const double t3 = __dmul_rn(g(0, 2), det2(g(1, 0), g(2, 1), g(1, 1), g(2, 0)));
+    J = __dadd_rn(__dsub_rn(t1, t2), t3);
     // conservative curl form: (Ja^i)_c = d_k[X_l d_j X_m] - d_j[X_l d_k X_m], (i,j,k), (c,m,l) cyclic
     for (int i = 0; i < 3; ++i) {
       const int j = (i + 1) % 3, k = (i + 2) % 3;
       for (int c = 0; c < 3; ++c) {
         const int mm = (c + 1) % 3, ll = (c + 2) % 3;
-        const double A = deriv([&](int r) { return X[ll * NN + r] * dX[(mm * 3 + j) * NN + r]; }, k);
-        const double B = deriv([&](int r) { return X[ll * NN + r] * dX[(mm * 3 + k) * NN + r]; }, j);
-        Ja[i * 3 + c] = A - B;
+        const double A = deriv([&](int r) { return __dmul_rn(X[ll * NN + r], dX[(mm * 3 + j) * NN + r]); }, k);
+        const double B = deriv([&](int r) { return __dmul_rn(X[ll * NN + r], dX[(mm * 3 + k) * NN + r]); }, j);
+        Ja[i * 3 + c] = __dsub_rn(A, B);
       }
     }
   }
-  double *out = metric_full + e * MD * NN;
-  for (int k = 0; k < DIM * DIM; ++k) out[k * NN + p] = Ja[k];
-  out[DIM * DIM * NN + p] = 1.0 / J;
   // element reductions: min J and affinity measure (max relative deviation from the node-0 values)
   if (p == 0) {
     double s = 0.0;
@@ -541,9 +547,17 @@ __global__ void metrics_kernel(const double *__restrict__ xyz, double *__restric
   if (p == 0) {
     double mn = redJ[0], mx = redD[0];
     for (int r = 1; r < NN; ++r) { mn = fmin(mn, redJ[r]); mx = fmax(mx, redD[r]); }
+    // affine element (R2b): metric terms constant to 1e-12 -> node-0 values at every node
+    if (mx < 1e-12) mn = ref[DIM * DIM];
     elem_info[e * 2 + 0] = mn;
     elem_info[e * 2 + 1] = mx;
+    ref[MD] = mx;
   }
+  __syncthreads();
+  const bool affine = ref[MD] < 1e-12;
+  double *out = metric_full + e * MD * NN;
+  for (int k = 0; k < DIM * DIM; ++k) out[k * NN + p] = affine ? ref[k] : Ja[k];
+  out[DIM * DIM * NN + p] = 1.0 / (affine ? ref[DIM * DIM] : J);
 }
 
 // affine meshes: keep one metric set per element (node 0)

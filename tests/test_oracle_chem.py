@@ -164,6 +164,6 @@ def test_c5_recipe_is_well_posed():
     dt = om.max_dt(c.u0, c.cfl)
     s = om.chem_source(c.u0)[:, :5, :]
     tau = (c.u0[:, :5, :] / np.maximum(np.abs(s), 1e-300)).min()
-    assert dt <= 0.05 * tau * (32 / 4), (dt, tau)  # the 4^3 instance has 8x larger cells than the 32^3 one
+    assert dt <= 0.05 * tau, (dt, tau)
     u, t, min_rho, min_p = om.run(c.u0, c.steps, cfl=c.cfl)
     assert min_rho > 0 and min_p > 0 and np.isfinite(u).all()

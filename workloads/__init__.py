@@ -540,7 +540,7 @@ class Case:
     cfl: float = 0.5
 
 
-C5_LENGTH = 2.0e-7  # metres; chosen per DESIGN.md section 5 (explicit-chemistry step <= 0.05 x fastest depletion time)
+C5_LENGTH = 2.0e-7  # metres (domain edge of the 32^3 instance); chosen per DESIGN.md section 5 (explicit-chemistry step <= 0.05 x fastest depletion time)
 
 
 def make_case(name: str, cells=None, steps=None, order="morton") -> Case:
@@ -568,7 +568,7 @@ def make_case(name: str, cells=None, steps=None, order="morton") -> Case:
         return Case(name, m, mach10_shock(m, half_width=6.0 * m.info["h_fine"]), steps or 20)
     if name == "c5":
         k = cells or 32
-        L = C5_LENGTH
+        L = C5_LENGTH * k / 32.0  # small instances keep the element size (and so dt / tau_chem) of the 32^3 one
         m = cartesian_mesh(3, 3, (k,) * 3, (0.0,) * 3, (L,) * 3, order=order)
         m.physics, m.mech = REACTING_EULER, air5_mechanism()
         return Case(name, m, reacting_field(m, L), steps or 10)
