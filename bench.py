@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- DG RHS + SSP-RK33 throughput of the CUDA path (DOF-stage updates / s, FP64) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4w|c4|c5|c1] [--impl reference]
+
+A "step" is one pass of the whole hot path over the workload: marut_max_dt (CFL reduction) followed by the
+three fused marut_ssprk_stage launches of one SSP-RK33 step (SURVEY 8(a) rows a1..a10 as the physics has
+them).  Default workload: BASELINE.json configs[1] (c2: 3-D Euler, N=4, 32^3 periodic hexes, ~20.5M DOF),
+synthetic seeded inputs.  One JSON line is printed by rank 0.
+
+N > 1 (torchrun): the path does not shard in this build ("replicas only"): every rank
+advances its own replica of the workload, no data-path collective; value = units of all ranks / max time.
+
+--impl reference: the CPU oracle (oracle/), as it stands, on the host cores, on a bounded sample of the
+same workload.  Rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "DG RHS+SSPRK3 DOF-stage updates/s (FP64)"
+UNIT = "DOF-stage/s"
+# bounded oracle samples: (cells per direction, target seconds)
+ORACLE_SAMPLE_CELLS = {"c1": None, "c2": 12, "c3": 16, "c4": 64, "c4w": 64, "c5": 8}
+
+
+def workload_name(case):
+    m = case.mesh
+    phys = {0: "Euler", 1: "Navier-Stokes (BR1)", 2: "reacting Euler, 5 species"}[m.physics]
+    return (f"{case.name}: {m.dim}-D {phys}, N={m.N}, {m.n_elem} elements, {m.n_elem * m.nn} nodes, "
+            f"{m.n_dof} DOF, {len(m.mortar)} mortars, {len(m.bface)} boundary faces")
+
+
+def algorithmic_bytes_per_dof_stage(mesh, affine=True):
+    """SURVEY 8(d) / DESIGN.md section 7: state traffic 16 B (stage 0) + 24 B + 24 B = 64/3 B per DOF-stage;
+    curved meshes add the per-node metric terms (d*d + 1 doubles per node per stage)."""
+    b = 64.0 / 3.0
+    if not affine:
+        b += 8.0 * (mesh.dim * mesh.dim + 1) / mesh.n_var
+    return b
+
+
+# --------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.QUERY}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        try:
+            for line in open(self.path):
+                f = [x.strip() for x in line.split(",")]
+                if len(f) < 9:
+                    continue
+                try:
+                    sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+                except ValueError:
+                    continue
+                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                    if val.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            # "under load" = samples in the upper half of the power range
+            thr = 0.5 * (min(power) + max(power)) if power else 0.0
+            load = [s for s, p in zip(sm, power) if p >= thr] or sm
+            load.sort()
+            out.update(sm_mhz=load[len(load) // 2], sm_max_mhz=max(smax), reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=max(power) if power else None)
+        return out
+
+
+# --------------------------------------------------------------------------------------------- oracle arm
+def oracle_sample(workload, budget_s):
+    """time the CPU oracle (as it stands, never tuned) on a bounded sample of the workload: the same config
+    at fewer elements per direction, as many SSP-RK33 steps (dt from its own CFL reduction) as fit budget_s."""
+    import oracle
+    import workloads as wl
+
+    cells = ORACLE_SAMPLE_CELLS[workload]
+    c = wl.make_case(workload, cells=cells)
+    om = oracle.OracleMesh(c.mesh)
+    t0 = time.perf_counter()
+    u = om.run(c.u0, 1, cfl=c.cfl)[0]          # calibration step (counted)
+    t1 = time.perf_counter() - t0
+    n = max(1, min(200, int(budget_s / max(t1, 1e-6)) - 1))
+    t0 = time.perf_counter()
+    om.run(u, n, cfl=c.cfl)
+    t = time.perf_counter() - t0
+    per_step = t / n
+    return {"case": c, "steps": n, "s_per_step": per_step, "value": c.mesh.n_dof * 3 / per_step,
+            "cores": oracle.num_threads(),
+            "sample": f"{workload} at {c.mesh.n_elem} elements ({c.mesh.n_dof} DOF), {n} SSP-RK33 steps incl. CFL reduction, "
+                      f"{t:.1f} s, g++ -O2 -ffp-contract=off + OpenMP over elements"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import workloads as wl
+
+    per_step_budget = 60.0 / max(1, args.steps + args.warmup)
+    import oracle
+
+    cells = ORACLE_SAMPLE_CELLS[args.workload]
+    c = wl.make_case(args.workload, cells=cells)
+    om = oracle.OracleMesh(c.mesh)
+    # one "step" of this arm = `inner` SSP-RK33 steps of the sample, sized to per_step_budget
+    t0 = time.perf_counter()
+    u = om.run(c.u0, 1, cfl=c.cfl)[0]
+    t1 = time.perf_counter() - t0
+    inner = max(1, min(50, int(per_step_budget / max(t1, 1e-6))))
+    for _ in range(args.warmup):
+        u = om.run(u, inner, cfl=c.cfl)[0]
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        u = om.run(u, inner, cfl=c.cfl)[0]
+    t = time.perf_counter() - t0
+    value = c.mesh.n_dof * 3 * inner * args.steps / t
+    sample = (f"{args.workload} at {c.mesh.n_elem} elements ({c.mesh.n_dof} DOF); one bench step = {inner} SSP-RK33 steps "
+              f"incl. CFL reduction; g++ -O2 -ffp-contract=off + OpenMP over elements")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(c), "full_workload": args.workload, "sampled": True},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------- CUDA arm
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def run_cuda(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import paper_2605_26388_b200 as mb
+    import workloads as wl
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    case = wl.make_case(args.workload)
+    mesh = case.mesh
+    gm = mb.MarutMesh(mesh)
+    affine = gm.is_affine
+    u0_host = torch.from_numpy(np.ascontiguousarray(case.u0)).pin_memory()
+    out_host = torch.empty_like(u0_host).pin_memory()
+    u = u0_host.cuda()
+    ua, ub = torch.empty_like(u), torch.empty_like(u)
+    stream = torch.cuda.current_stream()
+    n_dof = mesh.n_dof
+    cfl = case.cfl
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step(ev=None):
+        dt = gm.max_dt(u, cfl)
+        if ev is not None:
+            for s, (un, uin, uout) in enumerate(((u, u, ua), (u, ua, ub), (u, ub, u))):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                gm.stage(s, dt, 0.0, un, uin, uout)
+                e1.record(stream)
+                ev.append((e0, e1))
+        else:
+            gm.step(u, ua, ub, dt)
+        return dt
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = gm.launch_count
+    events = []
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_start.record(stream)
+    for _ in range(args.steps):
+        step(events)
+    t_end.record(stream)
+    barrier()
+    ms = t_start.elapsed_time(t_end)
+    launches = gm.launch_count - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    if not np.isfinite(u.sum().item()):
+        raise RuntimeError("solution became non-finite during the timed region")
+    stage_ms = [a.elapsed_time(b) for a, b in events]
+    # launches of the dominant kernel inside one marut_ssprk_stage call (NS: gradient + stage; REACT: eos + stage)
+    stage_ms_avg = sum(stage_ms) / len(stage_ms)
+
+    # ---- end to end: host buffers; H2D of the state, one step, D2H of the result, every step
+    u.copy_(u0_host, non_blocking=True)
+    for _ in range(2):
+        u.copy_(u0_host, non_blocking=True); step(); out_host.copy_(u, non_blocking=True)
+    barrier()
+    e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e_start.record(stream)
+    for _ in range(args.steps):
+        u.copy_(u0_host, non_blocking=True)
+        step()
+        out_host.copy_(u, non_blocking=True)
+    e_end.record(stream)
+    barrier()
+    e2e_ms = e_start.elapsed_time(e_end)
+
+    if world > 1:
+        t = torch.tensor([ms, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_ms = t.tolist()
+    units = n_dof * 3 * args.steps * world
+    value = units / (ms * 1e-3)
+    e2e_value = units / (e2e_ms * 1e-3)
+
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        b_alg = algorithmic_bytes_per_dof_stage(mesh, affine)
+        achieved = b_alg * n_dof / (stage_ms_avg * 1e-3) / 1e9
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu capture
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get(args.workload)
+            except Exception:
+                traffic = None
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": workload_name(case), "parallelism": "replicas only" if world > 1 else "1 GPU",
+                           "l2": f"inputs larger than L2 ({3 * n_dof * 8 / 1e6:.0f} MB of state buffers vs 126 MB)"
+                                 if 3 * n_dof * 8 > 126e6 else "state fits L2 (launch/latency-bound case; no flush)",
+                           "step": "marut_max_dt + 3 x marut_ssprk_stage", "cfl": cfl, "affine": bool(affine)},
+                "clocks": clocks,
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n_dof * 8, "d2h_bytes_per_step": n_dof * 8 + 8,
+                        "ms_per_step": e2e_ms / args.steps},
+                "gpu_launches": launches,
+                "roofline": {"bound": "hbm", "kernel": "marut_ssprk_stage (fused stage kernel" +
+                             (" + BR1 gradient kernel" if mesh.physics == 1 else " + EOS kernel" if mesh.physics == 2 else "") + ")",
+                             "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                             "traffic": traffic, "peak_source": peak_src, "bytes_per_dof_stage": b_alg,
+                             "stage_ms_avg": stage_ms_avg, "frac_of_8TBs_nominal": achieved / 8000.0}}
+        if world == 1 and not args.no_cpu_baseline:
+            o = oracle_sample(args.workload, args.cpu_seconds)
+            line["cpu_baseline"] = {"value": o["value"], "unit": UNIT, "cores": o["cores"], "kind": "oracle", "sample": o["sample"]}
+        print(json.dumps(line), flush=True)
+    gm.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="c2", choices=sorted(ORACLE_SAMPLE_CELLS))
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline leg")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()
