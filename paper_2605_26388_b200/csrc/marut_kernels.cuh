@@ -569,6 +569,22 @@ __global__ void compact_metrics_kernel(const double *__restrict__ metric_full, d
   metric_el[g] = metric_full[g * G::NN];
 }
 
+// affine meshes: lengths of the scaled face normals |Ja^l| per element (used by the line kernel)
+template <int DIM>
+__global__ void fnorm_kernel(const double *__restrict__ metric_el, double *__restrict__ fnorm, long ne) {
+  const long g = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= ne * DIM) return;
+  const long e = g / DIM;
+  const int l = (int)(g - e * DIM);
+  double n2 = 0.0;
+#pragma unroll
+  for (int c = 0; c < DIM; ++c) {
+    const double x = metric_el[e * (DIM * DIM + 1) + l * DIM + c];
+    n2 += x * x;
+  }
+  fnorm[g] = sqrt(n2);
+}
+
 // ---------------------------------------------------------------- launch helpers
 template <int NN>
 constexpr int elems_per_block() { return (256 / NN) < 1 ? 1 : 256 / NN; }
