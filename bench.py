@@ -205,17 +205,25 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    # The configs are short runs (BASELINE.json: 10-20 steps; c4/c5 leave their well-posed window after
+    # ~100-190 steps without the paper's limiter / implicit chemistry), so the bench
+    # repeats the config: every `case.steps` steps the next step starts again from the pristine u0 (its
+    # stages read u0 directly, so the restart costs no extra copy and no extra traffic).
+    u0_dev = u.clone()
+    counter = [0]
+
     def step(ev=None):
-        dt = gm.max_dt(u, cfl)
-        if ev is not None:
-            for s, (un, uin, uout) in enumerate(((u, u, ua), (u, ua, ub), (u, ub, u))):
+        src = u0_dev if counter[0] % case.steps == 0 else u
+        counter[0] += 1
+        dt = gm.max_dt(src, cfl)
+        for s, (un, uin, uout) in enumerate(((src, src, ua), (src, ua, ub), (src, ub, u))):
+            if ev is not None:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
-                gm.stage(s, dt, 0.0, un, uin, uout)
+            gm.stage(s, dt, 0.0, un, uin, uout)
+            if ev is not None:
                 e1.record(stream)
                 ev.append((e0, e1))
-        else:
-            gm.step(u, ua, ub, dt)
         return dt
 
     # ---- device-resident throughput: W warm-up steps, then exactly K timed steps
@@ -242,16 +250,19 @@ def run_cuda(args):
     # launches of the dominant kernel inside one marut_ssprk_stage call (NS: gradient + stage; REACT: eos + stage)
     stage_ms_avg = sum(stage_ms) / len(stage_ms)
 
+    def e2e_step():
+        gm.step(u, ua, ub, gm.max_dt(u, cfl))
+
     # ---- end to end: host buffers; H2D of the state, one step, D2H of the result, every step
     u.copy_(u0_host, non_blocking=True)
     for _ in range(2):
-        u.copy_(u0_host, non_blocking=True); step(); out_host.copy_(u, non_blocking=True)
+        u.copy_(u0_host, non_blocking=True); e2e_step(); out_host.copy_(u, non_blocking=True)
     barrier()
     e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e_start.record(stream)
     for _ in range(args.steps):
         u.copy_(u0_host, non_blocking=True)
-        step()
+        e2e_step()
         out_host.copy_(u, non_blocking=True)
     e_end.record(stream)
     barrier()
@@ -282,7 +293,7 @@ def run_cuda(args):
                 "config": {"workload": workload_name(case), "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": f"inputs larger than L2 ({3 * n_dof * 8 / 1e6:.0f} MB of state buffers vs 126 MB)"
                                  if 3 * n_dof * 8 > 126e6 else "state fits L2 (launch/latency-bound case; no flush)",
-                           "step": "marut_max_dt + 3 x marut_ssprk_stage", "cfl": cfl, "affine": bool(affine)},
+                           "step": "marut_max_dt + 3 x marut_ssprk_stage", "cfl": cfl, "restart_from_u0_every_steps": case.steps, "affine": bool(affine)},
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n_dof * 8, "d2h_bytes_per_step": n_dof * 8 + 8,
                         "ms_per_step": e2e_ms / args.steps},
