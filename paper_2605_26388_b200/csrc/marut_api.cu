@@ -43,7 +43,7 @@ struct marut_mesh {
   // device
   double *d_metric = nullptr;
   double *d_fnorm = nullptr;   // affine: [e][dim] |Ja^l|
-  bool use_line = true;        // fast line kernel (marut_line.cuh) unless MARUT_GENERIC=1
+  int kernel_sel = 0;          // Euler stage kernel: 0 node (marut_node.cuh), 1 line (marut_line.cuh), 2 generic; env MARUT_KERNEL
   int2 *d_conn = nullptr;
   int *d_mortar_fine = nullptr;
   double *d_mortar_mat = nullptr;
@@ -402,8 +402,8 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   if (m->physics == MARUT_NAVIER_STOKES) CUDA_TRY(cudaMalloc(&m->d_S, (size_t)ne * (dim + 2) * dim * nn * sizeof(double)));
   if (m->physics == MARUT_REACTING_EULER) CUDA_TRY(cudaMalloc(&m->d_T, (size_t)ne * nn * sizeof(double)));
 
-  const char *gen = getenv("MARUT_GENERIC");
-  m->use_line = !(gen && gen[0] == '1');
+  const char *sel = getenv("MARUT_KERNEL");   // A/B switch for profiling: node (default) | line | generic
+  m->kernel_sel = (sel && !strcmp(sel, "line")) ? 1 : ((sel && !strcmp(sel, "generic")) ? 2 : 0);
   return MARUT_OK;
 }
 
@@ -464,7 +464,8 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   switch (m->physics) {
     case MARUT_EULER:
       e = cudaErrorNotSupported;
-      if (m->use_line) e = (m->dim == 2) ? launch_stage_line2d(m->np, m->affine, P, st) : launch_stage_line3d(m->np, m->affine, P, st);
+      if (m->kernel_sel == 0) e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
+      if (m->kernel_sel == 1) e = (m->dim == 2) ? launch_stage_line2d(m->np, m->affine, P, st) : launch_stage_line3d(m->np, m->affine, P, st);
       if (e == cudaErrorNotSupported)
         e = (m->dim == 2) ? launch_stage_euler2d(m->np, m->affine, P, st) : launch_stage_euler3d(m->np, m->affine, P, st);
       break;

@@ -1,0 +1,519 @@
+// marut_node.cuh -- the fused stage kernel of the CUDA path, any dim / degree /
+// physics: one thread per LGL node, EB elements per CTA, small register and shared-memory footprint so that
+// 20-30 warps are resident per SM (the stage is latency-bound otherwise; profiles/r01_c2_stage_line_kernel.md).
+//
+//   phase N  per node: U from global (coalesced), primitives, contravariant fluxes (eq. 9) -> shared flux
+//            planes; U and (1/rho, p, a) stashed in shared memory for the face phase
+//   phase V  per node: volume term sum_l D_l Ftilde^l from the flux planes (broadcast line reads)
+//   phase S  per FACE node, densely mapped (task g = tid, tid + NT, ...: every lane of a warp has a face
+//            node): neighbour trace gathered from global (issued before phase V, consumed after), Rusanov /
+//            mortar / boundary flux (a2-a4), lift (F* - Ftilde.n)/w_b -> shared lift buffer
+//   phase D  per node: lifts of the faces the node lies on, 1/J, source, SSP-RK combination (eq. 12, 45),
+//            u_n read and u_out written straight from / to global (coalesced): one pass over u per stage
+//
+// Product code; shares nothing with oracle/.
+#pragma once
+#include "marut_kernels.cuh"
+
+namespace marut {
+
+// shared-memory layout of one variable plane of one element: node (i,j,k) at i + NP*j + KS*k, planes PS apart.
+// KS / PS / the lane order of the plane tasks are chosen so that the node threads (consecutive nodes), the
+// (v,k)-plane tasks (offset k*KS) and the (v,i)-plane tasks (offset i) all hit 16 distinct 8-byte banks per
+// half-warp (brute-force search over the strides).
+template <int DIM, int NP, int EB>
+struct NodeLayout {
+  static constexpr int KS = NP * NP;
+  static constexpr int PS = (DIM == 2) ? (NP * NP + 1) : ((NP * KS) | 1);
+  static constexpr bool K_FASTEST = true;
+};
+template <int EB>
+struct NodeLayout<3, 5, EB> {
+  static constexpr int KS = 25, PS = 133;
+  static constexpr bool K_FASTEST = false;
+};
+template <int EB>
+struct NodeLayout<3, 4, EB> {
+  static constexpr int KS = 17, PS = (EB == 1) ? 68 : 70;
+  static constexpr bool K_FASTEST = true;
+};
+
+template <int DIM, int NP, int NSP, int EB>
+struct NodeCfg {
+  using G = Geo<DIM, NP>;
+  using L = NodeLayout<DIM, NP, EB>;
+  static constexpr int NVAR = NSP + DIM + 1;
+  static constexpr int NN = G::NN, NF = G::NF;
+  static constexpr int TILE = EB * NN;
+  static constexpr int NFN = 2 * DIM * NF;          // face nodes per element
+  static constexpr int NTASK = EB * NFN;            // face tasks per CTA
+  static constexpr int NT = ((TILE + 31) / 32) * 32;
+  static constexpr int NW = NT / 32;
+  static constexpr int NST = NVAR + 3;              // stash planes: U, 1/rho, p, a
+  static constexpr int KS = L::KS, PS = L::PS;
+  static constexpr int NPL = DIM * NVAR * EB;       // flux planes
+  static constexpr int NVT = EB * NVAR * NP;        // plane tasks per derivative pass (3-D)
+  static constexpr int MDP = ((G::MD + DIM + 1) / 2) * 2;   // per-element affine metric slot (Ja, 1/J, |Ja^l|)
+  static constexpr size_t smem_doubles(bool affine) {
+    return (size_t)NPL * PS + (size_t)NST * TILE + (size_t)NVAR * NTASK + (affine ? EB * MDP : 0);
+  }
+};
+
+// 2-D mortar faces (R7): numerical flux F* (outward, own normal) at face node a0 of
+// face f of element e.  Fine side: coarse trace interpolated to this half of the coarse face; coarse side:
+// Riemann problem on both mortars with the fine-side normal, projected back with the area factor 2.
+// Rare path, kept out of line.
+template <int NP>
+__device__ __noinline__ void node_mortar_flux_2d(const StageParams &P, long e, int f, int a0, int2 cn, const double *U,
+                                                 const double *nv, double *Fs) {
+  using G = Geo<2, NP>;
+  constexpr int NVAR = 4, NN = NP * NP;
+  const int kind = cn.y & 3, fR = (cn.y >> 2) & 7, sub = (cn.y >> 8) & 1;
+  const double *Pf = P.mortar_mat, *Prv = P.mortar_mat + 2 * NP * NP;
+  const Prim<2> pr = prim_ideal<2, true>(U, P.gamma);
+  if (kind == FK_MORTAR_FINE) {
+    double Up[NVAR] = {0.0, 0.0, 0.0, 0.0};
+    for (int j = 0; j < NP; ++j) {
+      const double w = __ldg(&Pf[(sub * NP + a0) * NP + j]);
+      const double *uc = P.u_in + (long)cn.x * NVAR * NN + G::face_node(fR, j, 0);
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Up[v] += w * __ldg(uc + v * NN);
+    }
+    const Prim<2> qp = prim_ideal<2, true>(Up, P.gamma);
+    double Fm[NVAR];
+    flux_dot<2, 1>(U, pr, nv, Fm);
+    rusanov<2, 1>(U, pr, Fm, Up, qp, nv, Fs);
+  } else {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Fs[v] = 0.0;
+    for (int m = 0; m < 2; ++m) {
+      const long eF = __ldg(&P.mortar_fine[cn.x * 2 + m]);
+      const int lF = fR >> 1;
+      const double sF = (fR & 1) ? 1.0 : -1.0;
+      for (int a = 0; a < NP; ++a) {
+        const int pF = G::face_node(fR, a, 0);
+        double UF[NVAR], UC[NVAR], nF[2], FmF[NVAR], Fm_[NVAR];
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) {
+          UF[v] = __ldg(P.u_in + (eF * NVAR + v) * NN + pF);
+          UC[v] = 0.0;
+        }
+        for (int j = 0; j < NP; ++j) {
+          const double w = __ldg(&Pf[(m * NP + a) * NP + j]);
+          const double *uc = P.u_in + e * NVAR * NN + G::face_node(f, j, 0);
+#pragma unroll
+          for (int v = 0; v < NVAR; ++v) UC[v] += w * __ldg(uc + v * NN);
+        }
+        const bool aff = P.affine_flag != 0;
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+          nF[c] = sF * (aff ? __ldg(&P.metric[eF * 5 + lF * 2 + c]) : __ldg(&P.metric[(eF * 5 + lF * 2 + c) * NN + pF]));
+        const Prim<2> qF = prim_ideal<2, true>(UF, P.gamma);
+        const Prim<2> qC = prim_ideal<2, true>(UC, P.gamma);
+        flux_dot<2, 1>(UF, qF, nF, FmF);
+        rusanov<2, 1>(UF, qF, FmF, UC, qC, nF, Fm_);
+        const double w2 = -2.0 * __ldg(&Prv[(m * NP + a0) * NP + a]);
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Fs[v] += w2 * Fm_[v];
+      }
+    }
+  }
+}
+
+
+// decoded face task (no dynamically indexed local arrays: they would go to local memory)
+struct FaceTask {
+  int el, f, a0, a1, p;   // element in tile, face, face-node coordinates, volume node
+};
+template <int DIM, int NP>
+__device__ __forceinline__ int face_node_of(int f, int a0, int a1) {
+  const int l = f >> 1, s = (f & 1) ? NP - 1 : 0;
+  if (DIM == 2) return (l == 0) ? s + NP * a0 : a0 + NP * s;
+  return (l == 0) ? s + NP * (a0 + NP * a1) : ((l == 1) ? a0 + NP * (s + NP * a1) : a0 + NP * (a1 + NP * s));
+}
+template <int DIM, int NP>
+__device__ __forceinline__ FaceTask decode_task(int g) {
+  constexpr int NF = Geo<DIM, NP>::NF, NFN = 2 * DIM * NF;
+  FaceTask t;
+  t.el = g / NFN;
+  const int r = g - t.el * NFN;
+  t.f = r / NF;
+  const int a = r - t.f * NF;
+  t.a1 = (DIM == 3) ? a / NP : 0;
+  t.a0 = a - t.a1 * NP;
+  t.p = face_node_of<DIM, NP>(t.f, t.a0, t.a1);
+  return t;
+}
+
+// exterior state of a conforming / boundary face node (mortar faces: nothing to gather here)
+template <int DIM, int NP, int NVAR>
+__device__ __forceinline__ void gather_exterior(const StageParams &P, const FaceTask &t, int2 cn, double *Up) {
+  constexpr int NN = Geo<DIM, NP>::NN;
+  const int kind = cn.y & 3;
+  if (kind == FK_CONFORMING) {
+    const int fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7;
+    const int b0 = (DIM == 2 && orient) ? NP - 1 - t.a0 : t.a0;
+    const double *un = P.u_in + (long)cn.x * NVAR * NN + face_node_of<DIM, NP>(fR, b0, t.a1);
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
+  } else if (kind == FK_BOUNDARY) {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(&P.bc_state[cn.x * NVAR + v]);
+  } else {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Up[v] = 1.0;
+  }
+}
+
+// lift (F* - Ftilde.n)/w_b of one face node (Euler), written to the lift buffer.  Up = exterior state of a
+// conforming / boundary face (ignored for mortar faces).
+template <int DIM, int NP, bool AFFINE, int EB>
+__device__ __forceinline__ void euler_face_task(const StageParams &P, const double *Ust, const double *Msm, double *Lft,
+                                                long e0, int g, const FaceTask &t, int2 cn, const double *Up) {
+  using C = NodeCfg<DIM, NP, 1, EB>;
+  constexpr int NVAR = C::NVAR, NN = C::NN, TILE = C::TILE, NTASK = C::NTASK, MD = Geo<DIM, NP>::MD, MDP = C::MDP;
+  const int l = t.f >> 1;
+  const double sgn = (t.f & 1) ? 1.0 : -1.0;
+  const int idx = t.el * NN + t.p;
+  const long e = e0 + t.el;
+  double Um[NVAR], nv[DIM], nrm;
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) Um[v] = Ust[v * TILE + idx];
+  const double irhom = Ust[NVAR * TILE + idx], pm = Ust[(NVAR + 1) * TILE + idx], am = Ust[(NVAR + 2) * TILE + idx];
+  if constexpr (AFFINE) {
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) nv[c] = sgn * Msm[t.el * MDP + l * DIM + c];
+    nrm = Msm[t.el * MDP + MD + l];
+  } else {
+    double n2 = 0.0;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) {
+      nv[c] = sgn * __ldg(&P.metric[(e * MD + l * DIM + c) * NN + t.p]);
+      n2 += nv[c] * nv[c];
+    }
+    nrm = sqrt(n2);
+  }
+  // own normal flux F(U-).nv, recomputed from the stash (cheaper than five more shared loads)
+  double mnm = 0.0;
+#pragma unroll
+  for (int c = 0; c < DIM; ++c) mnm += Um[1 + c] * nv[c];
+  const double vnm = mnm * irhom;
+  double Fm[NVAR], lift[NVAR];
+  Fm[0] = mnm;
+#pragma unroll
+  for (int c = 0; c < DIM; ++c) Fm[1 + c] = Um[1 + c] * vnm + pm * nv[c];
+  Fm[DIM + 1] = (Um[DIM + 1] + pm) * vnm;
+  const int kind = cn.y & 3;
+  if (kind == FK_CONFORMING || kind == FK_BOUNDARY) {
+    // Rusanov with a scaled normal, division-free apart from 1/rho+ (R5):
+    //   lambda |nv| = max(|v-.nv| + a- |nv|, |v+.nv| + a+ |nv|);  lift = (F* - F-.nv)/w_b
+    const double irhop = 1.0 / Up[0];
+    double mnp = 0.0, kep = 0.0;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) {
+      mnp += Up[1 + c] * nv[c];
+      kep += Up[1 + c] * Up[1 + c];
+    }
+    const double pp = (P.gamma - 1.0) * (Up[DIM + 1] - 0.5 * kep * irhop);
+    const double ap = sqrt(P.gamma * pp * irhop);
+    const double vnp = mnp * irhop;
+    const double hl = 0.5 * fmax(fabs(vnm) + am * nrm, fabs(vnp) + ap * nrm);
+    double Fp[NVAR];
+    Fp[0] = mnp;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) Fp[1 + c] = Up[1 + c] * vnp + pp * nv[c];
+    Fp[DIM + 1] = (Up[DIM + 1] + pp) * vnp;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) lift[v] = P.inv_wb * (0.5 * (Fp[v] - Fm[v]) - hl * (Up[v] - Um[v]));
+  } else {
+    if constexpr (DIM == 2) {
+      double Fs[NVAR];
+      node_mortar_flux_2d<NP>(P, e, t.f, t.a0, cn, Um, nv, Fs);
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) lift[v] = P.inv_wb * (Fs[v] - Fm[v]);
+    } else {
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) lift[v] = 0.0;
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) Lft[v * NTASK + g] = lift[v];
+}
+
+// ---------------------------------------------------------------- derivative passes (plane tasks)
+// 3-D pass 1: task (element, variable v, zeta-plane k): R = D_xi Ftilde^xi + D_eta Ftilde^eta on the plane, in
+// registers with D as compile-time-indexed constant-bank operands; result in place of Ftilde^xi.
+template <int NP, int NVAR, int EB, int KS, int PS, bool K_FASTEST>
+__device__ __forceinline__ void plane_pass_xi_eta(const StageParams &P, double *Fsm, int t) {
+  const int el = t / (NP * NVAR), r = t - el * (NP * NVAR);
+  const int v = K_FASTEST ? r / NP : r % NVAR, k = K_FASTEST ? r % NP : r / NVAR;
+  double *px = Fsm + (v * EB + el) * PS + k * KS;
+  const double *pe = px + NVAR * EB * PS;
+  double R[NP][NP];
+#pragma unroll
+  for (int j = 0; j < NP; ++j) {
+    double f[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) f[m] = px[j * NP + m];
+#pragma unroll
+    for (int i = 0; i < NP; ++i) {
+      double acc = P.D[i * NP] * f[0];
+#pragma unroll
+      for (int m = 1; m < NP; ++m) acc += P.D[i * NP + m] * f[m];
+      R[j][i] = acc;
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < NP; ++i) {
+    double f[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) f[m] = pe[m * NP + i];
+#pragma unroll
+    for (int j = 0; j < NP; ++j) {
+      double acc = R[j][i];
+#pragma unroll
+      for (int m = 0; m < NP; ++m) acc += P.D[j * NP + m] * f[m];
+      R[j][i] = acc;
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < NP; ++j)
+#pragma unroll
+    for (int i = 0; i < NP; ++i) px[j * NP + i] = R[j][i];
+}
+// 3-D pass 2: task (element, variable v, xi-index i): R += D_zeta Ftilde^zeta on the (eta,zeta)-plane
+template <int NP, int NVAR, int EB, int KS, int PS>
+__device__ __forceinline__ void plane_pass_zeta(const StageParams &P, double *Fsm, int t) {
+  const int el = t / (NP * NVAR), r = t - el * (NP * NVAR);
+  const int v = r / NP, i = r - v * NP;
+  double *pr = Fsm + (v * EB + el) * PS + i;
+  const double *pz = pr + 2 * NVAR * EB * PS;
+  double R[NP][NP];
+#pragma unroll
+  for (int k = 0; k < NP; ++k)
+#pragma unroll
+    for (int j = 0; j < NP; ++j) R[k][j] = pr[k * KS + j * NP];
+#pragma unroll
+  for (int j = 0; j < NP; ++j) {
+    double f[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) f[m] = pz[m * KS + j * NP];
+#pragma unroll
+    for (int k = 0; k < NP; ++k) {
+      double acc = R[k][j];
+#pragma unroll
+      for (int m = 0; m < NP; ++m) acc += P.D[k * NP + m] * f[m];
+      R[k][j] = acc;
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < NP; ++k)
+#pragma unroll
+    for (int j = 0; j < NP; ++j) pr[k * KS + j * NP] = R[k][j];
+}
+// 2-D: task (variable v, element): both directions on the element plane
+template <int NP, int NVAR, int EB, int PS>
+__device__ __forceinline__ void plane_pass_2d(const StageParams &P, double *Fsm, int t) {
+  const int v = t / EB, el = t - v * EB;
+  double *px = Fsm + (v * EB + el) * PS;
+  const double *pe = px + NVAR * EB * PS;
+  double R[NP][NP];
+#pragma unroll
+  for (int j = 0; j < NP; ++j) {
+    double f[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) f[m] = px[j * NP + m];
+#pragma unroll
+    for (int i = 0; i < NP; ++i) {
+      double acc = P.D[i * NP] * f[0];
+#pragma unroll
+      for (int m = 1; m < NP; ++m) acc += P.D[i * NP + m] * f[m];
+      R[j][i] = acc;
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < NP; ++i) {
+    double f[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) f[m] = pe[m * NP + i];
+#pragma unroll
+    for (int j = 0; j < NP; ++j) {
+      double acc = R[j][i];
+#pragma unroll
+      for (int m = 0; m < NP; ++m) acc += P.D[j * NP + m] * f[m];
+      R[j][i] = acc;
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < NP; ++j)
+#pragma unroll
+    for (int i = 0; i < NP; ++i) px[j * NP + i] = R[j][i];
+}
+
+#ifndef MARUT_NODE_MINB128
+#define MARUT_NODE_MINB128 5
+#endif
+
+template <int DIM, int NP, bool AFFINE, int EB, int MINB>
+__global__ void __launch_bounds__((NodeCfg<DIM, NP, 1, EB>::NT), MINB)
+stage_node_kernel(const __grid_constant__ StageParams P) {
+  using C = NodeCfg<DIM, NP, 1, EB>;
+  using G = Geo<DIM, NP>;
+  constexpr int NVAR = C::NVAR, NN = C::NN, NF = C::NF, TILE = C::TILE, NFN = C::NFN, NTASK = C::NTASK, NT = C::NT;
+  constexpr int MD = G::MD, MDP = C::MDP, KS = C::KS, PS = C::PS, NW = C::NW;
+  constexpr int NVT = (DIM == 3) ? C::NVT : EB * NVAR;   // plane tasks per pass
+  constexpr int NVW = (NVT + 31) / 32;                   // warps a derivative pass occupies
+  extern __shared__ __align__(16) double smem[];
+  double *Fsm = smem;                       // [DIM][NVAR][EB] planes of PS doubles: contravariant fluxes
+  double *Ust = Fsm + C::NPL * PS;          // [NVAR + 3][TILE]  U, 1/rho, p, a
+  double *Lft = Ust + C::NST * TILE;        // [NVAR][NTASK]     lifts of the face nodes
+  double *Msm = Lft + NVAR * NTASK;         // affine: [EB][MDP] Ja, 1/J, |Ja^l|
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const long e0 = (long)blockIdx.x * EB;
+  const int nel = (int)((P.ne - e0 < EB) ? (P.ne - e0) : EB);
+  const int ntask = nel * NFN;
+  // the derivative passes occupy NVW warps; rotate them over the CTA's warps (and so over the SM's four
+  // schedulers) with the block index, and hand the face tasks to the other warps first
+  const int rot = (int)(blockIdx.x % NW);
+  const int vrank = (warp - rot + NW) % NW;                  // rank in the derivative passes
+  const int srank = (warp - rot - NVW + 2 * NW) % NW;        // rank in the face phase
+  const int vt0 = vrank * 32 + lane, g0 = srank * 32 + lane;
+
+  // first face task of this thread: connectivity load issued first (the neighbour gather depends on it)
+  const bool has0 = g0 < ntask;
+  const FaceTask t0 = decode_task<DIM, NP>(has0 ? g0 : 0);
+  int2 cn0 = make_int2(0, FK_BOUNDARY);
+  if (has0) cn0 = __ldg(&P.conn[(e0 + t0.el) * 2 * DIM + t0.f]);
+
+  if constexpr (AFFINE) {
+    for (int i = tid; i < nel * MDP; i += NT) {
+      const int el = i / MDP, k = i - el * MDP;
+      Msm[i] = (k < MD) ? __ldg(&P.metric[(e0 + el) * MD + k]) : ((k < MD + DIM) ? __ldg(&P.fnorm[(e0 + el) * DIM + (k - MD)]) : 0.0);
+    }
+  }
+
+  // ---- phase N: own node
+  const int el = tid / NN, p = tid - el * NN;
+  const long e = e0 + el;
+  const bool active = (tid < TILE) && (el < nel);
+  const int qi = p % NP, qj = (p / NP) % NP, qk = (DIM == 3) ? p / (NP * NP) : 0;
+  const int sp = p + (KS - NP * NP) * qk;   // node offset inside a flux plane
+  double U[NVAR], invJ = 0.0;
+  if (active) {
+    const double *up = P.u_in + e * NVAR * NN + p;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
+  }
+  // neighbour trace of the first face task: in flight during phase N and the first derivative pass
+  double Up0[NVAR];
+  if (has0) gather_exterior<DIM, NP, NVAR>(P, t0, cn0, Up0);
+  if (active) {
+    double Ja[DIM * DIM];
+#pragma unroll
+    for (int k = 0; k < DIM * DIM; ++k) Ja[k] = metric_at<DIM, NP, AFFINE>(P.metric, e, k, p);
+    invJ = metric_at<DIM, NP, AFFINE>(P.metric, e, DIM * DIM, p);
+    const Prim<DIM> pr = prim_ideal<DIM, true>(U, P.gamma);
+#pragma unroll
+    for (int l = 0; l < DIM; ++l) {
+      double F[NVAR];
+      flux_dot<DIM, 1>(U, pr, &Ja[l * DIM], F);
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Fsm[((l * NVAR + v) * EB + el) * PS + sp] = F[v];
+    }
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Ust[v * TILE + tid] = U[v];
+    Ust[NVAR * TILE + tid] = pr.irho;
+    Ust[(NVAR + 1) * TILE + tid] = pr.p;
+    Ust[(NVAR + 2) * TILE + tid] = pr.a;
+  }
+  __syncthreads();
+
+  // ---- phase V, pass 1 (eq. 9): xi and eta derivatives per (variable, zeta-plane) task
+  if constexpr (DIM == 3) {
+    for (int t = vt0; t < nel * NVAR * NP; t += NT) plane_pass_xi_eta<NP, NVAR, EB, KS, PS, C::L::K_FASTEST>(P, Fsm, t);
+  } else {
+    for (int t = vt0; t < NVT; t += NT)
+      if (t % EB < nel) plane_pass_2d<NP, NVAR, EB, PS>(P, Fsm, t);
+  }
+
+  // ---- phase S: face nodes, densely mapped
+  if (has0) euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, g0, t0, cn0, Up0);
+  for (int g = g0 + NT; g < ntask; g += NT) {
+    const FaceTask t = decode_task<DIM, NP>(g);
+    const int2 cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
+    double Up[NVAR];
+    gather_exterior<DIM, NP, NVAR>(P, t, cn, Up);
+    euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, g, t, cn, Up);
+  }
+  // u_n for the final combination: issued here, consumed after the last barrier
+  double Un[NVAR];
+  const bool use_un = (P.ca != 0.0);
+  if (active && use_un) {
+    const double *np_ = P.u_n + e * NVAR * NN + p;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Un[v] = np_[v * NN];
+  }
+  if constexpr (DIM == 3) {
+    __syncthreads();
+    // ---- phase V, pass 2: zeta derivative per (variable, xi-index) task
+    for (int t = vt0; t < nel * NVAR * NP; t += NT) plane_pass_zeta<NP, NVAR, EB, KS, PS>(P, Fsm, t);
+  }
+  __syncthreads();
+  if (!active) return;
+
+  // ---- phase D: volume term + lifts of the own faces, 1/J, SSP-RK combination (eq. 12, 45)
+  double R[NVAR];
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) R[v] = Fsm[(v * EB + el) * PS + sp];
+  {
+    const int gb = el * NFN;
+    if (qi == 0 || qi == NP - 1) {
+      const int g = gb + ((qi == 0) ? 0 : 1) * NF + qj + NP * qk;
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) R[v] += Lft[v * NTASK + g];
+    }
+    if (qj == 0 || qj == NP - 1) {
+      const int g = gb + (2 + ((qj == 0) ? 0 : 1)) * NF + qi + NP * qk;
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) R[v] += Lft[v * NTASK + g];
+    }
+    if (DIM == 3 && (qk == 0 || qk == NP - 1)) {
+      const int g = gb + (4 + ((qk == 0) ? 0 : 1)) * NF + qi + NP * qj;
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) R[v] += Lft[v * NTASK + g];
+    }
+  }
+  double *op = P.u_out + e * NVAR * NN + p;
+  if (use_un) {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.ca * Un[v] + (P.cb * U[v] + P.cc * (0.0 - invJ * R[v]));
+  } else {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.cb * U[v] + P.cc * (0.0 - invJ * R[v]);
+  }
+}
+
+// elements per CTA: ~128 threads
+template <int NN>
+constexpr int node_eb() { return (NN >= 96) ? 1 : 128 / NN; }
+
+template <int DIM, int NP, bool AFFINE>
+cudaError_t launch_stage_node_t(const StageParams &P, cudaStream_t st) {
+  constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
+  using C = NodeCfg<DIM, NP, 1, EB>;
+  constexpr size_t smem = C::smem_doubles(AFFINE) * sizeof(double);
+  constexpr int MINB = (C::NT <= 128) ? MARUT_NODE_MINB128 : ((C::NT <= 256) ? 2 : 1);
+  auto k = stage_node_kernel<DIM, NP, AFFINE, EB, MINB>;
+  static bool attr = false;
+  if (!attr) {
+    cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    attr = true;
+  }
+  const long grid = (P.ne + EB - 1) / EB;
+  k<<<(unsigned)grid, C::NT, smem, st>>>(P);
+  return cudaGetLastError();
+}
+
+}  // namespace marut
