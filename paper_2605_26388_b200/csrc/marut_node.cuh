@@ -240,118 +240,23 @@ __device__ __forceinline__ void euler_face_task(const StageParams &P, const doub
   for (int v = 0; v < NVAR; ++v) Lft[v * NTASK + g] = lift[v];
 }
 
-// ---------------------------------------------------------------- derivative passes (plane tasks)
-// 3-D pass 1: task (element, variable v, zeta-plane k): R = D_xi Ftilde^xi + D_eta Ftilde^eta on the plane, in
-// registers with D as compile-time-indexed constant-bank operands; result in place of Ftilde^xi.
-template <int NP, int NVAR, int EB, int KS, int PS, bool K_FASTEST>
-__device__ __forceinline__ void plane_pass_xi_eta(const StageParams &P, double *Fsm, int t) {
-  const int el = t / (NP * NVAR), r = t - el * (NP * NVAR);
-  const int v = K_FASTEST ? r / NP : r % NVAR, k = K_FASTEST ? r % NP : r / NVAR;
-  double *px = Fsm + (v * EB + el) * PS + k * KS;
-  const double *pe = px + NVAR * EB * PS;
-  double R[NP][NP];
-#pragma unroll
-  for (int j = 0; j < NP; ++j) {
-    double f[NP];
-#pragma unroll
-    for (int m = 0; m < NP; ++m) f[m] = px[j * NP + m];
-#pragma unroll
-    for (int i = 0; i < NP; ++i) {
-      double acc = P.D[i * NP] * f[0];
-#pragma unroll
-      for (int m = 1; m < NP; ++m) acc += P.D[i * NP + m] * f[m];
-      R[j][i] = acc;
-    }
-  }
+// ---------------------------------------------------------------- derivative passes (line tasks)
+// One task = one line of NP nodes of one variable: NP shared loads feed NP*NP FMAs whose D operands are
+// compile-time-indexed constant-bank values.  Tasks per pass = NVAR * NP^(DIM-1) per element (= the node count
+// for Euler at NP = 5): every warp of the CTA takes part with all lanes, so the passes are balanced.
+// The xi pass overwrites Ftilde^xi with D_xi Ftilde^xi; the eta pass adds D_eta Ftilde^eta to it; the last
+// pass (zeta in 3-D, eta in 2-D) keeps its NP results in registers and finishes those NP degrees of freedom.
+template <int NP>
+__device__ __forceinline__ void line_deriv(const StageParams &P, const double *f, double *acc) {
 #pragma unroll
   for (int i = 0; i < NP; ++i) {
-    double f[NP];
 #pragma unroll
-    for (int m = 0; m < NP; ++m) f[m] = pe[m * NP + i];
-#pragma unroll
-    for (int j = 0; j < NP; ++j) {
-      double acc = R[j][i];
-#pragma unroll
-      for (int m = 0; m < NP; ++m) acc += P.D[j * NP + m] * f[m];
-      R[j][i] = acc;
-    }
+    for (int m = 0; m < NP; ++m) acc[i] += P.D[i * NP + m] * f[m];
   }
-#pragma unroll
-  for (int j = 0; j < NP; ++j)
-#pragma unroll
-    for (int i = 0; i < NP; ++i) px[j * NP + i] = R[j][i];
-}
-// 3-D pass 2: task (element, variable v, xi-index i): R += D_zeta Ftilde^zeta on the (eta,zeta)-plane
-template <int NP, int NVAR, int EB, int KS, int PS>
-__device__ __forceinline__ void plane_pass_zeta(const StageParams &P, double *Fsm, int t) {
-  const int el = t / (NP * NVAR), r = t - el * (NP * NVAR);
-  const int v = r / NP, i = r - v * NP;
-  double *pr = Fsm + (v * EB + el) * PS + i;
-  const double *pz = pr + 2 * NVAR * EB * PS;
-  double R[NP][NP];
-#pragma unroll
-  for (int k = 0; k < NP; ++k)
-#pragma unroll
-    for (int j = 0; j < NP; ++j) R[k][j] = pr[k * KS + j * NP];
-#pragma unroll
-  for (int j = 0; j < NP; ++j) {
-    double f[NP];
-#pragma unroll
-    for (int m = 0; m < NP; ++m) f[m] = pz[m * KS + j * NP];
-#pragma unroll
-    for (int k = 0; k < NP; ++k) {
-      double acc = R[k][j];
-#pragma unroll
-      for (int m = 0; m < NP; ++m) acc += P.D[k * NP + m] * f[m];
-      R[k][j] = acc;
-    }
-  }
-#pragma unroll
-  for (int k = 0; k < NP; ++k)
-#pragma unroll
-    for (int j = 0; j < NP; ++j) pr[k * KS + j * NP] = R[k][j];
-}
-// 2-D: task (variable v, element): both directions on the element plane
-template <int NP, int NVAR, int EB, int PS>
-__device__ __forceinline__ void plane_pass_2d(const StageParams &P, double *Fsm, int t) {
-  const int v = t / EB, el = t - v * EB;
-  double *px = Fsm + (v * EB + el) * PS;
-  const double *pe = px + NVAR * EB * PS;
-  double R[NP][NP];
-#pragma unroll
-  for (int j = 0; j < NP; ++j) {
-    double f[NP];
-#pragma unroll
-    for (int m = 0; m < NP; ++m) f[m] = px[j * NP + m];
-#pragma unroll
-    for (int i = 0; i < NP; ++i) {
-      double acc = P.D[i * NP] * f[0];
-#pragma unroll
-      for (int m = 1; m < NP; ++m) acc += P.D[i * NP + m] * f[m];
-      R[j][i] = acc;
-    }
-  }
-#pragma unroll
-  for (int i = 0; i < NP; ++i) {
-    double f[NP];
-#pragma unroll
-    for (int m = 0; m < NP; ++m) f[m] = pe[m * NP + i];
-#pragma unroll
-    for (int j = 0; j < NP; ++j) {
-      double acc = R[j][i];
-#pragma unroll
-      for (int m = 0; m < NP; ++m) acc += P.D[j * NP + m] * f[m];
-      R[j][i] = acc;
-    }
-  }
-#pragma unroll
-  for (int j = 0; j < NP; ++j)
-#pragma unroll
-    for (int i = 0; i < NP; ++i) px[j * NP + i] = R[j][i];
 }
 
 #ifndef MARUT_NODE_MINB128
-#define MARUT_NODE_MINB128 5
+#define MARUT_NODE_MINB128 6
 #endif
 
 template <int DIM, int NP, bool AFFINE, int EB, int MINB>
@@ -361,136 +266,167 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   using G = Geo<DIM, NP>;
   constexpr int NVAR = C::NVAR, NN = C::NN, NF = C::NF, TILE = C::TILE, NFN = C::NFN, NTASK = C::NTASK, NT = C::NT;
   constexpr int MD = G::MD, MDP = C::MDP, KS = C::KS, PS = C::PS, NW = C::NW;
-  constexpr int NVT = (DIM == 3) ? C::NVT : EB * NVAR;   // plane tasks per pass
-  constexpr int NVW = (NVT + 31) / 32;                   // warps a derivative pass occupies
+  constexpr int NL = NF;                    // lines per direction and element
+  constexpr int NLT = NVAR * NL;            // line tasks per pass and element
   extern __shared__ __align__(16) double smem[];
   double *Fsm = smem;                       // [DIM][NVAR][EB] planes of PS doubles: contravariant fluxes
   double *Ust = Fsm + C::NPL * PS;          // [NVAR + 3][TILE]  U, 1/rho, p, a
   double *Lft = Ust + C::NST * TILE;        // [NVAR][NTASK]     lifts of the face nodes
   double *Msm = Lft + NVAR * NTASK;         // affine: [EB][MDP] Ja, 1/J, |Ja^l|
 
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tid = threadIdx.x;
   const long e0 = (long)blockIdx.x * EB;
   const int nel = (int)((P.ne - e0 < EB) ? (P.ne - e0) : EB);
-  const int ntask = nel * NFN;
-  // the derivative passes occupy NVW warps; rotate them over the CTA's warps (and so over the SM's four
-  // schedulers) with the block index, and hand the face tasks to the other warps first
-  const int rot = (int)(blockIdx.x % NW);
-  const int vrank = (warp - rot + NW) % NW;                  // rank in the derivative passes
-  const int srank = (warp - rot - NVW + 2 * NW) % NW;        // rank in the face phase
-  const int vt0 = vrank * 32 + lane, g0 = srank * 32 + lane;
+  const int ntask = nel * NFN, nline = nel * NLT;
 
   // first face task of this thread: connectivity load issued first (the neighbour gather depends on it)
-  const bool has0 = g0 < ntask;
-  const FaceTask t0 = decode_task<DIM, NP>(has0 ? g0 : 0);
+  const bool has0 = tid < ntask;
+  const FaceTask t0 = decode_task<DIM, NP>(has0 ? tid : 0);
   int2 cn0 = make_int2(0, FK_BOUNDARY);
   if (has0) cn0 = __ldg(&P.conn[(e0 + t0.el) * 2 * DIM + t0.f]);
 
   if constexpr (AFFINE) {
-    for (int i = tid; i < nel * MDP; i += NT) {
-      const int el = i / MDP, k = i - el * MDP;
-      Msm[i] = (k < MD) ? __ldg(&P.metric[(e0 + el) * MD + k]) : ((k < MD + DIM) ? __ldg(&P.fnorm[(e0 + el) * DIM + (k - MD)]) : 0.0);
+    if (tid < nel * MDP) {
+      const int el = tid / MDP, k = tid - el * MDP;
+      Msm[tid] = (k < MD) ? __ldg(&P.metric[(e0 + el) * MD + k]) : ((k < MD + DIM) ? __ldg(&P.fnorm[(e0 + el) * DIM + (k - MD)]) : 0.0);
     }
   }
 
   // ---- phase N: own node
-  const int el = tid / NN, p = tid - el * NN;
-  const long e = e0 + el;
-  const bool active = (tid < TILE) && (el < nel);
-  const int qi = p % NP, qj = (p / NP) % NP, qk = (DIM == 3) ? p / (NP * NP) : 0;
-  const int sp = p + (KS - NP * NP) * qk;   // node offset inside a flux plane
-  double U[NVAR], invJ = 0.0;
-  if (active) {
-    const double *up = P.u_in + e * NVAR * NN + p;
+  {
+    const int el = tid / NN, p = tid - el * NN;
+    const long e = e0 + el;
+    const bool active = (tid < TILE) && (el < nel);
+    double U[NVAR];
+    if (active) {
+      const double *up = P.u_in + e * NVAR * NN + p;
 #pragma unroll
-    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
+      for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
+    }
+    if (active) {
+      const int qk = (DIM == 3) ? p / (NP * NP) : 0;
+      const int sp = p + (KS - NP * NP) * qk;   // node offset inside a flux plane
+      double Ja[DIM * DIM];
+#pragma unroll
+      for (int k = 0; k < DIM * DIM; ++k) Ja[k] = metric_at<DIM, NP, AFFINE>(P.metric, e, k, p);
+      const Prim<DIM> pr = prim_ideal<DIM, true>(U, P.gamma);
+#pragma unroll
+      for (int l = 0; l < DIM; ++l) {
+        double F[NVAR];
+        flux_dot<DIM, 1>(U, pr, &Ja[l * DIM], F);
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Fsm[((l * NVAR + v) * EB + el) * PS + sp] = F[v];
+      }
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Ust[v * TILE + tid] = U[v];
+      Ust[NVAR * TILE + tid] = pr.irho;
+      Ust[(NVAR + 1) * TILE + tid] = pr.p;
+      Ust[(NVAR + 2) * TILE + tid] = pr.a;
+    }
   }
-  // neighbour trace of the first face task: in flight during phase N and the first derivative pass
+  // neighbour trace of the first face task: in flight during the xi pass
   double Up0[NVAR];
   if (has0) gather_exterior<DIM, NP, NVAR>(P, t0, cn0, Up0);
-  if (active) {
-    double Ja[DIM * DIM];
-#pragma unroll
-    for (int k = 0; k < DIM * DIM; ++k) Ja[k] = metric_at<DIM, NP, AFFINE>(P.metric, e, k, p);
-    invJ = metric_at<DIM, NP, AFFINE>(P.metric, e, DIM * DIM, p);
-    const Prim<DIM> pr = prim_ideal<DIM, true>(U, P.gamma);
-#pragma unroll
-    for (int l = 0; l < DIM; ++l) {
-      double F[NVAR];
-      flux_dot<DIM, 1>(U, pr, &Ja[l * DIM], F);
-#pragma unroll
-      for (int v = 0; v < NVAR; ++v) Fsm[((l * NVAR + v) * EB + el) * PS + sp] = F[v];
-    }
-#pragma unroll
-    for (int v = 0; v < NVAR; ++v) Ust[v * TILE + tid] = U[v];
-    Ust[NVAR * TILE + tid] = pr.irho;
-    Ust[(NVAR + 1) * TILE + tid] = pr.p;
-    Ust[(NVAR + 2) * TILE + tid] = pr.a;
-  }
   __syncthreads();
 
-  // ---- phase V, pass 1 (eq. 9): xi and eta derivatives per (variable, zeta-plane) task
-  if constexpr (DIM == 3) {
-    for (int t = vt0; t < nel * NVAR * NP; t += NT) plane_pass_xi_eta<NP, NVAR, EB, KS, PS, C::L::K_FASTEST>(P, Fsm, t);
-  } else {
-    for (int t = vt0; t < NVT; t += NT)
-      if (t % EB < nel) plane_pass_2d<NP, NVAR, EB, PS>(P, Fsm, t);
+  // ---- xi pass (eq. 9): lines (j,k) of variable v; lanes run over the lines first
+  for (int t = tid; t < nline; t += NT) {
+    const int el = t / NLT, r = t - el * NLT;
+    const int v = r / NL, ln = r - v * NL;
+    const int lj = ln % NP, lk = ln / NP;
+    double *px = Fsm + (v * EB + el) * PS + NP * lj + KS * lk;
+    double f[NP], acc[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) { f[m] = px[m]; acc[m] = 0.0; }
+    line_deriv<NP>(P, f, acc);
+#pragma unroll
+    for (int i = 0; i < NP; ++i) px[i] = acc[i];
   }
 
-  // ---- phase S: face nodes, densely mapped
-  if (has0) euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, g0, t0, cn0, Up0);
-  for (int g = g0 + NT; g < ntask; g += NT) {
+  // ---- face phase, first round: face nodes densely mapped
+  if (has0) euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
+  __syncthreads();
+
+  if constexpr (DIM == 3) {
+    // ---- eta pass: lines (i,k) of variable v; lane order (i, v, k) is bank-conflict-free
+    for (int t = tid; t < nline; t += NT) {
+      const int el = t / NLT, r = t - el * NLT;
+      const int li = r % NP, r2 = r / NP;
+      const int v = r2 % NVAR, lk = r2 / NVAR;
+      double *px = Fsm + (v * EB + el) * PS + li + KS * lk;
+      const double *pe = px + NVAR * EB * PS;
+      double f[NP], acc[NP];
+#pragma unroll
+      for (int m = 0; m < NP; ++m) { f[m] = pe[m * NP]; acc[m] = px[m * NP]; }
+      line_deriv<NP>(P, f, acc);
+#pragma unroll
+      for (int j = 0; j < NP; ++j) px[j * NP] = acc[j];
+    }
+  }
+  // ---- face phase, remaining rounds
+  for (int g = tid + NT; g < ntask; g += NT) {
     const FaceTask t = decode_task<DIM, NP>(g);
     const int2 cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
     double Up[NVAR];
     gather_exterior<DIM, NP, NVAR>(P, t, cn, Up);
     euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, g, t, cn, Up);
   }
-  // u_n for the final combination: issued here, consumed after the last barrier
-  double Un[NVAR];
-  const bool use_un = (P.ca != 0.0);
-  if (active && use_un) {
-    const double *np_ = P.u_n + e * NVAR * NN + p;
-#pragma unroll
-    for (int v = 0; v < NVAR; ++v) Un[v] = np_[v * NN];
-  }
-  if constexpr (DIM == 3) {
-    __syncthreads();
-    // ---- phase V, pass 2: zeta derivative per (variable, xi-index) task
-    for (int t = vt0; t < nel * NVAR * NP; t += NT) plane_pass_zeta<NP, NVAR, EB, KS, PS>(P, Fsm, t);
-  }
-  __syncthreads();
-  if (!active) return;
+  if constexpr (DIM == 3 || (NTASK > NT)) __syncthreads();
 
-  // ---- phase D: volume term + lifts of the own faces, 1/J, SSP-RK combination (eq. 12, 45)
-  double R[NVAR];
+  // ---- last pass (zeta in 3-D, eta in 2-D) fused with phase D: lifts, 1/J, SSP-RK combination (eq. 12, 45)
+  const bool use_un = (P.ca != 0.0);
+  for (int t = tid; t < nline; t += NT) {
+    const int el = t / NLT, r = t - el * NLT;
+    const int v = r / NL, ij = r - v * NL;       // 3-D: ij = i + NP*j ; 2-D: ij = i
+    constexpr int LS = (DIM == 3) ? KS : NP;      // stride of the line in the flux plane
+    constexpr int GS = (DIM == 3) ? NP * NP : NP; // stride of the line in global memory
+    const long e = e0 + el;
+    const double *px = Fsm + (v * EB + el) * PS + ij;
+    const double *pl = px + (DIM - 1) * NVAR * EB * PS;
+    const long gofs = (e * NVAR + v) * NN + ij;
+    double un[NP];
+    if (use_un) {
 #pragma unroll
-  for (int v = 0; v < NVAR; ++v) R[v] = Fsm[(v * EB + el) * PS + sp];
-  {
-    const int gb = el * NFN;
-    if (qi == 0 || qi == NP - 1) {
-      const int g = gb + ((qi == 0) ? 0 : 1) * NF + qj + NP * qk;
-#pragma unroll
-      for (int v = 0; v < NVAR; ++v) R[v] += Lft[v * NTASK + g];
+      for (int m = 0; m < NP; ++m) un[m] = P.u_n[gofs + m * GS];
     }
-    if (qj == 0 || qj == NP - 1) {
-      const int g = gb + (2 + ((qj == 0) ? 0 : 1)) * NF + qi + NP * qk;
+    double f[NP], acc[NP];
 #pragma unroll
-      for (int v = 0; v < NVAR; ++v) R[v] += Lft[v * NTASK + g];
+    for (int m = 0; m < NP; ++m) { f[m] = pl[m * LS]; acc[m] = px[m * LS]; }
+    line_deriv<NP>(P, f, acc);
+    // lifts of the faces the nodes of this line lie on
+    const double *lf = Lft + v * NTASK + el * NFN;
+    if constexpr (DIM == 3) {
+      const int qi = ij % NP, qj = ij / NP;
+      acc[0] += lf[4 * NF + ij];
+      acc[NP - 1] += lf[5 * NF + ij];
+      if (qi == 0 || qi == NP - 1) {
+        const double *l2 = lf + ((qi == 0) ? 0 : NF) + qj;
+#pragma unroll
+        for (int m = 0; m < NP; ++m) acc[m] += l2[NP * m];
+      }
+      if (qj == 0 || qj == NP - 1) {
+        const double *l2 = lf + ((qj == 0) ? 2 * NF : 3 * NF) + qi;
+#pragma unroll
+        for (int m = 0; m < NP; ++m) acc[m] += l2[NP * m];
+      }
+    } else {
+      acc[0] += lf[2 * NF + ij];
+      acc[NP - 1] += lf[3 * NF + ij];
+      if (ij == 0 || ij == NP - 1) {
+        const double *l2 = lf + ((ij == 0) ? 0 : NF);
+#pragma unroll
+        for (int m = 0; m < NP; ++m) acc[m] += l2[m];
+      }
     }
-    if (DIM == 3 && (qk == 0 || qk == NP - 1)) {
-      const int g = gb + (4 + ((qk == 0) ? 0 : 1)) * NF + qi + NP * qj;
+    const double *us = Ust + v * TILE + el * NN + ij;
+    double invJ = 0.0;
+    if constexpr (AFFINE) invJ = Msm[el * MDP + DIM * DIM];
 #pragma unroll
-      for (int v = 0; v < NVAR; ++v) R[v] += Lft[v * NTASK + g];
+    for (int m = 0; m < NP; ++m) {
+      if constexpr (!AFFINE) invJ = __ldg(&P.metric[(e * MD + DIM * DIM) * NN + ij + m * GS]);
+      const double val = P.cb * us[m * GS] + P.cc * (0.0 - invJ * acc[m]);
+      P.u_out[gofs + m * GS] = use_un ? (P.ca * un[m] + val) : val;
     }
-  }
-  double *op = P.u_out + e * NVAR * NN + p;
-  if (use_un) {
-#pragma unroll
-    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.ca * Un[v] + (P.cb * U[v] + P.cc * (0.0 - invJ * R[v]));
-  } else {
-#pragma unroll
-    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.cb * U[v] + P.cc * (0.0 - invJ * R[v]);
   }
 }
 
@@ -503,7 +439,7 @@ cudaError_t launch_stage_node_t(const StageParams &P, cudaStream_t st) {
   constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
   using C = NodeCfg<DIM, NP, 1, EB>;
   constexpr size_t smem = C::smem_doubles(AFFINE) * sizeof(double);
-  constexpr int MINB = (C::NT <= 128) ? MARUT_NODE_MINB128 : ((C::NT <= 256) ? 2 : 1);
+  constexpr int MINB = (C::NT <= 128) ? MARUT_NODE_MINB128 : ((C::NT <= 256) ? 3 : 1);
   auto k = stage_node_kernel<DIM, NP, AFFINE, EB, MINB>;
   static bool attr = false;
   if (!attr) {
