@@ -403,7 +403,7 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   if (m->physics == MARUT_REACTING_EULER) CUDA_TRY(cudaMalloc(&m->d_T, (size_t)ne * nn * sizeof(double)));
 
   const char *sel = getenv("MARUT_KERNEL");   // A/B switch for profiling: node (default) | line | generic
-  m->kernel_sel = (sel && !strcmp(sel, "line")) ? 1 : ((sel && !strcmp(sel, "generic")) ? 2 : 0);
+  m->kernel_sel = (sel && !strcmp(sel, "line")) ? 1 : ((sel && !strcmp(sel, "generic")) ? 2 : ((sel && !strcmp(sel, "line2")) ? 3 : 0));
   return MARUT_OK;
 }
 
@@ -464,7 +464,8 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   switch (m->physics) {
     case MARUT_EULER:
       e = cudaErrorNotSupported;
-      if (m->kernel_sel == 0) e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
+      if (m->kernel_sel == 3 && m->dim == 3 && m->affine && m->n_mortar == 0) e = launch_stage_line2_3d(m->np, P, st);
+      if (m->kernel_sel == 0 || (m->kernel_sel == 3 && e == cudaErrorNotSupported)) e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
       if (m->kernel_sel == 1) e = (m->dim == 2) ? launch_stage_line2d(m->np, m->affine, P, st) : launch_stage_line3d(m->np, m->affine, P, st);
       if (e == cudaErrorNotSupported)
         e = (m->dim == 2) ? launch_stage_euler2d(m->np, m->affine, P, st) : launch_stage_euler3d(m->np, m->affine, P, st);

@@ -29,8 +29,8 @@ struct NodeLayout {
 };
 template <int EB>
 struct NodeLayout<3, 5, EB> {
-  static constexpr int KS = 25, PS = 133;
-  static constexpr bool K_FASTEST = false;
+  static constexpr int KS = 25, PS = 125;   // unpadded: with the lane orders of the three passes below every
+  static constexpr bool K_FASTEST = false;  // half-warp hits 16 distinct banks in the xi and eta passes
 };
 template <int EB>
 struct NodeLayout<3, 4, EB> {
@@ -348,11 +348,11 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   __syncthreads();
 
   if constexpr (DIM == 3) {
-    // ---- eta pass: lines (i,k) of variable v; lane order (i, v, k) is bank-conflict-free
+    // ---- eta pass: lines (i,k) of variable v; lane order (k, v, i) is bank-conflict-free
     for (int t = tid; t < nline; t += NT) {
       const int el = t / NLT, r = t - el * NLT;
-      const int li = r % NP, r2 = r / NP;
-      const int v = r2 % NVAR, lk = r2 / NVAR;
+      const int lk = r % NP, r2 = r / NP;
+      const int v = r2 % NVAR, li = r2 / NVAR;
       double *px = Fsm + (v * EB + el) * PS + li + KS * lk;
       const double *pe = px + NVAR * EB * PS;
       double f[NP], acc[NP];

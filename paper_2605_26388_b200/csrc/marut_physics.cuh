@@ -144,6 +144,45 @@ __device__ __forceinline__ void rusanov(const double *Um, const Prim<DIM> &qm, c
   for (int v = 0; v < NVAR; ++v) Fs[v] = 0.5 * (Fm[v] + Fp[v]) - hl * (Up[v] - Um[v]);
 }
 
+// Rusanov lift of one face node from the two states (Euler; eq. 12; R5, R6), with a
+// scaled normal and division-free apart from 1/rho+:
+//   lambda |nv| = max(|v-.nv| + a- |nv|, |v+.nv| + a+ |nv|);  lift = (F*(U-,U+;nv) - F(U-).nv)/w_b
+// Fm_out = F(U-).nv (for the faces whose F* comes from elsewhere, e.g. mortars).
+template <int DIM>
+__device__ __forceinline__ void rusanov_lift(const double *Um, double irhom, double pm, double am, const double *Up,
+                                             const double *nv, double nrm, double gamma, double inv_wb, double *lift,
+                                             double *Fm_out) {
+  constexpr int NVAR = DIM + 2;
+  double mnm = 0.0, mnp = 0.0, kep = 0.0;
+#pragma unroll
+  for (int c = 0; c < DIM; ++c) {
+    mnm += Um[1 + c] * nv[c];
+    mnp += Up[1 + c] * nv[c];
+    kep += Up[1 + c] * Up[1 + c];
+  }
+  const double irhop = 1.0 / Up[0];
+  const double vnm = mnm * irhom;
+  const double pp = (gamma - 1.0) * (Up[DIM + 1] - 0.5 * kep * irhop);
+  const double ap = sqrt(gamma * pp * irhop);
+  const double vnp = mnp * irhop;
+  const double hl = 0.5 * fmax(fabs(vnm) + am * nrm, fabs(vnp) + ap * nrm);
+  double Fm[NVAR], Fp[NVAR];
+  Fm[0] = mnm;
+  Fp[0] = mnp;
+#pragma unroll
+  for (int c = 0; c < DIM; ++c) {
+    Fm[1 + c] = Um[1 + c] * vnm + pm * nv[c];
+    Fp[1 + c] = Up[1 + c] * vnp + pp * nv[c];
+  }
+  Fm[DIM + 1] = (Um[DIM + 1] + pm) * vnm;
+  Fp[DIM + 1] = (Up[DIM + 1] + pp) * vnp;
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) {
+    lift[v] = inv_wb * (0.5 * (Fp[v] - Fm[v]) - hl * (Up[v] - Um[v]));
+    Fm_out[v] = Fm[v];
+  }
+}
+
 // viscous flux F_v(U,S).nv (eq. 15; q = -k grad T, k = gamma mu/(Pr (gamma-1)))
 // S[w*DIM + c] = d W_w / d x_c, W = (rho, v_1..v_d, T); F has DIM+2 entries, F[0] = 0.
 template <int DIM>
