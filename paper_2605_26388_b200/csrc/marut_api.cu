@@ -271,12 +271,32 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
       for (int r = 0; r < 2; ++r)
         for (int c = 0; c < 7; ++c) h.nasa[s][r][c] = k->nasa[(s * 2 + r) * 7 + c];
     }
+    // reactions sorted (stably) by their net stoichiometric vector: reactions that differ only in the third body
+    // share K_c, so the kernel evaluates exp(-dG) once per group
+    std::vector<int> order(h.nr), grp(h.nr, -1);
+    int ngrp = 0;
     for (int r = 0; r < h.nr; ++r) {
-      h.A[r] = k->A[r]; h.b[r] = k->b[r]; h.Ea[r] = k->Ea[r];
       for (int s = 0; s < h.ns; ++s) {
         int a = k->nu_r[r * h.ns + s], b = k->nu_p[r * h.ns + s];
         if (a < 0 || a > 3 || b < 0 || b > 3) return fail(MARUT_EINVAL, "stoichiometric coefficient out of 0..3");
-        h.nu_r[r][s] = (signed char)a; h.nu_p[r][s] = (signed char)b;
+      }
+      for (int q = 0; q < r && grp[r] < 0; ++q) {
+        bool same = true;
+        for (int s = 0; s < h.ns; ++s)
+          same = same && (k->nu_p[r * h.ns + s] - k->nu_r[r * h.ns + s] == k->nu_p[q * h.ns + s] - k->nu_r[q * h.ns + s]);
+        if (same) grp[r] = grp[q];
+      }
+      if (grp[r] < 0) grp[r] = ngrp++;
+    }
+    for (int r = 0; r < h.nr; ++r) order[r] = r;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return grp[a] < grp[b]; });
+    for (int i = 0; i < h.nr; ++i) {
+      const int r = order[i];
+      h.A[i] = k->A[r]; h.b[i] = k->b[r]; h.Ea[i] = k->Ea[r];
+      h.new_group[i] = (i == 0 || grp[order[i - 1]] != grp[r]) ? 1 : 0;
+      for (int s = 0; s < h.ns; ++s) {
+        h.nu_r[i][s] = (signed char)k->nu_r[r * h.ns + s];
+        h.nu_p[i][s] = (signed char)k->nu_p[r * h.ns + s];
       }
     }
     m->nsp = h.ns;
@@ -470,8 +490,8 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
       if (e == cudaErrorNotSupported)
         e = (m->dim == 2) ? launch_stage_euler2d(m->np, m->affine, P, st) : launch_stage_euler3d(m->np, m->affine, P, st);
       break;
-    case MARUT_NAVIER_STOKES: e = launch_stage_ns(m->dim, m->np, m->affine, P, st); break;
-    default: e = launch_stage_react(m->dim, m->np, m->nsp, m->affine, P, st); break;
+    case MARUT_NAVIER_STOKES: e = launch_stage_ns(m->dim, m->np, m->affine, m->kernel_sel == 2, P, st); break;
+    default: e = launch_stage_react(m->dim, m->np, m->nsp, m->affine, m->kernel_sel == 2, P, st); break;
   }
   if (e == cudaErrorNotSupported) return fail(MARUT_EINVAL, "no kernel instantiated for dim=%d N=%d physics=%d", m->dim, m->N, m->physics);
   if (e != cudaSuccess) return fail(MARUT_ECUDA, "stage kernel: %s", cudaGetErrorString(e));

@@ -1,0 +1,334 @@
+// marut_node_phys.cuh -- the node kernel (marut_node.cuh) for the physics with extra per-node work:
+// Navier-Stokes with BR1 viscous fluxes (eq. 15-16) and the reacting
+// mixture with its chemistry source (a8, a9; eq. 20-22).  Same structure: thread-per-node
+// flux evaluation, balanced line-task derivative passes, densely mapped face tasks, last pass fused with the
+// lift + 1/J + source + SSP-RK combination.  Differences from the Euler instance: the derivative passes write
+// a separate result plane set (the flux planes stay intact because the viscous face tasks read the own
+// normal flux from them), the chemistry source goes through shared source planes, and the face tasks gather
+// the neighbour's BR1 gradient (NS) or temperature (reacting) as well.  Conforming interior faces only.
+//
+// Product code; shares nothing with oracle/.
+#pragma once
+#include "marut_node.cuh"
+
+namespace marut {
+
+template <int DIM, int NP, int NSP, int PHYS, int EB>
+struct PhysCfg {
+  using G = Geo<DIM, NP>;
+  static constexpr int NVAR = NSP + DIM + 1, NW = DIM + 2;
+  static constexpr int NN = G::NN, NF = G::NF;
+  static constexpr int TILE = EB * NN;
+  static constexpr int NFN = 2 * DIM * NF, NTASK = EB * NFN;
+  static constexpr int NT = ((TILE + 31) / 32) * 32;
+  static constexpr int NST = NVAR + 3;                       // stash planes: U, 1/rho, p, a
+  static constexpr int KS = NP * NP, PS = NN | 1;            // plane strides (odd plane stride)
+  static constexpr int NFP = DIM * NVAR * EB;                // flux planes
+  static constexpr int NRP = NVAR * EB;                      // result planes
+  static constexpr int NSRC = (PHYS == PH_REACT) ? NSP * TILE : 0;
+  static constexpr int MDP = ((G::MD + DIM + 1) / 2) * 2;
+  static constexpr size_t smem_doubles(bool affine) {
+    return (size_t)(NFP + NRP) * PS + (size_t)NST * TILE + (size_t)NVAR * NTASK + NSRC + (affine ? EB * MDP : 0);
+  }
+};
+
+template <int DIM, int NP, int NSP, int PHYS, bool AFFINE, int EB, int MINB>
+__global__ void __launch_bounds__((PhysCfg<DIM, NP, NSP, PHYS, EB>::NT), MINB)
+stage_phys_kernel(const __grid_constant__ StageParams P) {
+  using C = PhysCfg<DIM, NP, NSP, PHYS, EB>;
+  using G = Geo<DIM, NP>;
+  constexpr int NVAR = C::NVAR, NW = C::NW, NN = C::NN, NF = C::NF, TILE = C::TILE, NFN = C::NFN, NTASK = C::NTASK;
+  constexpr int NT = C::NT, MD = G::MD, MDP = C::MDP, KS = C::KS, PS = C::PS;
+  constexpr int NL = NF, NLT = NVAR * NL;
+  extern __shared__ __align__(16) double smem[];
+  double *Fsm = smem;                         // [DIM][NVAR][EB] flux planes (kept intact)
+  double *Rsm = Fsm + C::NFP * PS;            // [NVAR][EB] result planes of the derivative passes
+  double *Ust = Rsm + C::NRP * PS;            // [NVAR + 3][TILE]  U, 1/rho, p, a
+  double *Lft = Ust + C::NST * TILE;          // [NVAR][NTASK]     lifts of the face nodes
+  double *Src = Lft + NVAR * NTASK;           // reacting: [NSP][TILE] chemistry source
+  double *Msm = Src + C::NSRC;                // affine: [EB][MDP] Ja, 1/J, |Ja^l|
+  __shared__ MechDev mech_s;
+
+  const int tid = threadIdx.x;
+  const long e0 = (long)blockIdx.x * EB;
+  const int nel = (int)((P.ne - e0 < EB) ? (P.ne - e0) : EB);
+  const int ntask = nel * NFN, nline = nel * NLT;
+
+  // first face task of this thread: connectivity load first (the neighbour gather depends on it)
+  const bool has0 = tid < ntask;
+  const FaceTask t0 = decode_task<DIM, NP>(has0 ? tid : 0);
+  int2 cn0 = make_int2(0, 0);
+  if (has0) cn0 = __ldg(&P.conn[(e0 + t0.el) * 2 * DIM + t0.f]);
+
+  if constexpr (PHYS == PH_REACT) {
+    const int *src = reinterpret_cast<const int *>(P.mech);
+    int *dst = reinterpret_cast<int *>(&mech_s);
+    for (int i = tid; i < (int)(sizeof(MechDev) / sizeof(int)); i += NT) dst[i] = src[i];
+  }
+  if constexpr (AFFINE) {
+    if (tid < nel * MDP) {
+      const int me = tid / MDP, k = tid - me * MDP;
+      Msm[tid] = (k < MD) ? __ldg(&P.metric[(e0 + me) * MD + k]) : ((k < MD + DIM) ? __ldg(&P.fnorm[(e0 + me) * DIM + (k - MD)]) : 0.0);
+    }
+  }
+  const int el = tid / NN, p = tid - el * NN;
+  const long e = e0 + el;
+  const bool active = (tid < TILE) && (el < nel);
+  double U[NVAR], T = 0.0;
+  if (active) {
+    const double *up = P.u_in + e * NVAR * NN + p;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
+    if constexpr (PHYS == PH_REACT) T = __ldg(&P.Taux[e * NN + p]);
+  }
+  // neighbour trace of the first face task: in flight during phase N
+  double Up0[NVAR], Tp0 = 0.0;
+  int pR0 = 0;
+  if (has0) {
+    const int fR = (cn0.y >> 2) & 7, orient = (cn0.y >> 5) & 7;
+    const int b0 = (DIM == 2 && orient) ? NP - 1 - t0.a0 : t0.a0;
+    pR0 = face_node_of<DIM, NP>(fR, b0, t0.a1);
+    const double *un = P.u_in + (long)cn0.x * NVAR * NN + pR0;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Up0[v] = __ldg(un + v * NN);
+    if constexpr (PHYS == PH_REACT) Tp0 = __ldg(&P.Taux[(long)cn0.x * NN + pR0]);
+  }
+  if constexpr (PHYS == PH_REACT) __syncthreads();   // mechanism table in shared memory
+  const MechDev *mech = (PHYS == PH_REACT) ? &mech_s : nullptr;
+
+  // ---- phase N: own node
+  if (active) {
+    const int qk = (DIM == 3) ? p / (NP * NP) : 0;
+    const int sp = p + (KS - NP * NP) * qk;
+    double Ja[DIM * DIM];
+#pragma unroll
+    for (int k = 0; k < DIM * DIM; ++k) Ja[k] = metric_at<DIM, NP, AFFINE>(P.metric, e, k, p);
+    const Prim<DIM> pr = make_prim<DIM, NSP, PHYS, true>(U, T, P.gamma, mech);
+    double Sg[(PHYS == PH_NS) ? NW * DIM : 1];
+    if constexpr (PHYS == PH_NS) {
+#pragma unroll
+      for (int k = 0; k < NW * DIM; ++k) Sg[k] = __ldg(&P.S[(e * NW * DIM + k) * NN + p]);
+    }
+#pragma unroll
+    for (int l = 0; l < DIM; ++l) {
+      double F[NVAR];
+      flux_dot<DIM, NSP>(U, pr, &Ja[l * DIM], F);
+      if constexpr (PHYS == PH_NS) {
+        double Fv[NW];
+        viscous_flux_dot<DIM>(pr.v, Sg, &Ja[l * DIM], P.mu, P.kappa, Fv);
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) F[v] -= Fv[v];
+      }
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Fsm[((l * NVAR + v) * EB + el) * PS + sp] = F[v];
+    }
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Ust[v * TILE + tid] = U[v];
+    Ust[NVAR * TILE + tid] = pr.irho;
+    Ust[(NVAR + 1) * TILE + tid] = pr.p;
+    Ust[(NVAR + 2) * TILE + tid] = pr.a;
+    if constexpr (PHYS == PH_REACT) {
+      double om[NSP];
+      production_rates<NSP>(*mech, T, U, om);
+#pragma unroll
+      for (int s = 0; s < NSP; ++s) Src[s * TILE + tid] = om[s];
+    }
+  }
+  __syncthreads();
+
+  // ---- xi pass (eq. 9): lines (j,k) of variable v -> result planes
+  for (int t = tid; t < nline; t += NT) {
+    const int le = t / NLT, r = t - le * NLT;
+    const int v = r / NL, ln = r - v * NL;
+    const int lj = ln % NP, lk = ln / NP;
+    const int off = (v * EB + le) * PS + NP * lj + KS * lk;
+    double f[NP], acc[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) { f[m] = Fsm[off + m]; acc[m] = 0.0; }
+    line_deriv<NP>(P, f, acc);
+#pragma unroll
+    for (int i = 0; i < NP; ++i) Rsm[off + i] = acc[i];
+  }
+
+  // ---- face tasks, densely mapped (a2; NS: + BR1 viscous interface flux, eq. 16)
+  for (int g = tid; g < ntask; g += NT) {
+    FaceTask t;
+    int2 cn;
+    double Up[NVAR], Tp = 0.0;
+    int pR;
+    if (g == tid) {
+      t = t0; cn = cn0; pR = pR0; Tp = Tp0;
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Up[v] = Up0[v];
+    } else {
+      t = decode_task<DIM, NP>(g);
+      cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
+      const int fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7;
+      const int b0 = (DIM == 2 && orient) ? NP - 1 - t.a0 : t.a0;
+      pR = face_node_of<DIM, NP>(fR, b0, t.a1);
+      const double *un = P.u_in + (long)cn.x * NVAR * NN + pR;
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
+      if constexpr (PHYS == PH_REACT) Tp = __ldg(&P.Taux[(long)cn.x * NN + pR]);
+    }
+    const int l = t.f >> 1;
+    const double sgn = (t.f & 1) ? 1.0 : -1.0;
+    const int idx = t.el * NN + t.p;
+    const long ee = e0 + t.el;
+    double Um[NVAR], nv[DIM], nrm;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Um[v] = Ust[v * TILE + idx];
+    const double irhom = Ust[NVAR * TILE + idx], pm = Ust[(NVAR + 1) * TILE + idx], am = Ust[(NVAR + 2) * TILE + idx];
+    if constexpr (AFFINE) {
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) nv[c] = sgn * Msm[t.el * MDP + l * DIM + c];
+      nrm = Msm[t.el * MDP + MD + l];
+    } else {
+      double n2 = 0.0;
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) {
+        nv[c] = sgn * __ldg(&P.metric[(ee * MD + l * DIM + c) * NN + t.p]);
+        n2 += nv[c] * nv[c];
+      }
+      nrm = sqrt(n2);
+    }
+    const Prim<DIM> qp = make_prim<DIM, NSP, PHYS, true>(Up, Tp, P.gamma, mech);
+    double mnm = 0.0, vnp = 0.0;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) {
+      mnm += Um[NSP + c] * nv[c];
+      vnp += qp.v[c] * nv[c];
+    }
+    const double vnm = mnm * irhom;
+    const double hl = 0.5 * fmax(fabs(vnm) + am * nrm, fabs(vnp) + qp.a * nrm);
+    double Fm[NVAR], Fp[NVAR], lift[NVAR];
+#pragma unroll
+    for (int s = 0; s < NSP; ++s) {
+      Fm[s] = Um[s] * vnm;
+      Fp[s] = Up[s] * vnp;
+    }
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) {
+      Fm[NSP + c] = Um[NSP + c] * vnm + pm * nv[c];
+      Fp[NSP + c] = Up[NSP + c] * vnp + qp.p * nv[c];
+    }
+    Fm[NSP + DIM] = (Um[NSP + DIM] + pm) * vnm;
+    Fp[NSP + DIM] = (Up[NSP + DIM] + qp.p) * vnp;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) lift[v] = 0.5 * (Fp[v] - Fm[v]) - hl * (Up[v] - Um[v]);
+    if constexpr (PHYS == PH_NS) {
+      // viscous part: F_v* = mean of the two sides; own F_v.n = F_inv(U-).n - (own total normal flux in the plane)
+      double Sp[NW * DIM], Fvp[NW];
+#pragma unroll
+      for (int k = 0; k < NW * DIM; ++k) Sp[k] = __ldg(&P.S[((long)cn.x * NW * DIM + k) * NN + pR]);
+      viscous_flux_dot<DIM>(qp.v, Sp, nv, P.mu, P.kappa, Fvp);
+      const int qk = (DIM == 3) ? t.p / (NP * NP) : 0;
+      const int sp = t.p + (KS - NP * NP) * qk;
+#pragma unroll
+      for (int v = 1; v < NVAR; ++v) {
+        const double Fvm = Fm[v] - sgn * Fsm[((l * NVAR + v) * EB + t.el) * PS + sp];
+        lift[v] -= 0.5 * (Fvp[v] - Fvm);
+      }
+    }
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Lft[v * NTASK + g] = P.inv_wb * lift[v];
+  }
+  __syncthreads();
+
+  if constexpr (DIM == 3) {
+    // ---- eta pass: lines (i,k) of variable v; lane order (k, v, i)
+    for (int t = tid; t < nline; t += NT) {
+      const int le = t / NLT, r = t - le * NLT;
+      const int lk = r % NP, r2 = r / NP;
+      const int v = r2 % NVAR, li = r2 / NVAR;
+      const int off = (v * EB + le) * PS + li + KS * lk;
+      const double *pe = Fsm + NVAR * EB * PS + off;
+      double f[NP], acc[NP];
+#pragma unroll
+      for (int m = 0; m < NP; ++m) { f[m] = pe[m * NP]; acc[m] = Rsm[off + m * NP]; }
+      line_deriv<NP>(P, f, acc);
+#pragma unroll
+      for (int j = 0; j < NP; ++j) Rsm[off + j * NP] = acc[j];
+    }
+    __syncthreads();
+  }
+
+  // ---- last pass (zeta in 3-D, eta in 2-D) fused with phase D: lifts, 1/J, source, SSP-RK combination
+  const bool use_un = (P.ca != 0.0);
+  for (int t = tid; t < nline; t += NT) {
+    const int le = t / NLT, r = t - le * NLT;
+    const int v = r / NL, ij = r - v * NL;
+    constexpr int LS = (DIM == 3) ? KS : NP;
+    constexpr int GS = (DIM == 3) ? NP * NP : NP;
+    const long ee = e0 + le;
+    const int off = (v * EB + le) * PS + ij;
+    const double *pl = Fsm + (DIM - 1) * NVAR * EB * PS + off;
+    const long gofs = (ee * NVAR + v) * NN + ij;
+    double un[NP];
+    if (use_un) {
+#pragma unroll
+      for (int m = 0; m < NP; ++m) un[m] = P.u_n[gofs + m * GS];
+    }
+    double f[NP], acc[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) { f[m] = pl[m * LS]; acc[m] = Rsm[off + m * LS]; }
+    line_deriv<NP>(P, f, acc);
+    const double *lf = Lft + v * NTASK + le * NFN;
+    if constexpr (DIM == 3) {
+      const int li = ij % NP, lj = ij / NP;
+      acc[0] += lf[4 * NF + ij];
+      acc[NP - 1] += lf[5 * NF + ij];
+      if (li == 0 || li == NP - 1) {
+        const double *l2 = lf + ((li == 0) ? 0 : NF) + lj;
+#pragma unroll
+        for (int m = 0; m < NP; ++m) acc[m] += l2[NP * m];
+      }
+      if (lj == 0 || lj == NP - 1) {
+        const double *l2 = lf + ((lj == 0) ? 2 * NF : 3 * NF) + li;
+#pragma unroll
+        for (int m = 0; m < NP; ++m) acc[m] += l2[NP * m];
+      }
+    } else {
+      acc[0] += lf[2 * NF + ij];
+      acc[NP - 1] += lf[3 * NF + ij];
+      if (ij == 0 || ij == NP - 1) {
+        const double *l2 = lf + ((ij == 0) ? 0 : NF);
+#pragma unroll
+        for (int m = 0; m < NP; ++m) acc[m] += l2[m];
+      }
+    }
+    const double *us = Ust + v * TILE + le * NN + ij;
+    double invJ = 0.0;
+    if constexpr (AFFINE) invJ = Msm[le * MDP + DIM * DIM];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) {
+      if constexpr (!AFFINE) invJ = __ldg(&P.metric[(ee * MD + DIM * DIM) * NN + ij + m * GS]);
+      double src = 0.0;
+      if constexpr (PHYS == PH_REACT) {
+        if (v < NSP) src = Src[v * TILE + le * NN + ij + m * GS];
+      }
+      const double val = P.cb * us[m * GS] + P.cc * (src - invJ * acc[m]);
+      P.u_out[gofs + m * GS] = use_un ? (P.ca * un[m] + val) : val;
+    }
+  }
+}
+
+template <int DIM, int NP, int NSP, int PHYS, bool AFFINE>
+cudaError_t launch_stage_phys_t(const StageParams &P, cudaStream_t st) {
+  constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
+  using C = PhysCfg<DIM, NP, NSP, PHYS, EB>;
+  constexpr size_t smem = C::smem_doubles(AFFINE) * sizeof(double);
+  constexpr int MINB = (PHYS == PH_REACT) ? ((C::NT <= 128) ? 3 : 1) : ((C::NT <= 128) ? 4 : ((C::NT <= 256) ? 2 : 1));
+  auto k = stage_phys_kernel<DIM, NP, NSP, PHYS, AFFINE, EB, MINB>;
+  static bool attr = false;
+  if (!attr) {
+    cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    attr = true;
+  }
+  const long grid = (P.ne + EB - 1) / EB;
+  k<<<(unsigned)grid, C::NT, smem, st>>>(P);
+  return cudaGetLastError();
+}
+
+}  // namespace marut

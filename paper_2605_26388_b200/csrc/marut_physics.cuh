@@ -215,8 +215,10 @@ __device__ __forceinline__ void viscous_flux_dot(const double *vel, const double
 // K_c = exp(-sum dnu g_s/(R_u T)) (p_ref/(R_u T) 1e-6)^(sum dnu)  (R12)
 template <int NSP>
 __device__ inline void production_rates(const MechDev &m, double T, const double *rho_s, double *omega) {
+  // k_f = A exp(b ln T - Ea/T);  k_b = k_f / K_c = A exp(b ln T - Ea/T + dG - dnu ln c0): two exponentials per
+  // reaction, no pow() and no division (same value as the definition up to rounding)
   double X[NSP], g[NSP];
-  const double lnT = log(T);
+  const double lnT = log(T), invT = 1.0 / T;
 #pragma unroll
   for (int s = 0; s < NSP; ++s) {
     X[s] = rho_s[s] / m.W[s] * 1.0e-6;
@@ -224,27 +226,28 @@ __device__ inline void production_rates(const MechDev &m, double T, const double
     g[s] = Thermo::h_RT(a, T) - Thermo::s_R(a, T, lnT);
     omega[s] = 0.0;
   }
-  const double c0 = P_REF / (R_UNIVERSAL * T) * 1.0e-6;
+  const double lnc0 = log(P_REF / (R_UNIVERSAL * T) * 1.0e-6);
+  double ikc = 1.0;   // 1 / K_c of the current group of reactions (same net stoichiometric vector)
   for (int r = 0; r < m.nr; ++r) {
-    const double kf = m.A[r] * pow(T, m.b[r]) * exp(-m.Ea[r] / T);
     double dG = 0.0, pf = 1.0, pb = 1.0;
     int dnu = 0;
 #pragma unroll
     for (int s = 0; s < NSP; ++s) {
       const int nr_ = m.nu_r[r][s], np_ = m.nu_p[r][s];
       const int d = np_ - nr_;
-      dG += d * g[s];
-      dnu += d;
-      for (int k = 0; k < nr_; ++k) pf *= X[s];
-      for (int k = 0; k < np_; ++k) pb *= X[s];
+      if (d != 0) { dG += d * g[s]; dnu += d; }
+      if (nr_ > 0) pf *= (nr_ == 1) ? X[s] : ((nr_ == 2) ? X[s] * X[s] : X[s] * X[s] * X[s]);
+      if (np_ > 0) pb *= (np_ == 1) ? X[s] : ((np_ == 2) ? X[s] * X[s] : X[s] * X[s] * X[s]);
     }
-    double f = 1.0;
-    for (int k = 0; k < abs(dnu); ++k) f *= c0;
-    if (dnu < 0) f = 1.0 / f;
-    const double Kc = exp(-dG) * f;
-    const double Rr = kf * pf - (kf / Kc) * pb;
+    if (m.new_group[r]) ikc = exp(dG - dnu * lnc0);
+    const double kf = m.A[r] * exp(m.b[r] * lnT - m.Ea[r] * invT);
+    const double kb = kf * ikc;
+    const double Rr = kf * pf - kb * pb;
 #pragma unroll
-    for (int s = 0; s < NSP; ++s) omega[s] += (m.nu_p[r][s] - m.nu_r[r][s]) * Rr;
+    for (int s = 0; s < NSP; ++s) {
+      const int d = m.nu_p[r][s] - m.nu_r[r][s];
+      if (d != 0) omega[s] += d * Rr;
+    }
   }
 #pragma unroll
   for (int s = 0; s < NSP; ++s) omega[s] = m.W[s] * omega[s] * 1.0e6;
