@@ -39,11 +39,8 @@ class _MeshDesc(C.Structure):
                 ("mech", C.c_void_p)]
 
 
-def lib():
-    global _lib
-    if _lib is None:
-        _lib = C.CDLL(build())
-        L = _lib
+def _setup(L):
+    if True:
         dp, vp = C.POINTER(C.c_double), C.c_void_p
         L.oracle_mesh_create.restype = vp
         L.oracle_mesh_create.argtypes = [vp]
@@ -78,7 +75,37 @@ def lib():
         L.oracle_temperature.argtypes = [vp, vp, C.c_double]
         L.oracle_species_thermo.argtypes = [vp, C.c_int, C.c_double, vp]
         L.oracle_num_threads.restype = C.c_int
+    return L
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = _setup(C.CDLL(build()))
     return _lib
+
+
+_LIB_FMA = os.path.join(_HERE, "libmarut_oracle_fma.so")
+_lib_fma = None
+
+
+def lib_fma():
+    """The SAME source compiled with FMA contraction allowed (-ffp-contract=fast -mfma): a legal re-rounding of
+    the oracle's own arithmetic.  Used only to measure how far an oracle result moves under the one difference
+    the north star allows between the two sides ("reduction-order differences", FMA contraction) -- the
+    full-size parity tolerance of DESIGN.md reading T1.  None when the host CPU has no FMA unit."""
+    global _lib_fma
+    if _lib_fma is None:
+        try:
+            if "fma" not in open("/proc/cpuinfo").read().split("flags", 1)[1].split("\n", 1)[0].split():
+                return None
+        except Exception:
+            return None
+        if not os.path.exists(_LIB_FMA) or os.path.getmtime(_LIB_FMA) < os.path.getmtime(_SRC):
+            cmd = ["g++", "-O2", "-ffp-contract=fast", "-mfma", "-fopenmp", "-std=c++17", "-shared", "-fPIC", _SRC, "-o", _LIB_FMA]
+            subprocess.run(cmd, check=True)
+        _lib_fma = _setup(C.CDLL(_LIB_FMA))
+    return _lib_fma
 
 
 def _p(a):
@@ -129,8 +156,9 @@ class MechHandle:
 
 
 class OracleMesh:
-    def __init__(self, mesh):
-        L = lib()
+    def __init__(self, mesh, L=None):
+        L = L or lib()
+        self.L = L
         self.mesh = mesh
         self._keep = [_f64(mesh.node_xyz), _i32(mesh.iface), _i32(mesh.mortar), _i32(mesh.bface), _f64(mesh.bc_state)]
         k = self._keep
@@ -143,19 +171,19 @@ class OracleMesh:
         self.shape = (mesh.n_elem, self.nvar, mesh.nn)
 
     def __del__(self):
-        if getattr(self, "h", None):
-            lib().oracle_mesh_destroy(self.h)
+        if getattr(self, "h", None) and getattr(self, "L", None) is not None:
+            self.L.oracle_mesh_destroy(self.h)
             self.h = None
 
     @property
     def dx_min(self):
-        return lib().oracle_dx_min(self.h)
+        return self.L.oracle_dx_min(self.h)
 
     def metrics(self):
         m = self.mesh
         Ja = np.zeros((m.n_elem, m.nn, m.dim, m.dim))
         J = np.zeros((m.n_elem, m.nn))
-        lib().oracle_metrics(self.h, _p(Ja), _p(J))
+        self.L.oracle_metrics(self.h, _p(Ja), _p(J))
         return Ja, J
 
     def _call(self, fn, u, *extra):
@@ -165,47 +193,47 @@ class OracleMesh:
         return out
 
     def rhs(self, u, t=0.0):
-        return self._call(lib().oracle_rhs, u, t)
+        return self._call(self.L.oracle_rhs, u, t)
 
     def rhs_inviscid(self, u):
-        return self._call(lib().oracle_rhs_inviscid, u)
+        return self._call(self.L.oracle_rhs_inviscid, u)
 
     def rhs_viscous(self, u):
-        return self._call(lib().oracle_rhs_viscous, u)
+        return self._call(self.L.oracle_rhs_viscous, u)
 
     def chem_source(self, u):
-        return self._call(lib().oracle_chem_source, u)
+        return self._call(self.L.oracle_chem_source, u)
 
     def br1_gradient(self, u):
         m = self.mesh
         u = _f64(u)
         S = np.zeros((m.n_elem, m.nn, m.dim + 2, m.dim))
-        lib().oracle_br1_gradient(self.h, _p(u), _p(S))
+        self.L.oracle_br1_gradient(self.h, _p(u), _p(S))
         return S
 
     def primitives(self, U):
         U = _f64(U)
         out = np.zeros(7)
-        lib().oracle_primitives(self.h, _p(U), _p(out))
+        self.L.oracle_primitives(self.h, _p(U), _p(out))
         return dict(rho=out[0], p=out[1], a=out[2], T=out[3], vel=out[4:7].copy())
 
     def ssprk_stage(self, stage, dt, t_n, u_n, u_in):
         u_n, u_in = _f64(u_n), _f64(u_in)
         out = np.zeros(self.shape)
-        lib().oracle_ssprk_stage(self.h, stage, dt, t_n, _p(u_n), _p(u_in), _p(out))
+        self.L.oracle_ssprk_stage(self.h, stage, dt, t_n, _p(u_n), _p(u_in), _p(out))
         return out
 
     def max_dt(self, u, cfl, return_lambda=False):
         u = _f64(u)
         lam = C.c_double(0.0)
-        dt = lib().oracle_max_dt(self.h, _p(u), cfl, C.addressof(lam))
+        dt = self.L.oracle_max_dt(self.h, _p(u), cfl, C.addressof(lam))
         return (dt, lam.value) if return_lambda else dt
 
     def run(self, u, nsteps, cfl=0.5, dt=0.0, t0=0.0):
         """advance a copy of u by nsteps SSPRK3 steps; returns (u, t_end, min_rho, min_p)"""
         u = _f64(u).copy()
         mr, mp = C.c_double(0.0), C.c_double(0.0)
-        t = lib().oracle_run(self.h, _p(u), nsteps, cfl, dt, t0, C.addressof(mr), C.addressof(mp))
+        t = self.L.oracle_run(self.h, _p(u), nsteps, cfl, dt, t0, C.addressof(mr), C.addressof(mp))
         return u, t, mr.value, mp.value
 
 

@@ -268,6 +268,7 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
     for (int s = 0; s < h.ns; ++s) {
       if (!(k->W[s] > 0.0)) return fail(MARUT_EINVAL, "molar mass must be positive");
       h.W[s] = k->W[s];
+      h.Rs[s] = R_UNIVERSAL / k->W[s];
       for (int r = 0; r < 2; ++r)
         for (int c = 0; c < 7; ++c) h.nasa[s][r][c] = k->nasa[(s * 2 + r) * 7 + c];
     }

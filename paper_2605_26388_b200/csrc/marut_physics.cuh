@@ -30,7 +30,7 @@ __device__ inline double temperature_newton(const MechDev &m, const double *rho_
   double T = 4000.0;
   double rR[NSP];
 #pragma unroll
-  for (int s = 0; s < NSP; ++s) rR[s] = rho_s[s] * (R_UNIVERSAL / m.W[s]);
+  for (int s = 0; s < NSP; ++s) rR[s] = rho_s[s] * m.Rs[s];
   for (int it = 0; it < 50; ++it) {
     double f = -e_int, df = 0.0;
 #pragma unroll
@@ -78,7 +78,7 @@ __device__ inline Prim<DIM> prim_mixture(const double *U, double T, const MechDe
   double rho = 0.0, rhoR = 0.0, rhocp = 0.0;
 #pragma unroll
   for (int s = 0; s < NSP; ++s) {
-    double Rs = R_UNIVERSAL / m.W[s];
+    const double Rs = m.Rs[s];
     rho += U[s];
     rhoR += U[s] * Rs;
     if (WANT_A) rhocp += U[s] * Rs * Thermo::cp_R(Thermo::range(m, s, T), T);
