@@ -40,12 +40,27 @@ def workload_name(case):
 
 
 def algorithmic_bytes_per_dof_stage(mesh, affine=True):
-    """SURVEY 8(d) / DESIGN.md section 7: state traffic 16 B (stage 0) + 24 B + 24 B = 64/3 B per DOF-stage;
-    curved meshes add the per-node metric terms (d*d + 1 doubles per node per stage)."""
-    b = 64.0 / 3.0
-    if not affine:
-        b += 8.0 * (mesh.dim * mesh.dim + 1) / mesh.n_var
+    """state traffic 16 B (stage 0) + 24 B + 24 B = 64/3 B per DOF-stage; curved meshes add the
+    per-node metric terms (d*d + 1 doubles per node per sweep).  Navier-Stokes is the two-sweep BR1 form the
+    library implements: the gradient sweep reads u and the metrics and writes S, the stage
+    sweep reads u, S, the metrics and u_n and writes u_out."""
+    nv, d = mesh.n_var, mesh.dim
+    met = 0.0 if affine else 8.0 * (d * d + 1) / nv
+    b = 64.0 / 3.0 + met
+    if mesh.physics == 1:
+        grad = 8.0 * (d + 2) * d / nv          # S: (d+2)*d doubles per node
+        b += 8.0 + met + 2.0 * grad            # second read of u, second read of the metrics, S written + read
     return b
+
+
+def single_sweep_bytes_per_dof_stage(mesh, affine=True):
+    """the figure a one-sweep operator would need: context for the NS line"""
+    return 64.0 / 3.0 + (0.0 if affine else 8.0 * (mesh.dim * mesh.dim + 1) / mesh.n_var)
+
+
+# FP64 vector peak for the ALU-bound reacting stage (DESIGN.md section 7): 148 SMs x 64 DFMA/clk x 2 flop x max SM clock
+def fp64_peak_tflops(sm_mhz=1965.0):
+    return 148 * 64 * 2 * sm_mhz * 1e6 / 1e12
 
 
 # --------------------------------------------------------------------------------------------- clocks
@@ -280,13 +295,29 @@ def run_cuda(args):
         peak, peak_src = measured_peaks()
         b_alg = algorithmic_bytes_per_dof_stage(mesh, affine)
         achieved = b_alg * n_dof / (stage_ms_avg * 1e-3) / 1e9
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu capture
+        prof = {}
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")   # per-launch figures from the committed ncu captures
         if os.path.exists(tpath):
             try:
-                traffic = json.load(open(tpath)).get(args.workload)
+                prof = json.load(open(tpath))
             except Exception:
-                traffic = None
+                prof = {}
+        kernels = {0: "stage_node_kernel (fused Euler stage)", 1: "gradient_kernel + stage_phys_kernel (BR1 gradient sweep + fused NS stage)",
+                   2: "eos_kernel + stage_phys_kernel (mixture temperature + fused reacting stage)"}[mesh.physics]
+        roof = {"bound": "hbm", "kernel": "marut_ssprk_stage: " + kernels, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": prof.get(args.workload), "peak_source": peak_src, "bytes_per_dof_stage": b_alg,
+                "stage_ms_avg": stage_ms_avg, "frac_of_8TBs_nominal": achieved / 8000.0}
+        if mesh.physics == 1:
+            roof["single_sweep_bytes_per_dof_stage"] = single_sweep_bytes_per_dof_stage(mesh, affine)
+            roof["frac_vs_single_sweep_bytes"] = roof["single_sweep_bytes_per_dof_stage"] * n_dof / (stage_ms_avg * 1e-3) / 1e9 / peak
+        if mesh.physics == 2:
+            # ALU-bound (chemistry): executed FP64 flops per stage from the committed ncu capture over the live time
+            flops = prof.get(args.workload + "_fp64_flops_per_stage")
+            pk = fp64_peak_tflops((clocks or {}).get("sm_max_mhz") or 1965.0)
+            ach = flops / (stage_ms_avg * 1e-3) / 1e12 if flops else None
+            roof.update({"bound": "alu", "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": (ach / pk) if ach else None,
+                         "peak_source": "derived: 148 SMs x 64 FP64 FMA/clk x 2 x max SM clock (DESIGN.md section 7)",
+                         "hbm_frac": achieved / peak})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
@@ -298,11 +329,7 @@ def run_cuda(args):
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n_dof * 8, "d2h_bytes_per_step": n_dof * 8 + 8,
                         "ms_per_step": e2e_ms / args.steps},
                 "gpu_launches": launches,
-                "roofline": {"bound": "hbm", "kernel": "marut_ssprk_stage (fused stage kernel" +
-                             (" + BR1 gradient kernel" if mesh.physics == 1 else " + EOS kernel" if mesh.physics == 2 else "") + ")",
-                             "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                             "traffic": traffic, "peak_source": peak_src, "bytes_per_dof_stage": b_alg,
-                             "stage_ms_avg": stage_ms_avg, "frac_of_8TBs_nominal": achieved / 8000.0}}
+                "roofline": roof}
         if world == 1 and not args.no_cpu_baseline:
             o = oracle_sample(args.workload, args.cpu_seconds)
             line["cpu_baseline"] = {"value": o["value"], "unit": UNIT, "cores": o["cores"], "kind": "oracle", "sample": o["sample"]}
