@@ -177,6 +177,25 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# --------------------------------------------------------------------------------------------- N > 1
+def max_over_ranks(values, world, device="cpu"):
+    """element-wise MAX over the ranks of per-rank timings (the only cross-rank step of this bench: the path runs
+    as independent replicas)"""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def aggregate_value(n_dof, steps, world, ms):
+    """whole-job DOF-stage updates per second: every replica advances n_dof DOFs through 3 stages per step"""
+    return n_dof * 3 * steps * world / (ms * 1e-3)
+
+
 # --------------------------------------------------------------------------------------------- CUDA arm
 def measured_peaks():
     try:
@@ -283,13 +302,9 @@ def run_cuda(args):
     barrier()
     e2e_ms = e_start.elapsed_time(e_end)
 
-    if world > 1:
-        t = torch.tensor([ms, e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_ms = t.tolist()
-    units = n_dof * 3 * args.steps * world
-    value = units / (ms * 1e-3)
-    e2e_value = units / (e2e_ms * 1e-3)
+    ms, e2e_ms = max_over_ranks([ms, e2e_ms], world, device="cuda")
+    value = aggregate_value(n_dof, args.steps, world, ms)
+    e2e_value = aggregate_value(n_dof, args.steps, world, e2e_ms)
 
     if rank == 0:
         peak, peak_src = measured_peaks()
