@@ -295,6 +295,12 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
       const int r = order[i];
       h.A[i] = k->A[r]; h.b[i] = k->b[r]; h.Ea[i] = k->Ea[r];
       h.new_group[i] = (i == 0 || grp[order[i - 1]] != grp[r]) ? 1 : 0;
+      int nf = 0, nb = 0;
+      for (int q = 0; q < 4; ++q) h.fr[i][q] = h.br[i][q] = -1;
+      for (int s = 0; s < h.ns; ++s) {
+        for (int q = 0; q < k->nu_r[r * h.ns + s]; ++q) { if (nf >= 3) return fail(MARUT_EINVAL, "reaction order above 3"); h.fr[i][nf++] = (signed char)s; }
+        for (int q = 0; q < k->nu_p[r * h.ns + s]; ++q) { if (nb >= 3) return fail(MARUT_EINVAL, "reaction order above 3"); h.br[i][nb++] = (signed char)s; }
+      }
       for (int s = 0; s < h.ns; ++s) {
         h.nu_r[i][s] = (signed char)k->nu_r[r * h.ns + s];
         h.nu_p[i][s] = (signed char)k->nu_p[r * h.ns + s];

@@ -129,7 +129,7 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     Ust[(NVAR + 2) * TILE + tid] = pr.a;
     if constexpr (PHYS == PH_REACT) {
       double om[NSP];
-      production_rates<NSP>(*mech, T, U, om);
+      production_rates_listed<NSP>(*mech, T, U, Src + tid, TILE, om);
 #pragma unroll
       for (int s = 0; s < NSP; ++s) Src[s * TILE + tid] = om[s];
     }

@@ -253,4 +253,49 @@ __device__ inline void production_rates(const MechDev &m, double T, const double
   for (int s = 0; s < NSP; ++s) omega[s] = m.W[s] * omega[s] * 1.0e6;
 }
 
+// The same rates for the fused stage kernel: the concentrations X_s go through a per-thread shared-memory column
+// (Xs[s * stride]) so that the rate products can index the species listed per reaction (fr / br) instead of
+// looping over all species with runtime exponents.
+template <int NSP>
+__device__ inline void production_rates_listed(const MechDev &m, double T, const double *rho_s, double *Xs, int stride,
+                                               double *omega) {
+  double g[NSP];
+  const double lnT = log(T), invT = 1.0 / T;
+#pragma unroll
+  for (int s = 0; s < NSP; ++s) {
+    Xs[s * stride] = rho_s[s] / m.W[s] * 1.0e-6;
+    const double *a = Thermo::range(m, s, T);
+    g[s] = Thermo::h_RT(a, T) - Thermo::s_R(a, T, lnT);
+    omega[s] = 0.0;
+  }
+  const double lnc0 = log(P_REF / (R_UNIVERSAL * T) * 1.0e-6);
+  double ikc = 1.0;
+  for (int r = 0; r < m.nr; ++r) {
+    if (m.new_group[r]) {
+      double dG = 0.0;
+      int dnu = 0;
+#pragma unroll
+      for (int s = 0; s < NSP; ++s) {
+        const int d = m.nu_p[r][s] - m.nu_r[r][s];
+        dG += d * g[s];
+        dnu += d;
+      }
+      ikc = exp(dG - dnu * lnc0);
+    }
+    double pf = 1.0, pb = 1.0;
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+      const int a = m.fr[r][q], b = m.br[r][q];
+      if (a >= 0) pf *= Xs[a * stride];
+      if (b >= 0) pb *= Xs[b * stride];
+    }
+    const double kf = m.A[r] * exp(m.b[r] * lnT - m.Ea[r] * invT);
+    const double Rr = kf * (pf - ikc * pb);
+#pragma unroll
+    for (int s = 0; s < NSP; ++s) omega[s] += (double)(m.nu_p[r][s] - m.nu_r[r][s]) * Rr;
+  }
+#pragma unroll
+  for (int s = 0; s < NSP; ++s) omega[s] = m.W[s] * omega[s] * 1.0e6;
+}
+
 }  // namespace marut
