@@ -50,6 +50,8 @@ struct NodeCfg {
   static constexpr int NT = ((TILE + 31) / 32) * 32;
   static constexpr int NW = NT / 32;
   static constexpr int NST = NVAR + 3;              // stash planes: U, 1/rho, p, a
+  // plane of (variable, element) inside one direction's plane set: variable-major in 3-D, element-major in 2-D
+  __host__ __device__ static constexpr int plane(int v, int el) { return (DIM == 2) ? el * NVAR + v : v * EB + el; }
   static constexpr int KS = L::KS, PS = L::PS;
   static constexpr int NPL = DIM * NVAR * EB;       // flux planes
   static constexpr int NVT = EB * NVAR * NP;        // plane tasks per derivative pass (3-D)
@@ -315,7 +317,7 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
         double F[NVAR];
         flux_dot<DIM, 1>(U, pr, &Ja[l * DIM], F);
 #pragma unroll
-        for (int v = 0; v < NVAR; ++v) Fsm[((l * NVAR + v) * EB + el) * PS + sp] = F[v];
+        for (int v = 0; v < NVAR; ++v) Fsm[(l * NVAR * EB + C::plane(v, el)) * PS + sp] = F[v];
       }
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) Ust[v * TILE + tid] = U[v];
@@ -330,11 +332,22 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   __syncthreads();
 
   // ---- xi pass (eq. 9): lines (j,k) of variable v; lanes run over the lines first
-  for (int t = tid; t < nline; t += NT) {
-    const int el = t / NLT, r = t - el * NLT;
-    const int v = r / NL, ln = r - v * NL;
-    const int lj = ln % NP, lk = ln / NP;
-    double *px = Fsm + (v * EB + el) * PS + NP * lj + KS * lk;
+  for (int t = tid; t < EB * NLT; t += NT) {
+    int el, v, lj, lk = 0;
+    if constexpr (DIM == 3) {
+      el = t / NLT;
+      const int r = t - el * NLT;
+      v = r / NL;
+      const int ln = r - v * NL;
+      lj = ln % NP;
+      lk = ln / NP;
+    } else {   // 2-D lane order (v, element, j): bank-conflict-free with element-major planes
+      v = t % NVAR;
+      el = (t / NVAR) % EB;
+      lj = t / (NVAR * EB);
+    }
+    if (el >= nel) continue;
+    double *px = Fsm + C::plane(v, el) * PS + NP * lj + KS * lk;
     double f[NP], acc[NP];
 #pragma unroll
     for (int m = 0; m < NP; ++m) { f[m] = px[m]; acc[m] = 0.0; }
@@ -353,7 +366,7 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
       const int el = t / NLT, r = t - el * NLT;
       const int lk = r % NP, r2 = r / NP;
       const int v = r2 % NVAR, li = r2 / NVAR;
-      double *px = Fsm + (v * EB + el) * PS + li + KS * lk;
+      double *px = Fsm + C::plane(v, el) * PS + li + KS * lk;
       const double *pe = px + NVAR * EB * PS;
       double f[NP], acc[NP];
 #pragma unroll
@@ -375,13 +388,23 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
 
   // ---- last pass (zeta in 3-D, eta in 2-D) fused with phase D: lifts, 1/J, SSP-RK combination (eq. 12, 45)
   const bool use_un = (P.ca != 0.0);
-  for (int t = tid; t < nline; t += NT) {
-    const int el = t / NLT, r = t - el * NLT;
-    const int v = r / NL, ij = r - v * NL;       // 3-D: ij = i + NP*j ; 2-D: ij = i
+  for (int t = tid; t < EB * NLT; t += NT) {
+    int el, v, ij;                               // 3-D: ij = i + NP*j ; 2-D: ij = i
+    if constexpr (DIM == 3) {
+      el = t / NLT;
+      const int r = t - el * NLT;
+      v = r / NL;
+      ij = r - v * NL;
+    } else {   // 2-D lane order (i, element, v)
+      ij = t % NP;
+      el = (t / NP) % EB;
+      v = t / (NP * EB);
+    }
+    if (el >= nel) continue;
     constexpr int LS = (DIM == 3) ? KS : NP;      // stride of the line in the flux plane
     constexpr int GS = (DIM == 3) ? NP * NP : NP; // stride of the line in global memory
     const long e = e0 + el;
-    const double *px = Fsm + (v * EB + el) * PS + ij;
+    const double *px = Fsm + C::plane(v, el) * PS + ij;
     const double *pl = px + (DIM - 1) * NVAR * EB * PS;
     const long gofs = (e * NVAR + v) * NN + ij;
     double un[NP];
