@@ -48,8 +48,8 @@ def algorithmic_bytes_per_dof_stage(mesh, affine=True):
     met = 0.0 if affine else 8.0 * (d * d + 1) / nv
     b = 64.0 / 3.0 + met
     if mesh.physics == 1:
-        grad = 8.0 * (d + 2) * d / nv          # S: (d+2)*d doubles per node
-        b += 8.0 + met + 2.0 * grad            # second read of u, second read of the metrics, S written + read
+        grad = 8.0 * (d * (d + 1) // 2 + d) / nv   # stress tensor + heat flux from the BR1 gradient: d(d+1)/2 + d doubles per node
+        b += 8.0 + met + 2.0 * grad            # second read of u, second read of the metrics, viscous tensor written + read
     return b
 
 

@@ -48,7 +48,7 @@ struct marut_mesh {
   int *d_mortar_fine = nullptr;
   double *d_mortar_mat = nullptr;
   double *d_bc = nullptr;
-  double *d_S = nullptr;     // NS gradient scratch
+  double *d_S = nullptr;     // NS scratch: stress tensor + heat flux from the BR1 gradient, [e][d(d+1)/2 + d][node]
   double *d_T = nullptr;     // reacting temperature scratch
   MechDev *d_mech = nullptr;
   unsigned long long *d_red = nullptr;
@@ -426,7 +426,7 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   cleanup();
 
   // ---- scratch
-  if (m->physics == MARUT_NAVIER_STOKES) CUDA_TRY(cudaMalloc(&m->d_S, (size_t)ne * (dim + 2) * dim * nn * sizeof(double)));
+  if (m->physics == MARUT_NAVIER_STOKES) CUDA_TRY(cudaMalloc(&m->d_S, (size_t)ne * (dim * (dim + 1) / 2 + dim) * nn * sizeof(double)));
   if (m->physics == MARUT_REACTING_EULER) CUDA_TRY(cudaMalloc(&m->d_T, (size_t)ne * nn * sizeof(double)));
 
   const char *sel = getenv("MARUT_KERNEL");   // A/B switch for profiling: node (default) | line | generic
@@ -465,7 +465,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   if (m->physics == MARUT_NAVIER_STOKES) {
     GradParams G;
     G.u = u_in; G.S = m->d_S; G.metric = m->d_metric; G.conn = m->d_conn;
-    G.gamma = m->gamma; G.inv_wb = 1.0 / m->w[0]; G.ne = m->ne;
+    G.gamma = m->gamma; G.inv_wb = 1.0 / m->w[0]; G.mu = m->mu; G.kappa = m->kappa; G.ne = m->ne;
     memcpy(G.D, m->D, sizeof(G.D));
     cudaError_t e = launch_gradient(m->dim, m->np, m->affine, G, st);
     if (e != cudaSuccess) return fail(e == cudaErrorNotSupported ? MARUT_EINVAL : MARUT_ECUDA, "gradient kernel: %s", cudaGetErrorString(e));

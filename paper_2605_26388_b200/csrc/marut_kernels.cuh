@@ -110,7 +110,7 @@ stage_kernel(const __grid_constant__ StageParams P) {
     pr = make_prim<DIM, NSP, PHYS, true>(U, T, P.gamma, mech);
     if constexpr (PHYS == PH_NS) {
 #pragma unroll
-      for (int k = 0; k < NW * DIM; ++k) Sg[k] = __ldg(&P.S[(e * NW * DIM + k) * NN + p]);
+      for (int k = 0; k < Tau<DIM>::NTAU; ++k) Sg[k] = __ldg(&P.S[(e * Tau<DIM>::NTAU + k) * NN + p]);
     }
     // contravariant fluxes Ftilde^l = Ja^l . (F_inv - F_v)   (eq. 9)
 #pragma unroll
@@ -119,7 +119,7 @@ stage_kernel(const __grid_constant__ StageParams P) {
       flux_dot<DIM, NSP>(U, pr, &Ja[l * DIM], F);
       if constexpr (PHYS == PH_NS) {
         double Fv[NW];
-        viscous_flux_dot<DIM>(pr.v, Sg, &Ja[l * DIM], P.mu, P.kappa, Fv);
+        viscous_flux_dot_tau<DIM>(pr.v, Sg, &Ja[l * DIM], Fv);
 #pragma unroll
         for (int v = 0; v < NVAR; ++v) F[v] -= Fv[v];
       }
@@ -187,9 +187,9 @@ stage_kernel(const __grid_constant__ StageParams P) {
         // BR1 viscous interface flux: mean of the two sides (eq. 16)
         double Sp[NW * DIM], Fvm[NW], Fvp[NW];
 #pragma unroll
-        for (int k = 0; k < NW * DIM; ++k) Sp[k] = __ldg(&P.S[((long)cn.x * NW * DIM + k) * NN + pR]);
-        viscous_flux_dot<DIM>(pr.v, Sg, nv, P.mu, P.kappa, Fvm);
-        viscous_flux_dot<DIM>(qp.v, Sp, nv, P.mu, P.kappa, Fvp);
+        for (int k = 0; k < Tau<DIM>::NTAU; ++k) Sp[k] = __ldg(&P.S[((long)cn.x * Tau<DIM>::NTAU + k) * NN + pR]);
+        viscous_flux_dot_tau<DIM>(pr.v, Sg, nv, Fvm);
+        viscous_flux_dot_tau<DIM>(qp.v, Sp, nv, Fvp);
 #pragma unroll
         for (int v = 0; v < NVAR; ++v) Fs[v] -= 0.5 * (Fvm[v] + Fvp[v]);
       }
@@ -278,7 +278,7 @@ struct GradParams {
   double *__restrict__ S;
   const double *__restrict__ metric;
   const int2 *__restrict__ conn;
-  double gamma, inv_wb;
+  double gamma, inv_wb, mu, kappa;
   long ne;
   double D[MAX_NP * MAX_NP];
 };
@@ -361,7 +361,13 @@ gradient_kernel(const __grid_constant__ GradParams P) {
   }
   const double invJ = metric_at<DIM, NP, AFFINE>(P.metric, e, DIM * DIM, p);
 #pragma unroll
-  for (int k = 0; k < NW * DIM; ++k) P.S[(e * NW * DIM + k) * NN + p] = invJ * Sg[k];
+  for (int k = 0; k < NW * DIM; ++k) Sg[k] = invJ * Sg[k];
+  // stored in the compact form the viscous flux needs: stress tensor + heat flux (Tau<DIM>)
+  constexpr int NTAU = Tau<DIM>::NTAU;
+  double tau[NTAU];
+  gradient_to_tau<DIM>(Sg, P.mu, P.kappa, tau);
+#pragma unroll
+  for (int k = 0; k < NTAU; ++k) P.S[(e * NTAU + k) * NN + p] = tau[k];
 }
 
 // ======================================================================================

@@ -107,7 +107,7 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     double Sg[(PHYS == PH_NS) ? NW * DIM : 1];
     if constexpr (PHYS == PH_NS) {
 #pragma unroll
-      for (int k = 0; k < NW * DIM; ++k) Sg[k] = __ldg(&P.S[(e * NW * DIM + k) * NN + p]);
+      for (int k = 0; k < Tau<DIM>::NTAU; ++k) Sg[k] = __ldg(&P.S[(e * Tau<DIM>::NTAU + k) * NN + p]);
     }
 #pragma unroll
     for (int l = 0; l < DIM; ++l) {
@@ -115,7 +115,7 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       flux_dot<DIM, NSP>(U, pr, &Ja[l * DIM], F);
       if constexpr (PHYS == PH_NS) {
         double Fv[NW];
-        viscous_flux_dot<DIM>(pr.v, Sg, &Ja[l * DIM], P.mu, P.kappa, Fv);
+        viscous_flux_dot_tau<DIM>(pr.v, Sg, &Ja[l * DIM], Fv);
 #pragma unroll
         for (int v = 0; v < NVAR; ++v) F[v] -= Fv[v];
       }
@@ -220,8 +220,8 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       // viscous part: F_v* = mean of the two sides; own F_v.n = F_inv(U-).n - (own total normal flux in the plane)
       double Sp[NW * DIM], Fvp[NW];
 #pragma unroll
-      for (int k = 0; k < NW * DIM; ++k) Sp[k] = __ldg(&P.S[((long)cn.x * NW * DIM + k) * NN + pR]);
-      viscous_flux_dot<DIM>(qp.v, Sp, nv, P.mu, P.kappa, Fvp);
+      for (int k = 0; k < Tau<DIM>::NTAU; ++k) Sp[k] = __ldg(&P.S[((long)cn.x * Tau<DIM>::NTAU + k) * NN + pR]);
+      viscous_flux_dot_tau<DIM>(qp.v, Sp, nv, Fvp);
       const int qk = (DIM == 3) ? t.p / (NP * NP) : 0;
       const int sp = t.p + (KS - NP * NP) * qk;
 #pragma unroll

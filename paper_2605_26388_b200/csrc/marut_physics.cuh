@@ -210,6 +210,53 @@ __device__ __forceinline__ void viscous_flux_dot(const double *vel, const double
   F[1 + DIM] = Fe;
 }
 
+// Compact form of the BR1 gradient for the viscous flux (eq. 15): the symmetric stress tensor and
+// the heat-flux vector, NTAU = d(d+1)/2 + d doubles per node instead of the (d+2) d gradient components.
+//   tau[0..d)      = tau_ii = mu (2 S_ii - 2/3 div u)
+//   tau[d..d(d+1)/2) = tau_ij (i<j) = mu (S_ij + S_ji)   order: 2-D xy ; 3-D xy, xz, yz
+//   tau[last d]    = kappa dT/dx_j
+// Same expressions, in the same order, as viscous_flux_dot: the two forms give identical results.
+template <int DIM>
+struct Tau {
+  static constexpr int NTAU = DIM * (DIM + 1) / 2 + DIM;
+  __host__ __device__ static constexpr int off(int i, int j) {   // i < j
+    return (DIM == 2) ? 2 : ((i == 0) ? ((j == 1) ? 3 : 4) : 5);
+  }
+};
+template <int DIM>
+__device__ __forceinline__ void gradient_to_tau(const double *S, double mu, double kappa, double *tau) {
+  double divu = 0.0;
+#pragma unroll
+  for (int i = 0; i < DIM; ++i) divu += S[(1 + i) * DIM + i];
+#pragma unroll
+  for (int i = 0; i < DIM; ++i) {
+    tau[i] = mu * (2.0 * S[(1 + i) * DIM + i] - (2.0 / 3.0) * divu);
+#pragma unroll
+    for (int j = i + 1; j < DIM; ++j) tau[Tau<DIM>::off(i, j)] = mu * (S[(1 + i) * DIM + j] + S[(1 + j) * DIM + i]);
+  }
+#pragma unroll
+  for (int j = 0; j < DIM; ++j) tau[DIM * (DIM + 1) / 2 + j] = kappa * S[(1 + DIM) * DIM + j];
+}
+template <int DIM>
+__device__ __forceinline__ void viscous_flux_dot_tau(const double *vel, const double *tau, const double *nv, double *F) {
+  double Fe = 0.0;
+  F[0] = 0.0;
+#pragma unroll
+  for (int i = 0; i < DIM; ++i) {
+    double ti = 0.0;
+#pragma unroll
+    for (int j = 0; j < DIM; ++j) {
+      const double t = (i == j) ? tau[i] : tau[Tau<DIM>::off(i < j ? i : j, i < j ? j : i)];
+      ti += t * nv[j];
+    }
+    F[1 + i] = ti;
+    Fe += vel[i] * ti;
+  }
+#pragma unroll
+  for (int j = 0; j < DIM; ++j) Fe += tau[DIM * (DIM + 1) / 2 + j] * nv[j];
+  F[1 + DIM] = Fe;
+}
+
 // ---------------------------------------------------------------- chemistry (eq. 21-22)
 // omega_s [kg m^-3 s^-1] from T and partial densities; concentrations in mol/cm^3 inside the rate law,
 // K_c = exp(-sum dnu g_s/(R_u T)) (p_ref/(R_u T) 1e-6)^(sum dnu)  (R12)
