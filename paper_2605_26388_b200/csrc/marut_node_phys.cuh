@@ -11,6 +11,10 @@
 #pragma once
 #include "marut_node.cuh"
 
+#ifndef MARUT_PHYS_MINB128
+#define MARUT_PHYS_MINB128 5
+#endif
+
 namespace marut {
 
 template <int DIM, int NP, int NSP, int PHYS, int EB>
@@ -318,7 +322,7 @@ cudaError_t launch_stage_phys_t(const StageParams &P, cudaStream_t st) {
   constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
   using C = PhysCfg<DIM, NP, NSP, PHYS, EB>;
   constexpr size_t smem = C::smem_doubles(AFFINE) * sizeof(double);
-  constexpr int MINB = (PHYS == PH_REACT) ? ((C::NT <= 128) ? 3 : 1) : ((C::NT <= 128) ? 4 : ((C::NT <= 256) ? 2 : 1));
+  constexpr int MINB = (PHYS == PH_REACT) ? ((C::NT <= 128) ? 3 : 1) : ((C::NT <= 128) ? MARUT_PHYS_MINB128 : ((C::NT <= 256) ? 2 : 1));
   auto k = stage_phys_kernel<DIM, NP, NSP, PHYS, AFFINE, EB, MINB>;
   static bool attr = false;
   if (!attr) {
