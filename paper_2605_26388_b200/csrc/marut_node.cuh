@@ -288,9 +288,9 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   if (has0) cn0 = __ldg(&P.conn[(e0 + t0.el) * 2 * DIM + t0.f]);
 
   if constexpr (AFFINE) {
-    if (tid < nel * MDP) {
-      const int el = tid / MDP, k = tid - el * MDP;
-      Msm[tid] = (k < MD) ? __ldg(&P.metric[(e0 + el) * MD + k]) : ((k < MD + DIM) ? __ldg(&P.fnorm[(e0 + el) * DIM + (k - MD)]) : 0.0);
+    for (int i = tid; i < nel * MDP; i += NT) {
+      const int el = i / MDP, k = i - el * MDP;
+      Msm[i] = (k < MD) ? __ldg(&P.metric[(e0 + el) * MD + k]) : ((k < MD + DIM) ? __ldg(&P.fnorm[(e0 + el) * DIM + (k - MD)]) : 0.0);
     }
   }
 

@@ -70,9 +70,9 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     for (int i = tid; i < (int)(sizeof(MechDev) / sizeof(int)); i += NT) dst[i] = src[i];
   }
   if constexpr (AFFINE) {
-    if (tid < nel * MDP) {
-      const int me = tid / MDP, k = tid - me * MDP;
-      Msm[tid] = (k < MD) ? __ldg(&P.metric[(e0 + me) * MD + k]) : ((k < MD + DIM) ? __ldg(&P.fnorm[(e0 + me) * DIM + (k - MD)]) : 0.0);
+    for (int i = tid; i < nel * MDP; i += NT) {
+      const int me = i / MDP, k = i - me * MDP;
+      Msm[i] = (k < MD) ? __ldg(&P.metric[(e0 + me) * MD + k]) : ((k < MD + DIM) ? __ldg(&P.fnorm[(e0 + me) * DIM + (k - MD)]) : 0.0);
     }
   }
   const int el = tid / NN, p = tid - el * NN;

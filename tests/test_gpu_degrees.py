@@ -1,0 +1,58 @@
+"""GPU parity for polynomial degrees and mesh kinds beyond the five configs: every kernel instantiation the library
+dispatches (2-D / 3-D, N = 1..7, affine / curved, Euler / Navier-Stokes / reacting) against the oracle on one
+marut_rhs and one marut_ssprk_stage, on small periodic meshes with a ragged last CTA."""
+import math
+
+import numpy as np
+import pytest
+
+import workloads as wl
+from parity_util import RHS_TOL, parity_error
+
+pytestmark = pytest.mark.gpu
+
+
+def _mesh(dim, N, cells, curved):
+    lo, hi = (0.0,) * dim, ((10.0,) * 2 if dim == 2 else (2 * math.pi,) * 3)
+    counts = (cells,) * dim
+    warp = wl.sine_warp(counts, lo, hi, k=1) if curved else None
+    return wl.cartesian_mesh(dim, N, counts, lo, hi, warp=warp)
+
+
+CASES = [(2, N, 5, curved, "euler") for N in (1, 2, 3, 4, 5, 7) for curved in (False, True)] + \
+        [(3, N, 3, curved, "euler") for N in (1, 2, 3, 4, 5, 6) for curved in (False, True)] + \
+        [(3, 2, 3, True, "ns"), (3, 4, 3, False, "ns"), (2, 3, 5, True, "ns"), (3, 2, 3, False, "react"), (3, 4, 3, False, "react")]
+
+
+@pytest.mark.parametrize("dim,N,cells,curved,phys", CASES)
+def test_rhs_and_stage(dim, N, cells, curved, phys):
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    m = _mesh(dim, N, cells, curved and phys != "react")
+    if phys == "react":
+        L = wl.C5_LENGTH * cells / 32.0
+        m = wl.cartesian_mesh(3, N, (cells,) * 3, (0.0,) * 3, (L,) * 3)
+        m.physics, m.mech = wl.REACTING_EULER, wl.air5_mechanism()
+        u0 = wl.reacting_field(m, L)
+    else:
+        if phys == "ns":
+            m.physics, m.mu, m.Pr = wl.NAVIER_STOKES, 1.0 / 100.0, 0.72
+        u0 = wl.isentropic_vortex(m) if dim == 2 else wl.taylor_green(m, noise=1e-3)
+    om, gm = oracle.OracleMesh(m), mb.MarutMesh(m)
+    assert gm.is_affine == (not (curved and phys != "react"))
+    u = torch.from_numpy(u0).cuda()
+    du = torch.empty_like(u)
+    gm.rhs(u, du)
+    torch.cuda.synchronize()
+    assert parity_error(du.cpu().numpy(), om.rhs(u0)).max() <= RHS_TOL
+    dt = om.max_dt(u0, 0.5)
+    assert abs(gm.max_dt(u, 0.5) - dt) <= 1e-13 * dt
+    un_h = u0 * (1.0 + 1e-3)
+    out = torch.empty_like(u)
+    gm.stage(2, dt, 0.0, torch.from_numpy(un_h).cuda(), u, out)
+    torch.cuda.synchronize()
+    assert parity_error(out.cpu().numpy(), om.ssprk_stage(2, dt, 0.0, un_h, u0)).max() <= RHS_TOL
+    gm.close()
