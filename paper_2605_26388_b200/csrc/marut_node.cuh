@@ -47,6 +47,7 @@ struct NodeCfg {
   static constexpr int TILE = EB * NN;
   static constexpr int NFN = 2 * DIM * NF;          // face nodes per element
   static constexpr int NTASK = EB * NFN;            // face tasks per CTA
+  static constexpr int LFS = (DIM == 3 && NP == 5 && EB == 1) ? 160 : NTASK;   // stride of a variable in the lift buffer
   static constexpr int NT = ((TILE + 31) / 32) * 32;
   static constexpr int NW = NT / 32;
   static constexpr int NST = NVAR + 3;              // stash planes: U, 1/rho, p, a
@@ -57,7 +58,7 @@ struct NodeCfg {
   static constexpr int NVT = EB * NVAR * NP;        // plane tasks per derivative pass (3-D)
   static constexpr int MDP = ((G::MD + DIM + 1) / 2) * 2;   // per-element affine metric slot (Ja, 1/J, |Ja^l|)
   static constexpr size_t smem_doubles(bool affine) {
-    return (size_t)NPL * PS + (size_t)NST * TILE + (size_t)NVAR * NTASK + (affine ? EB * MDP : 0);
+    return (size_t)NPL * PS + (size_t)NST * TILE + (size_t)NVAR * LFS + (affine ? EB * MDP : 0);
   }
 };
 
@@ -239,7 +240,7 @@ __device__ __forceinline__ void euler_face_task(const StageParams &P, const doub
     }
   }
 #pragma unroll
-  for (int v = 0; v < NVAR; ++v) Lft[v * NTASK + g] = lift[v];
+  for (int v = 0; v < NVAR; ++v) Lft[v * C::LFS + g] = lift[v];
 }
 
 // ---------------------------------------------------------------- derivative passes (line tasks)
@@ -257,6 +258,31 @@ __device__ __forceinline__ void line_deriv(const StageParams &P, const double *f
   }
 }
 
+#ifndef MARUT_PREFETCH_UN
+#define MARUT_PREFETCH_UN 0
+#endif
+// last-pass task t -> (element in tile, variable, line): 3-D: ij = i + NP*j, lanes run over ij first;
+// 2-D: ij = i, lane order (i, element, v)
+template <int DIM, int NP, int NVAR, int EB>
+__device__ __forceinline__ void last_pass_task(int t, int &el, int &v, int &ij) {
+  constexpr int NL = (DIM == 3) ? NP * NP : NP, NLT = NVAR * NL;
+  if constexpr (DIM == 3) {
+    el = t / NLT;
+    const int r = t - el * NLT;
+    v = r / NL;
+    ij = r - v * NL;
+  } else {
+    ij = t % NP;
+    el = (t / NP) % EB;
+    v = t / (NP * EB);
+  }
+}
+#ifndef MARUT_EARLY_GATHER
+#define MARUT_EARLY_GATHER 0
+#endif
+#ifndef MARUT_ABLATE
+#define MARUT_ABLATE 0
+#endif
 #ifndef MARUT_NODE_MINB128
 #define MARUT_NODE_MINB128 6
 #endif
@@ -274,7 +300,7 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   double *Fsm = smem;                       // [DIM][NVAR][EB] planes of PS doubles: contravariant fluxes
   double *Ust = Fsm + C::NPL * PS;          // [NVAR + 3][TILE]  U, 1/rho, p, a
   double *Lft = Ust + C::NST * TILE;        // [NVAR][NTASK]     lifts of the face nodes
-  double *Msm = Lft + NVAR * NTASK;         // affine: [EB][MDP] Ja, 1/J, |Ja^l|
+  double *Msm = Lft + NVAR * C::LFS;         // affine: [EB][MDP] Ja, 1/J, |Ja^l|
 
   const int tid = threadIdx.x;
   const long e0 = (long)blockIdx.x * EB;
@@ -294,6 +320,21 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
     }
   }
 
+  // u_n of the degrees of freedom this thread finishes in the last pass: loaded now, so that the CTA has its
+  // whole DRAM read in flight from the start (u_out may alias u_n: only this thread writes these locations, later)
+  const bool use_un = (P.ca != 0.0);
+  double un0[NP];
+  {
+    int el, v, ij;
+    last_pass_task<DIM, NP, NVAR, EB>(tid, el, v, ij);
+    if (MARUT_PREFETCH_UN && use_un && tid < EB * NLT && el < nel) {
+      const long gofs = ((e0 + el) * NVAR + v) * NN + ij;
+#pragma unroll
+      for (int m = 0; m < NP; ++m) un0[m] = P.u_n[gofs + m * ((DIM == 3) ? NP * NP : NP)];
+    }
+  }
+  // neighbour trace of the first face task: issued in phase N, consumed after the xi pass
+  double Up0[NVAR];
   // ---- phase N: own node
   {
     const int el = tid / NN, p = tid - el * NN;
@@ -305,17 +346,28 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
     }
+#if MARUT_EARLY_GATHER
+    if (has0) gather_exterior<DIM, NP, NVAR>(P, t0, cn0, Up0);
+#endif
     if (active) {
       const int qk = (DIM == 3) ? p / (NP * NP) : 0;
       const int sp = p + (KS - NP * NP) * qk;   // node offset inside a flux plane
       double Ja[DIM * DIM];
 #pragma unroll
       for (int k = 0; k < DIM * DIM; ++k) Ja[k] = metric_at<DIM, NP, AFFINE>(P.metric, e, k, p);
+#if MARUT_ABLATE == 3
+      Prim<DIM> pr; pr.irho = U[0]; pr.p = U[1]; pr.a = U[2];
+#else
       const Prim<DIM> pr = prim_ideal<DIM, true>(U, P.gamma);
+#endif
 #pragma unroll
       for (int l = 0; l < DIM; ++l) {
         double F[NVAR];
+#if MARUT_ABLATE == 3
+        for (int v = 0; v < NVAR; ++v) F[v] = U[v] * Ja[l * DIM];
+#else
         flux_dot<DIM, 1>(U, pr, &Ja[l * DIM], F);
+#endif
 #pragma unroll
         for (int v = 0; v < NVAR; ++v) Fsm[(l * NVAR * EB + C::plane(v, el)) * PS + sp] = F[v];
       }
@@ -326,12 +378,15 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
       Ust[(NVAR + 2) * TILE + tid] = pr.a;
     }
   }
-  // neighbour trace of the first face task: in flight during the xi pass
-  double Up0[NVAR];
+#if !MARUT_EARLY_GATHER
   if (has0) gather_exterior<DIM, NP, NVAR>(P, t0, cn0, Up0);
+#endif
   __syncthreads();
 
   // ---- xi pass (eq. 9): lines (j,k) of variable v; lanes run over the lines first
+#if MARUT_ABLATE == 2 || MARUT_ABLATE == 3
+  if (false)
+#endif
   for (int t = tid; t < EB * NLT; t += NT) {
     int el, v, lj, lk = 0;
     if constexpr (DIM == 3) {
@@ -357,11 +412,18 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   }
 
   // ---- face phase, first round: face nodes densely mapped
+#if MARUT_ABLATE != 1 && MARUT_ABLATE != 3
   if (has0) euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
+#else
+  if (has0 && Up0[0] == 1.2345) Lft[tid] = Up0[1];
+#endif
   __syncthreads();
 
   if constexpr (DIM == 3) {
     // ---- eta pass: lines (i,k) of variable v; lane order (k, v, i) is bank-conflict-free
+#if MARUT_ABLATE == 2 || MARUT_ABLATE == 3
+    if (false)
+#endif
     for (int t = tid; t < nline; t += NT) {
       const int el = t / NLT, r = t - el * NLT;
       const int lk = r % NP, r2 = r / NP;
@@ -377,6 +439,9 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
     }
   }
   // ---- face phase, remaining rounds
+#if MARUT_ABLATE == 1 || MARUT_ABLATE == 3
+  if (false)
+#endif
   for (int g = tid + NT; g < ntask; g += NT) {
     const FaceTask t = decode_task<DIM, NP>(g);
     const int2 cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
@@ -387,19 +452,9 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   if constexpr (DIM == 3 || (NTASK > NT)) __syncthreads();
 
   // ---- last pass (zeta in 3-D, eta in 2-D) fused with phase D: lifts, 1/J, SSP-RK combination (eq. 12, 45)
-  const bool use_un = (P.ca != 0.0);
   for (int t = tid; t < EB * NLT; t += NT) {
     int el, v, ij;                               // 3-D: ij = i + NP*j ; 2-D: ij = i
-    if constexpr (DIM == 3) {
-      el = t / NLT;
-      const int r = t - el * NLT;
-      v = r / NL;
-      ij = r - v * NL;
-    } else {   // 2-D lane order (i, element, v)
-      ij = t % NP;
-      el = (t / NP) % EB;
-      v = t / (NP * EB);
-    }
+    last_pass_task<DIM, NP, NVAR, EB>(t, el, v, ij);
     if (el >= nel) continue;
     constexpr int LS = (DIM == 3) ? KS : NP;      // stride of the line in the flux plane
     constexpr int GS = (DIM == 3) ? NP * NP : NP; // stride of the line in global memory
@@ -409,15 +464,20 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
     const long gofs = (e * NVAR + v) * NN + ij;
     double un[NP];
     if (use_un) {
+      if (MARUT_PREFETCH_UN && t == tid) {
 #pragma unroll
-      for (int m = 0; m < NP; ++m) un[m] = P.u_n[gofs + m * GS];
+        for (int m = 0; m < NP; ++m) un[m] = un0[m];
+      } else {
+#pragma unroll
+        for (int m = 0; m < NP; ++m) un[m] = P.u_n[gofs + m * GS];
+      }
     }
     double f[NP], acc[NP];
 #pragma unroll
     for (int m = 0; m < NP; ++m) { f[m] = pl[m * LS]; acc[m] = px[m * LS]; }
     line_deriv<NP>(P, f, acc);
     // lifts of the faces the nodes of this line lie on
-    const double *lf = Lft + v * NTASK + el * NFN;
+    const double *lf = Lft + v * C::LFS + el * NFN;
     if constexpr (DIM == 3) {
       const int qi = ij % NP, qj = ij / NP;
       acc[0] += lf[4 * NF + ij];
