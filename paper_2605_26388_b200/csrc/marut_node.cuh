@@ -258,19 +258,30 @@ __device__ __forceinline__ void line_deriv(const StageParams &P, const double *f
   }
 }
 
+#ifndef MARUT_L2_PREFETCH
+#define MARUT_L2_PREFETCH 1024   // elements-per-CTA units ahead; 0 = off
+#endif
 #ifndef MARUT_PREFETCH_UN
 #define MARUT_PREFETCH_UN 0
 #endif
 // last-pass task t -> (element in tile, variable, line): 3-D: ij = i + NP*j, lanes run over ij first;
 // 2-D: ij = i, lane order (i, element, v)
+template <int DIM, int NP>
+struct LastPass {
+  static constexpr int NL = (DIM == 3) ? NP * NP : NP;
+  // 3-D, NP = 5: one warp per (element, variable) with 25 of 32 lanes active -- no warp straddles two variable
+  // planes, so the shared-memory line reads are conflict-free and every global access is one 200-byte run
+  static constexpr int SLOT = NL;   // (a 32-lane slot per plane for NP = 5 removes the bank conflicts but costs a second round: slower)
+};
 template <int DIM, int NP, int NVAR, int EB>
 __device__ __forceinline__ void last_pass_task(int t, int &el, int &v, int &ij) {
-  constexpr int NL = (DIM == 3) ? NP * NP : NP, NLT = NVAR * NL;
+  constexpr int NL = LastPass<DIM, NP>::NL, SLOT = LastPass<DIM, NP>::SLOT;
   if constexpr (DIM == 3) {
-    el = t / NLT;
-    const int r = t - el * NLT;
-    v = r / NL;
-    ij = r - v * NL;
+    const int w = t / SLOT;
+    ij = t - w * SLOT;
+    el = w / NVAR;
+    v = w - el * NVAR;
+    if (ij >= NL) el = EB;   // padding lane
   } else {
     ij = t % NP;
     el = (t / NP) % EB;
@@ -307,6 +318,26 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   const int nel = (int)((P.ne - e0 < EB) ? (P.ne - e0) : EB);
   const int ntask = nel * NFN, nline = nel * NLT;
 
+#if MARUT_L2_PREFETCH
+  // L2 prefetch of the tile a CTA launched ~one wave later will read (u_in and u_n): turns its DRAM latency into an
+  // L2 hit.  Bulk prefetch needs 16-byte alignment and size: round outwards, stay inside the array.
+  if (tid == 0) {
+    const long ep = e0 + (long)MARUT_L2_PREFETCH * EB;
+    if (ep + EB < P.ne) {
+      const size_t bytes = (size_t)EB * NVAR * NN * sizeof(double);
+      const char *a = reinterpret_cast<const char *>(P.u_in + ep * NVAR * NN);
+      const char *al = reinterpret_cast<const char *>(reinterpret_cast<uintptr_t>(a) & ~(uintptr_t)15);
+      const unsigned sz = (unsigned)(((a + bytes) - al + 15) & ~(size_t)15);
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(al), "r"(sz) : "memory");
+      if (P.ca != 0.0) {
+        const char *b = reinterpret_cast<const char *>(P.u_n + ep * NVAR * NN);
+        const char *bl = reinterpret_cast<const char *>(reinterpret_cast<uintptr_t>(b) & ~(uintptr_t)15);
+        const unsigned sb = (unsigned)(((b + bytes) - bl + 15) & ~(size_t)15);
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(bl), "r"(sb) : "memory");
+      }
+    }
+  }
+#endif
   // first face task of this thread: connectivity load issued first (the neighbour gather depends on it)
   const bool has0 = tid < ntask;
   const FaceTask t0 = decode_task<DIM, NP>(has0 ? tid : 0);
@@ -327,7 +358,7 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   {
     int el, v, ij;
     last_pass_task<DIM, NP, NVAR, EB>(tid, el, v, ij);
-    if (MARUT_PREFETCH_UN && use_un && tid < EB * NLT && el < nel) {
+    if (MARUT_PREFETCH_UN && use_un && el < nel && v < NVAR) {
       const long gofs = ((e0 + el) * NVAR + v) * NN + ij;
 #pragma unroll
       for (int m = 0; m < NP; ++m) un0[m] = P.u_n[gofs + m * ((DIM == 3) ? NP * NP : NP)];
@@ -452,7 +483,7 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   if constexpr (DIM == 3 || (NTASK > NT)) __syncthreads();
 
   // ---- last pass (zeta in 3-D, eta in 2-D) fused with phase D: lifts, 1/J, SSP-RK combination (eq. 12, 45)
-  for (int t = tid; t < EB * NLT; t += NT) {
+  for (int t = tid; t < EB * NVAR * LastPass<DIM, NP>::SLOT; t += NT) {
     int el, v, ij;                               // 3-D: ij = i + NP*j ; 2-D: ij = i
     last_pass_task<DIM, NP, NVAR, EB>(t, el, v, ij);
     if (el >= nel) continue;
