@@ -325,16 +325,8 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
     const long ep = e0 + (long)MARUT_L2_PREFETCH * EB;
     if (ep + EB < P.ne) {
       const size_t bytes = (size_t)EB * NVAR * NN * sizeof(double);
-      const char *a = reinterpret_cast<const char *>(P.u_in + ep * NVAR * NN);
-      const char *al = reinterpret_cast<const char *>(reinterpret_cast<uintptr_t>(a) & ~(uintptr_t)15);
-      const unsigned sz = (unsigned)(((a + bytes) - al + 15) & ~(size_t)15);
-      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(al), "r"(sz) : "memory");
-      if (P.ca != 0.0) {
-        const char *b = reinterpret_cast<const char *>(P.u_n + ep * NVAR * NN);
-        const char *bl = reinterpret_cast<const char *>(reinterpret_cast<uintptr_t>(b) & ~(uintptr_t)15);
-        const unsigned sb = (unsigned)(((b + bytes) - bl + 15) & ~(size_t)15);
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(bl), "r"(sb) : "memory");
-      }
+      l2_prefetch(P.u_in + ep * NVAR * NN, bytes);
+      if (P.ca != 0.0) l2_prefetch(P.u_n + ep * NVAR * NN, bytes);
     }
   }
 #endif
