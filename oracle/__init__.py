@@ -75,6 +75,11 @@ def _setup(L):
         L.oracle_temperature.argtypes = [vp, vp, C.c_double]
         L.oracle_species_thermo.argtypes = [vp, C.c_int, C.c_double, vp]
         L.oracle_num_threads.restype = C.c_int
+        L.oracle_set_volume_form.restype = C.c_int
+        L.oracle_set_volume_form.argtypes = [vp, C.c_int]
+        L.oracle_logmean.restype = C.c_double
+        L.oracle_logmean.argtypes = [C.c_double, C.c_double]
+        L.oracle_ranocha.argtypes = [C.c_int, C.c_double, vp, vp, vp, vp]
     return L
 
 
@@ -169,6 +174,9 @@ class OracleMesh:
         self.h = L.oracle_mesh_create(C.addressof(d))
         self.nvar = L.oracle_nvar(self.h)
         self.shape = (mesh.n_elem, self.nvar, mesh.nn)
+        if getattr(mesh, "volume_form", 0):
+            if L.oracle_set_volume_form(self.h, int(mesh.volume_form)) != 0:
+                raise ValueError("unsupported volume_form for this physics")
 
     def __del__(self):
         if getattr(self, "h", None) and getattr(self, "L", None) is not None:
@@ -263,6 +271,17 @@ def viscous_flux(dim, gamma, mu, Pr, U, S, nv):
     U, S, nv = _f64(U), _f64(S), _f64(nv)
     F = np.zeros(dim + 2)
     lib().oracle_viscous_flux(dim, gamma, mu, Pr, _p(U), _p(S), _p(nv), _p(F))
+    return F
+
+
+def logmean(aL, aR):
+    return lib().oracle_logmean(float(aL), float(aR))
+
+
+def ranocha(dim, gamma, UL, UR, nv):
+    UL, UR, nv = _f64(UL), _f64(UR), _f64(nv)
+    F = np.zeros(dim + 2)
+    lib().oracle_ranocha(dim, gamma, _p(UL), _p(UR), _p(nv), _p(F))
     return F
 
 

@@ -286,6 +286,7 @@ struct Mesh {
   Mech mech;
   std::vector<double> Pf[2], Pr_[2];
   double dx_min = 0.0;
+  int volume_form = 0;          // 0: standard strong form (eq. 9); 1: entropy-stable split form (eq. 10)
 };
 
 static inline int node_index(const Mesh &m, const int *ijk) {
@@ -457,6 +458,36 @@ static void flux_dot(const Mesh &m, const double *U, const Prim &q, const double
   for (int c = 0; c < d; ++c) F[ns + c] = U[ns + c] * vn + q.p * nv[c];
   F[ns + d] = (U[ns + d] + q.p) * vn;
 }
+// O13. Logarithmic mean {{a}}^ln = (aL - aR)/(ln aL - ln aR).  The paper gives no evaluation that
+// is stable near aL = aR; reading R13: Ismail & Roe's form, zeta = aL/aR, f = (zeta-1)/(zeta+1),
+// u = f^2, F = 1 + u/3 + u^2/5 + u^3/7 for u < 1e-2, else ln(zeta)/(2 f); {{a}}^ln = (aL + aR)/(2 F).
+static double logmean(double aL, double aR) {
+  const double zeta = aL / aR, f = (zeta - 1.0) / (zeta + 1.0), u = f * f;
+  const double F = (u < 1.0e-2) ? 1.0 + u / 3.0 + u * u / 5.0 + u * u * u / 7.0 : std::log(zeta) / (2.0 * f);
+  return (aL + aR) / (2.0 * F);
+}
+// O14. Two-point volume flux of Ranocha contracted with a (scaled, averaged) vector nv (eq. 41):
+//   F_rho = {{rho}}^ln {{v}}.n ;  F_rho v_c = {{rho}}^ln {{v}}.n {{v_c}} + {{p}} n_c ;
+//   F_E = ( 1/((gamma-1) {{T^-1}}^ln) + 1/2 sum_c {{v_c}}^2 ) {{rho}}^ln {{v}}.n + {{p v}}.n ,  T = p/rho.
+// The paper prints 1/(2 (gamma-1) {{T^-1}}^ln); with T = p/rho that contradicts the consistency F#(U,U) = F_inv(U)
+// it states in eq. 40 (the 2 belongs to beta = rho/(2p) of the cited flux): reading R13 takes eq. 40.
+static void ranocha_flux(const Mesh &m, const double *UL, const double *UR, const double *nv, double *F) {
+  const int d = m.dim;
+  const Prim L = primitives(m, UL), R = primitives(m, UR);
+  const double rho_ln = logmean(L.rho, R.rho);
+  const double tinv_ln = logmean(L.rho / L.p, R.rho / R.p);
+  double vavg[3] = {0.0, 0.0, 0.0}, vn = 0.0, v2 = 0.0, pvn = 0.0;
+  for (int c = 0; c < d; ++c) {
+    vavg[c] = 0.5 * (L.vel[c] + R.vel[c]);
+    vn += vavg[c] * nv[c];
+    v2 += vavg[c] * vavg[c];
+    pvn += 0.5 * (L.p * L.vel[c] + R.p * R.vel[c]) * nv[c];
+  }
+  const double pavg = 0.5 * (L.p + R.p);
+  F[0] = rho_ln * vn;
+  for (int c = 0; c < d; ++c) F[1 + c] = rho_ln * vn * vavg[c] + pavg * nv[c];
+  F[1 + d] = (1.0 / ((m.gamma - 1.0) * tinv_ln) + 0.5 * v2) * rho_ln * vn + pvn;
+}
 // O5. Local Lax-Friedrichs / Rusanov flux with scaled outward normal nv:
 //   F* = 1/2 (F(U-)+F(U+)).nv - 1/2 lambda |nv| (U+ - U-),
 //   lambda = max(|v-.nhat| + a-, |v+.nhat| + a+),  nhat = nv/|nv|.
@@ -492,6 +523,30 @@ static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
   // --- volume: R_i = -(1/J_i) sum_l sum_m D_{i_l m} Ftilde^l_m,  Ftilde^l = Ja^l . F_inv
 #pragma omp parallel for schedule(static)
   for (long e = 0; e < m.ne; ++e) {
+    if (m.volume_form == 1) {
+      // eq. 10: R_i = -(2/J_i) sum_l sum_m D_{i_l m} F#(U_i, U_m; 1/2 (Ja^l_i + Ja^l_m)),
+      // m running over the nodes of the line through i along direction l
+      for (int p = 0; p < nn; ++p) {
+        int ijk[3] = {0, 0, 0}; node_ijk(m, p, ijk);
+        double Ui[MAXV], acc[MAXV]; gather(m, u, e, p, Ui);
+        for (int v = 0; v < nvar; ++v) acc[v] = 0.0;
+        for (int l = 0; l < d; ++l) {
+          const double *Jai = &m.Ja[((size_t)e * nn + p) * d * d + l * d];
+          for (int mm = 0; mm < n; ++mm) {
+            int q[3] = {ijk[0], ijk[1], ijk[2]}; q[l] = mm;
+            const int pm = node_index(m, q);
+            const double *Jam = &m.Ja[((size_t)e * nn + pm) * d * d + l * d];
+            double Um[MAXV], nvv[3], F[MAXV]; gather(m, u, e, pm, Um);
+            for (int c = 0; c < d; ++c) nvv[c] = 0.5 * (Jai[c] + Jam[c]);
+            ranocha_flux(m, Ui, Um, nvv, F);
+            const double dim_ = m.ops.D[(size_t)ijk[l] * n + mm];
+            for (int v = 0; v < nvar; ++v) acc[v] += dim_ * F[v];
+          }
+        }
+        for (int v = 0; v < nvar; ++v) du[((size_t)e * nvar + v) * nn + p] = -2.0 * acc[v] / m.J[(size_t)e * nn + p];
+      }
+      continue;
+    }
     std::vector<double> Ft((size_t)d * nvar * nn);      // [l][v][node]
     for (int p = 0; p < nn; ++p) {
       double U[MAXV], F[MAXV]; gather(m, u, e, p, U);
@@ -826,6 +881,17 @@ void *oracle_mesh_create(const oracle_mesh_desc *d) {
   return m;
 }
 void oracle_mesh_destroy(void *h) { delete (Mesh *)h; }
+int oracle_set_volume_form(void *h, int form) {
+  Mesh *m = (Mesh *)h;
+  if (form < 0 || form > 1 || (form == 1 && m->physics == REACTING_EULER)) return 1;
+  m->volume_form = form;
+  return 0;
+}
+double oracle_logmean(double aL, double aR) { return logmean(aL, aR); }
+void oracle_ranocha(int dim, double gamma, const double *UL, const double *UR, const double *nv, double *F) {
+  Mesh m; m.dim = dim; m.gamma = gamma; m.nvar = dim + 2; m.ns = 1; m.physics = EULER;
+  ranocha_flux(m, UL, UR, nv, F);
+}
 int oracle_nvar(void *h) { return ((Mesh *)h)->nvar; }
 double oracle_dx_min(void *h) { return ((Mesh *)h)->dx_min; }
 // metrics out: Ja [e][node][l][c], J [e][node]

@@ -101,6 +101,7 @@ class Mesh:
     mu: float = 0.0
     Pr: float = 0.72
     mech: Mech | None = None
+    volume_form: int = 0   # 0: standard strong-form volume integral (eq. 9); 1: entropy-stable split form (eq. 10)
     info: dict = field(default_factory=dict)
 
     @property
