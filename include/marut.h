@@ -109,6 +109,14 @@ marut_status marut_max_dt(marut_mesh *mesh, const double *u, double cfl, double 
  * momentum and energy rows 0.  REACTING_EULER meshes only (else EINVAL). */
 marut_status marut_chem_source(marut_mesh *mesh, const double *u, double *s, void *cuda_stream);
 
+/* Volume-integral form of L.  MARUT_VOLUME_STRONG (default): eq. 9, the standard strong form.
+ * MARUT_VOLUME_SPLIT_RANOCHA: the entropy-stable split form, eq. 10,
+ *   R_i = -(2/J_i) sum_l sum_m D_{i_l m} F#(U_i, U_m; 1/2 (Ja^l_i + Ja^l_m)),
+ * with the two-point flux of Ranocha (eq. 41) and logarithmic means (R13); the surface
+ * terms are unchanged.  MARUT_EULER meshes with N <= 5 only (else EINVAL).  Takes effect from the next call. */
+enum { MARUT_VOLUME_STRONG = 0, MARUT_VOLUME_SPLIT_RANOCHA = 1 };
+marut_status marut_set_volume_form(marut_mesh *mesh, int form);
+
 /* --- introspection (used by the tests to check setup row a0; no compute path depends on them) --- */
 /* copy the device metric terms to HOST arrays: Ja [n_elem][n^dim][dim][dim] (Ja^l_c), J [n_elem][n^dim]. */
 marut_status marut_get_metrics(marut_mesh *mesh, double *Ja_host, double *J_host);

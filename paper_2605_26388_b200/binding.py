@@ -15,7 +15,7 @@ _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA"
 
 # every symbol include/marut.h declares
 SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt",
-           "marut_chem_source", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
+           "marut_chem_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
            "marut_last_error"]
 
 
@@ -64,6 +64,8 @@ def lib():
         L.marut_max_dt.argtypes = [vp, vp, dbl, C.POINTER(dbl), vp]
         L.marut_chem_source.restype = C.c_int
         L.marut_chem_source.argtypes = [vp, vp, vp, vp]
+        L.marut_set_volume_form.restype = C.c_int
+        L.marut_set_volume_form.argtypes = [vp, C.c_int]
         L.marut_get_metrics.restype = C.c_int
         L.marut_get_metrics.argtypes = [vp, vp, vp]
         L.marut_is_affine.restype = C.c_int
@@ -150,6 +152,10 @@ def marut_chem_source(h, u, s, stream=None):
     _check(lib().marut_chem_source(h, _dev(u), _dev(s), _stream(stream)))
 
 
+def marut_set_volume_form(h, form):
+    _check(lib().marut_set_volume_form(h, int(form)))
+
+
 def ssprk3_step(h, u, ua, ub, dt, t=0.0, stream=None):
     """one SSP-RK33 step = three marut_ssprk_stage calls; u is overwritten with u^{n+1}. ua, ub: scratch."""
     marut_ssprk_stage(h, 0, dt, t, u, u, ua, stream)
@@ -165,6 +171,8 @@ class MarutMesh:
         self.mesh = mesh
         ns = mesh.mech.ns if mesh.physics == REACTING_EULER else 1
         self.shape = (mesh.node_xyz.shape[0], ns + mesh.dim + 1, (mesh.N + 1) ** mesh.dim)
+        if getattr(mesh, "volume_form", 0):
+            marut_set_volume_form(self.h, mesh.volume_form)
 
     def close(self):
         if getattr(self, "h", None):

@@ -43,6 +43,7 @@ struct marut_mesh {
   // device
   double *d_metric = nullptr;
   double *d_fnorm = nullptr;   // affine: [e][dim] |Ja^l|
+  int volume_form = 0;         // MARUT_VOLUME_STRONG | MARUT_VOLUME_SPLIT_RANOCHA
   int kernel_sel = 0;          // Euler stage kernel: 0 node (marut_node.cuh), 1 line (marut_line.cuh), 2 generic; env MARUT_KERNEL
   int2 *d_conn = nullptr;
   int *d_mortar_fine = nullptr;
@@ -491,6 +492,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   switch (m->physics) {
     case MARUT_EULER:
       e = cudaErrorNotSupported;
+      if (m->volume_form == MARUT_VOLUME_SPLIT_RANOCHA) { e = launch_stage_split(m->dim, m->np, m->affine, P, st); break; }
       if (m->kernel_sel == 3 && m->dim == 3 && m->affine && m->n_mortar == 0) e = launch_stage_line2_3d(m->np, P, st);
       if (m->kernel_sel == 0 || (m->kernel_sel == 3 && e == cudaErrorNotSupported)) e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
       if (m->kernel_sel == 1) e = (m->dim == 2) ? launch_stage_line2d(m->np, m->affine, P, st) : launch_stage_line3d(m->np, m->affine, P, st);
@@ -503,6 +505,16 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   if (e == cudaErrorNotSupported) return fail(MARUT_EINVAL, "no kernel instantiated for dim=%d N=%d physics=%d", m->dim, m->N, m->physics);
   if (e != cudaSuccess) return fail(MARUT_ECUDA, "stage kernel: %s", cudaGetErrorString(e));
   m->launches++;
+  return MARUT_OK;
+}
+
+extern "C" marut_status marut_set_volume_form(marut_mesh *m, int form) {
+  if (!m) return fail(MARUT_EINVAL, "NULL argument");
+  if (form != MARUT_VOLUME_STRONG && form != MARUT_VOLUME_SPLIT_RANOCHA) return fail(MARUT_EINVAL, "unknown volume form %d", form);
+  if (form == MARUT_VOLUME_SPLIT_RANOCHA && m->physics != MARUT_EULER)
+    return fail(MARUT_EINVAL, "the split-form volume integral is implemented for MARUT_EULER only");
+  if (form == MARUT_VOLUME_SPLIT_RANOCHA && m->np > 6) return fail(MARUT_EINVAL, "split form: N <= 5");
+  m->volume_form = form;
   return MARUT_OK;
 }
 

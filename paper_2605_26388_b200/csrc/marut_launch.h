@@ -12,6 +12,7 @@ cudaError_t launch_stage_line3d(int np, bool affine, const StageParams &P, cudaS
 cudaError_t launch_stage_node2d(int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_stage_node3d(int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_stage_line2_3d(int np, const StageParams &P, cudaStream_t st);
+cudaError_t launch_stage_split(int dim, int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_stage_ns(int dim, int np, bool affine, bool generic, const StageParams &P, cudaStream_t st);
 cudaError_t launch_gradient(int dim, int np, bool affine, const GradParams &P, cudaStream_t st);
 cudaError_t launch_stage_react(int dim, int np, int nsp, bool affine, bool generic, const StageParams &P, cudaStream_t st);

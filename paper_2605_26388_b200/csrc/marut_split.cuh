@@ -1,0 +1,192 @@
+// marut_split.cuh -- fused Euler stage with the entropy-stable split-form volume integral (
+// PAPER.md:183-187 eq. 10, 594-627 eq. 39-41): R_i = -(2/J_i) sum_l sum_m D_{i_l m} F#(U_i, U_m; avg Ja^l), F# the
+// two-point flux of Ranocha with logarithmic means (reading R13).  Interface / mortar / boundary flux,
+// lift, 1/J and the SSP-RK combination are those of marut_node.cuh (same face tasks, same stash).
+//
+//   phase N  per node: U from global, primitives; stash U, 1/rho, p, a (face tasks) and ln rho, ln(rho/p)
+//            (so that a logarithmic mean costs no logarithm per pair)
+//   phase V  per node: for every direction and every node m of the line through the node: two-point flux with
+//            the partner's stash entries, accumulated with D from the constant bank -- ALU-bound
+//   phase S  face nodes, densely mapped (euler_face_task)
+//   phase D  per node: lifts, 1/J, SSP-RK combination, u_n / u_out straight from / to global
+//
+// Product code; shares nothing with oracle/.
+#pragma once
+#include "marut_node.cuh"
+
+namespace marut {
+
+// logarithmic mean from the two values and their logarithms: (aL + aR)/(2 F), F = ln(zeta)/(2 f) with
+// f = (aL - aR)/(aL + aR), replaced by its series 1 + u/3 + u^2/5 + u^3/7 (u = f^2) for u < 1e-2.
+// Returns F and 1/(aL + aR): callers need either the mean or its reciprocal.
+__device__ __forceinline__ double logmean_F(double aL, double aR, double lnL, double lnR, double &inv_sum) {
+  inv_sum = 1.0 / (aL + aR);
+  const double f = (aL - aR) * inv_sum, u = f * f;
+  return (u < 1.0e-2) ? 1.0 + u * (1.0 / 3.0) + u * u * (1.0 / 5.0) + u * u * u * (1.0 / 7.0) : (lnL - lnR) / (2.0 * f);
+}
+
+template <int DIM, int NP, bool AFFINE, int EB, int MINB>
+__global__ void __launch_bounds__((NodeCfg<DIM, NP, 1, EB>::NT), MINB)
+stage_split_kernel(const __grid_constant__ StageParams P) {
+  using C = NodeCfg<DIM, NP, 1, EB>;
+  using G = Geo<DIM, NP>;
+  constexpr int NVAR = C::NVAR, NN = C::NN, NF = C::NF, TILE = C::TILE, NFN = C::NFN, NT = C::NT;
+  constexpr int MD = G::MD, MDP = C::MDP, NST = C::NST;
+  extern __shared__ __align__(16) double smem[];
+  double *Ust = smem;                       // [NVAR + 3][TILE]  U, 1/rho, p, a
+  double *Lns = Ust + NST * TILE;           // [2][TILE]         ln rho, ln(rho/p)
+  double *Lft = Lns + 2 * TILE;             // [NVAR][LFS]       lifts of the face nodes
+  double *Msm = Lft + NVAR * C::LFS;        // affine: [EB][MDP] Ja, 1/J, |Ja^l|
+
+  const int tid = threadIdx.x;
+  const long e0 = (long)blockIdx.x * EB;
+  const int nel = (int)((P.ne - e0 < EB) ? (P.ne - e0) : EB);
+  const int ntask = nel * NFN;
+  const bool has0 = tid < ntask;
+  const FaceTask t0 = decode_task<DIM, NP>(has0 ? tid : 0);
+  int2 cn0 = make_int2(0, FK_BOUNDARY);
+  if (has0) cn0 = __ldg(&P.conn[(e0 + t0.el) * 2 * DIM + t0.f]);
+  if constexpr (AFFINE) {
+    for (int i = tid; i < nel * MDP; i += NT) {
+      const int me = i / MDP, k = i - me * MDP;
+      Msm[i] = (k < MD) ? __ldg(&P.metric[(e0 + me) * MD + k]) : ((k < MD + DIM) ? __ldg(&P.fnorm[(e0 + me) * DIM + (k - MD)]) : 0.0);
+    }
+  }
+  const int el = tid / NN, p = tid - el * NN;
+  const long e = e0 + el;
+  const bool active = (tid < TILE) && (el < nel);
+  const int qi = p % NP, qj = (p / NP) % NP, qk = (DIM == 3) ? p / (NP * NP) : 0;
+
+  // ---- phase N
+  double U[NVAR], vi[DIM], pi_ = 0.0, lnr = 0.0, lnb = 0.0;
+  if (active) {
+    const double *up = P.u_in + e * NVAR * NN + p;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
+    const Prim<DIM> pr = prim_ideal<DIM, true>(U, P.gamma);
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) vi[c] = pr.v[c];
+    pi_ = pr.p;
+    lnr = log(U[0]);
+    lnb = log(U[0] / pr.p);
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Ust[v * TILE + tid] = U[v];
+    Ust[NVAR * TILE + tid] = pr.irho;
+    Ust[(NVAR + 1) * TILE + tid] = pr.p;
+    Ust[(NVAR + 2) * TILE + tid] = pr.a;
+    Lns[tid] = lnr;
+    Lns[TILE + tid] = lnb;
+  }
+  double Up0[NVAR];
+  if (has0) gather_exterior<DIM, NP, NVAR>(P, t0, cn0, Up0);
+  __syncthreads();
+
+  // ---- phase V: split-form volume term (eq. 10)
+  double R[NVAR];
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) R[v] = 0.0;
+  if (active) {
+    const double bi = U[0] / pi_;
+#pragma unroll
+    for (int l = 0; l < DIM; ++l) {
+      const int ql = (l == 0) ? qi : ((l == 1) ? qj : qk);
+      const int st = G::stride(l);
+      const int base = tid - ql * st;
+      double Ji[DIM];
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) Ji[c] = AFFINE ? Msm[el * MDP + l * DIM + c] : __ldg(&P.metric[(e * MD + l * DIM + c) * NN + p]);
+#pragma unroll
+      for (int m = 0; m < NP; ++m) {
+        const int pm = base + m * st;            // stash index of the partner node
+        const double rm = Ust[pm], irm = Ust[NVAR * TILE + pm], pmm = Ust[(NVAR + 1) * TILE + pm];
+        double nv[DIM], vavg[DIM], vn = 0.0, v2 = 0.0, pvn = 0.0;
+#pragma unroll
+        for (int c = 0; c < DIM; ++c) {
+          const double vm = Ust[(1 + c) * TILE + pm] * irm;
+          if constexpr (AFFINE) nv[c] = Ji[c];
+          else nv[c] = 0.5 * (Ji[c] + __ldg(&P.metric[(e * MD + l * DIM + c) * NN + (pm - el * NN)]));
+          vavg[c] = 0.5 * (vi[c] + vm);
+          vn += vavg[c] * nv[c];
+          v2 += vavg[c] * vavg[c];
+          pvn += 0.5 * (pi_ * vi[c] + pmm * vm) * nv[c];
+        }
+        double inv_r, inv_b;
+        const double Fr = logmean_F(U[0], rm, lnr, Lns[pm], inv_r);
+        const double Fb = logmean_F(bi, rm / pmm, lnb, Lns[TILE + pm], inv_b);
+        const double rho_ln = (U[0] + rm) / (2.0 * Fr);
+        const double eint = 2.0 * Fb * inv_b / (P.gamma - 1.0);       // 1 / ((gamma-1) {{T^-1}}^ln)
+        const double pavg = 0.5 * (pi_ + pmm);
+        const double d = P.D[ql * NP + m];   // runtime row: constant-bank load with a lane-dependent index
+        const double mf = rho_ln * vn;
+        R[0] += d * mf;
+#pragma unroll
+        for (int c = 0; c < DIM; ++c) R[1 + c] += d * (mf * vavg[c] + pavg * nv[c]);
+        R[1 + DIM] += d * ((eint + 0.5 * v2) * mf + pvn);
+      }
+    }
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) R[v] *= 2.0;
+  }
+
+  // ---- phase S: face nodes, densely mapped
+  if (has0) euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
+  for (int g = tid + NT; g < ntask; g += NT) {
+    const FaceTask t = decode_task<DIM, NP>(g);
+    const int2 cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
+    double Up[NVAR];
+    gather_exterior<DIM, NP, NVAR>(P, t, cn, Up);
+    euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, g, t, cn, Up);
+  }
+  __syncthreads();
+  if (!active) return;
+
+  // ---- phase D
+  {
+    const double *lf = Lft + el * NFN;
+    if (qi == 0 || qi == NP - 1) {
+      const int g = ((qi == 0) ? 0 : 1) * NF + qj + NP * qk;
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) R[v] += lf[v * C::LFS + g];
+    }
+    if (qj == 0 || qj == NP - 1) {
+      const int g = (2 + ((qj == 0) ? 0 : 1)) * NF + qi + NP * qk;
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) R[v] += lf[v * C::LFS + g];
+    }
+    if (DIM == 3 && (qk == 0 || qk == NP - 1)) {
+      const int g = (4 + ((qk == 0) ? 0 : 1)) * NF + qi + NP * qj;
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) R[v] += lf[v * C::LFS + g];
+    }
+  }
+  const double invJ = AFFINE ? Msm[el * MDP + DIM * DIM] : __ldg(&P.metric[(e * MD + DIM * DIM) * NN + p]);
+  double *op = P.u_out + e * NVAR * NN + p;
+  if (P.ca != 0.0) {
+    const double *np_ = P.u_n + e * NVAR * NN + p;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.ca * np_[v * NN] + (P.cb * U[v] + P.cc * (0.0 - invJ * R[v]));
+  } else {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.cb * U[v] + P.cc * (0.0 - invJ * R[v]);
+  }
+}
+
+template <int DIM, int NP, bool AFFINE>
+cudaError_t launch_stage_split_t(const StageParams &P, cudaStream_t st) {
+  constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
+  using C = NodeCfg<DIM, NP, 1, EB>;
+  constexpr size_t smem = ((size_t)(C::NST + 2) * C::TILE + (size_t)C::NVAR * C::LFS + (AFFINE ? EB * C::MDP : 0)) * sizeof(double);
+  constexpr int MINB = (C::NT <= 128) ? 4 : ((C::NT <= 256) ? 2 : 1);
+  auto k = stage_split_kernel<DIM, NP, AFFINE, EB, MINB>;
+  static bool attr = false;
+  if (!attr) {
+    cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    attr = true;
+  }
+  const long grid = (P.ne + EB - 1) / EB;
+  k<<<(unsigned)grid, C::NT, smem, st>>>(P);
+  return cudaGetLastError();
+}
+
+}  // namespace marut

@@ -56,3 +56,36 @@ def test_rhs_and_stage(dim, N, cells, curved, phys):
     torch.cuda.synchronize()
     assert parity_error(out.cpu().numpy(), om.ssprk_stage(2, dt, 0.0, un_h, u0)).max() <= RHS_TOL
     gm.close()
+
+
+SPLIT = [(2, 3, 6, False), (2, 4, 5, True), (3, 4, 3, False), (3, 3, 3, True), (3, 1, 3, False), (3, 5, 2, False)]
+
+
+@pytest.mark.parametrize("dim,N,cells,curved", SPLIT)
+def test_split_form_rhs_stage_and_run(dim, N, cells, curved):
+    """entropy-stable split-form volume integral (marut_set_volume_form) against the oracle"""
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+    from parity_util import RUN_TOL, gpu_run
+
+    m = _mesh(dim, N, cells, curved)
+    m.volume_form = 1
+    u0 = wl.isentropic_vortex(m) if dim == 2 else wl.taylor_green(m, noise=1e-3)
+    om, gm = oracle.OracleMesh(m), mb.MarutMesh(m)
+    u = torch.from_numpy(u0).cuda()
+    du = torch.empty_like(u)
+    gm.rhs(u, du)
+    torch.cuda.synchronize()
+    assert parity_error(du.cpu().numpy(), om.rhs(u0)).max() <= RHS_TOL
+    dt = om.max_dt(u0, 0.4)
+    un_h = u0 * (1.0 + 1e-3)
+    out = torch.empty_like(u)
+    gm.stage(1, dt, 0.0, torch.from_numpy(un_h).cuda(), u, out)
+    torch.cuda.synchronize()
+    assert parity_error(out.cpu().numpy(), om.ssprk_stage(1, dt, 0.0, un_h, u0)).max() <= RHS_TOL
+    ug, tg = gpu_run(gm, u0, 5, 0.4, torch)
+    uc, tc, _, _ = om.run(u0, 5, cfl=0.4)
+    assert abs(tg - tc) <= 1e-12 * tc and parity_error(ug, uc).max() <= RUN_TOL
+    gm.close()
