@@ -29,12 +29,27 @@ if ROOT not in sys.path:
 METRIC = "DG RHS+SSPRK3 DOF-stage updates/s (FP64)"
 UNIT = "DOF-stage/s"
 # bounded oracle samples: (cells per direction, target seconds)
-ORACLE_SAMPLE_CELLS = {"c1": None, "c2": 12, "c3": 16, "c4": 64, "c4w": 64, "c5": 8}
+ORACLE_SAMPLE_CELLS = {"c1": None, "c2": 12, "c2s": 12, "c3": 16, "c4": 64, "c4w": 64, "c5": 8}
+
+
+def make_workload(name, cells=None):
+    """c1..c5, c4w: the configs of BASELINE.json (workloads.make_case); c2s: c2 with the entropy-stable split-form
+    volume integral"""
+    import workloads as wl
+
+    if name == "c2s":
+        c = wl.make_case("c2", cells=cells)
+        c.mesh.volume_form = 1
+        c.name = "c2s"
+        return c
+    return wl.make_case(name, cells=cells)
 
 
 def workload_name(case):
     m = case.mesh
     phys = {0: "Euler", 1: "Navier-Stokes (BR1)", 2: "reacting Euler, 5 species"}[m.physics]
+    if getattr(m, "volume_form", 0):
+        phys += " (entropy-stable split form, Ranocha flux)"
     return (f"{case.name}: {m.dim}-D {phys}, N={m.N}, {m.n_elem} elements, {m.n_elem * m.nn} nodes, "
             f"{m.n_dof} DOF, {len(m.mortar)} mortars, {len(m.bface)} boundary faces")
 
@@ -125,7 +140,7 @@ def oracle_sample(workload, budget_s):
     import workloads as wl
 
     cells = ORACLE_SAMPLE_CELLS[workload]
-    c = wl.make_case(workload, cells=cells)
+    c = make_workload(workload, cells=cells)
     om = oracle.OracleMesh(c.mesh)
     t0 = time.perf_counter()
     u = om.run(c.u0, 1, cfl=c.cfl)[0]          # calibration step (counted)
@@ -151,7 +166,7 @@ def run_reference(args):
     import oracle
 
     cells = ORACLE_SAMPLE_CELLS[args.workload]
-    c = wl.make_case(args.workload, cells=cells)
+    c = make_workload(args.workload, cells=cells)
     om = oracle.OracleMesh(c.mesh)
     # one "step" of this arm = `inner` SSP-RK33 steps of the sample, sized to per_step_budget
     t0 = time.perf_counter()
@@ -222,7 +237,7 @@ def run_cuda(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    case = wl.make_case(args.workload)
+    case = make_workload(args.workload)
     mesh = case.mesh
     gm = mb.MarutMesh(mesh)
     affine = gm.is_affine

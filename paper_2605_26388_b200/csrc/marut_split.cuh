@@ -16,13 +16,20 @@
 
 namespace marut {
 
-// logarithmic mean from the two values and their logarithms: (aL + aR)/(2 F), F = ln(zeta)/(2 f) with
-// f = (aL - aR)/(aL + aR), replaced by its series 1 + u/3 + u^2/5 + u^3/7 (u = f^2) for u < 1e-2.
-// Returns F and 1/(aL + aR): callers need either the mean or its reciprocal.
-__device__ __forceinline__ double logmean_F(double aL, double aR, double lnL, double lnR, double &inv_sum) {
-  inv_sum = 1.0 / (aL + aR);
-  const double f = (aL - aR) * inv_sum, u = f * f;
-  return (u < 1.0e-2) ? 1.0 + u * (1.0 / 3.0) + u * u * (1.0 / 5.0) + u * u * u * (1.0 / 7.0) : (lnL - lnR) / (2.0 * f);
+// logarithmic mean {{a}}^ln = num/den from the two values and their logarithms, one division for the caller (who
+// needs either the mean or its reciprocal).  With d = aL - aR, s = aL + aR, u = (d/s)^2:
+//   u >= 1e-2:  num = d, den = ln aL - ln aR                              (the definition)
+//   u <  1e-2:  {{a}}^ln = s/(2 (1 + u/3 + u^2/5 + u^3/7)), multiplied through by s^6 (R13)
+__device__ __forceinline__ void logmean_nd(double aL, double aR, double lnL, double lnR, double &num, double &den) {
+  const double d = aL - aR, s = aL + aR, X = s * s, Y = d * d;
+  if (Y < 1.0e-2 * X) {
+    const double X2 = X * X, Y2 = Y * Y;
+    num = s * X2 * X;
+    den = 2.0 * (X2 * X + X2 * Y * (1.0 / 3.0) + X * Y2 * (1.0 / 5.0) + Y2 * Y * (1.0 / 7.0));
+  } else {
+    num = d;
+    den = lnL - lnR;
+  }
 }
 
 template <int DIM, int NP, bool AFFINE, int EB, int MINB>
@@ -34,8 +41,8 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
   constexpr int MD = G::MD, MDP = C::MDP, NST = C::NST;
   extern __shared__ __align__(16) double smem[];
   double *Ust = smem;                       // [NVAR + 3][TILE]  U, 1/rho, p, a
-  double *Lns = Ust + NST * TILE;           // [2][TILE]         ln rho, ln(rho/p)
-  double *Lft = Lns + 2 * TILE;             // [NVAR][LFS]       lifts of the face nodes
+  double *Lns = Ust + NST * TILE;           // [3 + DIM][TILE]   ln rho, ln(rho/p), rho/p, velocity
+  double *Lft = Lns + (3 + DIM) * TILE;             // [NVAR][LFS]       lifts of the face nodes
   double *Msm = Lft + NVAR * C::LFS;        // affine: [EB][MDP] Ja, 1/J, |Ja^l|
 
   const int tid = threadIdx.x;
@@ -76,6 +83,9 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
     Ust[(NVAR + 2) * TILE + tid] = pr.a;
     Lns[tid] = lnr;
     Lns[TILE + tid] = lnb;
+    Lns[2 * TILE + tid] = U[0] / pr.p;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) Lns[(3 + c) * TILE + tid] = pr.v[c];
   }
   double Up0[NVAR];
   if (has0) gather_exterior<DIM, NP, NVAR>(P, t0, cn0, Up0);
@@ -86,7 +96,7 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
 #pragma unroll
   for (int v = 0; v < NVAR; ++v) R[v] = 0.0;
   if (active) {
-    const double bi = U[0] / pi_;
+    const double bi = U[0] / pi_, inv_gm1 = 1.0 / (P.gamma - 1.0);
 #pragma unroll
     for (int l = 0; l < DIM; ++l) {
       const int ql = (l == 0) ? qi : ((l == 1) ? qj : qk);
@@ -97,12 +107,13 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
       for (int c = 0; c < DIM; ++c) Ji[c] = AFFINE ? Msm[el * MDP + l * DIM + c] : __ldg(&P.metric[(e * MD + l * DIM + c) * NN + p]);
 #pragma unroll
       for (int m = 0; m < NP; ++m) {
+        if (m == ql && ql != 0 && ql != NP - 1) continue;   // D_ii = 0 at interior LGL nodes
         const int pm = base + m * st;            // stash index of the partner node
-        const double rm = Ust[pm], irm = Ust[NVAR * TILE + pm], pmm = Ust[(NVAR + 1) * TILE + pm];
+        const double rm = Ust[pm], pmm = Ust[(NVAR + 1) * TILE + pm];
         double nv[DIM], vavg[DIM], vn = 0.0, v2 = 0.0, pvn = 0.0;
 #pragma unroll
         for (int c = 0; c < DIM; ++c) {
-          const double vm = Ust[(1 + c) * TILE + pm] * irm;
+          const double vm = Lns[(3 + c) * TILE + pm];
           if constexpr (AFFINE) nv[c] = Ji[c];
           else nv[c] = 0.5 * (Ji[c] + __ldg(&P.metric[(e * MD + l * DIM + c) * NN + (pm - el * NN)]));
           vavg[c] = 0.5 * (vi[c] + vm);
@@ -110,11 +121,11 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
           v2 += vavg[c] * vavg[c];
           pvn += 0.5 * (pi_ * vi[c] + pmm * vm) * nv[c];
         }
-        double inv_r, inv_b;
-        const double Fr = logmean_F(U[0], rm, lnr, Lns[pm], inv_r);
-        const double Fb = logmean_F(bi, rm / pmm, lnb, Lns[TILE + pm], inv_b);
-        const double rho_ln = (U[0] + rm) / (2.0 * Fr);
-        const double eint = 2.0 * Fb * inv_b / (P.gamma - 1.0);       // 1 / ((gamma-1) {{T^-1}}^ln)
+        double nr, dr, nb, db;
+        logmean_nd(U[0], rm, lnr, Lns[pm], nr, dr);
+        logmean_nd(bi, Lns[2 * TILE + pm], lnb, Lns[TILE + pm], nb, db);
+        const double rho_ln = nr / dr;
+        const double eint = inv_gm1 * (db / nb);                      // 1 / ((gamma-1) {{T^-1}}^ln)
         const double pavg = 0.5 * (pi_ + pmm);
         const double d = P.D[ql * NP + m];   // runtime row: constant-bank load with a lane-dependent index
         const double mf = rho_ln * vn;
@@ -175,7 +186,7 @@ template <int DIM, int NP, bool AFFINE>
 cudaError_t launch_stage_split_t(const StageParams &P, cudaStream_t st) {
   constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
   using C = NodeCfg<DIM, NP, 1, EB>;
-  constexpr size_t smem = ((size_t)(C::NST + 2) * C::TILE + (size_t)C::NVAR * C::LFS + (AFFINE ? EB * C::MDP : 0)) * sizeof(double);
+  constexpr size_t smem = ((size_t)(C::NST + 3 + DIM) * C::TILE + (size_t)C::NVAR * C::LFS + (AFFINE ? EB * C::MDP : 0)) * sizeof(double);
   constexpr int MINB = (C::NT <= 128) ? 4 : ((C::NT <= 256) ? 2 : 1);
   auto k = stage_split_kernel<DIM, NP, AFFINE, EB, MINB>;
   static bool attr = false;

@@ -89,3 +89,34 @@ def test_split_form_rhs_stage_and_run(dim, N, cells, curved):
     uc, tc, _, _ = om.run(u0, 5, cfl=0.4)
     assert abs(tg - tc) <= 1e-12 * tc and parity_error(ug, uc).max() <= RUN_TOL
     gm.close()
+
+
+@pytest.mark.parametrize("dim,N,cells", [(2, 3, 6), (3, 4, 3)])
+def test_split_form_rough_states_take_the_logarithm_branch(dim, N, cells):
+    """node-to-node jumps of a factor up to 15 in density and pressure: most pairs leave the series branch of the
+    logarithmic mean (u = ((aL-aR)/(aL+aR))^2 >= 1e-2); one RHS against the oracle"""
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    m = _mesh(dim, N, cells, False)
+    m.volume_form = 1
+    shape = (m.n_elem, dim + 2, (N + 1) ** dim)
+    idx = np.arange(np.prod(shape), dtype=np.uint64).reshape(shape)
+    r = wl.uniform(wl.SEED, 77, idx)
+    rho, p = 0.2 + 2.8 * r[:, 0], 0.2 + 4.8 * r[:, -1]
+    vel = 2.0 * r[:, 1:1 + dim] - 1.0
+    u0 = np.empty(shape)
+    u0[:, 0] = rho
+    u0[:, 1:1 + dim] = rho[:, None] * vel
+    u0[:, -1] = p / 0.4 + 0.5 * rho * (vel ** 2).sum(axis=1)
+    ratio = rho[:, 1:] / rho[:, :-1]
+    assert (np.abs((ratio - 1) / (ratio + 1)) > 0.1).mean() > 0.5      # the logarithm branch is exercised
+    om, gm = oracle.OracleMesh(m), mb.MarutMesh(m)
+    u = torch.from_numpy(u0).cuda()
+    du = torch.empty_like(u)
+    gm.rhs(u, du)
+    torch.cuda.synchronize()
+    assert parity_error(du.cpu().numpy(), om.rhs(u0)).max() <= RHS_TOL
+    gm.close()
