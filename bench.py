@@ -332,7 +332,7 @@ def run_cuda(args):
                 prof = json.load(open(tpath))
             except Exception:
                 prof = {}
-        kernels = {0: "stage_node_kernel (fused Euler stage)", 1: "gradient_kernel + stage_phys_kernel (BR1 gradient sweep + fused NS stage)",
+        kernels = {0: "stage_split_kernel (fused Euler stage, split-form volume integral)" if getattr(mesh, "volume_form", 0) else "stage_node_kernel (fused Euler stage)", 1: "gradient_kernel + stage_phys_kernel (BR1 gradient sweep + fused NS stage)",
                    2: "eos_kernel + stage_phys_kernel (mixture temperature + fused reacting stage)"}[mesh.physics]
         roof = {"bound": "hbm", "kernel": "marut_ssprk_stage: " + kernels, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": prof.get(args.workload), "peak_source": peak_src, "bytes_per_dof_stage": b_alg,
@@ -340,8 +340,8 @@ def run_cuda(args):
         if mesh.physics == 1:
             roof["single_sweep_bytes_per_dof_stage"] = single_sweep_bytes_per_dof_stage(mesh, affine)
             roof["frac_vs_single_sweep_bytes"] = roof["single_sweep_bytes_per_dof_stage"] * n_dof / (stage_ms_avg * 1e-3) / 1e9 / peak
-        if mesh.physics == 2:
-            # ALU-bound (chemistry): executed FP64 flops per stage from the committed ncu capture over the live time
+        if mesh.physics == 2 or getattr(mesh, "volume_form", 0):
+            # ALU-bound (chemistry / two-point volume fluxes): executed FP64 flops per stage from the committed ncu capture over the live time
             flops = prof.get(args.workload + "_fp64_flops_per_stage")
             pk = fp64_peak_tflops((clocks or {}).get("sm_max_mhz") or 1965.0)
             ach = flops / (stage_ms_avg * 1e-3) / 1e12 if flops else None
