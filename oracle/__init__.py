@@ -75,6 +75,10 @@ def _setup(L):
         L.oracle_temperature.argtypes = [vp, vp, C.c_double]
         L.oracle_species_thermo.argtypes = [vp, C.c_int, C.c_double, vp]
         L.oracle_num_threads.restype = C.c_int
+        L.oracle_chem_implicit.restype = C.c_int
+        L.oracle_chem_implicit.argtypes = [vp, vp, C.c_double]
+        L.oracle_chem_implicit_node.restype = C.c_int
+        L.oracle_chem_implicit_node.argtypes = [vp, vp, C.c_double, C.c_double]
         L.oracle_set_volume_form.restype = C.c_int
         L.oracle_set_volume_form.argtypes = [vp, C.c_int]
         L.oracle_logmean.restype = C.c_double
@@ -154,6 +158,12 @@ class MechHandle:
         rho_s = _f64(rho_s)
         return lib().oracle_temperature(self.ptr, _p(rho_s), e_int)
 
+    def implicit_step(self, rho_s, e_int, dt):
+        """backward-Euler Newton source step of one node: returns (rho_s after dt, sweeps)"""
+        y = _f64(rho_s).copy()
+        it = lib().oracle_chem_implicit_node(self.ptr, _p(y), float(e_int), float(dt))
+        return y, it
+
     def species_thermo(self, s, T):
         out = np.zeros(5)
         lib().oracle_species_thermo(self.ptr, s, T, _p(out))
@@ -211,6 +221,14 @@ class OracleMesh:
 
     def chem_source(self, u):
         return self._call(self.L.oracle_chem_source, u)
+
+    def chem_implicit(self, u, dt):
+        """implicit source substep on every node (a copy of u is advanced); returns (u, worst sweep count)"""
+        u = _f64(u).copy()
+        it = self.L.oracle_chem_implicit(self.h, _p(u), float(dt))
+        if it < 0:
+            raise ValueError("chem_implicit needs a REACTING_EULER mesh")
+        return u, it
 
     def br1_gradient(self, u):
         m = self.mesh

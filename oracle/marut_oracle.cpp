@@ -785,6 +785,75 @@ static void chem_source(const Mesh &m, const double *u, double *s, bool accumula
     }
 }
 // the semi-discrete operator L(U,t); t unused (no time-dependent BC/source)
+// O15. Implicit source substep S_dt (eq. 24-25), single-temperature reading
+// (R12): per node the reduced state Y = (rho_1..rho_Ns) is advanced by Newton iteration on the
+// backward-Euler residual R(Y*) = Y* - Y^n - dt S_Y(Y*), S_Y = omega(T(Y*), Y*); total density, momentum and total
+// energy are fixed parameters.  One sweep: (i) temperature from the caloric equation with the fixed
+// momentum and energy, (ii) rates, (iii) Jacobian column by column from forward differences with
+// eps_k = max(1e-7 |Y_k|, 1e-12), (iv) Y* <- Y* - J^-1 R by Gauss-Jordan elimination.
+// Silent in the paper (R14): start Y* = Y^n; partial pivoting; stop when max_k |dY_k| <= 1e-13 rho,
+// at most 50 sweeps.  Returns the number of sweeps.
+static void implicit_residual(const Mech &k, const double *Y, const double *Yn, double dt, double e_kin_fixed_E,
+                              double *R) {
+  // e_kin_fixed_E = E - 1/2 rho |u|^2 with rho, momentum, E fixed (the internal energy available to the mixture)
+  const double T = temperature_from_energy(k, Y, e_kin_fixed_E);
+  double om[MAXV];
+  production_rates(k, T, Y, om);
+  for (int s = 0; s < k.ns; ++s) R[s] = Y[s] - Yn[s] - dt * om[s];
+}
+static int chem_implicit_node(const Mech &k, double *Y, double e_int, double dt) {
+  const int ns = k.ns;
+  double Yn[MAXV], rho = 0.0;
+  for (int s = 0; s < ns; ++s) { Yn[s] = Y[s]; rho += Y[s]; }
+  int it = 0;
+  for (it = 1; it <= 50; ++it) {
+    double R[MAXV], A[MAXV][MAXV + 1];
+    implicit_residual(k, Y, Yn, dt, e_int, R);
+    for (int c = 0; c < ns; ++c) {
+      const double eps = std::max(1e-7 * std::fabs(Y[c]), 1e-12);
+      double Yp[MAXV], Rp[MAXV];
+      for (int s = 0; s < ns; ++s) Yp[s] = Y[s];
+      Yp[c] += eps;
+      implicit_residual(k, Yp, Yn, dt, e_int, Rp);
+      for (int s = 0; s < ns; ++s) A[s][c] = (Rp[s] - R[s]) / eps;
+    }
+    for (int s = 0; s < ns; ++s) A[s][ns] = R[s];
+    // Gauss-Jordan with partial pivoting on [J | R]
+    for (int c = 0; c < ns; ++c) {
+      int piv = c;
+      for (int r = c + 1; r < ns; ++r) if (std::fabs(A[r][c]) > std::fabs(A[piv][c])) piv = r;
+      if (piv != c) for (int q = 0; q <= ns; ++q) std::swap(A[c][q], A[piv][q]);
+      const double inv = 1.0 / A[c][c];
+      for (int q = c; q <= ns; ++q) A[c][q] *= inv;
+      for (int r = 0; r < ns; ++r) {
+        if (r == c) continue;
+        const double f = A[r][c];
+        for (int q = c; q <= ns; ++q) A[r][q] -= f * A[c][q];
+      }
+    }
+    double dmax = 0.0;
+    for (int s = 0; s < ns; ++s) { Y[s] -= A[s][ns]; dmax = std::max(dmax, std::fabs(A[s][ns])); }
+    if (dmax <= 1e-13 * rho) break;
+  }
+  return it;
+}
+static int chem_implicit(const Mesh &m, double *u, double dt) {
+  const int nn = m.nn, ns = m.ns, d = m.dim, nvar = m.nvar;
+  int worst = 0;
+#pragma omp parallel for schedule(static) reduction(max : worst)
+  for (long e = 0; e < m.ne; ++e)
+    for (int p = 0; p < nn; ++p) {
+      double U[MAXV]; gather(m, u, e, p, U);
+      double rho = 0.0, m2 = 0.0;
+      for (int s = 0; s < ns; ++s) rho += U[s];
+      for (int c = 0; c < d; ++c) m2 += U[ns + c] * U[ns + c];
+      const double e_int = U[ns + d] - 0.5 * m2 / rho;
+      const int it = chem_implicit_node(m.mech, U, e_int, dt);
+      worst = std::max(worst, it);
+      for (int s = 0; s < ns; ++s) u[((size_t)e * nvar + s) * nn + p] = U[s];
+    }
+  return worst;
+}
 static void rhs_full(const Mesh &m, const double *u, double *du) {
   rhs_inviscid(m, u, du);
   if (m.physics == NAVIER_STOKES) rhs_viscous_add(m, u, du);
@@ -886,6 +955,15 @@ int oracle_set_volume_form(void *h, int form) {
   if (form < 0 || form > 1 || (form == 1 && m->physics == REACTING_EULER)) return 1;
   m->volume_form = form;
   return 0;
+}
+int oracle_chem_implicit(void *h, double *u, double dt) {
+  Mesh *m = (Mesh *)h;
+  if (m->physics != REACTING_EULER) return -1;
+  return chem_implicit(*m, u, dt);
+}
+int oracle_chem_implicit_node(const oracle_mech_desc *d, double *rho_s, double e_int, double dt) {
+  Mech k = to_mech(d);
+  return chem_implicit_node(k, rho_s, e_int, dt);
 }
 double oracle_logmean(double aL, double aR) { return logmean(aL, aR); }
 void oracle_ranocha(int dim, double gamma, const double *UL, const double *UR, const double *nv, double *F) {
