@@ -109,6 +109,14 @@ marut_status marut_max_dt(marut_mesh *mesh, const double *u, double cfl, double 
  * momentum and energy rows 0.  REACTING_EULER meshes only (else EINVAL). */
 marut_status marut_chem_source(marut_mesh *mesh, const double *u, double *s, void *cuda_stream);
 
+/* Implicit source substep S_dt of the Strang split (eq. 24-25; R14):
+ * per node, Newton on the backward-Euler residual Y* - Y^n - dt*omega(T(Y*), Y*) of the partial densities with a
+ * forward-difference Jacobian (eps_k = max(1e-7|Y_k|, 1e-12)) and Gauss-Jordan elimination; total density, momentum
+ * and total energy are fixed.  u (DEVICE, layout as above) is advanced IN PLACE: only its species rows change.
+ * sweeps_out (HOST, may be NULL): largest number of Newton sweeps any node needed; when given, the call synchronises
+ * the stream and returns ENOTFINITE if a node did not converge within 50 sweeps.  REACTING_EULER meshes only. */
+marut_status marut_chem_implicit(marut_mesh *mesh, double *u, double dt, int *sweeps_out, void *cuda_stream);
+
 /* Volume-integral form of L.  MARUT_VOLUME_STRONG (default): eq. 9, the standard strong form.
  * MARUT_VOLUME_SPLIT_RANOCHA: the entropy-stable split form, eq. 10,
  *   R_i = -(2/J_i) sum_l sum_m D_{i_l m} F#(U_i, U_m; 1/2 (Ja^l_i + Ja^l_m)),

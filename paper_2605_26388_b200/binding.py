@@ -15,7 +15,7 @@ _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA"
 
 # every symbol include/marut.h declares
 SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt",
-           "marut_chem_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
+           "marut_chem_source", "marut_chem_implicit", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
            "marut_last_error"]
 
 
@@ -64,6 +64,8 @@ def lib():
         L.marut_max_dt.argtypes = [vp, vp, dbl, C.POINTER(dbl), vp]
         L.marut_chem_source.restype = C.c_int
         L.marut_chem_source.argtypes = [vp, vp, vp, vp]
+        L.marut_chem_implicit.restype = C.c_int
+        L.marut_chem_implicit.argtypes = [vp, vp, dbl, C.POINTER(C.c_int), vp]
         L.marut_set_volume_form.restype = C.c_int
         L.marut_set_volume_form.argtypes = [vp, C.c_int]
         L.marut_get_metrics.restype = C.c_int
@@ -152,6 +154,12 @@ def marut_chem_source(h, u, s, stream=None):
     _check(lib().marut_chem_source(h, _dev(u), _dev(s), _stream(stream)))
 
 
+def marut_chem_implicit(h, u, dt, stream=None, want_sweeps=True):
+    sw = C.c_int(0)
+    _check(lib().marut_chem_implicit(h, _dev(u), dt, C.byref(sw) if want_sweeps else None, _stream(stream)))
+    return sw.value
+
+
 def marut_set_volume_form(h, form):
     _check(lib().marut_set_volume_form(h, int(form)))
 
@@ -192,6 +200,9 @@ class MarutMesh:
 
     def chem_source(self, u, s, stream=None):
         marut_chem_source(self.h, u, s, stream)
+
+    def chem_implicit(self, u, dt, stream=None, want_sweeps=True):
+        return marut_chem_implicit(self.h, u, dt, stream, want_sweeps)
 
     def step(self, u, ua, ub, dt, t=0.0, stream=None):
         ssprk3_step(self.h, u, ua, ub, dt, t, stream)

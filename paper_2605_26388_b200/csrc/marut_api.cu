@@ -552,6 +552,29 @@ extern "C" marut_status marut_chem_source(marut_mesh *m, const double *u, double
   return MARUT_OK;
 }
 
+extern "C" marut_status marut_chem_implicit(marut_mesh *m, double *u, double dt, int *sweeps_out, void *stream) {
+  if (!m || !u) return fail(MARUT_EINVAL, "NULL argument");
+  if (m->physics != MARUT_REACTING_EULER) return fail(MARUT_EINVAL, "marut_chem_implicit needs a REACTING_EULER mesh");
+  if (!(dt >= 0.0)) return fail(MARUT_EINVAL, "dt must be >= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  int *d_sw = reinterpret_cast<int *>(m->d_red + 3);
+  CUDA_TRY(cudaMemsetAsync(d_sw, 0, sizeof(unsigned long long), st));
+  const long total = m->ne * m->nn;
+  const unsigned grid = (unsigned)std::min<long>((total + 127) / 128, 148L * 8);
+  if (m->dim == 2) chem_implicit_kernel<2, 5><<<grid, 128, 0, st>>>(u, m->d_mech, dt, m->ne, m->nn, d_sw);
+  else chem_implicit_kernel<3, 5><<<grid, 128, 0, st>>>(u, m->d_mech, dt, m->ne, m->nn, d_sw);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "implicit chemistry kernel: %s", cudaGetErrorString(e));
+  m->launches++;
+  if (sweeps_out) {
+    CUDA_TRY(cudaMemcpyAsync(m->h_red + 3, d_sw, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    *sweeps_out = (int)(m->h_red[3] & 0xffffffffu);
+    if (*sweeps_out > 50) return fail(MARUT_ENOTFINITE, "implicit chemistry: Newton did not converge in 50 sweeps");
+  }
+  return MARUT_OK;
+}
+
 // ------------------------------------------------------------------------------------ time step
 template <int DIM>
 static cudaError_t run_wave_speed(marut_mesh *m, const double *u, unsigned grid, cudaStream_t st) {

@@ -419,6 +419,93 @@ __global__ void __launch_bounds__(256) chem_kernel(const double *__restrict__ u,
   }
 }
 
+// Implicit source substep S_dt (eq. 24-25; R14): per node, Newton on
+// the backward-Euler residual R(Y*) = Y* - Y^n - dt omega(T(Y*), Y*) of the partial densities, with total density,
+// momentum and total energy fixed.  One sweep = residual, NSP forward-difference Jacobian columns
+// (eps_k = max(1e-7 |Y_k|, 1e-12)), Gauss-Jordan with partial pivoting -- all in registers; the only global traffic
+// is one read of the nodal state and one write of its species rows.  In place.
+template <int NSP>
+__device__ __forceinline__ void implicit_residual(const MechDev &m, const double *Y, const double *Yn, double dt, double e_int,
+                                                  double *Xs, int stride, double *R) {
+  const double T = temperature_newton<NSP>(m, Y, e_int);
+  double om[NSP];
+  production_rates_listed<NSP>(m, T, Y, Xs, stride, om);
+#pragma unroll
+  for (int s = 0; s < NSP; ++s) R[s] = Y[s] - Yn[s] - dt * om[s];
+}
+template <int DIM, int NSP>
+__global__ void __launch_bounds__(128) chem_implicit_kernel(double *__restrict__ u, const MechDev *__restrict__ mech_g, double dt,
+                                                            long ne, int nn, int *__restrict__ max_sweeps) {
+  constexpr int NVAR = NSP + DIM + 1;
+  __shared__ MechDev mech;
+  __shared__ double Xs[NSP * 128];
+  load_mech(&mech, mech_g);
+  const long total = ne * nn;
+  int worst = 0;
+  for (long g = (long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
+    const long e = g / nn;
+    const int p = (int)(g - e * nn);
+    double U[NVAR], Y[NSP], Yn[NSP];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = u[(e * NVAR + v) * nn + p];
+    const double e_int = internal_energy<DIM, NSP>(U);
+    double rho = 0.0;
+#pragma unroll
+    for (int s = 0; s < NSP; ++s) { Y[s] = Yn[s] = U[s]; rho += U[s]; }
+    int it = 1;
+    for (; it <= 50; ++it) {
+      double R[NSP], A[NSP][NSP + 1];
+      implicit_residual<NSP>(mech, Y, Yn, dt, e_int, Xs + threadIdx.x, 128, R);
+#pragma unroll
+      for (int c = 0; c < NSP; ++c) {
+        const double eps = fmax(1e-7 * fabs(Y[c]), 1e-12);
+        double Yp[NSP], Rp[NSP];
+#pragma unroll
+        for (int s = 0; s < NSP; ++s) Yp[s] = (s == c) ? Y[s] + eps : Y[s];
+        implicit_residual<NSP>(mech, Yp, Yn, dt, e_int, Xs + threadIdx.x, 128, Rp);
+#pragma unroll
+        for (int s = 0; s < NSP; ++s) A[s][c] = (Rp[s] - R[s]) / eps;
+      }
+#pragma unroll
+      for (int s = 0; s < NSP; ++s) A[s][NSP] = R[s];
+      // Gauss-Jordan with partial pivoting; row swaps as predicated exchanges (no dynamically indexed registers)
+#pragma unroll
+      for (int c = 0; c < NSP; ++c) {
+        int piv = c;
+        double best = fabs(A[c][c]);
+#pragma unroll
+        for (int r = c + 1; r < NSP; ++r)
+          if (fabs(A[r][c]) > best) { best = fabs(A[r][c]); piv = r; }
+#pragma unroll
+        for (int r = c + 1; r < NSP; ++r)
+          if (r == piv) {
+#pragma unroll
+            for (int q = 0; q <= NSP; ++q) { const double t = A[c][q]; A[c][q] = A[r][q]; A[r][q] = t; }
+          }
+        const double inv = 1.0 / A[c][c];
+#pragma unroll
+        for (int q = c; q <= NSP; ++q) A[c][q] *= inv;
+#pragma unroll
+        for (int r = 0; r < NSP; ++r) {
+          if (r == c) continue;
+          const double f = A[r][c];
+#pragma unroll
+          for (int q = c; q <= NSP; ++q) A[r][q] -= f * A[c][q];
+        }
+      }
+      double dmax = 0.0;
+#pragma unroll
+      for (int s = 0; s < NSP; ++s) { Y[s] -= A[s][NSP]; dmax = fmax(dmax, fabs(A[s][NSP])); }
+      if (dmax <= 1e-13 * rho) break;
+    }
+    worst = max(worst, it);
+#pragma unroll
+    for (int s = 0; s < NSP; ++s) u[(e * NVAR + s) * nn + p] = Y[s];
+  }
+  worst = __reduce_max_sync(0xffffffffu, worst);
+  if ((threadIdx.x & 31) == 0) atomicMax(max_sweeps, worst);
+}
+
 // ======================================================================================
 // max wave speed / max diffusivity (a10; eq. 17-18): warp-shuffle reduction, one atomicMax per CTA.
 // red[0] = max(|u|_2 + a) ; red[1] = max(mu/rho) ; red[2] = count of non-finite/non-positive speeds

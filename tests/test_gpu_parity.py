@@ -133,3 +133,24 @@ def test_error_codes(torch, mb):
         gm.max_dt(un, 0.5)
     assert e.value.status == 5
     gm.close()
+
+
+@pytest.mark.parametrize("factor", [0.5, 20.0])
+def test_chem_implicit_parity(factor, torch, mb, oracle):
+    """implicit source substep (marut_chem_implicit) against the oracle's Newton, at a step below
+    and far above the fastest chemical time of the field"""
+    c = wl.make_case("c5", cells=3)
+    om = oracle.OracleMesh(c.mesh)
+    gm = mb.MarutMesh(c.mesh)
+    dt = factor * 20.0 * om.max_dt(c.u0, 0.5)      # the c5 recipe puts the CFL step at 0.05 x the depletion time
+    ref, it_ref = om.chem_implicit(c.u0, dt)
+    u = torch.from_numpy(c.u0).cuda()
+    it = gm.chem_implicit(u, dt)
+    g = u.cpu().numpy()
+    assert abs(it - it_ref) <= 1 and it < 50
+    assert np.array_equal(g[:, 5:, :], c.u0[:, 5:, :])                       # momentum / energy rows untouched
+    assert parity_error(g[:, :5, :], ref[:, :5, :]).max() <= RHS_TOL
+    assert np.abs(g[:, :5, :] - c.u0[:, :5, :]).max() > 1e-3 * np.abs(c.u0[:, :5, :]).max()   # the step did something
+    with pytest.raises(mb.MarutError):
+        mb.MarutMesh(wl.make_case("c1", cells=4).mesh).chem_implicit(u, dt)  # not a reacting mesh
+    gm.close()
