@@ -105,3 +105,25 @@ def test_full_size_conservation_c2():
     scale = np.einsum("evn,en,n->v", np.abs(d), J, W)
     assert np.all(np.abs(total) <= 1e-12 * scale), (total, scale)
     gm.close()
+
+
+def test_full_size_chem_implicit_c5():
+    """implicit source substep on the full c5 field, every node against the oracle"""
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    c = wl.make_case("c5")
+    om = oracle.OracleMesh(c.mesh)
+    gm = mb.MarutMesh(c.mesh)
+    dt = 100.0 * om.max_dt(c.u0, c.cfl)        # ~5 x the fastest depletion time of the field: stiff for an explicit step
+    ref, it_ref = om.chem_implicit(c.u0, dt)
+    u = torch.from_numpy(c.u0).cuda()
+    it = gm.chem_implicit(u, dt)
+    g = u.cpu().numpy()
+    print(f"c5 implicit substep: dt {dt:.3e}, sweeps gpu {it} oracle {it_ref}")
+    assert abs(it - it_ref) <= 1 and it < 50
+    assert np.array_equal(g[:, 5:, :], c.u0[:, 5:, :])
+    assert parity_error(g[:, :5, :], ref[:, :5, :]).max() <= RHS_TOL
+    gm.close()
