@@ -58,18 +58,6 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   const int nel = (int)((P.ne - e0 < EB) ? (P.ne - e0) : EB);
   const int ntask = nel * NFN, nline = nel * NLT;
 
-  // L2 prefetch of the tile a CTA launched ~one wave later will read
-  if (tid == 0) {
-    const long ep = e0 + (long)MARUT_L2_PREFETCH * EB;
-    if (MARUT_L2_PREFETCH && ep + EB < P.ne) {
-      const size_t nb = (size_t)EB * NN * sizeof(double);
-      l2_prefetch(P.u_in + ep * NVAR * NN, nb * NVAR);
-      if (P.ca != 0.0) l2_prefetch(P.u_n + ep * NVAR * NN, nb * NVAR);
-      if constexpr (PHYS == PH_NS) l2_prefetch(P.S + ep * Tau<DIM>::NTAU * NN, nb * Tau<DIM>::NTAU);
-      if constexpr (PHYS == PH_REACT) l2_prefetch(P.Taux + ep * NN, nb);
-      if constexpr (!AFFINE) l2_prefetch(P.metric + ep * MD * NN, nb * MD);
-    }
-  }
   // first face task of this thread: connectivity load first (the neighbour gather depends on it)
   const bool has0 = tid < ntask;
   const FaceTask t0 = decode_task<DIM, NP>(has0 ? tid : 0);
