@@ -42,7 +42,8 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
   extern __shared__ __align__(16) double smem[];
   double *Ust = smem;                       // [NVAR + 3][TILE]  U, 1/rho, p, a
   double *Lns = Ust + NST * TILE;           // [3 + DIM][TILE]   ln rho, ln(rho/p), rho/p, velocity
-  double *Lft = Lns + (3 + DIM) * TILE;             // [NVAR][LFS]       lifts of the face nodes
+  double *Pair = Lns + (3 + DIM) * TILE;    // [DIM][NP/2][NVAR][TILE] two-point fluxes left for the partner node
+  double *Lft = Pair + DIM * (NP / 2) * NVAR * TILE;             // [NVAR][LFS]       lifts of the face nodes
   double *Msm = Lft + NVAR * C::LFS;        // affine: [EB][MDP] Ja, 1/J, |Ja^l|
 
   const int tid = threadIdx.x;
@@ -91,7 +92,11 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
   if (has0) gather_exterior<DIM, NP, NVAR>(P, t0, cn0, Up0);
   __syncthreads();
 
-  // ---- phase V: split-form volume term (eq. 10)
+  // ---- phase V: split-form volume term (eq. 10).  F#(U_i, U_m) = F#(U_m, U_i) with the same averaged metric, so every
+  // pair of a line is evaluated ONCE: node i takes its partners at cyclic distance s = 1..NP/2 (m = (i + s) mod NP;
+  // for even NP the distance NP/2 only from the lower half), adds 2 D_im F# to its own residual and leaves F# in the
+  // pair buffer for node m, which adds 2 D_mi F# after the barrier.  Balanced: NP/2 evaluations per direction.
+  constexpr int NS = NP / 2;
   double R[NVAR];
 #pragma unroll
   for (int v = 0; v < NVAR; ++v) R[v] = 0.0;
@@ -105,9 +110,21 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
       double Ji[DIM];
 #pragma unroll
       for (int c = 0; c < DIM; ++c) Ji[c] = AFFINE ? Msm[el * MDP + l * DIM + c] : __ldg(&P.metric[(e * MD + l * DIM + c) * NN + p]);
+      if (ql == 0 || ql == NP - 1) {
+        // diagonal term 2 D_ii F#(U_i, U_i) = 2 D_ii F_inv(U_i).Ja^l_i (D_ii = 0 at interior LGL nodes)
+        const double d = P.D[ql * NP + ql];
+        double vn = 0.0;
 #pragma unroll
-      for (int m = 0; m < NP; ++m) {
-        if (m == ql && ql != 0 && ql != NP - 1) continue;   // D_ii = 0 at interior LGL nodes
+        for (int c = 0; c < DIM; ++c) vn += vi[c] * Ji[c];
+        R[0] += d * (U[0] * vn);
+#pragma unroll
+        for (int c = 0; c < DIM; ++c) R[1 + c] += d * (U[1 + c] * vn + pi_ * Ji[c]);
+        R[1 + DIM] += d * ((U[1 + DIM] + pi_) * vn);
+      }
+#pragma unroll
+      for (int sd = 1; sd <= NS; ++sd) {
+        if ((NP % 2 == 0) && sd == NS && ql >= NS) continue;
+        const int m = (ql + sd >= NP) ? ql + sd - NP : ql + sd;
         const int pm = base + m * st;            // stash index of the partner node
         const double rm = Ust[pm], pmm = Ust[(NVAR + 1) * TILE + pm];
         double nv[DIM], vavg[DIM], vn = 0.0, v2 = 0.0, pvn = 0.0;
@@ -127,12 +144,37 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
         const double rho_ln = nr / dr;
         const double eint = inv_gm1 * (db / nb);                      // 1 / ((gamma-1) {{T^-1}}^ln)
         const double pavg = 0.5 * (pi_ + pmm);
-        const double d = P.D[ql * NP + m];   // runtime row: constant-bank load with a lane-dependent index
         const double mf = rho_ln * vn;
-        R[0] += d * mf;
+        double F[NVAR];
+        F[0] = mf;
 #pragma unroll
-        for (int c = 0; c < DIM; ++c) R[1 + c] += d * (mf * vavg[c] + pavg * nv[c]);
-        R[1 + DIM] += d * ((eint + 0.5 * v2) * mf + pvn);
+        for (int c = 0; c < DIM; ++c) F[1 + c] = mf * vavg[c] + pavg * nv[c];
+        F[1 + DIM] = (eint + 0.5 * v2) * mf + pvn;
+        const double d = P.D[ql * NP + m];
+        double *pb = Pair + ((l * NS + (sd - 1)) * NVAR) * TILE + tid;
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) {
+          R[v] += d * F[v];
+          pb[v * TILE] = F[v];
+        }
+      }
+    }
+  }
+  __syncthreads();
+  if (active) {
+#pragma unroll
+    for (int l = 0; l < DIM; ++l) {
+      const int ql = (l == 0) ? qi : ((l == 1) ? qj : qk);
+      const int st = G::stride(l);
+      const int base = tid - ql * st;
+#pragma unroll
+      for (int sd = 1; sd <= NS; ++sd) {
+        const int i = (ql - sd < 0) ? ql - sd + NP : ql - sd;   // the node that evaluated the pair (i, ql)
+        if ((NP % 2 == 0) && sd == NS && i >= NS) continue;
+        const double d = P.D[ql * NP + i];
+        const double *pb = Pair + ((l * NS + (sd - 1)) * NVAR) * TILE + base + i * st;
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) R[v] += d * pb[v * TILE];
       }
     }
 #pragma unroll
@@ -186,7 +228,7 @@ template <int DIM, int NP, bool AFFINE>
 cudaError_t launch_stage_split_t(const StageParams &P, cudaStream_t st) {
   constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
   using C = NodeCfg<DIM, NP, 1, EB>;
-  constexpr size_t smem = ((size_t)(C::NST + 3 + DIM) * C::TILE + (size_t)C::NVAR * C::LFS + (AFFINE ? EB * C::MDP : 0)) * sizeof(double);
+  constexpr size_t smem = ((size_t)(C::NST + 3 + DIM + DIM * (NP / 2) * C::NVAR) * C::TILE + (size_t)C::NVAR * C::LFS + (AFFINE ? EB * C::MDP : 0)) * sizeof(double);
   constexpr int MINB = (C::NT <= 128) ? 4 : ((C::NT <= 256) ? 2 : 1);
   auto k = stage_split_kernel<DIM, NP, AFFINE, EB, MINB>;
   static bool attr = false;
