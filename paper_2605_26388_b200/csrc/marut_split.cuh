@@ -181,6 +181,15 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
     for (int v = 0; v < NVAR; ++v) R[v] *= 2.0;
   }
 
+  // u_n for the final combination: issued before the face tasks, consumed after the last barrier (u_out may alias
+  // u_n: only this thread writes these locations, later)
+  double Un[NVAR];
+  const bool use_un = (P.ca != 0.0);
+  if (active && use_un) {
+    const double *np_ = P.u_n + e * NVAR * NN + p;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Un[v] = np_[v * NN];
+  }
   // ---- phase S: face nodes, densely mapped
   if (has0) euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
   for (int g = tid + NT; g < ntask; g += NT) {
@@ -214,10 +223,9 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
   }
   const double invJ = AFFINE ? Msm[el * MDP + DIM * DIM] : __ldg(&P.metric[(e * MD + DIM * DIM) * NN + p]);
   double *op = P.u_out + e * NVAR * NN + p;
-  if (P.ca != 0.0) {
-    const double *np_ = P.u_n + e * NVAR * NN + p;
+  if (use_un) {
 #pragma unroll
-    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.ca * np_[v * NN] + (P.cb * U[v] + P.cc * (0.0 - invJ * R[v]));
+    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.ca * Un[v] + (P.cb * U[v] + P.cc * (0.0 - invJ * R[v]));
   } else {
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) op[v * NN] = P.cb * U[v] + P.cc * (0.0 - invJ * R[v]);
