@@ -258,20 +258,30 @@ __device__ __forceinline__ void line_deriv(const StageParams &P, const double *f
   }
 }
 
+// ---- compile-time switches of the node kernel; the defaults are the measured best (profiles/r01_c2_stage.md)
 #ifndef MARUT_L2_PREFETCH
-#define MARUT_L2_PREFETCH 1024   // elements-per-CTA units ahead; 0 = off
+#define MARUT_L2_PREFETCH 1024   // L2 bulk prefetch of the tile this many CTAs ahead; 0 = off            (on: -3 %)
 #endif
 #ifndef MARUT_PREFETCH_UN
-#define MARUT_PREFETCH_UN 0
+#define MARUT_PREFETCH_UN 0      // 1: load u_n of the last-pass task at kernel start                      (+8 %)
+#endif
+#ifndef MARUT_EARLY_GATHER
+#define MARUT_EARLY_GATHER 0     // 1: issue the neighbour gather before the flux arithmetic of phase N    (+4 %)
+#endif
+#ifndef MARUT_ABLATE
+#define MARUT_ABLATE 0           // timing ablations only (results are not physics): 1 no face tasks, 2 no xi/eta
+#endif                           // passes, 3 data-movement skeleton
+#ifndef MARUT_NODE_MINB128
+#define MARUT_NODE_MINB128 6     // CTAs of 128 threads per SM the register allocation is sized for (5..7: same speed)
 #endif
 // last-pass task t -> (element in tile, variable, line): 3-D: ij = i + NP*j, lanes run over ij first;
 // 2-D: ij = i, lane order (i, element, v)
 template <int DIM, int NP>
 struct LastPass {
   static constexpr int NL = (DIM == 3) ? NP * NP : NP;
-  // 3-D, NP = 5: one warp per (element, variable) with 25 of 32 lanes active -- no warp straddles two variable
-  // planes, so the shared-memory line reads are conflict-free and every global access is one 200-byte run
-  static constexpr int SLOT = NL;   // (a 32-lane slot per plane for NP = 5 removes the bank conflicts but costs a second round: slower)
+  // lanes per (element, variable) plane.  A 32-lane slot for NP = 5 (25 of 32 lanes active, no warp straddling two
+  // planes) removes the remaining bank conflicts of the last pass but needs a second round on one warp: slower.
+  static constexpr int SLOT = NL;
 };
 template <int DIM, int NP, int NVAR, int EB>
 __device__ __forceinline__ void last_pass_task(int t, int &el, int &v, int &ij) {
@@ -288,15 +298,6 @@ __device__ __forceinline__ void last_pass_task(int t, int &el, int &v, int &ij) 
     v = t / (NP * EB);
   }
 }
-#ifndef MARUT_EARLY_GATHER
-#define MARUT_EARLY_GATHER 0
-#endif
-#ifndef MARUT_ABLATE
-#define MARUT_ABLATE 0
-#endif
-#ifndef MARUT_NODE_MINB128
-#define MARUT_NODE_MINB128 6
-#endif
 
 template <int DIM, int NP, bool AFFINE, int EB, int MINB>
 __global__ void __launch_bounds__((NodeCfg<DIM, NP, 1, EB>::NT), MINB)
