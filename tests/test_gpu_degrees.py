@@ -120,3 +120,33 @@ def test_split_form_rough_states_take_the_logarithm_branch(dim, N, cells):
     torch.cuda.synchronize()
     assert parity_error(du.cpu().numpy(), om.rhs(u0)).max() <= RHS_TOL
     gm.close()
+
+
+@pytest.mark.parametrize("N,split", [(1, False), (2, False), (4, False), (5, False), (3, True), (4, True)])
+def test_quadtree_mortars_and_boundaries_other_degrees(N, split):
+    """2:1 mortar faces and prescribed-state boundary faces (a3, a4) at degrees other than config 4's N = 3, with the
+    strong and the split-form volume integral: RHS, dt and five steps against the oracle"""
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+    from parity_util import RUN_TOL, gpu_run
+
+    m = wl.quadtree_mesh(N, base=(16, 4), band=0.15, jitter=0.3)
+    m.bc_state = wl.shock_states(m.gamma)
+    if split:
+        m.volume_form = 1
+    assert len(m.mortar) > 0 and len(m.bface) > 0
+    u0 = wl.mach10_shock(m, half_width=6.0 * m.info["h_fine"])
+    om, gm = oracle.OracleMesh(m), mb.MarutMesh(m)
+    u = torch.from_numpy(u0).cuda()
+    du = torch.empty_like(u)
+    gm.rhs(u, du)
+    torch.cuda.synchronize()
+    assert parity_error(du.cpu().numpy(), om.rhs(u0)).max() <= RHS_TOL
+    dt = om.max_dt(u0, 0.3)
+    assert abs(gm.max_dt(u, 0.3) - dt) <= 1e-13 * dt
+    ug, tg = gpu_run(gm, u0, 5, 0.3, torch)
+    uc, tc, _, _ = om.run(u0, 5, cfl=0.3)
+    assert abs(tg - tc) <= 1e-12 * tc and parity_error(ug, uc).max() <= RUN_TOL
+    gm.close()
