@@ -117,6 +117,11 @@ marut_status marut_chem_source(marut_mesh *mesh, const double *u, double *s, voi
  * the stream and returns ENOTFINITE if a node did not converge within 50 sweeps.  REACTING_EULER meshes only. */
 marut_status marut_chem_implicit(marut_mesh *mesh, double *u, double dt, int *sweeps_out, void *cuda_stream);
 
+/* REACTING_EULER meshes: whether L(u) of marut_rhs / marut_ssprk_stage includes the explicit chemistry source S(u)
+ * (on != 0, the default) or is the transport operator T alone (on == 0), as the Strang split of eq. 24 needs:
+ *   u^{n+1} = S_{dt/2} o T_dt o S_{dt/2} (u^n) = marut_chem_implicit(dt/2), SSP-RK steps of T, marut_chem_implicit(dt/2). */
+marut_status marut_set_explicit_source(marut_mesh *mesh, int on);
+
 /* Volume-integral form of L.  MARUT_VOLUME_STRONG (default): eq. 9, the standard strong form.
  * MARUT_VOLUME_SPLIT_RANOCHA: the entropy-stable split form, eq. 10,
  *   R_i = -(2/J_i) sum_l sum_m D_{i_l m} F#(U_i, U_m; 1/2 (Ja^l_i + Ja^l_m)),

@@ -75,6 +75,7 @@ def _setup(L):
         L.oracle_temperature.argtypes = [vp, vp, C.c_double]
         L.oracle_species_thermo.argtypes = [vp, C.c_int, C.c_double, vp]
         L.oracle_num_threads.restype = C.c_int
+        L.oracle_set_explicit_source.argtypes = [vp, C.c_int]
         L.oracle_chem_implicit.restype = C.c_int
         L.oracle_chem_implicit.argtypes = [vp, vp, C.c_double]
         L.oracle_chem_implicit_node.restype = C.c_int
@@ -222,6 +223,21 @@ class OracleMesh:
     def chem_source(self, u):
         return self._call(self.L.oracle_chem_source, u)
 
+    def set_explicit_source(self, on):
+        """reacting meshes: whether L(U) includes the chemistry source (default) or is the transport operator only"""
+        self.L.oracle_set_explicit_source(self.h, int(bool(on)))
+
+    def strang_step(self, u, dt):
+        """eq. 24: S_{dt/2} o T_dt o S_{dt/2} with T = one SSP-RK33 step of the transport operator"""
+        self.set_explicit_source(False)
+        try:
+            u, _ = self.chem_implicit(u, 0.5 * dt)
+            u = self.run(u, 1, cfl=0.0, dt=dt)[0]   # cfl = 0: fixed dt
+            u, _ = self.chem_implicit(u, 0.5 * dt)
+        finally:
+            self.set_explicit_source(True)
+        return u
+
     def chem_implicit(self, u, dt):
         """implicit source substep on every node (a copy of u is advanced); returns (u, worst sweep count)"""
         u = _f64(u).copy()
@@ -256,7 +272,8 @@ class OracleMesh:
         return (dt, lam.value) if return_lambda else dt
 
     def run(self, u, nsteps, cfl=0.5, dt=0.0, t0=0.0):
-        """advance a copy of u by nsteps SSPRK3 steps; returns (u, t_end, min_rho, min_p)"""
+        """advance a copy of u by nsteps SSPRK3 steps, dt from the CFL reduction each step if cfl > 0, else the fixed dt;
+        returns (u, t_end, min_rho, min_p)"""
         u = _f64(u).copy()
         mr, mp = C.c_double(0.0), C.c_double(0.0)
         t = self.L.oracle_run(self.h, _p(u), nsteps, cfl, dt, t0, C.addressof(mr), C.addressof(mp))

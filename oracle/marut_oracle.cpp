@@ -286,6 +286,7 @@ struct Mesh {
   Mech mech;
   std::vector<double> Pf[2], Pr_[2];
   double dx_min = 0.0;
+  int explicit_source = 1;      // reacting: 1 = L includes the chemistry source S(U); 0 = transport operator only (Strang split)
   int volume_form = 0;          // 0: standard strong form (eq. 9); 1: entropy-stable split form (eq. 10)
 };
 
@@ -857,7 +858,7 @@ static int chem_implicit(const Mesh &m, double *u, double dt) {
 static void rhs_full(const Mesh &m, const double *u, double *du) {
   rhs_inviscid(m, u, du);
   if (m.physics == NAVIER_STOKES) rhs_viscous_add(m, u, du);
-  if (m.physics == REACTING_EULER) chem_source(m, u, du, true);
+  if (m.physics == REACTING_EULER && m.explicit_source) chem_source(m, u, du, true);
 }
 // O11. time step: dt = min(dt_C, dt_D)
 static double max_dt(const Mesh &m, const double *u, double cfl, double *lam_out) {
@@ -956,6 +957,7 @@ int oracle_set_volume_form(void *h, int form) {
   m->volume_form = form;
   return 0;
 }
+int oracle_set_explicit_source(void *h, int on) { ((Mesh *)h)->explicit_source = on ? 1 : 0; return 0; }
 int oracle_chem_implicit(void *h, double *u, double dt) {
   Mesh *m = (Mesh *)h;
   if (m->physics != REACTING_EULER) return -1;

@@ -15,7 +15,7 @@ _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA"
 
 # every symbol include/marut.h declares
 SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt",
-           "marut_chem_source", "marut_chem_implicit", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
+           "marut_chem_source", "marut_chem_implicit", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
            "marut_last_error"]
 
 
@@ -66,6 +66,8 @@ def lib():
         L.marut_chem_source.argtypes = [vp, vp, vp, vp]
         L.marut_chem_implicit.restype = C.c_int
         L.marut_chem_implicit.argtypes = [vp, vp, dbl, C.POINTER(C.c_int), vp]
+        L.marut_set_explicit_source.restype = C.c_int
+        L.marut_set_explicit_source.argtypes = [vp, C.c_int]
         L.marut_set_volume_form.restype = C.c_int
         L.marut_set_volume_form.argtypes = [vp, C.c_int]
         L.marut_get_metrics.restype = C.c_int
@@ -171,6 +173,23 @@ def ssprk3_step(h, u, ua, ub, dt, t=0.0, stream=None):
     marut_ssprk_stage(h, 2, dt, t, u, ub, u, stream)
 
 
+def marut_set_explicit_source(h, on):
+    _check(lib().marut_set_explicit_source(h, int(bool(on))))
+
+
+def strang_step(h, u, ua, ub, dt, t=0.0, stream=None):
+    """U^{n+1} = S_{dt/2} o T_dt o S_{dt/2} (U^n) (eq. 24): implicit chemistry half steps around one
+    SSP-RK33 step of the transport operator WITHOUT the explicit source.  u is overwritten; ua, ub: scratch.
+    Call sequence only -- every step runs in the library."""
+    marut_set_explicit_source(h, False)
+    try:
+        marut_chem_implicit(h, u, 0.5 * dt, stream, want_sweeps=False)
+        ssprk3_step(h, u, ua, ub, dt, t, stream)
+        marut_chem_implicit(h, u, 0.5 * dt, stream, want_sweeps=False)
+    finally:
+        marut_set_explicit_source(h, True)
+
+
 class MarutMesh:
     """RAII wrapper around the opaque marut_mesh handle."""
 
@@ -203,6 +222,9 @@ class MarutMesh:
 
     def chem_implicit(self, u, dt, stream=None, want_sweeps=True):
         return marut_chem_implicit(self.h, u, dt, stream, want_sweeps)
+
+    def strang_step(self, u, ua, ub, dt, t=0.0, stream=None):
+        strang_step(self.h, u, ua, ub, dt, t, stream)
 
     def step(self, u, ua, ub, dt, t=0.0, stream=None):
         ssprk3_step(self.h, u, ua, ub, dt, t, stream)

@@ -43,6 +43,7 @@ struct marut_mesh {
   // device
   double *d_metric = nullptr;
   double *d_fnorm = nullptr;   // affine: [e][dim] |Ja^l|
+  int explicit_source = 1;     // reacting: L includes S(U) (default) or is the transport operator only
   int volume_form = 0;         // MARUT_VOLUME_STRONG | MARUT_VOLUME_SPLIT_RANOCHA
   int kernel_sel = 0;          // Euler stage kernel: 0 node (marut_node.cuh), 1 line (marut_line.cuh), 2 generic; env MARUT_KERNEL
   int2 *d_conn = nullptr;
@@ -483,7 +484,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   }
   StageParams P;
   P.u_in = u_in; P.u_n = u_n; P.u_out = u_out;
-  P.metric = m->d_metric; P.fnorm = m->d_fnorm; P.affine_flag = m->affine ? 1 : 0; P.conn = m->d_conn; P.mortar_fine = m->d_mortar_fine; P.mortar_mat = m->d_mortar_mat;
+  P.metric = m->d_metric; P.fnorm = m->d_fnorm; P.affine_flag = m->affine ? 1 : 0; P.explicit_source = m->explicit_source; P.conn = m->d_conn; P.mortar_fine = m->d_mortar_fine; P.mortar_mat = m->d_mortar_mat;
   P.bc_state = m->d_bc; P.S = m->d_S; P.Taux = m->d_T; P.mech = m->d_mech;
   P.ca = ca; P.cb = cb; P.cc = cc;
   P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne;
@@ -549,6 +550,13 @@ extern "C" marut_status marut_chem_source(marut_mesh *m, const double *u, double
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(MARUT_ECUDA, "chem kernel: %s", cudaGetErrorString(e));
   m->launches++;
+  return MARUT_OK;
+}
+
+extern "C" marut_status marut_set_explicit_source(marut_mesh *m, int on) {
+  if (!m) return fail(MARUT_EINVAL, "NULL argument");
+  if (m->physics != MARUT_REACTING_EULER) return fail(MARUT_EINVAL, "marut_set_explicit_source needs a REACTING_EULER mesh");
+  m->explicit_source = on ? 1 : 0;
   return MARUT_OK;
 }
 

@@ -257,7 +257,9 @@ stage_kernel(const __grid_constant__ StageParams P) {
   double src[NVAR];
 #pragma unroll
   for (int v = 0; v < NVAR; ++v) src[v] = 0.0;
-  if constexpr (PHYS == PH_REACT) production_rates<NSP>(*mech, T, U, src);
+  if constexpr (PHYS == PH_REACT) {
+    if (P.explicit_source) production_rates<NSP>(*mech, T, U, src);
+  }
   double *op = P.u_out + e * NVAR * NN + p;
   if (P.ca != 0.0) {
     const double *np_ = P.u_n + e * NVAR * NN + p;

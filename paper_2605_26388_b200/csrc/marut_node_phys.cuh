@@ -133,7 +133,11 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     Ust[(NVAR + 2) * TILE + tid] = pr.a;
     if constexpr (PHYS == PH_REACT) {
       double om[NSP];
-      production_rates_listed<NSP>(*mech, T, U, Src + tid, TILE, om);
+      if (P.explicit_source) production_rates_listed<NSP>(*mech, T, U, Src + tid, TILE, om);
+      else {
+#pragma unroll
+        for (int s = 0; s < NSP; ++s) om[s] = 0.0;
+      }
 #pragma unroll
       for (int s = 0; s < NSP; ++s) Src[s * TILE + tid] = om[s];
     }
