@@ -427,13 +427,16 @@ __global__ void __launch_bounds__(256) chem_kernel(const double *__restrict__ u,
 // (eps_k = max(1e-7 |Y_k|, 1e-12)), Gauss-Jordan with partial pivoting -- all in registers; the only global traffic
 // is one read of the nodal state and one write of its species rows.  In place.
 template <int NSP>
-__device__ __forceinline__ void implicit_residual(const MechDev &m, const double *Y, const double *Yn, double dt, double e_int,
-                                                  double *Xs, int stride, double *R) {
-  const double T = temperature_newton<NSP>(m, Y, e_int);
+__device__ __forceinline__ double implicit_residual(const MechDev &m, const double *Y, const double *Yn, double dt, double e_int,
+                                                    double T_start, double *Xs, int stride, double *R) {
+  // the caloric Newton converges to the same root (|dT| <= 1e-13 T) from any start in the table range: warm starts
+  // from the temperature of the previous evaluation save most of its iterations
+  const double T = temperature_newton<NSP>(m, Y, e_int, T_start);
   double om[NSP];
   production_rates_listed<NSP>(m, T, Y, Xs, stride, om);
 #pragma unroll
   for (int s = 0; s < NSP; ++s) R[s] = Y[s] - Yn[s] - dt * om[s];
+  return T;
 }
 template <int DIM, int NSP>
 __global__ void __launch_bounds__(128) chem_implicit_kernel(double *__restrict__ u, const MechDev *__restrict__ mech_g, double dt,
@@ -455,16 +458,17 @@ __global__ void __launch_bounds__(128) chem_implicit_kernel(double *__restrict__
 #pragma unroll
     for (int s = 0; s < NSP; ++s) { Y[s] = Yn[s] = U[s]; rho += U[s]; }
     int it = 1;
+    double Tc = 4000.0;
     for (; it <= 50; ++it) {
       double R[NSP], A[NSP][NSP + 1];
-      implicit_residual<NSP>(mech, Y, Yn, dt, e_int, Xs + threadIdx.x, 128, R);
+      Tc = implicit_residual<NSP>(mech, Y, Yn, dt, e_int, Tc, Xs + threadIdx.x, 128, R);
 #pragma unroll
       for (int c = 0; c < NSP; ++c) {
         const double eps = fmax(1e-7 * fabs(Y[c]), 1e-12);
         double Yp[NSP], Rp[NSP];
 #pragma unroll
         for (int s = 0; s < NSP; ++s) Yp[s] = (s == c) ? Y[s] + eps : Y[s];
-        implicit_residual<NSP>(mech, Yp, Yn, dt, e_int, Xs + threadIdx.x, 128, Rp);
+        implicit_residual<NSP>(mech, Yp, Yn, dt, e_int, Tc, Xs + threadIdx.x, 128, Rp);
 #pragma unroll
         for (int s = 0; s < NSP; ++s) A[s][c] = (Rp[s] - R[s]) / eps;
       }

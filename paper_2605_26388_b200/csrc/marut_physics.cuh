@@ -26,8 +26,8 @@ struct Thermo {
 // Newton for T on sum_s rho_s e_s(T) = e_int (PAPER.md:288(i); R12: T0 = 4000 K,
 // stop |dT| <= 1e-13 T, cap 50 iterations).
 template <int NSP>
-__device__ inline double temperature_newton(const MechDev &m, const double *rho_s, double e_int) {
-  double T = 4000.0;
+__device__ inline double temperature_newton(const MechDev &m, const double *rho_s, double e_int, double T_start = 4000.0) {
+  double T = T_start;
   double rR[NSP];
 #pragma unroll
   for (int s = 0; s < NSP; ++s) rR[s] = rho_s[s] * m.Rs[s];
