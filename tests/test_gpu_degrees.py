@@ -21,6 +21,7 @@ def _mesh(dim, N, cells, curved):
 
 CASES = [(2, N, 5, curved, "euler") for N in (1, 2, 3, 4, 5, 7) for curved in (False, True)] + \
         [(3, N, 3, curved, "euler") for N in (1, 2, 3, 4, 5, 6) for curved in (False, True)] + \
+        [(3, 7, 2, False, "euler"), (3, 7, 2, True, "euler"), (2, 6, 4, True, "euler")] + \
         [(3, 2, 3, True, "ns"), (3, 4, 3, False, "ns"), (2, 3, 5, True, "ns"), (3, 2, 3, False, "react"), (3, 4, 3, False, "react")]
 
 
