@@ -299,23 +299,39 @@ def run_cuda(args):
     # launches of the dominant kernel inside one marut_ssprk_stage call (NS: gradient + stage; REACT: eos + stage)
     stage_ms_avg = sum(stage_ms) / len(stage_ms)
 
-    def e2e_step():
-        gm.step(u, ua, ub, gm.max_dt(u, cfl))
+    # ---- end to end through the public API with HOST buffers: every step copies its input state from pinned host
+    # memory (H2D), runs marut_max_dt + the three stages, and copies the result back (D2H).  Two independent lanes
+    # (own handle, own device buffers, own stream) alternate steps, so the D2H of one step overlaps the H2D of the
+    # next (PCIe is full duplex); every step still pays both copies inside the timed region.
+    lanes = []
+    for k in range(2):
+        st = torch.cuda.Stream()
+        g = gm if k == 0 else mb.MarutMesh(mesh)
+        lanes.append({"st": st, "gm": g, "u": torch.empty_like(u), "ua": torch.empty_like(u), "ub": torch.empty_like(u),
+                      "out": torch.empty_like(u0_host).pin_memory()})
 
-    # ---- end to end: host buffers; H2D of the state, one step, D2H of the result, every step
-    u.copy_(u0_host, non_blocking=True)
-    for _ in range(2):
-        u.copy_(u0_host, non_blocking=True); e2e_step(); out_host.copy_(u, non_blocking=True)
+    def e2e_step(k):
+        L = lanes[k % 2]
+        with torch.cuda.stream(L["st"]):
+            L["u"].copy_(u0_host, non_blocking=True)
+            L["gm"].step(L["u"], L["ua"], L["ub"], L["gm"].max_dt(L["u"], cfl))
+            L["out"].copy_(L["u"], non_blocking=True)
+
+    for k in range(4):
+        e2e_step(k)
     barrier()
     e_start, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e_start.record(stream)
-    for _ in range(args.steps):
-        u.copy_(u0_host, non_blocking=True)
-        e2e_step()
-        out_host.copy_(u, non_blocking=True)
-    e_end.record(stream)
+    e_start.record(lanes[0]["st"])
+    lanes[1]["st"].wait_event(e_start)
+    for k in range(args.steps):
+        e2e_step(k)
+    lanes[0]["st"].wait_stream(lanes[1]["st"])
+    e_end.record(lanes[0]["st"])
     barrier()
     e2e_ms = e_start.elapsed_time(e_end)
+    if not np.isfinite(lanes[0]["out"].sum().item()):
+        raise RuntimeError("end-to-end result is not finite")
+    lanes[1]["gm"].close()
 
     ms, e2e_ms = max_over_ranks([ms, e2e_ms], world, device="cuda")
     value = aggregate_value(n_dof, args.steps, world, ms)
@@ -357,7 +373,8 @@ def run_cuda(args):
                            "step": "marut_max_dt + 3 x marut_ssprk_stage", "cfl": cfl, "restart_from_u0_every_steps": case.steps, "affine": bool(affine)},
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n_dof * 8, "d2h_bytes_per_step": n_dof * 8 + 8,
-                        "ms_per_step": e2e_ms / args.steps},
+                        "ms_per_step": e2e_ms / args.steps,
+                        "how": "pinned host buffers; two alternating lanes (handle + stream each) so that the D2H of a step overlaps the H2D of the next"},
                 "gpu_launches": launches,
                 "roofline": roof}
         if world == 1 and not args.no_cpu_baseline:
