@@ -76,6 +76,8 @@ def _setup(L):
         L.oracle_species_thermo.argtypes = [vp, C.c_int, C.c_double, vp]
         L.oracle_num_threads.restype = C.c_int
         L.oracle_set_explicit_source.argtypes = [vp, C.c_int]
+        L.oracle_shock_indicator.argtypes = [vp, vp, C.c_double, C.c_double, C.c_double, vp, C.c_int]
+        L.oracle_modal_matrix.argtypes = [C.c_int, vp]
         L.oracle_chem_implicit.restype = C.c_int
         L.oracle_chem_implicit.argtypes = [vp, vp, C.c_double]
         L.oracle_chem_implicit_node.restype = C.c_int
@@ -223,6 +225,13 @@ class OracleMesh:
     def chem_source(self, u):
         return self._call(self.L.oracle_chem_source, u)
 
+    def shock_indicator(self, u, s=9.21024, alpha_min=0.001, alpha_max=0.5, smooth=True):
+        """Hennemann-Gassner blending coefficient alpha_e per element (with face-neighbour maximum if smooth)"""
+        u = _f64(u)
+        a = np.zeros(self.mesh.n_elem)
+        self.L.oracle_shock_indicator(self.h, _p(u), s, alpha_min, alpha_max, _p(a), int(smooth))
+        return a
+
     def set_explicit_source(self, on):
         """reacting meshes: whether L(U) includes the chemistry source (default) or is the transport operator only"""
         self.L.oracle_set_explicit_source(self.h, int(bool(on)))
@@ -307,6 +316,13 @@ def viscous_flux(dim, gamma, mu, Pr, U, S, nv):
     F = np.zeros(dim + 2)
     lib().oracle_viscous_flux(dim, gamma, mu, Pr, _p(U), _p(S), _p(nv), _p(F))
     return F
+
+
+def modal_matrix(N):
+    """V^-1 of the orthonormal Legendre basis on the LGL nodes: nodal values -> modal coefficients"""
+    V = np.zeros((N + 1, N + 1))
+    lib().oracle_modal_matrix(N, _p(V))
+    return V
 
 
 def logmean(aL, aR):

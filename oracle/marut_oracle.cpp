@@ -855,6 +855,77 @@ static int chem_implicit(const Mesh &m, double *u, double dt) {
     }
   return worst;
 }
+// O16. Hennemann-Gassner shock indicator with face-neighbour smoothing:
+// indicator field q = rho p; modal coefficients of its degree-N interpolant in the orthonormal tensor-product Legendre
+// basis (m = V^-1 q per direction, V_ik = sqrt((2k+1)/2) L_k(x_i)); E = max(E_high^N/E_tot^N, E_high^(N-1)/E_tot^(N-1));
+// alpha = 1/(1 + exp(-(s/T)(E - T))), T = 0.5 * 10^(-1.8 (N+1)^(1/4)); alpha < alpha_min -> 0, alpha > alpha_max ->
+// alpha_max (R15); then alpha_e <- max(alpha_e, alpha_e') over the elements e' sharing a face with e.
+static void modal_matrix(const Ops &o, std::vector<double> &Vinv) {
+  const int n = o.n;
+  std::vector<double> V((size_t)n * n), A((size_t)n * 2 * n, 0.0);
+  for (int i = 0; i < n; ++i)
+    for (int k = 0; k < n; ++k) {
+      double P, dP; legendre<double>(k, o.x[i], P, dP);
+      V[(size_t)i * n + k] = std::sqrt((2.0 * k + 1.0) / 2.0) * P;
+    }
+  for (int i = 0; i < n; ++i) { for (int k = 0; k < n; ++k) A[(size_t)i * 2 * n + k] = V[(size_t)i * n + k]; A[(size_t)i * 2 * n + n + i] = 1.0; }
+  for (int c = 0; c < n; ++c) {                      // Gauss-Jordan with partial pivoting on [V | I]
+    int piv = c;
+    for (int r = c + 1; r < n; ++r) if (std::fabs(A[(size_t)r * 2 * n + c]) > std::fabs(A[(size_t)piv * 2 * n + c])) piv = r;
+    if (piv != c) for (int q = 0; q < 2 * n; ++q) std::swap(A[(size_t)c * 2 * n + q], A[(size_t)piv * 2 * n + q]);
+    const double inv = 1.0 / A[(size_t)c * 2 * n + c];
+    for (int q = 0; q < 2 * n; ++q) A[(size_t)c * 2 * n + q] *= inv;
+    for (int r = 0; r < n; ++r) if (r != c) {
+      const double f = A[(size_t)r * 2 * n + c];
+      for (int q = 0; q < 2 * n; ++q) A[(size_t)r * 2 * n + q] -= f * A[(size_t)c * 2 * n + q];
+    }
+  }
+  Vinv.assign((size_t)n * n, 0.0);
+  for (int k = 0; k < n; ++k) for (int i = 0; i < n; ++i) Vinv[(size_t)k * n + i] = A[(size_t)k * 2 * n + n + i];
+}
+static void shock_indicator(const Mesh &m, const double *u, double s, double amin, double amax, double *alpha, bool smooth) {
+  const int n = m.n, nn = m.nn, d = m.dim, N = m.N;
+  std::vector<double> Vinv; modal_matrix(m.ops, Vinv);
+  const double T = 0.5 * std::pow(10.0, -1.8 * std::pow((double)(N + 1), 0.25));
+  std::vector<double> raw((size_t)m.ne);
+  for (long e = 0; e < m.ne; ++e) {
+    std::vector<double> q(nn), t(nn);
+    for (int p = 0; p < nn; ++p) { double U[MAXV]; gather(m, u, e, p, U); Prim pr = primitives(m, U); q[p] = pr.rho * pr.p; }
+    for (int l = 0; l < d; ++l) {                    // m = V^-1 q along every direction
+      for (int p = 0; p < nn; ++p) {
+        int ijk[3] = {0, 0, 0}; node_ijk(m, p, ijk);
+        double acc = 0.0;
+        for (int i = 0; i < n; ++i) { int r[3] = {ijk[0], ijk[1], ijk[2]}; r[l] = i; acc += Vinv[(size_t)ijk[l] * n + i] * q[node_index(m, r)]; }
+        t[p] = acc;
+      }
+      q.swap(t);
+    }
+    double etot[2] = {0.0, 0.0}, ehigh[2] = {0.0, 0.0};      // [0]: K = N, [1]: K = N-1
+    for (int p = 0; p < nn; ++p) {
+      int ijk[3] = {0, 0, 0}; node_ijk(m, p, ijk);
+      int mx = 0; for (int c = 0; c < d; ++c) mx = std::max(mx, ijk[c]);
+      const double m2 = q[p] * q[p];
+      etot[0] += m2; if (mx == N) ehigh[0] += m2;
+      if (mx <= N - 1) { etot[1] += m2; if (mx == N - 1) ehigh[1] += m2; }
+    }
+    double E = ehigh[0] / etot[0];
+    if (N >= 1 && etot[1] > 0.0) E = std::max(E, ehigh[1] / etot[1]);
+    double a = 1.0 / (1.0 + std::exp(-(s / T) * (E - T)));
+    if (a < amin) a = 0.0;
+    if (a > amax) a = amax;
+    raw[e] = a;
+  }
+  for (long e = 0; e < m.ne; ++e) alpha[e] = raw[e];
+  if (!smooth) return;
+  for (size_t f = 0; f < m.iface.size() / 5; ++f) {
+    const long a = m.iface[f * 5], b = m.iface[f * 5 + 2];
+    alpha[a] = std::max(alpha[a], raw[b]); alpha[b] = std::max(alpha[b], raw[a]);
+  }
+  for (size_t f = 0; f < m.mortar.size() / 6; ++f) {
+    const long c = m.mortar[f * 6];
+    for (int k = 2; k <= 3; ++k) { const long b = m.mortar[f * 6 + k]; alpha[c] = std::max(alpha[c], raw[b]); alpha[b] = std::max(alpha[b], raw[c]); }
+  }
+}
 static void rhs_full(const Mesh &m, const double *u, double *du) {
   rhs_inviscid(m, u, du);
   if (m.physics == NAVIER_STOKES) rhs_viscous_add(m, u, du);
@@ -956,6 +1027,12 @@ int oracle_set_volume_form(void *h, int form) {
   if (form < 0 || form > 1 || (form == 1 && m->physics == REACTING_EULER)) return 1;
   m->volume_form = form;
   return 0;
+}
+void oracle_shock_indicator(void *h, const double *u, double s, double amin, double amax, double *alpha, int smooth) {
+  shock_indicator(*(Mesh *)h, u, s, amin, amax, alpha, smooth != 0);
+}
+void oracle_modal_matrix(int N, double *Vinv) {
+  Ops o = make_ops(N); std::vector<double> V; modal_matrix(o, V); std::copy(V.begin(), V.end(), Vinv);
 }
 int oracle_set_explicit_source(void *h, int on) { ((Mesh *)h)->explicit_source = on ? 1 : 0; return 0; }
 int oracle_chem_implicit(void *h, double *u, double dt) {
