@@ -117,6 +117,15 @@ marut_status marut_chem_source(marut_mesh *mesh, const double *u, double *s, voi
  * the stream and returns ENOTFINITE if a node did not converge within 50 sweeps.  REACTING_EULER meshes only. */
 marut_status marut_chem_implicit(marut_mesh *mesh, double *u, double dt, int *sweeps_out, void *cuda_stream);
 
+/* Hennemann-Gassner shock indicator with face-neighbour smoothing (first part of 8(f) NEXT-3; PAPER.md:177,
+ * 629-653; R15): per element, the modal energy of rho*p in the two highest Legendre shells,
+ *   E = max(E_high^N/E_tot^N, E_high^(N-1)/E_tot^(N-1)),  alpha = 1/(1 + exp(-(s/T)(E - T))),
+ *   T = 0.5*10^(-1.8 (N+1)^(1/4)),  alpha < alpha_min -> 0,  alpha > alpha_max -> alpha_max,
+ * then, if smooth != 0, alpha_e <- max(alpha_e, alpha_e') over the elements e' sharing a face (conforming or mortar).
+ * alpha: DEVICE, [n_elem].  EULER / NAVIER_STOKES meshes.  The blended DG/FV residual (eq. 11, 42) is not built. */
+marut_status marut_shock_indicator(marut_mesh *mesh, const double *u, double s, double alpha_min, double alpha_max,
+                                   int smooth, double *alpha, void *cuda_stream);
+
 /* REACTING_EULER meshes: whether L(u) of marut_rhs / marut_ssprk_stage includes the explicit chemistry source S(u)
  * (on != 0, the default) or is the transport operator T alone (on == 0), as the Strang split of eq. 24 needs:
  *   u^{n+1} = S_{dt/2} o T_dt o S_{dt/2} (u^n) = marut_chem_implicit(dt/2), SSP-RK steps of T, marut_chem_implicit(dt/2). */

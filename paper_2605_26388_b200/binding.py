@@ -15,7 +15,7 @@ _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA"
 
 # every symbol include/marut.h declares
 SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt",
-           "marut_chem_source", "marut_chem_implicit", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
+           "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
            "marut_last_error"]
 
 
@@ -66,6 +66,8 @@ def lib():
         L.marut_chem_source.argtypes = [vp, vp, vp, vp]
         L.marut_chem_implicit.restype = C.c_int
         L.marut_chem_implicit.argtypes = [vp, vp, dbl, C.POINTER(C.c_int), vp]
+        L.marut_shock_indicator.restype = C.c_int
+        L.marut_shock_indicator.argtypes = [vp, vp, dbl, dbl, dbl, C.c_int, vp, vp]
         L.marut_set_explicit_source.restype = C.c_int
         L.marut_set_explicit_source.argtypes = [vp, C.c_int]
         L.marut_set_volume_form.restype = C.c_int
@@ -173,6 +175,10 @@ def ssprk3_step(h, u, ua, ub, dt, t=0.0, stream=None):
     marut_ssprk_stage(h, 2, dt, t, u, ub, u, stream)
 
 
+def marut_shock_indicator(h, u, alpha, s=9.21024, alpha_min=0.001, alpha_max=0.5, smooth=True, stream=None):
+    _check(lib().marut_shock_indicator(h, _dev(u), s, alpha_min, alpha_max, int(bool(smooth)), _dev(alpha), _stream(stream)))
+
+
 def marut_set_explicit_source(h, on):
     _check(lib().marut_set_explicit_source(h, int(bool(on))))
 
@@ -222,6 +228,9 @@ class MarutMesh:
 
     def chem_implicit(self, u, dt, stream=None, want_sweeps=True):
         return marut_chem_implicit(self.h, u, dt, stream, want_sweeps)
+
+    def shock_indicator(self, u, alpha, **kw):
+        marut_shock_indicator(self.h, u, alpha, **kw)
 
     def strang_step(self, u, ua, ub, dt, t=0.0, stream=None):
         strang_step(self.h, u, ua, ub, dt, t, stream)

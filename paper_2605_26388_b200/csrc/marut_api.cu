@@ -53,6 +53,8 @@ struct marut_mesh {
   double *d_S = nullptr;     // NS scratch: stress tensor + heat flux from the BR1 gradient, [e][d(d+1)/2 + d][node]
   double *d_T = nullptr;     // reacting temperature scratch
   MechDev *d_mech = nullptr;
+  double *d_Vinv = nullptr;  // [n][n] nodal -> orthonormal Legendre modal (shock indicator)
+  double *d_araw = nullptr;  // [ne] unsmoothed blending coefficient (allocated on first use)
   unsigned long long *d_red = nullptr;
   unsigned long long *h_red = nullptr;  // pinned
   long launches = 0;
@@ -227,7 +229,7 @@ extern "C" void marut_mesh_destroy(marut_mesh *m) {
   if (!m) return;
   cudaDeviceSynchronize();
   cudaFree(m->d_metric); cudaFree(m->d_fnorm); cudaFree(m->d_conn); cudaFree(m->d_mortar_fine); cudaFree(m->d_mortar_mat);
-  cudaFree(m->d_bc); cudaFree(m->d_S); cudaFree(m->d_T); cudaFree(m->d_mech); cudaFree(m->d_red);
+  cudaFree(m->d_Vinv); cudaFree(m->d_araw); cudaFree(m->d_bc); cudaFree(m->d_S); cudaFree(m->d_T); cudaFree(m->d_mech); cudaFree(m->d_red);
   if (m->h_red) cudaFreeHost(m->h_red);
   delete m;
 }
@@ -579,6 +581,80 @@ extern "C" marut_status marut_chem_implicit(marut_mesh *m, double *u, double dt,
     CUDA_TRY(cudaStreamSynchronize(st));
     *sweeps_out = (int)(m->h_red[3] & 0xffffffffu);
     if (*sweeps_out > 50) return fail(MARUT_ENOTFINITE, "implicit chemistry: Newton did not converge in 50 sweeps");
+  }
+  return MARUT_OK;
+}
+
+// ------------------------------------------------------------------------------------ shock indicator
+// V^-1 of the orthonormal Legendre basis on the LGL nodes: V_ik = sqrt((2k+1)/2) L_k(x_i), inverted by Gauss-Jordan
+static bool build_modal_matrix(int N, const double *x, double *Vinv) {
+  const int n = N + 1;
+  std::vector<double> A((size_t)n * 2 * n, 0.0);
+  for (int i = 0; i < n; ++i) {
+    double Pm = 1.0, Pc = x[i];
+    for (int k = 0; k < n; ++k) {
+      double Pk = (k == 0) ? 1.0 : ((k == 1) ? x[i] : 0.0);
+      if (k >= 2) { Pk = ((2.0 * k - 1.0) * x[i] * Pc - (k - 1.0) * Pm) / k; Pm = Pc; Pc = Pk; }
+      A[(size_t)i * 2 * n + k] = std::sqrt((2.0 * k + 1.0) / 2.0) * Pk;
+    }
+    A[(size_t)i * 2 * n + n + i] = 1.0;
+  }
+  for (int c = 0; c < n; ++c) {
+    int piv = c;
+    for (int r = c + 1; r < n; ++r) if (std::fabs(A[(size_t)r * 2 * n + c]) > std::fabs(A[(size_t)piv * 2 * n + c])) piv = r;
+    if (A[(size_t)piv * 2 * n + c] == 0.0) return false;
+    if (piv != c) for (int q = 0; q < 2 * n; ++q) std::swap(A[(size_t)c * 2 * n + q], A[(size_t)piv * 2 * n + q]);
+    const double inv = 1.0 / A[(size_t)c * 2 * n + c];
+    for (int q = 0; q < 2 * n; ++q) A[(size_t)c * 2 * n + q] *= inv;
+    for (int r = 0; r < n; ++r) if (r != c) {
+      const double f = A[(size_t)r * 2 * n + c];
+      for (int q = 0; q < 2 * n; ++q) A[(size_t)r * 2 * n + q] -= f * A[(size_t)c * 2 * n + q];
+    }
+  }
+  for (int k = 0; k < n; ++k) for (int i = 0; i < n; ++i) Vinv[k * n + i] = A[(size_t)k * 2 * n + n + i];
+  return true;
+}
+
+template <int DIM, int NP>
+static cudaError_t run_indicator(marut_mesh *m, const double *u, double s_over_T, double T, double amin, double amax,
+                                 double *out, cudaStream_t st) {
+  constexpr int NN = Geo<DIM, NP>::NN, EB = (NN >= 96) ? 1 : 128 / NN, NT = ((EB * NN + 31) / 32) * 32;
+  const unsigned grid = (unsigned)((m->ne + EB - 1) / EB);
+  indicator_kernel<DIM, NP, EB><<<grid, NT, 0, st>>>(u, m->d_Vinv, m->gamma, s_over_T, T, amin, amax, m->ne, out);
+  return cudaGetLastError();
+}
+
+extern "C" marut_status marut_shock_indicator(marut_mesh *m, const double *u, double s, double alpha_min, double alpha_max,
+                                              int smooth, double *alpha, void *stream) {
+  if (!m || !u || !alpha) return fail(MARUT_EINVAL, "NULL argument");
+  if (m->physics == MARUT_REACTING_EULER) return fail(MARUT_EINVAL, "marut_shock_indicator: ideal-gas meshes only");
+  if (!(s > 0.0) || !(alpha_min >= 0.0) || !(alpha_max >= alpha_min) || !(alpha_max <= 1.0))
+    return fail(MARUT_EINVAL, "need s > 0 and 0 <= alpha_min <= alpha_max <= 1");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!m->d_Vinv) {
+    double x[MAX_NP], w[MAX_NP], D[MAX_NP * MAX_NP], V[MAX_NP * MAX_NP];
+    build_operators(m->N, x, w, D);
+    if (!build_modal_matrix(m->N, x, V)) return fail(MARUT_EINVAL, "singular Vandermonde matrix");
+    CUDA_TRY(cudaMalloc(&m->d_Vinv, m->np * m->np * sizeof(double)));
+    CUDA_TRY(cudaMemcpy(m->d_Vinv, V, m->np * m->np * sizeof(double), cudaMemcpyHostToDevice));
+  }
+  if (smooth && !m->d_araw) CUDA_TRY(cudaMalloc(&m->d_araw, (size_t)m->ne * sizeof(double)));
+  const double T = 0.5 * std::pow(10.0, -1.8 * std::pow((double)(m->N + 1), 0.25));
+  double *raw = smooth ? m->d_araw : alpha;
+  cudaError_t e = cudaErrorNotSupported;
+#define MARUT_IND(D_, NP_) if (m->dim == D_ && m->np == NP_) e = run_indicator<D_, NP_>(m, u, s / T, T, alpha_min, alpha_max, raw, st);
+  MARUT_IND(2, 2) MARUT_IND(2, 3) MARUT_IND(2, 4) MARUT_IND(2, 5) MARUT_IND(2, 6) MARUT_IND(2, 7) MARUT_IND(2, 8)
+  MARUT_IND(3, 2) MARUT_IND(3, 3) MARUT_IND(3, 4) MARUT_IND(3, 5) MARUT_IND(3, 6) MARUT_IND(3, 7) MARUT_IND(3, 8)
+#undef MARUT_IND
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "indicator kernel: %s", cudaGetErrorString(e));
+  m->launches++;
+  if (smooth) {
+    const unsigned grid = (unsigned)((m->ne + 255) / 256);
+    if (m->dim == 2) indicator_smooth_kernel<2><<<grid, 256, 0, st>>>(raw, m->d_conn, m->d_mortar_fine, m->ne, alpha);
+    else indicator_smooth_kernel<3><<<grid, 256, 0, st>>>(raw, m->d_conn, m->d_mortar_fine, m->ne, alpha);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(MARUT_ECUDA, "indicator smoothing kernel: %s", cudaGetErrorString(e));
+    m->launches++;
   }
   return MARUT_OK;
 }

@@ -513,6 +513,104 @@ __global__ void __launch_bounds__(128) chem_implicit_kernel(double *__restrict__
 }
 
 // ======================================================================================
+// Hennemann-Gassner shock indicator (R15).
+// indicator_kernel: per element, q = rho p -> modal coefficients (V^-1 along every direction, ping-pong in shared
+// memory) -> E = max of the two top-shell energy ratios -> alpha = 1/(1 + exp(-(s/T)(E - T))), clipped.
+// indicator_smooth_kernel: alpha_e <- max over the face neighbours (conforming, both sides of a mortar).
+// ======================================================================================
+template <int DIM, int NP, int EB>
+__global__ void __launch_bounds__(((EB * Geo<DIM, NP>::NN + 31) / 32) * 32)
+indicator_kernel(const double *__restrict__ u, const double *__restrict__ Vinv_g, double gamma, double s_over_T, double T,
+                 double amin, double amax, long ne, double *__restrict__ alpha) {
+  using G = Geo<DIM, NP>;
+  constexpr int NN = G::NN, NVAR = DIM + 2, TILE = EB * NN;
+  __shared__ double A[TILE], B[TILE], Vs[NP * NP];
+  const int tid = threadIdx.x;
+  for (int i = tid; i < NP * NP; i += blockDim.x) Vs[i] = Vinv_g[i];
+  const int el = tid / NN, p = tid - el * NN;
+  const long e = (long)blockIdx.x * EB + el;
+  const bool active = (tid < TILE) && (e < ne);
+  const int qi = p % NP, qj = (p / NP) % NP, qk = (DIM == 3) ? p / (NP * NP) : 0;
+  if (active) {
+    double U[NVAR];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(u + (e * NVAR + v) * NN + p);
+    const Prim<DIM> pr = prim_ideal<DIM, false>(U, gamma);
+    A[tid] = pr.rho * pr.p;
+  }
+  __syncthreads();
+  // xi: A -> B
+  if (active) {
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < NP; ++i) acc += Vs[qi * NP + i] * A[tid - qi + i];
+    B[tid] = acc;
+  }
+  __syncthreads();
+  // eta: B -> A
+  if (active) {
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < NP; ++i) acc += Vs[qj * NP + i] * B[tid - qj * NP + i * NP];
+    A[tid] = acc;
+  }
+  __syncthreads();
+  double *src = A;
+  if constexpr (DIM == 3) {
+    // zeta: A -> B
+    if (active) {
+      double acc = 0.0;
+#pragma unroll
+      for (int i = 0; i < NP; ++i) acc += Vs[qk * NP + i] * A[tid - qk * NP * NP + i * NP * NP];
+      B[tid] = acc;
+    }
+    __syncthreads();
+    src = B;
+  }
+  // energies: one thread per element sums its NN modes (fixed order)
+  if (active && p == 0) {
+    constexpr int N = NP - 1;
+    double et0 = 0.0, eh0 = 0.0, et1 = 0.0, eh1 = 0.0;
+    int r = 0;
+    for (int k = 0; k < ((DIM == 3) ? NP : 1); ++k)
+      for (int j = 0; j < NP; ++j)
+        for (int i = 0; i < NP; ++i, ++r) {
+          int mx = i;
+          if (j > mx) mx = j;
+          if (k > mx) mx = k;
+          const double m2 = src[el * NN + r] * src[el * NN + r];
+          et0 += m2;
+          if (mx == N) eh0 += m2;
+          if (mx <= N - 1) {
+            et1 += m2;
+            if (mx == N - 1) eh1 += m2;
+          }
+        }
+    double E = eh0 / et0;
+    if (et1 > 0.0) E = fmax(E, eh1 / et1);
+    double a = 1.0 / (1.0 + exp(-s_over_T * (E - T)));
+    if (a < amin) a = 0.0;
+    if (a > amax) a = amax;
+    alpha[e] = a;
+  }
+}
+template <int DIM>
+__global__ void indicator_smooth_kernel(const double *__restrict__ raw, const int2 *__restrict__ conn,
+                                        const int *__restrict__ mortar_fine, long ne, double *__restrict__ alpha) {
+  const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= ne) return;
+  double a = raw[e];
+#pragma unroll
+  for (int f = 0; f < 2 * DIM; ++f) {
+    const int2 cn = __ldg(&conn[e * 2 * DIM + f]);
+    const int kind = cn.y & 3;
+    if (kind == FK_CONFORMING || kind == FK_MORTAR_FINE) a = fmax(a, raw[cn.x]);
+    else if (kind == FK_MORTAR_COARSE) a = fmax(a, fmax(raw[__ldg(&mortar_fine[cn.x * 2])], raw[__ldg(&mortar_fine[cn.x * 2 + 1])]));
+  }
+  alpha[e] = a;
+}
+
+// ======================================================================================
 // max wave speed / max diffusivity (a10; eq. 17-18): warp-shuffle reduction, one atomicMax per CTA.
 // red[0] = max(|u|_2 + a) ; red[1] = max(mu/rho) ; red[2] = count of non-finite/non-positive speeds
 // (bit patterns of non-negative doubles order like unsigned integers)

@@ -151,3 +151,36 @@ def test_quadtree_mortars_and_boundaries_other_degrees(N, split):
     uc, tc, _, _ = om.run(u0, 5, cfl=0.3)
     assert abs(tg - tc) <= 1e-12 * tc and parity_error(ug, uc).max() <= RUN_TOL
     gm.close()
+
+
+@pytest.mark.parametrize("kind,N", [("c4", 3), ("c4", 5), ("tgv3", 4), ("tgv3", 2), ("vortex", 7)])
+def test_shock_indicator_parity(kind, N):
+    """Hennemann-Gassner blending coefficient (marut_shock_indicator) against the oracle: raw and smoothed,
+    on the Mach-10 front of the quadtree mesh (mortar neighbours, alpha from 0 to alpha_max) and on smooth fields"""
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    if kind == "c4":
+        m = wl.quadtree_mesh(N, base=(32, 8), band=0.15, jitter=0.3)
+        m.bc_state = wl.shock_states(m.gamma)
+        u0 = wl.mach10_shock(m, half_width=1.0 * m.info["h_fine"])      # a front sharper than the bench recipe's
+    elif kind == "tgv3":
+        m = _mesh(3, N, 3, True)
+        u0 = wl.taylor_green(m, noise=5e-2)
+    else:
+        m = _mesh(2, N, 4, False)
+        u0 = wl.isentropic_vortex(m)
+    om, gm = oracle.OracleMesh(m), mb.MarutMesh(m)
+    u = torch.from_numpy(u0).cuda()
+    a = torch.empty(m.n_elem, dtype=torch.float64, device="cuda")
+    for smooth in (False, True):
+        for amin, amax in ((0.0, 1.0), (1e-3, 0.5)):
+            gm.shock_indicator(u, a, alpha_min=amin, alpha_max=amax, smooth=smooth)
+            ref = om.shock_indicator(u0, alpha_min=amin, alpha_max=amax, smooth=smooth)
+            g = a.cpu().numpy()
+            assert np.abs(g - ref).max() <= 1e-11 * max(ref.max(), 1e-300), (kind, N, smooth, amin)
+    if kind == "c4" and N == 3:
+        assert ref.max() == 0.5 and (ref == 0).sum() > 0          # the front saturates, the far field stays pure DG
+    gm.close()
