@@ -84,6 +84,10 @@ def _setup(L):
         L.oracle_chem_implicit_node.argtypes = [vp, vp, C.c_double, C.c_double]
         L.oracle_set_volume_form.restype = C.c_int
         L.oracle_set_volume_form.argtypes = [vp, C.c_int]
+        L.oracle_set_blend.restype = C.c_int
+        L.oracle_set_blend.argtypes = [vp, vp]
+        L.oracle_fv_volume.argtypes = [vp, vp, vp]
+        L.oracle_subcell_normal.argtypes = [vp, C.c_long, C.c_int, vp, C.c_int, vp]
         L.oracle_logmean.restype = C.c_double
         L.oracle_logmean.argtypes = [C.c_double, C.c_double]
         L.oracle_ranocha.argtypes = [C.c_int, C.c_double, vp, vp, vp, vp]
@@ -231,6 +235,31 @@ class OracleMesh:
         a = np.zeros(self.mesh.n_elem)
         self.L.oracle_shock_indicator(self.h, _p(u), s, alpha_min, alpha_max, _p(a), int(smooth))
         return a
+
+    def set_blend(self, alpha):
+        """eq. 11 / 42: per-element blending coefficients alpha_e (copied) of the DG / sub-cell FV volume residual;
+        None switches the blending off"""
+        if alpha is None:
+            self.L.oracle_set_blend(self.h, None)
+            return
+        a = _f64(alpha)
+        assert a.shape == (self.mesh.n_elem,)
+        if self.L.oracle_set_blend(self.h, _p(a)) != 0:
+            raise ValueError("blending is defined for the Euler equations only")
+
+    def fv_volume(self, u):
+        """O17: the first-order sub-cell finite-volume VOLUME residual R^FV (no surface lift), [e][v][node]"""
+        u = _f64(u)
+        r = np.empty_like(u)
+        self.L.oracle_fv_volume(self.h, _p(u), _p(r))
+        return r
+
+    def subcell_normal(self, e, l, ijk, mi):
+        """O17: sub-cell normal nhat^l_{mi+1/2} on the line through node ijk along direction l"""
+        q = np.ascontiguousarray(list(ijk) + [0] * (3 - len(ijk)), dtype=np.int32)
+        nh = np.zeros(3)
+        self.L.oracle_subcell_normal(self.h, int(e), int(l), q.ctypes.data_as(C.c_void_p), int(mi), _p(nh))
+        return nh[: self.mesh.dim]
 
     def set_explicit_source(self, on):
         """reacting meshes: whether L(U) includes the chemistry source (default) or is the transport operator only"""

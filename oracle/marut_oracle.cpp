@@ -288,6 +288,7 @@ struct Mesh {
   double dx_min = 0.0;
   int explicit_source = 1;      // reacting: 1 = L includes the chemistry source S(U); 0 = transport operator only (Strang split)
   int volume_form = 0;          // 0: standard strong form (eq. 9); 1: entropy-stable split form (eq. 10)
+  std::vector<double> alpha;    // per-element blending coefficient alpha_e of eq. 11 / 42; empty = no blending
 };
 
 static inline int node_index(const Mesh &m, const int *ijk) {
@@ -517,6 +518,72 @@ static inline void face_normal(const Mesh &m, long e, int f, int node, double *n
 }
 
 // ---------------------------------------------------------------------------
+// O17. First-order finite-volume residual on the LGL sub-cell grid (eq. 11, 42; the
+// construction of the cited framework [15], reading R16 -- the paper names it without printing it).
+// Along each reference direction l the N+1 nodes of a line own sub-cells of reference width w_0..w_N; the N interior
+// sub-cell interfaces m+1/2 (between line indices m and m+1) carry the matching surface flux (Rusanov, O5)
+//   fhat^l_{m+1/2} = F*(U_m, U_{m+1}; nhat^l_{m+1/2}),
+// with the sub-cell normal  nhat^l_{m+1/2} = Ja^l_0 + sum_{q<=m} w_q sum_r D_qr Ja^l_r  (telescopes from Ja^l_0 to
+// Ja^l_N by summation by parts; equals Ja^l on an affine element), and the two outermost interfaces carry the
+// element's own flux fhat^l_{-1/2} = F(U_0).Ja^l_0, fhat^l_{N+1/2} = F(U_N).Ja^l_N -- exactly the term the surface
+// lift of eq. 12, (F* - Ftilde)/(J w), which the DG and FV residuals share, replaces by the interface flux F*.
+//   R^FV_i = -(1/J_i) sum_l ( fhat^l_{i_l+1/2} - fhat^l_{i_l-1/2} ) / w_{i_l}
+// ---------------------------------------------------------------------------
+static void subcell_normal(const Mesh &m, long e, int l, const int *ijk_line, int mi, double *nh) {
+  const int d = m.dim, n = m.n, nn = m.nn;
+  int q[3] = {ijk_line[0], ijk_line[1], ijk_line[2]};
+  q[l] = 0;
+  const double *Ja0 = &m.Ja[((size_t)e * nn + node_index(m, q)) * d * d + l * d];
+  for (int c = 0; c < d; ++c) nh[c] = Ja0[c];
+  for (int qq = 0; qq <= mi; ++qq)
+    for (int r = 0; r < n; ++r) {
+      q[l] = r;
+      const double *Jar = &m.Ja[((size_t)e * nn + node_index(m, q)) * d * d + l * d];
+      for (int c = 0; c < d; ++c) nh[c] += m.ops.w[qq] * m.ops.D[(size_t)qq * n + r] * Jar[c];
+    }
+}
+static void fv_volume_residual(const Mesh &m, const double *u, long e, double *rfv /* [nvar][nn] */) {
+  const int nn = m.nn, d = m.dim, nvar = m.nvar, N = m.N;
+  for (int p = 0; p < nn; ++p) {
+    int ijk[3] = {0, 0, 0}; node_ijk(m, p, ijk);
+    double Ui[MAXV], acc[MAXV]; gather(m, u, e, p, Ui);
+    for (int v = 0; v < nvar; ++v) acc[v] = 0.0;
+    for (int l = 0; l < d; ++l) {
+      const int il = ijk[l];
+      const double *Jai = &m.Ja[((size_t)e * nn + p) * d * d + l * d];
+      double fp[MAXV], fm[MAXV], nh[3], Uo[MAXV];
+      int q[3] = {ijk[0], ijk[1], ijk[2]};
+      if (il == N) flux_dot(m, Ui, primitives(m, Ui), Jai, fp);
+      else {
+        q[l] = il + 1; gather(m, u, e, node_index(m, q), Uo);
+        subcell_normal(m, e, l, ijk, il, nh);
+        rusanov(m, Ui, Uo, nh, fp);
+      }
+      if (il == 0) flux_dot(m, Ui, primitives(m, Ui), Jai, fm);
+      else {
+        q[l] = il - 1; gather(m, u, e, node_index(m, q), Uo);
+        subcell_normal(m, e, l, ijk, il - 1, nh);
+        rusanov(m, Uo, Ui, nh, fm);
+      }
+      for (int v = 0; v < nvar; ++v) acc[v] += (fp[v] - fm[v]) / m.ops.w[il];
+    }
+    for (int v = 0; v < nvar; ++v) rfv[(size_t)v * nn + p] = -acc[v] / m.J[(size_t)e * nn + p];
+  }
+}
+// eq. 11 / 42: volume residual of element e <- (1 - alpha_e) R^DG + alpha_e R^FV (the surface lift is added afterwards)
+static void blend_fv(const Mesh &m, const double *u, long e, double *du) {
+  if (m.alpha.empty()) return;
+  const double a = m.alpha[e];
+  std::vector<double> rfv((size_t)m.nvar * m.nn);
+  fv_volume_residual(m, u, e, rfv.data());
+  for (int v = 0; v < m.nvar; ++v)
+    for (int p = 0; p < m.nn; ++p) {
+      double &x = du[((size_t)e * m.nvar + v) * m.nn + p];
+      x = (1.0 - a) * x + a * rfv[(size_t)v * m.nn + p];
+    }
+}
+
+// ---------------------------------------------------------------------------
 // O4 + O6. Inviscid residual: volume term (eq. 9) and surface lift (eq. 12).
 // ---------------------------------------------------------------------------
 static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
@@ -546,6 +613,7 @@ static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
         }
         for (int v = 0; v < nvar; ++v) du[((size_t)e * nvar + v) * nn + p] = -2.0 * acc[v] / m.J[(size_t)e * nn + p];
       }
+      blend_fv(m, u, e, du);
       continue;
     }
     std::vector<double> Ft((size_t)d * nvar * nn);      // [l][v][node]
@@ -564,6 +632,7 @@ static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
         for (int l = 0; l < d; ++l) s += dxi(m, &Ft[((size_t)l * nvar + v) * nn], p, l);
         du[((size_t)e * nvar + v) * nn + p] = -s / m.J[(size_t)e * nn + p];
       }
+    blend_fv(m, u, e, du);
   }
   const int nf = (d == 2) ? n : n * n;                  // nodes per face
   const double wb = m.ops.w[0];                         // LGL weight of the boundary index (w_0 = w_N)
@@ -1028,6 +1097,19 @@ int oracle_set_volume_form(void *h, int form) {
   m->volume_form = form;
   return 0;
 }
+// alpha: [n_elem] blending coefficients of eq. 11 (copied), or NULL to switch the blending off
+int oracle_set_blend(void *h, const double *alpha) {
+  Mesh *m = (Mesh *)h;
+  if (alpha && m->physics != EULER) return 1;
+  if (alpha) m->alpha.assign(alpha, alpha + m->ne); else m->alpha.clear();
+  return 0;
+}
+void oracle_fv_volume(void *h, const double *u, double *rfv) {
+  Mesh &m = *(Mesh *)h;
+#pragma omp parallel for schedule(static)
+  for (long e = 0; e < m.ne; ++e) fv_volume_residual(m, u, e, rfv + (size_t)e * m.nvar * m.nn);
+}
+void oracle_subcell_normal(void *h, long e, int l, const int *ijk, int mi, double *nh) { subcell_normal(*(Mesh *)h, e, l, ijk, mi, nh); }
 void oracle_shock_indicator(void *h, const double *u, double s, double amin, double amax, double *alpha, int smooth) {
   shock_indicator(*(Mesh *)h, u, s, amin, amax, alpha, smooth != 0);
 }
