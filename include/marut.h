@@ -122,9 +122,24 @@ marut_status marut_chem_implicit(marut_mesh *mesh, double *u, double dt, int *sw
  *   E = max(E_high^N/E_tot^N, E_high^(N-1)/E_tot^(N-1)),  alpha = 1/(1 + exp(-(s/T)(E - T))),
  *   T = 0.5*10^(-1.8 (N+1)^(1/4)),  alpha < alpha_min -> 0,  alpha > alpha_max -> alpha_max,
  * then, if smooth != 0, alpha_e <- max(alpha_e, alpha_e') over the elements e' sharing a face (conforming or mortar).
- * alpha: DEVICE, [n_elem].  EULER / NAVIER_STOKES meshes.  The blended DG/FV residual (eq. 11, 42) is not built. */
+ * alpha: DEVICE, [n_elem].  EULER / NAVIER_STOKES meshes.  Feed it to marut_set_blend for the blended residual. */
 marut_status marut_shock_indicator(marut_mesh *mesh, const double *u, double s, double alpha_min, double alpha_max,
                                    int smooth, double *alpha, void *cuda_stream);
+
+/* Blended DG / sub-cell finite-volume volume residual (eq. 11, 655-672 eq. 42; DESIGN.md
+ * reading R16):  R_i = (1 - alpha_e) R_i^(split) + alpha_e R_i^(FV), with the first-order finite-volume residual on the
+ * LGL sub-cell grid
+ *   R_i^FV = -(1/J_i) sum_l ( fhat^l_{i_l+1/2} - fhat^l_{i_l-1/2} ) / w_{i_l},
+ * interior sub-cell interfaces carrying the Rusanov flux F*(U_m, U_m+1; nhat^l_{m+1/2}) with the sub-cell normals
+ * nhat^l_{m+1/2} = Ja^l_0 + sum_{q<=m} w_q sum_r D_qr Ja^l_r, the two outermost ones the element's own flux (completed by
+ * the surface lift of eq. 12, which both residuals share).
+ * alpha: DEVICE, [n_elem], values in [0,1] -- normally the output of marut_shock_indicator for the same state.  The
+ * pointer is KEPT, not copied: the caller owns the buffer, may rewrite it between stages (the paper recomputes it once
+ * per Runge-Kutta substage), and must keep it alive until marut_set_blend(mesh, NULL) or marut_mesh_destroy.
+ * NULL switches the blending off (default).  MARUT_EULER meshes; marut_rhs / marut_ssprk_stage return EINVAL while a
+ * blending field is set unless the volume form is MARUT_VOLUME_SPLIT_RANOCHA (eq. 11 blends the split form).  On a
+ * curved mesh the first call allocates and fills the sub-cell normals ([n_elem][dim][dim][n^dim] doubles). */
+marut_status marut_set_blend(marut_mesh *mesh, const double *alpha);
 
 /* REACTING_EULER meshes: whether L(u) of marut_rhs / marut_ssprk_stage includes the explicit chemistry source S(u)
  * (on != 0, the default) or is the transport operator T alone (on == 0), as the Strang split of eq. 24 needs:

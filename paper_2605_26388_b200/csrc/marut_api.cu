@@ -55,6 +55,8 @@ struct marut_mesh {
   MechDev *d_mech = nullptr;
   double *d_Vinv = nullptr;  // [n][n] nodal -> orthonormal Legendre modal (shock indicator)
   double *d_araw = nullptr;  // [ne] unsmoothed blending coefficient (allocated on first use)
+  const double *d_alpha = nullptr;  // caller-owned blending field of eq. 11 (marut_set_blend), or NULL
+  double *d_subn = nullptr;  // curved meshes: sub-cell normals [e][l][c][node] (allocated by the first marut_set_blend)
   unsigned long long *d_red = nullptr;
   unsigned long long *h_red = nullptr;  // pinned
   long launches = 0;
@@ -229,7 +231,7 @@ extern "C" void marut_mesh_destroy(marut_mesh *m) {
   if (!m) return;
   cudaDeviceSynchronize();
   cudaFree(m->d_metric); cudaFree(m->d_fnorm); cudaFree(m->d_conn); cudaFree(m->d_mortar_fine); cudaFree(m->d_mortar_mat);
-  cudaFree(m->d_Vinv); cudaFree(m->d_araw); cudaFree(m->d_bc); cudaFree(m->d_S); cudaFree(m->d_T); cudaFree(m->d_mech); cudaFree(m->d_red);
+  cudaFree(m->d_Vinv); cudaFree(m->d_araw); cudaFree(m->d_subn); cudaFree(m->d_bc); cudaFree(m->d_S); cudaFree(m->d_T); cudaFree(m->d_mech); cudaFree(m->d_red);
   if (m->h_red) cudaFreeHost(m->h_red);
   delete m;
 }
@@ -491,6 +493,13 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.ca = ca; P.cb = cb; P.cc = cc;
   P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne;
   memcpy(P.D, m->D, sizeof(P.D));
+  P.alpha = nullptr; P.subn = m->d_subn;
+  for (int i = 0; i < MAX_NP; ++i) P.inv_w[i] = (i < m->np) ? 1.0 / m->w[i] : 0.0;
+  if (m->d_alpha) {
+    if (m->physics != MARUT_EULER || m->volume_form != MARUT_VOLUME_SPLIT_RANOCHA)
+      return fail(MARUT_EINVAL, "a blending field is set: the DG/FV blend needs MARUT_VOLUME_SPLIT_RANOCHA (eq. 11)");
+    P.alpha = m->d_alpha;
+  }
   cudaError_t e;
   switch (m->physics) {
     case MARUT_EULER:
@@ -508,6 +517,56 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   if (e == cudaErrorNotSupported) return fail(MARUT_EINVAL, "no kernel instantiated for dim=%d N=%d physics=%d", m->dim, m->N, m->physics);
   if (e != cudaSuccess) return fail(MARUT_ECUDA, "stage kernel: %s", cudaGetErrorString(e));
   m->launches++;
+  return MARUT_OK;
+}
+
+// sub-cell normals of a curved mesh (R16): nhat^l_{i+1/2} = Ja^l_0 + sum_{q<=i} w_q sum_r D_qr Ja^l_r along the
+// line through the node in direction l; one thread per (element, l, c, node); stored at the node on the interface's
+// lower side (the entry of the line's last node is Ja^l_N and unused)
+struct SubnParams {
+  const double *metric;
+  double *subn;
+  long ne;
+  int dim, np, nn;
+  double D[MAX_NP * MAX_NP], w[MAX_NP];
+};
+__global__ void subcell_normals_kernel(const __grid_constant__ SubnParams P) {
+  const long total = P.ne * P.dim * P.dim * P.nn;
+  const int md = P.dim * P.dim + 1;
+  for (long g = blockIdx.x * (long)blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
+    const int p = (int)(g % P.nn);
+    const long r1 = g / P.nn;
+    const int c = (int)(r1 % P.dim), l = (int)((r1 / P.dim) % P.dim);
+    const long e = r1 / (P.dim * P.dim);
+    int st = 1;
+    for (int k = 0; k < l; ++k) st *= P.np;
+    const int il = (p / st) % P.np;
+    const double *line = P.metric + (e * md + l * P.dim + c) * P.nn + (p - il * st);
+    double nh = line[0];
+    for (int q = 0; q <= il; ++q) {
+      double s = 0.0;
+      for (int r = 0; r < P.np; ++r) s += P.D[q * P.np + r] * line[r * st];
+      nh += P.w[q] * s;
+    }
+    P.subn[g] = nh;
+  }
+}
+
+extern "C" marut_status marut_set_blend(marut_mesh *m, const double *alpha) {
+  if (!m) return fail(MARUT_EINVAL, "NULL argument");
+  if (!alpha) { m->d_alpha = nullptr; return MARUT_OK; }
+  if (m->physics != MARUT_EULER) return fail(MARUT_EINVAL, "the DG/FV blend is implemented for MARUT_EULER only");
+  if (!m->affine && !m->d_subn) {
+    const size_t n = (size_t)m->ne * m->dim * m->dim * m->nn;
+    CUDA_TRY(cudaMalloc(&m->d_subn, n * sizeof(double)));
+    SubnParams S;
+    S.metric = m->d_metric; S.subn = m->d_subn; S.ne = m->ne; S.dim = m->dim; S.np = m->np; S.nn = m->nn;
+    memcpy(S.D, m->D, sizeof(S.D)); memcpy(S.w, m->w, sizeof(S.w));
+    subcell_normals_kernel<<<(unsigned)std::min<size_t>((n + 255) / 256, 148u * 16u), 256>>>(S);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaDeviceSynchronize());
+  }
+  m->d_alpha = alpha;
   return MARUT_OK;
 }
 

@@ -181,6 +181,94 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
     for (int v = 0; v < NVAR; ++v) R[v] *= 2.0;
   }
 
+  // ---- phase B (only with a blending field; block-uniform branch): first-order finite-volume residual on the LGL
+  // sub-cell grid and the convex blend of eq. 11 / 42 (reading R16).  Node i evaluates the Rusanov flux of the
+  // sub-cell interface i+1/2 of each direction from the stash (no division, no square root on affine elements) and
+  // leaves it in the pair buffer for node i+1; the outermost interfaces take the element's own flux, which the lift
+  // of phase D turns into the interface flux.
+  if (P.alpha != nullptr) {
+    __syncthreads();                         // the pair buffer is free again
+    double *Fv = Pair;                       // [l][v][TILE] at the slices of distance 1
+    double Rf[NVAR];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Rf[v] = 0.0;
+    if (active) {
+#pragma unroll
+      for (int l = 0; l < DIM; ++l) {
+        const int ql = (l == 0) ? qi : ((l == 1) ? qj : qk);
+        const int st = G::stride(l);
+        const double iw = P.inv_w[ql];
+        double Ji[DIM];
+#pragma unroll
+        for (int c = 0; c < DIM; ++c) Ji[c] = AFFINE ? Msm[el * MDP + l * DIM + c] : __ldg(&P.metric[(e * MD + l * DIM + c) * NN + p]);
+        if (ql == 0 || ql == NP - 1) {
+          const double sg = (ql == 0) ? -iw : iw;
+          double vn = 0.0;
+#pragma unroll
+          for (int c = 0; c < DIM; ++c) vn += vi[c] * Ji[c];
+          Rf[0] += sg * (U[0] * vn);
+#pragma unroll
+          for (int c = 0; c < DIM; ++c) Rf[1 + c] += sg * (U[1 + c] * vn + pi_ * Ji[c]);
+          Rf[1 + DIM] += sg * ((U[1 + DIM] + pi_) * vn);
+        }
+        if (ql < NP - 1) {
+          const int pm = tid + st;
+          double nv[DIM], nrm;
+          if constexpr (AFFINE) {
+#pragma unroll
+            for (int c = 0; c < DIM; ++c) nv[c] = Ji[c];
+            nrm = Msm[el * MDP + MD + l];
+          } else {
+            double n2 = 0.0;
+#pragma unroll
+            for (int c = 0; c < DIM; ++c) {
+              nv[c] = __ldg(&P.subn[((e * DIM + l) * DIM + c) * NN + p]);
+              n2 += nv[c] * nv[c];
+            }
+            nrm = sqrt(n2);
+          }
+          double Up[NVAR], vnm = 0.0, vnp = 0.0;
+#pragma unroll
+          for (int v = 0; v < NVAR; ++v) Up[v] = Ust[v * TILE + pm];
+          const double pp = Ust[(NVAR + 1) * TILE + pm], ap = Ust[(NVAR + 2) * TILE + pm];
+          const double am = Ust[(NVAR + 2) * TILE + tid];
+#pragma unroll
+          for (int c = 0; c < DIM; ++c) {
+            vnm += vi[c] * nv[c];
+            vnp += Lns[(3 + c) * TILE + pm] * nv[c];
+          }
+          const double hl = 0.5 * fmax(fabs(vnm) + am * nrm, fabs(vnp) + ap * nrm);
+          double F[NVAR];
+          F[0] = 0.5 * (U[0] * vnm + Up[0] * vnp) - hl * (Up[0] - U[0]);
+#pragma unroll
+          for (int c = 0; c < DIM; ++c)
+            F[1 + c] = 0.5 * ((U[1 + c] * vnm + pi_ * nv[c]) + (Up[1 + c] * vnp + pp * nv[c])) - hl * (Up[1 + c] - U[1 + c]);
+          F[1 + DIM] = 0.5 * ((U[1 + DIM] + pi_) * vnm + (Up[1 + DIM] + pp) * vnp) - hl * (Up[1 + DIM] - U[1 + DIM]);
+#pragma unroll
+          for (int v = 0; v < NVAR; ++v) {
+            Rf[v] += iw * F[v];
+            Fv[((l * NS) * NVAR + v) * TILE + tid] = F[v];
+          }
+        }
+      }
+    }
+    __syncthreads();
+    if (active) {
+#pragma unroll
+      for (int l = 0; l < DIM; ++l) {
+        const int ql = (l == 0) ? qi : ((l == 1) ? qj : qk);
+        if (ql == 0) continue;
+        const double iw = P.inv_w[ql];
+        const double *fb = Fv + (l * NS) * NVAR * TILE + tid - G::stride(l);
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Rf[v] -= iw * fb[v * TILE];
+      }
+      const double al = __ldg(&P.alpha[e]);
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) R[v] = (1.0 - al) * R[v] + al * Rf[v];
+    }
+  }
+
   // u_n for the final combination: issued before the face tasks, consumed after the last barrier (u_out may alias
   // u_n: only this thread writes these locations, later)
   double Un[NVAR];

@@ -1,0 +1,137 @@
+"""GPU parity of the blended DG / sub-cell finite-volume volume residual (PAPER.md:187-191
+eq. 11, 655-672 eq. 42; R16): marut_set_blend + marut_rhs / marut_ssprk_stage against the oracle, element by
+element, on affine and curved meshes in 2-D and 3-D, the quadtree mortar mesh, and the shock-capturing composition
+indicator -> blend -> stage on the Mach-10 shock."""
+import math
+
+import numpy as np
+import pytest
+
+import workloads as wl
+from parity_util import RHS_TOL, RUN_TOL, gpu_run, parity_error
+
+pytestmark = pytest.mark.gpu
+
+
+def _mesh(dim, N, cells, curved):
+    lo, hi = (0.0,) * dim, ((10.0,) * 2 if dim == 2 else (2 * math.pi,) * 3)
+    counts = (cells,) * dim
+    warp = wl.sine_warp(counts, lo, hi, k=1) if curved else None
+    return wl.cartesian_mesh(dim, N, counts, lo, hi, warp=warp)
+
+
+def _alpha(ne, seed=3):
+    a = np.random.default_rng(seed).uniform(0.0, 1.0, ne)
+    a[0], a[1], a[ne - 1] = 0.0, 1.0, 1.0          # pure DG, pure FV, and the (ragged) last CTA
+    return a
+
+
+CASES = [(2, N, 5, curved) for N in (1, 2, 3, 4, 5) for curved in (False, True)] + \
+        [(3, N, 3, curved) for N in (1, 2, 3, 4, 5) for curved in (False, True)]
+
+
+@pytest.mark.parametrize("dim,N,cells,curved", CASES)
+def test_blended_rhs_and_stage(dim, N, cells, curved):
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    m = _mesh(dim, N, cells, curved)
+    m.volume_form = 1
+    u0 = wl.isentropic_vortex(m) if dim == 2 else wl.taylor_green(m, noise=1e-2)
+    om, gm = oracle.OracleMesh(m), mb.MarutMesh(m)
+    a = _alpha(m.n_elem)
+    om.set_blend(a)
+    ad = torch.from_numpy(a).cuda()
+    gm.set_blend(ad)
+    u = torch.from_numpy(u0).cuda()
+    du = torch.empty_like(u)
+    gm.rhs(u, du)
+    torch.cuda.synchronize()
+    ref = om.rhs(u0)
+    assert parity_error(du.cpu().numpy(), ref).max() <= RHS_TOL
+    om.set_blend(None)
+    assert np.abs(ref - om.rhs(u0)).max() > 1e-3 * np.abs(ref).max()       # the blend is not a no-op on this input
+    om.set_blend(a)
+    dt = om.max_dt(u0, 0.5)
+    un_h = u0 * (1.0 + 1e-3)
+    out = torch.empty_like(u)
+    gm.stage(2, dt, 0.0, torch.from_numpy(un_h).cuda(), u, out)
+    torch.cuda.synchronize()
+    assert parity_error(out.cpu().numpy(), om.ssprk_stage(2, dt, 0.0, un_h, u0)).max() <= RHS_TOL
+    # the pointer is kept: rewriting the field takes effect at the next call; alpha = 0 is the split form bit for bit
+    ad.zero_()
+    gm.rhs(u, du)
+    gm.set_blend(None)
+    du0 = torch.empty_like(u)
+    gm.rhs(u, du0)
+    torch.cuda.synchronize()
+    assert torch.equal(du, du0)
+    gm.close()
+
+
+def test_blend_needs_the_split_form():
+    import torch
+
+    import paper_2605_26388_b200 as mb
+
+    m = _mesh(2, 3, 4, False)
+    gm = mb.MarutMesh(m)
+    u = torch.from_numpy(wl.isentropic_vortex(m)).cuda()
+    gm.set_blend(torch.zeros(m.n_elem, dtype=torch.float64, device="cuda"))
+    with pytest.raises(mb.MarutError):
+        gm.rhs(u, torch.empty_like(u))
+    gm.set_blend(None)
+    gm.rhs(u, torch.empty_like(u))
+    gm.close()
+    ns = _mesh(2, 3, 4, False)
+    ns.physics, ns.mu = wl.NAVIER_STOKES, 0.01
+    gn = mb.MarutMesh(ns)
+    with pytest.raises(mb.MarutError):
+        gn.set_blend(torch.zeros(ns.n_elem, dtype=torch.float64, device="cuda"))
+    gn.close()
+
+
+@pytest.mark.parametrize("cells", [16, 32])
+def test_shock_capturing_composition_on_the_mortar_mesh(cells):
+    """Mach-10 shock on the quadtree mesh (2:1 mortars, boundary states): per stage alpha = indicator(u), then the blended
+    stage -- the order the paper states -- for a few SSP-RK33 steps on both sides"""
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    c = wl.make_case("c4", cells=cells)
+    c.mesh.volume_form = 1
+    om, gm = oracle.OracleMesh(c.mesh), mb.MarutMesh(c.mesh)
+    ne = c.mesh.n_elem
+    kw = dict(s=9.21024, alpha_min=1e-3, alpha_max=0.5, smooth=True)
+    u = torch.from_numpy(c.u0).cuda()
+    ua, ub = torch.empty_like(u), torch.empty_like(u)
+    alpha = torch.zeros(ne, dtype=torch.float64, device="cuda")
+    gm.set_blend(alpha)
+    uh = c.u0.copy()
+    seen = 0.0
+    for _ in range(3):
+        dt = om.max_dt(uh, c.cfl)
+        assert abs(gm.max_dt(u, c.cfl) - dt) <= 1e-12 * dt
+        # oracle: three stages, each with its own indicator field
+        stage_in, un = uh, uh
+        gin = u
+        for k, gout in zip(range(3), (ua, ub, u)):
+            a_h = om.shock_indicator(stage_in, **kw)
+            om.set_blend(a_h)
+            gm.shock_indicator(gin, alpha, **kw)
+            torch.cuda.synchronize()
+            assert np.abs(alpha.cpu().numpy() - a_h).max() <= 1e-9
+            seen = max(seen, a_h.max())
+            stage_in = om.ssprk_stage(k, dt, 0.0, un, stage_in)
+            gm.stage(k, dt, 0.0, u, gin, gout)
+            gin = gout
+        uh = stage_in
+    torch.cuda.synchronize()
+    assert seen == 0.5                                                     # the shock saturates the indicator at alpha_max
+    assert parity_error(u.cpu().numpy(), uh).max() <= RUN_TOL
+    assert uh[:, 0, :].min() > 0
+    gm.close()
