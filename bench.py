@@ -29,14 +29,26 @@ if ROOT not in sys.path:
 METRIC = "DG RHS+SSPRK3 DOF-stage updates/s (FP64)"
 UNIT = "DOF-stage/s"
 # bounded oracle samples: (cells per direction, target seconds)
-ORACLE_SAMPLE_CELLS = {"c1": None, "c2": 12, "c2s": 12, "c3": 16, "c4": 64, "c4w": 64, "c5": 8}
+ORACLE_SAMPLE_CELLS = {"c1": None, "c2": 12, "c2s": 12, "c3": 16, "c4": 64, "c4w": 64, "c4b": 64, "c5": 8}
+# c4b: per-stage Hennemann-Gassner indicator (binding defaults, R15) feeding the DG/FV blend
+SHOCK_CAPTURE = dict(s=9.21024, alpha_min=1e-3, alpha_max=0.5, smooth=True)
 
 
 def make_workload(name, cells=None):
     """c1..c5, c4w: the configs of BASELINE.json (workloads.make_case); c2s: c2 with the entropy-stable split-form
-    volume integral"""
+    volume integral; c4b: c4w as a shock-capturing run -- split form, and in
+    every Runge-Kutta stage the shock indicator of the stage's input state followed by the blended DG/FV stage"""
     import workloads as wl
 
+    if name == "c4b":
+        c = wl.make_case("c4w", cells=cells)
+        c.mesh.volume_form = 1
+        c.name = "c4b"
+        c.shock_capture = dict(SHOCK_CAPTURE)
+        # shock profile one fine element wide: the indicator flags it (alpha_e reaches alpha_max along the shock); the
+        # 6-element profile of c4 / c4w is resolved at N = 3 and would leave alpha_e = 0 everywhere
+        c.u0 = wl.mach10_shock(c.mesh, half_width=1.0 * c.mesh.info["h_fine"])
+        return c
     if name == "c2s":
         c = wl.make_case("c2", cells=cells)
         c.mesh.volume_form = 1
@@ -50,6 +62,8 @@ def workload_name(case):
     phys = {0: "Euler", 1: "Navier-Stokes (BR1)", 2: "reacting Euler, 5 species"}[m.physics]
     if getattr(m, "volume_form", 0):
         phys += " (entropy-stable split form, Ranocha flux)"
+    if getattr(case, "shock_capture", None):
+        phys += " + per-stage shock indicator and DG/FV sub-cell blend"
     return (f"{case.name}: {m.dim}-D {phys}, N={m.N}, {m.n_elem} elements, {m.n_elem * m.nn} nodes, "
             f"{m.n_dof} DOF, {len(m.mortar)} mortars, {len(m.bface)} boundary faces")
 
@@ -133,6 +147,22 @@ class ClockSampler:
 
 
 # --------------------------------------------------------------------------------------------- oracle arm
+def oracle_advance(om, case, u, n):
+    """n SSP-RK33 steps of the oracle, dt from its own CFL reduction; shock-capturing workloads recompute the blending
+    field from the input state of every stage"""
+    sc = getattr(case, "shock_capture", None)
+    if not sc:
+        return om.run(u, n, cfl=case.cfl)[0]
+    for _ in range(n):
+        dt = om.max_dt(u, case.cfl)
+        un, uin = u, u
+        for k in range(3):
+            om.set_blend(om.shock_indicator(uin, **sc))
+            uin = om.ssprk_stage(k, dt, 0.0, un, uin)
+        u = uin
+    return u
+
+
 def oracle_sample(workload, budget_s):
     """time the CPU oracle (as it stands, never tuned) on a bounded sample of the workload: the same config
     at fewer elements per direction, as many SSP-RK33 steps (dt from its own CFL reduction) as fit budget_s."""
@@ -143,11 +173,11 @@ def oracle_sample(workload, budget_s):
     c = make_workload(workload, cells=cells)
     om = oracle.OracleMesh(c.mesh)
     t0 = time.perf_counter()
-    u = om.run(c.u0, 1, cfl=c.cfl)[0]          # calibration step (counted)
+    u = oracle_advance(om, c, c.u0, 1)          # calibration step (counted)
     t1 = time.perf_counter() - t0
     n = max(1, min(200, int(budget_s / max(t1, 1e-6)) - 1))
     t0 = time.perf_counter()
-    om.run(u, n, cfl=c.cfl)
+    oracle_advance(om, c, u, n)
     t = time.perf_counter() - t0
     per_step = t / n
     return {"case": c, "steps": n, "s_per_step": per_step, "value": c.mesh.n_dof * 3 / per_step,
@@ -170,14 +200,14 @@ def run_reference(args):
     om = oracle.OracleMesh(c.mesh)
     # one "step" of this arm = `inner` SSP-RK33 steps of the sample, sized to per_step_budget
     t0 = time.perf_counter()
-    u = om.run(c.u0, 1, cfl=c.cfl)[0]
+    u = oracle_advance(om, c, c.u0, 1)
     t1 = time.perf_counter() - t0
     inner = max(1, min(50, int(per_step_budget / max(t1, 1e-6))))
     for _ in range(args.warmup):
-        u = om.run(u, inner, cfl=c.cfl)[0]
+        u = oracle_advance(om, c, u, inner)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        u = om.run(u, inner, cfl=c.cfl)[0]
+        u = oracle_advance(om, c, u, inner)
     t = time.perf_counter() - t0
     value = c.mesh.n_dof * 3 * inner * args.steps / t
     sample = (f"{args.workload} at {c.mesh.n_elem} elements ({c.mesh.n_dof} DOF); one bench step = {inner} SSP-RK33 steps "
@@ -260,12 +290,19 @@ def run_cuda(args):
     # stages read u0 directly, so the restart costs no extra copy and no extra traffic).
     u0_dev = u.clone()
     counter = [0]
+    sc = getattr(case, "shock_capture", None)
+    alpha = None
+    if sc:
+        alpha = torch.zeros(mesh.n_elem, dtype=torch.float64, device=u.device)
+        gm.set_blend(alpha)
 
     def step(ev=None):
         src = u0_dev if counter[0] % case.steps == 0 else u
         counter[0] += 1
         dt = gm.max_dt(src, cfl)
         for s, (un, uin, uout) in enumerate(((src, src, ua), (src, ua, ub), (src, ub, u))):
+            if sc:
+                gm.shock_indicator(uin, alpha, **sc)
             if ev is not None:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
@@ -309,12 +346,21 @@ def run_cuda(args):
         g = gm if k == 0 else mb.MarutMesh(mesh)
         lanes.append({"st": st, "gm": g, "u": torch.empty_like(u), "ua": torch.empty_like(u), "ub": torch.empty_like(u),
                       "out": torch.empty_like(u0_host).pin_memory()})
+        if sc:
+            lanes[k]["alpha"] = alpha if k == 0 else torch.zeros_like(alpha)
+            g.set_blend(lanes[k]["alpha"])
 
     def e2e_step(k):
         L = lanes[k % 2]
         with torch.cuda.stream(L["st"]):
             L["u"].copy_(u0_host, non_blocking=True)
-            L["gm"].step(L["u"], L["ua"], L["ub"], L["gm"].max_dt(L["u"], cfl))
+            g, dt = L["gm"], L["gm"].max_dt(L["u"], cfl)
+            if sc:
+                for s_, (uin, uout) in enumerate(((L["u"], L["ua"]), (L["ua"], L["ub"]), (L["ub"], L["u"]))):
+                    g.shock_indicator(uin, L["alpha"], **sc)
+                    g.stage(s_, dt, 0.0, L["u"], uin, uout)
+            else:
+                g.step(L["u"], L["ua"], L["ub"], dt)
             L["out"].copy_(L["u"], non_blocking=True)
 
     for k in range(4):
@@ -348,7 +394,7 @@ def run_cuda(args):
                 prof = json.load(open(tpath))
             except Exception:
                 prof = {}
-        kernels = {0: "stage_split_kernel (fused Euler stage, split-form volume integral)" if getattr(mesh, "volume_form", 0) else "stage_node_kernel (fused Euler stage)", 1: "gradient_kernel + stage_phys_kernel (BR1 gradient sweep + fused NS stage)",
+        kernels = {0: ("stage_split_kernel (fused Euler stage, split-form volume integral" + (" blended with the sub-cell FV residual)" if sc else ")")) if getattr(mesh, "volume_form", 0) else "stage_node_kernel (fused Euler stage)", 1: "gradient_kernel + stage_phys_kernel (BR1 gradient sweep + fused NS stage)",
                    2: "eos_kernel + stage_phys_kernel (mixture temperature + fused reacting stage)"}[mesh.physics]
         roof = {"bound": "hbm", "kernel": "marut_ssprk_stage: " + kernels, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": prof.get(args.workload), "peak_source": peak_src, "bytes_per_dof_stage": b_alg,
@@ -370,7 +416,7 @@ def run_cuda(args):
                 "config": {"workload": workload_name(case), "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": f"inputs larger than L2 ({3 * n_dof * 8 / 1e6:.0f} MB of state buffers vs 126 MB)"
                                  if 3 * n_dof * 8 > 126e6 else "state fits L2 (launch/latency-bound case; no flush)",
-                           "step": "marut_max_dt + 3 x marut_ssprk_stage", "cfl": cfl, "restart_from_u0_every_steps": case.steps, "affine": bool(affine)},
+                           "step": "marut_max_dt + 3 x (marut_shock_indicator + blended marut_ssprk_stage)" if sc else "marut_max_dt + 3 x marut_ssprk_stage", "cfl": cfl, "restart_from_u0_every_steps": case.steps, "affine": bool(affine)},
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n_dof * 8, "d2h_bytes_per_step": n_dof * 8 + 8,
                         "ms_per_step": e2e_ms / args.steps,
