@@ -84,6 +84,8 @@ def _setup(L):
         L.oracle_chem_implicit_node.argtypes = [vp, vp, C.c_double, C.c_double]
         L.oracle_set_volume_form.restype = C.c_int
         L.oracle_set_volume_form.argtypes = [vp, C.c_int]
+        L.oracle_positivity_floor.restype = C.c_long
+        L.oracle_positivity_floor.argtypes = [vp, vp, C.c_double, C.c_double]
         L.oracle_set_blend.restype = C.c_int
         L.oracle_set_blend.argtypes = [vp, vp]
         L.oracle_fv_volume.argtypes = [vp, vp, vp]
@@ -235,6 +237,14 @@ class OracleMesh:
         a = np.zeros(self.mesh.n_elem)
         self.L.oracle_shock_indicator(self.h, _p(u), s, alpha_min, alpha_max, _p(a), int(smooth))
         return a
+
+    def positivity_floor(self, u, rho_min=1e-6, p_min=5e-7):
+        """O18 (reading R17): returns (floored copy of u, number of nodes changed)"""
+        v = _f64(u).copy()
+        n = self.L.oracle_positivity_floor(self.h, _p(v), rho_min, p_min)
+        if n < 0:
+            raise ValueError("the positivity floor is defined for the ideal-gas systems only")
+        return v, int(n)
 
     def set_blend(self, alpha):
         """eq. 11 / 42: per-element blending coefficients alpha_e (copied) of the DG / sub-cell FV volume residual;

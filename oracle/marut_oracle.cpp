@@ -584,6 +584,32 @@ static void blend_fv(const Mesh &m, const double *u, long e, double *du) {
 }
 
 // ---------------------------------------------------------------------------
+// O18. Per-stage positivity floor ("a per-stage positivity floor enforces rho >= 1e-6 and
+// p >= 5e-7"; how is not stated -- DESIGN.md reading R17): at every node, first rho <- max(rho, rho_min) with the
+// momentum kept, then with p = (gamma-1)(E - |m|^2/(2 rho)) of the floored density, if p < p_min the total energy is
+// raised to E = p_min/(gamma-1) + |m|^2/(2 rho).  Nodes already above both floors are not touched.  Returns the
+// number of nodes changed.  Ideal gas (EULER / NAVIER_STOKES).
+// ---------------------------------------------------------------------------
+static long positivity_floor(const Mesh &m, double *u, double rho_min, double p_min) {
+  const int nn = m.nn, d = m.dim, nvar = m.nvar;
+  long changed = 0;
+  for (long e = 0; e < m.ne; ++e)
+    for (int p = 0; p < nn; ++p) {
+      double *U = &u[(size_t)e * nvar * nn + p];     // variable v at U[v * nn]
+      bool ch = false;
+      double rho = U[0];
+      if (rho < rho_min) { rho = rho_min; U[0] = rho; ch = true; }
+      double m2 = 0.0;
+      for (int c = 0; c < d; ++c) m2 += U[(size_t)(1 + c) * nn] * U[(size_t)(1 + c) * nn];
+      const double ke = 0.5 * m2 / rho;
+      const double pr = (m.gamma - 1.0) * (U[(size_t)(1 + d) * nn] - ke);
+      if (pr < p_min) { U[(size_t)(1 + d) * nn] = p_min / (m.gamma - 1.0) + ke; ch = true; }
+      changed += ch ? 1 : 0;
+    }
+  return changed;
+}
+
+// ---------------------------------------------------------------------------
 // O4 + O6. Inviscid residual: volume term (eq. 9) and surface lift (eq. 12).
 // ---------------------------------------------------------------------------
 static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
@@ -1103,6 +1129,11 @@ int oracle_set_blend(void *h, const double *alpha) {
   if (alpha && m->physics != EULER) return 1;
   if (alpha) m->alpha.assign(alpha, alpha + m->ne); else m->alpha.clear();
   return 0;
+}
+long oracle_positivity_floor(void *h, double *u, double rho_min, double p_min) {
+  Mesh &m = *(Mesh *)h;
+  if (m.physics == REACTING_EULER) return -1;
+  return positivity_floor(m, u, rho_min, p_min);
 }
 void oracle_fv_volume(void *h, const double *u, double *rfv) {
   Mesh &m = *(Mesh *)h;

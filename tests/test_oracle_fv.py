@@ -150,3 +150,31 @@ def test_pure_fv_run_converges_to_the_vortex_at_first_order():
         errs_dg.append(np.einsum("en,en,n->", np.abs(udg - exact)[:, 0, :], J, W) / 100.0)
     assert all(f > 3 * d for f, d in zip(errs, errs_dg)) and errs[2] > 100 * errs_dg[2]
     assert 1.3 < errs[0] / errs[1] < 2.2 and 1.5 < errs[1] / errs[2] < 2.2
+
+
+def test_positivity_floor_closed_forms():
+    """O18 (reading R17): hand-built nodes below / above the floors"""
+    m = wl.cartesian_mesh(2, 1, (2, 1), (0.0, 0.0), (2.0, 1.0))
+    om = oracle.OracleMesh(m)
+    g, rmin, pmin = 1.4, 1e-6, 5e-7
+    u = np.empty((2, 4, 4))
+    good = _cons(1.2, [0.3, -0.4], 0.9)
+    u[:] = good[None, :, None]
+    u[0, :, 1] = [1e-9, 2e-7, -1e-7, 3.0]                      # density below the floor, pressure fine afterwards
+    u[0, :, 2] = _cons(0.8, [2.0, 1.0], 1.0) - [0, 0, 0, 2.6]   # negative pressure (p = 1 - 0.4*2.6 < 0)
+    u[1, :, 3] = [1e-8, 0.0, 0.0, 0.0]                          # both: vacuum
+    u[1, :, 0] = _cons(2.0, [0.0, 0.0], pmin)                   # exactly at the pressure floor: untouched
+    v, n = om.positivity_floor(u, rmin, pmin)
+    assert n == 3
+    untouched = np.ones((2, 4), bool)
+    untouched[0, 1] = untouched[0, 2] = untouched[1, 3] = False
+    assert np.array_equal(v.transpose(0, 2, 1)[untouched], u.transpose(0, 2, 1)[untouched])   # bit for bit
+    a = v[0, :, 1]
+    assert a[0] == rmin and np.array_equal(a[1:], u[0, 1:, 1])
+    b = v[0, :, 2]
+    assert np.array_equal(b[:3], u[0, :3, 2])
+    assert (g - 1) * (b[3] - 0.5 * (b[1] ** 2 + b[2] ** 2) / b[0]) == pytest.approx(pmin, rel=1e-9)
+    c = v[1, :, 3]
+    assert c[0] == rmin and c[1] == 0 and c[2] == 0 and c[3] == pytest.approx(pmin / (g - 1), rel=1e-15)
+    w, n2 = om.positivity_floor(v, rmin, pmin)                  # idempotent up to the rounding of p at the floor
+    assert np.allclose(w, v, rtol=1e-15, atol=0)
