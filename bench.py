@@ -37,7 +37,7 @@ SHOCK_CAPTURE = dict(s=9.21024, alpha_min=1e-3, alpha_max=0.5, smooth=True)
 def make_workload(name, cells=None):
     """c1..c5, c4w: the configs of BASELINE.json (workloads.make_case); c2s: c2 with the entropy-stable split-form
     volume integral; c4b: c4w as a shock-capturing run -- split form, and in
-    every Runge-Kutta stage the shock indicator of the stage's input state followed by the blended DG/FV stage"""
+    every Runge-Kutta stage the shock indicator of the stage's input state, the blended DG/FV stage and the positivity floor"""
     import workloads as wl
 
     if name == "c4b":
@@ -158,7 +158,7 @@ def oracle_advance(om, case, u, n):
         un, uin = u, u
         for k in range(3):
             om.set_blend(om.shock_indicator(uin, **sc))
-            uin = om.ssprk_stage(k, dt, 0.0, un, uin)
+            uin = om.positivity_floor(om.ssprk_stage(k, dt, 0.0, un, uin))[0]
         u = uin
     return u
 
@@ -310,6 +310,8 @@ def run_cuda(args):
             if ev is not None:
                 e1.record(stream)
                 ev.append((e0, e1))
+            if sc:
+                gm.positivity_floor(uout)
         return dt
 
     # ---- device-resident throughput: W warm-up steps, then exactly K timed steps
@@ -359,6 +361,7 @@ def run_cuda(args):
                 for s_, (uin, uout) in enumerate(((L["u"], L["ua"]), (L["ua"], L["ub"]), (L["ub"], L["u"]))):
                     g.shock_indicator(uin, L["alpha"], **sc)
                     g.stage(s_, dt, 0.0, L["u"], uin, uout)
+                    g.positivity_floor(uout)
             else:
                 g.step(L["u"], L["ua"], L["ub"], dt)
             L["out"].copy_(L["u"], non_blocking=True)
@@ -416,7 +419,7 @@ def run_cuda(args):
                 "config": {"workload": workload_name(case), "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": f"inputs larger than L2 ({3 * n_dof * 8 / 1e6:.0f} MB of state buffers vs 126 MB)"
                                  if 3 * n_dof * 8 > 126e6 else "state fits L2 (launch/latency-bound case; no flush)",
-                           "step": "marut_max_dt + 3 x (marut_shock_indicator + blended marut_ssprk_stage)" if sc else "marut_max_dt + 3 x marut_ssprk_stage", "cfl": cfl, "restart_from_u0_every_steps": case.steps, "affine": bool(affine)},
+                           "step": "marut_max_dt + 3 x (marut_shock_indicator + blended marut_ssprk_stage + marut_positivity_floor)" if sc else "marut_max_dt + 3 x marut_ssprk_stage", "cfl": cfl, "restart_from_u0_every_steps": case.steps, "affine": bool(affine)},
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n_dof * 8, "d2h_bytes_per_step": n_dof * 8 + 8,
                         "ms_per_step": e2e_ms / args.steps,

@@ -141,6 +141,14 @@ marut_status marut_shock_indicator(marut_mesh *mesh, const double *u, double s, 
  * curved mesh the first call allocates and fills the sub-cell normals ([n_elem][dim][dim][n^dim] doubles). */
 marut_status marut_set_blend(marut_mesh *mesh, const double *alpha);
 
+/* Per-stage positivity floor ("a per-stage positivity floor enforces rho >= 1e-6 and
+ * p >= 5e-7"; reading R17), in place on u (DEVICE, [n_elem][nvar][n^dim]): at every node
+ *   rho <- max(rho, rho_min), momentum kept;  if (gamma-1)(E - |m|^2/(2 rho)) < p_min:  E <- p_min/(gamma-1) + |m|^2/(2 rho).
+ * Nodes above both floors are not written.  changed_out (HOST, may be NULL): number of nodes changed; asking for it
+ * synchronises the stream.  EULER / NAVIER_STOKES meshes; rho_min, p_min > 0 (else EINVAL). */
+marut_status marut_positivity_floor(marut_mesh *mesh, double *u, double rho_min, double p_min, long *changed_out,
+                                    void *cuda_stream);
+
 /* REACTING_EULER meshes: whether L(u) of marut_rhs / marut_ssprk_stage includes the explicit chemistry source S(u)
  * (on != 0, the default) or is the transport operator T alone (on == 0), as the Strang split of eq. 24 needs:
  *   u^{n+1} = S_{dt/2} o T_dt o S_{dt/2} (u^n) = marut_chem_implicit(dt/2), SSP-RK steps of T, marut_chem_implicit(dt/2). */

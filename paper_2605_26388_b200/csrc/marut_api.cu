@@ -377,8 +377,8 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   const size_t nbc = (size_t)std::max(1, d->n_bc) * m->nvar;
   CUDA_TRY(cudaMalloc(&m->d_bc, nbc * sizeof(double)));
   if (d->n_bc) CUDA_TRY(cudaMemcpy(m->d_bc, d->bc_state, (size_t)d->n_bc * m->nvar * sizeof(double), cudaMemcpyHostToDevice));
-  CUDA_TRY(cudaMalloc(&m->d_red, 4 * sizeof(unsigned long long)));
-  CUDA_TRY(cudaMallocHost(&m->h_red, 4 * sizeof(unsigned long long)));
+  CUDA_TRY(cudaMalloc(&m->d_red, 5 * sizeof(unsigned long long)));   // [0..2] marut_max_dt, [3] marut_chem_implicit, [4] marut_positivity_floor
+  CUDA_TRY(cudaMallocHost(&m->h_red, 5 * sizeof(unsigned long long)));
 
   // ---- metric terms on the device
   const int MD = dim * dim + 1;
@@ -640,6 +640,30 @@ extern "C" marut_status marut_chem_implicit(marut_mesh *m, double *u, double dt,
     CUDA_TRY(cudaStreamSynchronize(st));
     *sweeps_out = (int)(m->h_red[3] & 0xffffffffu);
     if (*sweeps_out > 50) return fail(MARUT_ENOTFINITE, "implicit chemistry: Newton did not converge in 50 sweeps");
+  }
+  return MARUT_OK;
+}
+
+// ------------------------------------------------------------------------------------ positivity floor
+extern "C" marut_status marut_positivity_floor(marut_mesh *m, double *u, double rho_min, double p_min, long *changed_out,
+                                               void *stream) {
+  if (!m || !u) return fail(MARUT_EINVAL, "NULL argument");
+  if (m->physics == MARUT_REACTING_EULER) return fail(MARUT_EINVAL, "marut_positivity_floor: ideal-gas meshes only");
+  if (!(rho_min > 0.0) || !(p_min > 0.0)) return fail(MARUT_EINVAL, "the floors must be > 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  unsigned long long *d_cnt = m->d_red + 4;
+  if (changed_out) CUDA_TRY(cudaMemsetAsync(d_cnt, 0, sizeof(unsigned long long), st));
+  const long total = m->ne * m->nn;
+  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * 32);
+  if (m->dim == 2) positivity_floor_kernel<2><<<grid, 256, 0, st>>>(u, m->gamma, rho_min, p_min, m->ne, m->nn, changed_out ? d_cnt : nullptr);
+  else positivity_floor_kernel<3><<<grid, 256, 0, st>>>(u, m->gamma, rho_min, p_min, m->ne, m->nn, changed_out ? d_cnt : nullptr);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "positivity floor kernel: %s", cudaGetErrorString(e));
+  m->launches++;
+  if (changed_out) {
+    CUDA_TRY(cudaMemcpyAsync(m->h_red + 4, d_cnt, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    *changed_out = (long)m->h_red[4];
   }
   return MARUT_OK;
 }

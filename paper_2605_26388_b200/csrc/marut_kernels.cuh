@@ -611,6 +611,49 @@ __global__ void indicator_smooth_kernel(const double *__restrict__ raw, const in
 }
 
 // ======================================================================================
+// Per-stage positivity floor (R17): one thread per node, in place;
+// rho <- max(rho, rho_min) with the momentum kept, then E raised so that p >= p_min.  Nodes above both floors are not
+// written.  count (may be NULL): number of nodes changed, one atomicAdd per warp that changed any.
+// ======================================================================================
+template <int DIM>
+__global__ void __launch_bounds__(256) positivity_floor_kernel(double *u, double gamma, double rho_min, double p_min, long ne,
+                                                               int nn, unsigned long long *count) {
+  constexpr int NVAR = DIM + 2;
+  const long total = ne * nn;
+  const long span = (long)gridDim.x * blockDim.x;
+  const long rounds = (total + span - 1) / span;     // whole warps stay in the loop for the ballot
+  for (long r = 0; r < rounds; ++r) {
+    const long g = r * span + (long)blockIdx.x * blockDim.x + threadIdx.x;
+    bool ch = false;
+    if (g < total) {
+      const long e = g / nn;
+      double *U = u + e * NVAR * nn + (g - e * nn);
+      double rho = U[0], m2 = 0.0;
+      const double E = U[(long)(1 + DIM) * nn];
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) {
+        const double mc = U[(long)(1 + c) * nn];
+        m2 += mc * mc;
+      }
+      if (rho < rho_min) {
+        rho = rho_min;
+        U[0] = rho;
+        ch = true;
+      }
+      const double ke = 0.5 * m2 / rho;
+      if ((gamma - 1.0) * (E - ke) < p_min) {
+        U[(long)(1 + DIM) * nn] = p_min / (gamma - 1.0) + ke;
+        ch = true;
+      }
+    }
+    if (count != nullptr) {
+      const unsigned b = __ballot_sync(0xffffffffu, ch);
+      if (b != 0u && (threadIdx.x & 31) == 0) atomicAdd(count, (unsigned long long)__popc(b));
+    }
+  }
+}
+
+// ======================================================================================
 // max wave speed / max diffusivity (a10; eq. 17-18): warp-shuffle reduction, one atomicMax per CTA.
 // red[0] = max(|u|_2 + a) ; red[1] = max(mu/rho) ; red[2] = count of non-finite/non-positive speeds
 // (bit patterns of non-negative doubles order like unsigned integers)

@@ -129,12 +129,53 @@ def test_shock_capturing_composition_on_the_mortar_mesh(name, cells, width):
             torch.cuda.synchronize()
             assert np.abs(alpha.cpu().numpy() - a_h).max() <= 1e-9
             seen = max(seen, a_h.max())
-            stage_in = om.ssprk_stage(k, dt, 0.0, un, stage_in)
+            stage_in, n_h = om.positivity_floor(om.ssprk_stage(k, dt, 0.0, un, stage_in))
             gm.stage(k, dt, 0.0, u, gin, gout)
+            assert gm.positivity_floor(gout, want_count=True) == n_h           # per-stage floor
             gin = gout
         uh = stage_in
     torch.cuda.synchronize()
     assert seen == 0.5                                                     # the shock saturates the indicator at alpha_max
     assert parity_error(u.cpu().numpy(), uh).max() <= RUN_TOL
     assert uh[:, 0, :].min() > 0
+    gm.close()
+
+
+@pytest.mark.parametrize("dim,N,cells,ns", [(2, 3, 9, False), (3, 4, 3, False), (3, 2, 4, True)])
+def test_positivity_floor(dim, N, cells, ns):
+    """marut_positivity_floor against the oracle (reading R17): a smooth field with seeded nodes pushed below the density
+    floor, below the pressure floor, and into vacuum; untouched nodes bit for bit, the count exactly"""
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    m = _mesh(dim, N, cells, False)
+    if ns:
+        m.physics, m.mu = wl.NAVIER_STOKES, 0.01
+    u0 = (wl.isentropic_vortex(m) if dim == 2 else wl.taylor_green(m, noise=1e-2)).copy()
+    rng = np.random.default_rng(17)
+    ne, nn = m.n_elem, m.nn
+    pick = rng.random((ne, nn))
+    low_rho, low_p, vac = pick < 0.05, (pick >= 0.05) & (pick < 0.12), (pick >= 0.12) & (pick < 0.15)
+    u0[:, 0, :][low_rho] = 1e-6 * rng.uniform(0.01, 0.99, low_rho.sum())
+    u0[:, dim + 1, :][low_p] *= rng.uniform(-0.5, -0.01, low_p.sum())
+    for v in range(dim + 2):
+        u0[:, v, :][vac] = 1e-9 * rng.uniform(-1, 1, vac.sum())
+    u0[:, 0, :][vac] = 1e-9
+    om, gm = oracle.OracleMesh(m), mb.MarutMesh(m)
+    ref, n_ref = om.positivity_floor(u0)
+    assert n_ref >= (low_rho | low_p | vac).sum() > 10
+    u = torch.from_numpy(u0).cuda()
+    n = gm.positivity_floor(u, want_count=True)
+    g = u.cpu().numpy()
+    assert n == n_ref
+    same = ref == u0
+    assert np.array_equal(g[same], u0[same])
+    assert np.allclose(g, ref, rtol=1e-14, atol=0)
+    gm.positivity_floor(u)                                                # without the count: no synchronisation, same result
+    torch.cuda.synchronize()
+    assert np.allclose(u.cpu().numpy(), ref, rtol=1e-14, atol=0)
+    with pytest.raises(mb.MarutError):
+        gm.positivity_floor(u, rho_min=0.0)
     gm.close()
