@@ -178,3 +178,40 @@ def test_positivity_floor_closed_forms():
     assert c[0] == rmin and c[1] == 0 and c[2] == 0 and c[3] == pytest.approx(pmin / (g - 1), rel=1e-15)
     w, n2 = om.positivity_floor(v, rmin, pmin)                  # idempotent up to the rounding of p at the floor
     assert np.allclose(w, v, rtol=1e-15, atol=0)
+
+
+def _oracle_sod(ne, capture, T=0.2):
+    from sod_util import SHOCK_CAPTURE, sod_exact_on, sod_strip
+
+    m, u = sod_strip(ne)
+    om = oracle.OracleMesh(m)
+    t = 0.0
+    while t < T - 1e-14:
+        dt = min(om.max_dt(u, 0.5), T - t)
+        un, uin = u, u
+        for k in range(3):
+            if capture:
+                om.set_blend(om.shock_indicator(uin, **SHOCK_CAPTURE))
+            uin, _ = om.positivity_floor(om.ssprk_stage(k, dt, 0.0, un, uin))
+        u, t = uin, t + dt
+    _, J = om.metrics()
+    _, w, _ = oracle.operators(m.N)
+    W = np.einsum("j,i->ji", w, w).reshape(-1)
+    l1 = np.einsum("en,en,n->", np.abs(u[:, 0, :] - sod_exact_on(m, T)), J, W) / (2.0 * 2.0 / ne)
+    return l1, u
+
+
+def test_shock_capturing_step_solves_the_sod_problem():
+    """the whole shock-capturing step (indicator -> blended DG/FV stage -> floor) against the exact Riemann solution:
+    first-order L1 convergence (the best a discontinuous solution allows; measured 2.15e-2, 1.13e-2), and the density /
+    pressure stay within the initial bounds, where the unblended split-form DG run undershoots by 23 %"""
+    from sod_util import pressure
+
+    e32, u32 = _oracle_sod(32, True)
+    e64, u64 = _oracle_sod(64, True)
+    assert e32 < 0.025 and 1.6 < e32 / e64 < 2.3
+    for u in (u32, u64):
+        assert u[:, 0].min() > 0.125 - 1e-4 and u[:, 0].max() < 1.0 + 1e-4
+        assert pressure(u).min() > 0.1 - 1e-4
+    _, udg = _oracle_sod(32, False)
+    assert udg[:, 0].min() < 0.11 and pressure(udg).min() < 0.08
