@@ -84,6 +84,8 @@ def _setup(L):
         L.oracle_chem_implicit_node.argtypes = [vp, vp, C.c_double, C.c_double]
         L.oracle_set_volume_form.restype = C.c_int
         L.oracle_set_volume_form.argtypes = [vp, C.c_int]
+        L.oracle_set_boundary_kinds.restype = C.c_int
+        L.oracle_set_boundary_kinds.argtypes = [vp, vp, C.c_int]
         L.oracle_positivity_floor.restype = C.c_long
         L.oracle_positivity_floor.argtypes = [vp, vp, C.c_double, C.c_double]
         L.oracle_set_blend.restype = C.c_int
@@ -237,6 +239,16 @@ class OracleMesh:
         a = np.zeros(self.mesh.n_elem)
         self.L.oracle_shock_indicator(self.h, _p(u), s, alpha_min, alpha_max, _p(a), int(smooth))
         return a
+
+    def set_boundary_kinds(self, kinds):
+        """O8b: per bc id 0 = prescribed exterior state, 1 = outflow (interior state), 2 = inviscid slip wall"""
+        if kinds is None:
+            self.L.oracle_set_boundary_kinds(self.h, None, 0)
+            return
+        k = np.ascontiguousarray(kinds, dtype=np.int32)
+        assert k.shape == (self.mesh.bc_state.shape[0],)
+        if self.L.oracle_set_boundary_kinds(self.h, k.ctypes.data_as(C.c_void_p), len(k)) != 0:
+            raise ValueError("boundary kinds: Euler meshes, values 0..2")
 
     def positivity_floor(self, u, rho_min=1e-6, p_min=5e-7):
         """O18 (reading R17): returns (floored copy of u, number of nodes changed)"""

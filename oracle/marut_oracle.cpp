@@ -289,6 +289,7 @@ struct Mesh {
   int explicit_source = 1;      // reacting: 1 = L includes the chemistry source S(U); 0 = transport operator only (Strang split)
   int volume_form = 0;          // 0: standard strong form (eq. 9); 1: entropy-stable split form (eq. 10)
   std::vector<double> alpha;    // per-element blending coefficient alpha_e of eq. 11 / 42; empty = no blending
+  std::vector<int> bc_kind;     // per bc id: 0 prescribed exterior state, 1 outflow, 2 slip wall (O8b); empty = all 0
 };
 
 static inline int node_index(const Mesh &m, const int *ijk) {
@@ -725,7 +726,20 @@ static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
       const int p = face_node(m, f, a);
       double Um[MAXV], nv[3], Fs[MAXV], Fo[MAXV];
       gather(m, u, e, p, Um); face_normal(m, e, f, p, nv);
-      rusanov(m, Um, &m.bc_state[(size_t)bc * nvar], nv, Fs);
+      // O8b ("enforced weakly through the numerical surface flux"; reading R18): the exterior
+      // state of an outflow face is the interior state, that of an inviscid slip wall the interior state with the
+      // normal momentum reflected, m+ = m- - 2 (m- . nhat) nhat
+      const int bk = m.bc_kind.empty() ? 0 : m.bc_kind[bc];
+      double Ue[MAXV];
+      for (int v = 0; v < nvar; ++v) Ue[v] = (bk == 0) ? m.bc_state[(size_t)bc * nvar + v] : Um[v];
+      if (bk == 2) {
+        double nrm = 0.0, mn = 0.0;
+        for (int c = 0; c < d; ++c) nrm += nv[c] * nv[c];
+        nrm = std::sqrt(nrm);
+        for (int c = 0; c < d; ++c) mn += Um[m.ns + c] * (nv[c] / nrm);
+        for (int c = 0; c < d; ++c) Ue[m.ns + c] = Um[m.ns + c] - 2.0 * mn * (nv[c] / nrm);
+      }
+      rusanov(m, Um, Ue, nv, Fs);
       flux_dot(m, Um, primitives(m, Um), nv, Fo);   lift(e, p, Fs, Fo);
     }
   }
@@ -1128,6 +1142,15 @@ int oracle_set_blend(void *h, const double *alpha) {
   Mesh *m = (Mesh *)h;
   if (alpha && m->physics != EULER) return 1;
   if (alpha) m->alpha.assign(alpha, alpha + m->ne); else m->alpha.clear();
+  return 0;
+}
+// kinds: [n_bc] 0 prescribed state / 1 outflow / 2 slip wall (copied), or NULL for all prescribed
+int oracle_set_boundary_kinds(void *h, const int *kinds, int n) {
+  Mesh *m = (Mesh *)h;
+  if (!kinds) { m->bc_kind.clear(); return 0; }
+  if (m->physics != EULER) return 1;
+  for (int i = 0; i < n; ++i) if (kinds[i] < 0 || kinds[i] > 2) return 2;
+  m->bc_kind.assign(kinds, kinds + n);
   return 0;
 }
 long oracle_positivity_floor(void *h, double *u, double rho_min, double p_min) {
