@@ -141,6 +141,16 @@ marut_status marut_shock_indicator(marut_mesh *mesh, const double *u, double s, 
  * curved mesh the first call allocates and fills the sub-cell normals ([n_elem][dim][dim][n^dim] doubles). */
 marut_status marut_set_blend(marut_mesh *mesh, const double *alpha);
 
+/* Boundary kinds ("wall/slip/outflow"; "enforced weakly through the numerical surface
+ * flux"; reading R18).  kinds: HOST, [n_bc], one per boundary id of the mesh description:
+ *   MARUT_BC_PRESCRIBED  exterior state = bc_state[id] (default),
+ *   MARUT_BC_OUTFLOW     exterior state = interior state (F* = F(U-).n, no lift),
+ *   MARUT_BC_SLIP_WALL   exterior state = interior state with the normal momentum reflected, m+ = m- - 2 (m-.nhat) nhat.
+ * Rewrites the connectivity table on the device (synchronises); takes effect from the next call.  Kinds other than
+ * PRESCRIBED need a MARUT_EULER mesh (else EINVAL); n_bc must equal the description's. */
+enum { MARUT_BC_PRESCRIBED = 0, MARUT_BC_OUTFLOW = 1, MARUT_BC_SLIP_WALL = 2 };
+marut_status marut_set_boundary_kinds(marut_mesh *mesh, const int *kinds, int n_bc);
+
 /* Per-stage positivity floor ("a per-stage positivity floor enforces rho >= 1e-6 and
  * p >= 5e-7"; reading R17), in place on u (DEVICE, [n_elem][nvar][n^dim]): at every node
  *   rho <- max(rho, rho_min), momentum kept;  if (gamma-1)(E - |m|^2/(2 rho)) < p_min:  E <- p_min/(gamma-1) + |m|^2/(2 rho).

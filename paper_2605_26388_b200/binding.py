@@ -15,7 +15,7 @@ _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA"
 
 # every symbol include/marut.h declares
 SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt",
-           "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_set_blend", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
+           "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
            "marut_last_error"]
 
 
@@ -68,6 +68,8 @@ def lib():
         L.marut_chem_implicit.argtypes = [vp, vp, dbl, C.POINTER(C.c_int), vp]
         L.marut_shock_indicator.restype = C.c_int
         L.marut_shock_indicator.argtypes = [vp, vp, dbl, dbl, dbl, C.c_int, vp, vp]
+        L.marut_set_boundary_kinds.restype = C.c_int
+        L.marut_set_boundary_kinds.argtypes = [vp, vp, C.c_int]
         L.marut_positivity_floor.restype = C.c_int
         L.marut_positivity_floor.argtypes = [vp, vp, dbl, dbl, vp, vp]
         L.marut_set_blend.restype = C.c_int
@@ -183,6 +185,12 @@ def marut_shock_indicator(h, u, alpha, s=9.21024, alpha_min=0.001, alpha_max=0.5
     _check(lib().marut_shock_indicator(h, _dev(u), s, alpha_min, alpha_max, int(bool(smooth)), _dev(alpha), _stream(stream)))
 
 
+def marut_set_boundary_kinds(h, kinds):
+    """kinds: one of 0 (prescribed state) / 1 (outflow) / 2 (slip wall) per boundary id (host integers)"""
+    k = np.ascontiguousarray(kinds, dtype=np.int32)
+    _check(lib().marut_set_boundary_kinds(h, k.ctypes.data_as(C.c_void_p), int(k.size)))
+
+
 def marut_positivity_floor(h, u, rho_min=1e-6, p_min=5e-7, stream=None, want_count=False):
     """in place on u; returns the number of nodes changed if want_count (synchronises), else None"""
     n = C.c_long(0)
@@ -250,6 +258,9 @@ class MarutMesh:
 
     def positivity_floor(self, u, rho_min=1e-6, p_min=5e-7, stream=None, want_count=False):
         return marut_positivity_floor(self.h, u, rho_min, p_min, stream, want_count)
+
+    def set_boundary_kinds(self, kinds):
+        marut_set_boundary_kinds(self.h, kinds)
 
     def set_blend(self, alpha):
         self._alpha = alpha          # the library keeps the pointer: hold the tensor

@@ -36,6 +36,8 @@ static marut_status fail(marut_status st, const char *fmt, ...) {
 struct marut_mesh {
   int dim = 0, N = 0, np = 0, nn = 0, nvar = 0, nsp = 1, physics = 0;
   long ne = 0, n_mortar = 0;
+  int n_bc = 0;
+  bool bc_kinds = false;       // some boundary id is an outflow / slip-wall face
   double gamma = 1.4, mu = 0.0, Pr = 0.72, kappa = 0.0;
   bool affine = false;
   double dx_min = 0.0;
@@ -374,6 +376,7 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   CUDA_TRY(cudaMemcpy(m->d_mortar_fine, mfine.data(), mfine.size() * sizeof(int), cudaMemcpyHostToDevice));
   CUDA_TRY(cudaMalloc(&m->d_mortar_mat, mort.size() * sizeof(double)));
   CUDA_TRY(cudaMemcpy(m->d_mortar_mat, mort.data(), mort.size() * sizeof(double), cudaMemcpyHostToDevice));
+  m->n_bc = d->n_bc;
   const size_t nbc = (size_t)std::max(1, d->n_bc) * m->nvar;
   CUDA_TRY(cudaMalloc(&m->d_bc, nbc * sizeof(double)));
   if (d->n_bc) CUDA_TRY(cudaMemcpy(m->d_bc, d->bc_state, (size_t)d->n_bc * m->nvar * sizeof(double), cudaMemcpyHostToDevice));
@@ -493,7 +496,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.ca = ca; P.cb = cb; P.cc = cc;
   P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne;
   memcpy(P.D, m->D, sizeof(P.D));
-  P.alpha = nullptr; P.subn = m->d_subn;
+  P.alpha = nullptr; P.subn = m->d_subn; P.bc_kinds = m->bc_kinds ? 1 : 0;
   for (int i = 0; i < MAX_NP; ++i) P.inv_w[i] = (i < m->np) ? 1.0 / m->w[i] : 0.0;
   if (m->d_alpha) {
     if (m->physics != MARUT_EULER || m->volume_form != MARUT_VOLUME_SPLIT_RANOCHA)
@@ -641,6 +644,43 @@ extern "C" marut_status marut_chem_implicit(marut_mesh *m, double *u, double dt,
     *sweeps_out = (int)(m->h_red[3] & 0xffffffffu);
     if (*sweeps_out > 50) return fail(MARUT_ENOTFINITE, "implicit chemistry: Newton did not converge in 50 sweeps");
   }
+  return MARUT_OK;
+}
+
+// ------------------------------------------------------------------------------------ boundary kinds
+__global__ void patch_boundary_kinds_kernel(int2 *conn, long n, const int *kinds) {
+  for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
+    int2 cn = conn[i];
+    if ((cn.y & 3) == FK_BOUNDARY) {
+      cn.y = FK_BOUNDARY | (kinds[cn.x] << 2);
+      conn[i] = cn;
+    }
+  }
+}
+
+extern "C" marut_status marut_set_boundary_kinds(marut_mesh *m, const int *kinds, int n_bc) {
+  if (!m || !kinds) return fail(MARUT_EINVAL, "NULL argument");
+  if (n_bc != m->n_bc) return fail(MARUT_EINVAL, "n_bc = %d, the mesh has %d boundary ids", n_bc, m->n_bc);
+  bool special = false;
+  for (int i = 0; i < n_bc; ++i) {
+    if (kinds[i] < MARUT_BC_PRESCRIBED || kinds[i] > MARUT_BC_SLIP_WALL) return fail(MARUT_EINVAL, "unknown boundary kind %d", kinds[i]);
+    special = special || kinds[i] != MARUT_BC_PRESCRIBED;
+  }
+  if (special && (m->physics != MARUT_EULER || m->kernel_sel != 0))
+    return fail(MARUT_EINVAL, "outflow / slip-wall faces are implemented for MARUT_EULER (default kernels) only");
+  if (n_bc == 0) return MARUT_OK;
+  int *d_k = nullptr;
+  CUDA_TRY(cudaMalloc(&d_k, n_bc * sizeof(int)));
+  cudaError_t e = cudaMemcpy(d_k, kinds, n_bc * sizeof(int), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    const long n = m->ne * 2 * m->dim;
+    patch_boundary_kinds_kernel<<<(unsigned)std::min<long>((n + 255) / 256, 148L * 8), 256>>>(m->d_conn, n, d_k);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  }
+  cudaFree(d_k);
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "boundary kinds: %s", cudaGetErrorString(e));
+  m->bc_kinds = special;
   return MARUT_OK;
 }
 

@@ -168,9 +168,10 @@ __device__ __forceinline__ void gather_exterior(const StageParams &P, const Face
   }
 }
 
-// lift (F* - Ftilde.n)/w_b of one face node (Euler), written to the lift buffer.  Up = exterior state of a
+// lift (F* - Ftilde.n)/w_b of one face node (Euler), written to the lift buffer.  BCK: the instantiation that knows
+// outflow / slip-wall faces (selected by StageParams::bc_kinds; the default one carries no code for them).  Up = exterior state of a
 // conforming / boundary face (ignored for mortar faces).
-template <int DIM, int NP, bool AFFINE, int EB>
+template <int DIM, int NP, bool AFFINE, int EB, bool BCK = false>
 __device__ __forceinline__ void euler_face_task(const StageParams &P, const double *Ust, const double *Msm, double *Lft,
                                                 long e0, int g, const FaceTask &t, int2 cn, const double *Up) {
   using C = NodeCfg<DIM, NP, 1, EB>;
@@ -207,7 +208,25 @@ __device__ __forceinline__ void euler_face_task(const StageParams &P, const doub
   for (int c = 0; c < DIM; ++c) Fm[1 + c] = Um[1 + c] * vnm + pm * nv[c];
   Fm[DIM + 1] = (Um[DIM + 1] + pm) * vnm;
   const int kind = cn.y & 3;
-  if (kind == FK_CONFORMING || kind == FK_BOUNDARY) {
+  if (BCK && kind == FK_BOUNDARY && (cn.y & (3 << 2)) != 0) {
+    // outflow / slip-wall face (marut_set_boundary_kinds; R18), the Rusanov flux in closed form:
+    // outflow U+ = U-: F* = F(U-).nv, no lift.  Slip wall U+ = U- with m+ = m- - 2 (m-.nhat) nhat: same rho, E, p, a and
+    // v+.nv = -v-.nv, so the mass and energy components of F* vanish.
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) lift[v] = 0.0;
+    if (((cn.y >> 2) & 3) == BC_SLIP_WALL) {
+      const double hl = 0.5 * (fabs(vnm) + am * nrm);
+      const double r = 2.0 * mnm / (nrm * nrm);
+      lift[0] = -P.inv_wb * Fm[0];
+      lift[DIM + 1] = -P.inv_wb * Fm[DIM + 1];
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) {
+        const double dm = -r * nv[c];                                      // m+ - m-
+        const double Fp = (Um[1 + c] + dm) * (0.0 - vnm) + pm * nv[c];
+        lift[1 + c] = P.inv_wb * (0.5 * (Fp - Fm[1 + c]) - hl * dm);
+      }
+    }
+  } else if (kind == FK_CONFORMING || kind == FK_BOUNDARY) {
     // Rusanov with a scaled normal, division-free apart from 1/rho+ (R5):
     //   lambda |nv| = max(|v-.nv| + a- |nv|, |v+.nv| + a+ |nv|);  lift = (F* - F-.nv)/w_b
     const double irhop = 1.0 / Up[0];
@@ -299,7 +318,7 @@ __device__ __forceinline__ void last_pass_task(int t, int &el, int &v, int &ij) 
   }
 }
 
-template <int DIM, int NP, bool AFFINE, int EB, int MINB>
+template <int DIM, int NP, bool AFFINE, int EB, int MINB, bool BCK = false>
 __global__ void __launch_bounds__((NodeCfg<DIM, NP, 1, EB>::NT), MINB)
 stage_node_kernel(const __grid_constant__ StageParams P) {
   using C = NodeCfg<DIM, NP, 1, EB>;
@@ -437,7 +456,7 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
 
   // ---- face phase, first round: face nodes densely mapped
 #if MARUT_ABLATE != 1 && MARUT_ABLATE != 3
-  if (has0) euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
+  if (has0) euler_face_task<DIM, NP, AFFINE, EB, BCK>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
 #else
   if (has0 && Up0[0] == 1.2345) Lft[tid] = Up0[1];
 #endif
@@ -471,7 +490,7 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
     const int2 cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
     double Up[NVAR];
     gather_exterior<DIM, NP, NVAR>(P, t, cn, Up);
-    euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, g, t, cn, Up);
+    euler_face_task<DIM, NP, AFFINE, EB, BCK>(P, Ust, Msm, Lft, e0, g, t, cn, Up);
   }
   if constexpr (DIM == 3 || (NTASK > NT)) __syncthreads();
 
@@ -541,13 +560,16 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
 template <int NN>
 constexpr int node_eb() { return (NN >= 96) ? 1 : 128 / NN; }
 
-template <int DIM, int NP, bool AFFINE>
+template <int DIM, int NP, bool AFFINE, bool BCK = false>
 cudaError_t launch_stage_node_t(const StageParams &P, cudaStream_t st) {
+  if constexpr (!BCK) {
+    if (P.bc_kinds) return launch_stage_node_t<DIM, NP, AFFINE, true>(P, st);
+  }
   constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
   using C = NodeCfg<DIM, NP, 1, EB>;
   constexpr size_t smem = C::smem_doubles(AFFINE) * sizeof(double);
   constexpr int MINB = (C::NT <= 128) ? MARUT_NODE_MINB128 : ((C::NT <= 256) ? 3 : 1);
-  auto k = stage_node_kernel<DIM, NP, AFFINE, EB, MINB>;
+  auto k = stage_node_kernel<DIM, NP, AFFINE, EB, MINB, BCK>;
   static bool attr = false;
   if (!attr) {
     cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

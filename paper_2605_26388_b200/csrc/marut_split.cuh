@@ -279,13 +279,13 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
     for (int v = 0; v < NVAR; ++v) Un[v] = np_[v * NN];
   }
   // ---- phase S: face nodes, densely mapped
-  if (has0) euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
+  if (has0) euler_face_task<DIM, NP, AFFINE, EB, true>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
   for (int g = tid + NT; g < ntask; g += NT) {
     const FaceTask t = decode_task<DIM, NP>(g);
     const int2 cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
     double Up[NVAR];
     gather_exterior<DIM, NP, NVAR>(P, t, cn, Up);
-    euler_face_task<DIM, NP, AFFINE, EB>(P, Ust, Msm, Lft, e0, g, t, cn, Up);
+    euler_face_task<DIM, NP, AFFINE, EB, true>(P, Ust, Msm, Lft, e0, g, t, cn, Up);
   }
   __syncthreads();
   if (!active) return;
