@@ -84,6 +84,10 @@ def _setup(L):
         L.oracle_chem_implicit_node.argtypes = [vp, vp, C.c_double, C.c_double]
         L.oracle_set_volume_form.restype = C.c_int
         L.oracle_set_volume_form.argtypes = [vp, C.c_int]
+        L.oracle_ssprk54_table.argtypes = [vp, vp]
+        L.oracle_ssprk54_step.argtypes = [vp, vp, C.c_double]
+        L.oracle_ssprk54_scalar.restype = C.c_double
+        L.oracle_ssprk54_scalar.argtypes = [C.c_double] * 5
         L.oracle_set_boundary_kinds.restype = C.c_int
         L.oracle_set_boundary_kinds.argtypes = [vp, vp, C.c_int]
         L.oracle_positivity_floor.restype = C.c_long
@@ -240,6 +244,12 @@ class OracleMesh:
         self.L.oracle_shock_indicator(self.h, _p(u), s, alpha_min, alpha_max, _p(a), int(smooth))
         return a
 
+    def ssprk54_step(self, u, dt):
+        """O19: one SSP-RK54 step (eq. 45 with the Spiteri-Ruuth table); returns the new state"""
+        v = _f64(u).copy()
+        self.L.oracle_ssprk54_step(self.h, _p(v), float(dt))
+        return v
+
     def set_boundary_kinds(self, kinds):
         """O8b: per bc id 0 = prescribed exterior state, 1 = outflow (interior state), 2 = inviscid slip wall"""
         if kinds is None:
@@ -352,6 +362,16 @@ def mortar_matrices(N):
     M = [np.zeros((n, n)) for _ in range(4)]
     lib().oracle_mortar_matrices(N, *[_p(a) for a in M])
     return M  # Pf_lo, Pf_up, Pr_lo, Pr_up
+
+
+def ssprk54_table():
+    a, b = np.zeros((5, 5)), np.zeros((5, 5))
+    lib().oracle_ssprk54_table(_p(a), _p(b))
+    return a, b
+
+
+def ssprk54_scalar(y0, lam, c2, t0, dt):
+    return lib().oracle_ssprk54_scalar(y0, lam, c2, t0, dt)
 
 
 def rusanov(dim, gamma, Um, Up, nv):

@@ -1219,6 +1219,58 @@ void oracle_ssprk_stage(void *h, int stage, double dt, double t_n, const double 
   rhs_full(*m, u_in, L.data());
   for (size_t i = 0; i < len; ++i) u_out[i] = a[stage] * u_n[i] + b[stage] * (u_in[i] + dt * L[i]);
 }
+// O19. SSP-RK54 of Spiteri and Ruuth (five stages, fourth order, SSP coefficient ~1.508) in the
+// Shu-Osher form of eq. 45, U^(i) = sum_k alpha_ik U^(k) + dt beta_ik L(U^(k)).  The paper does not
+// print the coefficients; these are the published ones of the cited scheme (reading R19), pinned by the
+// fourth-order conditions, the row sums of eq. 45 and the SSP coefficient the paper states.
+static const double RK54_ALPHA[5][5] = {
+    {1.0, 0, 0, 0, 0},
+    {0.444370493651235, 0.555629506348765, 0, 0, 0},
+    {0.620101851488403, 0, 0.379898148511597, 0, 0},
+    {0.178079954393132, 0, 0, 0.821920045606868, 0},
+    {0, 0, 0.517231671970585, 0.096059710526147, 0.386708617503269}};
+static const double RK54_BETA[5][5] = {
+    {0.391752226571890, 0, 0, 0, 0},
+    {0, 0.368410593050371, 0, 0, 0},
+    {0, 0, 0.251891774271694, 0, 0},
+    {0, 0, 0, 0.544974750228521, 0},
+    {0, 0, 0, 0.063692468666290, 0.226007483236906}};
+void oracle_ssprk54_table(double *alpha, double *beta) {
+  for (int i = 0; i < 5; ++i)
+    for (int k = 0; k < 5; ++k) { alpha[i * 5 + k] = RK54_ALPHA[i][k]; beta[i * 5 + k] = RK54_BETA[i][k]; }
+}
+// one SSP-RK54 step of the semi-discrete system, u advanced in place (the operator is autonomous)
+void oracle_ssprk54_step(void *h, double *u, double dt) {
+  Mesh *m = (Mesh *)h;
+  const size_t len = (size_t)m->ne * m->nvar * m->nn;
+  std::vector<std::vector<double>> U(6, std::vector<double>(len)), L(5, std::vector<double>(len));
+  U[0].assign(u, u + len);
+  for (int i = 0; i < 5; ++i) {
+    rhs_full(*m, U[i].data(), L[i].data());
+    for (size_t q = 0; q < len; ++q) {
+      double acc = 0.0;
+      for (int k = 0; k <= i; ++k) acc += RK54_ALPHA[i][k] * U[k][q] + dt * RK54_BETA[i][k] * L[k][q];
+      U[i + 1][q] = acc;
+    }
+  }
+  std::copy(U[5].begin(), U[5].end(), u);
+}
+// the same table on the scalar ODE y' = lam*y + c2*t^2, stage times from the table (c_i = sum_k of the Butcher row)
+double oracle_ssprk54_scalar(double y0, double lam, double c2, double t0, double dt) {
+  double Y[6], Lv[5], c[6];
+  Y[0] = y0; c[0] = 0.0;
+  for (int i = 0; i < 5; ++i) {
+    const double t = t0 + c[i] * dt;
+    Lv[i] = lam * Y[i] + c2 * t * t;
+    double acc = 0.0, ci = 0.0;
+    for (int k = 0; k <= i; ++k) {
+      acc += RK54_ALPHA[i][k] * Y[k] + dt * RK54_BETA[i][k] * Lv[k];
+      ci += RK54_ALPHA[i][k] * c[k] + RK54_BETA[i][k];
+    }
+    Y[i + 1] = acc; c[i + 1] = ci;
+  }
+  return Y[5];
+}
 // generic SSPRK3 driver on a user ODE y' = lam*y + c2*t^2 (for the scalar pins of O10)
 double oracle_ssprk3_scalar(double y0, double lam, double c2, double t0, double dt) {
   auto L = [&](double y, double t) { return lam * y + c2 * t * t; };
