@@ -99,6 +99,21 @@ marut_status marut_rhs(marut_mesh *mesh, const double *u, double *du, double t, 
 marut_status marut_ssprk_stage(marut_mesh *mesh, int stage, double dt, double t_n, const double *u_n,
                                const double *u_in, double *u_out, void *cuda_stream);
 
+/* General stage of the Shu-Osher form, eq. 45, with two earlier stages, fused with the operator:
+ *   u_out = a*u_a + b*u_in + c_dt*L(u_in)
+ * (marut_ssprk_stage is this call with the SSP-RK33 table).  u_out must not alias u_in; it may alias u_a; u_a is not
+ * read when a == 0.  With marut_lincomb it composes SSP-RK54 (SURVEY 8(f) NEXT-2b; R19):
+ *   U1 = U0 + b10 dt L(U0); U2 = a20 U0 + a21 U1 + b21 dt L(U1); U3 = a30 U0 + a32 U2 + b32 dt L(U2);
+ *   U4 = a40 U0 + a43 U3 + b43 dt L(U3);
+ *   U5 = [a52 U2 + a53 U3 + a54 U4 + (b53/b43)(U4 - a40 U0 - a43 U3)] + b54 dt L(U4)   (bracket: marut_lincomb). */
+marut_status marut_rk_stage(marut_mesh *mesh, double a, double b, double c_dt, const double *u_a, const double *u_in,
+                            double *u_out, void *cuda_stream);
+
+/* out = sum_{k<n} coef[k]*u[k], 1 <= n <= 4.  coef: HOST [n]; u: HOST array of n DEVICE pointers, each
+ * [n_elem][n_var][n^dim]; out: DEVICE, may alias any u[k] (elementwise). */
+marut_status marut_lincomb(marut_mesh *mesh, int n, const double *coef, const double *const *u, double *out,
+                           void *cuda_stream);
+
 /* dt = min(dt_C, dt_D) (eq. 17-18; R11):
  *   dt_C = cfl*dx_min/((2N+1)*max_i(|u_i|_2 + a_i)),  dt_D = cfl*dx_min^2/((2N+1)^2*nu_max) (NAVIER_STOKES),
  *   dx_min = min_e 2*(min_i J_i)^(1/dim),  nu_max = max_i(mu/rho_i)*max(1, 1/Pr).

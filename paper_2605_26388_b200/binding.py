@@ -15,7 +15,7 @@ _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA"
 
 # every symbol include/marut.h declares
 SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt",
-           "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
+           "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_rk_stage", "marut_lincomb", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
            "marut_last_error"]
 
 
@@ -68,6 +68,10 @@ def lib():
         L.marut_chem_implicit.argtypes = [vp, vp, dbl, C.POINTER(C.c_int), vp]
         L.marut_shock_indicator.restype = C.c_int
         L.marut_shock_indicator.argtypes = [vp, vp, dbl, dbl, dbl, C.c_int, vp, vp]
+        L.marut_rk_stage.restype = C.c_int
+        L.marut_rk_stage.argtypes = [vp, dbl, dbl, dbl, vp, vp, vp, vp]
+        L.marut_lincomb.restype = C.c_int
+        L.marut_lincomb.argtypes = [vp, C.c_int, vp, vp, vp, vp]
         L.marut_set_boundary_kinds.restype = C.c_int
         L.marut_set_boundary_kinds.argtypes = [vp, vp, C.c_int]
         L.marut_positivity_floor.restype = C.c_int
@@ -181,6 +185,36 @@ def ssprk3_step(h, u, ua, ub, dt, t=0.0, stream=None):
     marut_ssprk_stage(h, 2, dt, t, u, ub, u, stream)
 
 
+def marut_rk_stage(h, a, b, c_dt, u_a, u_in, u_out, stream=None):
+    _check(lib().marut_rk_stage(h, a, b, c_dt, _dev(u_a), _dev(u_in), _dev(u_out), _stream(stream)))
+
+
+def marut_lincomb(h, coef, us, out, stream=None):
+    n = len(us)
+    cf = (C.c_double * n)(*[float(x) for x in coef])
+    ptrs = (C.c_void_p * n)(*[_dev(t).value for t in us])
+    _check(lib().marut_lincomb(h, n, cf, ptrs, _dev(out), _stream(stream)))
+
+
+# SSP-RK54 of Spiteri and Ruuth in the Shu-Osher form of eq. 45 (R19): (alpha_i0, alpha_i,i-1, beta_i,i-1)
+_RK54 = ((1.0, 0.0, 0.391752226571890), (0.444370493651235, 0.555629506348765, 0.368410593050371),
+         (0.620101851488403, 0.379898148511597, 0.251891774271694), (0.178079954393132, 0.821920045606868, 0.544974750228521))
+_RK54_LAST = (0.517231671970585, 0.096059710526147, 0.063692468666290, 0.386708617503269, 0.226007483236906)
+
+
+def ssprk54_step(h, u, ua, ub, uc, dt, stream=None):
+    """one SSP-RK54 step, u advanced in place; ua, ub, uc: scratch.  Call sequence only -- every stage runs in the
+    library (marut_rk_stage x 5, marut_lincomb x 1)."""
+    a, b = _RK54, _RK54_LAST
+    marut_rk_stage(h, 0.0, 1.0, a[0][2] * dt, None, u, ua, stream)                      # U1 -> ua
+    marut_rk_stage(h, a[1][0], a[1][1], a[1][2] * dt, u, ua, ub, stream)                # U2 -> ub
+    marut_rk_stage(h, a[2][0], a[2][1], a[2][2] * dt, u, ub, ua, stream)                # U3 -> ua
+    marut_rk_stage(h, a[3][0], a[3][1], a[3][2] * dt, u, ua, uc, stream)                # U4 -> uc
+    r = b[2] / a[3][2]                                                                   # dt L(U3) = (U4 - a40 U0 - a43 U3)/b43
+    marut_lincomb(h, (-r * a[3][0], b[0], b[1] - r * a[3][1], b[3] + r), (u, ub, ua, uc), ua, stream)
+    marut_rk_stage(h, 1.0, 0.0, b[4] * dt, ua, uc, u, stream)                           # U5 -> u
+
+
 def marut_shock_indicator(h, u, alpha, s=9.21024, alpha_min=0.001, alpha_max=0.5, smooth=True, stream=None):
     _check(lib().marut_shock_indicator(h, _dev(u), s, alpha_min, alpha_max, int(bool(smooth)), _dev(alpha), _stream(stream)))
 
@@ -261,6 +295,15 @@ class MarutMesh:
 
     def set_boundary_kinds(self, kinds):
         marut_set_boundary_kinds(self.h, kinds)
+
+    def rk_stage(self, a, b, c_dt, u_a, u_in, u_out, stream=None):
+        marut_rk_stage(self.h, a, b, c_dt, u_a, u_in, u_out, stream)
+
+    def lincomb(self, coef, us, out, stream=None):
+        marut_lincomb(self.h, coef, us, out, stream)
+
+    def ssprk54_step(self, u, ua, ub, uc, dt, stream=None):
+        ssprk54_step(self.h, u, ua, ub, uc, dt, stream)
 
     def set_blend(self, alpha):
         self._alpha = alpha          # the library keeps the pointer: hold the tensor

@@ -602,6 +602,50 @@ extern "C" marut_status marut_ssprk_stage(marut_mesh *m, int stage, double dt, d
   return run_operator(m, a[stage], b[stage], b[stage] * dt, u_n, u_in, u_out, (cudaStream_t)stream);
 }
 
+// ======================================================================================
+// out = sum_k c_k u_k, k < n <= 4 (the stage combinations of eq. 45 that involve more than two earlier stages: last
+// stage of SSP-RK54).  Elementwise, so out may alias any u_k.  HBM-bound: (n + 1) * 8 B per value.
+// ======================================================================================
+struct LincombParams {
+  const double *u[4];
+  double c[4];
+  double *out;
+  long len;
+  int n;
+};
+__global__ void __launch_bounds__(256) lincomb_kernel(const __grid_constant__ LincombParams P) {
+  for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < P.len; i += (long)gridDim.x * blockDim.x) {
+    double acc = P.c[0] * P.u[0][i];
+    for (int k = 1; k < P.n; ++k) acc += P.c[k] * P.u[k][i];
+    P.out[i] = acc;
+  }
+}
+
+// general stage of eq. 45 with two earlier stages: u_out = a u_a + b u_in + c_dt L(u_in)
+extern "C" marut_status marut_rk_stage(marut_mesh *m, double a, double b, double c_dt, const double *u_a, const double *u_in,
+                                       double *u_out, void *stream) {
+  if (!m || !u_in || !u_out) return fail(MARUT_EINVAL, "NULL argument");
+  if (a != 0.0 && !u_a) return fail(MARUT_EINVAL, "u_a is NULL");
+  if (u_out == u_in) return fail(MARUT_EINVAL, "u_out must not alias u_in");
+  if (misaligned(u_in) || misaligned(u_out) || (a != 0.0 && misaligned(u_a))) return fail(MARUT_EINVAL, "buffers must be 16-byte aligned");
+  return run_operator(m, a, b, c_dt, u_a, u_in, u_out, (cudaStream_t)stream);
+}
+
+extern "C" marut_status marut_lincomb(marut_mesh *m, int n, const double *coef, const double *const *u, double *out, void *stream) {
+  if (!m || !coef || !u || !out) return fail(MARUT_EINVAL, "NULL argument");
+  if (n < 1 || n > 4) return fail(MARUT_EINVAL, "marut_lincomb: 1 <= n <= 4");
+  LincombParams P;
+  for (int k = 0; k < 4; ++k) { P.u[k] = (k < n) ? u[k] : nullptr; P.c[k] = (k < n) ? coef[k] : 0.0; }
+  for (int k = 0; k < n; ++k) if (!u[k]) return fail(MARUT_EINVAL, "marut_lincomb: u[%d] is NULL", k);
+  P.out = out; P.len = m->ne * m->nvar * m->nn; P.n = n;
+  const unsigned grid = (unsigned)std::min<long>((P.len + 255) / 256, 148L * 32);
+  lincomb_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(P);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "lincomb kernel: %s", cudaGetErrorString(e));
+  m->launches++;
+  return MARUT_OK;
+}
+
 extern "C" marut_status marut_chem_source(marut_mesh *m, const double *u, double *s, void *stream) {
   if (!m || !u || !s) return fail(MARUT_EINVAL, "NULL argument");
   if (m->physics != MARUT_REACTING_EULER) return fail(MARUT_EINVAL, "marut_chem_source needs a REACTING_EULER mesh");
