@@ -323,10 +323,17 @@ static int face_node(const Mesh &m, int f, int a) {
   }
   return node_index(m, ijk);
 }
-// partner face-node index under `orient` (2-D: 1 = reversed; 3-D: only 0)
+// partner face-node index under `orient` ("face-indexing tables, which encode the relative orientation of
+// the two elements that share a face"; reading R20).  2-D: 1 = reversed.  3-D: a = a0 + n a1 -> b = b0 + n b1,
+//   (c0, c1) = (a1, a0) if orient & 4 else (a0, a1);  b0 = N - c0 if orient & 1 else c0;  b1 = N - c1 if orient & 2 else c1
 static int orient_map(const Mesh &m, int a, int orient) {
   if (orient == 0) return a;
-  return m.N - a;     // 2-D flipped
+  if (m.dim == 2) return m.N - a;
+  int c0 = a % m.n, c1 = a / m.n;
+  if (orient & 4) std::swap(c0, c1);
+  if (orient & 1) c0 = m.N - c0;
+  if (orient & 2) c1 = m.N - c1;
+  return c0 + m.n * c1;
 }
 
 // O2. Metric terms.

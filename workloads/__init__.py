@@ -190,6 +190,104 @@ def cartesian_mesh(dim, N, counts, lo, hi, order="morton", warp=None, periodic=T
     return m
 
 
+def _cube_rotations():
+    """the 24 proper rotations of the reference cube as (perm, sign): new axis d runs along old axis perm[d], reversed
+    where sign[d] < 0"""
+    import itertools
+    out = []
+    for perm in itertools.permutations(range(3)):
+        for sign in itertools.product((1, -1), repeat=3):
+            M = np.zeros((3, 3))
+            for d in range(3):
+                M[d, perm[d]] = sign[d]
+            if round(np.linalg.det(M)) == 1:
+                out.append((perm, sign))
+    return out
+
+
+def face_orientation(n, pairs):
+    """3-D orientation code of a conforming face from node pairs ((a0, a1) on the left, (b0, b1) on the right):
+    (c0, c1) = (a1, a0) if code & 4 else (a0, a1);  b0 = n-1-c0 if code & 1 else c0;  b1 = n-1-c1 if code & 2 else c1"""
+    for code in range(8):
+        ok = True
+        for (a0, a1), (b0, b1) in pairs:
+            c0, c1 = (a1, a0) if code & 4 else (a0, a1)
+            if code & 1:
+                c0 = n - 1 - c0
+            if code & 2:
+                c1 = n - 1 - c1
+            if (c0, c1) != (b0, b1):
+                ok = False
+                break
+        if ok:
+            return code
+    raise ValueError("face nodes do not match under any orientation")
+
+
+def rotate_elements(mesh: Mesh, seed=SEED, frac=0.6):
+    """3-D conforming mesh -> the same mesh with the local axes of a seeded subset of elements rotated (one of the 24
+    proper rotations each), as an unstructured hexahedral mesh presents them: face numbers and the relative orientation
+    of the two sides of an interface change, the geometry does not.  Returns (new mesh, node_map) with
+    node_map[e][new_node] = old_node, so that field_new[e, :, :] = field_old[e, :, node_map[e]]."""
+    assert mesh.dim == 3 and len(mesh.mortar) == 0
+    n, ne = mesh.n, mesh.n_elem
+    rots = _cube_rotations()
+    pick = uniform(seed, 77, np.arange(ne))
+    which = (uniform(seed, 78, np.arange(ne)) * 24).astype(int) % 24
+    rot = [rots[which[e]] if pick[e] < frac else ((0, 1, 2), (1, 1, 1)) for e in range(ne)]
+    idx = np.indices((n, n, n)).reshape(3, -1)[::-1]              # idx[c][node] = index along axis c, i fastest
+    node_map = np.empty((ne, n ** 3), dtype=np.int64)
+    new_of_old = np.empty((ne, n ** 3), dtype=np.int64)
+    for e in range(ne):
+        perm, sign = rot[e]
+        # new multi-index (i'_0, i'_1, i'_2) -> old multi-index: old[perm[d]] = i'_d or n-1-i'_d
+        old = [None] * 3
+        for d in range(3):
+            old[perm[d]] = idx[d] if sign[d] > 0 else n - 1 - idx[d]
+        node_map[e] = old[0] + n * (old[1] + n * old[2])
+        new_of_old[e, node_map[e]] = np.arange(n ** 3)
+    X = np.stack([mesh.node_xyz[e][:, node_map[e]] for e in range(ne)])
+
+    def face_of(node_new):
+        """(face id, a0, a1) candidates of a node given by its new multi-index"""
+        return [node_new % n, (node_new // n) % n, node_new // (n * n)]
+
+    def new_face(e, f_old):
+        l, side = f_old // 2, f_old % 2
+        perm, sign = rot[e]
+        d = perm.index(l)
+        return 2 * d + (side if sign[d] > 0 else 1 - side)
+
+    def face_local(e, f_new, node_new):
+        ijk = face_of(node_new)
+        rest = [c for c in range(3) if c != f_new // 2]
+        return int(ijk[rest[0]]), int(ijk[rest[1]])
+
+    def old_face_node(f, a0, a1):
+        l, side = f // 2, f % 2
+        ijk = [0, 0, 0]
+        rest = [c for c in range(3) if c != l]
+        ijk[l] = (n - 1) if side else 0
+        ijk[rest[0]], ijk[rest[1]] = a0, a1
+        return ijk[0] + n * (ijk[1] + n * ijk[2])
+
+    iface = np.empty_like(mesh.iface)
+    probes = [(0, 0), (n - 1, 0), (0, n - 1), (1 % n, 0)] if n > 2 else [(0, 0), (1, 0), (0, 1), (1, 1)]
+    for q, (eL, fL, eR, fR, orient) in enumerate(mesh.iface):
+        assert orient == 0
+        fLn, fRn = new_face(eL, fL), new_face(eR, fR)
+        pairs = []
+        for a0, a1 in probes:
+            pL = new_of_old[eL, old_face_node(fL, a0, a1)]
+            pR = new_of_old[eR, old_face_node(fR, a0, a1)]
+            pairs.append((face_local(eL, fLn, pL), face_local(eR, fRn, pR)))
+        iface[q] = (eL, fLn, eR, fRn, face_orientation(n, pairs))
+    m = Mesh(dim=3, N=mesh.N, node_xyz=np.ascontiguousarray(X), iface=np.ascontiguousarray(iface), physics=mesh.physics,
+             gamma=mesh.gamma, mu=mesh.mu, Pr=mesh.Pr, mech=mesh.mech, volume_form=mesh.volume_form)
+    m.info = dict(mesh.info, rotated=int(sum(r != ((0, 1, 2), (1, 1, 1)) for r in rot)))
+    return m, node_map
+
+
 def sine_warp(counts, lo, hi, amp_frac=0.05, k=8, seed=SEED):
     """config 3: x_c = X_c + amp*h * prod_d sin(k X_d + phi_{c,d}), seeded phases."""
     dim = len(counts)
