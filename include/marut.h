@@ -14,7 +14,9 @@
  *  - Faces: f = 2*l + side (l = reference direction, side 0: xi_l = -1, 1: xi_l = +1).
  *    Face nodes are indexed by the remaining directions in increasing order
  *    (a = a0 + n*a1).  orient = 0: face node a of L meets face node a of R;
- *    orient = 1 (2-D only): a meets N - a.  3-D meshes must have orient = 0.
+ *    2-D: orient = 1: a meets N - a.  3-D: orient in 0..7 ("relative orientation"; R20): node
+ *    (a0, a1) of L meets node (b0, b1) of R, (c0, c1) = (a1, a0) if orient & 4 else (a0, a1),
+ *    b0 = N - c0 if orient & 1 else c0,  b1 = N - c1 if orient & 2 else c1; any face of L may meet any face of R.
  *  - Descriptor arrays are HOST pointers, copied at create; the handle owns all
  *    device geometry, connectivity and scratch.
  *  - Every call returns a status; no exceptions, no abort, nothing on stdout.

@@ -37,6 +37,7 @@ struct marut_mesh {
   int dim = 0, N = 0, np = 0, nn = 0, nvar = 0, nsp = 1, physics = 0;
   long ne = 0, n_mortar = 0;
   int n_bc = 0;
+  bool oriented = false;       // some 3-D interface has a non-trivial orientation code (R20)
   bool bc_kinds = false;       // some boundary id is an outflow / slip-wall face
   double gamma = 1.4, mu = 0.0, Pr = 0.72, kappa = 0.0;
   bool affine = false;
@@ -333,12 +334,13 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   };
   for (long i = 0; i < d->n_iface; ++i) {
     const int *I = d->iface + i * 5;
-    if (I[4] < 0 || (dim == 3 && I[4] != 0) || (dim == 2 && I[4] > 1))
+    if (I[4] < 0 || (dim == 3 && I[4] > 7) || (dim == 2 && I[4] > 1))
       return fail(MARUT_ETOPOLOGY, "iface %ld: unsupported orient %d", i, I[4]);
+    if (dim == 3 && I[4] != 0) m->oriented = true;
     if (I[0] < 0 || I[0] >= ne || I[2] < 0 || I[2] >= ne || I[1] < 0 || I[1] >= nf2 || I[3] < 0 || I[3] >= nf2)
       return fail(MARUT_ETOPOLOGY, "iface %ld: index out of range", i);
     if (!claim(I[0], I[1], I[2], pack_info(FK_CONFORMING, I[3], I[4], 0)) ||
-        !claim(I[2], I[3], I[0], pack_info(FK_CONFORMING, I[1], I[4], 0)))
+        !claim(I[2], I[3], I[0], pack_info(FK_CONFORMING, I[1], inverse_orientation(dim, I[4]), 0)))
       return fail(MARUT_ETOPOLOGY, "iface %ld: face listed twice", i);
   }
   std::vector<int> mfine((size_t)std::max<long>(1, d->n_mortar) * 2, 0);
@@ -474,7 +476,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   if (m->physics == MARUT_NAVIER_STOKES) {
     GradParams G;
     G.u = u_in; G.S = m->d_S; G.metric = m->d_metric; G.conn = m->d_conn;
-    G.gamma = m->gamma; G.inv_wb = 1.0 / m->w[0]; G.mu = m->mu; G.kappa = m->kappa; G.ne = m->ne;
+    G.gamma = m->gamma; G.inv_wb = 1.0 / m->w[0]; G.mu = m->mu; G.kappa = m->kappa; G.ne = m->ne; G.oriented = m->oriented ? 1 : 0;
     memcpy(G.D, m->D, sizeof(G.D));
     cudaError_t e = launch_gradient(m->dim, m->np, m->affine, G, st);
     if (e != cudaSuccess) return fail(e == cudaErrorNotSupported ? MARUT_EINVAL : MARUT_ECUDA, "gradient kernel: %s", cudaGetErrorString(e));
@@ -508,7 +510,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
     case MARUT_EULER:
       e = cudaErrorNotSupported;
       if (m->volume_form == MARUT_VOLUME_SPLIT_RANOCHA) { e = launch_stage_split(m->dim, m->np, m->affine, P, st); break; }
-      if (m->kernel_sel == 3 && m->dim == 3 && m->affine && m->n_mortar == 0) e = launch_stage_line2_3d(m->np, P, st);
+      if (m->kernel_sel == 3 && m->dim == 3 && m->affine && m->n_mortar == 0 && !m->oriented) e = launch_stage_line2_3d(m->np, P, st);
       if (m->kernel_sel == 0 || (m->kernel_sel == 3 && e == cudaErrorNotSupported)) e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
       if (m->kernel_sel == 1) e = (m->dim == 2) ? launch_stage_line2d(m->np, m->affine, P, st) : launch_stage_line3d(m->np, m->affine, P, st);
       if (e == cudaErrorNotSupported)

@@ -169,8 +169,9 @@ stage_kernel(const __grid_constant__ StageParams P) {
       double Up[NVAR], Tp = 0.0;
       int pR = 0;
       if (kind == FK_CONFORMING) {
-        const int b0 = (DIM == 2 && orient) ? NP - 1 - a0 : a0;
-        pR = G::face_node(fR, b0, a1);
+        int b0, b1;
+    partner_index<DIM, NP>(orient, a0, a1, b0, b1);
+        pR = G::face_node(fR, b0, b1);
         const double *un = P.u_in + (long)cn.x * NVAR * NN + pR;
 #pragma unroll
         for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
@@ -283,9 +284,12 @@ struct GradParams {
   double gamma, inv_wb, mu, kappa;
   long ne;
   double D[MAX_NP * MAX_NP];
+  int oriented;                        // 3-D: some interface has a non-trivial orientation code
 };
 
-template <int DIM, int NP, bool AFFINE, int EB>
+// ORIENT3: the instantiation for 3-D meshes with non-trivial face orientation codes (R20); the default one
+// keeps the identity pairing folded at compile time (the decode costs 12 registers here: 64 -> 76, one CTA less per SM)
+template <int DIM, int NP, bool AFFINE, int EB, bool ORIENT3 = false>
 __global__ void __launch_bounds__(((EB * Geo<DIM, NP>::NN + 31) / 32) * 32)
 gradient_kernel(const __grid_constant__ GradParams P) {
   using G = Geo<DIM, NP>;
@@ -340,11 +344,12 @@ gradient_kernel(const __grid_constant__ GradParams P) {
     const int side = (q[l] == 0) ? 0 : 1, f = 2 * l + side;
     const double sgn = side ? 1.0 : -1.0;
     const int2 cn = __ldg(&P.conn[e * 2 * DIM + f]);
-    const int fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7;
+    const int fR = (cn.y >> 2) & 7, orient = (DIM == 2 || ORIENT3) ? ((cn.y >> 5) & 7) : 0;
     int a0, a1;
     G::face_coords(q, l, a0, a1);
-    const int b0 = (DIM == 2 && orient) ? NP - 1 - a0 : a0;
-    const int pR = G::face_node(fR, b0, a1);
+    int b0, b1;
+    partner_index<DIM, NP>(orient, a0, a1, b0, b1);
+    const int pR = G::face_node(fR, b0, b1);
     double Up[NVAR];
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(P.u + ((long)cn.x * NVAR + v) * NN + pR);
@@ -846,12 +851,15 @@ cudaError_t launch_stage_t(const StageParams &P, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-template <int DIM, int NP, bool AFFINE>
+template <int DIM, int NP, bool AFFINE, bool ORIENT3 = false>
 cudaError_t launch_gradient_t(const GradParams &P, cudaStream_t st) {
+  if constexpr (DIM == 3 && !ORIENT3) {
+    if (P.oriented) return launch_gradient_t<DIM, NP, AFFINE, true>(P, st);
+  }
   constexpr int NN = Geo<DIM, NP>::NN, EB = elems_per_block<NN>();
   constexpr int threads = ((EB * NN + 31) / 32) * 32;
   constexpr size_t smem = (size_t)((DIM + 2) * EB * NN + NP * NP) * sizeof(double);
-  auto k = gradient_kernel<DIM, NP, AFFINE, EB>;
+  auto k = gradient_kernel<DIM, NP, AFFINE, EB, ORIENT3>;
   static bool attr = false;
   if (!attr) {
     cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -167,8 +167,9 @@ __device__ __forceinline__ void face_flux(const StageParams &P, long e, int f, i
     double Up[NVAR];
     if (kind == FK_CONFORMING) {
       const int fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7;
-      const int b0 = (DIM == 2 && orient) ? NP - 1 - a0 : a0;
-      const double *un = P.u_in + (long)cn.x * NVAR * NN + G::face_node(fR, b0, a1);
+      int b0, b1;
+    partner_index<DIM, NP>(orient, a0, a1, b0, b1);
+      const double *un = P.u_in + (long)cn.x * NVAR * NN + G::face_node(fR, b0, b1);
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
     } else {

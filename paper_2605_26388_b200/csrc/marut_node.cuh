@@ -155,8 +155,9 @@ __device__ __forceinline__ void gather_exterior(const StageParams &P, const Face
   const int kind = cn.y & 3;
   if (kind == FK_CONFORMING) {
     const int fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7;
-    const int b0 = (DIM == 2 && orient) ? NP - 1 - t.a0 : t.a0;
-    const double *un = P.u_in + (long)cn.x * NVAR * NN + face_node_of<DIM, NP>(fR, b0, t.a1);
+    int b0, b1;
+    partner_index<DIM, NP>(orient, t.a0, t.a1, b0, b1);
+    const double *un = P.u_in + (long)cn.x * NVAR * NN + face_node_of<DIM, NP>(fR, b0, b1);
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
   } else if (kind == FK_BOUNDARY) {

@@ -90,8 +90,9 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   int pR0 = 0;
   if (has0) {
     const int fR = (cn0.y >> 2) & 7, orient = (cn0.y >> 5) & 7;
-    const int b0 = (DIM == 2 && orient) ? NP - 1 - t0.a0 : t0.a0;
-    pR0 = face_node_of<DIM, NP>(fR, b0, t0.a1);
+    int b0, b1;
+    partner_index<DIM, NP>(orient, t0.a0, t0.a1, b0, b1);
+    pR0 = face_node_of<DIM, NP>(fR, b0, b1);
     const double *un = P.u_in + (long)cn0.x * NVAR * NN + pR0;
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) Up0[v] = __ldg(un + v * NN);
@@ -172,8 +173,9 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       t = decode_task<DIM, NP>(g);
       cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
       const int fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7;
-      const int b0 = (DIM == 2 && orient) ? NP - 1 - t.a0 : t.a0;
-      pR = face_node_of<DIM, NP>(fR, b0, t.a1);
+      int b0, b1;
+      partner_index<DIM, NP>(orient, t.a0, t.a1, b0, b1);
+      pR = face_node_of<DIM, NP>(fR, b0, b1);
       const double *un = P.u_in + (long)cn.x * NVAR * NN + pR;
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
