@@ -185,7 +185,7 @@ marut_status marut_set_explicit_source(marut_mesh *mesh, int on);
  * MARUT_VOLUME_SPLIT_RANOCHA: the entropy-stable split form, eq. 10,
  *   R_i = -(2/J_i) sum_l sum_m D_{i_l m} F#(U_i, U_m; 1/2 (Ja^l_i + Ja^l_m)),
  * with the two-point flux of Ranocha (eq. 41) and logarithmic means (R13); the surface
- * terms are unchanged.  MARUT_EULER meshes with N <= 5 only (else EINVAL).  Takes effect from the next call. */
+ * terms are unchanged.  MARUT_EULER meshes with N <= 7 (2-D) / N <= 6 (3-D) only (else EINVAL).  Takes effect from the next call. */
 enum { MARUT_VOLUME_STRONG = 0, MARUT_VOLUME_SPLIT_RANOCHA = 1 };
 marut_status marut_set_volume_form(marut_mesh *mesh, int form);
 

@@ -580,7 +580,7 @@ extern "C" marut_status marut_set_volume_form(marut_mesh *m, int form) {
   if (form != MARUT_VOLUME_STRONG && form != MARUT_VOLUME_SPLIT_RANOCHA) return fail(MARUT_EINVAL, "unknown volume form %d", form);
   if (form == MARUT_VOLUME_SPLIT_RANOCHA && m->physics != MARUT_EULER)
     return fail(MARUT_EINVAL, "the split-form volume integral is implemented for MARUT_EULER only");
-  if (form == MARUT_VOLUME_SPLIT_RANOCHA && m->np > 6) return fail(MARUT_EINVAL, "split form: N <= 5");
+  if (form == MARUT_VOLUME_SPLIT_RANOCHA && m->np > (m->dim == 2 ? 8 : 7)) return fail(MARUT_EINVAL, "split form: N <= 7 in 2-D, N <= 6 in 3-D");
   m->volume_form = form;
   return MARUT_OK;
 }

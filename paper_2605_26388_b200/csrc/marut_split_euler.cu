@@ -1,4 +1,5 @@
-// split-form (entropy-stable) Euler stage kernel instantiations (marut_split.cuh): 2-D and 3-D, N = 1..5
+// split-form (entropy-stable) Euler stage kernel instantiations (marut_split.cuh): 2-D N = 1..7, 3-D N = 1..6
+// (3-D N = 7 would need 303 KB of shared memory for the pair buffer)
 #include "marut_split.cuh"
 #include "marut_launch.h"
 namespace marut {
@@ -13,6 +14,8 @@ cudaError_t launch_stage_split(int dim, int np, bool affine, const StageParams &
       case 4: return go<2, 4>(affine, P, st);
       case 5: return go<2, 5>(affine, P, st);
       case 6: return go<2, 6>(affine, P, st);
+      case 7: return go<2, 7>(affine, P, st);
+      case 8: return go<2, 8>(affine, P, st);
     }
   if (dim == 3) switch (np) {
       case 2: return go<3, 2>(affine, P, st);
@@ -20,6 +23,7 @@ cudaError_t launch_stage_split(int dim, int np, bool affine, const StageParams &
       case 4: return go<3, 4>(affine, P, st);
       case 5: return go<3, 5>(affine, P, st);
       case 6: return go<3, 6>(affine, P, st);
+      case 7: return go<3, 7>(affine, P, st);
     }
   return cudaErrorNotSupported;
 }

@@ -27,7 +27,7 @@ def _alpha(ne, seed=3):
 
 
 CASES = [(2, N, 5, curved) for N in (1, 2, 3, 4, 5) for curved in (False, True)] + \
-        [(3, N, 3, curved) for N in (1, 2, 3, 4, 5) for curved in (False, True)]
+        [(3, N, 3, curved) for N in (1, 2, 3, 4, 5) for curved in (False, True)] + [(3, 6, 2, True), (2, 7, 3, True)]
 
 
 @pytest.mark.parametrize("dim,N,cells,curved", CASES)

@@ -59,7 +59,8 @@ def test_rhs_and_stage(dim, N, cells, curved, phys):
     gm.close()
 
 
-SPLIT = [(2, 3, 6, False), (2, 4, 5, True), (3, 4, 3, False), (3, 3, 3, True), (3, 1, 3, False), (3, 5, 2, False)]
+SPLIT = [(2, 3, 6, False), (2, 4, 5, True), (3, 4, 3, False), (3, 3, 3, True), (3, 1, 3, False), (3, 5, 2, False),
+         (3, 6, 2, False), (3, 6, 2, True), (2, 6, 4, True), (2, 7, 3, False)]      # N = 6: the degree of the paper's TGV runs
 
 
 @pytest.mark.parametrize("dim,N,cells,curved", SPLIT)
