@@ -141,8 +141,10 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
         double nr, dr, nb, db;
         logmean_nd(U[0], rm, lnr, Lns[pm], nr, dr);
         logmean_nd(bi, Lns[2 * TILE + pm], lnb, Lns[TILE + pm], nb, db);
-        const double rho_ln = nr / dr;
-        const double eint = inv_gm1 * (db / nb);                      // 1 / ((gamma-1) {{T^-1}}^ln)
+        // one reciprocal for both means: rho_ln = nr/dr, 1/((gamma-1) {{T^-1}}^ln) = db/((gamma-1) nb)
+        const double inv = 1.0 / (dr * nb);
+        const double rho_ln = nr * (nb * inv);
+        const double eint = inv_gm1 * (db * (dr * inv));
         const double pavg = 0.5 * (pi_ + pmm);
         const double mf = rho_ln * vn;
         double F[NVAR];
