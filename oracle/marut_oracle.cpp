@@ -24,7 +24,9 @@
 //   node_xyz [e][c][node]     node = i + n*(j + n*k), n = N+1
 //   u, du    [e][v][node]     v = rho_1..rho_ns, rho*u_1..rho*u_d, E
 //   iface    [f][5] = eL,fL,eR,fR,orient      face f = 2*l + side
-//   mortar   [m][6] = eC,fC,eF_lo,eF_up,fF,orient   (2-D only)
+//   mortar   2-D: [m][6] = eC,fC,eF_lo,eF_up,fF,orient
+//            3-D: [m][8] = eC,fC,eF_00,eF_10,eF_01,eF_11,fF,orient (eF_{s0 s1}: half s0 of the first, s1 of the
+//            second face-local direction of the coarse face; orient must be 0)
 //   bface    [b][3] = e,f,bc_id ;  bc_state [bc][nvar]
 // ============================================================================
 #include <cmath>
@@ -693,8 +695,47 @@ static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
       flux_dot(m, Up, primitives(m, Up), nR, Fo);   lift(eR, pR, Fs, Fo);
     }
   }
-  // --- 2:1 mortars (O7), 2-D only
-  for (size_t q = 0; q < m.mortar.size() / 6; ++q) {
+  // --- 4:1 mortars in 3-D (O7b; "factor 2 in 2D / 4 in 3D"; reading R21): the tensor product of the
+  // 2-D construction.  The coarse trace is interpolated to each of the four sub-faces (Pf[s0] x Pf[s1]); the Riemann
+  // problem is solved at the fine side's face nodes with the fine side's normal; the fine side lifts F*; the coarse
+  // side receives the L2 projection (Pr[s0] x Pr[s1]) of the outward flux -F*, times the area ratio 4.
+  for (size_t q = 0; d == 3 && q < m.mortar.size() / 8; ++q) {
+    const int *M = &m.mortar[q * 8];
+    const long eC = M[0]; const int fC = M[1], fF = M[6];
+    std::vector<double> UC((size_t)nf * nvar), FC((size_t)nf * nvar, 0.0);
+    for (int j = 0; j < nf; ++j) gather(m, u, eC, face_node(m, fC, j), &UC[(size_t)j * nvar]);
+    for (int s = 0; s < 4; ++s) {
+      const int s0 = s % 2, s1 = s / 2;
+      const long eF = M[2 + s];
+      for (int a = 0; a < nf; ++a) {
+        const int a0 = a % n, a1 = a / n, pF = face_node(m, fF, a);
+        double UF[MAXV], Ui[MAXV], nF[3], Fs[MAXV], Fo[MAXV];
+        gather(m, u, eF, pF, UF);
+        for (int v = 0; v < nvar; ++v) {
+          double acc = 0.0;
+          for (int j1 = 0; j1 < n; ++j1)
+            for (int j0 = 0; j0 < n; ++j0) acc += m.Pf[s0][a0 * n + j0] * m.Pf[s1][a1 * n + j1] * UC[(size_t)(j0 + n * j1) * nvar + v];
+          Ui[v] = acc;
+        }
+        face_normal(m, eF, fF, pF, nF);
+        rusanov(m, UF, Ui, nF, Fs);
+        flux_dot(m, UF, primitives(m, UF), nF, Fo);  lift(eF, pF, Fs, Fo);
+        for (int i1 = 0; i1 < n; ++i1)
+          for (int i0 = 0; i0 < n; ++i0)
+            for (int v = 0; v < nvar; ++v)
+              FC[(size_t)(i0 + n * i1) * nvar + v] += m.Pr_[s0][i0 * n + a0] * m.Pr_[s1][i1 * n + a1] * (4.0 * (-Fs[v]));
+      }
+    }
+    for (int i = 0; i < nf; ++i) {
+      const int pC = face_node(m, fC, i);
+      double nC[3], Fo[MAXV];
+      face_normal(m, eC, fC, pC, nC);
+      flux_dot(m, &UC[(size_t)i * nvar], primitives(m, &UC[(size_t)i * nvar]), nC, Fo);
+      lift(eC, pC, &FC[(size_t)i * nvar], Fo);
+    }
+  }
+  // --- 2:1 mortars (O7), 2-D
+  for (size_t q = 0; d == 2 && q < m.mortar.size() / 6; ++q) {
     const int *M = &m.mortar[q * 6];
     const long eC = M[0]; const int fC = M[1], fF = M[4];
     std::vector<double> UC((size_t)n * nvar), FC((size_t)n * nvar, 0.0);
@@ -1037,9 +1078,10 @@ static void shock_indicator(const Mesh &m, const double *u, double s, double ami
     const long a = m.iface[f * 5], b = m.iface[f * 5 + 2];
     alpha[a] = std::max(alpha[a], raw[b]); alpha[b] = std::max(alpha[b], raw[a]);
   }
-  for (size_t f = 0; f < m.mortar.size() / 6; ++f) {
-    const long c = m.mortar[f * 6];
-    for (int k = 2; k <= 3; ++k) { const long b = m.mortar[f * 6 + k]; alpha[c] = std::max(alpha[c], raw[b]); alpha[b] = std::max(alpha[b], raw[c]); }
+  const int mstride = (m.dim == 2) ? 6 : 8, mlast = (m.dim == 2) ? 3 : 5;
+  for (size_t f = 0; f < m.mortar.size() / mstride; ++f) {
+    const long c = m.mortar[f * mstride];
+    for (int k = 2; k <= mlast; ++k) { const long b = m.mortar[f * mstride + k]; alpha[c] = std::max(alpha[c], raw[b]); alpha[b] = std::max(alpha[b], raw[c]); }
   }
 }
 static void rhs_full(const Mesh &m, const double *u, double *du) {
@@ -1131,7 +1173,7 @@ void *oracle_mesh_create(const oracle_mesh_desc *d) {
   make_mortar(m->ops, m->Pf, m->Pr_);
   m->xyz.assign(d->node_xyz, d->node_xyz + (size_t)m->ne * m->dim * m->nn);
   if (d->n_iface) m->iface.assign(d->iface, d->iface + d->n_iface * 5);
-  if (d->n_mortar) m->mortar.assign(d->mortar, d->mortar + d->n_mortar * 6);
+  if (d->n_mortar) m->mortar.assign(d->mortar, d->mortar + d->n_mortar * (m->dim == 2 ? 6 : 8));
   if (d->n_bface) m->bface.assign(d->bface, d->bface + d->n_bface * 3);
   if (d->n_bc) m->bc_state.assign(d->bc_state, d->bc_state + (size_t)d->n_bc * m->nvar);
   compute_metrics(*m);

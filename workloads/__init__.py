@@ -190,6 +190,73 @@ def cartesian_mesh(dim, N, counts, lo, hi, order="morton", warp=None, periodic=T
     return m
 
 
+def octree_box_mesh(N, K=4, lo=(0.0, 0.0, 0.0), hi=(1.0, 1.0, 1.0), refine=None) -> Mesh:
+    """3-D periodic box of K^3 cells, the cells selected by `refine(ix, iy, iz) -> bool` (default: ix < K/2) split once
+    into 2x2x2 children: conforming faces between cells of equal size, 4:1 mortar faces (rows of 8 ints:
+    eC, fC, eF_00, eF_10, eF_01, eF_11, fF, 0; eF_{s0 s1} = the fine element on half s0 / s1 of the coarse face's first /
+    second face-local direction) between a cell and a split neighbour.  Affine elements."""
+    if refine is None:
+        refine = lambda ix, iy, iz: ix < K // 2
+    n = N + 1
+    xi = lgl_points(N)
+    h = [(hi[c] - lo[c]) / K for c in range(3)]
+    ref = np.indices((n, n, n)).reshape(3, -1)[::-1]
+    frac = (xi[ref] + 1.0) / 2.0
+    split = {(ix, iy, iz): bool(refine(ix, iy, iz)) for ix in range(K) for iy in range(K) for iz in range(K)}
+    ids, X = {}, []
+
+    def add(key, origin, size):
+        ids[key] = len(X)
+        X.append(np.stack([origin[c] + frac[c] * size[c] for c in range(3)]))
+
+    for iz in range(K):
+        for iy in range(K):
+            for ix in range(K):
+                cell = (ix, iy, iz)
+                o = [lo[c] + cell[c] * h[c] for c in range(3)]
+                if not split[cell]:
+                    add((cell, None), o, h)
+                else:
+                    for cz in range(2):
+                        for cy in range(2):
+                            for cx in range(2):
+                                ch = (cx, cy, cz)
+                                add((cell, ch), [o[c] + 0.5 * h[c] * ch[c] for c in range(3)], [0.5 * hc for hc in h])
+    iface, mortar = [], []
+
+    def child(l, side, s0, s1):
+        rest = [c for c in range(3) if c != l]
+        ch = [0, 0, 0]
+        ch[l], ch[rest[0]], ch[rest[1]] = side, s0, s1
+        return tuple(ch)
+
+    for cell in split:
+        for l in range(3):
+            nb = list(cell)
+            nb[l] = (nb[l] + 1) % K
+            nb = tuple(nb)
+            if split[cell]:                                   # faces between the children of this cell
+                for s1 in range(2):
+                    for s0 in range(2):
+                        iface.append((ids[(cell, child(l, 0, s0, s1))], 2 * l + 1, ids[(cell, child(l, 1, s0, s1))], 2 * l, 0))
+            if not split[cell] and not split[nb]:
+                iface.append((ids[(cell, None)], 2 * l + 1, ids[(nb, None)], 2 * l, 0))
+            elif split[cell] and split[nb]:
+                for s1 in range(2):
+                    for s0 in range(2):
+                        iface.append((ids[(cell, child(l, 1, s0, s1))], 2 * l + 1, ids[(nb, child(l, 0, s0, s1))], 2 * l, 0))
+            elif not split[cell]:                             # coarse cell, split neighbour on its + side
+                fine = [ids[(nb, child(l, 0, s0, s1))] for s1 in range(2) for s0 in range(2)]
+                mortar.append((ids[(cell, None)], 2 * l + 1, *fine, 2 * l, 0))
+            else:                                             # split cell, coarse neighbour on its + side
+                fine = [ids[(cell, child(l, 1, s0, s1))] for s1 in range(2) for s0 in range(2)]
+                mortar.append((ids[(nb, None)], 2 * l, *fine, 2 * l + 1, 0))
+    m = Mesh(dim=3, N=N, node_xyz=np.ascontiguousarray(np.stack(X)), iface=np.ascontiguousarray(np.array(iface, dtype=np.int32)),
+             mortar=np.ascontiguousarray(np.array(mortar, dtype=np.int32).reshape(-1, 8)))
+    m.info = dict(K=K, lo=tuple(lo), hi=tuple(hi), n_split=int(sum(split.values())))
+    return m
+
+
 def _cube_rotations():
     """the 24 proper rotations of the reference cube as (perm, sign): new axis d runs along old axis perm[d], reversed
     where sign[d] < 0"""
