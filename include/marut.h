@@ -68,8 +68,12 @@ typedef struct {
   long n_iface;
   const int *iface;       /* [n_iface][5]  = eL,fL,eR,fR,orient : conforming interior faces */
   long n_mortar;
-  const int *mortar;      /* [n_mortar][6] = eC,fC,eF_lo,eF_up,fF,orient : 2-D 2:1 hanging faces;
-                             eF_lo covers the coarse face parameter [-1,0], eF_up covers [0,1]; orient must be 0 */
+  const int *mortar;      /* 2-D: [n_mortar][6] = eC,fC,eF_lo,eF_up,fF,orient : 2:1 hanging faces;
+                             eF_lo covers the coarse face parameter [-1,0], eF_up covers [0,1]; orient must be 0.
+                             3-D: [n_mortar][8] = eC,fC,eF_00,eF_10,eF_01,eF_11,fF,orient : 4:1 hanging faces (DESIGN.md
+                             R21); eF_{s0 s1} covers half s0 / s1 of the coarse face's first / second face-local direction
+                             (the remaining reference directions in increasing order); orient must be 0; EULER, affine
+                             meshes only (else EINVAL) */
   long n_bface;
   const int *bface;       /* [n_bface][3]  = e,f,bc_id : boundary faces with a prescribed exterior state */
   int n_bc;

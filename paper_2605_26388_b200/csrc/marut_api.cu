@@ -248,7 +248,6 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   if ((d->n_iface && !d->iface) || (d->n_mortar && !d->mortar) || (d->n_bface && !d->bface) || (d->n_bc && !d->bc_state))
     return fail(MARUT_EINVAL, "NULL connectivity array with non-zero count");
   if (d->physics < 0 || d->physics > 2) return fail(MARUT_EINVAL, "unknown physics %d", d->physics);
-  if (d->n_mortar && d->dim != 2) return fail(MARUT_EINVAL, "mortars are implemented for 2-D meshes only");
   if (d->physics != MARUT_EULER && (d->n_mortar || d->n_bface))
     return fail(MARUT_EINVAL, "NAVIER_STOKES / REACTING_EULER support conforming interior faces only");
   if (d->physics != MARUT_REACTING_EULER && !(d->gamma > 1.0)) return fail(MARUT_EINVAL, "gamma must be > 1");
@@ -343,17 +342,22 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
         !claim(I[2], I[3], I[0], pack_info(FK_CONFORMING, I[1], inverse_orientation(dim, I[4]), 0)))
       return fail(MARUT_ETOPOLOGY, "iface %ld: face listed twice", i);
   }
-  std::vector<int> mfine((size_t)std::max<long>(1, d->n_mortar) * 2, 0);
+  // mortar rows: 2-D [6] = eC,fC,eF_lo,eF_up,fF,orient; 3-D [8] = eC,fC,eF_00,eF_10,eF_01,eF_11,fF,orient (R21)
+  const int nfine = (dim == 2) ? 2 : 4, mstride = nfine + 4;
+  if (dim == 3 && d->n_mortar > 0 && m->physics != MARUT_EULER)
+    return fail(MARUT_EINVAL, "3-D mortar faces are implemented for MARUT_EULER only");
+  std::vector<int> mfine((size_t)std::max<long>(1, d->n_mortar) * nfine, 0);
   for (long i = 0; i < d->n_mortar; ++i) {
-    const int *M = d->mortar + i * 6;
-    if (M[5] != 0) return fail(MARUT_ETOPOLOGY, "mortar %ld: orient must be 0", i);
-    for (int k : {0, 2, 3}) if (M[k] < 0 || M[k] >= ne) return fail(MARUT_ETOPOLOGY, "mortar %ld: element out of range", i);
-    if (M[1] < 0 || M[1] >= nf2 || M[4] < 0 || M[4] >= nf2) return fail(MARUT_ETOPOLOGY, "mortar %ld: face out of range", i);
-    if (!claim(M[0], M[1], (int)i, pack_info(FK_MORTAR_COARSE, M[4], 0, 0)) ||
-        !claim(M[2], M[4], M[0], pack_info(FK_MORTAR_FINE, M[1], 0, 0)) ||
-        !claim(M[3], M[4], M[0], pack_info(FK_MORTAR_FINE, M[1], 0, 1)))
-      return fail(MARUT_ETOPOLOGY, "mortar %ld: face listed twice", i);
-    mfine[i * 2] = M[2]; mfine[i * 2 + 1] = M[3];
+    const int *M = d->mortar + i * mstride;
+    const int fC = M[1], fF = M[2 + nfine];
+    if (M[3 + nfine] != 0) return fail(MARUT_ETOPOLOGY, "mortar %ld: orient must be 0", i);
+    if (M[0] < 0 || M[0] >= ne) return fail(MARUT_ETOPOLOGY, "mortar %ld: element out of range", i);
+    for (int k = 0; k < nfine; ++k) if (M[2 + k] < 0 || M[2 + k] >= ne) return fail(MARUT_ETOPOLOGY, "mortar %ld: element out of range", i);
+    if (fC < 0 || fC >= nf2 || fF < 0 || fF >= nf2) return fail(MARUT_ETOPOLOGY, "mortar %ld: face out of range", i);
+    bool ok = claim(M[0], fC, (int)i, pack_info(FK_MORTAR_COARSE, fF, 0, 0));
+    for (int k = 0; k < nfine && ok; ++k) ok = claim(M[2 + k], fF, M[0], pack_info(FK_MORTAR_FINE, fC, 0, k));
+    if (!ok) return fail(MARUT_ETOPOLOGY, "mortar %ld: face listed twice", i);
+    for (int k = 0; k < nfine; ++k) mfine[i * nfine + k] = M[2 + k];
   }
   for (long i = 0; i < d->n_bface; ++i) {
     const int *B = d->bface + i * 3;
@@ -442,6 +446,8 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
 
   const char *sel = getenv("MARUT_KERNEL");   // A/B switch for profiling: node (default) | line | generic
   m->kernel_sel = (sel && !strcmp(sel, "line")) ? 1 : ((sel && !strcmp(sel, "generic")) ? 2 : ((sel && !strcmp(sel, "line2")) ? 3 : 0));
+  if (dim == 3 && d->n_mortar > 0 && (m->kernel_sel != 0 || !m->affine))
+    return fail(MARUT_EINVAL, "3-D mortar faces need an affine mesh and the default kernels (MARUT_KERNEL unset)");
   return MARUT_OK;
 }
 
@@ -498,7 +504,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.ca = ca; P.cb = cb; P.cc = cc;
   P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne;
   memcpy(P.D, m->D, sizeof(P.D));
-  P.alpha = nullptr; P.subn = m->d_subn; P.bc_kinds = m->bc_kinds ? 1 : 0;
+  P.alpha = nullptr; P.subn = m->d_subn; P.bc_kinds = (m->bc_kinds || (m->dim == 3 && m->n_mortar > 0)) ? 1 : 0;
   for (int i = 0; i < MAX_NP; ++i) P.inv_w[i] = (i < m->np) ? 1.0 / m->w[i] : 0.0;
   if (m->d_alpha) {
     if (m->physics != MARUT_EULER || m->volume_form != MARUT_VOLUME_SPLIT_RANOCHA)

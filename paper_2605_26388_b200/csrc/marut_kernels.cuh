@@ -610,7 +610,11 @@ __global__ void indicator_smooth_kernel(const double *__restrict__ raw, const in
     const int2 cn = __ldg(&conn[e * 2 * DIM + f]);
     const int kind = cn.y & 3;
     if (kind == FK_CONFORMING || kind == FK_MORTAR_FINE) a = fmax(a, raw[cn.x]);
-    else if (kind == FK_MORTAR_COARSE) a = fmax(a, fmax(raw[__ldg(&mortar_fine[cn.x * 2])], raw[__ldg(&mortar_fine[cn.x * 2 + 1])]));
+    else if (kind == FK_MORTAR_COARSE) {
+      constexpr int NFINE = (DIM == 2) ? 2 : 4;
+#pragma unroll
+      for (int k = 0; k < NFINE; ++k) a = fmax(a, raw[__ldg(&mortar_fine[cn.x * NFINE + k])]);
+    }
   }
   alpha[e] = a;
 }

@@ -124,6 +124,77 @@ __device__ __noinline__ void node_mortar_flux_2d(const StageParams &P, long e, i
 }
 
 
+// 3-D 4:1 mortar faces (R21): the tensor product of the 2-D construction.  sub = s0 + 2 s1 names
+// the half of the coarse face's first / second face-local direction; the fine elements of coarse mortar m are
+// mortar_fine[4 m + sub].  Affine meshes.  Rare path, kept out of line.
+template <int NP>
+__device__ __noinline__ void node_mortar_flux_3d(const StageParams &P, long e, int f, int a0, int a1, int2 cn, const double *U,
+                                                 const double *nv, double *Fs) {
+  using G = Geo<3, NP>;
+  constexpr int NVAR = 5, NN = NP * NP * NP, MD = 10;
+  const int kind = cn.y & 3, fR = (cn.y >> 2) & 7, sub = (cn.y >> 8) & 3;
+  const double *Pf = P.mortar_mat, *Prv = P.mortar_mat + 2 * NP * NP;
+  const Prim<3> pr = prim_ideal<3, true>(U, P.gamma);
+  if (kind == FK_MORTAR_FINE) {
+    const int s0 = sub & 1, s1 = sub >> 1;
+    double Up[NVAR] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    for (int j1 = 0; j1 < NP; ++j1) {
+      const double w1 = __ldg(&Pf[(s1 * NP + a1) * NP + j1]);
+      for (int j0 = 0; j0 < NP; ++j0) {
+        const double w = w1 * __ldg(&Pf[(s0 * NP + a0) * NP + j0]);
+        const double *uc = P.u_in + (long)cn.x * NVAR * NN + G::face_node(fR, j0, j1);
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Up[v] += w * __ldg(uc + v * NN);
+      }
+    }
+    const Prim<3> qp = prim_ideal<3, true>(Up, P.gamma);
+    double Fm[NVAR];
+    flux_dot<3, 1>(U, pr, nv, Fm);
+    rusanov<3, 1>(U, pr, Fm, Up, qp, nv, Fs);
+  } else {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Fs[v] = 0.0;
+    const int lF = fR >> 1;
+    const double sF = (fR & 1) ? 1.0 : -1.0;
+    for (int m = 0; m < 4; ++m) {
+      const int s0 = m & 1, s1 = m >> 1;
+      const long eF = __ldg(&P.mortar_fine[cn.x * 4 + m]);
+      double nF[3];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) nF[c] = sF * __ldg(&P.metric[eF * MD + lF * 3 + c]);
+      for (int b1 = 0; b1 < NP; ++b1) {
+        const double r1 = __ldg(&Prv[(s1 * NP + a1) * NP + b1]);
+        for (int b0 = 0; b0 < NP; ++b0) {
+          const int pF = G::face_node(fR, b0, b1);
+          double UF[NVAR], UC[NVAR], FmF[NVAR], Fm_[NVAR];
+#pragma unroll
+          for (int v = 0; v < NVAR; ++v) {
+            UF[v] = __ldg(P.u_in + (eF * NVAR + v) * NN + pF);
+            UC[v] = 0.0;
+          }
+          for (int j1 = 0; j1 < NP; ++j1) {
+            const double w1 = __ldg(&Pf[(s1 * NP + b1) * NP + j1]);
+            for (int j0 = 0; j0 < NP; ++j0) {
+              const double w = w1 * __ldg(&Pf[(s0 * NP + b0) * NP + j0]);
+              const double *uc = P.u_in + e * NVAR * NN + G::face_node(f, j0, j1);
+#pragma unroll
+              for (int v = 0; v < NVAR; ++v) UC[v] += w * __ldg(uc + v * NN);
+            }
+          }
+          const Prim<3> qF = prim_ideal<3, true>(UF, P.gamma);
+          const Prim<3> qC = prim_ideal<3, true>(UC, P.gamma);
+          flux_dot<3, 1>(UF, qF, nF, FmF);
+          rusanov<3, 1>(UF, qF, FmF, UC, qC, nF, Fm_);
+          const double w2 = -4.0 * r1 * __ldg(&Prv[(s0 * NP + a0) * NP + b0]);
+#pragma unroll
+          for (int v = 0; v < NVAR; ++v) Fs[v] += w2 * Fm_[v];
+        }
+      }
+    }
+  }
+}
+
+
 // decoded face task (no dynamically indexed local arrays: they would go to local memory)
 struct FaceTask {
   int el, f, a0, a1, p;   // element in tile, face, face-node coordinates, volume node
@@ -170,7 +241,8 @@ __device__ __forceinline__ void gather_exterior(const StageParams &P, const Face
 }
 
 // lift (F* - Ftilde.n)/w_b of one face node (Euler), written to the lift buffer.  BCK: the instantiation that knows
-// outflow / slip-wall faces (selected by StageParams::bc_kinds; the default one carries no code for them).  Up = exterior state of a
+// outflow / slip-wall faces and 3-D mortar faces (selected by StageParams::bc_kinds; the default one carries no code
+// for them: the out-of-line 3-D mortar call alone costs the default 3-D kernel 30 %).  Up = exterior state of a
 // conforming / boundary face (ignored for mortar faces).
 template <int DIM, int NP, bool AFFINE, int EB, bool BCK = false>
 __device__ __forceinline__ void euler_face_task(const StageParams &P, const double *Ust, const double *Msm, double *Lft,
@@ -254,9 +326,14 @@ __device__ __forceinline__ void euler_face_task(const StageParams &P, const doub
       node_mortar_flux_2d<NP>(P, e, t.f, t.a0, cn, Um, nv, Fs);
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) lift[v] = P.inv_wb * (Fs[v] - Fm[v]);
+    } else if constexpr (BCK) {
+      double Fs[NVAR];
+      node_mortar_flux_3d<NP>(P, e, t.f, t.a0, t.a1, cn, Um, nv, Fs);
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) lift[v] = P.inv_wb * (Fs[v] - Fm[v]);
     } else {
 #pragma unroll
-      for (int v = 0; v < NVAR; ++v) lift[v] = 0.0;
+      for (int v = 0; v < NVAR; ++v) lift[v] = 0.0;     // 3-D mortar faces run in the BCK instantiation only
     }
   }
 #pragma unroll

@@ -32,7 +32,7 @@ __device__ __forceinline__ void logmean_nd(double aL, double aR, double lnL, dou
   }
 }
 
-template <int DIM, int NP, bool AFFINE, int EB, int MINB>
+template <int DIM, int NP, bool AFFINE, int EB, int MINB, bool BCK = false>
 __global__ void __launch_bounds__((NodeCfg<DIM, NP, 1, EB>::NT), MINB)
 stage_split_kernel(const __grid_constant__ StageParams P) {
   using C = NodeCfg<DIM, NP, 1, EB>;
@@ -281,13 +281,13 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
     for (int v = 0; v < NVAR; ++v) Un[v] = np_[v * NN];
   }
   // ---- phase S: face nodes, densely mapped
-  if (has0) euler_face_task<DIM, NP, AFFINE, EB, true>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
+  if (has0) euler_face_task<DIM, NP, AFFINE, EB, BCK>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
   for (int g = tid + NT; g < ntask; g += NT) {
     const FaceTask t = decode_task<DIM, NP>(g);
     const int2 cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
     double Up[NVAR];
     gather_exterior<DIM, NP, NVAR>(P, t, cn, Up);
-    euler_face_task<DIM, NP, AFFINE, EB, true>(P, Ust, Msm, Lft, e0, g, t, cn, Up);
+    euler_face_task<DIM, NP, AFFINE, EB, BCK>(P, Ust, Msm, Lft, e0, g, t, cn, Up);
   }
   __syncthreads();
   if (!active) return;
@@ -322,13 +322,16 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
   }
 }
 
-template <int DIM, int NP, bool AFFINE>
+template <int DIM, int NP, bool AFFINE, bool BCK = false>
 cudaError_t launch_stage_split_t(const StageParams &P, cudaStream_t st) {
+  if constexpr (!BCK) {
+    if (P.bc_kinds) return launch_stage_split_t<DIM, NP, AFFINE, true>(P, st);
+  }
   constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
   using C = NodeCfg<DIM, NP, 1, EB>;
   constexpr size_t smem = ((size_t)(C::NST + 3 + DIM + DIM * (NP / 2) * C::NVAR) * C::TILE + (size_t)C::NVAR * C::LFS + (AFFINE ? EB * C::MDP : 0)) * sizeof(double);
   constexpr int MINB = (C::NT <= 128) ? 4 : ((C::NT <= 256) ? 2 : 1);
-  auto k = stage_split_kernel<DIM, NP, AFFINE, EB, MINB>;
+  auto k = stage_split_kernel<DIM, NP, AFFINE, EB, MINB, BCK>;
   static bool attr = false;
   if (!attr) {
     cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
