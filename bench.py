@@ -17,6 +17,7 @@ same workload.  Rank 0 only.
 from __future__ import annotations
 
 import argparse
+import math
 import json
 import os
 import sys
@@ -29,7 +30,7 @@ if ROOT not in sys.path:
 METRIC = "DG RHS+SSPRK3 DOF-stage updates/s (FP64)"
 UNIT = "DOF-stage/s"
 # bounded oracle samples: (cells per direction, target seconds)
-ORACLE_SAMPLE_CELLS = {"c1": None, "c2": 12, "c2s": 12, "c3": 16, "c4": 64, "c4w": 64, "c4b": 64, "c5": 8}
+ORACLE_SAMPLE_CELLS = {"c1": None, "c2": 12, "c2s": 12, "c3": 16, "c4": 64, "c4w": 64, "c4b": 64, "c5": 8, "c2m": 8}
 # c4b: per-stage Hennemann-Gassner indicator (binding defaults, R15) feeding the DG/FV blend
 SHOCK_CAPTURE = dict(s=9.21024, alpha_min=1e-3, alpha_max=0.5, smooth=True)
 
@@ -37,9 +38,15 @@ SHOCK_CAPTURE = dict(s=9.21024, alpha_min=1e-3, alpha_max=0.5, smooth=True)
 def make_workload(name, cells=None):
     """c1..c5, c4w: the configs of BASELINE.json (workloads.make_case); c2s: c2 with the entropy-stable split-form
     volume integral; c4b: c4w as a shock-capturing run -- split form, and in
-    every Runge-Kutta stage the shock indicator of the stage's input state, the blended DG/FV stage and the positivity floor"""
+    every Runge-Kutta stage the shock indicator of the stage's input state, the blended DG/FV stage and the positivity floor;
+    c2m: the Taylor-Green flow of c2 on a box with one half refined once (3-D 4:1 mortar faces, NEXT-4)"""
     import workloads as wl
 
+    if name == "c2m":
+        # c2's flow on a box whose x < pi half is split once: 3-D 4:1 mortar faces (SURVEY 8(f) NEXT-4; DESIGN.md R21)
+        K = cells or 24
+        m = wl.octree_box_mesh(4, K=K, lo=(0.0,) * 3, hi=(2 * math.pi,) * 3)
+        return wl.Case("c2m", m, wl.taylor_green(m, noise=1e-3), 20, cfl=0.4)
     if name == "c4b":
         c = wl.make_case("c4w", cells=cells)
         c.mesh.volume_form = 1

@@ -51,6 +51,8 @@ struct marut_mesh {
   int kernel_sel = 0;          // Euler stage kernel: 0 node (marut_node.cuh), 1 line (marut_line.cuh), 2 generic; env MARUT_KERNEL
   int2 *d_conn = nullptr;
   int *d_mortar_fine = nullptr;
+  int *d_mortar_info = nullptr;   // 3-D: [m][3] = eC, fC, fF
+  double *d_mflux = nullptr;      // 3-D: F* at the fine face nodes of every mortar, [m][4][n*n][nvar]
   double *d_mortar_mat = nullptr;
   double *d_bc = nullptr;
   double *d_S = nullptr;     // NS scratch: stress tensor + heat flux from the BR1 gradient, [e][d(d+1)/2 + d][node]
@@ -233,7 +235,7 @@ static cudaError_t run_compact(int np, const double *d_full, double *d_el, long 
 extern "C" void marut_mesh_destroy(marut_mesh *m) {
   if (!m) return;
   cudaDeviceSynchronize();
-  cudaFree(m->d_metric); cudaFree(m->d_fnorm); cudaFree(m->d_conn); cudaFree(m->d_mortar_fine); cudaFree(m->d_mortar_mat);
+  cudaFree(m->d_metric); cudaFree(m->d_fnorm); cudaFree(m->d_conn); cudaFree(m->d_mortar_fine); cudaFree(m->d_mortar_info); cudaFree(m->d_mflux); cudaFree(m->d_mortar_mat);
   cudaFree(m->d_Vinv); cudaFree(m->d_araw); cudaFree(m->d_subn); cudaFree(m->d_bc); cudaFree(m->d_S); cudaFree(m->d_T); cudaFree(m->d_mech); cudaFree(m->d_red);
   if (m->h_red) cudaFreeHost(m->h_red);
   delete m;
@@ -346,7 +348,7 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   const int nfine = (dim == 2) ? 2 : 4, mstride = nfine + 4;
   if (dim == 3 && d->n_mortar > 0 && m->physics != MARUT_EULER)
     return fail(MARUT_EINVAL, "3-D mortar faces are implemented for MARUT_EULER only");
-  std::vector<int> mfine((size_t)std::max<long>(1, d->n_mortar) * nfine, 0);
+  std::vector<int> mfine((size_t)std::max<long>(1, d->n_mortar) * nfine, 0), minfo((size_t)std::max<long>(1, d->n_mortar) * 3, 0);
   for (long i = 0; i < d->n_mortar; ++i) {
     const int *M = d->mortar + i * mstride;
     const int fC = M[1], fF = M[2 + nfine];
@@ -358,6 +360,7 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
     for (int k = 0; k < nfine && ok; ++k) ok = claim(M[2 + k], fF, M[0], pack_info(FK_MORTAR_FINE, fC, 0, k));
     if (!ok) return fail(MARUT_ETOPOLOGY, "mortar %ld: face listed twice", i);
     for (int k = 0; k < nfine; ++k) mfine[i * nfine + k] = M[2 + k];
+    minfo[i * 3] = M[0]; minfo[i * 3 + 1] = fC; minfo[i * 3 + 2] = fF;
   }
   for (long i = 0; i < d->n_bface; ++i) {
     const int *B = d->bface + i * 3;
@@ -380,6 +383,11 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   CUDA_TRY(cudaMemcpy(m->d_conn, conn.data(), conn.size() * sizeof(int2), cudaMemcpyHostToDevice));
   CUDA_TRY(cudaMalloc(&m->d_mortar_fine, mfine.size() * sizeof(int)));
   CUDA_TRY(cudaMemcpy(m->d_mortar_fine, mfine.data(), mfine.size() * sizeof(int), cudaMemcpyHostToDevice));
+  if (dim == 3 && d->n_mortar > 0) {
+    CUDA_TRY(cudaMalloc(&m->d_mortar_info, minfo.size() * sizeof(int)));
+    CUDA_TRY(cudaMemcpy(m->d_mortar_info, minfo.data(), minfo.size() * sizeof(int), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMalloc(&m->d_mflux, (size_t)d->n_mortar * 4 * np * np * m->nvar * sizeof(double)));
+  }
   CUDA_TRY(cudaMalloc(&m->d_mortar_mat, mort.size() * sizeof(double)));
   CUDA_TRY(cudaMemcpy(m->d_mortar_mat, mort.data(), mort.size() * sizeof(double), cudaMemcpyHostToDevice));
   m->n_bc = d->n_bc;
@@ -504,6 +512,13 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.ca = ca; P.cb = cb; P.cc = cc;
   P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne;
   memcpy(P.D, m->D, sizeof(P.D));
+  P.mflux = m->d_mflux;
+  if (m->dim == 3 && m->n_mortar > 0) {
+    cudaError_t em = launch_mortar_flux3d(m->np, u_in, m->d_metric, m->d_mortar_info, m->d_mortar_fine, m->d_mortar_mat, m->gamma,
+                                          m->d_mflux, m->n_mortar, st);
+    if (em != cudaSuccess) return fail(MARUT_ECUDA, "mortar flux kernel: %s", cudaGetErrorString(em));
+    m->launches++;
+  }
   P.alpha = nullptr; P.subn = m->d_subn; P.bc_kinds = (m->bc_kinds || (m->dim == 3 && m->n_mortar > 0)) ? 1 : 0;
   for (int i = 0; i < MAX_NP; ++i) P.inv_w[i] = (i < m->np) ? 1.0 / m->w[i] : 0.0;
   if (m->d_alpha) {

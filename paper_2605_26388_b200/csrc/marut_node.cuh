@@ -152,48 +152,79 @@ __device__ __noinline__ void node_mortar_flux_3d(const StageParams &P, long e, i
     flux_dot<3, 1>(U, pr, nv, Fm);
     rusanov<3, 1>(U, pr, Fm, Up, qp, nv, Fs);
   } else {
+    // coarse side: the fluxes F*(U_F, U_i; n_F) at the 4 n^2 fine face nodes of this mortar were evaluated once by
+    // mortar_flux3d_kernel (every coarse face node needs all of them); here only their L2 projection, times -4
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) Fs[v] = 0.0;
-    const int lF = fR >> 1;
-    const double sF = (fR & 1) ? 1.0 : -1.0;
     for (int m = 0; m < 4; ++m) {
       const int s0 = m & 1, s1 = m >> 1;
-      const long eF = __ldg(&P.mortar_fine[cn.x * 4 + m]);
-      double nF[3];
-#pragma unroll
-      for (int c = 0; c < 3; ++c) nF[c] = sF * __ldg(&P.metric[eF * MD + lF * 3 + c]);
+      const double *Fm_ = P.mflux + ((long)cn.x * 4 + m) * NP * NP * NVAR;
       for (int b1 = 0; b1 < NP; ++b1) {
-        const double r1 = __ldg(&Prv[(s1 * NP + a1) * NP + b1]);
+        const double r1 = -4.0 * __ldg(&Prv[(s1 * NP + a1) * NP + b1]);
         for (int b0 = 0; b0 < NP; ++b0) {
-          const int pF = G::face_node(fR, b0, b1);
-          double UF[NVAR], UC[NVAR], FmF[NVAR], Fm_[NVAR];
+          const double w2 = r1 * __ldg(&Prv[(s0 * NP + a0) * NP + b0]);
+          const double *F = Fm_ + (b0 + NP * b1) * NVAR;
 #pragma unroll
-          for (int v = 0; v < NVAR; ++v) {
-            UF[v] = __ldg(P.u_in + (eF * NVAR + v) * NN + pF);
-            UC[v] = 0.0;
-          }
-          for (int j1 = 0; j1 < NP; ++j1) {
-            const double w1 = __ldg(&Pf[(s1 * NP + b1) * NP + j1]);
-            for (int j0 = 0; j0 < NP; ++j0) {
-              const double w = w1 * __ldg(&Pf[(s0 * NP + b0) * NP + j0]);
-              const double *uc = P.u_in + e * NVAR * NN + G::face_node(f, j0, j1);
-#pragma unroll
-              for (int v = 0; v < NVAR; ++v) UC[v] += w * __ldg(uc + v * NN);
-            }
-          }
-          const Prim<3> qF = prim_ideal<3, true>(UF, P.gamma);
-          const Prim<3> qC = prim_ideal<3, true>(UC, P.gamma);
-          flux_dot<3, 1>(UF, qF, nF, FmF);
-          rusanov<3, 1>(UF, qF, FmF, UC, qC, nF, Fm_);
-          const double w2 = -4.0 * r1 * __ldg(&Prv[(s0 * NP + a0) * NP + b0]);
-#pragma unroll
-          for (int v = 0; v < NVAR; ++v) Fs[v] += w2 * Fm_[v];
+          for (int v = 0; v < NVAR; ++v) Fs[v] += w2 * __ldg(F + v);
         }
       }
     }
   }
 }
 
+// F* at the fine face nodes of every 3-D mortar (R21): one CTA per mortar, one thread per (sub-face, fine face
+// node).  The coarse trace is staged in shared memory, interpolated to the thread's node (Pf[s0] x Pf[s1]), and the
+// Rusanov flux is evaluated with the fine element's own normal.  info[m] = (eC, fC, fF).  Affine meshes.
+template <int NP>
+__global__ void __launch_bounds__(4 * NP * NP) mortar_flux3d_kernel(const double *__restrict__ u, const double *__restrict__ metric,
+                                                                    const int *__restrict__ info, const int *__restrict__ mortar_fine,
+                                                                    const double *__restrict__ mortar_mat, double gamma,
+                                                                    double *__restrict__ mflux) {
+  using G = Geo<3, NP>;
+  constexpr int NVAR = 5, NN = NP * NP * NP, NF = NP * NP, MD = 10;
+  __shared__ double UC[NF * NVAR], Pfs[2 * NP * NP];
+  const long m = blockIdx.x;
+  const int tid = threadIdx.x;
+  const int eC = info[m * 3], fC = info[m * 3 + 1], fF = info[m * 3 + 2];
+  for (int i = tid; i < NF * NVAR; i += 4 * NF) {
+    const int j = i / NVAR, v = i - j * NVAR;
+    UC[i] = __ldg(u + ((long)eC * NVAR + v) * NN + G::face_node(fC, j % NP, j / NP));
+  }
+  for (int i = tid; i < 2 * NP * NP; i += 4 * NF) Pfs[i] = __ldg(&mortar_mat[i]);
+  __syncthreads();
+  const int s = tid / NF, b = tid - s * NF, b0 = b % NP, b1 = b / NP, s0 = s & 1, s1 = s >> 1;
+  const long eF = mortar_fine[m * 4 + s];
+  const int pF = G::face_node(fF, b0, b1), lF = fF >> 1;
+  const double sF = (fF & 1) ? 1.0 : -1.0;
+  double UF[NVAR], Ui[NVAR], nF[3], FmF[NVAR], Fs[NVAR];
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) {
+    UF[v] = __ldg(u + (eF * NVAR + v) * NN + pF);
+    Ui[v] = 0.0;
+  }
+  for (int j1 = 0; j1 < NP; ++j1) {
+    const double w1 = Pfs[(s1 * NP + b1) * NP + j1];
+    for (int j0 = 0; j0 < NP; ++j0) {
+      const double w = w1 * Pfs[(s0 * NP + b0) * NP + j0];
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Ui[v] += w * UC[(j0 + NP * j1) * NVAR + v];
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) nF[c] = sF * __ldg(&metric[eF * MD + lF * 3 + c]);
+  const Prim<3> qF = prim_ideal<3, true>(UF, gamma);
+  const Prim<3> qC = prim_ideal<3, true>(Ui, gamma);
+  flux_dot<3, 1>(UF, qF, nF, FmF);
+  rusanov<3, 1>(UF, qF, FmF, Ui, qC, nF, Fs);
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) mflux[((m * 4 + s) * NF + b) * NVAR + v] = Fs[v];
+}
+template <int NP>
+cudaError_t launch_mortar_flux3d_t(const double *u, const double *metric, const int *info, const int *fine, const double *mat,
+                                   double gamma, double *mflux, long n_mortar, cudaStream_t st) {
+  mortar_flux3d_kernel<NP><<<(unsigned)n_mortar, 4 * NP * NP, 0, st>>>(u, metric, info, fine, mat, gamma, mflux);
+  return cudaGetLastError();
+}
 
 // decoded face task (no dynamically indexed local arrays: they would go to local memory)
 struct FaceTask {
