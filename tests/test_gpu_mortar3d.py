@@ -65,3 +65,39 @@ def test_mortar3d_is_rejected_where_it_is_not_built():
     m.physics, m.mu = wl.NAVIER_STOKES, 0.01
     with pytest.raises(mb.MarutError):
         mb.MarutMesh(m)
+
+
+def test_mortar3d_full_size_c2m():
+    """the instance bench.py times as workload c2m (62,208 elements, 1,152 mortars), every element of one RHS and one
+    stage against the oracle"""
+    import math
+
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    m = wl.octree_box_mesh(4, K=24, lo=(0.0,) * 3, hi=(2 * math.pi,) * 3)
+    u0 = wl.taylor_green(m, noise=1e-3)
+    om, gm = oracle.OracleMesh(m), mb.MarutMesh(m)
+    u = torch.from_numpy(u0).cuda()
+    du = torch.empty_like(u)
+    gm.rhs(u, du)
+    torch.cuda.synchronize()
+    ref = om.rhs(u0)
+    err = parity_error(du.cpu().numpy(), ref).max()
+    print(f"c2m: {m.n_elem} elements, {len(m.mortar)} mortars, rhs err {err:.2e}")
+    tol = RHS_TOL
+    if err > RHS_TOL:                      # DESIGN.md reading T1, as in test_gpu_fullsize.py
+        Lf = oracle.lib_fma()
+        if Lf is not None:
+            tol = max(RHS_TOL, 2.0 * float(parity_error(oracle.OracleMesh(m, L=Lf).rhs(u0), ref).max()))
+    assert err <= tol
+    dt = om.max_dt(u0, 0.4)
+    assert abs(gm.max_dt(u, 0.4) - dt) <= 1e-13 * dt
+    un_h = u0 * (1.0 + 1e-3)
+    out = torch.empty_like(u)
+    gm.stage(2, dt, 0.0, torch.from_numpy(un_h).cuda(), u, out)
+    torch.cuda.synchronize()
+    assert parity_error(out.cpu().numpy(), om.ssprk_stage(2, dt, 0.0, un_h, u0)).max() <= tol
+    gm.close()
