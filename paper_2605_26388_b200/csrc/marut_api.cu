@@ -357,7 +357,7 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
     for (int k = 0; k < nfine; ++k) if (M[2 + k] < 0 || M[2 + k] >= ne) return fail(MARUT_ETOPOLOGY, "mortar %ld: element out of range", i);
     if (fC < 0 || fC >= nf2 || fF < 0 || fF >= nf2) return fail(MARUT_ETOPOLOGY, "mortar %ld: face out of range", i);
     bool ok = claim(M[0], fC, (int)i, pack_info(FK_MORTAR_COARSE, fF, 0, 0));
-    for (int k = 0; k < nfine && ok; ++k) ok = claim(M[2 + k], fF, M[0], pack_info(FK_MORTAR_FINE, fC, 0, k));
+    for (int k = 0; k < nfine && ok; ++k) ok = claim(M[2 + k], fF, (dim == 2) ? M[0] : (int)i, pack_info(FK_MORTAR_FINE, fC, 0, k));   // 3-D: the mortar index
     if (!ok) return fail(MARUT_ETOPOLOGY, "mortar %ld: face listed twice", i);
     for (int k = 0; k < nfine; ++k) mfine[i * nfine + k] = M[2 + k];
     minfo[i * 3] = M[0]; minfo[i * 3 + 1] = fC; minfo[i * 3 + 2] = fF;
@@ -840,8 +840,8 @@ extern "C" marut_status marut_shock_indicator(marut_mesh *m, const double *u, do
   m->launches++;
   if (smooth) {
     const unsigned grid = (unsigned)((m->ne + 255) / 256);
-    if (m->dim == 2) indicator_smooth_kernel<2><<<grid, 256, 0, st>>>(raw, m->d_conn, m->d_mortar_fine, m->ne, alpha);
-    else indicator_smooth_kernel<3><<<grid, 256, 0, st>>>(raw, m->d_conn, m->d_mortar_fine, m->ne, alpha);
+    if (m->dim == 2) indicator_smooth_kernel<2><<<grid, 256, 0, st>>>(raw, m->d_conn, m->d_mortar_fine, m->d_mortar_info, m->ne, alpha);
+    else indicator_smooth_kernel<3><<<grid, 256, 0, st>>>(raw, m->d_conn, m->d_mortar_fine, m->d_mortar_info, m->ne, alpha);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail(MARUT_ECUDA, "indicator smoothing kernel: %s", cudaGetErrorString(e));
     m->launches++;

@@ -599,9 +599,11 @@ indicator_kernel(const double *__restrict__ u, const double *__restrict__ Vinv_g
     alpha[e] = a;
   }
 }
+// (3-D: a fine element's mortar entry names the mortar, mortar_info[3 m] its coarse element)
 template <int DIM>
 __global__ void indicator_smooth_kernel(const double *__restrict__ raw, const int2 *__restrict__ conn,
-                                        const int *__restrict__ mortar_fine, long ne, double *__restrict__ alpha) {
+                                        const int *__restrict__ mortar_fine, const int *__restrict__ mortar_info, long ne,
+                                        double *__restrict__ alpha) {
   const long e = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= ne) return;
   double a = raw[e];
@@ -609,7 +611,8 @@ __global__ void indicator_smooth_kernel(const double *__restrict__ raw, const in
   for (int f = 0; f < 2 * DIM; ++f) {
     const int2 cn = __ldg(&conn[e * 2 * DIM + f]);
     const int kind = cn.y & 3;
-    if (kind == FK_CONFORMING || kind == FK_MORTAR_FINE) a = fmax(a, raw[cn.x]);
+    if (kind == FK_CONFORMING || (DIM == 2 && kind == FK_MORTAR_FINE)) a = fmax(a, raw[cn.x]);
+    else if (kind == FK_MORTAR_FINE) a = fmax(a, raw[__ldg(&mortar_info[cn.x * 3])]);
     else if (kind == FK_MORTAR_COARSE) {
       constexpr int NFINE = (DIM == 2) ? 2 : 4;
 #pragma unroll

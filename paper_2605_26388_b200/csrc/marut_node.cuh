@@ -124,41 +124,26 @@ __device__ __noinline__ void node_mortar_flux_2d(const StageParams &P, long e, i
 }
 
 
-// 3-D 4:1 mortar faces (R21): the tensor product of the 2-D construction.  sub = s0 + 2 s1 names
-// the half of the coarse face's first / second face-local direction; the fine elements of coarse mortar m are
-// mortar_fine[4 m + sub].  Affine meshes.  Rare path, kept out of line.
+// 3-D 4:1 mortar faces (R21): the tensor product of the 2-D construction.  The Riemann fluxes
+// F*(U_F, U_i; n_F) at the 4 n^2 fine face nodes of every mortar are evaluated once by mortar_flux3d_kernel before the
+// stage (every coarse face node needs all of them); cn.x = mortar index on both sides, sub = s0 + 2 s1 names the half
+// of the coarse face's first / second face-local direction.  Fine side: its own flux is the stored one.  Coarse side:
+// L2 projection (Pr[s0] x Pr[s1]) of the outward flux -F*, times the area ratio 4.
 template <int NP>
-__device__ __noinline__ void node_mortar_flux_3d(const StageParams &P, long e, int f, int a0, int a1, int2 cn, const double *U,
-                                                 const double *nv, double *Fs) {
-  using G = Geo<3, NP>;
-  constexpr int NVAR = 5, NN = NP * NP * NP, MD = 10;
-  const int kind = cn.y & 3, fR = (cn.y >> 2) & 7, sub = (cn.y >> 8) & 3;
-  const double *Pf = P.mortar_mat, *Prv = P.mortar_mat + 2 * NP * NP;
-  const Prim<3> pr = prim_ideal<3, true>(U, P.gamma);
+__device__ __forceinline__ void node_mortar_flux_3d(const StageParams &P, int a0, int a1, int2 cn, double *Fs) {
+  constexpr int NVAR = 5, NF = NP * NP;
+  const int kind = cn.y & 3, sub = (cn.y >> 8) & 3;
   if (kind == FK_MORTAR_FINE) {
-    const int s0 = sub & 1, s1 = sub >> 1;
-    double Up[NVAR] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    for (int j1 = 0; j1 < NP; ++j1) {
-      const double w1 = __ldg(&Pf[(s1 * NP + a1) * NP + j1]);
-      for (int j0 = 0; j0 < NP; ++j0) {
-        const double w = w1 * __ldg(&Pf[(s0 * NP + a0) * NP + j0]);
-        const double *uc = P.u_in + (long)cn.x * NVAR * NN + G::face_node(fR, j0, j1);
+    const double *F = P.mflux + (((long)cn.x * 4 + sub) * NF + a0 + NP * a1) * NVAR;
 #pragma unroll
-        for (int v = 0; v < NVAR; ++v) Up[v] += w * __ldg(uc + v * NN);
-      }
-    }
-    const Prim<3> qp = prim_ideal<3, true>(Up, P.gamma);
-    double Fm[NVAR];
-    flux_dot<3, 1>(U, pr, nv, Fm);
-    rusanov<3, 1>(U, pr, Fm, Up, qp, nv, Fs);
+    for (int v = 0; v < NVAR; ++v) Fs[v] = __ldg(F + v);
   } else {
-    // coarse side: the fluxes F*(U_F, U_i; n_F) at the 4 n^2 fine face nodes of this mortar were evaluated once by
-    // mortar_flux3d_kernel (every coarse face node needs all of them); here only their L2 projection, times -4
+    const double *Prv = P.mortar_mat + 2 * NP * NP;
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) Fs[v] = 0.0;
     for (int m = 0; m < 4; ++m) {
       const int s0 = m & 1, s1 = m >> 1;
-      const double *Fm_ = P.mflux + ((long)cn.x * 4 + m) * NP * NP * NVAR;
+      const double *Fm_ = P.mflux + ((long)cn.x * 4 + m) * NF * NVAR;
       for (int b1 = 0; b1 < NP; ++b1) {
         const double r1 = -4.0 * __ldg(&Prv[(s1 * NP + a1) * NP + b1]);
         for (int b0 = 0; b0 < NP; ++b0) {
@@ -359,7 +344,7 @@ __device__ __forceinline__ void euler_face_task(const StageParams &P, const doub
       for (int v = 0; v < NVAR; ++v) lift[v] = P.inv_wb * (Fs[v] - Fm[v]);
     } else if constexpr (BCK) {
       double Fs[NVAR];
-      node_mortar_flux_3d<NP>(P, e, t.f, t.a0, t.a1, cn, Um, nv, Fs);
+      node_mortar_flux_3d<NP>(P, t.a0, t.a1, cn, Fs);
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) lift[v] = P.inv_wb * (Fs[v] - Fm[v]);
     } else {
