@@ -303,17 +303,29 @@ def run_cuda(args):
         alpha = torch.zeros(mesh.n_elem, dtype=torch.float64, device=u.device)
         gm.set_blend(alpha)
 
+    # dt stays on the device (marut_max_dt_async -> marut_ssprk_stage_dev: the same dt and the same stage results bit
+    # for bit, tests/test_gpu_async_dt.py), so the host queues the whole step without waiting for the CFL reduction;
+    # --sync-dt times the host-synchronised marut_max_dt instead
+    dt_dev = torch.zeros(1, dtype=torch.float64, device=u.device)
+
     def step(ev=None):
         src = u0_dev if counter[0] % case.steps == 0 else u
         counter[0] += 1
-        dt = gm.max_dt(src, cfl)
+        if args.sync_dt:
+            dt = gm.max_dt(src, cfl)
+        else:
+            gm.max_dt_async(src, cfl, dt_dev)
+            dt = None
         for s, (un, uin, uout) in enumerate(((src, src, ua), (src, ua, ub), (src, ub, u))):
             if sc:
                 gm.shock_indicator(uin, alpha, **sc)
             if ev is not None:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
-            gm.stage(s, dt, 0.0, un, uin, uout)
+            if args.sync_dt:
+                gm.stage(s, dt, 0.0, un, uin, uout)
+            else:
+                gm.stage_dev(s, dt_dev, 0.0, un, uin, uout)
             if ev is not None:
                 e1.record(stream)
                 ev.append((e0, e1))
@@ -354,7 +366,8 @@ def run_cuda(args):
         st = torch.cuda.Stream()
         g = gm if k == 0 else mb.MarutMesh(mesh)
         lanes.append({"st": st, "gm": g, "u": torch.empty_like(u), "ua": torch.empty_like(u), "ub": torch.empty_like(u),
-                      "out": torch.empty_like(u0_host).pin_memory()})
+                      "out": torch.empty_like(u0_host).pin_memory(),
+                      "dt": torch.zeros(1, dtype=torch.float64, device=u.device), "dt_out": torch.zeros(1, dtype=torch.float64).pin_memory()})
         if sc:
             lanes[k]["alpha"] = alpha if k == 0 else torch.zeros_like(alpha)
             g.set_blend(lanes[k]["alpha"])
@@ -363,15 +376,23 @@ def run_cuda(args):
         L = lanes[k % 2]
         with torch.cuda.stream(L["st"]):
             L["u"].copy_(u0_host, non_blocking=True)
-            g, dt = L["gm"], L["gm"].max_dt(L["u"], cfl)
-            if sc:
-                for s_, (uin, uout) in enumerate(((L["u"], L["ua"]), (L["ua"], L["ub"]), (L["ub"], L["u"]))):
-                    g.shock_indicator(uin, L["alpha"], **sc)
-                    g.stage(s_, dt, 0.0, L["u"], uin, uout)
-                    g.positivity_floor(uout)
+            g = L["gm"]
+            if args.sync_dt:
+                dt = g.max_dt(L["u"], cfl)
             else:
-                g.step(L["u"], L["ua"], L["ub"], dt)
+                g.max_dt_async(L["u"], cfl, L["dt"])
+            for s_, (uin, uout) in enumerate(((L["u"], L["ua"]), (L["ua"], L["ub"]), (L["ub"], L["u"]))):
+                if sc:
+                    g.shock_indicator(uin, L["alpha"], **sc)
+                if args.sync_dt:
+                    g.stage(s_, dt, 0.0, L["u"], uin, uout)
+                else:
+                    g.stage_dev(s_, L["dt"], 0.0, L["u"], uin, uout)
+                if sc:
+                    g.positivity_floor(uout)
             L["out"].copy_(L["u"], non_blocking=True)
+            if not args.sync_dt:
+                L["dt_out"].copy_(L["dt"], non_blocking=True)
 
     for k in range(4):
         e2e_step(k)
@@ -426,7 +447,7 @@ def run_cuda(args):
                 "config": {"workload": workload_name(case), "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": f"inputs larger than L2 ({3 * n_dof * 8 / 1e6:.0f} MB of state buffers vs 126 MB)"
                                  if 3 * n_dof * 8 > 126e6 else "state fits L2 (launch/latency-bound case; no flush)",
-                           "step": "marut_max_dt + 3 x (marut_shock_indicator + blended marut_ssprk_stage + marut_positivity_floor)" if sc else "marut_max_dt + 3 x marut_ssprk_stage", "cfl": cfl, "restart_from_u0_every_steps": case.steps, "affine": bool(affine)},
+                           "step": ("marut_max_dt" if args.sync_dt else "marut_max_dt_async (dt stays on the device)") + (" + 3 x (marut_shock_indicator + blended marut_ssprk_stage + marut_positivity_floor)" if sc else " + 3 x marut_ssprk_stage"), "cfl": cfl, "restart_from_u0_every_steps": case.steps, "affine": bool(affine)},
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n_dof * 8, "d2h_bytes_per_step": n_dof * 8 + 8,
                         "ms_per_step": e2e_ms / args.steps,
@@ -451,6 +472,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sync-dt", action="store_true", help="host-synchronised marut_max_dt every step instead of the device-resident dt")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3

@@ -126,6 +126,18 @@ marut_status marut_lincomb(marut_mesh *mesh, int n, const double *coef, const do
  * Warp-shuffle max reduction on the device; dt_out is a HOST pointer; synchronises the stream. */
 marut_status marut_max_dt(marut_mesh *mesh, const double *u, double cfl, double *dt_out, void *cuda_stream);
 
+/* The same dt (bit for bit: the same reduction, eq. 17-18 evaluated on the device with the host's operation order),
+ * written to DEVICE memory dt_dev (one double, caller-owned) without synchronising: the step's stages are queued
+ * behind it on the same stream by marut_ssprk_stage_dev.  A non-finite
+ * or non-positive wave speed cannot be reported here: dt_dev is then NaN and poisons the solution; marut_max_dt is
+ * the checked call.  Uses the handle's reduction scratch: one stream per handle at a time. */
+marut_status marut_max_dt_async(marut_mesh *mesh, const double *u, double cfl, double *dt_dev, void *cuda_stream);
+
+/* marut_ssprk_stage with dt read from DEVICE memory (dt_dev, written earlier on the same stream); the kernel forms
+ * b_s*dt with the rounding of the host product, so results equal marut_ssprk_stage's bit for bit (eq. 45). */
+marut_status marut_ssprk_stage_dev(marut_mesh *mesh, int stage, const double *dt_dev, double t_n, const double *u_n,
+                                   const double *u_in, double *u_out, void *cuda_stream);
+
 /* s = S(u): per-node finite-rate chemistry source (eq. 21-22); species rows omega_s,
  * momentum and energy rows 0.  REACTING_EULER meshes only (else EINVAL). */
 marut_status marut_chem_source(marut_mesh *mesh, const double *u, double *s, void *cuda_stream);

@@ -14,7 +14,7 @@ _lib = None
 _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA", 4: "MARUT_ETOPOLOGY", 5: "MARUT_ENOTFINITE"}
 
 # every symbol include/marut.h declares
-SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt",
+SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt", "marut_max_dt_async", "marut_ssprk_stage_dev",
            "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_rk_stage", "marut_lincomb", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
            "marut_last_error"]
 
@@ -62,6 +62,10 @@ def lib():
         L.marut_ssprk_stage.argtypes = [vp, C.c_int, dbl, dbl, vp, vp, vp, vp]
         L.marut_max_dt.restype = C.c_int
         L.marut_max_dt.argtypes = [vp, vp, dbl, C.POINTER(dbl), vp]
+        L.marut_max_dt_async.restype = C.c_int
+        L.marut_max_dt_async.argtypes = [vp, vp, dbl, vp, vp]
+        L.marut_ssprk_stage_dev.restype = C.c_int
+        L.marut_ssprk_stage_dev.argtypes = [vp, C.c_int, vp, dbl, vp, vp, vp, vp]
         L.marut_chem_source.restype = C.c_int
         L.marut_chem_source.argtypes = [vp, vp, vp, vp]
         L.marut_chem_implicit.restype = C.c_int
@@ -162,6 +166,14 @@ def marut_max_dt(h, u, cfl, stream=None):
     dt = C.c_double(0.0)
     _check(lib().marut_max_dt(h, _dev(u), cfl, C.byref(dt), _stream(stream)))
     return dt.value
+
+
+def marut_max_dt_async(h, u, cfl, dt_dev, stream=None):
+    _check(lib().marut_max_dt_async(h, _dev(u), cfl, _dev(dt_dev), _stream(stream)))
+
+
+def marut_ssprk_stage_dev(h, stage, dt_dev, t_n, u_n, u_in, u_out, stream=None):
+    _check(lib().marut_ssprk_stage_dev(h, stage, _dev(dt_dev), t_n, _dev(u_n), _dev(u_in), _dev(u_out), _stream(stream)))
 
 
 def marut_chem_source(h, u, s, stream=None):
@@ -280,6 +292,12 @@ class MarutMesh:
 
     def max_dt(self, u, cfl, stream=None):
         return marut_max_dt(self.h, u, cfl, stream)
+
+    def max_dt_async(self, u, cfl, dt_dev, stream=None):
+        marut_max_dt_async(self.h, u, cfl, dt_dev, stream)
+
+    def stage_dev(self, stage, dt_dev, t_n, u_n, u_in, u_out, stream=None):
+        marut_ssprk_stage_dev(self.h, stage, dt_dev, t_n, u_n, u_in, u_out, stream)
 
     def chem_source(self, u, s, stream=None):
         marut_chem_source(self.h, u, s, stream)

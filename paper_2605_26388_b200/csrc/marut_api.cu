@@ -486,7 +486,7 @@ extern "C" marut_status marut_mesh_create(const marut_mesh_desc *desc, marut_mes
 static bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
 static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc, const double *u_n, const double *u_in,
-                                 double *u_out, cudaStream_t st) {
+                                 double *u_out, cudaStream_t st, const double *dt_dev = nullptr) {
   if (m->physics == MARUT_NAVIER_STOKES) {
     GradParams G;
     G.u = u_in; G.S = m->d_S; G.metric = m->d_metric; G.conn = m->d_conn;
@@ -509,7 +509,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.u_in = u_in; P.u_n = u_n; P.u_out = u_out;
   P.metric = m->d_metric; P.fnorm = m->d_fnorm; P.affine_flag = m->affine ? 1 : 0; P.explicit_source = m->explicit_source; P.conn = m->d_conn; P.mortar_fine = m->d_mortar_fine; P.mortar_mat = m->d_mortar_mat;
   P.bc_state = m->d_bc; P.S = m->d_S; P.Taux = m->d_T; P.mech = m->d_mech;
-  P.ca = ca; P.cb = cb; P.cc = cc;
+  P.ca = ca; P.cb = cb; P.cc = cc; P.dt_dev = dt_dev;
   P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne;
   memcpy(P.D, m->D, sizeof(P.D));
   P.mflux = m->d_mflux;
@@ -623,6 +623,19 @@ extern "C" marut_status marut_ssprk_stage(marut_mesh *m, int stage, double dt, d
   // Shu-Osher SSP-RK33: u_out = a u_n + b (u_in + dt L(u_in))
   static const double a[3] = {0.0, 0.75, 1.0 / 3.0}, b[3] = {1.0, 0.25, 2.0 / 3.0};
   return run_operator(m, a[stage], b[stage], b[stage] * dt, u_n, u_in, u_out, (cudaStream_t)stream);
+}
+
+// the same stage with the time step read from device memory (written by marut_max_dt_async on the same stream): no
+// host synchronisation between the CFL reduction and the stages.  The kernel forms b * dt as the host does.
+extern "C" marut_status marut_ssprk_stage_dev(marut_mesh *m, int stage, const double *dt_dev, double /*t_n*/, const double *u_n,
+                                              const double *u_in, double *u_out, void *stream) {
+  if (!m || !u_in || !u_out || !dt_dev) return fail(MARUT_EINVAL, "NULL argument");
+  if (stage < 0 || stage > 2) return fail(MARUT_EINVAL, "stage must be 0, 1 or 2");
+  if (stage > 0 && !u_n) return fail(MARUT_EINVAL, "u_n is NULL");
+  if (u_out == u_in) return fail(MARUT_EINVAL, "u_out must not alias u_in");
+  if (misaligned(u_in) || misaligned(u_out) || (stage > 0 && misaligned(u_n))) return fail(MARUT_EINVAL, "buffers must be 16-byte aligned");
+  static const double a[3] = {0.0, 0.75, 1.0 / 3.0}, b[3] = {1.0, 0.25, 2.0 / 3.0};
+  return run_operator(m, a[stage], b[stage], b[stage], u_n, u_in, u_out, (cudaStream_t)stream, dt_dev);
 }
 
 // ======================================================================================
@@ -858,6 +871,40 @@ static cudaError_t run_wave_speed(marut_mesh *m, const double *u, unsigned grid,
     default: wave_speed_kernel<DIM, 5, PH_REACT><<<grid, 256, 0, st>>>(u, m->d_mech, m->gamma, m->mu, m->ne, m->nn, m->d_red); break;
   }
   return cudaGetLastError();
+}
+
+// eq. 17-18 from the reduced maxima, on the device: the expressions of marut_max_dt below, operation for operation
+// (products and quotients only, so no contraction can change a rounding).  A non-finite or non-positive wave speed
+// poisons dt with NaN.
+__global__ void dt_finalize_kernel(const unsigned long long *__restrict__ red, double cfl, double dx_min, double P2, double Pr,
+                                   int ns, double *__restrict__ dt_out) {
+  const double lam = __longlong_as_double((long long)red[0]), nu = __longlong_as_double((long long)red[1]);
+  double dt;
+  if (red[2] != 0ULL || !(lam > 0.0) || !isfinite(lam)) dt = __longlong_as_double(0x7ff8000000000000LL);
+  else {
+    dt = __ddiv_rn(__dmul_rn(cfl, dx_min), __dmul_rn(P2, lam));
+    if (ns && nu > 0.0) {
+      const double numax = __dmul_rn(nu, fmax(1.0, __ddiv_rn(1.0, Pr)));
+      dt = fmin(dt, __ddiv_rn(__dmul_rn(__dmul_rn(cfl, dx_min), dx_min), __dmul_rn(__dmul_rn(P2, P2), numax)));
+    }
+  }
+  *dt_out = dt;
+}
+
+extern "C" marut_status marut_max_dt_async(marut_mesh *m, const double *u, double cfl, double *dt_dev, void *stream) {
+  if (!m || !u || !dt_dev) return fail(MARUT_EINVAL, "NULL argument");
+  if (!(cfl > 0.0)) return fail(MARUT_EINVAL, "cfl must be positive");
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(cudaMemsetAsync(m->d_red, 0, 3 * sizeof(unsigned long long), st));
+  const long total = m->ne * m->nn;
+  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * 8);
+  cudaError_t e = (m->dim == 2) ? run_wave_speed<2>(m, u, grid, st) : run_wave_speed<3>(m, u, grid, st);
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "wave speed kernel: %s", cudaGetErrorString(e));
+  dt_finalize_kernel<<<1, 1, 0, st>>>(m->d_red, cfl, m->dx_min, 2.0 * m->N + 1.0, m->Pr, m->physics == MARUT_NAVIER_STOKES ? 1 : 0, dt_dev);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "dt kernel: %s", cudaGetErrorString(e));
+  m->launches += 2;
+  return MARUT_OK;
 }
 
 extern "C" marut_status marut_max_dt(marut_mesh *m, const double *u, double cfl, double *dt_out, void *stream) {

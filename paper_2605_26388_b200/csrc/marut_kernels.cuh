@@ -266,10 +266,10 @@ stage_kernel(const __grid_constant__ StageParams P) {
     const double *np_ = P.u_n + e * NVAR * NN + p;
 #pragma unroll
     for (int v = 0; v < NVAR; ++v)
-      op[v * NN] = P.ca * np_[v * NN] + (P.cb * U[v] + P.cc * (src[v] - invJ * R[v]));
+      op[v * NN] = P.ca * np_[v * NN] + (P.cb * U[v] + stage_cc(P) * (src[v] - invJ * R[v]));
   } else {
 #pragma unroll
-    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.cb * U[v] + P.cc * (src[v] - invJ * R[v]);
+    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.cb * U[v] + stage_cc(P) * (src[v] - invJ * R[v]);
   }
 }
 

@@ -398,7 +398,7 @@ __global__ void __launch_bounds__((LineCfg<DIM, NP, 1, EB>::NT)) stage_line_kern
         double r = R[i][v];
         if (on_eta) r += fl[v * EB * NNP + i];
         if (on_zeta) r += fl[FPL + v * EB * NNP + i];
-        const double val = P.cb * ul[v * NN + i] + P.cc * (0.0 - invJ * r);
+        const double val = P.cb * ul[v * NN + i] + stage_cc(P) * (0.0 - invJ * r);
         nl[v * NN + i] = use_un ? (P.ca * nl[v * NN + i] + val) : val;
       }
     }

@@ -262,7 +262,7 @@ __global__ void __launch_bounds__((Line2Cfg<NP, EB>::NT), 2) stage_line2_kernel(
         for (int i = 0; i < NP; ++i) r[i] += lzz[v * NL + i];
       }
 #pragma unroll
-      for (int i = 0; i < NP; ++i) nl[v * NN + i] = P.ca * un[i] + (P.cb * uu[i] + P.cc * (0.0 - invJ * (R[i][v] + r[i])));
+      for (int i = 0; i < NP; ++i) nl[v * NN + i] = P.ca * un[i] + (P.cb * uu[i] + stage_cc(P) * (0.0 - invJ * (R[i][v] + r[i])));
     }
   }
   fence_async_smem();

@@ -644,7 +644,7 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
 #pragma unroll
     for (int m = 0; m < NP; ++m) {
       if constexpr (!AFFINE) invJ = __ldg(&P.metric[(e * MD + DIM * DIM) * NN + ij + m * GS]);
-      const double val = P.cb * us[m * GS] + P.cc * (0.0 - invJ * acc[m]);
+      const double val = P.cb * us[m * GS] + stage_cc(P) * (0.0 - invJ * acc[m]);
       P.u_out[gofs + m * GS] = use_un ? (P.ca * un[m] + val) : val;
     }
   }

@@ -317,7 +317,7 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       if constexpr (PHYS == PH_REACT) {
         if (v < NSP) src = Src[v * TILE + le * NN + ij + m * GS];
       }
-      const double val = P.cb * us[m * GS] + P.cc * (src - invJ * acc[m]);
+      const double val = P.cb * us[m * GS] + stage_cc(P) * (src - invJ * acc[m]);
       P.u_out[gofs + m * GS] = use_un ? (P.ca * un[m] + val) : val;
     }
   }

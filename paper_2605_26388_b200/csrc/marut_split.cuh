@@ -315,10 +315,10 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
   double *op = P.u_out + e * NVAR * NN + p;
   if (use_un) {
 #pragma unroll
-    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.ca * Un[v] + (P.cb * U[v] + P.cc * (0.0 - invJ * R[v]));
+    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.ca * Un[v] + (P.cb * U[v] + stage_cc(P) * (0.0 - invJ * R[v]));
   } else {
 #pragma unroll
-    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.cb * U[v] + P.cc * (0.0 - invJ * R[v]);
+    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.cb * U[v] + stage_cc(P) * (0.0 - invJ * R[v]);
   }
 }
 

@@ -1,0 +1,72 @@
+"""Device-resident time step (eq. 45): marut_max_dt_async writes the dt
+marut_max_dt returns, bit for bit, and marut_ssprk_stage_dev reproduces marut_ssprk_stage bit for bit, so the step
+needs no host synchronisation; the composed run is compared with the oracle as every other run is."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from parity_util import RUN_TOL, parity_error
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("name,cells,split", [("c1", 8, 0), ("c1", 8, 1), ("c2", 3, 0), ("c3", 3, 0), ("c4", 32, 0), ("c5", 4, 0)])
+def test_async_dt_steps(name, cells, split):
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    c = wl.make_case(name, cells=cells)
+    c.mesh.volume_form = split
+    om, gm = oracle.OracleMesh(c.mesh), mb.MarutMesh(c.mesh)
+    u = torch.from_numpy(c.u0).cuda()
+    v = u.clone()
+    ua, ub = torch.empty_like(u), torch.empty_like(u)
+    dt_dev = torch.zeros(1, dtype=torch.float64, device=u.device)
+    uh = c.u0
+    for _ in range(3):
+        # host-synchronised step
+        dt = gm.max_dt(u, c.cfl)
+        gm.step(u, ua, ub, dt)
+        # the same step with dt resident on the device: nothing below waits for the GPU
+        gm.max_dt_async(v, c.cfl, dt_dev)
+        gm.stage_dev(0, dt_dev, 0.0, v, v, ua)
+        gm.stage_dev(1, dt_dev, 0.0, v, ua, ub)
+        gm.stage_dev(2, dt_dev, 0.0, v, ub, v)
+        torch.cuda.synchronize()
+        assert dt_dev.item() == dt
+        assert torch.equal(u, v)
+        dth = om.max_dt(uh, c.cfl)
+        assert abs(dt - dth) <= 1e-12 * dth
+        uh = om.run(uh, 1, cfl=c.cfl)[0]
+    assert parity_error(v.cpu().numpy(), uh).max() <= RUN_TOL
+    gm.close()
+
+
+def test_async_dt_poison_and_arguments():
+    import torch
+
+    import paper_2605_26388_b200 as mb
+
+    c = wl.make_case("c1", cells=4)
+    gm = mb.MarutMesh(c.mesh)
+    u = torch.from_numpy(c.u0).cuda()
+    a = torch.empty_like(u)
+    dt_dev = torch.zeros(1, dtype=torch.float64, device=u.device)
+    bad = u.clone()
+    bad[3, 0, 2] = -1.0                                      # negative density: the checked call reports it ...
+    with pytest.raises(mb.MarutError):
+        gm.max_dt(bad, 0.5)
+    gm.max_dt_async(bad, 0.5, dt_dev)                        # ... the asynchronous one poisons dt
+    torch.cuda.synchronize()
+    assert np.isnan(dt_dev.item())
+    with pytest.raises(mb.MarutError):
+        gm.max_dt_async(u, -1.0, dt_dev)
+    with pytest.raises(mb.MarutError):
+        gm.stage_dev(3, dt_dev, 0.0, u, u, a)
+    with pytest.raises(mb.MarutError):
+        gm.stage_dev(0, dt_dev, 0.0, u, a, a)                # u_out aliases u_in
+    with pytest.raises(mb.MarutError):
+        gm.stage_dev(0, None, 0.0, u, u, a)
+    gm.close()
