@@ -138,6 +138,12 @@ marut_status marut_max_dt_async(marut_mesh *mesh, const double *u, double cfl, d
 marut_status marut_ssprk_stage_dev(marut_mesh *mesh, int stage, const double *dt_dev, double t_n, const double *u_n,
                                    const double *u_in, double *u_out, void *cuda_stream);
 
+/* marut_rk_stage with c_dt = c*dt formed in the kernel from dt_dev (DEVICE, one double): u_out = a*u_a + b*u_in +
+ * (c*dt)*L(u_in) (eq. 45); equal to marut_rk_stage(a, b, c*dt, ...) bit for bit.  With
+ * marut_lincomb (which needs no dt) it composes an SSP-RK54 step without a host synchronisation. */
+marut_status marut_rk_stage_dev(marut_mesh *mesh, double a, double b, double c, const double *dt_dev, const double *u_a,
+                                const double *u_in, double *u_out, void *cuda_stream);
+
 /* s = S(u): per-node finite-rate chemistry source (eq. 21-22); species rows omega_s,
  * momentum and energy rows 0.  REACTING_EULER meshes only (else EINVAL). */
 marut_status marut_chem_source(marut_mesh *mesh, const double *u, double *s, void *cuda_stream);

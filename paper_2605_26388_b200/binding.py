@@ -14,7 +14,7 @@ _lib = None
 _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA", 4: "MARUT_ETOPOLOGY", 5: "MARUT_ENOTFINITE"}
 
 # every symbol include/marut.h declares
-SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt", "marut_max_dt_async", "marut_ssprk_stage_dev",
+SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt", "marut_max_dt_async", "marut_ssprk_stage_dev", "marut_rk_stage_dev",
            "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_rk_stage", "marut_lincomb", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
            "marut_last_error"]
 
@@ -72,6 +72,8 @@ def lib():
         L.marut_chem_implicit.argtypes = [vp, vp, dbl, C.POINTER(C.c_int), vp]
         L.marut_shock_indicator.restype = C.c_int
         L.marut_shock_indicator.argtypes = [vp, vp, dbl, dbl, dbl, C.c_int, vp, vp]
+        L.marut_rk_stage_dev.restype = C.c_int
+        L.marut_rk_stage_dev.argtypes = [vp, dbl, dbl, dbl, vp, vp, vp, vp, vp]
         L.marut_rk_stage.restype = C.c_int
         L.marut_rk_stage.argtypes = [vp, dbl, dbl, dbl, vp, vp, vp, vp]
         L.marut_lincomb.restype = C.c_int
@@ -201,6 +203,10 @@ def marut_rk_stage(h, a, b, c_dt, u_a, u_in, u_out, stream=None):
     _check(lib().marut_rk_stage(h, a, b, c_dt, _dev(u_a), _dev(u_in), _dev(u_out), _stream(stream)))
 
 
+def marut_rk_stage_dev(h, a, b, c, dt_dev, u_a, u_in, u_out, stream=None):
+    _check(lib().marut_rk_stage_dev(h, a, b, c, _dev(dt_dev), _dev(u_a), _dev(u_in), _dev(u_out), _stream(stream)))
+
+
 def marut_lincomb(h, coef, us, out, stream=None):
     n = len(us)
     cf = (C.c_double * n)(*[float(x) for x in coef])
@@ -225,6 +231,18 @@ def ssprk54_step(h, u, ua, ub, uc, dt, stream=None):
     r = b[2] / a[3][2]                                                                   # dt L(U3) = (U4 - a40 U0 - a43 U3)/b43
     marut_lincomb(h, (-r * a[3][0], b[0], b[1] - r * a[3][1], b[3] + r), (u, ub, ua, uc), ua, stream)
     marut_rk_stage(h, 1.0, 0.0, b[4] * dt, ua, uc, u, stream)                           # U5 -> u
+
+
+def ssprk54_step_dev(h, u, ua, ub, uc, dt_dev, stream=None):
+    """ssprk54_step with the time step in device memory (marut_max_dt_async): nothing here waits for the GPU"""
+    a, b = _RK54, _RK54_LAST
+    marut_rk_stage_dev(h, 0.0, 1.0, a[0][2], dt_dev, None, u, ua, stream)
+    marut_rk_stage_dev(h, a[1][0], a[1][1], a[1][2], dt_dev, u, ua, ub, stream)
+    marut_rk_stage_dev(h, a[2][0], a[2][1], a[2][2], dt_dev, u, ub, ua, stream)
+    marut_rk_stage_dev(h, a[3][0], a[3][1], a[3][2], dt_dev, u, ua, uc, stream)
+    r = b[2] / a[3][2]
+    marut_lincomb(h, (-r * a[3][0], b[0], b[1] - r * a[3][1], b[3] + r), (u, ub, ua, uc), ua, stream)
+    marut_rk_stage_dev(h, 1.0, 0.0, b[4], dt_dev, ua, uc, u, stream)
 
 
 def marut_shock_indicator(h, u, alpha, s=9.21024, alpha_min=0.001, alpha_max=0.5, smooth=True, stream=None):
@@ -322,6 +340,12 @@ class MarutMesh:
 
     def ssprk54_step(self, u, ua, ub, uc, dt, stream=None):
         ssprk54_step(self.h, u, ua, ub, uc, dt, stream)
+
+    def rk_stage_dev(self, a, b, c, dt_dev, u_a, u_in, u_out, stream=None):
+        marut_rk_stage_dev(self.h, a, b, c, dt_dev, u_a, u_in, u_out, stream)
+
+    def ssprk54_step_dev(self, u, ua, ub, uc, dt_dev, stream=None):
+        ssprk54_step_dev(self.h, u, ua, ub, uc, dt_dev, stream)
 
     def set_blend(self, alpha):
         self._alpha = alpha          # the library keeps the pointer: hold the tensor

@@ -667,6 +667,16 @@ extern "C" marut_status marut_rk_stage(marut_mesh *m, double a, double b, double
   return run_operator(m, a, b, c_dt, u_a, u_in, u_out, (cudaStream_t)stream);
 }
 
+// marut_rk_stage with c_dt = c * dt formed in the kernel from the device-resident dt (marut_max_dt_async)
+extern "C" marut_status marut_rk_stage_dev(marut_mesh *m, double a, double b, double c, const double *dt_dev, const double *u_a,
+                                           const double *u_in, double *u_out, void *stream) {
+  if (!m || !u_in || !u_out || !dt_dev) return fail(MARUT_EINVAL, "NULL argument");
+  if (a != 0.0 && !u_a) return fail(MARUT_EINVAL, "u_a is NULL");
+  if (u_out == u_in) return fail(MARUT_EINVAL, "u_out must not alias u_in");
+  if (misaligned(u_in) || misaligned(u_out) || (a != 0.0 && misaligned(u_a))) return fail(MARUT_EINVAL, "buffers must be 16-byte aligned");
+  return run_operator(m, a, b, c, u_a, u_in, u_out, (cudaStream_t)stream, dt_dev);
+}
+
 extern "C" marut_status marut_lincomb(marut_mesh *m, int n, const double *coef, const double *const *u, double *out, void *stream) {
   if (!m || !coef || !u || !out) return fail(MARUT_EINVAL, "NULL argument");
   if (n < 1 || n > 4) return fail(MARUT_EINVAL, "marut_lincomb: 1 <= n <= 4");

@@ -44,6 +44,32 @@ def test_async_dt_steps(name, cells, split):
     gm.close()
 
 
+@pytest.mark.parametrize("name,cells", [("c1", 8), ("c2", 3), ("c3", 3), ("c4", 32)])
+def test_async_dt_ssprk54(name, cells):
+    """SSP-RK54 (R19) composed from marut_rk_stage_dev: bit-identical to the host-dt composition, whose
+    parity with the oracle tests/test_gpu_rk54.py establishes"""
+    import torch
+
+    import paper_2605_26388_b200 as mb
+
+    c = wl.make_case(name, cells=cells)
+    gm = mb.MarutMesh(c.mesh)
+    u = torch.from_numpy(c.u0).cuda()
+    v = u.clone()
+    ua, ub, uc = torch.empty_like(u), torch.empty_like(u), torch.empty_like(u)
+    dt_dev = torch.zeros(1, dtype=torch.float64, device=u.device)
+    for _ in range(3):
+        dt = gm.max_dt(u, 1.5 * c.cfl)
+        gm.ssprk54_step(u, ua, ub, uc, dt)
+        gm.max_dt_async(v, 1.5 * c.cfl, dt_dev)
+        gm.ssprk54_step_dev(v, ua, ub, uc, dt_dev)
+        torch.cuda.synchronize()
+        assert dt_dev.item() == dt
+        assert torch.equal(u, v)
+    assert torch.isfinite(v).all()
+    gm.close()
+
+
 def test_async_dt_poison_and_arguments():
     import torch
 
@@ -69,4 +95,8 @@ def test_async_dt_poison_and_arguments():
         gm.stage_dev(0, dt_dev, 0.0, u, a, a)                # u_out aliases u_in
     with pytest.raises(mb.MarutError):
         gm.stage_dev(0, None, 0.0, u, u, a)
+    with pytest.raises(mb.MarutError):
+        gm.rk_stage_dev(1.0, 1.0, 1.0, dt_dev, None, u, a)    # a != 0 needs u_a
+    with pytest.raises(mb.MarutError):
+        gm.rk_stage_dev(0.0, 1.0, 1.0, dt_dev, None, a, a)    # u_out aliases u_in
     gm.close()
