@@ -100,3 +100,52 @@ def test_async_dt_poison_and_arguments():
     with pytest.raises(mb.MarutError):
         gm.rk_stage_dev(0.0, 1.0, 1.0, dt_dev, None, a, a)    # u_out aliases u_in
     gm.close()
+
+
+@pytest.mark.parametrize("name,cells", [("c1", 16), ("c4", 32), ("c3", 3)])
+def test_step_in_cuda_graph(name, cells):
+    """with dt on the device the whole step (CFL reduction + three stages) has no host dependence: captured once in a
+    CUDA graph and replayed, it advances the solution exactly as the eager calls do (launch-bound small meshes,
+    PAPER.md:436)"""
+    import torch
+
+    import paper_2605_26388_b200 as mb
+
+    c = wl.make_case(name, cells=cells)
+    gm = mb.MarutMesh(c.mesh)
+    u = torch.from_numpy(c.u0).cuda()
+    v = u.clone()
+    ua, ub = torch.empty_like(u), torch.empty_like(u)
+    dt_dev = torch.zeros(1, dtype=torch.float64, device=u.device)
+
+    def step(w):
+        gm.max_dt_async(w, c.cfl, dt_dev)
+        gm.stage_dev(0, dt_dev, 0.0, w, w, ua)
+        gm.stage_dev(1, dt_dev, 0.0, w, ua, ub)
+        gm.stage_dev(2, dt_dev, 0.0, w, ub, w)
+
+    nsteps = 6
+    for _ in range(nsteps):
+        step(u)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        step(v)
+    v.copy_(torch.from_numpy(c.u0))                           # capture does not execute; start from u0 all the same
+    for _ in range(nsteps):
+        graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(u, v)
+    # timing, informational (CUDA events on the current stream)
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    e0.record()
+    for _ in range(50):
+        step(u)
+    e1.record()
+    for _ in range(50):
+        graph.replay()
+    e2.record()
+    torch.cuda.synchronize()
+    print(f"\n{name} cells={cells}: eager {e0.elapsed_time(e1) / 50 * 1e3:.1f} us/step, graph {e1.elapsed_time(e2) / 50 * 1e3:.1f} us/step")
+    del graph
+    gm.close()
