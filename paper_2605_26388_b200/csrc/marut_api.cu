@@ -873,14 +873,27 @@ extern "C" marut_status marut_shock_indicator(marut_mesh *m, const double *u, do
 }
 
 // ------------------------------------------------------------------------------------ time step
-template <int DIM>
-static cudaError_t run_wave_speed(marut_mesh *m, const double *u, unsigned grid, cudaStream_t st) {
-  switch (m->physics) {
-    case MARUT_EULER: wave_speed_kernel<DIM, 1, PH_EULER><<<grid, 256, 0, st>>>(u, nullptr, m->gamma, m->mu, m->ne, m->nn, m->d_red); break;
-    case MARUT_NAVIER_STOKES: wave_speed_kernel<DIM, 1, PH_NS><<<grid, 256, 0, st>>>(u, nullptr, m->gamma, m->mu, m->ne, m->nn, m->d_red); break;
-    default: wave_speed_kernel<DIM, 5, PH_REACT><<<grid, 256, 0, st>>>(u, m->d_mech, m->gamma, m->mu, m->ne, m->nn, m->d_red); break;
+template <int DIM, int NSP, int PHYS>
+static cudaError_t launch_wave_speed(marut_mesh *m, const double *u, const MechDev *mech, cudaStream_t st) {
+  // one resident wave: grid = SMs x the CTAs per SM this instantiation's registers allow
+  static int occ = 0;
+  if (occ == 0) {
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, wave_speed_kernel<DIM, NSP, PHYS>, 256, 0);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) occ = 1;
   }
+  const long total = m->ne * m->nn;
+  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * occ);
+  wave_speed_kernel<DIM, NSP, PHYS><<<grid, 256, 0, st>>>(u, mech, m->gamma, m->mu, m->ne, m->nn, m->d_red);
   return cudaGetLastError();
+}
+template <int DIM>
+static cudaError_t run_wave_speed(marut_mesh *m, const double *u, unsigned /*grid*/, cudaStream_t st) {
+  switch (m->physics) {
+    case MARUT_EULER: return launch_wave_speed<DIM, 1, PH_EULER>(m, u, nullptr, st);
+    case MARUT_NAVIER_STOKES: return launch_wave_speed<DIM, 1, PH_NS>(m, u, nullptr, st);
+    default: return launch_wave_speed<DIM, 5, PH_REACT>(m, u, m->d_mech, st);
+  }
 }
 
 // eq. 17-18 from the reduced maxima, on the device: the expressions of marut_max_dt below, operation for operation

@@ -682,24 +682,39 @@ __global__ void __launch_bounds__(256) wave_speed_kernel(const double *__restric
   double lam = 0.0, nu = 0.0;
   int bad = 0;
   const long total = ne * nn;
-  for (long g = (long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
-    const long e = g / nn;
-    const int p = (int)(g - e * nn);
-    double U[NVAR];
+  // two nodes per trip (one grid stride apart), all loads of both issued before either is used: twice the bytes in
+  // flight per thread; the maxima do not depend on the order
+  constexpr int UNR = (PHYS == PH_REACT) ? 1 : 2;
+  const long stride = (long)gridDim.x * blockDim.x;
+  for (long g0 = (long)blockIdx.x * blockDim.x + threadIdx.x; g0 < total; g0 += UNR * stride) {
+    double U[UNR][NVAR];
+    bool on[UNR];
 #pragma unroll
-    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(u + (e * NVAR + v) * nn + p);
-    Prim<DIM> q;
-    if constexpr (PHYS == PH_REACT) {
-      const double T = temperature_newton<NSP>(mech, U, internal_energy<DIM, NSP>(U));
-      q = prim_mixture<DIM, NSP, true>(U, T, mech);
-    } else q = prim_ideal<DIM, true>(U, gamma);
-    double v2 = 0.0;
+    for (int k = 0; k < UNR; ++k) {
+      const long g = g0 + k * stride;
+      on[k] = g < total;
+      const long gc = on[k] ? g : g0;
+      const long e = gc / nn;
+      const int p = (int)(gc - e * nn);
 #pragma unroll
-    for (int c = 0; c < DIM; ++c) v2 += q.v[c] * q.v[c];
-    const double l = sqrt(v2) + q.a;
-    if (!(l > 0.0) || !isfinite(l)) bad = 1;
-    lam = fmax(lam, l);
-    if constexpr (PHYS == PH_NS) nu = fmax(nu, mu / q.rho);
+      for (int v = 0; v < NVAR; ++v) U[k][v] = __ldg(u + (e * NVAR + v) * nn + p);
+    }
+#pragma unroll
+    for (int k = 0; k < UNR; ++k) {
+      if (!on[k]) continue;
+      Prim<DIM> q;
+      if constexpr (PHYS == PH_REACT) {
+        const double T = temperature_newton<NSP>(mech, U[k], internal_energy<DIM, NSP>(U[k]));
+        q = prim_mixture<DIM, NSP, true>(U[k], T, mech);
+      } else q = prim_ideal<DIM, true>(U[k], gamma);
+      double v2 = 0.0;
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) v2 += q.v[c] * q.v[c];
+      const double l = sqrt(v2) + q.a;
+      if (!(l > 0.0) || !isfinite(l)) bad = 1;
+      lam = fmax(lam, l);
+      if constexpr (PHYS == PH_NS) nu = fmax(nu, mu / q.rho);
+    }
   }
   lam = warp_max(lam);
   nu = warp_max(nu);
