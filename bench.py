@@ -427,7 +427,7 @@ def run_cuda(args):
                 prof = {}
         kernels = {0: ("stage_split_kernel (fused Euler stage, split-form volume integral" + (" blended with the sub-cell FV residual)" if sc else ")")) if getattr(mesh, "volume_form", 0) else ("mortar_flux3d_kernel + stage_node_kernel (fused Euler stage, 3-D mortar instantiation)" if (mesh.dim == 3 and len(mesh.mortar)) else "stage_node_kernel (fused Euler stage)"), 1: "gradient_kernel + stage_phys_kernel (BR1 gradient sweep + fused NS stage)",
                    2: "eos_kernel + stage_phys_kernel (mixture temperature + fused reacting stage)"}[mesh.physics]
-        roof = {"bound": "hbm", "kernel": "marut_ssprk_stage: " + kernels, "achieved": achieved, "peak": peak, "unit": "GB/s",
+        roof = {"bound": "hbm", "kernel": ("marut_ssprk_stage: " if args.sync_dt else "marut_ssprk_stage_dev: ") + kernels, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": prof.get(args.workload), "peak_source": peak_src, "bytes_per_dof_stage": b_alg,
                 "stage_ms_avg": stage_ms_avg, "frac_of_8TBs_nominal": achieved / 8000.0}
         if mesh.physics == 1:
