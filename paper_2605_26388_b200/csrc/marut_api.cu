@@ -1,6 +1,7 @@
 // marut_api.cu -- the C ABI of include/marut.h: setup, dispatch of the fused stage
 // kernels, the CFL reduction and the chemistry source.  Product code; shares nothing with oracle/.
 #include "../../include/marut.h"
+#include <atomic>
 #include "marut_kernels.cuh"
 #include "marut_launch.h"
 
@@ -48,7 +49,6 @@ struct marut_mesh {
   double *d_fnorm = nullptr;   // affine: [e][dim] |Ja^l|
   int explicit_source = 1;     // reacting: L includes S(U) (default) or is the transport operator only
   int volume_form = 0;         // MARUT_VOLUME_STRONG | MARUT_VOLUME_SPLIT_RANOCHA
-  int kernel_sel = 0;          // Euler stage kernel: 0 node (marut_node.cuh), 1 line (marut_line.cuh), 2 generic; env MARUT_KERNEL
   int2 *d_conn = nullptr;
   int *d_mortar_fine = nullptr;
   int *d_mortar_info = nullptr;   // 3-D: [m][3] = eC, fC, fF
@@ -64,7 +64,9 @@ struct marut_mesh {
   double *d_subn = nullptr;  // curved meshes: sub-cell normals [e][l][c][node] (allocated by the first marut_set_blend)
   unsigned long long *d_red = nullptr;
   unsigned long long *h_red = nullptr;  // pinned
-  long launches = 0;
+  std::atomic<long> launches{0};   // kernels launched through this handle (introspection; any thread)
+  int ws_occ = 0;                  // resident CTAs per SM of this handle's wave_speed_kernel (queried on first use)
+  int device = 0, num_sms = 148;   // the device the handle was created on and its multiprocessor count
 };
 
 // ------------------------------------------------------------------------------------ 1-D operators
@@ -452,10 +454,8 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   if (m->physics == MARUT_NAVIER_STOKES) CUDA_TRY(cudaMalloc(&m->d_S, (size_t)ne * (dim * (dim + 1) / 2 + dim) * nn * sizeof(double)));
   if (m->physics == MARUT_REACTING_EULER) CUDA_TRY(cudaMalloc(&m->d_T, (size_t)ne * nn * sizeof(double)));
 
-  const char *sel = getenv("MARUT_KERNEL");   // A/B switch for profiling: node (default) | line | generic
-  m->kernel_sel = (sel && !strcmp(sel, "line")) ? 1 : ((sel && !strcmp(sel, "generic")) ? 2 : ((sel && !strcmp(sel, "line2")) ? 3 : 0));
-  if (dim == 3 && d->n_mortar > 0 && (m->kernel_sel != 0 || !m->affine))
-    return fail(MARUT_EINVAL, "3-D mortar faces need an affine mesh and the default kernels (MARUT_KERNEL unset)");
+  if (dim == 3 && d->n_mortar > 0 && !m->affine)
+    return fail(MARUT_EINVAL, "3-D mortar faces need an affine mesh");
   return MARUT_OK;
 }
 
@@ -469,6 +469,12 @@ extern "C" marut_status marut_mesh_create(const marut_mesh_desc *desc, marut_mes
   }
   marut_mesh *m = new (std::nothrow) marut_mesh;
   if (!m) return fail(MARUT_ENOMEM, "host allocation failed");
+  if (cudaGetDevice(&m->device) != cudaSuccess ||
+      cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, m->device) != cudaSuccess || m->num_sms < 1) {
+    delete m;
+    cudaGetLastError();
+    return fail(MARUT_ECUDA, "cannot query the current CUDA device");
+  }
   marut_status st = create_impl(desc, m);
   if (st != MARUT_OK) {
     char keep[sizeof(g_err)];
@@ -498,7 +504,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   }
   if (m->physics == MARUT_REACTING_EULER) {
     const long total = m->ne * m->nn;
-    const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * 16);
+    const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, (long)m->num_sms * 16);
     if (m->dim == 2) eos_kernel<2, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn);
     else eos_kernel<3, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn);
     cudaError_t e = cudaGetLastError();
@@ -510,7 +516,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.metric = m->d_metric; P.fnorm = m->d_fnorm; P.affine_flag = m->affine ? 1 : 0; P.explicit_source = m->explicit_source; P.conn = m->d_conn; P.mortar_fine = m->d_mortar_fine; P.mortar_mat = m->d_mortar_mat;
   P.bc_state = m->d_bc; P.S = m->d_S; P.Taux = m->d_T; P.mech = m->d_mech;
   P.ca = ca; P.cb = cb; P.cc = cc; P.dt_dev = dt_dev;
-  P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne;
+  P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne; P.num_sms = m->num_sms;
   memcpy(P.D, m->D, sizeof(P.D));
   P.mflux = m->d_mflux;
   if (m->dim == 3 && m->n_mortar > 0) {
@@ -529,16 +535,11 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   cudaError_t e;
   switch (m->physics) {
     case MARUT_EULER:
-      e = cudaErrorNotSupported;
-      if (m->volume_form == MARUT_VOLUME_SPLIT_RANOCHA) { e = launch_stage_split(m->dim, m->np, m->affine, P, st); break; }
-      if (m->kernel_sel == 3 && m->dim == 3 && m->affine && m->n_mortar == 0 && !m->oriented) e = launch_stage_line2_3d(m->np, P, st);
-      if (m->kernel_sel == 0 || (m->kernel_sel == 3 && e == cudaErrorNotSupported)) e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
-      if (m->kernel_sel == 1) e = (m->dim == 2) ? launch_stage_line2d(m->np, m->affine, P, st) : launch_stage_line3d(m->np, m->affine, P, st);
-      if (e == cudaErrorNotSupported)
-        e = (m->dim == 2) ? launch_stage_euler2d(m->np, m->affine, P, st) : launch_stage_euler3d(m->np, m->affine, P, st);
+      if (m->volume_form == MARUT_VOLUME_SPLIT_RANOCHA) e = launch_stage_split(m->dim, m->np, m->affine, P, st);
+      else e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
       break;
-    case MARUT_NAVIER_STOKES: e = launch_stage_ns(m->dim, m->np, m->affine, m->kernel_sel == 2, P, st); break;
-    default: e = launch_stage_react(m->dim, m->np, m->nsp, m->affine, m->kernel_sel == 2, P, st); break;
+    case MARUT_NAVIER_STOKES: e = launch_stage_ns(m->dim, m->np, m->affine, P, st); break;
+    default: e = launch_stage_react(m->dim, m->np, m->nsp, m->affine, P, st); break;
   }
   if (e == cudaErrorNotSupported) return fail(MARUT_EINVAL, "no kernel instantiated for dim=%d N=%d physics=%d", m->dim, m->N, m->physics);
   if (e != cudaSuccess) return fail(MARUT_ECUDA, "stage kernel: %s", cudaGetErrorString(e));
@@ -588,7 +589,7 @@ extern "C" marut_status marut_set_blend(marut_mesh *m, const double *alpha) {
     SubnParams S;
     S.metric = m->d_metric; S.subn = m->d_subn; S.ne = m->ne; S.dim = m->dim; S.np = m->np; S.nn = m->nn;
     memcpy(S.D, m->D, sizeof(S.D)); memcpy(S.w, m->w, sizeof(S.w));
-    subcell_normals_kernel<<<(unsigned)std::min<size_t>((n + 255) / 256, 148u * 16u), 256>>>(S);
+    subcell_normals_kernel<<<(unsigned)std::min<size_t>((n + 255) / 256, (size_t)m->num_sms * 16u), 256>>>(S);
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaDeviceSynchronize());
   }
@@ -684,7 +685,7 @@ extern "C" marut_status marut_lincomb(marut_mesh *m, int n, const double *coef, 
   for (int k = 0; k < 4; ++k) { P.u[k] = (k < n) ? u[k] : nullptr; P.c[k] = (k < n) ? coef[k] : 0.0; }
   for (int k = 0; k < n; ++k) if (!u[k]) return fail(MARUT_EINVAL, "marut_lincomb: u[%d] is NULL", k);
   P.out = out; P.len = m->ne * m->nvar * m->nn; P.n = n;
-  const unsigned grid = (unsigned)std::min<long>((P.len + 255) / 256, 148L * 32);
+  const unsigned grid = (unsigned)std::min<long>((P.len + 255) / 256, (long)m->num_sms * 32);
   lincomb_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(P);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(MARUT_ECUDA, "lincomb kernel: %s", cudaGetErrorString(e));
@@ -697,7 +698,7 @@ extern "C" marut_status marut_chem_source(marut_mesh *m, const double *u, double
   if (m->physics != MARUT_REACTING_EULER) return fail(MARUT_EINVAL, "marut_chem_source needs a REACTING_EULER mesh");
   if (u == s) return fail(MARUT_EINVAL, "s must not alias u");
   const long total = m->ne * m->nn;
-  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * 16);
+  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, (long)m->num_sms * 16);
   cudaStream_t st = (cudaStream_t)stream;
   if (m->dim == 2) chem_kernel<2, 5><<<grid, 256, 0, st>>>(u, s, m->d_mech, m->ne, m->nn);
   else chem_kernel<3, 5><<<grid, 256, 0, st>>>(u, s, m->d_mech, m->ne, m->nn);
@@ -722,7 +723,7 @@ extern "C" marut_status marut_chem_implicit(marut_mesh *m, double *u, double dt,
   int *d_sw = reinterpret_cast<int *>(m->d_red + 3);
   CUDA_TRY(cudaMemsetAsync(d_sw, 0, sizeof(unsigned long long), st));
   const long total = m->ne * m->nn;
-  const unsigned grid = (unsigned)std::min<long>((total + 127) / 128, 148L * 8);
+  const unsigned grid = (unsigned)std::min<long>((total + 127) / 128, (long)m->num_sms * 8);
   if (m->dim == 2) chem_implicit_kernel<2, 5><<<grid, 128, 0, st>>>(u, m->d_mech, dt, m->ne, m->nn, d_sw);
   else chem_implicit_kernel<3, 5><<<grid, 128, 0, st>>>(u, m->d_mech, dt, m->ne, m->nn, d_sw);
   cudaError_t e = cudaGetLastError();
@@ -756,7 +757,7 @@ extern "C" marut_status marut_set_boundary_kinds(marut_mesh *m, const int *kinds
     if (kinds[i] < MARUT_BC_PRESCRIBED || kinds[i] > MARUT_BC_SLIP_WALL) return fail(MARUT_EINVAL, "unknown boundary kind %d", kinds[i]);
     special = special || kinds[i] != MARUT_BC_PRESCRIBED;
   }
-  if (special && (m->physics != MARUT_EULER || m->kernel_sel != 0))
+  if (special && m->physics != MARUT_EULER)
     return fail(MARUT_EINVAL, "outflow / slip-wall faces are implemented for MARUT_EULER (default kernels) only");
   if (n_bc == 0) return MARUT_OK;
   int *d_k = nullptr;
@@ -764,7 +765,7 @@ extern "C" marut_status marut_set_boundary_kinds(marut_mesh *m, const int *kinds
   cudaError_t e = cudaMemcpy(d_k, kinds, n_bc * sizeof(int), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) {
     const long n = m->ne * 2 * m->dim;
-    patch_boundary_kinds_kernel<<<(unsigned)std::min<long>((n + 255) / 256, 148L * 8), 256>>>(m->d_conn, n, d_k);
+    patch_boundary_kinds_kernel<<<(unsigned)std::min<long>((n + 255) / 256, (long)m->num_sms * 8), 256>>>(m->d_conn, n, d_k);
     e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
   }
@@ -784,7 +785,7 @@ extern "C" marut_status marut_positivity_floor(marut_mesh *m, double *u, double 
   unsigned long long *d_cnt = m->d_red + 4;
   if (changed_out) CUDA_TRY(cudaMemsetAsync(d_cnt, 0, sizeof(unsigned long long), st));
   const long total = m->ne * m->nn;
-  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * 32);
+  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, (long)m->num_sms * 32);
   if (m->dim == 2) positivity_floor_kernel<2><<<grid, 256, 0, st>>>(u, m->gamma, rho_min, p_min, m->ne, m->nn, changed_out ? d_cnt : nullptr);
   else positivity_floor_kernel<3><<<grid, 256, 0, st>>>(u, m->gamma, rho_min, p_min, m->ne, m->nn, changed_out ? d_cnt : nullptr);
   cudaError_t e = cudaGetLastError();
@@ -876,14 +877,14 @@ extern "C" marut_status marut_shock_indicator(marut_mesh *m, const double *u, do
 template <int DIM, int NSP, int PHYS>
 static cudaError_t launch_wave_speed(marut_mesh *m, const double *u, const MechDev *mech, cudaStream_t st) {
   // one resident wave: grid = SMs x the CTAs per SM this instantiation's registers allow
-  static int occ = 0;
+  int &occ = m->ws_occ;   // per handle (= per device)
   if (occ == 0) {
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, wave_speed_kernel<DIM, NSP, PHYS>, 256, 0);
     if (e != cudaSuccess) return e;
     if (occ < 1) occ = 1;
   }
   const long total = m->ne * m->nn;
-  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * occ);
+  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, (long)m->num_sms * occ);
   wave_speed_kernel<DIM, NSP, PHYS><<<grid, 256, 0, st>>>(u, mech, m->gamma, m->mu, m->ne, m->nn, m->d_red);
   return cudaGetLastError();
 }
@@ -920,7 +921,7 @@ extern "C" marut_status marut_max_dt_async(marut_mesh *m, const double *u, doubl
   cudaStream_t st = (cudaStream_t)stream;
   CUDA_TRY(cudaMemsetAsync(m->d_red, 0, 3 * sizeof(unsigned long long), st));
   const long total = m->ne * m->nn;
-  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * 8);
+  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, (long)m->num_sms * 8);
   cudaError_t e = (m->dim == 2) ? run_wave_speed<2>(m, u, grid, st) : run_wave_speed<3>(m, u, grid, st);
   if (e != cudaSuccess) return fail(MARUT_ECUDA, "wave speed kernel: %s", cudaGetErrorString(e));
   dt_finalize_kernel<<<1, 1, 0, st>>>(m->d_red, cfl, m->dx_min, 2.0 * m->N + 1.0, m->Pr, m->physics == MARUT_NAVIER_STOKES ? 1 : 0, dt_dev);
@@ -936,7 +937,7 @@ extern "C" marut_status marut_max_dt(marut_mesh *m, const double *u, double cfl,
   cudaStream_t st = (cudaStream_t)stream;
   CUDA_TRY(cudaMemsetAsync(m->d_red, 0, 4 * sizeof(unsigned long long), st));
   const long total = m->ne * m->nn;
-  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, 148L * 8);
+  const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, (long)m->num_sms * 8);
   cudaError_t e = (m->dim == 2) ? run_wave_speed<2>(m, u, grid, st) : run_wave_speed<3>(m, u, grid, st);
   if (e != cudaSuccess) return fail(MARUT_ECUDA, "wave speed kernel: %s", cudaGetErrorString(e));
   m->launches++;
@@ -974,5 +975,5 @@ extern "C" marut_status marut_get_metrics(marut_mesh *m, double *Ja, double *J) 
 }
 extern "C" int marut_is_affine(const marut_mesh *m) { return m && m->affine ? 1 : 0; }
 extern "C" double marut_dx_min(const marut_mesh *m) { return m ? m->dx_min : 0.0; }
-extern "C" long marut_launch_count(const marut_mesh *m) { return m ? m->launches : 0; }
+extern "C" long marut_launch_count(const marut_mesh *m) { return m ? m->launches.load() : 0; }
 extern "C" const char *marut_last_error(void) { return g_err; }

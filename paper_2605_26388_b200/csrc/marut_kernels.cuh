@@ -1,6 +1,4 @@
-// marut_kernels.cuh -- the generic (any dim / degree / physics) kernels of the CUDA path:
-//   stage_kernel    : volume integral + interface/mortar/boundary flux + surface lift + 1/J
-//                     + source + SSP-RK33 combination, one pass over u
+// marut_kernels.cuh -- the per-node kernels of the CUDA path around the fused stage kernels:
 //   gradient_kernel : BR1 gradient S = grad W (a6)
 //   eos_kernel      : mixture temperature by Newton (a8)
 //   chem_kernel     : chemistry source alone (marut_chem_source)
@@ -65,212 +63,6 @@ template <int DIM, int NSP, int PHYS, bool WANT_A>
 __device__ __forceinline__ Prim<DIM> make_prim(const double *U, double T, double gamma, const MechDev *mech) {
   if constexpr (PHYS == PH_REACT) return prim_mixture<DIM, NSP, WANT_A>(U, T, *mech);
   else return prim_ideal<DIM, WANT_A>(U, gamma);
-}
-
-// ======================================================================================
-// fused stage kernel
-// ======================================================================================
-template <int DIM, int NP, int NSP, int PHYS, bool AFFINE, int EB>
-__global__ void __launch_bounds__(((EB * Geo<DIM, NP>::NN + 31) / 32) * 32)
-stage_kernel(const __grid_constant__ StageParams P) {
-  using G = Geo<DIM, NP>;
-  constexpr int NN = G::NN, NVAR = NSP + DIM + 1, NW = DIM + 2, MD = G::MD;
-  constexpr int TILE = EB * NN;
-  extern __shared__ double smem[];
-  double *Fsm = smem;                         // [DIM][NVAR][TILE] contravariant fluxes
-  double *Dsm = smem + DIM * NVAR * TILE;     // [NP*NP]
-  __shared__ MechDev mech_s;
-
-  const int tid = threadIdx.x;
-  for (int i = tid; i < NP * NP; i += blockDim.x) Dsm[i] = P.D[i];
-  if constexpr (PHYS == PH_REACT) {
-    const int *src = reinterpret_cast<const int *>(P.mech);
-    int *dst = reinterpret_cast<int *>(&mech_s);
-    for (int i = tid; i < (int)(sizeof(MechDev) / sizeof(int)); i += blockDim.x) dst[i] = src[i];
-    __syncthreads();
-  }
-  const MechDev *mech = (PHYS == PH_REACT) ? &mech_s : nullptr;
-
-  const int el = tid / NN, p = tid - el * NN;
-  const long e = (long)blockIdx.x * EB + el;
-  const bool active = (tid < TILE) && (e < P.ne);
-  int q[3] = {0, 0, 0};
-  G::ijk(p, q);
-
-  double U[NVAR], Ja[DIM * DIM], invJ = 0.0, T = 0.0, Sg[(PHYS == PH_NS) ? NW * DIM : 1];
-  Prim<DIM> pr;
-  if (active) {
-    const double *up = P.u_in + e * NVAR * NN + p;
-#pragma unroll
-    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
-#pragma unroll
-    for (int k = 0; k < DIM * DIM; ++k) Ja[k] = metric_at<DIM, NP, AFFINE>(P.metric, e, k, p);
-    invJ = metric_at<DIM, NP, AFFINE>(P.metric, e, DIM * DIM, p);
-    if constexpr (PHYS == PH_REACT) T = __ldg(&P.Taux[e * NN + p]);
-    pr = make_prim<DIM, NSP, PHYS, true>(U, T, P.gamma, mech);
-    if constexpr (PHYS == PH_NS) {
-#pragma unroll
-      for (int k = 0; k < Tau<DIM>::NTAU; ++k) Sg[k] = __ldg(&P.S[(e * Tau<DIM>::NTAU + k) * NN + p]);
-    }
-    // contravariant fluxes Ftilde^l = Ja^l . (F_inv - F_v)   (eq. 9)
-#pragma unroll
-    for (int l = 0; l < DIM; ++l) {
-      double F[NVAR];
-      flux_dot<DIM, NSP>(U, pr, &Ja[l * DIM], F);
-      if constexpr (PHYS == PH_NS) {
-        double Fv[NW];
-        viscous_flux_dot_tau<DIM>(pr.v, Sg, &Ja[l * DIM], Fv);
-#pragma unroll
-        for (int v = 0; v < NVAR; ++v) F[v] -= Fv[v];
-      }
-#pragma unroll
-      for (int v = 0; v < NVAR; ++v) Fsm[(l * NVAR + v) * TILE + tid] = F[v];
-    }
-  }
-  __syncthreads();
-  if (!active) return;
-
-  // ---- volume term: sum_l sum_m D[i_l][m] Ftilde^l(m)
-  double R[NVAR];
-#pragma unroll
-  for (int v = 0; v < NVAR; ++v) R[v] = 0.0;
-#pragma unroll
-  for (int l = 0; l < DIM; ++l) {
-    const int st = G::stride(l);
-    const int base = tid - q[l] * st;
-    double Drow[NP];
-#pragma unroll
-    for (int m = 0; m < NP; ++m) Drow[m] = Dsm[q[l] * NP + m];
-#pragma unroll
-    for (int v = 0; v < NVAR; ++v) {
-      const double *Fl = &Fsm[(l * NVAR + v) * TILE + base];
-      double acc = 0.0;
-#pragma unroll
-      for (int m = 0; m < NP; ++m) acc += Drow[m] * Fl[m * st];
-      R[v] += acc;
-    }
-  }
-
-  // ---- surface term: (1/w_b) sum_f (F* - Ftilde).n_ref   (eq. 12)
-#pragma unroll
-  for (int l = 0; l < DIM; ++l) {
-    if (q[l] != 0 && q[l] != NP - 1) continue;
-    const int side = (q[l] == 0) ? 0 : 1;
-    const int f = 2 * l + side;
-    const double sgn = side ? 1.0 : -1.0;
-    const int2 cn = __ldg(&P.conn[e * 2 * DIM + f]);
-    const int kind = cn.y & 3, fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7, sub = (cn.y >> 8) & 1;
-    double nv[DIM], Fown[NVAR], Fs[NVAR];
-#pragma unroll
-    for (int c = 0; c < DIM; ++c) nv[c] = sgn * Ja[l * DIM + c];
-    int a0, a1;
-    G::face_coords(q, l, a0, a1);
-    if (kind == FK_CONFORMING || kind == FK_BOUNDARY) {
-      double Up[NVAR], Tp = 0.0;
-      int pR = 0;
-      if (kind == FK_CONFORMING) {
-        int b0, b1;
-    partner_index<DIM, NP>(orient, a0, a1, b0, b1);
-        pR = G::face_node(fR, b0, b1);
-        const double *un = P.u_in + (long)cn.x * NVAR * NN + pR;
-#pragma unroll
-        for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
-        if constexpr (PHYS == PH_REACT) Tp = __ldg(&P.Taux[(long)cn.x * NN + pR]);
-      } else {
-#pragma unroll
-        for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(&P.bc_state[cn.x * NVAR + v]);
-      }
-      const Prim<DIM> qp = make_prim<DIM, NSP, PHYS, true>(Up, Tp, P.gamma, mech);
-      double Fm[NVAR];
-      flux_dot<DIM, NSP>(U, pr, nv, Fm);
-      rusanov<DIM, NSP>(U, pr, Fm, Up, qp, nv, Fs);
-      if constexpr (PHYS == PH_NS) {
-        // BR1 viscous interface flux: mean of the two sides (eq. 16)
-        double Sp[NW * DIM], Fvm[NW], Fvp[NW];
-#pragma unroll
-        for (int k = 0; k < Tau<DIM>::NTAU; ++k) Sp[k] = __ldg(&P.S[((long)cn.x * Tau<DIM>::NTAU + k) * NN + pR]);
-        viscous_flux_dot_tau<DIM>(pr.v, Sg, nv, Fvm);
-        viscous_flux_dot_tau<DIM>(qp.v, Sp, nv, Fvp);
-#pragma unroll
-        for (int v = 0; v < NVAR; ++v) Fs[v] -= 0.5 * (Fvm[v] + Fvp[v]);
-      }
-    } else if constexpr (DIM == 2) {
-      const double *Pf = P.mortar_mat, *Prv = P.mortar_mat + 2 * NP * NP;
-      if (kind == FK_MORTAR_FINE) {
-        // exterior state = coarse trace interpolated to this half of the coarse face
-        double Up[NVAR];
-#pragma unroll
-        for (int v = 0; v < NVAR; ++v) Up[v] = 0.0;
-        for (int j = 0; j < NP; ++j) {
-          const double w = __ldg(&Pf[(sub * NP + a0) * NP + j]);
-          const double *uc = P.u_in + (long)cn.x * NVAR * NN + G::face_node(fR, j, 0);
-#pragma unroll
-          for (int v = 0; v < NVAR; ++v) Up[v] += w * __ldg(uc + v * NN);
-        }
-        const Prim<DIM> qp = make_prim<DIM, NSP, PHYS, true>(Up, 0.0, P.gamma, mech);
-        double Fm[NVAR];
-        flux_dot<DIM, NSP>(U, pr, nv, Fm);
-        rusanov<DIM, NSP>(U, pr, Fm, Up, qp, nv, Fs);
-      } else {
-        // coarse side: Riemann problem on both mortars with the fine-side normal, projected back with
-        // the area factor 2:  F*_C = sum_m P_rev^m (2 * (-F*_m))
-#pragma unroll
-        for (int v = 0; v < NVAR; ++v) Fs[v] = 0.0;
-        for (int m = 0; m < 2; ++m) {
-          const long eF = __ldg(&P.mortar_fine[cn.x * 2 + m]);
-          const int lF = fR >> 1;
-          const double sF = (fR & 1) ? 1.0 : -1.0;
-          for (int a = 0; a < NP; ++a) {
-            const int pF = G::face_node(fR, a, 0);
-            double UF[NVAR], UC[NVAR], nF[DIM], FmF[NVAR], Fsm_[NVAR];
-#pragma unroll
-            for (int v = 0; v < NVAR; ++v) {
-              UF[v] = __ldg(P.u_in + (eF * NVAR + v) * NN + pF);
-              UC[v] = 0.0;
-            }
-            for (int j = 0; j < NP; ++j) {
-              const double w = __ldg(&Pf[(m * NP + a) * NP + j]);
-              const double *uc = P.u_in + e * NVAR * NN + G::face_node(f, j, 0);
-#pragma unroll
-              for (int v = 0; v < NVAR; ++v) UC[v] += w * __ldg(uc + v * NN);
-            }
-#pragma unroll
-            for (int c = 0; c < DIM; ++c) nF[c] = sF * metric_at<DIM, NP, AFFINE>(P.metric, eF, lF * DIM + c, pF);
-            const Prim<DIM> qF = make_prim<DIM, NSP, PHYS, true>(UF, 0.0, P.gamma, mech);
-            const Prim<DIM> qC = make_prim<DIM, NSP, PHYS, true>(UC, 0.0, P.gamma, mech);
-            flux_dot<DIM, NSP>(UF, qF, nF, FmF);
-            rusanov<DIM, NSP>(UF, qF, FmF, UC, qC, nF, Fsm_);
-            const double w2 = -2.0 * __ldg(&Prv[(m * NP + a0) * NP + a]);
-#pragma unroll
-            for (int v = 0; v < NVAR; ++v) Fs[v] += w2 * Fsm_[v];
-          }
-        }
-      }
-    }
-#pragma unroll
-    for (int v = 0; v < NVAR; ++v) {
-      Fown[v] = sgn * Fsm[(l * NVAR + v) * TILE + tid];
-      R[v] += P.inv_wb * (Fs[v] - Fown[v]);
-    }
-  }
-
-  // ---- 1/J, source, SSP-RK combination (eq. 45)
-  double src[NVAR];
-#pragma unroll
-  for (int v = 0; v < NVAR; ++v) src[v] = 0.0;
-  if constexpr (PHYS == PH_REACT) {
-    if (P.explicit_source) production_rates<NSP>(*mech, T, U, src);
-  }
-  double *op = P.u_out + e * NVAR * NN + p;
-  if (P.ca != 0.0) {
-    const double *np_ = P.u_n + e * NVAR * NN + p;
-#pragma unroll
-    for (int v = 0; v < NVAR; ++v)
-      op[v * NN] = P.ca * np_[v * NN] + (P.cb * U[v] + stage_cc(P) * (src[v] - invJ * R[v]));
-  } else {
-#pragma unroll
-    for (int v = 0; v < NVAR; ++v) op[v * NN] = P.cb * U[v] + stage_cc(P) * (src[v] - invJ * R[v]);
-  }
 }
 
 // ======================================================================================
@@ -856,23 +648,6 @@ __global__ void fnorm_kernel(const double *__restrict__ metric_el, double *__res
 template <int NN>
 constexpr int elems_per_block() { return (256 / NN) < 1 ? 1 : 256 / NN; }
 
-template <int DIM, int NP, int NSP, int PHYS, bool AFFINE>
-cudaError_t launch_stage_t(const StageParams &P, cudaStream_t st) {
-  constexpr int NN = Geo<DIM, NP>::NN, EB = elems_per_block<NN>();
-  constexpr int threads = ((EB * NN + 31) / 32) * 32;
-  constexpr size_t smem = (size_t)(DIM * (NSP + DIM + 1) * EB * NN + NP * NP) * sizeof(double);
-  auto k = stage_kernel<DIM, NP, NSP, PHYS, AFFINE, EB>;
-  static bool attr = false;
-  if (!attr) {
-    cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    attr = true;
-  }
-  const long grid = (P.ne + EB - 1) / EB;
-  k<<<(unsigned)grid, threads, smem, st>>>(P);
-  return cudaGetLastError();
-}
-
 template <int DIM, int NP, bool AFFINE, bool ORIENT3 = false>
 cudaError_t launch_gradient_t(const GradParams &P, cudaStream_t st) {
   if constexpr (DIM == 3 && !ORIENT3) {
@@ -882,12 +657,8 @@ cudaError_t launch_gradient_t(const GradParams &P, cudaStream_t st) {
   constexpr int threads = ((EB * NN + 31) / 32) * 32;
   constexpr size_t smem = (size_t)((DIM + 2) * EB * NN + NP * NP) * sizeof(double);
   auto k = gradient_kernel<DIM, NP, AFFINE, EB, ORIENT3>;
-  static bool attr = false;
-  if (!attr) {
-    cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    attr = true;
-  }
+  static std::atomic<unsigned long long> attr_done{0};
+  if (cudaError_t err = set_smem_once((const void *)k, smem, attr_done); err != cudaSuccess) return err;
   const long grid = (P.ne + EB - 1) / EB;
   k<<<(unsigned)grid, threads, smem, st>>>(P);
   return cudaGetLastError();

@@ -5,17 +5,12 @@
 
 namespace marut {
 struct GradParams;
-cudaError_t launch_stage_euler2d(int np, bool affine, const StageParams &P, cudaStream_t st);
-cudaError_t launch_stage_euler3d(int np, bool affine, const StageParams &P, cudaStream_t st);
-cudaError_t launch_stage_line2d(int np, bool affine, const StageParams &P, cudaStream_t st);
-cudaError_t launch_stage_line3d(int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_stage_node2d(int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_stage_node3d(int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_mortar_flux3d(int np, const double *u, const double *metric, const int *info, const int *fine, const double *mat,
                                  double gamma, double *mflux, long n_mortar, cudaStream_t st);
-cudaError_t launch_stage_line2_3d(int np, const StageParams &P, cudaStream_t st);
 cudaError_t launch_stage_split(int dim, int np, bool affine, const StageParams &P, cudaStream_t st);
-cudaError_t launch_stage_ns(int dim, int np, bool affine, bool generic, const StageParams &P, cudaStream_t st);
+cudaError_t launch_stage_ns(int dim, int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_gradient(int dim, int np, bool affine, const GradParams &P, cudaStream_t st);
-cudaError_t launch_stage_react(int dim, int np, int nsp, bool affine, bool generic, const StageParams &P, cudaStream_t st);
+cudaError_t launch_stage_react(int dim, int np, int nsp, bool affine, const StageParams &P, cudaStream_t st);
 }  // namespace marut

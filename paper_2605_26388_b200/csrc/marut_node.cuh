@@ -371,22 +371,10 @@ __device__ __forceinline__ void line_deriv(const StageParams &P, const double *f
   }
 }
 
-// ---- compile-time switches of the node kernel; the defaults are the measured best (profiles/r01_c2_stage.md)
-#ifndef MARUT_L2_PREFETCH
-#define MARUT_L2_PREFETCH 1024   // L2 bulk prefetch of the tile this many CTAs ahead; 0 = off            (on: -3 %)
-#endif
-#ifndef MARUT_PREFETCH_UN
-#define MARUT_PREFETCH_UN 0      // 1: load u_n of the last-pass task at kernel start                      (+8 %)
-#endif
-#ifndef MARUT_EARLY_GATHER
-#define MARUT_EARLY_GATHER 0     // 1: issue the neighbour gather before the flux arithmetic of phase N    (+4 %)
-#endif
-#ifndef MARUT_ABLATE
-#define MARUT_ABLATE 0           // timing ablations only (results are not physics): 1 no face tasks, 2 no xi/eta
-#endif                           // passes, 3 data-movement skeleton
-#ifndef MARUT_NODE_MINB128
-#define MARUT_NODE_MINB128 6     // CTAs of 128 threads per SM the register allocation is sized for (5..7: same speed)
-#endif
+// L2 bulk prefetch of the tile this many CTAs ahead (measured: -3 % on c2) and the CTAs of 128 threads per SM the
+// register allocation is sized for
+constexpr int NODE_L2_PREFETCH = 1024;
+constexpr int NODE_MINB128 = 6;
 // last-pass task t -> (element in tile, variable, line): 3-D: ij = i + NP*j, lanes run over ij first;
 // 2-D: ij = i, lane order (i, element, v)
 template <int DIM, int NP>
@@ -432,18 +420,16 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   const int nel = (int)((P.ne - e0 < EB) ? (P.ne - e0) : EB);
   const int ntask = nel * NFN, nline = nel * NLT;
 
-#if MARUT_L2_PREFETCH
   // L2 prefetch of the tile a CTA launched ~one wave later will read (u_in and u_n): turns its DRAM latency into an
   // L2 hit.  Bulk prefetch needs 16-byte alignment and size: round outwards, stay inside the array.
   if (tid == 0) {
-    const long ep = e0 + (long)MARUT_L2_PREFETCH * EB;
+    const long ep = e0 + (long)NODE_L2_PREFETCH * EB;
     if (ep + EB < P.ne) {
       const size_t bytes = (size_t)EB * NVAR * NN * sizeof(double);
       l2_prefetch(P.u_in + ep * NVAR * NN, bytes);
       if (P.ca != 0.0) l2_prefetch(P.u_n + ep * NVAR * NN, bytes);
     }
   }
-#endif
   // first face task of this thread: connectivity load issued first (the neighbour gather depends on it)
   const bool has0 = tid < ntask;
   const FaceTask t0 = decode_task<DIM, NP>(has0 ? tid : 0);
@@ -457,19 +443,7 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
     }
   }
 
-  // u_n of the degrees of freedom this thread finishes in the last pass: loaded now, so that the CTA has its
-  // whole DRAM read in flight from the start (u_out may alias u_n: only this thread writes these locations, later)
   const bool use_un = (P.ca != 0.0);
-  double un0[NP];
-  {
-    int el, v, ij;
-    last_pass_task<DIM, NP, NVAR, EB>(tid, el, v, ij);
-    if (MARUT_PREFETCH_UN && use_un && el < nel && v < NVAR) {
-      const long gofs = ((e0 + el) * NVAR + v) * NN + ij;
-#pragma unroll
-      for (int m = 0; m < NP; ++m) un0[m] = P.u_n[gofs + m * ((DIM == 3) ? NP * NP : NP)];
-    }
-  }
   // neighbour trace of the first face task: issued in phase N, consumed after the xi pass
   double Up0[NVAR];
   // ---- phase N: own node
@@ -483,28 +457,17 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
     }
-#if MARUT_EARLY_GATHER
-    if (has0) gather_exterior<DIM, NP, NVAR>(P, t0, cn0, Up0);
-#endif
     if (active) {
       const int qk = (DIM == 3) ? p / (NP * NP) : 0;
       const int sp = p + (KS - NP * NP) * qk;   // node offset inside a flux plane
       double Ja[DIM * DIM];
 #pragma unroll
       for (int k = 0; k < DIM * DIM; ++k) Ja[k] = metric_at<DIM, NP, AFFINE>(P.metric, e, k, p);
-#if MARUT_ABLATE == 3
-      Prim<DIM> pr; pr.irho = U[0]; pr.p = U[1]; pr.a = U[2];
-#else
       const Prim<DIM> pr = prim_ideal<DIM, true>(U, P.gamma);
-#endif
 #pragma unroll
       for (int l = 0; l < DIM; ++l) {
         double F[NVAR];
-#if MARUT_ABLATE == 3
-        for (int v = 0; v < NVAR; ++v) F[v] = U[v] * Ja[l * DIM];
-#else
         flux_dot<DIM, 1>(U, pr, &Ja[l * DIM], F);
-#endif
 #pragma unroll
         for (int v = 0; v < NVAR; ++v) Fsm[(l * NVAR * EB + C::plane(v, el)) * PS + sp] = F[v];
       }
@@ -515,15 +478,10 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
       Ust[(NVAR + 2) * TILE + tid] = pr.a;
     }
   }
-#if !MARUT_EARLY_GATHER
   if (has0) gather_exterior<DIM, NP, NVAR>(P, t0, cn0, Up0);
-#endif
   __syncthreads();
 
   // ---- xi pass (eq. 9): lines (j,k) of variable v; lanes run over the lines first
-#if MARUT_ABLATE == 2 || MARUT_ABLATE == 3
-  if (false)
-#endif
   for (int t = tid; t < EB * NLT; t += NT) {
     int el, v, lj, lk = 0;
     if constexpr (DIM == 3) {
@@ -549,18 +507,11 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
   }
 
   // ---- face phase, first round: face nodes densely mapped
-#if MARUT_ABLATE != 1 && MARUT_ABLATE != 3
   if (has0) euler_face_task<DIM, NP, AFFINE, EB, BCK>(P, Ust, Msm, Lft, e0, tid, t0, cn0, Up0);
-#else
-  if (has0 && Up0[0] == 1.2345) Lft[tid] = Up0[1];
-#endif
   __syncthreads();
 
   if constexpr (DIM == 3) {
     // ---- eta pass: lines (i,k) of variable v; lane order (k, v, i) is bank-conflict-free
-#if MARUT_ABLATE == 2 || MARUT_ABLATE == 3
-    if (false)
-#endif
     for (int t = tid; t < nline; t += NT) {
       const int el = t / NLT, r = t - el * NLT;
       const int lk = r % NP, r2 = r / NP;
@@ -576,9 +527,6 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
     }
   }
   // ---- face phase, remaining rounds
-#if MARUT_ABLATE == 1 || MARUT_ABLATE == 3
-  if (false)
-#endif
   for (int g = tid + NT; g < ntask; g += NT) {
     const FaceTask t = decode_task<DIM, NP>(g);
     const int2 cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
@@ -601,13 +549,8 @@ stage_node_kernel(const __grid_constant__ StageParams P) {
     const long gofs = (e * NVAR + v) * NN + ij;
     double un[NP];
     if (use_un) {
-      if (MARUT_PREFETCH_UN && t == tid) {
 #pragma unroll
-        for (int m = 0; m < NP; ++m) un[m] = un0[m];
-      } else {
-#pragma unroll
-        for (int m = 0; m < NP; ++m) un[m] = P.u_n[gofs + m * GS];
-      }
+      for (int m = 0; m < NP; ++m) un[m] = P.u_n[gofs + m * GS];
     }
     double f[NP], acc[NP];
 #pragma unroll
@@ -662,14 +605,10 @@ cudaError_t launch_stage_node_t(const StageParams &P, cudaStream_t st) {
   constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
   using C = NodeCfg<DIM, NP, 1, EB>;
   constexpr size_t smem = C::smem_doubles(AFFINE) * sizeof(double);
-  constexpr int MINB = (C::NT <= 128) ? MARUT_NODE_MINB128 : ((C::NT <= 256) ? 3 : 1);
+  constexpr int MINB = (C::NT <= 128) ? NODE_MINB128 : ((C::NT <= 256) ? 3 : 1);
   auto k = stage_node_kernel<DIM, NP, AFFINE, EB, MINB, BCK>;
-  static bool attr = false;
-  if (!attr) {
-    cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    attr = true;
-  }
+  static std::atomic<unsigned long long> attr_done{0};
+  if (cudaError_t err = set_smem_once((const void *)k, smem, attr_done); err != cudaSuccess) return err;
   const long grid = (P.ne + EB - 1) / EB;
   k<<<(unsigned)grid, C::NT, smem, st>>>(P);
   return cudaGetLastError();

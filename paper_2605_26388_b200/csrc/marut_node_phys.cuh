@@ -330,12 +330,8 @@ cudaError_t launch_stage_phys_t(const StageParams &P, cudaStream_t st) {
   constexpr size_t smem = C::smem_doubles(AFFINE) * sizeof(double);
   constexpr int MINB = (PHYS == PH_REACT) ? ((C::NT <= 128) ? 3 : 1) : ((C::NT <= 128) ? MARUT_PHYS_MINB128 : ((C::NT <= 256) ? 2 : 1));
   auto k = stage_phys_kernel<DIM, NP, NSP, PHYS, AFFINE, EB, MINB>;
-  static bool attr = false;
-  if (!attr) {
-    cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    attr = true;
-  }
+  static std::atomic<unsigned long long> attr_done{0};
+  if (cudaError_t err = set_smem_once((const void *)k, smem, attr_done); err != cudaSuccess) return err;
   const long grid = (P.ne + EB - 1) / EB;
   k<<<(unsigned)grid, C::NT, smem, st>>>(P);
   return cudaGetLastError();

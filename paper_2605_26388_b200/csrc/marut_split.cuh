@@ -332,12 +332,8 @@ cudaError_t launch_stage_split_t(const StageParams &P, cudaStream_t st) {
   constexpr size_t smem = ((size_t)(C::NST + 3 + DIM + DIM * (NP / 2) * C::NVAR) * C::TILE + (size_t)C::NVAR * C::LFS + (AFFINE ? EB * C::MDP : 0)) * sizeof(double);
   constexpr int MINB = (C::NT <= 128) ? 4 : ((C::NT <= 256) ? 2 : 1);
   auto k = stage_split_kernel<DIM, NP, AFFINE, EB, MINB, BCK>;
-  static bool attr = false;
-  if (!attr) {
-    cudaError_t err = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    attr = true;
-  }
+  static std::atomic<unsigned long long> attr_done{0};
+  if (cudaError_t err = set_smem_once((const void *)k, smem, attr_done); err != cudaSuccess) return err;
   const long grid = (P.ne + EB - 1) / EB;
   k<<<(unsigned)grid, C::NT, smem, st>>>(P);
   return cudaGetLastError();

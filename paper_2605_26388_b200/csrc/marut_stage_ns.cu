@@ -3,8 +3,7 @@
 #include "marut_launch.h"
 namespace marut {
 template <int DIM, int NP>
-static cudaError_t go(bool affine, bool generic, const StageParams &P, cudaStream_t st) {
-  if (generic) return affine ? launch_stage_t<DIM, NP, 1, PH_NS, true>(P, st) : launch_stage_t<DIM, NP, 1, PH_NS, false>(P, st);
+static cudaError_t go(bool affine, const StageParams &P, cudaStream_t st) {
   return affine ? launch_stage_phys_t<DIM, NP, 1, PH_NS, true>(P, st) : launch_stage_phys_t<DIM, NP, 1, PH_NS, false>(P, st);
 }
 template <int DIM, int NP>
@@ -27,8 +26,8 @@ static cudaError_t gr(bool affine, const GradParams &P, cudaStream_t st) {
       case 6: return FN<3, 6>(__VA_ARGS__);                       \
     }                                                             \
   return cudaErrorNotSupported;
-cudaError_t launch_stage_ns(int dim, int np, bool affine, bool generic, const StageParams &P, cudaStream_t st) {
-  MARUT_NS_CASES(go, affine, generic, P, st)
+cudaError_t launch_stage_ns(int dim, int np, bool affine, const StageParams &P, cudaStream_t st) {
+  MARUT_NS_CASES(go, affine, P, st)
 }
 cudaError_t launch_gradient(int dim, int np, bool affine, const GradParams &P, cudaStream_t st) {
   MARUT_NS_CASES(gr, affine, P, st)
