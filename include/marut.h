@@ -220,6 +220,18 @@ double marut_dx_min(const marut_mesh *mesh);
 /* number of kernel launches issued through this handle so far (bench.py's gpu_launches) */
 long marut_launch_count(const marut_mesh *mesh);
 
+/* Euler strong-form stage on affine meshes: which of the two stage kernels runs.  0 (default): the line kernel
+ * (csrc/marut_pencil.cuh) when the mesh has enough elements to fill the device with its tiles, else the thread-per-node
+ * kernel (csrc/marut_node.cuh); 1: always the thread-per-node kernel; 2: the line kernel whenever the mesh kind allows
+ * it, whatever its size.  Both kernels compute the same operator; the parity tests use 1 / 2 to cover both on small
+ * meshes.  No effect on other physics / volume forms. */
+marut_status marut_debug_stage_kernel(marut_mesh *mesh, int which);
+
+/* the kernels' branch-free 1/x and sqrt(x) for positive normal-range operands (csrc/marut_common.cuh) evaluated on n
+ * DEVICE doubles x -> rcp, sq (DEVICE, n doubles each); the tests compare them bit for bit with IEEE division and
+ * square root.  Asynchronous on the stream. */
+marut_status marut_debug_rcp_sqrt(const double *x, double *rcp, double *sq, long n, void *cuda_stream);
+
 const char *marut_last_error(void);
 
 #ifdef __cplusplus

@@ -15,7 +15,7 @@ _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA"
 
 # every symbol include/marut.h declares
 SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt", "marut_max_dt_async", "marut_ssprk_stage_dev", "marut_rk_stage_dev",
-           "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_rk_stage", "marut_lincomb", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count",
+           "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_rk_stage", "marut_lincomb", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count", "marut_debug_rcp_sqrt", "marut_debug_stage_kernel",
            "marut_last_error"]
 
 
@@ -96,6 +96,10 @@ def lib():
         L.marut_dx_min.argtypes = [vp]
         L.marut_launch_count.restype = C.c_long
         L.marut_launch_count.argtypes = [vp]
+        L.marut_debug_stage_kernel.restype = C.c_int
+        L.marut_debug_stage_kernel.argtypes = [vp, C.c_int]
+        L.marut_debug_rcp_sqrt.restype = C.c_int
+        L.marut_debug_rcp_sqrt.argtypes = [vp, vp, vp, C.c_long, vp]
         L.marut_last_error.restype = C.c_char_p
         _lib = L
     return _lib
@@ -267,6 +271,10 @@ def marut_set_blend(h, alpha):
     _check(lib().marut_set_blend(h, None if alpha is None else _dev(alpha)))
 
 
+def marut_debug_rcp_sqrt(x, rcp, sq, stream=None):
+    _check(lib().marut_debug_rcp_sqrt(_dev(x), _dev(rcp), _dev(sq), x.numel(), _stream(stream)))
+
+
 def marut_set_explicit_source(h, on):
     _check(lib().marut_set_explicit_source(h, int(bool(on))))
 
@@ -371,6 +379,9 @@ class MarutMesh:
     @property
     def dx_min(self):
         return lib().marut_dx_min(self.h)
+
+    def debug_stage_kernel(self, which):
+        _check(lib().marut_debug_stage_kernel(self.h, which))
 
     @property
     def launch_count(self):

@@ -65,6 +65,7 @@ struct marut_mesh {
   unsigned long long *d_red = nullptr;
   unsigned long long *h_red = nullptr;  // pinned
   std::atomic<long> launches{0};   // kernels launched through this handle (introspection; any thread)
+  int stage_kernel_pref = 0;       // marut_debug_stage_kernel: 0 automatic, 1 thread-per-node kernel, 2 line kernel where eligible
   int ws_occ = 0;                  // resident CTAs per SM of this handle's wave_speed_kernel (queried on first use)
   int device = 0, num_sms = 148;   // the device the handle was created on and its multiprocessor count
 };
@@ -536,7 +537,15 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   switch (m->physics) {
     case MARUT_EULER:
       if (m->volume_form == MARUT_VOLUME_SPLIT_RANOCHA) e = launch_stage_split(m->dim, m->np, m->affine, P, st);
-      else e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
+      else {
+        // affine meshes with conforming / prescribed-state / 2-D mortar faces: the persistent TMA-fed line kernel;
+        // curved meshes, outflow / slip-wall faces and 3-D mortars: the thread-per-node kernel
+        e = cudaErrorNotSupported;
+        if (m->affine && !P.bc_kinds && m->stage_kernel_pref != 1)
+          e = launch_stage_pencil(m->dim, m->np, m->n_mortar > 0, m->stage_kernel_pref == 2, P, st);
+        if (e == cudaErrorNotSupported)
+          e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
+      }
       break;
     case MARUT_NAVIER_STOKES: e = launch_stage_ns(m->dim, m->np, m->affine, P, st); break;
     default: e = launch_stage_react(m->dim, m->np, m->nsp, m->affine, P, st); break;
@@ -976,4 +985,22 @@ extern "C" marut_status marut_get_metrics(marut_mesh *m, double *Ja, double *J) 
 extern "C" int marut_is_affine(const marut_mesh *m) { return m && m->affine ? 1 : 0; }
 extern "C" double marut_dx_min(const marut_mesh *m) { return m ? m->dx_min : 0.0; }
 extern "C" long marut_launch_count(const marut_mesh *m) { return m ? m->launches.load() : 0; }
+extern "C" marut_status marut_debug_stage_kernel(marut_mesh *m, int which) {
+  if (!m || which < 0 || which > 2) return fail(MARUT_EINVAL, "bad argument");
+  m->stage_kernel_pref = which;
+  return MARUT_OK;
+}
+__global__ void debug_rcp_sqrt_kernel(const double *__restrict__ x, double *__restrict__ r, double *__restrict__ s, long n) {
+  for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
+    r[i] = rcp_pos(x[i]);
+    s[i] = sqrt_pos(x[i]);
+  }
+}
+extern "C" marut_status marut_debug_rcp_sqrt(const double *x, double *rcp, double *sq, long n, void *stream) {
+  if (!x || !rcp || !sq || n < 0) return fail(MARUT_EINVAL, "bad argument");
+  if (n == 0) return MARUT_OK;
+  debug_rcp_sqrt_kernel<<<(unsigned)std::min<long>((n + 255) / 256, 148L * 8), 256, 0, (cudaStream_t)stream>>>(x, rcp, sq, n);
+  CUDA_TRY(cudaGetLastError());
+  return MARUT_OK;
+}
 extern "C" const char *marut_last_error(void) { return g_err; }

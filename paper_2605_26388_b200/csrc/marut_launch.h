@@ -5,6 +5,8 @@
 
 namespace marut {
 struct GradParams;
+// marut_pencil.cuh: Euler, strong form, affine meshes (mortar: the 2-D instantiation that knows 2:1 mortar faces)
+cudaError_t launch_stage_pencil(int dim, int np, bool mortar, bool force, const StageParams &P, cudaStream_t st);
 cudaError_t launch_stage_node2d(int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_stage_node3d(int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_mortar_flux3d(int np, const double *u, const double *metric, const int *info, const int *fine, const double *mat,

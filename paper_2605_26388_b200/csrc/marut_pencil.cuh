@@ -1,0 +1,390 @@
+// marut_pencil.cuh -- the fused stage kernel of compressible Euler on affine meshes: persistent
+// CTAs, element tiles brought in by TMA bulk copies two tiles ahead (cp.async.bulk + mbarrier), one thread per LINE of
+// n nodes with all variables of the line in registers.
+//
+//   tile   = ET consecutive elements, ET * n^(d-1) <= 128 lines per direction: one line per thread.  The tile's u_in
+//            block is contiguous in global memory ([e][v][node]): ONE bulk copy per tile into a two-deep ring; thread 0
+//            issues the copy for the tile after next when the current tile is finished.  N = 4 in 3-D has 5000-byte
+//            elements: the 16-byte window the copy needs is obtained by starting one double early (`shift`).
+//            The tile's connectivity and metric terms come in by 8-byte cp.async one tile ahead; u_n of the tile is
+//            L2-prefetched (cp.async.bulk.prefetch.L2) after the first phase, two phases before it is read.
+//   phase l (l = 0 .. d-1): the thread owns the line of direction l through (a0, a1): it reads the line's U from the
+//            tile, evaluates the contravariant flux Ftilde^l (eq. 9) at its n nodes, applies D along the line in
+//            registers, and -- because the line's two end nodes ARE the face nodes (a0, a1) of faces 2l and 2l+1 --
+//            evaluates both Rusanov lifts (eq. 12) from registers: no stash, no lift buffer, no divergence.
+//            Exterior traces: from the tile itself when the neighbour is one of the tile's elements, else gathered from
+//            global memory (L2); issued at the start of the phase, consumed at its end.
+//            The partial residual goes through one shared buffer R: phase 0 writes, phase 1 adds, the last phase
+//            adds, applies 1/J and the SSP-RK combination (eq. 45) and writes u_out (zeta lines: coalesced).
+//   Per node: 15 shared loads of U and 20 accesses of R, against ~115 shared accesses of the thread-per-node kernel;
+//   3 CTA barriers per tile; 1.0/x and sqrt(x) are evaluated by the branch-free sequences of marut_common.cuh.
+//
+// Selected for MARUT_EULER with the strong form on affine meshes without outflow / slip-wall faces and without 3-D
+// mortars (those run stage_node_kernel).  PAPER.md:179-204, 713-725; R4-R8, R10.
+// Product code; shares nothing with oracle/.
+#pragma once
+#include "marut_node.cuh"
+
+namespace marut {
+
+// ---------------------------------------------------------------- PTX wrappers (sm_100a)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void bulk_load(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst_smem)),
+               "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void bulk_prefetch_l2(const void *src_gmem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src_gmem), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void *dst_smem, const void *src_gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// ---------------------------------------------------------------- compile-time geometry
+template <int DIM, int NP>
+struct PencilCfg {
+  static constexpr int NVAR = DIM + 2;
+  static constexpr int NN = Geo<DIM, NP>::NN;
+  static constexpr int NL = Geo<DIM, NP>::NF;        // lines per element and direction
+  static constexpr int NT = 128;                     // threads per CTA
+  static constexpr int ET = NT / NL;                 // elements per tile
+  static constexpr int ED = NVAR * NN;               // doubles per element
+  static constexpr int TD = ET * ED;                 // doubles per tile
+  static constexpr int UB = (TD + 3) & ~1;           // ring slot: tile + the alignment window, itself 16-byte aligned
+  // per-tile metadata, prefetched one tile ahead: conn[ET][2d] (int2), metric[ET][d*d+1], fnorm[ET][d]
+  static constexpr int NCN = ET * 2 * DIM, NMT = ET * (DIM * DIM + 1), NFN = ET * DIM;
+  static constexpr int MW = NCN + NMT + NFN;         // 8-byte words of one metadata slot
+  static constexpr size_t smem_bytes = (size_t)(2 * UB + TD + 2 * MW) * sizeof(double) + 2 * sizeof(uint64_t);
+  static_assert(ET >= 1, "a direction's lines of one element must fit one CTA");
+  // CTAs per SM the shared memory allows (228 KB per SM, 1 KB reserved per CTA), at most 3
+  static constexpr int MINB = (233472 / (int)(smem_bytes + 1024)) >= 3 ? 3 : ((233472 / (int)(smem_bytes + 1024)) >= 2 ? 2 : 1);
+};
+
+// exterior state of face node (a0, a1) across the face described by cn: a conforming neighbour's trace (from the tile
+// in shared memory when the neighbour is one of its elements, else from global memory) or a prescribed boundary state
+template <int DIM, int NP>
+__device__ __forceinline__ void pencil_gather(const StageParams &P, int2 cn, int a0, int a1, const double *__restrict__ Ut,
+                                              long e0, int nel, double *Up) {
+  constexpr int NVAR = DIM + 2, NN = Geo<DIM, NP>::NN;
+  const int kind = cn.y & 3;
+  if (kind == FK_CONFORMING) {
+    const int fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7;
+    int b0, b1;
+    partner_index<DIM, NP>(orient, a0, a1, b0, b1);
+    const int node = face_node_of<DIM, NP>(fR, b0, b1);
+    const long de = (long)cn.x - e0;
+    if (de >= 0 && de < nel) {
+      const double *us = Ut + (int)de * NVAR * NN + node;
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Up[v] = us[v * NN];
+    } else {
+      const double *un = P.u_in + (long)cn.x * NVAR * NN + node;
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
+    }
+  } else if (kind == FK_BOUNDARY) {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(&P.bc_state[cn.x * NVAR + v]);
+  } else {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Up[v] = 1.0;   // mortar faces: F* comes from node_mortar_flux_2d
+  }
+}
+
+// scalars of one face node that the per-variable lift needs (Rusanov with the scaled normal sgn * Ja^l; R5)
+struct PencilFace {
+  double hl;        // 1/2 lambda |n|
+  double vnp, pp;   // exterior contravariant velocity Ja^l . v+ and pressure
+  double mnp;       // Ja^l . m+
+};
+template <int DIM>
+__device__ __forceinline__ PencilFace pencil_face(const double *Up, const double *Ja, double nrm, double gamma, double vnm,
+                                                  double pm, double rinvm) {
+  PencilFace F;
+  const double rinvp = rcp_pos(Up[0]);
+  double mnp = 0.0, kep = 0.0;
+#pragma unroll
+  for (int c = 0; c < DIM; ++c) {
+    mnp += Up[1 + c] * Ja[c];
+    kep += Up[1 + c] * Up[1 + c];
+  }
+  F.mnp = mnp;
+  F.pp = (gamma - 1.0) * (Up[DIM + 1] - 0.5 * kep * rinvp);
+  F.vnp = mnp * rinvp;
+  const double ap = sqrt_pos(gamma * F.pp * rinvp), am = sqrt_pos(gamma * pm * rinvm);
+  F.hl = 0.5 * fmax(fabs(vnm) + am * nrm, fabs(F.vnp) + ap * nrm);
+  return F;
+}
+// contravariant flux component v of a state (for the exterior side of a face)
+template <int DIM>
+__device__ __forceinline__ double pencil_flux_comp(int v, const double *Up, const PencilFace &F, const double *Ja) {
+  if (v == 0) return F.mnp;
+  if (v == DIM + 1) return (Up[DIM + 1] + F.pp) * F.vnp;
+  return Up[v] * F.vnp + F.pp * Ja[v - 1];
+}
+
+// One phase of one line.  L = direction, FIRST / LAST = position of the phase in the element's sequence.
+// Ut: the tile; Rs: partial residual; Md: the tile's metadata slot: conn (int2) | metric | fnorm.
+template <int DIM, int NP, int L, bool MORTAR>
+__device__ __forceinline__ void pencil_phase(const StageParams &P, const double *__restrict__ Ut, double *__restrict__ Rs,
+                                             const double *__restrict__ Md, long e0, int nel, int t, double cc) {
+  using C = PencilCfg<DIM, NP>;
+  constexpr int NVAR = C::NVAR, NN = C::NN, NL = C::NL, ED = C::ED, MD = Geo<DIM, NP>::MD;
+  constexpr bool FIRST = (L == 0), LAST = (L == DIM - 1);
+  constexpr int SM = (L == 0) ? 1 : ((L == 1) ? NP : NP * NP);
+  if (t >= nel * NL) return;
+  const int el = t / NL, r = t - el * NL;
+  const int a1 = (DIM == 3) ? r / NP : 0, a0 = r - a1 * NP;
+  const int p0 = (L == 0) ? NP * r : ((L == 1 && DIM == 3) ? a0 + NP * NP * a1 : r);
+  const long e = e0 + el;
+  const int2 *cs = reinterpret_cast<const int2 *>(Md) + el * 2 * DIM + 2 * L;
+  const int2 c0 = cs[0], c1 = cs[1];
+  double Up0[NVAR], Up1[NVAR];
+  pencil_gather<DIM, NP>(P, c0, a0, a1, Ut, e0, nel, Up0);
+  pencil_gather<DIM, NP>(P, c1, a0, a1, Ut, e0, nel, Up1);
+  double U[NVAR][NP];
+  const int ofs = el * ED + p0;
+  {
+    const double *ul = Ut + ofs;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) {
+#pragma unroll
+      for (int m = 0; m < NP; ++m) U[v][m] = ul[v * NN + m * SM];
+    }
+  }
+  const bool use_un = LAST && (P.ca != 0.0);
+  const long gofs = e * ED + p0;
+  const double *met = Md + C::NCN + el * MD;
+  double Ja[DIM];
+#pragma unroll
+  for (int c = 0; c < DIM; ++c) Ja[c] = met[L * DIM + c];
+  const double nrm = Md[C::NCN + C::NMT + el * DIM + L];
+  double invJ = 0.0;
+  if constexpr (LAST) invJ = met[DIM * DIM];
+  double rinv[NP], pr[NP], vn[NP];
+#pragma unroll
+  for (int m = 0; m < NP; ++m) {
+    rinv[m] = rcp_pos(U[0][m]);
+    double mn = 0.0, ke = 0.0;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) {
+      mn += U[1 + c][m] * Ja[c];
+      ke += U[1 + c][m] * (U[1 + c][m] * rinv[m]);
+    }
+    pr[m] = (P.gamma - 1.0) * (U[DIM + 1][m] - 0.5 * ke);
+    vn[m] = mn * rinv[m];
+  }
+  double *rl = Rs + ofs;
+  double accE[NVAR][2];
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) {
+    double un[NP];
+    if constexpr (LAST) {
+      if (use_un) {
+#pragma unroll
+        for (int m = 1; m < NP - 1; ++m) un[m] = P.u_n[gofs + v * NN + m * SM];
+      }
+    }
+    double f[NP], acc[NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) {
+      if (v == 0) f[m] = U[0][m] * vn[m];
+      else if (v == DIM + 1) f[m] = (U[DIM + 1][m] + pr[m]) * vn[m];
+      else f[m] = U[v][m] * vn[m] + pr[m] * Ja[v - 1];
+    }
+    if constexpr (FIRST) {
+#pragma unroll
+      for (int i = 0; i < NP; ++i) acc[i] = 0.0;
+    } else {
+#pragma unroll
+      for (int i = 0; i < NP; ++i) acc[i] = rl[v * NN + i * SM];
+    }
+    line_deriv<NP>(P, f, acc);
+    accE[v][0] = acc[0];
+    accE[v][1] = acc[NP - 1];
+    if constexpr (!LAST) {
+#pragma unroll
+      for (int i = 1; i < NP - 1; ++i) rl[v * NN + i * SM] = acc[i];
+    } else {
+#pragma unroll
+      for (int m = 1; m < NP - 1; ++m) {
+        const double val = P.cb * U[v][m] + cc * (0.0 - invJ * acc[m]);
+        P.u_out[gofs + v * NN + m * SM] = use_un ? (P.ca * un[m] + val) : val;
+      }
+    }
+  }
+  double unE[NVAR][2];
+  if constexpr (LAST) {
+    if (use_un) {
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) {
+        unE[v][0] = P.u_n[gofs + v * NN];
+        unE[v][1] = P.u_n[gofs + v * NN + (NP - 1) * SM];
+      }
+    }
+  }
+  const int k0 = c0.y & 3, k1 = c1.y & 3;
+  const PencilFace F0 = pencil_face<DIM>(Up0, Ja, nrm, P.gamma, vn[0], pr[0], rinv[0]);
+  const PencilFace F1 = pencil_face<DIM>(Up1, Ja, nrm, P.gamma, vn[NP - 1], pr[NP - 1], rinv[NP - 1]);
+  double Fs0[NVAR], Fs1[NVAR];   // mortar faces only: F* (outward) from the mortar routine
+  if constexpr (MORTAR && DIM == 2) {
+    if (k0 >= FK_MORTAR_FINE) {
+      double Um[NVAR], nv[DIM];
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Um[v] = U[v][0];
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) nv[c] = 0.0 - Ja[c];
+      node_mortar_flux_2d<NP>(P, e, 2 * L, a0, c0, Um, nv, Fs0);
+    }
+    if (k1 >= FK_MORTAR_FINE) {
+      double Um[NVAR], nv[DIM];
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Um[v] = U[v][NP - 1];
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) nv[c] = Ja[c];
+      node_mortar_flux_2d<NP>(P, e, 2 * L + 1, a0, c1, Um, nv, Fs1);
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) {
+    double f0, f1;
+    if (v == 0) { f0 = U[0][0] * vn[0]; f1 = U[0][NP - 1] * vn[NP - 1]; }
+    else if (v == DIM + 1) { f0 = (U[v][0] + pr[0]) * vn[0]; f1 = (U[v][NP - 1] + pr[NP - 1]) * vn[NP - 1]; }
+    else { f0 = U[v][0] * vn[0] + pr[0] * Ja[v - 1]; f1 = U[v][NP - 1] * vn[NP - 1] + pr[NP - 1] * Ja[v - 1]; }
+    double lift0, lift1;
+    if (MORTAR && DIM == 2 && k0 >= FK_MORTAR_FINE) lift0 = P.inv_wb * (Fs0[v] + f0);
+    else lift0 = P.inv_wb * (0.5 * (f0 - pencil_flux_comp<DIM>(v, Up0, F0, Ja)) - F0.hl * (Up0[v] - U[v][0]));
+    if (MORTAR && DIM == 2 && k1 >= FK_MORTAR_FINE) lift1 = P.inv_wb * (Fs1[v] - f1);
+    else lift1 = P.inv_wb * (0.5 * (pencil_flux_comp<DIM>(v, Up1, F1, Ja) - f1) - F1.hl * (Up1[v] - U[v][NP - 1]));
+    const double r0 = accE[v][0] + lift0, r1 = accE[v][1] + lift1;
+    if constexpr (!LAST) {
+      rl[v * NN] = r0;
+      rl[v * NN + (NP - 1) * SM] = r1;
+    } else {
+      const double v0 = P.cb * U[v][0] + cc * (0.0 - invJ * r0), v1 = P.cb * U[v][NP - 1] + cc * (0.0 - invJ * r1);
+      P.u_out[gofs + v * NN] = use_un ? (P.ca * unE[v][0] + v0) : v0;
+      P.u_out[gofs + v * NN + (NP - 1) * SM] = use_un ? (P.ca * unE[v][1] + v1) : v1;
+    }
+  }
+}
+
+template <int DIM, int NP, bool MORTAR>
+__global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MINB) stage_pencil_kernel(const __grid_constant__ StageParams P) {
+  using C = PencilCfg<DIM, NP>;
+  constexpr int ET = C::ET, ED = C::ED, TD = C::TD, UB = C::UB, NT = C::NT, MW = C::MW, MD = Geo<DIM, NP>::MD;
+  extern __shared__ __align__(16) double smem[];
+  double *Ub = smem;
+  double *Rs = smem + 2 * UB;
+  double *Mds = Rs + TD;
+  uint64_t *bars = reinterpret_cast<uint64_t *>(Mds + 2 * MW);
+  const int tid = threadIdx.x;
+  const long ntile = (P.ne + ET - 1) / ET;
+  const long total = P.ne * ED;
+  const bool use_un = (P.ca != 0.0);
+  auto window = [&](long tile, long &ws, int &wl, int &shift) -> bool {
+    const long b = tile * TD;
+    const long nel = (P.ne - tile * ET < ET) ? (P.ne - tile * ET) : ET;
+    shift = (int)(b & 1);
+    ws = b - shift;
+    wl = (int)((nel * ED + shift + 1) & ~1L);
+    return ws + wl <= total;
+  };
+  auto issue = [&](long tile, int buf) {
+    long ws;
+    int wl, shift;
+    if (tile < ntile && window(tile, ws, wl, shift)) {
+      mbar_expect_tx(&bars[buf], (uint32_t)wl * 8u);
+      bulk_load(Ub + buf * UB, P.u_in + ws, (uint32_t)wl * 8u, &bars[buf]);
+    }
+  };
+  auto fetch_meta = [&](long tile, int buf) {
+    if (tile >= ntile) return;
+    const long e0 = tile * ET;
+    const int nel = (int)((P.ne - e0 < ET) ? (P.ne - e0) : ET);
+    double *dst = Mds + buf * MW;
+    for (int i = tid; i < nel * 2 * DIM; i += NT) cp_async8(dst + i, P.conn + e0 * 2 * DIM + i);
+    for (int i = tid; i < nel * MD; i += NT) cp_async8(dst + C::NCN + i, P.metric + e0 * MD + i);
+    for (int i = tid; i < nel * DIM; i += NT) cp_async8(dst + C::NCN + C::NMT + i, P.fnorm + e0 * DIM + i);
+  };
+  if (tid == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  fetch_meta(blockIdx.x, 0);
+  cp_async_wait_all();
+  __syncthreads();
+  if (tid == 0) {
+    issue(blockIdx.x, 0);
+    issue((long)blockIdx.x + gridDim.x, 1);
+  }
+  const double cc = stage_cc(P);
+  int it = 0;
+  for (long tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+    const int buf = it & 1;
+    const long e0 = tile * ET;
+    const int nel = (int)((P.ne - e0 < ET) ? (P.ne - e0) : ET);
+    long ws;
+    int wl, shift;
+    const bool by_tma = window(tile, ws, wl, shift);
+    const double *Ut = Ub + buf * UB + shift;
+    const double *Md = Mds + buf * MW;
+    fetch_meta(tile + gridDim.x, buf ^ 1);
+    if (by_tma) {
+      mbar_wait(&bars[buf], (uint32_t)((it >> 1) & 1));
+    } else {
+      double *dst = Ub + buf * UB + shift;
+      for (int i = tid; i < nel * ED; i += NT) dst[i] = __ldg(P.u_in + e0 * ED + i);
+      __syncthreads();
+    }
+    pencil_phase<DIM, NP, 0, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc);
+    __syncthreads();
+    // u_n of this tile is read by the last phase: bring it into L2 now (earlier, and part of it is evicted again)
+    if (tid == 0 && use_un && by_tma) bulk_prefetch_l2(P.u_n + ws, (uint32_t)wl * 8u);
+    if constexpr (DIM == 3) {
+      pencil_phase<DIM, NP, 1, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc);
+      __syncthreads();
+    }
+    pencil_phase<DIM, NP, DIM - 1, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc);
+    cp_async_wait_all();
+    __syncthreads();
+    if (tid == 0) issue(tile + 2L * gridDim.x, buf);
+  }
+}
+
+template <int DIM, int NP, bool MORTAR>
+cudaError_t launch_stage_pencil_t(const StageParams &P, bool force, cudaStream_t st) {
+  using C = PencilCfg<DIM, NP>;
+  auto k = stage_pencil_kernel<DIM, NP, MORTAR>;
+  static std::atomic<unsigned long long> attr_done{0};
+  if (cudaError_t err = set_smem_once((const void *)k, C::smem_bytes, attr_done); err != cudaSuccess) return err;
+  const long ntile = (P.ne + C::ET - 1) / C::ET;
+  const long nres = (long)C::MINB * P.num_sms;   // one resident wave
+  // a mesh that cannot fill the GPU with tiles runs the thread-per-node kernel (its smaller CTAs spread it better),
+  // unless the caller insists (marut_debug_stage_kernel: the parity tests of small meshes)
+  if (ntile < nres && !force) return cudaErrorNotSupported;
+  const long grid = ntile < nres ? ntile : nres;
+  k<<<(unsigned)grid, C::NT, C::smem_bytes, st>>>(P);
+  return cudaGetLastError();
+}
+
+}  // namespace marut
