@@ -480,25 +480,30 @@ static double logmean(double aL, double aR) {
 }
 // O14. Two-point volume flux of Ranocha contracted with a (scaled, averaged) vector nv (eq. 41):
 //   F_rho = {{rho}}^ln {{v}}.n ;  F_rho v_c = {{rho}}^ln {{v}}.n {{v_c}} + {{p}} n_c ;
-//   F_E = ( 1/((gamma-1) {{T^-1}}^ln) + 1/2 sum_c {{v_c}}^2 ) {{rho}}^ln {{v}}.n + {{p v}}.n ,  T = p/rho.
-// The paper prints 1/(2 (gamma-1) {{T^-1}}^ln); with T = p/rho that contradicts the consistency F#(U,U) = F_inv(U)
-// it states in eq. 40 (the 2 belongs to beta = rho/(2p) of the cited flux): reading R13 takes eq. 40.
+//   F_E = ( 1/((gamma-1) {{rho/p}}^ln) + 1/2 v_L.v_R ) {{rho}}^ln {{v}}.n + 1/2 (p_L v_R + p_R v_L).n ,  T = p/rho.
+// Reading R13.  The paper prints the energy flux with 1/(2 (gamma-1) {{T^-1}}^ln), the kinetic term
+// 1/2 sum_c {{v_c}}^2 and the pressure work {{p v}}.n.  The first contradicts the consistency F#(U,U) = F_inv(U) it
+// states in eq. 40 (the 2 belongs to beta = rho/(2p) of the cited flux); the other two contradict the property it
+// names on PAPER.md:611, "the kinetic energy preserving and entropy-conservative flux of Ranocha [19]": with them
+// (w_R - w_L).F# != psi_R - psi_L at second order in the jump.  The stated properties fix the flux: 1/2 v_L.v_R and
+// 1/2 (p_L v_R + p_R v_L) are the terms of the cited flux, and the only ones of this form that satisfy Tadmor's
+// condition (pinned in tests/test_oracle_split.py).
 static void ranocha_flux(const Mesh &m, const double *UL, const double *UR, const double *nv, double *F) {
   const int d = m.dim;
   const Prim L = primitives(m, UL), R = primitives(m, UR);
   const double rho_ln = logmean(L.rho, R.rho);
   const double tinv_ln = logmean(L.rho / L.p, R.rho / R.p);
-  double vavg[3] = {0.0, 0.0, 0.0}, vn = 0.0, v2 = 0.0, pvn = 0.0;
+  double vavg[3] = {0.0, 0.0, 0.0}, vn = 0.0, vLvR = 0.0, pvn = 0.0;
   for (int c = 0; c < d; ++c) {
     vavg[c] = 0.5 * (L.vel[c] + R.vel[c]);
     vn += vavg[c] * nv[c];
-    v2 += vavg[c] * vavg[c];
-    pvn += 0.5 * (L.p * L.vel[c] + R.p * R.vel[c]) * nv[c];
+    vLvR += L.vel[c] * R.vel[c];
+    pvn += 0.5 * (L.p * R.vel[c] + R.p * L.vel[c]) * nv[c];
   }
   const double pavg = 0.5 * (L.p + R.p);
   F[0] = rho_ln * vn;
   for (int c = 0; c < d; ++c) F[1 + c] = rho_ln * vn * vavg[c] + pavg * nv[c];
-  F[1 + d] = (1.0 / ((m.gamma - 1.0) * tinv_ln) + 0.5 * v2) * rho_ln * vn + pvn;
+  F[1 + d] = (1.0 / ((m.gamma - 1.0) * tinv_ln) + 0.5 * vLvR) * rho_ln * vn + pvn;
 }
 // O5. Local Lax-Friedrichs / Rusanov flux with scaled outward normal nv:
 //   F* = 1/2 (F(U-)+F(U+)).nv - 1/2 lambda |nv| (U+ - U-),
