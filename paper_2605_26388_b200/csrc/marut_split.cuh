@@ -127,6 +127,8 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
         const int m = (ql + sd >= NP) ? ql + sd - NP : ql + sd;
         const int pm = base + m * st;            // stash index of the partner node
         const double rm = Ust[pm], pmm = Ust[(NVAR + 1) * TILE + pm];
+        // energy flux of the cited entropy-conservative flux (R13): kinetic term 1/2 v_i.v_m, pressure work
+        // 1/2 (p_i v_m + p_m v_i).n
         double nv[DIM], vavg[DIM], vn = 0.0, v2 = 0.0, pvn = 0.0;
 #pragma unroll
         for (int c = 0; c < DIM; ++c) {
@@ -135,8 +137,8 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
           else nv[c] = 0.5 * (Ji[c] + __ldg(&P.metric[(e * MD + l * DIM + c) * NN + (pm - el * NN)]));
           vavg[c] = 0.5 * (vi[c] + vm);
           vn += vavg[c] * nv[c];
-          v2 += vavg[c] * vavg[c];
-          pvn += 0.5 * (pi_ * vi[c] + pmm * vm) * nv[c];
+          v2 += vi[c] * vm;
+          pvn += 0.5 * (pi_ * vm + pmm * vi[c]) * nv[c];
         }
         double nr, dr, nb, db;
         logmean_nd(U[0], rm, lnr, Lns[pm], nr, dr);

@@ -1,0 +1,47 @@
+"""Mutants of the oracle: the oracle source with ONE named line changed, compiled into a scratch library.  The pin tests
+run their checks against a mutant as well and assert that the check FAILS there -- the committed proof that a pin
+would catch the plausible mistake it is meant to catch (VERDICT r1 'oracle parts with no effective pin')."""
+import ctypes
+import os
+import subprocess
+import tempfile
+
+import oracle
+
+_SRC = os.path.join(os.path.dirname(os.path.abspath(oracle.__file__)), "marut_oracle.cpp")
+
+# name -> (text in oracle/marut_oracle.cpp, its replacement, what the mutant gets wrong)
+MUTATIONS = {
+    "mortar2d_lo_up_swapped": (
+        "acc += m.Pf[s][a * n + j] * UC[(size_t)j * nvar + v];",
+        "acc += m.Pf[1 - s][a * n + j] * UC[(size_t)j * nvar + v];",
+        "2-D mortar: the coarse trace is interpolated to the wrong half of the coarse face"),
+    "boundary_state_ignored": (
+        "Ue[v] = (bk == 0) ? m.bc_state[(size_t)bc * nvar + v] : Um[v];",
+        "Ue[v] = Um[v];",
+        "prescribed exterior state ignored: every Dirichlet face becomes an outflow"),
+    "br1_trace_not_central": (
+        "double What = 0.5 * (Wm[w] + Wp[w]);",
+        "double What = 0.75 * Wm[w] + 0.25 * Wp[w];",
+        "BR1 interface trace is not the arithmetic mean of eq. 13"),
+    "ranocha_printed_energy_flux": (
+        "pvn += 0.5 * (L.p * R.vel[c] + R.p * L.vel[c]) * nv[c];",
+        "pvn += 0.5 * (L.p * L.vel[c] + R.p * R.vel[c]) * nv[c];",
+        "pressure work {{p v}} as PAPER.md:621 prints it: not entropy conservative"),
+}
+
+_cache = {}
+
+
+def mutant(name):
+    """ctypes library of the oracle with mutation `name` applied (compiled once per test session)"""
+    if name not in _cache:
+        old, new, _ = MUTATIONS[name]
+        src = open(_SRC).read()
+        assert src.count(old) == 1, f"mutation site of {name!r} not found exactly once in the oracle source"
+        d = tempfile.mkdtemp(prefix="marut_mutant_")
+        cpp, so = os.path.join(d, "mutant.cpp"), os.path.join(d, "mutant.so")
+        open(cpp, "w").write(src.replace(old, new))
+        subprocess.run(["g++", "-O1", "-ffp-contract=off", "-fopenmp", "-std=c++17", "-shared", "-fPIC", cpp, "-o", so], check=True)
+        _cache[name] = oracle._setup(ctypes.CDLL(so))
+    return _cache[name]
