@@ -198,6 +198,27 @@ marut_status marut_set_boundary_kinds(marut_mesh *mesh, const int *kinds, int n_
 marut_status marut_positivity_floor(marut_mesh *mesh, double *u, double rho_min, double p_min, long *changed_out,
                                     void *cuda_stream);
 
+/* Whole time steps (SURVEY 8(f) NEXT-2 / NEXT-2b), composed inside the library from the stage calls above, so that no
+ * caller has to carry a coefficient table.  u (DEVICE) is advanced in place; scratch[k] are state-sized DEVICE buffers
+ * owned by the caller, 16-byte aligned, distinct from u and from one another.  dt_dev != NULL: the time step is read
+ * from that DEVICE double inside the kernels (marut_max_dt_async; `dt` is ignored and nothing waits for the GPU), else
+ * the HOST value `dt` is used.  Asynchronous on the stream.
+ *   marut_ssprk33_step: eq. 44-46 (R10), three marut_ssprk_stage calls; 2 scratch buffers.
+ *   marut_ssprk54_step: the five-stage fourth-order scheme PAPER.md:725 names (table: DESIGN.md R19), five stage
+ *                       kernels and one four-term combination; 3 scratch buffers.
+ *   marut_strang_step : eq. 24, u <- S_{dt/2} T_dt S_{dt/2} u with S = marut_chem_implicit and
+ *                       T_dt = one SSP-RK33 step of the transport operator without the explicit source (the handle's
+ *                       marut_set_explicit_source setting is restored); REACTING_EULER meshes, HOST dt; 2 scratch
+ *                       buffers.  sweeps_out (HOST, may be NULL): the larger Newton sweep count of the two substeps;
+ *                       asking for it synchronises, and > 50 returns MARUT_ENOTFINITE.  Whether or not it is asked
+ *                       for, a node whose Newton iteration does not converge gets NaN species densities. */
+marut_status marut_ssprk33_step(marut_mesh *mesh, double *u, double *const *scratch, double dt, const double *dt_dev,
+                                void *cuda_stream);
+marut_status marut_ssprk54_step(marut_mesh *mesh, double *u, double *const *scratch, double dt, const double *dt_dev,
+                                void *cuda_stream);
+marut_status marut_strang_step(marut_mesh *mesh, double *u, double *const *scratch, double dt, int *sweeps_out,
+                               void *cuda_stream);
+
 /* REACTING_EULER meshes: whether L(u) of marut_rhs / marut_ssprk_stage includes the explicit chemistry source S(u)
  * (on != 0, the default) or is the transport operator T alone (on == 0), as the Strang split of eq. 24 needs:
  *   u^{n+1} = S_{dt/2} o T_dt o S_{dt/2} (u^n) = marut_chem_implicit(dt/2), SSP-RK steps of T, marut_chem_implicit(dt/2). */

@@ -15,7 +15,7 @@ _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA"
 
 # every symbol include/marut.h declares
 SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt", "marut_max_dt_async", "marut_ssprk_stage_dev", "marut_rk_stage_dev",
-           "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_rk_stage", "marut_lincomb", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count", "marut_debug_rcp_sqrt", "marut_debug_stage_kernel",
+           "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_rk_stage", "marut_lincomb", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count", "marut_debug_rcp_sqrt", "marut_debug_stage_kernel", "marut_ssprk33_step", "marut_ssprk54_step", "marut_strang_step",
            "marut_last_error"]
 
 
@@ -96,6 +96,12 @@ def lib():
         L.marut_dx_min.argtypes = [vp]
         L.marut_launch_count.restype = C.c_long
         L.marut_launch_count.argtypes = [vp]
+        L.marut_ssprk33_step.restype = C.c_int
+        L.marut_ssprk33_step.argtypes = [vp, vp, vp, dbl, vp, vp]
+        L.marut_ssprk54_step.restype = C.c_int
+        L.marut_ssprk54_step.argtypes = [vp, vp, vp, dbl, vp, vp]
+        L.marut_strang_step.restype = C.c_int
+        L.marut_strang_step.argtypes = [vp, vp, vp, dbl, vp, vp]
         L.marut_debug_stage_kernel.restype = C.c_int
         L.marut_debug_stage_kernel.argtypes = [vp, C.c_int]
         L.marut_debug_rcp_sqrt.restype = C.c_int
@@ -218,35 +224,22 @@ def marut_lincomb(h, coef, us, out, stream=None):
     _check(lib().marut_lincomb(h, n, cf, ptrs, _dev(out), _stream(stream)))
 
 
-# SSP-RK54 of Spiteri and Ruuth in the Shu-Osher form of eq. 45 (R19): (alpha_i0, alpha_i,i-1, beta_i,i-1)
-_RK54 = ((1.0, 0.0, 0.391752226571890), (0.444370493651235, 0.555629506348765, 0.368410593050371),
-         (0.620101851488403, 0.379898148511597, 0.251891774271694), (0.178079954393132, 0.821920045606868, 0.544974750228521))
-_RK54_LAST = (0.517231671970585, 0.096059710526147, 0.063692468666290, 0.386708617503269, 0.226007483236906)
+def _bufs(ts):
+    return (C.c_void_p * len(ts))(*[_dev(t).value for t in ts])
 
 
 def ssprk54_step(h, u, ua, ub, uc, dt, stream=None):
-    """one SSP-RK54 step, u advanced in place; ua, ub, uc: scratch.  Call sequence only -- every stage runs in the
-    library (marut_rk_stage x 5, marut_lincomb x 1)."""
-    a, b = _RK54, _RK54_LAST
-    marut_rk_stage(h, 0.0, 1.0, a[0][2] * dt, None, u, ua, stream)                      # U1 -> ua
-    marut_rk_stage(h, a[1][0], a[1][1], a[1][2] * dt, u, ua, ub, stream)                # U2 -> ub
-    marut_rk_stage(h, a[2][0], a[2][1], a[2][2] * dt, u, ub, ua, stream)                # U3 -> ua
-    marut_rk_stage(h, a[3][0], a[3][1], a[3][2] * dt, u, ua, uc, stream)                # U4 -> uc
-    r = b[2] / a[3][2]                                                                   # dt L(U3) = (U4 - a40 U0 - a43 U3)/b43
-    marut_lincomb(h, (-r * a[3][0], b[0], b[1] - r * a[3][1], b[3] + r), (u, ub, ua, uc), ua, stream)
-    marut_rk_stage(h, 1.0, 0.0, b[4] * dt, ua, uc, u, stream)                           # U5 -> u
+    """one SSP-RK54 step (marut_ssprk54_step), u advanced in place; ua, ub, uc: scratch"""
+    _check(lib().marut_ssprk54_step(h, _dev(u), _bufs((ua, ub, uc)), float(dt), None, _stream(stream)))
 
 
 def ssprk54_step_dev(h, u, ua, ub, uc, dt_dev, stream=None):
     """ssprk54_step with the time step in device memory (marut_max_dt_async): nothing here waits for the GPU"""
-    a, b = _RK54, _RK54_LAST
-    marut_rk_stage_dev(h, 0.0, 1.0, a[0][2], dt_dev, None, u, ua, stream)
-    marut_rk_stage_dev(h, a[1][0], a[1][1], a[1][2], dt_dev, u, ua, ub, stream)
-    marut_rk_stage_dev(h, a[2][0], a[2][1], a[2][2], dt_dev, u, ub, ua, stream)
-    marut_rk_stage_dev(h, a[3][0], a[3][1], a[3][2], dt_dev, u, ua, uc, stream)
-    r = b[2] / a[3][2]
-    marut_lincomb(h, (-r * a[3][0], b[0], b[1] - r * a[3][1], b[3] + r), (u, ub, ua, uc), ua, stream)
-    marut_rk_stage_dev(h, 1.0, 0.0, b[4], dt_dev, ua, uc, u, stream)
+    _check(lib().marut_ssprk54_step(h, _dev(u), _bufs((ua, ub, uc)), 0.0, _dev(dt_dev), _stream(stream)))
+
+
+def marut_ssprk33_step(h, u, ua, ub, dt=0.0, dt_dev=None, stream=None):
+    _check(lib().marut_ssprk33_step(h, _dev(u), _bufs((ua, ub)), float(dt), None if dt_dev is None else _dev(dt_dev), _stream(stream)))
 
 
 def marut_shock_indicator(h, u, alpha, s=9.21024, alpha_min=0.001, alpha_max=0.5, smooth=True, stream=None):
@@ -279,17 +272,12 @@ def marut_set_explicit_source(h, on):
     _check(lib().marut_set_explicit_source(h, int(bool(on))))
 
 
-def strang_step(h, u, ua, ub, dt, t=0.0, stream=None):
-    """U^{n+1} = S_{dt/2} o T_dt o S_{dt/2} (U^n) (eq. 24): implicit chemistry half steps around one
-    SSP-RK33 step of the transport operator WITHOUT the explicit source.  u is overwritten; ua, ub: scratch.
-    Call sequence only -- every step runs in the library."""
-    marut_set_explicit_source(h, False)
-    try:
-        marut_chem_implicit(h, u, 0.5 * dt, stream, want_sweeps=False)
-        ssprk3_step(h, u, ua, ub, dt, t, stream)
-        marut_chem_implicit(h, u, 0.5 * dt, stream, want_sweeps=False)
-    finally:
-        marut_set_explicit_source(h, True)
+def strang_step(h, u, ua, ub, dt, t=0.0, stream=None, want_sweeps=False):
+    """U^{n+1} = S_{dt/2} o T_dt o S_{dt/2} (U^n) (eq. 24) = marut_strang_step; u is overwritten; ua, ub:
+    scratch.  Returns the larger Newton sweep count of the two implicit substeps if want_sweeps (synchronises)."""
+    n = C.c_int(0)
+    _check(lib().marut_strang_step(h, _dev(u), _bufs((ua, ub)), float(dt), C.byref(n) if want_sweeps else None, _stream(stream)))
+    return n.value if want_sweeps else None
 
 
 class MarutMesh:
@@ -359,8 +347,11 @@ class MarutMesh:
         self._alpha = alpha          # the library keeps the pointer: hold the tensor
         marut_set_blend(self.h, alpha)
 
-    def strang_step(self, u, ua, ub, dt, t=0.0, stream=None):
-        strang_step(self.h, u, ua, ub, dt, t, stream)
+    def strang_step(self, u, ua, ub, dt, t=0.0, stream=None, want_sweeps=False):
+        return strang_step(self.h, u, ua, ub, dt, t, stream, want_sweeps)
+
+    def ssprk33_step(self, u, ua, ub, dt=0.0, dt_dev=None, stream=None):
+        marut_ssprk33_step(self.h, u, ua, ub, dt, dt_dev, stream)
 
     def step(self, u, ua, ub, dt, t=0.0, stream=None):
         ssprk3_step(self.h, u, ua, ub, dt, t, stream)

@@ -747,6 +747,84 @@ extern "C" marut_status marut_chem_implicit(marut_mesh *m, double *u, double dt,
   return MARUT_OK;
 }
 
+// ------------------------------------------------------------------------------------ whole time steps
+// The step compositions of the paper's integrators, so that a C caller gets them without re-typing a coefficient
+// table: SSP-RK33 (eq. 44-46, R10), SSP-RK54 (R19) and the Strang split of eq. 24.
+// SSP-RK54 of Spiteri and Ruuth in the Shu-Osher form of eq. 45: rows (alpha_i0, alpha_i,i-1, beta_i,i-1) of stages
+// 1-4, then (alpha_52, alpha_53, beta_53, alpha_54, beta_54) of the last stage (15 digits as published).
+static const double RK54[4][3] = {{1.0, 0.0, 0.391752226571890},
+                                  {0.444370493651235, 0.555629506348765, 0.368410593050371},
+                                  {0.620101851488403, 0.379898148511597, 0.251891774271694},
+                                  {0.178079954393132, 0.821920045606868, 0.544974750228521}};
+static const double RK54_LAST[5] = {0.517231671970585, 0.096059710526147, 0.063692468666290, 0.386708617503269, 0.226007483236906};
+
+static marut_status check_step_buffers(marut_mesh *m, const double *u, double *const *scratch, int ns) {
+  if (!m || !u || !scratch) return fail(MARUT_EINVAL, "NULL argument");
+  if (misaligned(u)) return fail(MARUT_EINVAL, "buffers must be 16-byte aligned");
+  for (int i = 0; i < ns; ++i) {
+    if (!scratch[i]) return fail(MARUT_EINVAL, "scratch[%d] is NULL", i);
+    if (misaligned(scratch[i])) return fail(MARUT_EINVAL, "buffers must be 16-byte aligned");
+    if (scratch[i] == u) return fail(MARUT_EINVAL, "scratch[%d] aliases u", i);
+    for (int j = 0; j < i; ++j)
+      if (scratch[i] == scratch[j]) return fail(MARUT_EINVAL, "scratch[%d] aliases scratch[%d]", i, j);
+  }
+  return MARUT_OK;
+}
+
+// c = b * dt on the host, or b with dt read from dt_dev inside the kernel (the same single rounded product)
+static marut_status stage_any(marut_mesh *m, double a, double b, double c, double dt, const double *dt_dev, const double *u_a,
+                              const double *u_in, double *u_out, cudaStream_t st) {
+  return dt_dev ? run_operator(m, a, b, c, u_a, u_in, u_out, st, dt_dev) : run_operator(m, a, b, c * dt, u_a, u_in, u_out, st);
+}
+
+extern "C" marut_status marut_ssprk33_step(marut_mesh *m, double *u, double *const *scratch, double dt, const double *dt_dev,
+                                           void *stream) {
+  if (marut_status s = check_step_buffers(m, u, scratch, 2); s != MARUT_OK) return s;
+  cudaStream_t st = (cudaStream_t)stream;
+  double *ua = scratch[0], *ub = scratch[1];
+  marut_status s;
+  if ((s = stage_any(m, 0.0, 1.0, 1.0, dt, dt_dev, u, u, ua, st)) != MARUT_OK) return s;
+  if ((s = stage_any(m, 0.75, 0.25, 0.25, dt, dt_dev, u, ua, ub, st)) != MARUT_OK) return s;
+  return stage_any(m, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, dt, dt_dev, u, ub, u, st);
+}
+
+extern "C" marut_status marut_ssprk54_step(marut_mesh *m, double *u, double *const *scratch, double dt, const double *dt_dev,
+                                           void *stream) {
+  if (marut_status s = check_step_buffers(m, u, scratch, 3); s != MARUT_OK) return s;
+  cudaStream_t st = (cudaStream_t)stream;
+  double *ua = scratch[0], *ub = scratch[1], *uc = scratch[2];
+  const double(*a)[3] = RK54;
+  const double *b = RK54_LAST;
+  marut_status s;
+  if ((s = stage_any(m, 0.0, 1.0, a[0][2], dt, dt_dev, nullptr, u, ua, st)) != MARUT_OK) return s;      // U1 -> ua
+  if ((s = stage_any(m, a[1][0], a[1][1], a[1][2], dt, dt_dev, u, ua, ub, st)) != MARUT_OK) return s;   // U2 -> ub
+  if ((s = stage_any(m, a[2][0], a[2][1], a[2][2], dt, dt_dev, u, ub, ua, st)) != MARUT_OK) return s;   // U3 -> ua
+  if ((s = stage_any(m, a[3][0], a[3][1], a[3][2], dt, dt_dev, u, ua, uc, st)) != MARUT_OK) return s;   // U4 -> uc
+  // last stage: dt L(U3) = (U4 - a40 U0 - a43 U3)/b43 (reading R19), so
+  // U5 = [a52 U2 + a53 U3 + a54 U4 + (b53/b43)(U4 - a40 U0 - a43 U3)] + b54 dt L(U4)
+  const double r = b[2] / a[3][2];
+  const double coef[4] = {-r * a[3][0], b[0], b[1] - r * a[3][1], b[3] + r};
+  const double *us[4] = {u, ub, ua, uc};
+  if ((s = marut_lincomb(m, 4, coef, us, ua, stream)) != MARUT_OK) return s;
+  return stage_any(m, 1.0, 0.0, b[4], dt, dt_dev, ua, uc, u, st);                                        // U5 -> u
+}
+
+extern "C" marut_status marut_strang_step(marut_mesh *m, double *u, double *const *scratch, double dt, int *sweeps_out,
+                                          void *stream) {
+  if (marut_status s = check_step_buffers(m, u, scratch, 2); s != MARUT_OK) return s;
+  if (m->physics != MARUT_REACTING_EULER) return fail(MARUT_EINVAL, "marut_strang_step needs a REACTING_EULER mesh");
+  if (!(dt >= 0.0)) return fail(MARUT_EINVAL, "dt must be >= 0");
+  const int keep = m->explicit_source;
+  m->explicit_source = 0;                        // T = transport operator alone
+  int sw1 = 0, sw2 = 0;
+  marut_status s = marut_chem_implicit(m, u, 0.5 * dt, sweeps_out ? &sw1 : nullptr, stream);
+  if (s == MARUT_OK) s = marut_ssprk33_step(m, u, scratch, dt, nullptr, stream);
+  if (s == MARUT_OK) s = marut_chem_implicit(m, u, 0.5 * dt, sweeps_out ? &sw2 : nullptr, stream);
+  m->explicit_source = keep;
+  if (sweeps_out) *sweeps_out = std::max(sw1, sw2);
+  return s;
+}
+
 // ------------------------------------------------------------------------------------ boundary kinds
 __global__ void patch_boundary_kinds_kernel(int2 *conn, long n, const int *kinds) {
   for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {

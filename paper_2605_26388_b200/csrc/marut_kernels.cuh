@@ -302,8 +302,11 @@ __global__ void __launch_bounds__(128) chem_implicit_kernel(double *__restrict__
       if (dmax <= 1e-13 * rho) break;
     }
     worst = max(worst, it);
+    // a node whose Newton iteration did not converge within 50 sweeps (it == 51) is poisoned, so that an unchecked call
+    // (sweeps_out == NULL) cannot carry an unconverged state forward silently: the next marut_max_dt reports it
+    const bool failed = it > 50;
 #pragma unroll
-    for (int s = 0; s < NSP; ++s) u[(e * NVAR + s) * nn + p] = Y[s];
+    for (int s = 0; s < NSP; ++s) u[(e * NVAR + s) * nn + p] = failed ? __longlong_as_double(0x7ff8000000000000LL) : Y[s];
   }
   worst = __reduce_max_sync(0xffffffffu, worst);
   if ((threadIdx.x & 31) == 0) atomicMax(max_sweeps, worst);
