@@ -1,12 +1,18 @@
 #!/usr/bin/env python
 """bench.py -- DG RHS + SSP-RK33 throughput of the CUDA path (DOF-stage updates / s, FP64) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4w|c4|c5|c1] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4w|c4|c5|c1|...] [--impl reference]
 
-A "step" is one pass of the whole hot path over the workload: marut_max_dt (CFL reduction) followed by the
-three fused marut_ssprk_stage launches of one SSP-RK33 step (SURVEY 8(a) rows a1..a10 as the physics has
-them).  Default workload: BASELINE.json configs[1] (c2: 3-D Euler, N=4, 32^3 periodic hexes, ~20.5M DOF),
+A "step" is one pass of the whole hot path over the workload: the CFL reduction (marut_max_dt_async, dt stays on the
+device) followed by the three fused marut_ssprk_stage launches of one SSP-RK33 step (SURVEY 8(a) rows a1..a10 as the
+physics has them).  Default workload: BASELINE.json configs[1] (c2: 3-D Euler, N=4, 32^3 periodic hexes, ~20.5M DOF),
 synthetic seeded inputs.  One JSON line is printed by rank 0.
+
+Timing: W warm-up steps, then blocks of EXACTLY K steps, each block between one CUDA-event pair on the
+launching stream, repeated (>= 5 times) until the timed region is >= 1 s; value / ms_per_step are the MEDIAN block
+(min / max beside it); the step is replayed as a CUDA graph (--no-graph: eager launches; ms_per_step_eager is always
+reported).  roofline: CUDA events around every marut_ssprk_stage call of one eager K-step block.  The default run also
+measures the other configs of BASELINE.json (c1, c3, c4w, c5) with the same protocol -> "configs".
 
 N > 1 (torchrun): the path does not shard in this build ("replicas only"): every rank
 advances its own replica of the workload, no data-path collective; value = units of all ranks / max time.
@@ -171,26 +177,35 @@ def oracle_advance(om, case, u, n):
 
 
 def oracle_sample(workload, budget_s):
-    """time the CPU oracle (as it stands, never tuned) on a bounded sample of the workload: the same config
-    at fewer elements per direction, as many SSP-RK33 steps (dt from its own CFL reduction) as fit budget_s."""
+    """time the CPU oracle (as it stands, never tuned) on a bounded sample of the workload: the same config at fewer
+    elements per direction, as many SSP-RK33 steps (dt from its own CFL reduction) as fit the budget: two thirds of it
+    on all host cores, one third on ONE core (SURVEY 8(d) 'Timing')."""
     import oracle
-    import workloads as wl
 
     cells = ORACLE_SAMPLE_CELLS[workload]
     c = make_workload(workload, cells=cells)
     om = oracle.OracleMesh(c.mesh)
-    t0 = time.perf_counter()
-    u = oracle_advance(om, c, c.u0, 1)          # calibration step (counted)
-    t1 = time.perf_counter() - t0
-    n = max(1, min(200, int(budget_s / max(t1, 1e-6)) - 1))
-    t0 = time.perf_counter()
-    oracle_advance(om, c, u, n)
-    t = time.perf_counter() - t0
-    per_step = t / n
-    return {"case": c, "steps": n, "s_per_step": per_step, "value": c.mesh.n_dof * 3 / per_step,
-            "cores": oracle.num_threads(),
-            "sample": f"{workload} at {c.mesh.n_elem} elements ({c.mesh.n_dof} DOF), {n} SSP-RK33 steps incl. CFL reduction, "
-                      f"{t:.1f} s, g++ -O2 -ffp-contract=off + OpenMP over elements"}
+    ncores = oracle.num_threads()
+
+    def timed(budget):
+        t0 = time.perf_counter()
+        u = oracle_advance(om, c, c.u0, 1)          # calibration step
+        t1 = time.perf_counter() - t0
+        n = max(1, min(200, int(budget / max(t1, 1e-6)) - 1))
+        t0 = time.perf_counter()
+        oracle_advance(om, c, u, n)
+        return n, time.perf_counter() - t0
+
+    n, t = timed(budget_s * 2.0 / 3.0)
+    oracle.set_num_threads(1)
+    try:
+        n1, t1 = timed(budget_s / 3.0)
+    finally:
+        oracle.set_num_threads(ncores)
+    return {"case": c, "steps": n, "s_per_step": t / n, "value": c.mesh.n_dof * 3 * n / t, "value_1core": c.mesh.n_dof * 3 * n1 / t1,
+            "cores": ncores,
+            "sample": f"{workload} at {c.mesh.n_elem} elements ({c.mesh.n_dof} DOF), {n} SSP-RK33 steps incl. CFL reduction in "
+                      f"{t:.1f} s on {ncores} cores and {n1} steps in {t1:.1f} s on 1 core, g++ -O2 -ffp-contract=off + OpenMP over elements"}
 
 
 def run_reference(args):
@@ -257,125 +272,217 @@ def measured_peaks():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def run_cuda(args):
-    import numpy as np
-    import torch
-    import torch.distributed as dist
+KERNELS = {"euler": "stage_pencil_kernel (fused Euler stage: persistent TMA-fed line kernel)",
+           "euler_node": "stage_node_kernel (fused Euler stage, thread per node)",
+           "euler_mortar3d": "mortar_flux3d_kernel + stage_node_kernel (fused Euler stage, 3-D mortar instantiation)",
+           "split": "stage_split_kernel (fused Euler stage, split-form volume integral)",
+           "split_blend": "stage_split_kernel (fused Euler stage, split-form volume integral blended with the sub-cell FV residual)",
+           "ns": "gradient_kernel + stage_phys_kernel (BR1 gradient sweep + fused NS stage)",
+           "react": "eos_kernel + stage_phys_kernel (mixture temperature + fused reacting stage)"}
 
-    import paper_2605_26388_b200 as mb
-    import workloads as wl
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+class Workload:
+    """one workload on the current device: library handle, state buffers, and one step of the hot path (the CFL
+    reduction with dt left on the device + the three fused stages) in eager form and as a replayable CUDA graph"""
 
-    case = make_workload(args.workload)
-    mesh = case.mesh
-    gm = mb.MarutMesh(mesh)
-    affine = gm.is_affine
-    u0_host = torch.from_numpy(np.ascontiguousarray(case.u0)).pin_memory()
-    out_host = torch.empty_like(u0_host).pin_memory()
-    u = u0_host.cuda()
-    ua, ub = torch.empty_like(u), torch.empty_like(u)
-    stream = torch.cuda.current_stream()
-    n_dof = mesh.n_dof
-    cfl = case.cfl
+    def __init__(self, name, args, torch, mb):
+        import numpy as np
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        self.torch, self.args, self.name = torch, args, name
+        self.case = make_workload(name)
+        self.mesh = self.case.mesh
+        self.gm = mb.MarutMesh(self.mesh)
+        self.affine = self.gm.is_affine
+        self.u0_host = torch.from_numpy(np.ascontiguousarray(self.case.u0)).pin_memory()
+        self.u = self.u0_host.cuda()
+        self.ua, self.ub = torch.empty_like(self.u), torch.empty_like(self.u)
+        # The configs are short runs (BASELINE.json: 10-20 steps; c4/c5 leave their well-posed window after ~100-190
+        # steps without the paper's limiter / implicit chemistry, DESIGN.md section 5), so the bench repeats the config:
+        # every `case.steps` steps the next step starts again from the pristine u0 (its stages read u0 directly, so the
+        # restart costs no extra copy and no extra traffic).
+        self.u0_dev = self.u.clone()
+        self.counter = 0
+        self.sc = getattr(self.case, "shock_capture", None)
+        self.alpha = None
+        if self.sc:
+            self.alpha = torch.zeros(self.mesh.n_elem, dtype=torch.float64, device=self.u.device)
+            self.gm.set_blend(self.alpha)
+        # dt stays on the device (marut_max_dt_async -> marut_ssprk_stage_dev: the same dt and the same stage results bit
+        # for bit, tests/test_gpu_async_dt.py), so the host queues the whole step without waiting for the CFL reduction
+        self.dt_dev = torch.zeros(1, dtype=torch.float64, device=self.u.device)
+        self.graphs = None
 
-    # The configs are short runs (BASELINE.json: 10-20 steps; c4/c5 leave their well-posed window after
-    # ~100-190 steps without the paper's limiter / implicit chemistry), so the bench
-    # repeats the config: every `case.steps` steps the next step starts again from the pristine u0 (its
-    # stages read u0 directly, so the restart costs no extra copy and no extra traffic).
-    u0_dev = u.clone()
-    counter = [0]
-    sc = getattr(case, "shock_capture", None)
-    alpha = None
-    if sc:
-        alpha = torch.zeros(mesh.n_elem, dtype=torch.float64, device=u.device)
-        gm.set_blend(alpha)
+    def kernel_label(self):
+        m = self.mesh
+        if m.physics == 1:
+            return KERNELS["ns"]
+        if m.physics == 2:
+            return KERNELS["react"]
+        if getattr(m, "volume_form", 0):
+            return KERNELS["split_blend" if self.sc else "split"]
+        if m.dim == 3 and len(m.mortar):
+            return KERNELS["euler_mortar3d"]
+        return KERNELS["euler" if self.affine else "euler_node"]
 
-    # dt stays on the device (marut_max_dt_async -> marut_ssprk_stage_dev: the same dt and the same stage results bit
-    # for bit, tests/test_gpu_async_dt.py), so the host queues the whole step without waiting for the CFL reduction;
-    # --sync-dt times the host-synchronised marut_max_dt instead
-    dt_dev = torch.zeros(1, dtype=torch.float64, device=u.device)
-
-    def step(ev=None):
-        src = u0_dev if counter[0] % case.steps == 0 else u
-        counter[0] += 1
-        if args.sync_dt:
+    def _step(self, src, ev=None):
+        torch, gm, sc, stream = self.torch, self.gm, self.sc, self.torch.cuda.current_stream()
+        cfl = self.case.cfl
+        if self.args.sync_dt:
             dt = gm.max_dt(src, cfl)
         else:
-            gm.max_dt_async(src, cfl, dt_dev)
-            dt = None
-        for s, (un, uin, uout) in enumerate(((src, src, ua), (src, ua, ub), (src, ub, u))):
+            gm.max_dt_async(src, cfl, self.dt_dev)
+        for s, (un, uin, uout) in enumerate(((src, src, self.ua), (src, self.ua, self.ub), (src, self.ub, self.u))):
             if sc:
-                gm.shock_indicator(uin, alpha, **sc)
+                gm.shock_indicator(uin, self.alpha, **sc)
             if ev is not None:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
-            if args.sync_dt:
+            if self.args.sync_dt:
                 gm.stage(s, dt, 0.0, un, uin, uout)
             else:
-                gm.stage_dev(s, dt_dev, 0.0, un, uin, uout)
+                gm.stage_dev(s, self.dt_dev, 0.0, un, uin, uout)
             if ev is not None:
                 e1.record(stream)
                 ev.append((e0, e1))
             if sc:
                 gm.positivity_floor(uout)
-        return dt
 
-    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps
+    def step(self, ev=None, graph=False):
+        first = self.counter % self.case.steps == 0
+        self.counter += 1
+        if graph and self.graphs is not None:
+            self.graphs[0 if first else 1].replay()
+        else:
+            self._step(self.u0_dev if first else self.u, ev)
+
+    def capture(self):
+        """the two variants of the step (from u0 / from u) as CUDA graphs: the library only launches on the stream it
+        is given, so a step is capturable as it stands (tests/test_gpu_async_dt.py: replay equals eager bit for bit)"""
+        if self.args.sync_dt or self.args.no_graph:
+            return
+        torch = self.torch
+        gs = []
+        for src in (self.u0_dev, self.u):
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                self._step(src)
+            gs.append(g)
+        self.graphs = gs
+
+    def block(self, K, graph, ev=None):
+        """K steps bracketed by an event pair on the current stream; returns the pair"""
+        torch = self.torch
+        stream = torch.cuda.current_stream()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(K):
+            self.step(ev, graph)
+        b.record(stream)
+        return a, b
+
+
+def measure(w, args, barrier, world, rank, local):
+    """timing protocol of one workload (SURVEY 8(d) 'Timing'): W warm-up steps; one eager block of K steps with an event
+    pair around every marut_ssprk_stage call (roofline of the dominant kernel); then R >= 5 blocks of exactly K steps
+    each, replayed as CUDA graphs, until the timed region is >= 1 s; the headline is the MEDIAN block."""
+    import numpy as np
+
+    torch = w.torch
+    K = args.steps
     for _ in range(args.warmup):
-        step()
+        w.step()
+    w.capture()
+    for _ in range(args.warmup):
+        w.step(graph=True)
     barrier()
+    # eager block with per-stage events
+    l0 = w.gm.launch_count
+    ev = []
+    a, b = w.block(K, graph=False, ev=ev)
+    barrier()
+    eager_ms = a.elapsed_time(b)
+    launches_per_block = w.gm.launch_count - l0
+    stage_ms = [x.elapsed_time(y) for x, y in ev]
+    # graph blocks
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    launches0 = gm.launch_count
-    events = []
-    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t_start.record(stream)
-    for _ in range(args.steps):
-        step(events)
-    t_end.record(stream)
+    use_graph = w.graphs is not None
+    blocks = []
+    first = w.block(K, graph=use_graph)
     barrier()
-    ms = t_start.elapsed_time(t_end)
-    launches = gm.launch_count - launches0
+    blocks.append(first[0].elapsed_time(first[1]))
+    reps = int(min(400, max(5, math.ceil(args.min_ms / max(blocks[0], 1e-3)))))
+    pairs = [w.block(K, graph=use_graph) for _ in range(reps - 1)]
+    barrier()
+    blocks += [x.elapsed_time(y) for x, y in pairs]
     clocks = sampler.stop() if rank == 0 else None
-    if not np.isfinite(u.sum().item()):
-        raise RuntimeError("solution became non-finite during the timed region")
-    stage_ms = [a.elapsed_time(b) for a, b in events]
-    # launches of the dominant kernel inside one marut_ssprk_stage call (NS: gradient + stage; REACT: eos + stage)
-    stage_ms_avg = sum(stage_ms) / len(stage_ms)
+    if not np.isfinite(w.u.sum().item()):
+        raise RuntimeError(f"{w.name}: solution became non-finite during the timed region")
+    blocks_max = [max_over_ranks([t], world, device="cuda")[0] for t in blocks] if world > 1 else blocks
+    med = float(np.median(blocks_max))
+    return {"ms_block_median": med, "ms_blocks_min": min(blocks_max), "ms_blocks_max": max(blocks_max), "repeats": len(blocks_max),
+            "timed_region_ms": float(sum(blocks_max)), "eager_ms_block": eager_ms, "stage_ms": stage_ms,
+            "launches_per_block": launches_per_block, "clocks": clocks, "graph": use_graph}
 
-    # ---- end to end through the public API with HOST buffers: every step copies its input state from pinned host
-    # memory (H2D), runs marut_max_dt + the three stages, and copies the result back (D2H).  Two independent lanes
-    # (own handle, own device buffers, own stream) alternate steps, so the D2H of one step overlaps the H2D of the
-    # next (PCIe is full duplex); every step still pays both copies inside the timed region.
+
+def roofline_of(w, r, clocks):
+    mesh, args = w.mesh, w.args
+    peak, peak_src = measured_peaks()
+    n_dof = mesh.n_dof
+    stage_ms_avg = sum(r["stage_ms"]) / len(r["stage_ms"])
+    b_alg = algorithmic_bytes_per_dof_stage(mesh, w.affine)
+    achieved = b_alg * n_dof / (stage_ms_avg * 1e-3) / 1e9
+    prof = {}
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # per-launch figures from the committed ncu captures
+    if os.path.exists(tpath):
+        try:
+            prof = json.load(open(tpath))
+        except Exception:
+            prof = {}
+    roof = {"bound": "hbm", "kernel": ("marut_ssprk_stage: " if args.sync_dt else "marut_ssprk_stage_dev: ") + w.kernel_label(),
+            "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": prof.get(w.name),
+            "traffic_source": "profiles/traffic.json (ncu --set full capture of the same command, committed; not measured in this run)",
+            "peak_source": peak_src, "bytes_per_dof_stage": b_alg, "stage_ms_avg": stage_ms_avg,
+            "stage_ms_by_stage": [sum(r["stage_ms"][k::3]) / len(r["stage_ms"][k::3]) for k in range(3)],
+            "frac_of_8TBs_nominal": achieved / 8000.0}
+    if mesh.physics == 1:
+        roof["single_sweep_bytes_per_dof_stage"] = single_sweep_bytes_per_dof_stage(mesh, w.affine)
+        roof["frac_vs_single_sweep_bytes"] = roof["single_sweep_bytes_per_dof_stage"] * n_dof / (stage_ms_avg * 1e-3) / 1e9 / peak
+    if mesh.physics == 2 or getattr(mesh, "volume_form", 0):
+        # ALU-bound (chemistry / two-point volume fluxes): executed FP64 flops per stage from the committed ncu capture over the live time
+        flops = prof.get(w.name + "_fp64_flops_per_stage")
+        pk = fp64_peak_tflops((clocks or {}).get("sm_max_mhz") or 1965.0)
+        ach = flops / (stage_ms_avg * 1e-3) / 1e12 if flops else None
+        roof.update({"bound": "alu", "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": (ach / pk) if ach else None,
+                     "peak_source": "derived: 148 SMs x 64 FP64 FMA/clk x 2 x max SM clock (DESIGN.md section 7)",
+                     "hbm_frac": achieved / peak})
+    return roof
+
+
+def measure_e2e(w, args, barrier, mb):
+    """end to end through the public API with HOST buffers: every step copies its input state from pinned host memory
+    (H2D), runs marut_max_dt_async + the three stages, and copies the result back (D2H).  Two independent lanes (own
+    handle, own device buffers, own stream) alternate steps, so the D2H of one step overlaps the H2D of the next (PCIe
+    is full duplex); every step still pays both copies inside the timed region."""
+    import numpy as np
+
+    torch, mesh, sc, cfl = w.torch, w.mesh, w.sc, w.case.cfl
     lanes = []
     for k in range(2):
         st = torch.cuda.Stream()
-        g = gm if k == 0 else mb.MarutMesh(mesh)
-        lanes.append({"st": st, "gm": g, "u": torch.empty_like(u), "ua": torch.empty_like(u), "ub": torch.empty_like(u),
-                      "out": torch.empty_like(u0_host).pin_memory(),
-                      "dt": torch.zeros(1, dtype=torch.float64, device=u.device), "dt_out": torch.zeros(1, dtype=torch.float64).pin_memory()})
+        g = w.gm if k == 0 else mb.MarutMesh(mesh)
+        lanes.append({"st": st, "gm": g, "u": torch.empty_like(w.u), "ua": torch.empty_like(w.u), "ub": torch.empty_like(w.u),
+                      "out": torch.empty_like(w.u0_host).pin_memory(),
+                      "dt": torch.zeros(1, dtype=torch.float64, device=w.u.device), "dt_out": torch.zeros(1, dtype=torch.float64).pin_memory()})
         if sc:
-            lanes[k]["alpha"] = alpha if k == 0 else torch.zeros_like(alpha)
+            lanes[k]["alpha"] = w.alpha if k == 0 else torch.zeros_like(w.alpha)
             g.set_blend(lanes[k]["alpha"])
 
     def e2e_step(k):
         L = lanes[k % 2]
         with torch.cuda.stream(L["st"]):
-            L["u"].copy_(u0_host, non_blocking=True)
+            L["u"].copy_(w.u0_host, non_blocking=True)
             g = L["gm"]
             if args.sync_dt:
                 dt = g.max_dt(L["u"], cfl)
@@ -409,56 +516,95 @@ def run_cuda(args):
     if not np.isfinite(lanes[0]["out"].sum().item()):
         raise RuntimeError("end-to-end result is not finite")
     lanes[1]["gm"].close()
+    return e2e_ms
 
-    ms, e2e_ms = max_over_ranks([ms, e2e_ms], world, device="cuda")
-    value = aggregate_value(n_dof, args.steps, world, ms)
-    e2e_value = aggregate_value(n_dof, args.steps, world, e2e_ms)
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2605_26388_b200 as mb
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def summary(w, r):
+        n_dof, K = w.mesh.n_dof, args.steps
+        return {"workload": workload_name(w.case), "value": aggregate_value(n_dof, K, world, r["ms_block_median"]), "unit": UNIT,
+                "ms_per_step": r["ms_block_median"] / K, "ms_per_step_min": r["ms_blocks_min"] / K, "ms_per_step_max": r["ms_blocks_max"] / K,
+                "ms_per_step_eager": r["eager_ms_block"] / K, "repeats": r["repeats"], "timed_region_ms": r["timed_region_ms"],
+                "step_replayed_as_cuda_graph": r["graph"], "cfl": w.case.cfl, "restart_from_u0_every_steps": w.case.steps,
+                "affine": bool(w.affine), "gpu_launches_per_step": r["launches_per_block"] / K,
+                "roofline": roofline_of(w, r, r["clocks"]), "clocks": r["clocks"]}
+
+    w = Workload(args.workload, args, torch, mb)
+    r = measure(w, args, barrier, world, rank, local)
+    e2e_ms = measure_e2e(w, args, barrier, mb)
+    e2e_ms = max_over_ranks([e2e_ms], world, device="cuda")[0]
+    mesh, n_dof, K = w.mesh, w.mesh.n_dof, args.steps
+    main_sum = summary(w, r)
+    value = main_sum["value"]
+    e2e_value = aggregate_value(n_dof, K, world, e2e_ms)
+    w.gm.close()
+    del w
+    torch.cuda.empty_cache()
+
+    # the other configs of BASELINE.json, same protocol, device-resident figure only (N = 1, default workload only)
+    others = {}
+    if world == 1 and args.workload == "c2" and not args.no_configs:
+        for name in ("c1", "c3", "c4w", "c5"):
+            try:
+                wo = Workload(name, args, torch, mb)
+                ro = measure(wo, args, barrier, world, rank, local)
+                others[name] = summary(wo, ro)
+                wo.gm.close()
+                del wo
+                torch.cuda.empty_cache()
+            except Exception as exc:                      # a config that cannot run is reported, never hidden
+                others[name] = {"error": f"{type(exc).__name__}: {exc}"}
 
     if rank == 0:
-        peak, peak_src = measured_peaks()
-        b_alg = algorithmic_bytes_per_dof_stage(mesh, affine)
-        achieved = b_alg * n_dof / (stage_ms_avg * 1e-3) / 1e9
-        prof = {}
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")   # per-launch figures from the committed ncu captures
-        if os.path.exists(tpath):
-            try:
-                prof = json.load(open(tpath))
-            except Exception:
-                prof = {}
-        kernels = {0: ("stage_split_kernel (fused Euler stage, split-form volume integral" + (" blended with the sub-cell FV residual)" if sc else ")")) if getattr(mesh, "volume_form", 0) else ("mortar_flux3d_kernel + stage_node_kernel (fused Euler stage, 3-D mortar instantiation)" if (mesh.dim == 3 and len(mesh.mortar)) else "stage_node_kernel (fused Euler stage)"), 1: "gradient_kernel + stage_phys_kernel (BR1 gradient sweep + fused NS stage)",
-                   2: "eos_kernel + stage_phys_kernel (mixture temperature + fused reacting stage)"}[mesh.physics]
-        roof = {"bound": "hbm", "kernel": ("marut_ssprk_stage: " if args.sync_dt else "marut_ssprk_stage_dev: ") + kernels, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": prof.get(args.workload), "peak_source": peak_src, "bytes_per_dof_stage": b_alg,
-                "stage_ms_avg": stage_ms_avg, "frac_of_8TBs_nominal": achieved / 8000.0}
-        if mesh.physics == 1:
-            roof["single_sweep_bytes_per_dof_stage"] = single_sweep_bytes_per_dof_stage(mesh, affine)
-            roof["frac_vs_single_sweep_bytes"] = roof["single_sweep_bytes_per_dof_stage"] * n_dof / (stage_ms_avg * 1e-3) / 1e9 / peak
-        if mesh.physics == 2 or getattr(mesh, "volume_form", 0):
-            # ALU-bound (chemistry / two-point volume fluxes): executed FP64 flops per stage from the committed ncu capture over the live time
-            flops = prof.get(args.workload + "_fp64_flops_per_stage")
-            pk = fp64_peak_tflops((clocks or {}).get("sm_max_mhz") or 1965.0)
-            ach = flops / (stage_ms_avg * 1e-3) / 1e12 if flops else None
-            roof.update({"bound": "alu", "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": (ach / pk) if ach else None,
-                         "peak_source": "derived: 148 SMs x 64 FP64 FMA/clk x 2 x max SM clock (DESIGN.md section 7)",
-                         "hbm_frac": achieved / peak})
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+                "ms_per_step": main_sum["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": workload_name(case), "parallelism": "replicas only" if world > 1 else "1 GPU",
+                "config": {"workload": main_sum["workload"], "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": f"inputs larger than L2 ({3 * n_dof * 8 / 1e6:.0f} MB of state buffers vs 126 MB)"
                                  if 3 * n_dof * 8 > 126e6 else "state fits L2 (launch/latency-bound case; no flush)",
-                           "step": ("marut_max_dt" if args.sync_dt else "marut_max_dt_async (dt stays on the device)") + (" + 3 x (marut_shock_indicator + blended marut_ssprk_stage + marut_positivity_floor)" if sc else " + 3 x marut_ssprk_stage"), "cfl": cfl, "restart_from_u0_every_steps": case.steps, "affine": bool(affine)},
-                "clocks": clocks,
+                           "step": ("marut_max_dt" if args.sync_dt else "marut_max_dt_async (dt stays on the device)")
+                                   + (" + 3 x (marut_shock_indicator + blended marut_ssprk_stage + marut_positivity_floor)"
+                                      if main_sum["roofline"]["kernel"].endswith("FV residual)") else " + 3 x marut_ssprk_stage"),
+                           "timing": f"median of {main_sum['repeats']} blocks of exactly {K} steps each (timed region "
+                                     f"{main_sum['timed_region_ms']:.0f} ms), every block one CUDA-event pair"
+                                     + (", the step replayed as a CUDA graph" if main_sum["step_replayed_as_cuda_graph"] else ", eager launches"),
+                           "cfl": main_sum["cfl"], "restart_from_u0_every_steps": main_sum["restart_from_u0_every_steps"],
+                           "affine": main_sum["affine"]},
+                "ms_per_step_min": main_sum["ms_per_step_min"], "ms_per_step_max": main_sum["ms_per_step_max"],
+                "ms_per_step_eager": main_sum["ms_per_step_eager"], "repeats": main_sum["repeats"],
+                "timed_region_ms": main_sum["timed_region_ms"],
+                "clocks": main_sum["clocks"],
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n_dof * 8, "d2h_bytes_per_step": n_dof * 8 + 8,
-                        "ms_per_step": e2e_ms / args.steps,
+                        "ms_per_step": e2e_ms / K,
                         "how": "pinned host buffers; two alternating lanes (handle + stream each) so that the D2H of a step overlaps the H2D of the next"},
-                "gpu_launches": launches,
-                "roofline": roof}
+                "gpu_launches": int(round(main_sum["gpu_launches_per_step"] * K)),
+                "roofline": main_sum["roofline"]}
+        if others:
+            line["configs"] = others
         if world == 1 and not args.no_cpu_baseline:
             o = oracle_sample(args.workload, args.cpu_seconds)
-            line["cpu_baseline"] = {"value": o["value"], "unit": UNIT, "cores": o["cores"], "kind": "oracle", "sample": o["sample"]}
+            line["cpu_baseline"] = {"value": o["value"], "value_1core": o["value_1core"], "unit": UNIT, "cores": o["cores"], "kind": "oracle",
+                                    "sample": o["sample"]}
         print(json.dumps(line), flush=True)
-    gm.close()
     if world > 1:
         dist.destroy_process_group()
 
@@ -466,13 +612,16 @@ def run_cuda(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--workload", default="c2", choices=sorted(ORACLE_SAMPLE_CELLS))
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sync-dt", action="store_true", help="host-synchronised marut_max_dt every step instead of the device-resident dt")
+    ap.add_argument("--no-graph", action="store_true", help="eager launches in the timed blocks instead of CUDA-graph replay")
+    ap.add_argument("--no-configs", action="store_true", help="skip the other BASELINE.json configs (c1, c3, c4w, c5) of the default run")
+    ap.add_argument("--min-ms", type=float, default=1000.0, help="repeat the K-step block until the timed region is at least this long")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3

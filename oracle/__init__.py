@@ -413,3 +413,7 @@ def ssprk3_scalar(y0, lam, c2, t0, dt):
 
 def num_threads():
     return lib().oracle_num_threads()
+
+
+def set_num_threads(n):
+    lib().oracle_set_num_threads(int(n))

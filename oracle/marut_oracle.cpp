@@ -1401,5 +1401,13 @@ int oracle_num_threads(void) {
   return 1;
 #endif
 }
+// number of OpenMP threads of the element loops from now on (bench.py's 1-core / all-core timings; no arithmetic)
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n >= 1) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
 
 }  // extern "C"
