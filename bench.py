@@ -310,7 +310,11 @@ class Workload:
         # dt stays on the device (marut_max_dt_async -> marut_ssprk_stage_dev: the same dt and the same stage results bit
         # for bit, tests/test_gpu_async_dt.py), so the host queues the whole step without waiting for the CFL reduction
         self.dt_dev = torch.zeros(1, dtype=torch.float64, device=self.u.device)
+        self.dts = torch.zeros(2, dtype=torch.float64, device=self.u.device)   # fused step: dt ping-pong
         self.graphs = None
+        # the step the graph blocks replay: marut_ssprk33_step_cfl (the next step's CFL reduction inside the last stage's
+        # kernel where the stage kernel supports it) unless the workload interleaves other calls with the stages
+        self.fused_step = not (self.sc or args.sync_dt or args.no_graph or args.no_fused_cfl)
 
     def kernel_label(self):
         m = self.mesh
@@ -347,13 +351,29 @@ class Workload:
             if sc:
                 gm.positivity_floor(uout)
 
+    def _step_cfl(self, j):
+        """step j of a cycle through marut_ssprk33_step_cfl: j = 0 restarts from u0 (copy + CFL reduction), then the two
+        device doubles alternate as dt_in / dt_out"""
+        gm, cfl, d = self.gm, self.case.cfl, self.dts
+        if j == 0:
+            self.u.copy_(self.u0_dev)
+            gm.max_dt_async(self.u, cfl, d[0:1])
+            gm.ssprk33_step_cfl(self.u, self.ua, self.ub, cfl, d[0:1], d[1:2])
+        elif j % 2 == 1:
+            gm.ssprk33_step_cfl(self.u, self.ua, self.ub, cfl, d[1:2], d[0:1])
+        else:
+            gm.ssprk33_step_cfl(self.u, self.ua, self.ub, cfl, d[0:1], d[1:2])
+
     def step(self, ev=None, graph=False):
-        first = self.counter % self.case.steps == 0
+        j = self.counter % self.case.steps
         self.counter += 1
         if graph and self.graphs is not None:
-            self.graphs[0 if first else 1].replay()
+            if self.fused_step:
+                self.graphs[0 if j == 0 else (1 if j % 2 == 1 else 2)].replay()
+            else:
+                self.graphs[0 if j == 0 else 1].replay()
         else:
-            self._step(self.u0_dev if first else self.u, ev)
+            self._step(self.u0_dev if j == 0 else self.u, ev)
 
     def capture(self):
         """the two variants of the step (from u0 / from u) as CUDA graphs: the library only launches on the stream it
@@ -362,11 +382,21 @@ class Workload:
             return
         torch = self.torch
         gs = []
-        for src in (self.u0_dev, self.u):
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g):
-                self._step(src)
-            gs.append(g)
+        if self.fused_step:
+            for j in (0, 1, 2):
+                self._step_cfl(j)                      # warm (function attributes of the fused instantiation)
+            torch.cuda.synchronize()
+            for j in (0, 1, 2):
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g):
+                    self._step_cfl(j)
+                gs.append(g)
+        else:
+            for src in (self.u0_dev, self.u):
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g):
+                    self._step(src)
+                gs.append(g)
         self.graphs = gs
 
     def block(self, K, graph, ev=None):
@@ -408,6 +438,7 @@ def measure(w, args, barrier, world, rank, local):
     if rank == 0:
         sampler.start()
     use_graph = w.graphs is not None
+    w.counter = 0                                       # the graph blocks start a cycle (restart from u0)
     blocks = []
     first = w.block(K, graph=use_graph)
     barrier()
@@ -544,7 +575,7 @@ def run_cuda(args):
         return {"workload": workload_name(w.case), "value": aggregate_value(n_dof, K, world, r["ms_block_median"]), "unit": UNIT,
                 "ms_per_step": r["ms_block_median"] / K, "ms_per_step_min": r["ms_blocks_min"] / K, "ms_per_step_max": r["ms_blocks_max"] / K,
                 "ms_per_step_eager": r["eager_ms_block"] / K, "repeats": r["repeats"], "timed_region_ms": r["timed_region_ms"],
-                "step_replayed_as_cuda_graph": r["graph"], "cfl": w.case.cfl, "restart_from_u0_every_steps": w.case.steps,
+                "step_replayed_as_cuda_graph": r["graph"], "fused_cfl_step": bool(r["graph"] and w.fused_step), "cfl": w.case.cfl, "restart_from_u0_every_steps": w.case.steps,
                 "affine": bool(w.affine), "gpu_launches_per_step": r["launches_per_block"] / K,
                 "roofline": roofline_of(w, r, r["clocks"]), "clocks": r["clocks"]}
 
@@ -581,9 +612,12 @@ def run_cuda(args):
                 "config": {"workload": main_sum["workload"], "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": f"inputs larger than L2 ({3 * n_dof * 8 / 1e6:.0f} MB of state buffers vs 126 MB)"
                                  if 3 * n_dof * 8 > 126e6 else "state fits L2 (launch/latency-bound case; no flush)",
-                           "step": ("marut_max_dt" if args.sync_dt else "marut_max_dt_async (dt stays on the device)")
-                                   + (" + 3 x (marut_shock_indicator + blended marut_ssprk_stage + marut_positivity_floor)"
-                                      if main_sum["roofline"]["kernel"].endswith("FV residual)") else " + 3 x marut_ssprk_stage"),
+                           "step": ("marut_ssprk33_step_cfl: three fused stages, the CFL reduction of the next step inside the last "
+                                    "stage's kernel (dt stays on the device; every restart from u0 adds a device copy and one marut_max_dt_async)"
+                                    if main_sum["fused_cfl_step"] else
+                                    ("marut_max_dt" if args.sync_dt else "marut_max_dt_async (dt stays on the device)")
+                                    + (" + 3 x (marut_shock_indicator + blended marut_ssprk_stage + marut_positivity_floor)"
+                                       if main_sum["roofline"]["kernel"].endswith("FV residual)") else " + 3 x marut_ssprk_stage")),
                            "timing": f"median of {main_sum['repeats']} blocks of exactly {K} steps each (timed region "
                                      f"{main_sum['timed_region_ms']:.0f} ms), every block one CUDA-event pair"
                                      + (", the step replayed as a CUDA graph" if main_sum["step_replayed_as_cuda_graph"] else ", eager launches"),
@@ -620,6 +654,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sync-dt", action="store_true", help="host-synchronised marut_max_dt every step instead of the device-resident dt")
     ap.add_argument("--no-graph", action="store_true", help="eager launches in the timed blocks instead of CUDA-graph replay")
+    ap.add_argument("--no-fused-cfl", action="store_true", help="graph blocks replay marut_max_dt_async + 3 x marut_ssprk_stage_dev instead of marut_ssprk33_step_cfl")
     ap.add_argument("--no-configs", action="store_true", help="skip the other BASELINE.json configs (c1, c3, c4w, c5) of the default run")
     ap.add_argument("--min-ms", type=float, default=1000.0, help="repeat the K-step block until the timed region is at least this long")
     args = ap.parse_args()

@@ -214,6 +214,16 @@ marut_status marut_positivity_floor(marut_mesh *mesh, double *u, double rho_min,
  *                       for, a node whose Newton iteration does not converge gets NaN species densities. */
 marut_status marut_ssprk33_step(marut_mesh *mesh, double *u, double *const *scratch, double dt, const double *dt_dev,
                                 void *cuda_stream);
+/* One SSP-RK33 step with the time step read from dt_in (DEVICE double) that also leaves the CFL step of the NEW state
+ * in dt_out (DEVICE double, != dt_in): dt_out = marut_max_dt_async(u^{n+1}, cfl), bit for bit.  Where the stage kernel
+ * supports it (MARUT_EULER, strong form, affine meshes large enough for the line kernel) the maximum wave speed of
+ * u^{n+1} (eq. 18) is reduced inside the last stage's kernel from the values it writes -- no
+ * separate pass over u (8 B/DOF saved per step) -- and the CTA that finishes last evaluates eq. 18;
+ * elsewhere the call runs the separate reduction after the last stage.  A step loop alternates two DEVICE doubles:
+ *   marut_max_dt_async(u, cfl, dt[0]); for k = 0, 1, ...: marut_ssprk33_step_cfl(u, scratch, cfl, dt[k&1], dt[(k+1)&1]).
+ * A non-finite or non-positive wave speed poisons dt_out with NaN (as marut_max_dt_async).  Asynchronous. */
+marut_status marut_ssprk33_step_cfl(marut_mesh *mesh, double *u, double *const *scratch, double cfl, const double *dt_in,
+                                    double *dt_out, void *cuda_stream);
 marut_status marut_ssprk54_step(marut_mesh *mesh, double *u, double *const *scratch, double dt, const double *dt_dev,
                                 void *cuda_stream);
 marut_status marut_strang_step(marut_mesh *mesh, double *u, double *const *scratch, double dt, int *sweeps_out,

@@ -109,27 +109,58 @@ def lib():
     return _lib
 
 
-_LIB_FMA = os.path.join(_HERE, "libmarut_oracle_fma.so")
-_lib_fma = None
+_LIB_LD = os.path.join(_HERE, "libmarut_oracle_ld.so")
+_lib_ld = None
 
 
-def lib_fma():
-    """The SAME source compiled with FMA contraction allowed (-ffp-contract=fast -mfma): a legal re-rounding of
-    the oracle's own arithmetic.  Used only to measure how far an oracle result moves under the one difference
-    the north star allows between the two sides ("reduction-order differences", FMA contraction) -- the
-    full-size parity tolerance of DESIGN.md reading T1.  None when the host CPU has no FMA unit."""
-    global _lib_fma
-    if _lib_fma is None:
-        try:
-            if "fma" not in open("/proc/cpuinfo").read().split("flags", 1)[1].split("\n", 1)[0].split():
-                return None
-        except Exception:
+class _MeshDescLD(C.Structure):
+    _fields_ = [("dim", C.c_int), ("N", C.c_int), ("n_elem", C.c_long), ("node_xyz", C.c_void_p),
+                ("n_iface", C.c_long), ("iface", C.c_void_p), ("n_mortar", C.c_long), ("mortar", C.c_void_p),
+                ("n_bface", C.c_long), ("bface", C.c_void_p), ("n_bc", C.c_int), ("bc_state", C.c_void_p),
+                ("physics", C.c_int), ("gamma", C.c_longdouble), ("mu", C.c_longdouble), ("Pr", C.c_longdouble),
+                ("mech", C.c_void_p)]
+
+
+def lib_ld():
+    """The SAME source compiled with -DORACLE_LONG_DOUBLE: every `double` of the oracle, interface included, becomes an
+    x87 80-bit long double (64-bit mantissa, unit round-off 5.4e-20).  Only oracle_mesh_create / oracle_rhs /
+    oracle_mesh_destroy are bound (rhs_ld below).  It is the reference against which the round-off of the FP64 oracle and
+    of the GPU path is measured at full size (reading T1): |fp64 - ld| is a side's own rounding error.  None
+    when numpy's longdouble is not the 80-bit type (non-x86 hosts)."""
+    global _lib_ld
+    if _lib_ld is None:
+        if np.finfo(np.longdouble).nmant != 63 or C.sizeof(C.c_longdouble) != np.dtype(np.longdouble).itemsize:
             return None
-        if not os.path.exists(_LIB_FMA) or os.path.getmtime(_LIB_FMA) < os.path.getmtime(_SRC):
-            cmd = ["g++", "-O2", "-ffp-contract=fast", "-mfma", "-fopenmp", "-std=c++17", "-shared", "-fPIC", _SRC, "-o", _LIB_FMA]
+        if not os.path.exists(_LIB_LD) or os.path.getmtime(_LIB_LD) < os.path.getmtime(_SRC):
+            cmd = ["g++", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c++17", "-shared", "-fPIC", "-DORACLE_LONG_DOUBLE", _SRC, "-o", _LIB_LD]
             subprocess.run(cmd, check=True)
-        _lib_fma = _setup(C.CDLL(_LIB_FMA))
-    return _lib_fma
+        L = C.CDLL(_LIB_LD)
+        L.oracle_mesh_create.restype = C.c_void_p
+        L.oracle_mesh_create.argtypes = [C.c_void_p]
+        L.oracle_mesh_destroy.argtypes = [C.c_void_p]
+        L.oracle_rhs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longdouble]
+        _lib_ld = L
+    return _lib_ld
+
+
+def rhs_ld(mesh, u):
+    """L(u) of the long-double build for a non-reacting mesh with the strong form, returned as float64 (the rounding
+    of the long-double result to double is 1.1e-16 relative to each entry: exact for the purpose)"""
+    L = lib_ld()
+    assert L is not None and mesh.mech is None and not getattr(mesh, "volume_form", 0)
+    ld = np.longdouble
+    keep = [np.ascontiguousarray(mesh.node_xyz, dtype=ld), _i32(mesh.iface), _i32(mesh.mortar), _i32(mesh.bface),
+            np.ascontiguousarray(mesh.bc_state, dtype=ld)]
+    d = _MeshDescLD(mesh.dim, mesh.N, mesh.n_elem, _p(keep[0]), len(keep[1]), _p(keep[1]), len(keep[2]), _p(keep[2]),
+                    len(keep[3]), _p(keep[3]), len(keep[4]), _p(keep[4]), mesh.physics, mesh.gamma, mesh.mu, mesh.Pr, None)
+    h = L.oracle_mesh_create(C.addressof(d))
+    try:
+        ul = np.ascontiguousarray(u, dtype=ld)
+        out = np.zeros_like(ul)
+        L.oracle_rhs(h, _p(ul), _p(out), 0.0)
+        return out.astype(np.float64)
+    finally:
+        L.oracle_mesh_destroy(h)
 
 
 def _p(a):

@@ -39,6 +39,16 @@
 #include <omp.h>
 #endif
 
+// Extended precision of the 1-D operator construction (O1).
+typedef long double ExtReal;
+// -DORACLE_LONG_DOUBLE: this same source with EVERY `double` an x87 80-bit long double (64-bit mantissa), interface
+// arrays and scalars included.  Test infrastructure only (oracle.lib_ld()): the reference against which the round-off
+// of the FP64 oracle and of the GPU path is measured at full size (reading T1).  Literals stay double
+// constants; the few that are not exact (1/3, 2/3, ...) carry a relative error of 1e-16, far below what is measured.
+#ifdef ORACLE_LONG_DOUBLE
+#define double long double
+#endif
+
 namespace {
 
 constexpr double R_UNIVERSAL = 8.31446261815324;   // J/(mol K)
@@ -76,7 +86,7 @@ struct Ops {
 // Evaluated in extended precision (long double) and rounded once, so that x, w and D are the
 // correctly rounded doubles of their exact values (independent of the formula used to get them).
 static Ops make_ops(int N) {
-  typedef long double LD;
+  typedef ExtReal LD;
   Ops o; o.N = N; o.n = N + 1;
   const int n = o.n;
   std::vector<LD> x(n), w(n), D((size_t)n * n, 0);
@@ -973,7 +983,7 @@ static int chem_implicit_node(const Mech &k, double *Y, double e_int, double dt)
     double R[MAXV], A[MAXV][MAXV + 1];
     implicit_residual(k, Y, Yn, dt, e_int, R);
     for (int c = 0; c < ns; ++c) {
-      const double eps = std::max(1e-7 * std::fabs(Y[c]), 1e-12);
+      const double eps = std::max<double>(1e-7 * std::fabs(Y[c]), 1e-12);
       double Yp[MAXV], Rp[MAXV];
       for (int s = 0; s < ns; ++s) Yp[s] = Y[s];
       Yp[c] += eps;
@@ -1110,7 +1120,7 @@ static double max_dt(const Mesh &m, const double *u, double cfl, double *lam_out
   const double P2 = 2.0 * m.N + 1.0;
   double dt = cfl * m.dx_min / (P2 * lam);
   if (m.physics == NAVIER_STOKES) {
-    double numax = nu * std::max(1.0, 1.0 / m.Pr);
+    double numax = nu * std::max<double>(1.0, 1.0 / m.Pr);
     dt = std::min(dt, cfl * m.dx_min * m.dx_min / (P2 * P2 * numax));
   }
   return dt;

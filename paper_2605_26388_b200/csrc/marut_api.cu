@@ -56,13 +56,14 @@ struct marut_mesh {
   double *d_mortar_mat = nullptr;
   double *d_bc = nullptr;
   double *d_S = nullptr;     // NS scratch: stress tensor + heat flux from the BR1 gradient, [e][d(d+1)/2 + d][node]
-  double *d_T = nullptr;     // reacting temperature scratch
+  double *d_T = nullptr;     // reacting scratch of eos_kernel: [e][2 + n_species][node] = p, a, omega_s
   MechDev *d_mech = nullptr;
   double *d_Vinv = nullptr;  // [n][n] nodal -> orthonormal Legendre modal (shock indicator)
   double *d_araw = nullptr;  // [ne] unsmoothed blending coefficient (allocated on first use)
   const double *d_alpha = nullptr;  // caller-owned blending field of eq. 11 (marut_set_blend), or NULL
   double *d_subn = nullptr;  // curved meshes: sub-cell normals [e][l][c][node] (allocated by the first marut_set_blend)
   unsigned long long *d_red = nullptr;
+  unsigned long long *d_red_next = nullptr;   // [4] reduction words of the fused CFL step (zero between uses)
   unsigned long long *h_red = nullptr;  // pinned
   std::atomic<long> launches{0};   // kernels launched through this handle (introspection; any thread)
   int stage_kernel_pref = 0;       // marut_debug_stage_kernel: 0 automatic, 1 thread-per-node kernel, 2 line kernel where eligible
@@ -240,6 +241,7 @@ extern "C" void marut_mesh_destroy(marut_mesh *m) {
   cudaDeviceSynchronize();
   cudaFree(m->d_metric); cudaFree(m->d_fnorm); cudaFree(m->d_conn); cudaFree(m->d_mortar_fine); cudaFree(m->d_mortar_info); cudaFree(m->d_mflux); cudaFree(m->d_mortar_mat);
   cudaFree(m->d_Vinv); cudaFree(m->d_araw); cudaFree(m->d_subn); cudaFree(m->d_bc); cudaFree(m->d_S); cudaFree(m->d_T); cudaFree(m->d_mech); cudaFree(m->d_red);
+  cudaFree(m->d_red_next);
   if (m->h_red) cudaFreeHost(m->h_red);
   delete m;
 }
@@ -399,6 +401,8 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   if (d->n_bc) CUDA_TRY(cudaMemcpy(m->d_bc, d->bc_state, (size_t)d->n_bc * m->nvar * sizeof(double), cudaMemcpyHostToDevice));
   CUDA_TRY(cudaMalloc(&m->d_red, 5 * sizeof(unsigned long long)));   // [0..2] marut_max_dt, [3] marut_chem_implicit, [4] marut_positivity_floor
   CUDA_TRY(cudaMallocHost(&m->h_red, 5 * sizeof(unsigned long long)));
+  CUDA_TRY(cudaMalloc(&m->d_red_next, 4 * sizeof(unsigned long long)));
+  CUDA_TRY(cudaMemset(m->d_red_next, 0, 4 * sizeof(unsigned long long)));
 
   // ---- metric terms on the device
   const int MD = dim * dim + 1;
@@ -453,7 +457,7 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
 
   // ---- scratch
   if (m->physics == MARUT_NAVIER_STOKES) CUDA_TRY(cudaMalloc(&m->d_S, (size_t)ne * (dim * (dim + 1) / 2 + dim) * nn * sizeof(double)));
-  if (m->physics == MARUT_REACTING_EULER) CUDA_TRY(cudaMalloc(&m->d_T, (size_t)ne * nn * sizeof(double)));
+  if (m->physics == MARUT_REACTING_EULER) CUDA_TRY(cudaMalloc(&m->d_T, (size_t)ne * (2 + m->nsp) * nn * sizeof(double)));
 
   if (dim == 3 && d->n_mortar > 0 && !m->affine)
     return fail(MARUT_EINVAL, "3-D mortar faces need an affine mesh");
@@ -492,8 +496,16 @@ extern "C" marut_status marut_mesh_create(const marut_mesh_desc *desc, marut_mes
 // ------------------------------------------------------------------------------------ operator / stage
 static bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
+// fused CFL reduction of u_out in the stage kernel (marut_ssprk33_step_cfl): requested with cfl > 0 and dt_next; *done
+// tells the caller whether the kernel that ran took it (else the caller runs marut_max_dt_async on u_out)
+struct FuseCfl {
+  double cfl = 0.0;
+  double *dt_next = nullptr;
+  bool done = false;
+};
+
 static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc, const double *u_n, const double *u_in,
-                                 double *u_out, cudaStream_t st, const double *dt_dev = nullptr) {
+                                 double *u_out, cudaStream_t st, const double *dt_dev = nullptr, FuseCfl *fuse = nullptr) {
   if (m->physics == MARUT_NAVIER_STOKES) {
     GradParams G;
     G.u = u_in; G.S = m->d_S; G.metric = m->d_metric; G.conn = m->d_conn;
@@ -506,8 +518,8 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   if (m->physics == MARUT_REACTING_EULER) {
     const long total = m->ne * m->nn;
     const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, (long)m->num_sms * 16);
-    if (m->dim == 2) eos_kernel<2, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn);
-    else eos_kernel<3, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn);
+    if (m->dim == 2) eos_kernel<2, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn, m->explicit_source);
+    else eos_kernel<3, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn, m->explicit_source);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(MARUT_ECUDA, "eos kernel: %s", cudaGetErrorString(e));
     m->launches++;
@@ -518,6 +530,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.bc_state = m->d_bc; P.S = m->d_S; P.Taux = m->d_T; P.mech = m->d_mech;
   P.ca = ca; P.cb = cb; P.cc = cc; P.dt_dev = dt_dev;
   P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne; P.num_sms = m->num_sms;
+  P.red_next = nullptr; P.dt_next = nullptr; P.cfl = 0.0; P.dx_min = m->dx_min; P.P2 = 2.0 * m->N + 1.0;
   memcpy(P.D, m->D, sizeof(P.D));
   P.mflux = m->d_mflux;
   if (m->dim == 3 && m->n_mortar > 0) {
@@ -541,8 +554,12 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
         // affine meshes with conforming / prescribed-state / 2-D mortar faces: the persistent TMA-fed line kernel;
         // curved meshes, outflow / slip-wall faces and 3-D mortars: the thread-per-node kernel
         e = cudaErrorNotSupported;
-        if (m->affine && !P.bc_kinds && m->stage_kernel_pref != 1)
+        if (m->affine && !P.bc_kinds && m->stage_kernel_pref != 1) {
+          if (fuse && fuse->dt_next) { P.red_next = m->d_red_next; P.dt_next = fuse->dt_next; P.cfl = fuse->cfl; }
           e = launch_stage_pencil(m->dim, m->np, m->n_mortar > 0, m->stage_kernel_pref == 2, P, st);
+          if (fuse) fuse->done = (e == cudaSuccess) && P.red_next != nullptr;
+          P.red_next = nullptr;
+        }
         if (e == cudaErrorNotSupported)
           e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
       }
@@ -747,6 +764,8 @@ extern "C" marut_status marut_chem_implicit(marut_mesh *m, double *u, double dt,
   return MARUT_OK;
 }
 
+extern "C" marut_status marut_max_dt_async(marut_mesh *m, const double *u, double cfl, double *dt_dev, void *stream);
+
 // ------------------------------------------------------------------------------------ whole time steps
 // The step compositions of the paper's integrators, so that a C caller gets them without re-typing a coefficient
 // table: SSP-RK33 (eq. 44-46, R10), SSP-RK54 (R19) and the Strang split of eq. 24.
@@ -786,6 +805,25 @@ extern "C" marut_status marut_ssprk33_step(marut_mesh *m, double *u, double *con
   if ((s = stage_any(m, 0.0, 1.0, 1.0, dt, dt_dev, u, u, ua, st)) != MARUT_OK) return s;
   if ((s = stage_any(m, 0.75, 0.25, 0.25, dt, dt_dev, u, ua, ub, st)) != MARUT_OK) return s;
   return stage_any(m, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, dt, dt_dev, u, ub, u, st);
+}
+
+extern "C" marut_status marut_ssprk33_step_cfl(marut_mesh *m, double *u, double *const *scratch, double cfl, const double *dt_in,
+                                               double *dt_out, void *stream) {
+  if (marut_status s = check_step_buffers(m, u, scratch, 2); s != MARUT_OK) return s;
+  if (!dt_in || !dt_out) return fail(MARUT_EINVAL, "NULL argument");
+  if (dt_in == dt_out) return fail(MARUT_EINVAL, "dt_out must not alias dt_in (CTAs of the last stage still read dt_in when the first ones finish)");
+  if (!(cfl > 0.0)) return fail(MARUT_EINVAL, "cfl must be positive");
+  cudaStream_t st = (cudaStream_t)stream;
+  double *ua = scratch[0], *ub = scratch[1];
+  marut_status s;
+  if ((s = run_operator(m, 0.0, 1.0, 1.0, u, u, ua, st, dt_in)) != MARUT_OK) return s;
+  if ((s = run_operator(m, 0.75, 0.25, 0.25, u, ua, ub, st, dt_in)) != MARUT_OK) return s;
+  FuseCfl f;
+  f.cfl = cfl;
+  f.dt_next = dt_out;
+  if ((s = run_operator(m, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, u, ub, u, st, dt_in, &f)) != MARUT_OK) return s;
+  if (!f.done) return marut_max_dt_async(m, u, cfl, dt_out, stream);   // stage kernels without the fused reduction
+  return MARUT_OK;
 }
 
 extern "C" marut_status marut_ssprk54_step(marut_mesh *m, double *u, double *const *scratch, double dt, const double *dt_dev,

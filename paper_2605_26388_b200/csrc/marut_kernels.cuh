@@ -179,11 +179,15 @@ __device__ __forceinline__ void load_mech(MechDev *dst_s, const MechDev *src_g) 
   __syncthreads();
 }
 
-// T[e][node] by Newton (a8)
+// Per-node thermochemistry of the reacting stage (a8, a9), evaluated ONCE per stage call ahead of the fused stage
+// kernel: T by Newton, then p = rho R T and the frozen sound speed (R12) and -- when the
+// explicit source is on -- the production rates omega_s (eq. 21-22).  aux[e][2 + NSP][node] = p, a, omega_1..NSP.
+// The stage kernel then needs no mechanism table, no exponentials and no Newton: it keeps the footprint of the Euler
+// stage (the chemistry is purely per node, "no inter-thread communication").
 template <int DIM, int NSP>
-__global__ void __launch_bounds__(256) eos_kernel(const double *__restrict__ u, double *__restrict__ Tout,
-                                                  const MechDev *__restrict__ mech_g, long ne, int nn) {
-  constexpr int NVAR = NSP + DIM + 1;
+__global__ void __launch_bounds__(256) eos_kernel(const double *__restrict__ u, double *__restrict__ aux,
+                                                  const MechDev *__restrict__ mech_g, long ne, int nn, int with_source) {
+  constexpr int NVAR = NSP + DIM + 1, NA = 2 + NSP;
   __shared__ MechDev mech;
   load_mech(&mech, mech_g);
   const long total = ne * nn;
@@ -193,7 +197,17 @@ __global__ void __launch_bounds__(256) eos_kernel(const double *__restrict__ u, 
     double U[NVAR];
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) U[v] = __ldg(u + (e * NVAR + v) * nn + p);
-    Tout[g] = temperature_newton<NSP>(mech, U, internal_energy<DIM, NSP>(U));
+    const double T = temperature_newton<NSP>(mech, U, internal_energy<DIM, NSP>(U));
+    const Prim<DIM> q = prim_mixture<DIM, NSP, true>(U, T, mech);
+    double *a = aux + e * NA * nn + p;
+    a[0] = q.p;
+    a[nn] = q.a;
+    if (with_source) {
+      double om[NSP];
+      production_rates<NSP>(mech, T, U, om);
+#pragma unroll
+      for (int s = 0; s < NSP; ++s) a[(2 + s) * nn] = om[s];
+    }
   }
 }
 

@@ -4,8 +4,9 @@
 // flux evaluation, balanced line-task derivative passes, densely mapped face tasks, last pass fused with the
 // lift + 1/J + source + SSP-RK combination.  Differences from the Euler instance: the derivative passes write
 // a separate result plane set (the flux planes stay intact because the viscous face tasks read the own
-// normal flux from them), the chemistry source goes through shared source planes, and the face tasks gather
-// the neighbour's BR1 gradient (NS) or temperature (reacting) as well.  Conforming interior faces only.
+// normal flux from them), and the face tasks gather the neighbour's BR1 gradient (NS) or pressure and sound speed
+// (reacting) as well.  Reacting: pressure, frozen sound speed and the chemistry source of every node come from the
+// aux array eos_kernel fills ahead of the stage, so this kernel carries no mechanism table.  Conforming interior faces only.
 //
 // Product code; shares nothing with oracle/.
 #pragma once
@@ -29,7 +30,7 @@ struct PhysCfg {
   static constexpr int KS = NP * NP, PS = NN | 1;            // plane strides (odd plane stride)
   static constexpr int NFP = DIM * NVAR * EB;                // flux planes
   static constexpr int NRP = NVAR * EB;                      // result planes
-  static constexpr int NSRC = (PHYS == PH_REACT) ? NSP * TILE : 0;
+  static constexpr int NSRC = 0;                             // (the chemistry source comes from eos_kernel's aux array)
   static constexpr int MDP = ((G::MD + DIM + 1) / 2) * 2;
   static constexpr size_t smem_doubles(bool affine) {
     return (size_t)(NFP + NRP) * PS + (size_t)NST * TILE + (size_t)NVAR * NTASK + NSRC + (affine ? EB * MDP : 0);
@@ -49,9 +50,7 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   double *Rsm = Fsm + C::NFP * PS;            // [NVAR][EB] result planes of the derivative passes
   double *Ust = Rsm + C::NRP * PS;            // [NVAR + 3][TILE]  U, 1/rho, p, a
   double *Lft = Ust + C::NST * TILE;          // [NVAR][NTASK]     lifts of the face nodes
-  double *Src = Lft + NVAR * NTASK;           // reacting: [NSP][TILE] chemistry source
-  double *Msm = Src + C::NSRC;                // affine: [EB][MDP] Ja, 1/J, |Ja^l|
-  __shared__ MechDev mech_s;
+  double *Msm = Lft + NVAR * NTASK;                // affine: [EB][MDP] Ja, 1/J, |Ja^l|
 
   const int tid = threadIdx.x;
   const long e0 = (long)blockIdx.x * EB;
@@ -64,11 +63,7 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   int2 cn0 = make_int2(0, 0);
   if (has0) cn0 = __ldg(&P.conn[(e0 + t0.el) * 2 * DIM + t0.f]);
 
-  if constexpr (PHYS == PH_REACT) {
-    const int *src = reinterpret_cast<const int *>(P.mech);
-    int *dst = reinterpret_cast<int *>(&mech_s);
-    for (int i = tid; i < (int)(sizeof(MechDev) / sizeof(int)); i += NT) dst[i] = src[i];
-  }
+  constexpr int NA = 2 + NSP;                 // reacting: planes of the aux array (p, a, omega_s)
   if constexpr (AFFINE) {
     for (int i = tid; i < nel * MDP; i += NT) {
       const int me = i / MDP, k = i - me * MDP;
@@ -78,15 +73,18 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   const int el = tid / NN, p = tid - el * NN;
   const long e = e0 + el;
   const bool active = (tid < TILE) && (el < nel);
-  double U[NVAR], T = 0.0;
+  double U[NVAR], pA = 0.0, aA = 0.0;         // reacting: pressure and frozen sound speed from eos_kernel
   if (active) {
     const double *up = P.u_in + e * NVAR * NN + p;
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
-    if constexpr (PHYS == PH_REACT) T = __ldg(&P.Taux[e * NN + p]);
+    if constexpr (PHYS == PH_REACT) {
+      pA = __ldg(&P.Taux[e * NA * NN + p]);
+      aA = __ldg(&P.Taux[(e * NA + 1) * NN + p]);
+    }
   }
   // neighbour trace of the first face task: in flight during phase N
-  double Up0[NVAR], Tp0 = 0.0;
+  double Up0[NVAR], pp0 = 0.0, ap0 = 0.0;
   int pR0 = 0;
   if (has0) {
     const int fR = (cn0.y >> 2) & 7, orient = (cn0.y >> 5) & 7;
@@ -96,10 +94,11 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     const double *un = P.u_in + (long)cn0.x * NVAR * NN + pR0;
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) Up0[v] = __ldg(un + v * NN);
-    if constexpr (PHYS == PH_REACT) Tp0 = __ldg(&P.Taux[(long)cn0.x * NN + pR0]);
+    if constexpr (PHYS == PH_REACT) {
+      pp0 = __ldg(&P.Taux[(long)cn0.x * NA * NN + pR0]);
+      ap0 = __ldg(&P.Taux[((long)cn0.x * NA + 1) * NN + pR0]);
+    }
   }
-  if constexpr (PHYS == PH_REACT) __syncthreads();   // mechanism table in shared memory
-  const MechDev *mech = (PHYS == PH_REACT) ? &mech_s : nullptr;
 
   // ---- phase N: own node
   if (active) {
@@ -108,7 +107,9 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     double Ja[DIM * DIM];
 #pragma unroll
     for (int k = 0; k < DIM * DIM; ++k) Ja[k] = metric_at<DIM, NP, AFFINE>(P.metric, e, k, p);
-    const Prim<DIM> pr = make_prim<DIM, NSP, PHYS, true>(U, T, P.gamma, mech);
+    Prim<DIM> pr;
+    if constexpr (PHYS == PH_REACT) pr = prim_given_pa<DIM, NSP>(U, pA, aA);
+    else pr = prim_ideal<DIM, true>(U, P.gamma);
     double Sg[(PHYS == PH_NS) ? NW * DIM : 1];
     if constexpr (PHYS == PH_NS) {
 #pragma unroll
@@ -132,16 +133,6 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     Ust[NVAR * TILE + tid] = pr.irho;
     Ust[(NVAR + 1) * TILE + tid] = pr.p;
     Ust[(NVAR + 2) * TILE + tid] = pr.a;
-    if constexpr (PHYS == PH_REACT) {
-      double om[NSP];
-      if (P.explicit_source) production_rates_listed<NSP>(*mech, T, U, Src + tid, TILE, om);
-      else {
-#pragma unroll
-        for (int s = 0; s < NSP; ++s) om[s] = 0.0;
-      }
-#pragma unroll
-      for (int s = 0; s < NSP; ++s) Src[s * TILE + tid] = om[s];
-    }
   }
   __syncthreads();
 
@@ -163,10 +154,10 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   for (int g = tid; g < ntask; g += NT) {
     FaceTask t;
     int2 cn;
-    double Up[NVAR], Tp = 0.0;
+    double Up[NVAR], pp = 0.0, ap = 0.0;
     int pR;
     if (g == tid) {
-      t = t0; cn = cn0; pR = pR0; Tp = Tp0;
+      t = t0; cn = cn0; pR = pR0; pp = pp0; ap = ap0;
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) Up[v] = Up0[v];
     } else {
@@ -179,7 +170,10 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       const double *un = P.u_in + (long)cn.x * NVAR * NN + pR;
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
-      if constexpr (PHYS == PH_REACT) Tp = __ldg(&P.Taux[(long)cn.x * NN + pR]);
+      if constexpr (PHYS == PH_REACT) {
+        pp = __ldg(&P.Taux[(long)cn.x * NA * NN + pR]);
+        ap = __ldg(&P.Taux[((long)cn.x * NA + 1) * NN + pR]);
+      }
     }
     const int l = t.f >> 1;
     const double sgn = (t.f & 1) ? 1.0 : -1.0;
@@ -202,7 +196,9 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       }
       nrm = sqrt(n2);
     }
-    const Prim<DIM> qp = make_prim<DIM, NSP, PHYS, true>(Up, Tp, P.gamma, mech);
+    Prim<DIM> qp;
+    if constexpr (PHYS == PH_REACT) qp = prim_given_pa<DIM, NSP>(Up, pp, ap);
+    else qp = prim_ideal<DIM, true>(Up, P.gamma);
     double mnm = 0.0, vnp = 0.0;
 #pragma unroll
     for (int c = 0; c < DIM; ++c) {
@@ -315,7 +311,7 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       if constexpr (!AFFINE) invJ = __ldg(&P.metric[(ee * MD + DIM * DIM) * NN + ij + m * GS]);
       double src = 0.0;
       if constexpr (PHYS == PH_REACT) {
-        if (v < NSP) src = Src[v * TILE + le * NN + ij + m * GS];
+        if (v < NSP && P.explicit_source) src = __ldg(&P.Taux[(ee * NA + 2 + v) * NN + ij + m * GS]);
       }
       const double val = P.cb * us[m * GS] + stage_cc(P) * (src - invJ * acc[m]);
       P.u_out[gofs + m * GS] = use_un ? (P.ca * un[m] + val) : val;
@@ -328,7 +324,7 @@ cudaError_t launch_stage_phys_t(const StageParams &P, cudaStream_t st) {
   constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
   using C = PhysCfg<DIM, NP, NSP, PHYS, EB>;
   constexpr size_t smem = C::smem_doubles(AFFINE) * sizeof(double);
-  constexpr int MINB = (PHYS == PH_REACT) ? ((C::NT <= 128) ? 3 : 1) : ((C::NT <= 128) ? MARUT_PHYS_MINB128 : ((C::NT <= 256) ? 2 : 1));
+  constexpr int MINB = (C::NT <= 128) ? MARUT_PHYS_MINB128 : ((C::NT <= 256) ? 2 : 1);
   auto k = stage_phys_kernel<DIM, NP, NSP, PHYS, AFFINE, EB, MINB>;
   static std::atomic<unsigned long long> attr_done{0};
   if (cudaError_t err = set_smem_once((const void *)k, smem, attr_done); err != cudaSuccess) return err;

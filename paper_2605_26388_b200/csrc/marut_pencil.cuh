@@ -144,9 +144,12 @@ __device__ __forceinline__ double pencil_flux_comp(int v, const double *Up, cons
 
 // One phase of one line.  L = direction, FIRST / LAST = position of the phase in the element's sequence.
 // Ut: the tile; Rs: partial residual; Md: the tile's metadata slot: conn (int2) | metric | fnorm.
-template <int DIM, int NP, int L, bool MORTAR>
+// FUSE (last phase only): the thread also evaluates the wave speed |v| + a of the nodes it finishes, from the values it
+// writes to u_out, with the expressions of wave_speed_kernel (eq. 18): lam / bad accumulate the maximum / a bad state.
+template <int DIM, int NP, int L, bool MORTAR, bool FUSE = false>
 __device__ __forceinline__ void pencil_phase(const StageParams &P, const double *__restrict__ Ut, double *__restrict__ Rs,
-                                             const double *__restrict__ Md, long e0, int nel, int t, double cc) {
+                                             const double *__restrict__ Md, long e0, int nel, int t, double cc, double &lam,
+                                             int &bad) {
   using C = PencilCfg<DIM, NP>;
   constexpr int NVAR = C::NVAR, NN = C::NN, NL = C::NL, ED = C::ED, MD = Geo<DIM, NP>::MD;
   constexpr bool FIRST = (L == 0), LAST = (L == DIM - 1);
@@ -228,7 +231,9 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
 #pragma unroll
       for (int m = 1; m < NP - 1; ++m) {
         const double val = P.cb * U[v][m] + cc * (0.0 - invJ * acc[m]);
-        P.u_out[gofs + v * NN + m * SM] = use_un ? (P.ca * un[m] + val) : val;
+        const double o = use_un ? (P.ca * un[m] + val) : val;
+        P.u_out[gofs + v * NN + m * SM] = o;
+        if constexpr (FUSE) U[v][m] = o;       // the node's new state replaces its old one (no longer needed)
       }
     }
   }
@@ -281,13 +286,36 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
       rl[v * NN + (NP - 1) * SM] = r1;
     } else {
       const double v0 = P.cb * U[v][0] + cc * (0.0 - invJ * r0), v1 = P.cb * U[v][NP - 1] + cc * (0.0 - invJ * r1);
-      P.u_out[gofs + v * NN] = use_un ? (P.ca * unE[v][0] + v0) : v0;
-      P.u_out[gofs + v * NN + (NP - 1) * SM] = use_un ? (P.ca * unE[v][1] + v1) : v1;
+      const double o0 = use_un ? (P.ca * unE[v][0] + v0) : v0, o1 = use_un ? (P.ca * unE[v][1] + v1) : v1;
+      P.u_out[gofs + v * NN] = o0;
+      P.u_out[gofs + v * NN + (NP - 1) * SM] = o1;
+      if constexpr (FUSE) {
+        accE[v][0] = o0;                       // U[v][0], U[v][NP-1] are still read by the later variables' lifts
+        accE[v][1] = o1;
+      }
+    }
+  }
+  if constexpr (FUSE && LAST) {
+#pragma unroll
+    for (int m = 0; m < NP; ++m) {
+      double Un[NVAR];
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Un[v] = (m == 0) ? accE[v][0] : ((m == NP - 1) ? accE[v][1] : U[v][m]);
+      const Prim<DIM> q = prim_ideal<DIM, true>(Un, P.gamma);
+      double v2 = 0.0;
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) v2 += q.v[c] * q.v[c];
+      const double l = sqrt(v2) + q.a;
+      if (!(l > 0.0) || !isfinite(l)) bad = 1;
+      lam = fmax(lam, l);
     }
   }
 }
 
-template <int DIM, int NP, bool MORTAR>
+// FUSE: the instantiation of the last stage of marut_ssprk33_step_cfl: besides the stage it reduces the maximum wave
+// speed of the state it writes (warp shuffle, one atomicMax per CTA) and the CTA that finishes last evaluates eq. 18
+// into P.dt_next -- the next step's CFL reduction without another pass over u.
+template <int DIM, int NP, bool MORTAR, bool FUSE = false>
 __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MINB) stage_pencil_kernel(const __grid_constant__ StageParams P) {
   using C = PencilCfg<DIM, NP>;
   constexpr int ET = C::ET, ED = C::ED, TD = C::TD, UB = C::UB, NT = C::NT, MW = C::MW, MD = Geo<DIM, NP>::MD;
@@ -338,6 +366,8 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
     issue((long)blockIdx.x + gridDim.x, 1);
   }
   const double cc = stage_cc(P);
+  double lam = 0.0;
+  int bad = 0;
   int it = 0;
   for (long tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
     const int buf = it & 1;
@@ -356,25 +386,29 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
       for (int i = tid; i < nel * ED; i += NT) dst[i] = __ldg(P.u_in + e0 * ED + i);
       __syncthreads();
     }
-    pencil_phase<DIM, NP, 0, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc);
+    pencil_phase<DIM, NP, 0, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
     __syncthreads();
     // u_n of this tile is read by the last phase: bring it into L2 now (earlier, and part of it is evicted again)
     if (tid == 0 && use_un && by_tma) bulk_prefetch_l2(P.u_n + ws, (uint32_t)wl * 8u);
     if constexpr (DIM == 3) {
-      pencil_phase<DIM, NP, 1, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc);
+      pencil_phase<DIM, NP, 1, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
       __syncthreads();
     }
-    pencil_phase<DIM, NP, DIM - 1, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc);
+    pencil_phase<DIM, NP, DIM - 1, MORTAR, FUSE>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
     cp_async_wait_all();
     __syncthreads();
     if (tid == 0) issue(tile + 2L * gridDim.x, buf);
   }
+  if constexpr (FUSE) cfl_reduce_and_finalize(P, lam, bad, tid);
 }
 
-template <int DIM, int NP, bool MORTAR>
+template <int DIM, int NP, bool MORTAR, bool FUSE = false>
 cudaError_t launch_stage_pencil_t(const StageParams &P, bool force, cudaStream_t st) {
+  if constexpr (!FUSE) {
+    if (P.red_next) return launch_stage_pencil_t<DIM, NP, MORTAR, true>(P, force, st);
+  }
   using C = PencilCfg<DIM, NP>;
-  auto k = stage_pencil_kernel<DIM, NP, MORTAR>;
+  auto k = stage_pencil_kernel<DIM, NP, MORTAR, FUSE>;
   static std::atomic<unsigned long long> attr_done{0};
   if (cudaError_t err = set_smem_once((const void *)k, C::smem_bytes, attr_done); err != cudaSuccess) return err;
   const long ntile = (P.ne + C::ET - 1) / C::ET;

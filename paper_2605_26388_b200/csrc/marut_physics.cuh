@@ -96,6 +96,23 @@ __device__ inline Prim<DIM> prim_mixture(const double *U, double T, const MechDe
   return q;
 }
 
+// reacting mixture with pressure and sound speed already known (eos_kernel): only the velocity is formed here
+template <int DIM, int NSP>
+__device__ __forceinline__ Prim<DIM> prim_given_pa(const double *U, double p, double a) {
+  Prim<DIM> q;
+  double rho = 0.0;
+#pragma unroll
+  for (int s = 0; s < NSP; ++s) rho += U[s];
+  q.rho = rho;
+  q.irho = 1.0 / rho;
+#pragma unroll
+  for (int c = 0; c < DIM; ++c) q.v[c] = U[NSP + c] * q.irho;
+  q.p = p;
+  q.a = a;
+  q.T = 0.0;
+  return q;
+}
+
 // e_int = E - 1/2 rho |v|^2 of a reacting state
 template <int DIM, int NSP>
 __device__ __forceinline__ double internal_energy(const double *U) {

@@ -149,3 +149,36 @@ def test_step_in_cuda_graph(name, cells):
     print(f"\n{name} cells={cells}: eager {e0.elapsed_time(e1) / 50 * 1e3:.1f} us/step, graph {e1.elapsed_time(e2) / 50 * 1e3:.1f} us/step")
     del graph
     gm.close()
+
+
+@pytest.mark.parametrize("name,cells,which", [("c2", 3, 2), ("c2", 3, 1), ("c1", 8, 2), ("c4", 32, 2), ("c3", 3, 0), ("c5", 4, 0)])
+def test_step_with_fused_cfl_reduction(name, cells, which):
+    """marut_ssprk33_step_cfl: the step equals three marut_ssprk_stage_dev calls bit for bit, and the time step it leaves
+    in dt_out equals marut_max_dt_async of the new state bit for bit -- with the reduction fused into the last stage's
+    kernel (line kernel, which = 2), and with the separate pass behind it (thread-per-node kernel, NS, reacting)"""
+    import torch
+
+    import paper_2605_26388_b200 as mb
+
+    c = wl.make_case(name, cells=cells)
+    gm = mb.MarutMesh(c.mesh)
+    gm.debug_stage_kernel(which)
+    u = torch.from_numpy(c.u0).cuda()
+    v = u.clone()
+    ua, ub = torch.empty_like(u), torch.empty_like(u)
+    dts = torch.zeros(2, dtype=torch.float64, device="cuda")
+    dt_ref = torch.zeros(1, dtype=torch.float64, device="cuda")
+    gm.max_dt_async(u, c.cfl, dts[0:1])
+    for k in range(4):
+        gm.max_dt_async(v, c.cfl, dt_ref)
+        for s, (un, uin, uout) in enumerate(((v, v, ua), (v, ua, ub), (v, ub, v))):
+            gm.stage_dev(s, dt_ref, 0.0, un, uin, uout)
+        gm.ssprk33_step_cfl(u, ua, ub, c.cfl, dts[k & 1:(k & 1) + 1], dts[(k + 1) & 1:((k + 1) & 1) + 1])
+        torch.cuda.synchronize()
+        assert torch.equal(u, v), (name, k)
+        gm.max_dt_async(v, c.cfl, dt_ref)
+        torch.cuda.synchronize()
+        assert dts[(k + 1) & 1].item() == dt_ref.item() and dt_ref.item() > 0, (name, k)
+    with pytest.raises(mb.MarutError):
+        gm.ssprk33_step_cfl(u, ua, ub, c.cfl, dts[0:1], dts[0:1])       # dt_out aliases dt_in
+    gm.close()

@@ -1,14 +1,17 @@
 """GPU parity at BASELINE.json's FULL sizes, through the C ABI in the launch configuration bench.py times:
 every output element against the CPU oracle (the oracle evaluates a full-size RHS in seconds on the box's
-host cores, so nothing is sampled).  One marut_rhs, marut_max_dt, one marut_ssprk_stage of each kind and a
-short run per config; the run covers the config's full step count for c2 / c4 / c4w and a bounded number of
-steps for c3 / c5 (each oracle step costs 3 full-size RHS evaluations).
+host cores, so nothing is sampled).  One marut_rhs, marut_max_dt, one marut_ssprk_stage and the config's own number
+of SSP-RK33 steps (c2 20, c3 10, c4 / c4w 20, c5 10; the split-form variant c2s 3).
 
-Tolerance (reading T1): 1e-11 on one RHS as BASELINE.json states, unless the ORACLE ITSELF moves by
-more than that when its own arithmetic is re-rounded in the one way the north star allows the two sides to
-differ (FMA contraction: the same source built with -ffp-contract=fast).  Then the bound is twice that
-self-sensitivity -- the case for c3 at 64^3, where round-off ~ eps * p0 * |D| / J (p0 = 71, Mach 0.1) meets a
-smooth flow whose time derivative is O(0.1)."""
+Tolerance: 1e-11 on one RHS and 1e-9 after the run, as BASELINE.json states, HARD for every config but one named
+exception (reading T1): c3 at 64^3, where round-off ~ eps * p0 * |D| / J (p0 = 71, Mach 0.1, h = 2 pi / 64)
+meets a smooth flow whose time derivative is O(0.1), so that the FP64 ORACLE ITSELF is 2-3e-11 away from the exact
+value of its own formulas.  There both sides are measured against the long-double build of the oracle
+(oracle.rhs_ld: the same source with every double an 80-bit long double): the GPU result must be as close to that
+truth as the FP64 oracle is, |gpu - truth| <= 1.5 |oracle - truth|, and the test prints the three numbers
+(measured: |gpu - oracle| 3.5e-11, |gpu - truth| 1.44e-10, |oracle - truth| 1.54e-10: the two FP64 sides share the
+round-off of the FP64 metric terms, which they compute to the same bits, and differ from one another by less than
+either differs from the exact value of the formulas)."""
 import numpy as np
 import pytest
 
@@ -19,17 +22,26 @@ pytestmark = pytest.mark.gpu
 
 # (config, steps of the run; None = the config's own step count)
 # c2s = c2 with the entropy-stable split-form volume integral
-FULL = [("c2", None), ("c2s", 3), ("c3", 2), ("c4", None), ("c4w", None), ("c5", 3)]
+# c3n = the c3 mesh and physics with seeded node-wise velocity noise (1e-3, as c2): jumps at every interface, so the
+#       Rusanov dissipation, the BR1 trace What - W and F_v* - F_v are exercised at N = 3 on the curved mesh at t = 0
+FULL = [("c2", None), ("c2s", 3), ("c3", None), ("c3n", 0), ("c4", None), ("c4w", None), ("c5", None)]
+T1_EXCEPTION = ("c3", "c3n")      # the only configs allowed to use the truth-based bound of reading T1
 
 
-def derived_tol(oracle, mesh, u0, ref):
-    """max(1e-11, 2 x the oracle's own FMA-contraction sensitivity) -- see the module docstring"""
-    Lf = oracle.lib_fma()
-    if Lf is None:
-        return RHS_TOL, 0.0
-    alt = oracle.OracleMesh(mesh, L=Lf).rhs(u0)
-    delta = float(parity_error(alt, ref).max())
-    return max(RHS_TOL, 2.0 * delta), delta
+def check_rhs(name, oracle, mesh, u0, gpu, ref, what):
+    """1e-11 against the FP64 oracle; for the named exception: as close to the long-double truth as the oracle is"""
+    err = parity_error(gpu, ref).max()
+    if err <= RHS_TOL:
+        print(f"{name} {what}: err {err:.2e} <= 1e-11")
+        return RHS_TOL
+    assert name in T1_EXCEPTION, (name, what, err)
+    truth = oracle.rhs_ld(mesh, u0) if what == "rhs" else None
+    assert truth is not None
+    e_gpu, e_orc = parity_error(gpu, truth).max(), parity_error(ref, truth).max()
+    print(f"{name} {what}: KNOWN T1 EXCEPTION: |gpu - oracle| {err:.2e} > 1e-11; against the long-double truth: "
+          f"gpu {e_gpu:.2e}, fp64 oracle {e_orc:.2e}")
+    assert e_gpu <= 1.5 * e_orc and e_gpu <= 1e-9, (name, e_gpu, e_orc)
+    return max(RHS_TOL, e_gpu + e_orc)
 
 
 @pytest.mark.parametrize("name,run_steps", FULL)
@@ -39,9 +51,11 @@ def test_full_size_parity(name, run_steps):
     import oracle
     import paper_2605_26388_b200 as mb
 
-    c = wl.make_case("c2" if name == "c2s" else name)
+    c = wl.make_case({"c2s": "c2", "c3n": "c3"}.get(name, name))
     if name == "c2s":
         c.mesh.volume_form = 1
+    if name == "c3n":
+        c.u0 = wl.taylor_green(c.mesh, noise=1e-3)
     om = oracle.OracleMesh(c.mesh)
     gm = mb.MarutMesh(c.mesh)
     u = torch.from_numpy(c.u0).cuda()
@@ -49,12 +63,7 @@ def test_full_size_parity(name, run_steps):
     gm.rhs(u, du)
     torch.cuda.synchronize()
     ref = om.rhs(c.u0)
-    err = parity_error(du.cpu().numpy(), ref)
-    tol, delta = (RHS_TOL, 0.0)
-    if err.max() > RHS_TOL:
-        tol, delta = derived_tol(oracle, c.mesh, c.u0, ref)
-    print(f"{name}: {c.mesh.n_elem} elements, rhs err {err.max():.2e} (tol {tol:.1e}, oracle FMA self-sensitivity {delta:.1e})")
-    assert err.max() <= tol, (name, err, tol)
+    tol = check_rhs(name, oracle, c.mesh, c.u0, du.cpu().numpy(), ref, "rhs")
     del du, ref
 
     dt_g, dt_c = gm.max_dt(u, c.cfl), om.max_dt(c.u0, c.cfl)
@@ -72,6 +81,9 @@ def test_full_size_parity(name, run_steps):
     assert parity_error(out.cpu().numpy(), ref).max() <= tol, name
     del un, out, ref, un_h
 
+    if run_steps == 0:
+        gm.close()
+        return
     steps = run_steps or c.steps
     ug, tg = gpu_run(gm, c.u0, steps, c.cfl, torch)
     uc, tc, min_rho, min_p = om.run(c.u0, steps, cfl=c.cfl)
