@@ -189,6 +189,7 @@ __global__ void __launch_bounds__(256) eos_kernel(const double *__restrict__ u, 
                                                   const MechDev *__restrict__ mech_g, long ne, int nn, int with_source) {
   constexpr int NVAR = NSP + DIM + 1, NA = 2 + NSP;
   __shared__ MechDev mech;
+  __shared__ double Xs[NSP * 256];           // per-thread concentration columns of production_rates_listed
   load_mech(&mech, mech_g);
   const long total = ne * nn;
   for (long g = (long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
@@ -204,7 +205,7 @@ __global__ void __launch_bounds__(256) eos_kernel(const double *__restrict__ u, 
     a[nn] = q.a;
     if (with_source) {
       double om[NSP];
-      production_rates<NSP>(mech, T, U, om);
+      production_rates_listed<NSP>(mech, T, U, Xs + threadIdx.x, 256, om);
 #pragma unroll
       for (int s = 0; s < NSP; ++s) a[(2 + s) * nn] = om[s];
     }
@@ -511,18 +512,18 @@ __global__ void __launch_bounds__(256) wave_speed_kernel(const double *__restric
 #pragma unroll
     for (int k = 0; k < UNR; ++k) {
       if (!on[k]) continue;
-      Prim<DIM> q;
+      double l;
       if constexpr (PHYS == PH_REACT) {
         const double T = temperature_newton<NSP>(mech, U[k], internal_energy<DIM, NSP>(U[k]));
-        q = prim_mixture<DIM, NSP, true>(U[k], T, mech);
-      } else q = prim_ideal<DIM, true>(U[k], gamma);
-      double v2 = 0.0;
+        const Prim<DIM> q = prim_mixture<DIM, NSP, true>(U[k], T, mech);
+        double v2 = 0.0;
 #pragma unroll
-      for (int c = 0; c < DIM; ++c) v2 += q.v[c] * q.v[c];
-      const double l = sqrt(v2) + q.a;
+        for (int c = 0; c < DIM; ++c) v2 += q.v[c] * q.v[c];
+        l = sqrt(v2) + q.a;
+      } else l = wave_speed_ideal<DIM>(U[k], gamma);
       if (!(l > 0.0) || !isfinite(l)) bad = 1;
       lam = fmax(lam, l);
-      if constexpr (PHYS == PH_NS) nu = fmax(nu, mu / q.rho);
+      if constexpr (PHYS == PH_NS) nu = fmax(nu, mu / U[k][0]);
     }
   }
   lam = warp_max(lam);

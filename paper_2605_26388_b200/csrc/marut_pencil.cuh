@@ -301,11 +301,7 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
       double Un[NVAR];
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) Un[v] = (m == 0) ? accE[v][0] : ((m == NP - 1) ? accE[v][1] : U[v][m]);
-      const Prim<DIM> q = prim_ideal<DIM, true>(Un, P.gamma);
-      double v2 = 0.0;
-#pragma unroll
-      for (int c = 0; c < DIM; ++c) v2 += q.v[c] * q.v[c];
-      const double l = sqrt(v2) + q.a;
+      const double l = wave_speed_ideal<DIM>(Un, P.gamma);
       if (!(l > 0.0) || !isfinite(l)) bad = 1;
       lam = fmax(lam, l);
     }

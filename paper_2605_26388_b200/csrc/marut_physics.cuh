@@ -96,6 +96,20 @@ __device__ inline Prim<DIM> prim_mixture(const double *U, double T, const MechDe
   return q;
 }
 
+// |v| + a of an ideal-gas state (eq. 18; R11): the ONE expression both wave_speed_kernel and the
+// fused reduction of the stage kernels evaluate, so that marut_max_dt, marut_max_dt_async and marut_ssprk33_step_cfl give
+// the same time step bit for bit.  A state with rho <= 0 < p or p < 0 < rho gives NaN (caught by the callers).
+template <int DIM>
+__device__ __forceinline__ double wave_speed_ideal(const double *U, double gamma) {
+  const double rinv = rcp_pos(U[0]);
+  double m2 = 0.0;
+#pragma unroll
+  for (int c = 0; c < DIM; ++c) m2 += U[1 + c] * U[1 + c];
+  const double p = (gamma - 1.0) * (U[DIM + 1] - 0.5 * m2 * rinv);
+  const double vabs = (m2 > 0.0) ? sqrt_pos(m2) * fabs(rinv) : 0.0;     // a fluid at rest: sqrt_pos(0) is not defined
+  return vabs + sqrt_pos(gamma * p * rinv);
+}
+
 // reacting mixture with pressure and sound speed already known (eos_kernel): only the velocity is formed here
 template <int DIM, int NSP>
 __device__ __forceinline__ Prim<DIM> prim_given_pa(const double *U, double p, double a) {
