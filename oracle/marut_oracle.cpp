@@ -301,7 +301,8 @@ struct Mesh {
   int explicit_source = 1;      // reacting: 1 = L includes the chemistry source S(U); 0 = transport operator only (Strang split)
   int volume_form = 0;          // 0: standard strong form (eq. 9); 1: entropy-stable split form (eq. 10)
   std::vector<double> alpha;    // per-element blending coefficient alpha_e of eq. 11 / 42; empty = no blending
-  std::vector<int> bc_kind;     // per bc id: 0 prescribed exterior state, 1 outflow, 2 slip wall (O8b); empty = all 0
+  std::vector<int> bc_kind;     // per bc id: 0 prescribed exterior state, 1 outflow, 2 slip wall (O8b), 3 no-slip adiabatic
+                                // wall, 4 no-slip isothermal wall (O9b, Navier-Stokes only); empty = all 0
 };
 
 static inline int node_index(const Mesh &m, const int *ijk) {
@@ -795,7 +796,8 @@ static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
       const int bk = m.bc_kind.empty() ? 0 : m.bc_kind[bc];
       double Ue[MAXV];
       for (int v = 0; v < nvar; ++v) Ue[v] = (bk == 0) ? m.bc_state[(size_t)bc * nvar + v] : Um[v];
-      if (bk == 2) {
+      // viscous walls (kinds 3, 4; reading R22): the hyperbolic surface flux of a no-slip wall is the slip wall's
+      if (bk >= 2) {
         double nrm = 0.0, mn = 0.0;
         for (int c = 0; c < d; ++c) nrm += nv[c] * nv[c];
         nrm = std::sqrt(nrm);
@@ -809,7 +811,7 @@ static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
 }
 
 // ---------------------------------------------------------------------------
-// O9. BR1 viscous residual; conforming faces only.
+// O9. BR1 viscous residual; conforming interfaces and boundary faces (O9b).
 // W = (rho, u_1..u_d, T), T = p/rho.  S[e][node][w][c] = d W_w / d x_c.
 // ---------------------------------------------------------------------------
 static void prim_gradient_vars(const Mesh &m, const double *U, double *W) {
@@ -891,6 +893,36 @@ static void br1_gradient(const Mesh &m, const double *u, std::vector<double> &S)
       }
     }
   }
+  // O9b. boundary faces (reading R22): the trace What is fixed by the boundary kind --
+  //   prescribed state: the central trace with W(U_bc);  outflow: W- (no jump);  slip wall: "mirrors the velocity across
+  //   the boundary normal", W+ = (rho-, v- - 2 (v-.nhat) nhat, T-), central trace;  no-slip adiabatic wall: "sets the wall
+  //   velocity to zero and inherits interior (rho, T)", What = (rho-, 0, T-);  isothermal wall: "additionally fixes
+  //   T = T_wall", What = (rho-, 0, T_wall), T_wall = the temperature of the boundary id's prescribed state.
+  for (size_t b = 0; b < m.bface.size() / 3; ++b) {
+    const long e = m.bface[b * 3]; const int f = m.bface[b * 3 + 1], bc = m.bface[b * 3 + 2];
+    const int bk = m.bc_kind.empty() ? 0 : m.bc_kind[bc];
+    for (int a = 0; a < nf; ++a) {
+      const int p = face_node(m, f, a);
+      double Um[MAXV], Wm[MAXV], What[MAXV], nv[3];
+      gather(m, u, e, p, Um); prim_gradient_vars(m, Um, Wm); face_normal(m, e, f, p, nv);
+      for (int w = 0; w < nw; ++w) What[w] = Wm[w];
+      if (bk == 0) {
+        double Wb[MAXV]; prim_gradient_vars(m, &m.bc_state[(size_t)bc * m.nvar], Wb);
+        for (int w = 0; w < nw; ++w) What[w] = 0.5 * (Wm[w] + Wb[w]);
+      } else if (bk == 2) {
+        double nrm = 0.0, vn = 0.0;
+        for (int c = 0; c < d; ++c) nrm += nv[c] * nv[c];
+        nrm = std::sqrt(nrm);
+        for (int c = 0; c < d; ++c) vn += Wm[1 + c] * (nv[c] / nrm);
+        for (int c = 0; c < d; ++c) What[1 + c] = 0.5 * (Wm[1 + c] + (Wm[1 + c] - 2.0 * vn * (nv[c] / nrm)));
+      } else if (bk == 3 || bk == 4) {
+        for (int c = 0; c < d; ++c) What[1 + c] = 0.0;
+        if (bk == 4) { double Wb[MAXV]; prim_gradient_vars(m, &m.bc_state[(size_t)bc * m.nvar], Wb); What[1 + d] = Wb[1 + d]; }
+      }
+      for (int w = 0; w < nw; ++w)
+        for (int c = 0; c < d; ++c) S[(((size_t)e * nn + p) * nw + w) * d + c] += (What[w] - Wm[w]) * nv[c] / wb;
+    }
+  }
   // rescale by the inverse Jacobian
   for (long e = 0; e < m.ne; ++e)
     for (int p = 0; p < nn; ++p)
@@ -938,6 +970,29 @@ static void rhs_viscous_add(const Mesh &m, const double *u, double *du) {
         du[((size_t)eL * nvar + v) * nn + pL] += (0.5 * (FmL[v] + FpL[v]) - FmL[v]) / (JL * wb);
         du[((size_t)eR * nvar + v) * nn + pR] += (0.5 * (FpR[v] + FmR[v]) - FpR[v]) / (JR * wb);
       }
+    }
+  }
+  // O9b. boundary faces ("boundary kernels"; the wall flux is not printed: DESIGN.md reading R22).
+  //   prescribed state, outflow, slip wall: F_v* = F_v(U-, S-), no viscous surface term;
+  //   no-slip walls: F_v* is evaluated with the wall velocity (zero) and the interior gradient, F_v*(U_w, S-): the
+  //   momentum rows carry the wall shear stress tau(S-).n (unchanged), the energy row loses the work of the stress
+  //   (v_w = 0) and keeps the heat flux k grad T . n at an isothermal wall; at an adiabatic wall the heat flux through
+  //   the wall vanishes as well: energy row of F_v* = 0.
+  for (size_t b = 0; b < m.bface.size() / 3; ++b) {
+    const long e = m.bface[b * 3]; const int f = m.bface[b * 3 + 1], bc = m.bface[b * 3 + 2];
+    const int bk = m.bc_kind.empty() ? 0 : m.bc_kind[bc];
+    if (bk != 3 && bk != 4) continue;
+    for (int a = 0; a < nf; ++a) {
+      const int p = face_node(m, f, a);
+      double Um[MAXV], Uw[MAXV], nv[3], Fm[MAXV], Fw[MAXV];
+      gather(m, u, e, p, Um); face_normal(m, e, f, p, nv);
+      for (int v = 0; v < nvar; ++v) Uw[v] = Um[v];
+      for (int c = 0; c < d; ++c) Uw[1 + c] = 0.0;          // wall velocity zero
+      const double *Sm = &S[((size_t)e * nn + p) * nw * d];
+      viscous_flux_dot(m, Um, Sm, nv, Fm); viscous_flux_dot(m, Uw, Sm, nv, Fw);
+      if (bk == 3) Fw[1 + d] = 0.0;                          // adiabatic: no heat through the wall either
+      const double Jp = m.J[(size_t)e * nn + p];
+      for (int v = 0; v < nvar; ++v) du[((size_t)e * nvar + v) * nn + p] += (Fw[v] - Fm[v]) / (Jp * wb);
     }
   }
 }
@@ -1212,8 +1267,8 @@ int oracle_set_blend(void *h, const double *alpha) {
 int oracle_set_boundary_kinds(void *h, const int *kinds, int n) {
   Mesh *m = (Mesh *)h;
   if (!kinds) { m->bc_kind.clear(); return 0; }
-  if (m->physics != EULER) return 1;
-  for (int i = 0; i < n; ++i) if (kinds[i] < 0 || kinds[i] > 2) return 2;
+  if (m->physics == REACTING_EULER) return 1;
+  for (int i = 0; i < n; ++i) if (kinds[i] < 0 || kinds[i] > (m->physics == NAVIER_STOKES ? 4 : 2)) return 2;
   m->bc_kind.assign(kinds, kinds + n);
   return 0;
 }

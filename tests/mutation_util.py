@@ -24,6 +24,14 @@ MUTATIONS = {
         "double What = 0.5 * (Wm[w] + Wp[w]);",
         "double What = 0.75 * Wm[w] + 0.25 * Wp[w];",
         "BR1 interface trace is not the arithmetic mean of eq. 13"),
+    "wall_trace_keeps_velocity": (
+        "for (int c = 0; c < d; ++c) What[1 + c] = 0.0;",
+        "for (int c = 0; c < d; ++c) What[1 + c] = Wm[1 + c];",
+        "no-slip wall: the BR1 trace keeps the interior velocity instead of the wall's (zero)"),
+    "adiabatic_wall_energy_flux_kept": (
+        "if (bk == 3) Fw[1 + d] = 0.0;",
+        "if (bk == 3) Fw[1 + d] = Fm[1 + d];",
+        "adiabatic wall: the energy row of the wall's viscous flux keeps the stress work and the heat flux"),
     "ranocha_printed_energy_flux": (
         "pvn += 0.5 * (L.p * R.vel[c] + R.p * L.vel[c]) * nv[c];",
         "pvn += 0.5 * (L.p * L.vel[c] + R.p * R.vel[c]) * nv[c];",

@@ -190,6 +190,21 @@ def cartesian_mesh(dim, N, counts, lo, hi, order="morton", warp=None, periodic=T
     return m
 
 
+def open_direction(mesh: Mesh, axis=0, bc_lo=0, bc_hi=1) -> Mesh:
+    """turn the periodic wrap-around interfaces of a Cartesian mesh in direction `axis` into boundary faces
+    (boundary id bc_lo on the low side, bc_hi on the high side); rows are appended to mesh.bface"""
+    xc = mesh.node_xyz[:, axis, :].mean(axis=1)
+    first, last = np.isclose(xc, xc.min()), np.isclose(xc, xc.max())
+    wrap = (mesh.iface[:, 1] == 2 * axis + 1) & last[mesh.iface[:, 0]] & first[mesh.iface[:, 2]]
+    assert wrap.sum() == last.sum() > 0
+    w = mesh.iface[wrap]
+    new = np.concatenate([np.stack([w[:, 0], w[:, 1], np.full(len(w), bc_hi, np.int32)], axis=1),
+                          np.stack([w[:, 2], w[:, 3], np.full(len(w), bc_lo, np.int32)], axis=1)]).astype(np.int32)
+    mesh.bface = np.ascontiguousarray(np.concatenate([mesh.bface.reshape(-1, 3), new]).astype(np.int32))
+    mesh.iface = np.ascontiguousarray(mesh.iface[~wrap])
+    return mesh
+
+
 def octree_box_mesh(N, K=4, lo=(0.0, 0.0, 0.0), hi=(1.0, 1.0, 1.0), refine=None) -> Mesh:
     """3-D periodic box of K^3 cells, the cells selected by `refine(ix, iy, iz) -> bool` (default: ix < K/2) split once
     into 2x2x2 children: conforming faces between cells of equal size, 4:1 mortar faces (rows of 8 ints:
