@@ -181,13 +181,20 @@ marut_status marut_shock_indicator(marut_mesh *mesh, const double *u, double s, 
 marut_status marut_set_blend(marut_mesh *mesh, const double *alpha);
 
 /* Boundary kinds ("wall/slip/outflow"; "enforced weakly through the numerical surface
- * flux"; reading R18).  kinds: HOST, [n_bc], one per boundary id of the mesh description:
- *   MARUT_BC_PRESCRIBED  exterior state = bc_state[id] (default),
- *   MARUT_BC_OUTFLOW     exterior state = interior state (F* = F(U-).n, no lift),
- *   MARUT_BC_SLIP_WALL   exterior state = interior state with the normal momentum reflected, m+ = m- - 2 (m-.nhat) nhat.
- * Rewrites the connectivity table on the device (synchronises); takes effect from the next call.  Kinds other than
- * PRESCRIBED need a MARUT_EULER mesh (else EINVAL); n_bc must equal the description's. */
-enum { MARUT_BC_PRESCRIBED = 0, MARUT_BC_OUTFLOW = 1, MARUT_BC_SLIP_WALL = 2 };
+ * flux", PAPER.md:223 the wall traces of the BR1 gradient; readings R18, R22).  kinds: HOST, [n_bc], one per
+ * boundary id of the mesh description:
+ *   MARUT_BC_PRESCRIBED       exterior state = bc_state[id] (default); Navier-Stokes: BR1 trace = mean of W- and W(bc_state),
+ *                             no viscous surface term,
+ *   MARUT_BC_OUTFLOW          exterior state = interior state (F* = F(U-).n, no lift; no BR1 jump),
+ *   MARUT_BC_SLIP_WALL        exterior state = interior state with the normal momentum reflected, m+ = m- - 2 (m-.nhat) nhat;
+ *                             Navier-Stokes: the BR1 trace mirrors the velocity across the normal,
+ *   MARUT_BC_WALL_ADIABATIC   (MARUT_NAVIER_STOKES only) no-slip adiabatic wall: hyperbolic flux of the slip wall, BR1 trace
+ *                             (rho-, 0, T-), viscous wall flux with v_w = 0 and no heat flux through the wall,
+ *   MARUT_BC_WALL_ISOTHERMAL  (MARUT_NAVIER_STOKES only) as above with T_wall = temperature p/rho of bc_state[id] in the
+ *                             trace and the heat flux k grad T . n kept in the wall flux.
+ * Rewrites the connectivity table on the device (synchronises); takes effect from the next call.  MARUT_EULER and
+ * MARUT_NAVIER_STOKES meshes (REACTING_EULER: PRESCRIBED only, else EINVAL); n_bc must equal the description's. */
+enum { MARUT_BC_PRESCRIBED = 0, MARUT_BC_OUTFLOW = 1, MARUT_BC_SLIP_WALL = 2, MARUT_BC_WALL_ADIABATIC = 3, MARUT_BC_WALL_ISOTHERMAL = 4 };
 marut_status marut_set_boundary_kinds(marut_mesh *mesh, const int *kinds, int n_bc);
 
 /* Per-stage positivity floor ("a per-stage positivity floor enforces rho >= 1e-6 and

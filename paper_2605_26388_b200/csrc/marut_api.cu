@@ -36,7 +36,7 @@ static marut_status fail(marut_status st, const char *fmt, ...) {
 // ------------------------------------------------------------------------------------ mesh handle
 struct marut_mesh {
   int dim = 0, N = 0, np = 0, nn = 0, nvar = 0, nsp = 1, physics = 0;
-  long ne = 0, n_mortar = 0;
+  long ne = 0, n_mortar = 0, n_bface = 0;
   int n_bc = 0;
   bool oriented = false;       // some 3-D interface has a non-trivial orientation code (R20)
   bool bc_kinds = false;       // some boundary id is an outflow / slip-wall face
@@ -255,8 +255,10 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   if ((d->n_iface && !d->iface) || (d->n_mortar && !d->mortar) || (d->n_bface && !d->bface) || (d->n_bc && !d->bc_state))
     return fail(MARUT_EINVAL, "NULL connectivity array with non-zero count");
   if (d->physics < 0 || d->physics > 2) return fail(MARUT_EINVAL, "unknown physics %d", d->physics);
-  if (d->physics != MARUT_EULER && (d->n_mortar || d->n_bface))
-    return fail(MARUT_EINVAL, "NAVIER_STOKES / REACTING_EULER support conforming interior faces only");
+  if (d->physics == MARUT_REACTING_EULER && (d->n_mortar || d->n_bface))
+    return fail(MARUT_EINVAL, "REACTING_EULER supports conforming interior faces only");
+  if (d->physics == MARUT_NAVIER_STOKES && d->n_mortar)
+    return fail(MARUT_EINVAL, "NAVIER_STOKES supports conforming interior faces and boundary faces, no mortars");
   if (d->physics != MARUT_REACTING_EULER && !(d->gamma > 1.0)) return fail(MARUT_EINVAL, "gamma must be > 1");
   if (d->physics == MARUT_NAVIER_STOKES && (!(d->mu >= 0.0) || !(d->Pr > 0.0))) return fail(MARUT_EINVAL, "need mu >= 0, Pr > 0");
 
@@ -396,6 +398,7 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   CUDA_TRY(cudaMalloc(&m->d_mortar_mat, mort.size() * sizeof(double)));
   CUDA_TRY(cudaMemcpy(m->d_mortar_mat, mort.data(), mort.size() * sizeof(double), cudaMemcpyHostToDevice));
   m->n_bc = d->n_bc;
+  m->n_bface = d->n_bface;
   const size_t nbc = (size_t)std::max(1, d->n_bc) * m->nvar;
   CUDA_TRY(cudaMalloc(&m->d_bc, nbc * sizeof(double)));
   if (d->n_bc) CUDA_TRY(cudaMemcpy(m->d_bc, d->bc_state, (size_t)d->n_bc * m->nvar * sizeof(double), cudaMemcpyHostToDevice));
@@ -510,6 +513,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
     GradParams G;
     G.u = u_in; G.S = m->d_S; G.metric = m->d_metric; G.conn = m->d_conn;
     G.gamma = m->gamma; G.inv_wb = 1.0 / m->w[0]; G.mu = m->mu; G.kappa = m->kappa; G.ne = m->ne; G.oriented = m->oriented ? 1 : 0;
+    G.bc_state = m->d_bc; G.boundary = m->n_bface > 0 ? 1 : 0;
     memcpy(G.D, m->D, sizeof(G.D));
     cudaError_t e = launch_gradient(m->dim, m->np, m->affine, G, st);
     if (e != cudaSuccess) return fail(e == cudaErrorNotSupported ? MARUT_EINVAL : MARUT_ECUDA, "gradient kernel: %s", cudaGetErrorString(e));
@@ -539,7 +543,9 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
     if (em != cudaSuccess) return fail(MARUT_ECUDA, "mortar flux kernel: %s", cudaGetErrorString(em));
     m->launches++;
   }
-  P.alpha = nullptr; P.subn = m->d_subn; P.bc_kinds = (m->bc_kinds || (m->dim == 3 && m->n_mortar > 0)) ? 1 : 0;
+  P.alpha = nullptr; P.subn = m->d_subn;
+  // Euler: outflow / slip-wall faces or 3-D mortars exist; Navier-Stokes: the mesh has boundary faces of any kind
+  P.bc_kinds = (m->bc_kinds || (m->dim == 3 && m->n_mortar > 0) || (m->physics == MARUT_NAVIER_STOKES && m->n_bface > 0)) ? 1 : 0;
   for (int i = 0; i < MAX_NP; ++i) P.inv_w[i] = (i < m->np) ? 1.0 / m->w[i] : 0.0;
   if (m->d_alpha) {
     if (m->physics != MARUT_EULER || m->volume_form != MARUT_VOLUME_SPLIT_RANOCHA)
@@ -879,11 +885,13 @@ extern "C" marut_status marut_set_boundary_kinds(marut_mesh *m, const int *kinds
   if (n_bc != m->n_bc) return fail(MARUT_EINVAL, "n_bc = %d, the mesh has %d boundary ids", n_bc, m->n_bc);
   bool special = false;
   for (int i = 0; i < n_bc; ++i) {
-    if (kinds[i] < MARUT_BC_PRESCRIBED || kinds[i] > MARUT_BC_SLIP_WALL) return fail(MARUT_EINVAL, "unknown boundary kind %d", kinds[i]);
+    const int kmax = (m->physics == MARUT_NAVIER_STOKES) ? MARUT_BC_WALL_ISOTHERMAL : MARUT_BC_SLIP_WALL;
+    if (kinds[i] < MARUT_BC_PRESCRIBED || kinds[i] > kmax)
+      return fail(MARUT_EINVAL, "boundary kind %d is unknown or not available for this physics (no-slip walls: MARUT_NAVIER_STOKES)", kinds[i]);
     special = special || kinds[i] != MARUT_BC_PRESCRIBED;
   }
-  if (special && m->physics != MARUT_EULER)
-    return fail(MARUT_EINVAL, "outflow / slip-wall faces are implemented for MARUT_EULER (default kernels) only");
+  if (special && m->physics == MARUT_REACTING_EULER)
+    return fail(MARUT_EINVAL, "boundary kinds are implemented for MARUT_EULER and MARUT_NAVIER_STOKES");
   if (n_bc == 0) return MARUT_OK;
   int *d_k = nullptr;
   CUDA_TRY(cudaMalloc(&d_k, n_bc * sizeof(int)));

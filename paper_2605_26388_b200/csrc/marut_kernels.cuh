@@ -77,11 +77,48 @@ struct GradParams {
   long ne;
   double D[MAX_NP * MAX_NP];
   int oriented;                        // 3-D: some interface has a non-trivial orientation code
+  const double *__restrict__ bc_state; // [bc][nvar] prescribed states of the boundary ids (kind 0; kind 4: their T is T_wall)
+  int boundary;                        // the mesh has boundary faces: launch the instantiation that knows them
 };
+
+// BR1 trace jump What - W at a boundary face node (reading R22).  kind: 0 prescribed state
+// (central trace with W(U_bc)), 1 outflow (no jump), 2 slip wall (velocity mirrored across the normal), 3 no-slip
+// adiabatic wall (What = (rho-, 0, T-)), 4 isothermal wall (What = (rho-, 0, T_wall), T_wall = T of the prescribed state)
+template <int DIM>
+__device__ __forceinline__ void br1_boundary_jump(int kind, const double *W, const double *Ub, const double *nv, double gamma,
+                                                  double *jump) {
+  constexpr int NW = DIM + 2;
+#pragma unroll
+  for (int w = 0; w < NW; ++w) jump[w] = 0.0;
+  if (kind == BC_PRESCRIBED || kind == BC_WALL_ISOTHERMAL) {
+    const Prim<DIM> qb = prim_ideal<DIM, false>(Ub, gamma);
+    if (kind == BC_PRESCRIBED) {
+      jump[0] = 0.5 * (W[0] + qb.rho) - W[0];
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) jump[1 + c] = 0.5 * (W[1 + c] + qb.v[c]) - W[1 + c];
+      jump[1 + DIM] = 0.5 * (W[1 + DIM] + qb.T) - W[1 + DIM];
+    } else jump[1 + DIM] = qb.T - W[1 + DIM];
+  }
+  if (kind == BC_SLIP_WALL) {
+    double n2 = 0.0, vn = 0.0;
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) n2 += nv[c] * nv[c];
+    const double inrm = 1.0 / sqrt(n2);
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) vn += W[1 + c] * (nv[c] * inrm);
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) jump[1 + c] = 0.5 * (W[1 + c] + (W[1 + c] - 2.0 * vn * (nv[c] * inrm))) - W[1 + c];
+  }
+  if (kind == BC_WALL_ADIABATIC || kind == BC_WALL_ISOTHERMAL) {
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) jump[1 + c] = 0.0 - W[1 + c];
+  }
+}
 
 // ORIENT3: the instantiation for 3-D meshes with non-trivial face orientation codes (R20); the default one
 // keeps the identity pairing folded at compile time (the decode costs 12 registers here: 64 -> 76, one CTA less per SM)
-template <int DIM, int NP, bool AFFINE, int EB, bool ORIENT3 = false>
+// BND: the instantiation for meshes with boundary faces (prescribed states, outflow, walls; reading R22)
+template <int DIM, int NP, bool AFFINE, int EB, bool ORIENT3 = false, bool BND = false>
 __global__ void __launch_bounds__(((EB * Geo<DIM, NP>::NN + 31) / 32) * 32)
 gradient_kernel(const __grid_constant__ GradParams P) {
   using G = Geo<DIM, NP>;
@@ -136,6 +173,23 @@ gradient_kernel(const __grid_constant__ GradParams P) {
     const int side = (q[l] == 0) ? 0 : 1, f = 2 * l + side;
     const double sgn = side ? 1.0 : -1.0;
     const int2 cn = __ldg(&P.conn[e * 2 * DIM + f]);
+    if constexpr (BND) {
+      if ((cn.y & 3) == FK_BOUNDARY) {
+        double nv[DIM], Ub[NVAR], jump[NW];
+#pragma unroll
+        for (int c = 0; c < DIM; ++c) nv[c] = sgn * metric_at<DIM, NP, AFFINE>(P.metric, e, l * DIM + c, p);
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Ub[v] = __ldg(&P.bc_state[cn.x * NVAR + v]);
+        br1_boundary_jump<DIM>((cn.y >> 2) & 7, W, Ub, nv, P.gamma, jump);
+#pragma unroll
+        for (int c = 0; c < DIM; ++c) {
+          const double nc = nv[c] * P.inv_wb;
+#pragma unroll
+          for (int w = 0; w < NW; ++w) Sg[w * DIM + c] += jump[w] * nc;
+        }
+        continue;
+      }
+    }
     const int fR = (cn.y >> 2) & 7, orient = (DIM == 2 || ORIENT3) ? ((cn.y >> 5) & 7) : 0;
     int a0, a1;
     G::face_coords(q, l, a0, a1);
@@ -666,15 +720,19 @@ __global__ void fnorm_kernel(const double *__restrict__ metric_el, double *__res
 template <int NN>
 constexpr int elems_per_block() { return (256 / NN) < 1 ? 1 : 256 / NN; }
 
-template <int DIM, int NP, bool AFFINE, bool ORIENT3 = false>
+template <int DIM, int NP, bool AFFINE, bool ORIENT3 = false, bool BND = false>
 cudaError_t launch_gradient_t(const GradParams &P, cudaStream_t st) {
-  if constexpr (DIM == 3 && !ORIENT3) {
+  if constexpr (!BND) {
+    // meshes with boundary faces: the general instantiation (orientation decode included)
+    if (P.boundary) return launch_gradient_t<DIM, NP, AFFINE, (DIM == 3), true>(P, st);
+  }
+  if constexpr (DIM == 3 && !ORIENT3 && !BND) {
     if (P.oriented) return launch_gradient_t<DIM, NP, AFFINE, true>(P, st);
   }
   constexpr int NN = Geo<DIM, NP>::NN, EB = elems_per_block<NN>();
   constexpr int threads = ((EB * NN + 31) / 32) * 32;
   constexpr size_t smem = (size_t)((DIM + 2) * EB * NN + NP * NP) * sizeof(double);
-  auto k = gradient_kernel<DIM, NP, AFFINE, EB, ORIENT3>;
+  auto k = gradient_kernel<DIM, NP, AFFINE, EB, ORIENT3, BND>;
   static std::atomic<unsigned long long> attr_done{0};
   if (cudaError_t err = set_smem_once((const void *)k, smem, attr_done); err != cudaSuccess) return err;
   const long grid = (P.ne + EB - 1) / EB;

@@ -37,7 +37,10 @@ struct PhysCfg {
   }
 };
 
-template <int DIM, int NP, int NSP, int PHYS, bool AFFINE, int EB, int MINB>
+// BND (Navier-Stokes): the instantiation for meshes with boundary faces -- prescribed states, outflow, slip walls and the
+// no-slip adiabatic / isothermal walls of PAPER.md:223 (readings R18, R22); the default one carries no code
+// for them.
+template <int DIM, int NP, int NSP, int PHYS, bool AFFINE, int EB, int MINB, bool BND = false>
 __global__ void __launch_bounds__((PhysCfg<DIM, NP, NSP, PHYS, EB>::NT), MINB)
 stage_phys_kernel(const __grid_constant__ StageParams P) {
   using C = PhysCfg<DIM, NP, NSP, PHYS, EB>;
@@ -86,7 +89,7 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   // neighbour trace of the first face task: in flight during phase N
   double Up0[NVAR], pp0 = 0.0, ap0 = 0.0;
   int pR0 = 0;
-  if (has0) {
+  if (has0 && (!BND || (cn0.y & 3) == FK_CONFORMING)) {
     const int fR = (cn0.y >> 2) & 7, orient = (cn0.y >> 5) & 7;
     int b0, b1;
     partner_index<DIM, NP>(orient, t0.a0, t0.a1, b0, b1);
@@ -163,18 +166,23 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     } else {
       t = decode_task<DIM, NP>(g);
       cn = __ldg(&P.conn[(e0 + t.el) * 2 * DIM + t.f]);
-      const int fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7;
-      int b0, b1;
-      partner_index<DIM, NP>(orient, t.a0, t.a1, b0, b1);
-      pR = face_node_of<DIM, NP>(fR, b0, b1);
-      const double *un = P.u_in + (long)cn.x * NVAR * NN + pR;
+      pR = 0;
+      if (!BND || (cn.y & 3) == FK_CONFORMING) {
+        const int fR = (cn.y >> 2) & 7, orient = (cn.y >> 5) & 7;
+        int b0, b1;
+        partner_index<DIM, NP>(orient, t.a0, t.a1, b0, b1);
+        pR = face_node_of<DIM, NP>(fR, b0, b1);
+        const double *un = P.u_in + (long)cn.x * NVAR * NN + pR;
 #pragma unroll
-      for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
-      if constexpr (PHYS == PH_REACT) {
-        pp = __ldg(&P.Taux[(long)cn.x * NA * NN + pR]);
-        ap = __ldg(&P.Taux[((long)cn.x * NA + 1) * NN + pR]);
+        for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
+        if constexpr (PHYS == PH_REACT) {
+          pp = __ldg(&P.Taux[(long)cn.x * NA * NN + pR]);
+          ap = __ldg(&P.Taux[((long)cn.x * NA + 1) * NN + pR]);
+        }
       }
     }
+    const bool bnd = BND && (cn.y & 3) == FK_BOUNDARY;
+    const int bk = (cn.y >> 2) & 7;                 // boundary kind (boundary faces only)
     const int l = t.f >> 1;
     const double sgn = (t.f & 1) ? 1.0 : -1.0;
     const int idx = t.el * NN + t.p;
@@ -195,6 +203,21 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
         n2 += nv[c] * nv[c];
       }
       nrm = sqrt(n2);
+    }
+    if constexpr (BND) {
+      if (bnd) {
+        // exterior state of the hyperbolic surface flux (R8, R18, R22): prescribed state; outflow: the interior
+        // state; slip wall and the two no-slip walls: the interior state with the normal momentum reflected
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Up[v] = (bk == BC_PRESCRIBED) ? __ldg(&P.bc_state[cn.x * NVAR + v]) : Um[v];
+        if (bk >= BC_SLIP_WALL) {
+          double mn = 0.0;
+#pragma unroll
+          for (int c = 0; c < DIM; ++c) mn += Um[NSP + c] * (nv[c] / nrm);
+#pragma unroll
+          for (int c = 0; c < DIM; ++c) Up[NSP + c] = Um[NSP + c] - 2.0 * mn * (nv[c] / nrm);
+        }
+      }
     }
     Prim<DIM> qp;
     if constexpr (PHYS == PH_REACT) qp = prim_given_pa<DIM, NSP>(Up, pp, ap);
@@ -224,16 +247,32 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     for (int v = 0; v < NVAR; ++v) lift[v] = 0.5 * (Fp[v] - Fm[v]) - hl * (Up[v] - Um[v]);
     if constexpr (PHYS == PH_NS) {
       // viscous part: F_v* = mean of the two sides; own F_v.n = F_inv(U-).n - (own total normal flux in the plane)
-      double Sp[NW * DIM], Fvp[NW];
-#pragma unroll
-      for (int k = 0; k < Tau<DIM>::NTAU; ++k) Sp[k] = __ldg(&P.S[((long)cn.x * Tau<DIM>::NTAU + k) * NN + pR]);
-      viscous_flux_dot_tau<DIM>(qp.v, Sp, nv, Fvp);
       const int qk = (DIM == 3) ? t.p / (NP * NP) : 0;
       const int sp = t.p + (KS - NP * NP) * qk;
+      if (bnd) {
+        // viscous wall flux F_v*(U_w, S-) (reading R22): momentum rows = the wall shear stress, as the element's own;
+        // energy row: no stress work (v_w = 0), the heat flux k grad T . n at an isothermal wall, nothing at an
+        // adiabatic one.  Prescribed / outflow / slip faces: F_v* = F_v(U-, S-), no viscous surface term.
+        if (bk >= BC_WALL_ADIABATIC) {
+          double FwE = 0.0;
+          if (bk == BC_WALL_ISOTHERMAL) {
 #pragma unroll
-      for (int v = 1; v < NVAR; ++v) {
-        const double Fvm = Fm[v] - sgn * Fsm[((l * NVAR + v) * EB + t.el) * PS + sp];
-        lift[v] -= 0.5 * (Fvp[v] - Fvm);
+            for (int j = 0; j < DIM; ++j)
+              FwE += __ldg(&P.S[(ee * Tau<DIM>::NTAU + DIM * (DIM + 1) / 2 + j) * NN + t.p]) * nv[j];
+          }
+          const double FvmE = Fm[NVAR - 1] - sgn * Fsm[((l * NVAR + NVAR - 1) * EB + t.el) * PS + sp];
+          lift[NVAR - 1] -= FwE - FvmE;
+        }
+      } else {
+        double Sp[NW * DIM], Fvp[NW];
+#pragma unroll
+        for (int k = 0; k < Tau<DIM>::NTAU; ++k) Sp[k] = __ldg(&P.S[((long)cn.x * Tau<DIM>::NTAU + k) * NN + pR]);
+        viscous_flux_dot_tau<DIM>(qp.v, Sp, nv, Fvp);
+#pragma unroll
+        for (int v = 1; v < NVAR; ++v) {
+          const double Fvm = Fm[v] - sgn * Fsm[((l * NVAR + v) * EB + t.el) * PS + sp];
+          lift[v] -= 0.5 * (Fvp[v] - Fvm);
+        }
       }
     }
 #pragma unroll
@@ -319,13 +358,16 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   }
 }
 
-template <int DIM, int NP, int NSP, int PHYS, bool AFFINE>
+template <int DIM, int NP, int NSP, int PHYS, bool AFFINE, bool BND = false>
 cudaError_t launch_stage_phys_t(const StageParams &P, cudaStream_t st) {
+  if constexpr (PHYS == PH_NS && !BND) {
+    if (P.bc_kinds) return launch_stage_phys_t<DIM, NP, NSP, PHYS, AFFINE, true>(P, st);
+  }
   constexpr int NN = Geo<DIM, NP>::NN, EB = node_eb<NN>();
   using C = PhysCfg<DIM, NP, NSP, PHYS, EB>;
   constexpr size_t smem = C::smem_doubles(AFFINE) * sizeof(double);
   constexpr int MINB = (C::NT <= 128) ? MARUT_PHYS_MINB128 : ((C::NT <= 256) ? 2 : 1);
-  auto k = stage_phys_kernel<DIM, NP, NSP, PHYS, AFFINE, EB, MINB>;
+  auto k = stage_phys_kernel<DIM, NP, NSP, PHYS, AFFINE, EB, MINB, BND>;
   static std::atomic<unsigned long long> attr_done{0};
   if (cudaError_t err = set_smem_once((const void *)k, smem, attr_done); err != cudaSuccess) return err;
   const long grid = (P.ne + EB - 1) / EB;
