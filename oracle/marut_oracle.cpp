@@ -1259,7 +1259,7 @@ int oracle_set_volume_form(void *h, int form) {
 // alpha: [n_elem] blending coefficients of eq. 11 (copied), or NULL to switch the blending off
 int oracle_set_blend(void *h, const double *alpha) {
   Mesh *m = (Mesh *)h;
-  if (alpha && m->physics != EULER) return 1;
+  if (alpha && m->physics == REACTING_EULER) return 1;   // eq. 11 blends the hyperbolic volume residual (Euler, Navier-Stokes)
   if (alpha) m->alpha.assign(alpha, alpha + m->ne); else m->alpha.clear();
   return 0;
 }

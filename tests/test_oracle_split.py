@@ -186,3 +186,43 @@ def test_split_form_semi_discrete_entropy_rate_is_the_interface_dissipation():
             prod += w[j] * ((wp - wm) @ Fs - (mp - mm) @ nv)
     assert prod < 0.0
     assert abs(rate - prod) <= 1e-9 * abs(prod)      # the series branch of the logarithmic mean again (1.2e-11 here)
+
+
+def test_split_form_and_blend_with_the_viscous_terms():
+    """'Three operators are available and selected once at solver setup' -- the split form and the
+    DG/FV blend replace the HYPERBOLIC volume integral; the parabolic RHS (Table 2) is added unchanged.
+    On the curved periodic Navier-Stokes mesh of config 3: free stream, conservation of mass, momentum and energy with a
+    random blending field, and the viscous contribution (difference to the Euler operator on the same mesh) equal for
+    the three volume operators."""
+    c = wl.make_case("c3", cells=3)
+    rng = np.random.default_rng(9)
+    alpha = rng.uniform(0, 1, c.mesh.n_elem)
+    u = wl.taylor_green(c.mesh, noise=1e-2)
+
+    def operators(physics, mu):
+        out = []
+        for form, a in ((0, None), (1, None), (1, alpha)):
+            c.mesh.physics, c.mesh.mu, c.mesh.volume_form = physics, mu, form
+            om = oracle.OracleMesh(c.mesh)
+            om.set_blend(a)
+            out.append(om)
+        return out
+
+    ns = operators(wl.NAVIER_STOKES, 1.0 / 100.0)
+    eu = operators(wl.EULER, 0.0)
+    _, J = ns[0].metrics()
+    _, w, _ = oracle.operators(c.mesh.N)
+    W = np.einsum("k,j,i->kji", w, w, w).reshape(-1)
+    const = np.broadcast_to(_cons(1.3, [0.4, -0.2, 0.7], 2.1)[None, :, None], u.shape).copy()
+    visc = []
+    for om_ns, om_eu in zip(ns, eu):
+        assert np.abs(om_ns.rhs(const)).max() < 2e-11
+        r = om_ns.rhs(u)
+        total = np.einsum("evn,en,n->v", r, J, W)
+        scale = np.einsum("evn,en,n->v", np.abs(r), J, W)
+        assert np.all(np.abs(total) <= 1e-12 * scale)
+        visc.append(r - om_eu.rhs(u))
+    assert np.abs(visc[0]).max() > 1e-3
+    assert np.abs(visc[1] - visc[0]).max() <= 1e-12 * np.abs(ns[0].rhs(u)).max()
+    assert np.abs(visc[2] - visc[0]).max() <= 1e-12 * np.abs(ns[0].rhs(u)).max()
+    c.mesh.volume_form = 0
