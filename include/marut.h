@@ -175,7 +175,8 @@ marut_status marut_shock_indicator(marut_mesh *mesh, const double *u, double s, 
  * alpha: DEVICE, [n_elem], values in [0,1] -- normally the output of marut_shock_indicator for the same state.  The
  * pointer is KEPT, not copied: the caller owns the buffer, may rewrite it between stages (the paper recomputes it once
  * per Runge-Kutta substage), and must keep it alive until marut_set_blend(mesh, NULL) or marut_mesh_destroy.
- * NULL switches the blending off (default).  MARUT_EULER meshes; marut_rhs / marut_ssprk_stage return EINVAL while a
+ * NULL switches the blending off (default).  MARUT_EULER and MARUT_NAVIER_STOKES meshes (the blend acts on the hyperbolic
+ * volume residual); marut_rhs / marut_ssprk_stage return EINVAL while a
  * blending field is set unless the volume form is MARUT_VOLUME_SPLIT_RANOCHA (eq. 11 blends the split form).  On a
  * curved mesh the first call allocates and fills the sub-cell normals ([n_elem][dim][dim][n^dim] doubles). */
 marut_status marut_set_blend(marut_mesh *mesh, const double *alpha);
@@ -245,7 +246,9 @@ marut_status marut_set_explicit_source(marut_mesh *mesh, int on);
  * MARUT_VOLUME_SPLIT_RANOCHA: the entropy-stable split form, eq. 10,
  *   R_i = -(2/J_i) sum_l sum_m D_{i_l m} F#(U_i, U_m; 1/2 (Ja^l_i + Ja^l_m)),
  * with the two-point flux of Ranocha (eq. 41) and logarithmic means (R13); the surface
- * terms are unchanged.  MARUT_EULER meshes with N <= 7 (2-D) / N <= 6 (3-D) only (else EINVAL).  Takes effect from the next call. */
+ * terms are unchanged.  MARUT_EULER and MARUT_NAVIER_STOKES meshes with N <= 7 (2-D) / N <= 6 (3-D) (else EINVAL).  The
+ * form replaces the HYPERBOLIC volume integral only: on a Navier-Stokes mesh the parabolic RHS (eq. 13-16) is added
+ * unchanged by a second kernel launch of the stage.  Takes effect from the next call. */
 enum { MARUT_VOLUME_STRONG = 0, MARUT_VOLUME_SPLIT_RANOCHA = 1 };
 marut_status marut_set_volume_form(marut_mesh *mesh, int form);
 

@@ -534,6 +534,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.bc_state = m->d_bc; P.S = m->d_S; P.Taux = m->d_T; P.mech = m->d_mech;
   P.ca = ca; P.cb = cb; P.cc = cc; P.dt_dev = dt_dev;
   P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne; P.num_sms = m->num_sms;
+  P.visc_only = 0;
   P.red_next = nullptr; P.dt_next = nullptr; P.cfl = 0.0; P.dx_min = m->dx_min; P.P2 = 2.0 * m->N + 1.0;
   memcpy(P.D, m->D, sizeof(P.D));
   P.mflux = m->d_mflux;
@@ -548,7 +549,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.bc_kinds = (m->bc_kinds || (m->dim == 3 && m->n_mortar > 0) || (m->physics == MARUT_NAVIER_STOKES && m->n_bface > 0)) ? 1 : 0;
   for (int i = 0; i < MAX_NP; ++i) P.inv_w[i] = (i < m->np) ? 1.0 / m->w[i] : 0.0;
   if (m->d_alpha) {
-    if (m->physics != MARUT_EULER || m->volume_form != MARUT_VOLUME_SPLIT_RANOCHA)
+    if (m->physics == MARUT_REACTING_EULER || m->volume_form != MARUT_VOLUME_SPLIT_RANOCHA)
       return fail(MARUT_EINVAL, "a blending field is set: the DG/FV blend needs MARUT_VOLUME_SPLIT_RANOCHA (eq. 11)");
     P.alpha = m->d_alpha;
   }
@@ -570,7 +571,17 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
           e = (m->dim == 2) ? launch_stage_node2d(m->np, m->affine, P, st) : launch_stage_node3d(m->np, m->affine, P, st);
       }
       break;
-    case MARUT_NAVIER_STOKES: e = launch_stage_ns(m->dim, m->np, m->affine, P, st); break;
+    case MARUT_NAVIER_STOKES:
+      if (m->volume_form == MARUT_VOLUME_SPLIT_RANOCHA) {
+        // hyperbolic part with the split-form (and blended) volume integral, then the parabolic part added to u_out
+        // (the two pipelines add their contributions into one residual)
+        e = launch_stage_split(m->dim, m->np, m->affine, P, st);
+        if (e != cudaSuccess) break;
+        m->launches++;
+        P.visc_only = 1;
+        e = launch_stage_ns(m->dim, m->np, m->affine, P, st);
+      } else e = launch_stage_ns(m->dim, m->np, m->affine, P, st);
+      break;
     default: e = launch_stage_react(m->dim, m->np, m->nsp, m->affine, P, st); break;
   }
   if (e == cudaErrorNotSupported) return fail(MARUT_EINVAL, "no kernel instantiated for dim=%d N=%d physics=%d", m->dim, m->N, m->physics);
@@ -614,7 +625,7 @@ __global__ void subcell_normals_kernel(const __grid_constant__ SubnParams P) {
 extern "C" marut_status marut_set_blend(marut_mesh *m, const double *alpha) {
   if (!m) return fail(MARUT_EINVAL, "NULL argument");
   if (!alpha) { m->d_alpha = nullptr; return MARUT_OK; }
-  if (m->physics != MARUT_EULER) return fail(MARUT_EINVAL, "the DG/FV blend is implemented for MARUT_EULER only");
+  if (m->physics == MARUT_REACTING_EULER) return fail(MARUT_EINVAL, "the DG/FV blend is implemented for MARUT_EULER and MARUT_NAVIER_STOKES");
   if (!m->affine && !m->d_subn) {
     const size_t n = (size_t)m->ne * m->dim * m->dim * m->nn;
     CUDA_TRY(cudaMalloc(&m->d_subn, n * sizeof(double)));
@@ -632,8 +643,8 @@ extern "C" marut_status marut_set_blend(marut_mesh *m, const double *alpha) {
 extern "C" marut_status marut_set_volume_form(marut_mesh *m, int form) {
   if (!m) return fail(MARUT_EINVAL, "NULL argument");
   if (form != MARUT_VOLUME_STRONG && form != MARUT_VOLUME_SPLIT_RANOCHA) return fail(MARUT_EINVAL, "unknown volume form %d", form);
-  if (form == MARUT_VOLUME_SPLIT_RANOCHA && m->physics != MARUT_EULER)
-    return fail(MARUT_EINVAL, "the split-form volume integral is implemented for MARUT_EULER only");
+  if (form == MARUT_VOLUME_SPLIT_RANOCHA && m->physics == MARUT_REACTING_EULER)
+    return fail(MARUT_EINVAL, "the split-form volume integral is implemented for MARUT_EULER and MARUT_NAVIER_STOKES");
   if (form == MARUT_VOLUME_SPLIT_RANOCHA && m->np > (m->dim == 2 ? 8 : 7)) return fail(MARUT_EINVAL, "split form: N <= 7 in 2-D, N <= 6 in 3-D");
   m->volume_form = form;
   return MARUT_OK;

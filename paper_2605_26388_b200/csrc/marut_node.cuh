@@ -297,13 +297,13 @@ __device__ __forceinline__ void euler_face_task(const StageParams &P, const doub
   for (int c = 0; c < DIM; ++c) Fm[1 + c] = Um[1 + c] * vnm + pm * nv[c];
   Fm[DIM + 1] = (Um[DIM + 1] + pm) * vnm;
   const int kind = cn.y & 3;
-  if (BCK && kind == FK_BOUNDARY && (cn.y & (3 << 2)) != 0) {
+  if (BCK && kind == FK_BOUNDARY && ((cn.y >> 2) & 7) != BC_PRESCRIBED) {
     // outflow / slip-wall face (marut_set_boundary_kinds; R18), the Rusanov flux in closed form:
     // outflow U+ = U-: F* = F(U-).nv, no lift.  Slip wall U+ = U- with m+ = m- - 2 (m-.nhat) nhat: same rho, E, p, a and
     // v+.nv = -v-.nv, so the mass and energy components of F* vanish.
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) lift[v] = 0.0;
-    if (((cn.y >> 2) & 3) == BC_SLIP_WALL) {
+    if (((cn.y >> 2) & 7) >= BC_SLIP_WALL) {      // slip wall; the no-slip walls of a Navier-Stokes mesh use its hyperbolic flux (R22)
       const double hl = 0.5 * (fabs(vnm) + am * nrm);
       const double r = 2.0 * mnm / (nrm * nrm);
       lift[0] = -P.inv_wb * Fm[0];

@@ -40,7 +40,10 @@ struct PhysCfg {
 // BND (Navier-Stokes): the instantiation for meshes with boundary faces -- prescribed states, outflow, slip walls and the
 // no-slip adiabatic / isothermal walls of PAPER.md:223 (readings R18, R22); the default one carries no code
 // for them.
-template <int DIM, int NP, int NSP, int PHYS, bool AFFINE, int EB, int MINB, bool BND = false>
+// VONLY (Navier-Stokes): the parabolic operator alone, ADDED to u_out: u_out += cc * L_visc(u_in).  Second launch of a
+// stage whose hyperbolic part ran in stage_split_kernel (split-form / blended volume integral, PAPER.md:183-191, 208:
+// the two pipelines "add their contributions into a shared residual buffer").
+template <int DIM, int NP, int NSP, int PHYS, bool AFFINE, int EB, int MINB, bool BND = false, bool VONLY = false>
 __global__ void __launch_bounds__((PhysCfg<DIM, NP, NSP, PHYS, EB>::NT), MINB)
 stage_phys_kernel(const __grid_constant__ StageParams P) {
   using C = PhysCfg<DIM, NP, NSP, PHYS, EB>;
@@ -121,7 +124,10 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
 #pragma unroll
     for (int l = 0; l < DIM; ++l) {
       double F[NVAR];
-      flux_dot<DIM, NSP>(U, pr, &Ja[l * DIM], F);
+      if constexpr (VONLY) {
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) F[v] = 0.0;
+      } else flux_dot<DIM, NSP>(U, pr, &Ja[l * DIM], F);
       if constexpr (PHYS == PH_NS) {
         double Fv[NW];
         viscous_flux_dot_tau<DIM>(pr.v, Sg, &Ja[l * DIM], Fv);
@@ -245,6 +251,10 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     Fp[NSP + DIM] = (Up[NSP + DIM] + qp.p) * vnp;
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) lift[v] = 0.5 * (Fp[v] - Fm[v]) - hl * (Up[v] - Um[v]);
+    if constexpr (VONLY) {      // no hyperbolic surface term; the flux planes hold -F_v . Ja, so the own F_v.n = -(plane) sgn
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) { lift[v] = 0.0; Fm[v] = 0.0; }
+    }
     if constexpr (PHYS == PH_NS) {
       // viscous part: F_v* = mean of the two sides; own F_v.n = F_inv(U-).n - (own total normal flux in the plane)
       const int qk = (DIM == 3) ? t.p / (NP * NP) : 0;
@@ -299,7 +309,7 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   }
 
   // ---- last pass (zeta in 3-D, eta in 2-D) fused with phase D: lifts, 1/J, source, SSP-RK combination
-  const bool use_un = (P.ca != 0.0);
+  const bool use_un = !VONLY && (P.ca != 0.0);
   for (int t = tid; t < nline; t += NT) {
     const int le = t / NLT, r = t - le * NLT;
     const int v = r / NL, ij = r - v * NL;
@@ -352,14 +362,21 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       if constexpr (PHYS == PH_REACT) {
         if (v < NSP && P.explicit_source) src = __ldg(&P.Taux[(ee * NA + 2 + v) * NN + ij + m * GS]);
       }
-      const double val = P.cb * us[m * GS] + stage_cc(P) * (src - invJ * acc[m]);
-      P.u_out[gofs + m * GS] = use_un ? (P.ca * un[m] + val) : val;
+      if constexpr (VONLY) {
+        P.u_out[gofs + m * GS] += stage_cc(P) * (0.0 - invJ * acc[m]);
+      } else {
+        const double val = P.cb * us[m * GS] + stage_cc(P) * (src - invJ * acc[m]);
+        P.u_out[gofs + m * GS] = use_un ? (P.ca * un[m] + val) : val;
+      }
     }
   }
 }
 
-template <int DIM, int NP, int NSP, int PHYS, bool AFFINE, bool BND = false>
+template <int DIM, int NP, int NSP, int PHYS, bool AFFINE, bool BND = false, bool VONLY = false>
 cudaError_t launch_stage_phys_t(const StageParams &P, cudaStream_t st) {
+  if constexpr (PHYS == PH_NS && !VONLY) {
+    if (P.visc_only) return launch_stage_phys_t<DIM, NP, NSP, PHYS, AFFINE, true, true>(P, st);   // (one instantiation: with boundary code)
+  }
   if constexpr (PHYS == PH_NS && !BND) {
     if (P.bc_kinds) return launch_stage_phys_t<DIM, NP, NSP, PHYS, AFFINE, true>(P, st);
   }
@@ -367,7 +384,7 @@ cudaError_t launch_stage_phys_t(const StageParams &P, cudaStream_t st) {
   using C = PhysCfg<DIM, NP, NSP, PHYS, EB>;
   constexpr size_t smem = C::smem_doubles(AFFINE) * sizeof(double);
   constexpr int MINB = (C::NT <= 128) ? MARUT_PHYS_MINB128 : ((C::NT <= 256) ? 2 : 1);
-  auto k = stage_phys_kernel<DIM, NP, NSP, PHYS, AFFINE, EB, MINB, BND>;
+  auto k = stage_phys_kernel<DIM, NP, NSP, PHYS, AFFINE, EB, MINB, BND, VONLY>;
   static std::atomic<unsigned long long> attr_done{0};
   if (cudaError_t err = set_smem_once((const void *)k, smem, attr_done); err != cudaSuccess) return err;
   const long grid = (P.ne + EB - 1) / EB;

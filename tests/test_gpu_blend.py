@@ -85,11 +85,10 @@ def test_blend_needs_the_split_form():
     gm.set_blend(None)
     gm.rhs(u, torch.empty_like(u))
     gm.close()
-    ns = _mesh(2, 3, 4, False)
-    ns.physics, ns.mu = wl.NAVIER_STOKES, 0.01
-    gn = mb.MarutMesh(ns)
+    rc = wl.make_case("c5", cells=3)                 # reacting meshes have no blend (Navier-Stokes ones do: test_gpu_ns_split.py)
+    gn = mb.MarutMesh(rc.mesh)
     with pytest.raises(mb.MarutError):
-        gn.set_blend(torch.zeros(ns.n_elem, dtype=torch.float64, device="cuda"))
+        gn.set_blend(torch.zeros(rc.mesh.n_elem, dtype=torch.float64, device="cuda"))
     gn.close()
 
 
