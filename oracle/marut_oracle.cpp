@@ -811,7 +811,7 @@ static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
 }
 
 // ---------------------------------------------------------------------------
-// O9. BR1 viscous residual; conforming interfaces and boundary faces (O9b).
+// O9. BR1 viscous residual; conforming interfaces, boundary faces (O9b), 2-D mortars (O9c).
 // W = (rho, u_1..u_d, T), T = p/rho.  S[e][node][w][c] = d W_w / d x_c.
 // ---------------------------------------------------------------------------
 static void prim_gradient_vars(const Mesh &m, const double *U, double *W) {
@@ -893,6 +893,41 @@ static void br1_gradient(const Mesh &m, const double *u, std::vector<double> &S)
       }
     }
   }
+  // O9c. 2:1 mortars, 2-D ("Non-conforming faces use the same forward and reverse projections as the
+  // hyperbolic side"; reading R23): the coarse trace of W is interpolated to each mortar (P_fwd), the central
+  // trace What is formed at the fine face nodes; the fine side lifts (What - W_F) n_F; the coarse side lifts the L2
+  // projection (P_rev, area factor 2) of the mortar's outward What n, G*_C = sum_m P_rev^m (2 (-What_m n_F)), against
+  // its own W_C n_C -- the hyperbolic mortar with the flux F.n replaced by W n.
+  for (size_t q = 0; d == 2 && q < m.mortar.size() / 6; ++q) {
+    const int *M = &m.mortar[q * 6];
+    const long eC = M[0]; const int fC = M[1], fF = M[4];
+    std::vector<double> WC((size_t)n * nw), GC((size_t)n * nw * d, 0.0);
+    for (int j = 0; j < n; ++j) { double U[MAXV]; gather(m, u, eC, face_node(m, fC, j), U); prim_gradient_vars(m, U, &WC[(size_t)j * nw]); }
+    for (int s = 0; s < 2; ++s) {
+      const long eF = M[2 + s];
+      for (int a = 0; a < n; ++a) {
+        const int pF = face_node(m, fF, a);
+        double UF[MAXV], WF[MAXV], nF[3];
+        gather(m, u, eF, pF, UF); prim_gradient_vars(m, UF, WF); face_normal(m, eF, fF, pF, nF);
+        for (int w = 0; w < nw; ++w) {
+          double Wi = 0.0;
+          for (int j = 0; j < n; ++j) Wi += m.Pf[s][a * n + j] * WC[(size_t)j * nw + w];
+          const double What = 0.5 * (WF[w] + Wi);
+          for (int c = 0; c < d; ++c) {
+            S[(((size_t)eF * nn + pF) * nw + w) * d + c] += (What - WF[w]) * nF[c] / wb;
+            for (int i = 0; i < n; ++i) GC[((size_t)i * nw + w) * d + c] += m.Pr_[s][i * n + a] * (2.0 * (-(What * nF[c])));
+          }
+        }
+      }
+    }
+    for (int i = 0; i < n; ++i) {
+      const int pC = face_node(m, fC, i);
+      double nC[3]; face_normal(m, eC, fC, pC, nC);
+      for (int w = 0; w < nw; ++w)
+        for (int c = 0; c < d; ++c)
+          S[(((size_t)eC * nn + pC) * nw + w) * d + c] += (GC[((size_t)i * nw + w) * d + c] - WC[(size_t)i * nw + w] * nC[c]) / wb;
+    }
+  }
   // O9b. boundary faces (reading R22): the trace What is fixed by the boundary kind --
   //   prescribed state: the central trace with W(U_bc);  outflow: W- (no jump);  slip wall: "mirrors the velocity across
   //   the boundary normal", W+ = (rho-, v- - 2 (v-.nhat) nhat, T-), central trace;  no-slip adiabatic wall: "sets the wall
@@ -970,6 +1005,47 @@ static void rhs_viscous_add(const Mesh &m, const double *u, double *du) {
         du[((size_t)eL * nvar + v) * nn + pL] += (0.5 * (FmL[v] + FpL[v]) - FmL[v]) / (JL * wb);
         du[((size_t)eR * nvar + v) * nn + pR] += (0.5 * (FpR[v] + FmR[v]) - FpR[v]) / (JR * wb);
       }
+    }
+  }
+  // O9c. 2:1 mortars, 2-D ("a central surface pipeline (interface, mortar, and boundary kernels)"; reading
+  // R23): state AND gradient of the coarse side are interpolated to the mortar (P_fwd), F_v* = mean of the two sides'
+  // viscous fluxes with the fine-side normal; the fine side lifts F_v* - F_v,F; the coarse side lifts the projection
+  // sum_m P_rev^m (2 (-F_v*_m)) against its own F_v(U_C, S_C).n_C.
+  for (size_t q = 0; d == 2 && q < m.mortar.size() / 6; ++q) {
+    const int *M = &m.mortar[q * 6];
+    const long eC = M[0]; const int fC = M[1], fF = M[4];
+    const int ng = nw * d;
+    std::vector<double> UC((size_t)n * nvar), SC((size_t)n * ng), FC((size_t)n * nvar, 0.0);
+    for (int j = 0; j < n; ++j) {
+      const int pC = face_node(m, fC, j);
+      gather(m, u, eC, pC, &UC[(size_t)j * nvar]);
+      for (int k = 0; k < ng; ++k) SC[(size_t)j * ng + k] = S[((size_t)eC * nn + pC) * ng + k];
+    }
+    for (int s = 0; s < 2; ++s) {
+      const long eF = M[2 + s];
+      for (int a = 0; a < n; ++a) {
+        const int pF = face_node(m, fF, a);
+        double UF[MAXV], Ui[MAXV], Si[MAXV * 3], nF[3], FvF[MAXV], FvC[MAXV];
+        gather(m, u, eF, pF, UF); face_normal(m, eF, fF, pF, nF);
+        for (int v = 0; v < nvar; ++v) { double ui = 0.0; for (int j = 0; j < n; ++j) ui += m.Pf[s][a * n + j] * UC[(size_t)j * nvar + v]; Ui[v] = ui; }
+        for (int k = 0; k < ng; ++k) { double si = 0.0; for (int j = 0; j < n; ++j) si += m.Pf[s][a * n + j] * SC[(size_t)j * ng + k]; Si[k] = si; }
+        viscous_flux_dot(m, UF, &S[((size_t)eF * nn + pF) * ng], nF, FvF);
+        viscous_flux_dot(m, Ui, Si, nF, FvC);
+        const double JF = m.J[(size_t)eF * nn + pF];
+        for (int v = 0; v < nvar; ++v) {
+          const double Fs = 0.5 * (FvF[v] + FvC[v]);
+          du[((size_t)eF * nvar + v) * nn + pF] += (Fs - FvF[v]) / (JF * wb);
+          for (int i = 0; i < n; ++i) FC[(size_t)i * nvar + v] += m.Pr_[s][i * n + a] * (2.0 * (-Fs));
+        }
+      }
+    }
+    for (int i = 0; i < n; ++i) {
+      const int pC = face_node(m, fC, i);
+      double nC[3], Fo[MAXV];
+      face_normal(m, eC, fC, pC, nC);
+      viscous_flux_dot(m, &UC[(size_t)i * nvar], &SC[(size_t)i * ng], nC, Fo);
+      const double JC = m.J[(size_t)eC * nn + pC];
+      for (int v = 0; v < nvar; ++v) du[((size_t)eC * nvar + v) * nn + pC] += (FC[(size_t)i * nvar + v] - Fo[v]) / (JC * wb);
     }
   }
   // O9b. boundary faces ("boundary kernels"; the wall flux is not printed: DESIGN.md reading R22).

@@ -36,6 +36,22 @@ MUTATIONS = {
         "pvn += 0.5 * (L.p * R.vel[c] + R.p * L.vel[c]) * nv[c];",
         "pvn += 0.5 * (L.p * L.vel[c] + R.p * R.vel[c]) * nv[c];",
         "pressure work {{p v}} as PAPER.md:621 prints it: not entropy conservative"),
+    "br1_mortar_wrong_half": (
+        "Wi += m.Pf[s][a * n + j] * WC[(size_t)j * nw + w];",
+        "Wi += m.Pf[1 - s][a * n + j] * WC[(size_t)j * nw + w];",
+        "BR1 gradient across a 2-D mortar: the coarse trace of W is interpolated to the wrong half"),
+    "br1_mortar_no_area_factor": (
+        "m.Pr_[s][i * n + a] * (2.0 * (-(What * nF[c])));",
+        "m.Pr_[s][i * n + a] * (1.0 * (-(What * nF[c])));",
+        "BR1 gradient across a 2-D mortar: the coarse side's projected trace misses the 2:1 area factor"),
+    "viscous_mortar_gradient_wrong_half": (
+        "si += m.Pf[s][a * n + j] * SC[(size_t)j * ng + k];",
+        "si += m.Pf[1 - s][a * n + j] * SC[(size_t)j * ng + k];",
+        "viscous flux across a 2-D mortar: the coarse gradient is interpolated to the wrong half"),
+    "viscous_mortar_no_area_factor": (
+        "m.Pr_[s][i * n + a] * (2.0 * (-Fs));",
+        "m.Pr_[s][i * n + a] * (1.0 * (-Fs));",
+        "viscous flux across a 2-D mortar: the coarse side's projected flux misses the 2:1 area factor"),
 }
 
 _cache = {}
