@@ -36,7 +36,7 @@ if ROOT not in sys.path:
 METRIC = "DG RHS+SSPRK3 DOF-stage updates/s (FP64)"
 UNIT = "DOF-stage/s"
 # bounded oracle samples: (cells per direction, target seconds)
-ORACLE_SAMPLE_CELLS = {"c1": None, "c2": 12, "c2s": 12, "c3": 16, "c4": 64, "c4w": 64, "c4b": 64, "c5": 8, "c2m": 8}
+ORACLE_SAMPLE_CELLS = {"c1": None, "c2": 12, "c2s": 12, "c3": 16, "c4": 64, "c4w": 64, "c4b": 64, "c4v": 64, "c5": 8, "c2m": 8}
 # c4b: per-stage Hennemann-Gassner indicator (binding defaults, R15) feeding the DG/FV blend
 SHOCK_CAPTURE = dict(s=9.21024, alpha_min=1e-3, alpha_max=0.5, smooth=True)
 
@@ -45,7 +45,8 @@ def make_workload(name, cells=None):
     """c1..c5, c4w: the configs of BASELINE.json (workloads.make_case); c2s: c2 with the entropy-stable split-form
     volume integral; c4b: c4w as a shock-capturing run -- split form, and in
     every Runge-Kutta stage the shock indicator of the stage's input state, the blended DG/FV stage and the positivity floor;
-    c2m: the Taylor-Green flow of c2 on a box with one half refined once (3-D 4:1 mortar faces, NEXT-4)"""
+    c2m: the Taylor-Green flow of c2 on a box with one half refined once (3-D 4:1 mortar faces, NEXT-4);
+    c4v: c4w as a Navier-Stokes problem (BR1 across the 2-D mortars, NEXT-4)"""
     import workloads as wl
 
     if name == "c2m":
@@ -61,6 +62,12 @@ def make_workload(name, cells=None):
         # shock profile one fine element wide: the indicator flags it (alpha_e reaches alpha_max along the shock); the
         # 6-element profile of c4 / c4w is resolved at N = 3 and would leave alpha_e = 0 everywhere
         c.u0 = wl.mach10_shock(c.mesh, half_width=1.0 * c.mesh.info["h_fine"])
+        return c
+    if name == "c4v":
+        # c4w's mesh and shock as a Navier-Stokes problem: BR1 across 2-D 2:1 mortars (NEXT-4; R23)
+        c = wl.make_case("c4w", cells=cells)
+        c.mesh.physics, c.mesh.mu, c.mesh.Pr = wl.NAVIER_STOKES, 1e-3, 0.72
+        c.name = "c4v"
         return c
     if name == "c2s":
         c = wl.make_case("c2", cells=cells)

@@ -70,6 +70,7 @@ typedef struct {
   long n_mortar;
   const int *mortar;      /* 2-D: [n_mortar][6] = eC,fC,eF_lo,eF_up,fF,orient : 2:1 hanging faces;
                              eF_lo covers the coarse face parameter [-1,0], eF_up covers [0,1]; orient must be 0.
+                             EULER and NAVIER_STOKES (BR1 across the mortar: PAPER.md:223, R23).
                              3-D: [n_mortar][8] = eC,fC,eF_00,eF_10,eF_01,eF_11,fF,orient : 4:1 hanging faces (DESIGN.md
                              R21); eF_{s0 s1} covers half s0 / s1 of the coarse face's first / second face-local direction
                              (the remaining reference directions in increasing order); orient must be 0; EULER, affine

@@ -257,8 +257,8 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   if (d->physics < 0 || d->physics > 2) return fail(MARUT_EINVAL, "unknown physics %d", d->physics);
   if (d->physics == MARUT_REACTING_EULER && (d->n_mortar || d->n_bface))
     return fail(MARUT_EINVAL, "REACTING_EULER supports conforming interior faces only");
-  if (d->physics == MARUT_NAVIER_STOKES && d->n_mortar)
-    return fail(MARUT_EINVAL, "NAVIER_STOKES supports conforming interior faces and boundary faces, no mortars");
+  if (d->physics == MARUT_NAVIER_STOKES && d->n_mortar && d->dim == 3)
+    return fail(MARUT_EINVAL, "NAVIER_STOKES: mortar faces are implemented in 2-D only");
   if (d->physics != MARUT_REACTING_EULER && !(d->gamma > 1.0)) return fail(MARUT_EINVAL, "gamma must be > 1");
   if (d->physics == MARUT_NAVIER_STOKES && (!(d->mu >= 0.0) || !(d->Pr > 0.0))) return fail(MARUT_EINVAL, "need mu >= 0, Pr > 0");
 
@@ -513,7 +513,8 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
     GradParams G;
     G.u = u_in; G.S = m->d_S; G.metric = m->d_metric; G.conn = m->d_conn;
     G.gamma = m->gamma; G.inv_wb = 1.0 / m->w[0]; G.mu = m->mu; G.kappa = m->kappa; G.ne = m->ne; G.oriented = m->oriented ? 1 : 0;
-    G.bc_state = m->d_bc; G.boundary = m->n_bface > 0 ? 1 : 0;
+    G.bc_state = m->d_bc; G.boundary = (m->n_bface > 0 || m->n_mortar > 0) ? 1 : 0;
+    G.mortar_fine = m->d_mortar_fine; G.mortar_mat = m->d_mortar_mat;
     memcpy(G.D, m->D, sizeof(G.D));
     cudaError_t e = launch_gradient(m->dim, m->np, m->affine, G, st);
     if (e != cudaSuccess) return fail(e == cudaErrorNotSupported ? MARUT_EINVAL : MARUT_ECUDA, "gradient kernel: %s", cudaGetErrorString(e));
@@ -545,8 +546,8 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
     m->launches++;
   }
   P.alpha = nullptr; P.subn = m->d_subn;
-  // Euler: outflow / slip-wall faces or 3-D mortars exist; Navier-Stokes: the mesh has boundary faces of any kind
-  P.bc_kinds = (m->bc_kinds || (m->dim == 3 && m->n_mortar > 0) || (m->physics == MARUT_NAVIER_STOKES && m->n_bface > 0)) ? 1 : 0;
+  // Euler: outflow / slip-wall faces or 3-D mortars exist; Navier-Stokes: the mesh has boundary faces of any kind or mortars
+  P.bc_kinds = (m->bc_kinds || (m->dim == 3 && m->n_mortar > 0) || (m->physics == MARUT_NAVIER_STOKES && (m->n_bface > 0 || m->n_mortar > 0))) ? 1 : 0;
   for (int i = 0; i < MAX_NP; ++i) P.inv_w[i] = (i < m->np) ? 1.0 / m->w[i] : 0.0;
   if (m->d_alpha) {
     if (m->physics == MARUT_REACTING_EULER || m->volume_form != MARUT_VOLUME_SPLIT_RANOCHA)

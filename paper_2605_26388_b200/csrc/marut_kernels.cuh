@@ -78,7 +78,9 @@ struct GradParams {
   double D[MAX_NP * MAX_NP];
   int oriented;                        // 3-D: some interface has a non-trivial orientation code
   const double *__restrict__ bc_state; // [bc][nvar] prescribed states of the boundary ids (kind 0; kind 4: their T is T_wall)
-  int boundary;                        // the mesh has boundary faces: launch the instantiation that knows them
+  int boundary;                        // the mesh has boundary or mortar faces: launch the instantiation that knows them
+  const int *__restrict__ mortar_fine; // 2-D mortars: [m][2] fine elements (lo, up)
+  const double *__restrict__ mortar_mat; // [4][n*n]: Pf_lo, Pf_up, Pr_lo, Pr_up
 };
 
 // BR1 trace jump What - W at a boundary face node (reading R22).  kind: 0 prescribed state
@@ -115,9 +117,85 @@ __device__ __forceinline__ void br1_boundary_jump(int kind, const double *W, con
   }
 }
 
+// W = (rho, v, T) of a conserved state (the BR1 gradient variables)
+template <int DIM>
+__device__ __forceinline__ void br1_vars(const double *U, double gamma, double *W) {
+  const Prim<DIM> q = prim_ideal<DIM, false>(U, gamma);
+  W[0] = q.rho;
+#pragma unroll
+  for (int c = 0; c < DIM; ++c) W[1 + c] = q.v[c];
+  W[1 + DIM] = q.T;
+}
+
+// BR1 surface term of the gradient at face node a0 of a 2-D mortar face f of element e ("Non-conforming
+// faces use the same forward and reverse projections as the hyperbolic side"; reading R23): the hyperbolic
+// mortar with the flux replaced by the central trace.  add[w][c] = (What - W) n_c on the fine side (What = mean of the
+// own W and the coarse trace interpolated to this half), and  sum_m P_rev^m (2 (-What_m n_F)) - W n_c  on the coarse
+// side.  Wc: the own element's W planes in shared memory (plane stride wstride), used for the coarse trace.
+// Rare path, kept out of line.
+template <int NP, bool AFFINE>
+__device__ __noinline__ void br1_mortar_jump_2d(const GradParams &P, long e, int f, int a0, int2 cn, const double *W,
+                                                const double *Wc, int wstride, const double *nv, double *add) {
+  using G = Geo<2, NP>;
+  constexpr int NVAR = 4, NW = 4, NN = NP * NP;
+  const int kind = cn.y & 3, fR = (cn.y >> 2) & 7, sub = (cn.y >> 8) & 1;
+  const double *Pf = P.mortar_mat, *Prv = P.mortar_mat + 2 * NP * NP;
+  if (kind == FK_MORTAR_FINE) {
+    double Wi[NW] = {0.0, 0.0, 0.0, 0.0};
+    for (int j = 0; j < NP; ++j) {
+      const double pw = __ldg(&Pf[(sub * NP + a0) * NP + j]);
+      const double *uc = P.u + (long)cn.x * NVAR * NN + G::face_node(fR, j, 0);
+      double UC[NVAR], WC[NW];
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) UC[v] = __ldg(uc + v * NN);
+      br1_vars<2>(UC, P.gamma, WC);
+#pragma unroll
+      for (int w = 0; w < NW; ++w) Wi[w] += pw * WC[w];
+    }
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+      const double What = 0.5 * (W[w] + Wi[w]);
+#pragma unroll
+      for (int c = 0; c < 2; ++c) add[w * 2 + c] = (What - W[w]) * nv[c];
+    }
+  } else {
+    double GC[NW * 2];
+#pragma unroll
+    for (int k = 0; k < NW * 2; ++k) GC[k] = 0.0;
+    const int lF = fR >> 1;
+    const double sF = (fR & 1) ? 1.0 : -1.0;
+    for (int m = 0; m < 2; ++m) {
+      const long eF = __ldg(&P.mortar_fine[cn.x * 2 + m]);
+      for (int a = 0; a < NP; ++a) {
+        const int pF = G::face_node(fR, a, 0);
+        double UF[NVAR], WF[NW], nF[2];
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) UF[v] = __ldg(P.u + (eF * NVAR + v) * NN + pF);
+        br1_vars<2>(UF, P.gamma, WF);
+#pragma unroll
+        for (int c = 0; c < 2; ++c) nF[c] = sF * metric_at<2, NP, AFFINE>(P.metric, eF, lF * 2 + c, pF);
+        const double pr = __ldg(&Prv[(m * NP + a0) * NP + a]);
+#pragma unroll
+        for (int w = 0; w < NW; ++w) {
+          double Wi = 0.0;
+          for (int j = 0; j < NP; ++j) Wi += __ldg(&Pf[(m * NP + a) * NP + j]) * Wc[w * wstride + G::face_node(f, j, 0)];
+          const double What = 0.5 * (WF[w] + Wi);
+#pragma unroll
+          for (int c = 0; c < 2; ++c) GC[w * 2 + c] += pr * (2.0 * (-(What * nF[c])));
+        }
+      }
+    }
+#pragma unroll
+    for (int w = 0; w < NW; ++w)
+#pragma unroll
+      for (int c = 0; c < 2; ++c) add[w * 2 + c] = GC[w * 2 + c] - W[w] * nv[c];
+  }
+}
+
 // ORIENT3: the instantiation for 3-D meshes with non-trivial face orientation codes (R20); the default one
 // keeps the identity pairing folded at compile time (the decode costs 12 registers here: 64 -> 76, one CTA less per SM)
-// BND: the instantiation for meshes with boundary faces (prescribed states, outflow, walls; reading R22)
+// BND: the instantiation for meshes with boundary faces (prescribed states, outflow, walls; reading R22) or 2-D mortars
+// (reading R23)
 template <int DIM, int NP, bool AFFINE, int EB, bool ORIENT3 = false, bool BND = false>
 __global__ void __launch_bounds__(((EB * Geo<DIM, NP>::NN + 31) / 32) * 32)
 gradient_kernel(const __grid_constant__ GradParams P) {
@@ -188,6 +266,17 @@ gradient_kernel(const __grid_constant__ GradParams P) {
           for (int w = 0; w < NW; ++w) Sg[w * DIM + c] += jump[w] * nc;
         }
         continue;
+      }
+      if constexpr (DIM == 2) {
+        if ((cn.y & 3) != FK_CONFORMING) {          // 2:1 mortar face (reading R23)
+          double nv[DIM], add[NW * DIM];
+#pragma unroll
+          for (int c = 0; c < DIM; ++c) nv[c] = sgn * metric_at<DIM, NP, AFFINE>(P.metric, e, l * DIM + c, p);
+          br1_mortar_jump_2d<NP, AFFINE>(P, e, f, q[1 - l], cn, W, Wsm + el * NN, TILE, nv, add);
+#pragma unroll
+          for (int k = 0; k < NW * DIM; ++k) Sg[k] += add[k] * P.inv_wb;
+          continue;
+        }
       }
     }
     const int fR = (cn.y >> 2) & 7, orient = (DIM == 2 || ORIENT3) ? ((cn.y >> 5) & 7) : 0;
@@ -723,7 +812,7 @@ constexpr int elems_per_block() { return (256 / NN) < 1 ? 1 : 256 / NN; }
 template <int DIM, int NP, bool AFFINE, bool ORIENT3 = false, bool BND = false>
 cudaError_t launch_gradient_t(const GradParams &P, cudaStream_t st) {
   if constexpr (!BND) {
-    // meshes with boundary faces: the general instantiation (orientation decode included)
+    // meshes with boundary or mortar faces: the general instantiation (orientation decode included)
     if (P.boundary) return launch_gradient_t<DIM, NP, AFFINE, (DIM == 3), true>(P, st);
   }
   if constexpr (DIM == 3 && !ORIENT3 && !BND) {

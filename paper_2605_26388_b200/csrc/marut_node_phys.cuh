@@ -6,7 +6,8 @@
 // a separate result plane set (the flux planes stay intact because the viscous face tasks read the own
 // normal flux from them), and the face tasks gather the neighbour's BR1 gradient (NS) or pressure and sound speed
 // (reacting) as well.  Reacting: pressure, frozen sound speed and the chemistry source of every node come from the
-// aux array eos_kernel fills ahead of the stage, so this kernel carries no mechanism table.  Conforming interior faces only.
+// aux array eos_kernel fills ahead of the stage, so this kernel carries no mechanism table.  Interior faces: conforming;
+// Navier-Stokes in 2-D also 2:1 mortars (reading R23).
 //
 // Product code; shares nothing with oracle/.
 #pragma once
@@ -36,6 +37,76 @@ struct PhysCfg {
     return (size_t)(NFP + NRP) * PS + (size_t)NST * TILE + (size_t)NVAR * NTASK + NSRC + (affine ? EB * MDP : 0);
   }
 };
+
+// Viscous numerical flux F_v* (outward, own normal) at face node a0 of a 2-D mortar face f of element e (PAPER.md:223,
+// 234; reading R23): the central flux of eq. 16 on the mortar.  The coarse side's state and its BR1 gradient
+// (stored as stress tensor + heat flux, linear in the gradient) are interpolated to the mortar with P_fwd; fine side:
+// F_v* = (F_v,own + F_v(P U_C, P tau_C).n)/2; coarse side: sum_m P_rev^m (2 (-(F_v(U_F, tau_F) + F_v(P U_C, P tau_C)).n_F / 2)).
+// Fvm: the own viscous normal flux.  Rare path, kept out of line.
+template <int NP>
+__device__ __noinline__ void ns_mortar_viscous_2d(const StageParams &P, long e, int f, int a0, int2 cn, const double *Fvm,
+                                                  const double *nv, double *Fvs) {
+  using G = Geo<2, NP>;
+  constexpr int NVAR = 4, NN = NP * NP, NTAU = Tau<2>::NTAU;
+  const int kind = cn.y & 3, fR = (cn.y >> 2) & 7, sub = (cn.y >> 8) & 1;
+  const double *Pf = P.mortar_mat, *Prv = P.mortar_mat + 2 * NP * NP;
+  if (kind == FK_MORTAR_FINE) {
+    double Ui[NVAR] = {0.0, 0.0, 0.0, 0.0}, ti[NTAU], Fvp[NVAR];
+#pragma unroll
+    for (int k = 0; k < NTAU; ++k) ti[k] = 0.0;
+    for (int j = 0; j < NP; ++j) {
+      const double w = __ldg(&Pf[(sub * NP + a0) * NP + j]);
+      const int pC = G::face_node(fR, j, 0);
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) Ui[v] += w * __ldg(P.u_in + ((long)cn.x * NVAR + v) * NN + pC);
+#pragma unroll
+      for (int k = 0; k < NTAU; ++k) ti[k] += w * __ldg(P.S + ((long)cn.x * NTAU + k) * NN + pC);
+    }
+    const Prim<2> qi = prim_ideal<2, false>(Ui, P.gamma);
+    viscous_flux_dot_tau<2>(qi.v, ti, nv, Fvp);
+    Fvs[0] = 0.0;
+#pragma unroll
+    for (int v = 1; v < NVAR; ++v) Fvs[v] = 0.5 * (Fvm[v] + Fvp[v]);
+  } else {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Fvs[v] = 0.0;
+    const int lF = fR >> 1;
+    const double sF = (fR & 1) ? 1.0 : -1.0;
+    const bool aff = P.affine_flag != 0;
+    for (int m = 0; m < 2; ++m) {
+      const long eF = __ldg(&P.mortar_fine[cn.x * 2 + m]);
+      for (int a = 0; a < NP; ++a) {
+        const int pF = G::face_node(fR, a, 0);
+        double UF[NVAR], tF[NTAU], Ui[NVAR] = {0.0, 0.0, 0.0, 0.0}, ti[NTAU], nF[2], FvF[NVAR], FvC[NVAR];
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) UF[v] = __ldg(P.u_in + (eF * NVAR + v) * NN + pF);
+#pragma unroll
+        for (int k = 0; k < NTAU; ++k) {
+          tF[k] = __ldg(P.S + (eF * NTAU + k) * NN + pF);
+          ti[k] = 0.0;
+        }
+        for (int j = 0; j < NP; ++j) {
+          const double w = __ldg(&Pf[(m * NP + a) * NP + j]);
+          const int pC = G::face_node(f, j, 0);
+#pragma unroll
+          for (int v = 0; v < NVAR; ++v) Ui[v] += w * __ldg(P.u_in + (e * NVAR + v) * NN + pC);
+#pragma unroll
+          for (int k = 0; k < NTAU; ++k) ti[k] += w * __ldg(P.S + (e * NTAU + k) * NN + pC);
+        }
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+          nF[c] = sF * (aff ? __ldg(&P.metric[eF * 5 + lF * 2 + c]) : __ldg(&P.metric[(eF * 5 + lF * 2 + c) * NN + pF]));
+        const Prim<2> qF = prim_ideal<2, false>(UF, P.gamma);
+        const Prim<2> qi = prim_ideal<2, false>(Ui, P.gamma);
+        viscous_flux_dot_tau<2>(qF.v, tF, nF, FvF);
+        viscous_flux_dot_tau<2>(qi.v, ti, nF, FvC);
+        const double w2 = -2.0 * __ldg(&Prv[(m * NP + a0) * NP + a]);
+#pragma unroll
+        for (int v = 1; v < NVAR; ++v) Fvs[v] += w2 * (0.5 * (FvF[v] + FvC[v]));
+      }
+    }
+  }
+}
 
 // BND (Navier-Stokes): the instantiation for meshes with boundary faces -- prescribed states, outflow, slip walls and the
 // no-slip adiabatic / isothermal walls of PAPER.md:223 (readings R18, R22); the default one carries no code
@@ -210,7 +281,12 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       }
       nrm = sqrt(n2);
     }
+    const bool mort = BND && DIM == 2 && PHYS == PH_NS && (cn.y & 3) >= FK_MORTAR_FINE;   // 2-D 2:1 mortar face (reading R23)
     if constexpr (BND) {
+      if (mort) {
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Up[v] = Um[v];       // (placeholder: the mortar flux replaces the lift below)
+      }
       if (bnd) {
         // exterior state of the hyperbolic surface flux (R8, R18, R22): prescribed state; outflow: the interior
         // state; slip wall and the two no-slip walls: the interior state with the normal momentum reflected
@@ -259,7 +335,25 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       // viscous part: F_v* = mean of the two sides; own F_v.n = F_inv(U-).n - (own total normal flux in the plane)
       const int qk = (DIM == 3) ? t.p / (NP * NP) : 0;
       const int sp = t.p + (KS - NP * NP) * qk;
-      if (bnd) {
+      if constexpr (BND && DIM == 2) {
+        if (mort) {
+          double Fvm[NVAR], Fvs[NVAR];
+          Fvm[0] = 0.0;
+#pragma unroll
+          for (int v = 1; v < NVAR; ++v) Fvm[v] = Fm[v] - sgn * Fsm[((l * NVAR + v) * EB + t.el) * PS + sp];
+          if constexpr (!VONLY) {
+            double Fs[NVAR];
+            node_mortar_flux_2d<NP>(P, ee, t.f, t.a0, cn, Um, nv, Fs);
+#pragma unroll
+            for (int v = 0; v < NVAR; ++v) lift[v] = Fs[v] - Fm[v];
+          }
+          ns_mortar_viscous_2d<NP>(P, ee, t.f, t.a0, cn, Fvm, nv, Fvs);
+#pragma unroll
+          for (int v = 1; v < NVAR; ++v) lift[v] -= Fvs[v] - Fvm[v];
+        }
+      }
+      if (mort) {
+      } else if (bnd) {
         // viscous wall flux F_v*(U_w, S-) (reading R22): momentum rows = the wall shear stress, as the element's own;
         // energy row: no stress work (v_w = 0), the heat flux k grad T . n at an isothermal wall, nothing at an
         // adiabatic one.  Prescribed / outflow / slip faces: F_v* = F_v(U-, S-), no viscous surface term.
