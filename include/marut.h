@@ -270,9 +270,11 @@ long marut_launch_count(const marut_mesh *mesh);
 marut_status marut_debug_stage_kernel(marut_mesh *mesh, int which);
 
 /* the kernels' branch-free 1/x and sqrt(x) for positive normal-range operands (csrc/marut_common.cuh) evaluated on n
- * DEVICE doubles x -> rcp, sq (DEVICE, n doubles each); the tests compare them bit for bit with IEEE division and
- * square root.  Asynchronous on the stream. */
-marut_status marut_debug_rcp_sqrt(const double *x, double *rcp, double *sq, long n, void *cuda_stream);
+ * DEVICE doubles x -> rcp, sq (DEVICE, n doubles each).  variant 0: rcp_pos / sqrt_pos (the CFL reduction's: equal to
+ * IEEE division and square root bit for bit, the tests check it); variant 1: rcp_pos_2ulp / sqrt_pos_2ulp (the line
+ * kernel's: the same sequences without the final correction step, at most 2 ulp from the exact value).  Asynchronous on
+ * the stream.  EINVAL for another variant. */
+marut_status marut_debug_rcp_sqrt(const double *x, double *rcp, double *sq, long n, int variant, void *cuda_stream);
 
 const char *marut_last_error(void);
 

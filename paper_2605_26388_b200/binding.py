@@ -107,7 +107,7 @@ def lib():
         L.marut_debug_stage_kernel.restype = C.c_int
         L.marut_debug_stage_kernel.argtypes = [vp, C.c_int]
         L.marut_debug_rcp_sqrt.restype = C.c_int
-        L.marut_debug_rcp_sqrt.argtypes = [vp, vp, vp, C.c_long, vp]
+        L.marut_debug_rcp_sqrt.argtypes = [vp, vp, vp, C.c_long, C.c_int, vp]
         L.marut_last_error.restype = C.c_char_p
         _lib = L
     return _lib
@@ -270,8 +270,8 @@ def marut_set_blend(h, alpha):
     _check(lib().marut_set_blend(h, None if alpha is None else _dev(alpha)))
 
 
-def marut_debug_rcp_sqrt(x, rcp, sq, stream=None):
-    _check(lib().marut_debug_rcp_sqrt(_dev(x), _dev(rcp), _dev(sq), x.numel(), _stream(stream)))
+def marut_debug_rcp_sqrt(x, rcp, sq, variant=0, stream=None):
+    _check(lib().marut_debug_rcp_sqrt(_dev(x), _dev(rcp), _dev(sq), x.numel(), int(variant), _stream(stream)))
 
 
 def marut_set_explicit_source(h, on):

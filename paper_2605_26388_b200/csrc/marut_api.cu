@@ -40,6 +40,7 @@ struct marut_mesh {
   int n_bc = 0;
   bool oriented = false;       // some 3-D interface has a non-trivial orientation code (R20)
   bool bc_kinds = false;       // some boundary id is an outflow / slip-wall face
+  int pencil_reverse = 0;      // tile direction of the next launch of the persistent line kernel (alternates)
   double gamma = 1.4, mu = 0.0, Pr = 0.72, kappa = 0.0;
   bool affine = false;
   double dx_min = 0.0;
@@ -564,7 +565,12 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
         e = cudaErrorNotSupported;
         if (m->affine && !P.bc_kinds && m->stage_kernel_pref != 1) {
           if (fuse && fuse->dt_next) { P.red_next = m->d_red_next; P.dt_next = fuse->dt_next; P.cfl = fuse->cfl; }
+          // consecutive launches walk the tiles in opposite directions (the start of one finds the end of the previous
+          // one in L2); the result does not depend on the direction
+          P.zero = 0;
+          P.reverse = m->pencil_reverse;
           e = launch_stage_pencil(m->dim, m->np, m->n_mortar > 0, m->stage_kernel_pref == 2, P, st);
+          if (e == cudaSuccess) m->pencil_reverse ^= 1;
           if (fuse) fuse->done = (e == cudaSuccess) && P.red_next != nullptr;
           P.red_next = nullptr;
         }
@@ -1126,16 +1132,19 @@ extern "C" marut_status marut_debug_stage_kernel(marut_mesh *m, int which) {
   m->stage_kernel_pref = which;
   return MARUT_OK;
 }
+template <bool FAST>
 __global__ void debug_rcp_sqrt_kernel(const double *__restrict__ x, double *__restrict__ r, double *__restrict__ s, long n) {
   for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
-    r[i] = rcp_pos(x[i]);
-    s[i] = sqrt_pos(x[i]);
+    r[i] = FAST ? rcp_pos_2ulp(x[i]) : rcp_pos(x[i]);
+    s[i] = FAST ? sqrt_pos_2ulp(x[i]) : sqrt_pos(x[i]);
   }
 }
-extern "C" marut_status marut_debug_rcp_sqrt(const double *x, double *rcp, double *sq, long n, void *stream) {
-  if (!x || !rcp || !sq || n < 0) return fail(MARUT_EINVAL, "bad argument");
+extern "C" marut_status marut_debug_rcp_sqrt(const double *x, double *rcp, double *sq, long n, int variant, void *stream) {
+  if (!x || !rcp || !sq || n < 0 || variant < 0 || variant > 1) return fail(MARUT_EINVAL, "bad argument");
   if (n == 0) return MARUT_OK;
-  debug_rcp_sqrt_kernel<<<(unsigned)std::min<long>((n + 255) / 256, 148L * 8), 256, 0, (cudaStream_t)stream>>>(x, rcp, sq, n);
+  const unsigned grid = (unsigned)std::min<long>((n + 255) / 256, 148L * 8);
+  if (variant) debug_rcp_sqrt_kernel<true><<<grid, 256, 0, (cudaStream_t)stream>>>(x, rcp, sq, n);
+  else debug_rcp_sqrt_kernel<false><<<grid, 256, 0, (cudaStream_t)stream>>>(x, rcp, sq, n);
   CUDA_TRY(cudaGetLastError());
   return MARUT_OK;
 }

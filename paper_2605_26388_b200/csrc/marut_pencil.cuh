@@ -120,7 +120,7 @@ template <int DIM>
 __device__ __forceinline__ PencilFace pencil_face(const double *Up, const double *Ja, double nrm, double gamma, double vnm,
                                                   double pm, double rinvm) {
   PencilFace F;
-  const double rinvp = rcp_pos(Up[0]);
+  const double rinvp = rcp_pos_2ulp(Up[0]);
   double mnp = 0.0, kep = 0.0;
 #pragma unroll
   for (int c = 0; c < DIM; ++c) {
@@ -130,7 +130,7 @@ __device__ __forceinline__ PencilFace pencil_face(const double *Up, const double
   F.mnp = mnp;
   F.pp = (gamma - 1.0) * (Up[DIM + 1] - 0.5 * kep * rinvp);
   F.vnp = mnp * rinvp;
-  const double ap = sqrt_pos(gamma * F.pp * rinvp), am = sqrt_pos(gamma * pm * rinvm);
+  const double ap = sqrt_pos_2ulp(gamma * F.pp * rinvp), am = sqrt_pos_2ulp(gamma * pm * rinvm);
   F.hl = 0.5 * fmax(fabs(vnm) + am * nrm, fabs(F.vnp) + ap * nrm);
   return F;
 }
@@ -153,6 +153,10 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
   using C = PencilCfg<DIM, NP>;
   constexpr int NVAR = C::NVAR, NN = C::NN, NL = C::NL, ED = C::ED, MD = Geo<DIM, NP>::MD;
   constexpr bool FIRST = (L == 0), LAST = (L == DIM - 1);
+  // 3-D: the u_n term of eq. 45 enters the partial residual in the MIDDLE phase, R += g u_n with g = -ca J / cc, so that
+  // the last phase's  cb U + cc (0 - R / J)  already contains ca u_n: the loads run one variable ahead of their use in a
+  // phase that has the registers for it (in the last phase they stall the combination: 13 % of its issue slots)
+  constexpr bool FOLD3 = (DIM == 3), FOLD_HERE = FOLD3 && (L == 1);
   constexpr int SM = (L == 0) ? 1 : ((L == 1) ? NP : NP * NP);
   if (t >= nel * NL) return;
   const int el = t / NL, r = t - el * NL;
@@ -174,7 +178,8 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
       for (int m = 0; m < NP; ++m) U[v][m] = ul[v * NN + m * SM];
     }
   }
-  const bool use_un = LAST && (P.ca != 0.0);
+  const bool use_un = LAST && !FOLD3 && (P.ca != 0.0);
+  const bool fold_un = FOLD_HERE && (P.ca != 0.0);
   const long gofs = e * ED + p0;
   const double *met = Md + C::NCN + el * MD;
   double Ja[DIM];
@@ -182,11 +187,19 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
   for (int c = 0; c < DIM; ++c) Ja[c] = met[L * DIM + c];
   const double nrm = Md[C::NCN + C::NMT + el * DIM + L];
   double invJ = 0.0;
-  if constexpr (LAST) invJ = met[DIM * DIM];
+  if constexpr (LAST || FOLD_HERE) invJ = met[DIM * DIM];
+  double g = 0.0, unb[2][NP];      // u_n of variable v in unb[v & 1]: loaded while variable v - 1 is worked on
+  if constexpr (FOLD_HERE) {
+    if (fold_un) {
+      g = (0.0 - P.ca) / (cc * invJ);
+#pragma unroll
+      for (int m = 0; m < NP; ++m) unb[0][m] = __ldcs(P.u_n + gofs + m * SM);
+    }
+  }
   double rinv[NP], pr[NP], vn[NP];
 #pragma unroll
   for (int m = 0; m < NP; ++m) {
-    rinv[m] = rcp_pos(U[0][m]);
+    rinv[m] = rcp_pos_2ulp(U[0][m]);
     double mn = 0.0, ke = 0.0;
 #pragma unroll
     for (int c = 0; c < DIM; ++c) {
@@ -204,7 +217,13 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
     if constexpr (LAST) {
       if (use_un) {
 #pragma unroll
-        for (int m = 1; m < NP - 1; ++m) un[m] = P.u_n[gofs + v * NN + m * SM];
+        for (int m = 1; m < NP - 1; ++m) un[m] = __ldcs(P.u_n + gofs + v * NN + m * SM);
+      }
+    }
+    if constexpr (FOLD_HERE) {
+      if (fold_un && v + 1 < NVAR) {
+#pragma unroll
+        for (int m = 0; m < NP; ++m) unb[(v + 1) & 1][m] = __ldcs(P.u_n + gofs + (v + 1) * NN + m * SM);
       }
     }
     double f[NP], acc[NP];
@@ -222,6 +241,12 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
       for (int i = 0; i < NP; ++i) acc[i] = rl[v * NN + i * SM];
     }
     line_deriv<NP>(P, f, acc);
+    if constexpr (FOLD_HERE) {
+      if (fold_un) {
+#pragma unroll
+        for (int i = 0; i < NP; ++i) acc[i] = fma(g, unb[v & 1][i], acc[i]);
+      }
+    }
     accE[v][0] = acc[0];
     accE[v][1] = acc[NP - 1];
     if constexpr (!LAST) {
@@ -242,12 +267,23 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
     if (use_un) {
 #pragma unroll
       for (int v = 0; v < NVAR; ++v) {
-        unE[v][0] = P.u_n[gofs + v * NN];
-        unE[v][1] = P.u_n[gofs + v * NN + (NP - 1) * SM];
+        unE[v][0] = __ldcs(P.u_n + gofs + v * NN);
+        unE[v][1] = __ldcs(P.u_n + gofs + v * NN + (NP - 1) * SM);
       }
     }
   }
   const int k0 = c0.y & 3, k1 = c1.y & 3;
+  {
+    // Keep every consumer of the gathered traces below the volume loop: ptxas otherwise schedules the reciprocal of the
+    // neighbour's density right behind its load and the warp sits out the gather's latency there (9 % of the samples).
+    // The exclusive-or with a zero that is only known at run time and depends on the loop's last result ties them down.
+    const int late = __double2loint(accE[NVAR - 1][1]) & P.zero;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) {
+      Up0[v] = __hiloint2double(__double2hiint(Up0[v]), __double2loint(Up0[v]) ^ late);
+      Up1[v] = __hiloint2double(__double2hiint(Up1[v]), __double2loint(Up1[v]) ^ late);
+    }
+  }
   const PencilFace F0 = pencil_face<DIM>(Up0, Ja, nrm, P.gamma, vn[0], pr[0], rinv[0]);
   const PencilFace F1 = pencil_face<DIM>(Up1, Ja, nrm, P.gamma, vn[NP - 1], pr[NP - 1], rinv[NP - 1]);
   double Fs0[NVAR], Fs1[NVAR];   // mortar faces only: F* (outward) from the mortar routine
@@ -332,16 +368,21 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
     wl = (int)((nel * ED + shift + 1) & ~1L);
     return ws + wl <= total;
   };
-  auto issue = [&](long tile, int buf) {
+  // P.reverse: the tiles are walked from the last to the first.  Consecutive stage launches alternate the direction, so
+  // that a launch starts on the part of its input that the previous launch wrote or read last (still in L2).
+  auto phys = [&](long k) -> long { return P.reverse ? ntile - 1 - k : k; };
+  auto issue = [&](long k, int buf) {
+    const long tile = phys(k);
     long ws;
     int wl, shift;
-    if (tile < ntile && window(tile, ws, wl, shift)) {
+    if (k < ntile && window(tile, ws, wl, shift)) {
       mbar_expect_tx(&bars[buf], (uint32_t)wl * 8u);
       bulk_load(Ub + buf * UB, P.u_in + ws, (uint32_t)wl * 8u, &bars[buf]);
     }
   };
-  auto fetch_meta = [&](long tile, int buf) {
-    if (tile >= ntile) return;
+  auto fetch_meta = [&](long k, int buf) {
+    if (k >= ntile) return;
+    const long tile = phys(k);
     const long e0 = tile * ET;
     const int nel = (int)((P.ne - e0 < ET) ? (P.ne - e0) : ET);
     double *dst = Mds + buf * MW;
@@ -365,7 +406,8 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
   double lam = 0.0;
   int bad = 0;
   int it = 0;
-  for (long tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+  for (long k = blockIdx.x; k < ntile; k += gridDim.x, ++it) {
+    const long tile = phys(k);
     const int buf = it & 1;
     const long e0 = tile * ET;
     const int nel = (int)((P.ne - e0 < ET) ? (P.ne - e0) : ET);
@@ -374,7 +416,7 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
     const bool by_tma = window(tile, ws, wl, shift);
     const double *Ut = Ub + buf * UB + shift;
     const double *Md = Mds + buf * MW;
-    fetch_meta(tile + gridDim.x, buf ^ 1);
+    fetch_meta(k + gridDim.x, buf ^ 1);
     if (by_tma) {
       mbar_wait(&bars[buf], (uint32_t)((it >> 1) & 1));
     } else {
@@ -382,10 +424,12 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
       for (int i = tid; i < nel * ED; i += NT) dst[i] = __ldg(P.u_in + e0 * ED + i);
       __syncthreads();
     }
+    // u_n of this tile is read one phase (3-D: by the middle phase) or two phases (2-D) later: bring it into L2 now
+    // (earlier, and part of it is evicted again)
+    if (DIM == 3 && tid == 0 && use_un && by_tma) bulk_prefetch_l2(P.u_n + ws, (uint32_t)wl * 8u);
     pencil_phase<DIM, NP, 0, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
     __syncthreads();
-    // u_n of this tile is read by the last phase: bring it into L2 now (earlier, and part of it is evicted again)
-    if (tid == 0 && use_un && by_tma) bulk_prefetch_l2(P.u_n + ws, (uint32_t)wl * 8u);
+    if (DIM == 2 && tid == 0 && use_un && by_tma) bulk_prefetch_l2(P.u_n + ws, (uint32_t)wl * 8u);
     if constexpr (DIM == 3) {
       pencil_phase<DIM, NP, 1, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
       __syncthreads();
@@ -393,7 +437,7 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
     pencil_phase<DIM, NP, DIM - 1, MORTAR, FUSE>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
     cp_async_wait_all();
     __syncthreads();
-    if (tid == 0) issue(tile + 2L * gridDim.x, buf);
+    if (tid == 0) issue(k + 2L * gridDim.x, buf);
   }
   if constexpr (FUSE) cfl_reduce_and_finalize(P, lam, bad, tid);
 }

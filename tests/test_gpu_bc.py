@@ -70,12 +70,11 @@ def test_boundary_kinds_are_validated():
     gm.close()
     ns = wl.make_case("c4", cells=16)
     ns.mesh.physics, ns.mesh.mu = wl.NAVIER_STOKES, 0.01
-    try:
-        gn = mb.MarutMesh(ns.mesh)
-    except mb.MarutError:
-        return                                  # BR1 across mortars is not built: nothing to validate
+    gn = mb.MarutMesh(ns.mesh)                  # Navier-Stokes on the mortar mesh (reading R23): kinds 0..4 (R22)
     with pytest.raises(mb.MarutError):
-        gn.set_boundary_kinds((1, 2))
+        gn.set_boundary_kinds((5, 0))
+    gn.set_boundary_kinds((1, 2))
+    gn.set_boundary_kinds((3, 4))
     gn.set_boundary_kinds((0, 0))
     gn.close()
 
