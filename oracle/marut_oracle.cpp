@@ -811,7 +811,7 @@ static void rhs_inviscid(const Mesh &m, const double *u, double *du) {
 }
 
 // ---------------------------------------------------------------------------
-// O9. BR1 viscous residual; conforming interfaces, boundary faces (O9b), 2-D mortars (O9c).
+// O9. BR1 viscous residual; conforming interfaces, boundary faces (O9b), 2-D mortars (O9c), 3-D mortars (O9d).
 // W = (rho, u_1..u_d, T), T = p/rho.  S[e][node][w][c] = d W_w / d x_c.
 // ---------------------------------------------------------------------------
 static void prim_gradient_vars(const Mesh &m, const double *U, double *W) {
@@ -921,6 +921,43 @@ static void br1_gradient(const Mesh &m, const double *u, std::vector<double> &S)
       }
     }
     for (int i = 0; i < n; ++i) {
+      const int pC = face_node(m, fC, i);
+      double nC[3]; face_normal(m, eC, fC, pC, nC);
+      for (int w = 0; w < nw; ++w)
+        for (int c = 0; c < d; ++c)
+          S[(((size_t)eC * nn + pC) * nw + w) * d + c] += (GC[((size_t)i * nw + w) * d + c] - WC[(size_t)i * nw + w] * nC[c]) / wb;
+    }
+  }
+  // O9d. 4:1 mortars, 3-D (same passage; readings R21 + R23): the tensor product of O9c -- the coarse trace of W goes
+  // to each of the four sub-faces with Pf[s0] x Pf[s1], the coarse side lifts the projection Pr[s0] x Pr[s1] of the
+  // mortars' outward What n with the area factor 4.
+  for (size_t q = 0; d == 3 && q < m.mortar.size() / 8; ++q) {
+    const int *M = &m.mortar[q * 8];
+    const long eC = M[0]; const int fC = M[1], fF = M[6];
+    std::vector<double> WC((size_t)nf * nw), GC((size_t)nf * nw * d, 0.0);
+    for (int j = 0; j < nf; ++j) { double U[MAXV]; gather(m, u, eC, face_node(m, fC, j), U); prim_gradient_vars(m, U, &WC[(size_t)j * nw]); }
+    for (int s = 0; s < 4; ++s) {
+      const int s0 = s % 2, s1 = s / 2;
+      const long eF = M[2 + s];
+      for (int a = 0; a < nf; ++a) {
+        const int a0 = a % n, a1 = a / n, pF = face_node(m, fF, a);
+        double UF[MAXV], WF[MAXV], nF[3];
+        gather(m, u, eF, pF, UF); prim_gradient_vars(m, UF, WF); face_normal(m, eF, fF, pF, nF);
+        for (int w = 0; w < nw; ++w) {
+          double Wt = 0.0;
+          for (int j1 = 0; j1 < n; ++j1)
+            for (int j0 = 0; j0 < n; ++j0) Wt += m.Pf[s0][a0 * n + j0] * m.Pf[s1][a1 * n + j1] * WC[(size_t)(j0 + n * j1) * nw + w];
+          const double What = 0.5 * (WF[w] + Wt);
+          for (int c = 0; c < d; ++c) {
+            S[(((size_t)eF * nn + pF) * nw + w) * d + c] += (What - WF[w]) * nF[c] / wb;
+            for (int i1 = 0; i1 < n; ++i1)
+              for (int i0 = 0; i0 < n; ++i0)
+                GC[((size_t)(i0 + n * i1) * nw + w) * d + c] += m.Pr_[s0][i0 * n + a0] * m.Pr_[s1][i1 * n + a1] * (4.0 * (-(What * nF[c])));
+          }
+        }
+      }
+    }
+    for (int i = 0; i < nf; ++i) {
       const int pC = face_node(m, fC, i);
       double nC[3]; face_normal(m, eC, fC, pC, nC);
       for (int w = 0; w < nw; ++w)
@@ -1040,6 +1077,54 @@ static void rhs_viscous_add(const Mesh &m, const double *u, double *du) {
       }
     }
     for (int i = 0; i < n; ++i) {
+      const int pC = face_node(m, fC, i);
+      double nC[3], Fo[MAXV];
+      face_normal(m, eC, fC, pC, nC);
+      viscous_flux_dot(m, &UC[(size_t)i * nvar], &SC[(size_t)i * ng], nC, Fo);
+      const double JC = m.J[(size_t)eC * nn + pC];
+      for (int v = 0; v < nvar; ++v) du[((size_t)eC * nvar + v) * nn + pC] += (FC[(size_t)i * nvar + v] - Fo[v]) / (JC * wb);
+    }
+  }
+  // O9d. 4:1 mortars, 3-D: the tensor product of O9c (state and gradient of the coarse side to the four sub-faces with
+  // Pf[s0] x Pf[s1]; the coarse side lifts Pr[s0] x Pr[s1] of the mortars' outward central flux with the area factor 4).
+  for (size_t q = 0; d == 3 && q < m.mortar.size() / 8; ++q) {
+    const int *M = &m.mortar[q * 8];
+    const long eC = M[0]; const int fC = M[1], fF = M[6];
+    const int ng = nw * d;
+    std::vector<double> UC((size_t)nf * nvar), SC((size_t)nf * ng), FC((size_t)nf * nvar, 0.0);
+    for (int j = 0; j < nf; ++j) {
+      const int pC = face_node(m, fC, j);
+      gather(m, u, eC, pC, &UC[(size_t)j * nvar]);
+      for (int k = 0; k < ng; ++k) SC[(size_t)j * ng + k] = S[((size_t)eC * nn + pC) * ng + k];
+    }
+    for (int s = 0; s < 4; ++s) {
+      const int s0 = s % 2, s1 = s / 2;
+      const long eF = M[2 + s];
+      for (int a = 0; a < nf; ++a) {
+        const int a0 = a % n, a1 = a / n, pF = face_node(m, fF, a);
+        double UF[MAXV], Ut[MAXV], St[MAXV * 3], nF[3], FvF[MAXV], FvC[MAXV];
+        gather(m, u, eF, pF, UF); face_normal(m, eF, fF, pF, nF);
+        for (int v = 0; v < nvar; ++v) Ut[v] = 0.0;
+        for (int k = 0; k < ng; ++k) St[k] = 0.0;
+        for (int j1 = 0; j1 < n; ++j1)
+          for (int j0 = 0; j0 < n; ++j0) {
+            const double pw = m.Pf[s0][a0 * n + j0] * m.Pf[s1][a1 * n + j1];
+            for (int v = 0; v < nvar; ++v) Ut[v] += pw * UC[(size_t)(j0 + n * j1) * nvar + v];
+            for (int k = 0; k < ng; ++k) St[k] += pw * SC[(size_t)(j0 + n * j1) * ng + k];
+          }
+        viscous_flux_dot(m, UF, &S[((size_t)eF * nn + pF) * ng], nF, FvF);
+        viscous_flux_dot(m, Ut, St, nF, FvC);
+        const double JF = m.J[(size_t)eF * nn + pF];
+        for (int v = 0; v < nvar; ++v) {
+          const double Fc = 0.5 * (FvF[v] + FvC[v]);
+          du[((size_t)eF * nvar + v) * nn + pF] += (Fc - FvF[v]) / (JF * wb);
+          for (int i1 = 0; i1 < n; ++i1)
+            for (int i0 = 0; i0 < n; ++i0)
+              FC[(size_t)(i0 + n * i1) * nvar + v] += m.Pr_[s0][i0 * n + a0] * m.Pr_[s1][i1 * n + a1] * (4.0 * (-Fc));
+        }
+      }
+    }
+    for (int i = 0; i < nf; ++i) {
       const int pC = face_node(m, fC, i);
       double nC[3], Fo[MAXV];
       face_normal(m, eC, fC, pC, nC);

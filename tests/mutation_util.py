@@ -52,6 +52,22 @@ MUTATIONS = {
         "m.Pr_[s][i * n + a] * (2.0 * (-Fs));",
         "m.Pr_[s][i * n + a] * (1.0 * (-Fs));",
         "viscous flux across a 2-D mortar: the coarse side's projected flux misses the 2:1 area factor"),
+    "br1_mortar3d_wrong_subface": (
+        "Wt += m.Pf[s0][a0 * n + j0] * m.Pf[s1][a1 * n + j1] * WC[(size_t)(j0 + n * j1) * nw + w];",
+        "Wt += m.Pf[1 - s0][a0 * n + j0] * m.Pf[s1][a1 * n + j1] * WC[(size_t)(j0 + n * j1) * nw + w];",
+        "BR1 gradient across a 3-D mortar: the coarse trace of W goes to the wrong sub-face in the first face direction"),
+    "br1_mortar3d_area_factor_2": (
+        "(4.0 * (-(What * nF[c])));",
+        "(2.0 * (-(What * nF[c])));",
+        "BR1 gradient across a 3-D mortar: the 2-D area factor"),
+    "viscous_mortar3d_wrong_subface": (
+        "const double pw = m.Pf[s0][a0 * n + j0] * m.Pf[s1][a1 * n + j1];",
+        "const double pw = m.Pf[s0][a0 * n + j0] * m.Pf[1 - s1][a1 * n + j1];",
+        "viscous flux across a 3-D mortar: coarse state and gradient go to the wrong sub-face in the second face direction"),
+    "viscous_mortar3d_area_factor_2": (
+        "(4.0 * (-Fc));",
+        "(2.0 * (-Fc));",
+        "viscous flux across a 3-D mortar: the 2-D area factor"),
 }
 
 _cache = {}
