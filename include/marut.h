@@ -73,8 +73,8 @@ typedef struct {
                              EULER and NAVIER_STOKES (BR1 across the mortar: PAPER.md:223, R23).
                              3-D: [n_mortar][8] = eC,fC,eF_00,eF_10,eF_01,eF_11,fF,orient : 4:1 hanging faces (DESIGN.md
                              R21); eF_{s0 s1} covers half s0 / s1 of the coarse face's first / second face-local direction
-                             (the remaining reference directions in increasing order); orient must be 0; EULER, affine
-                             meshes only (else EINVAL) */
+                             (the remaining reference directions in increasing order); orient must be 0; EULER and
+                             NAVIER_STOKES (BR1 across the mortar: DESIGN.md R23), affine meshes only (else EINVAL) */
   long n_bface;
   const int *bface;       /* [n_bface][3]  = e,f,bc_id : boundary faces with a prescribed exterior state */
   int n_bc;

@@ -55,6 +55,7 @@ struct marut_mesh {
   int *d_mortar_info = nullptr;   // 3-D: [m][3] = eC, fC, fF
   double *d_mflux = nullptr;      // 3-D: F* at the fine face nodes of every mortar, [m][4][n*n][nvar]
   double *d_mortar_mat = nullptr;
+  double *d_mW = nullptr;       // Navier-Stokes, 3-D mortars: central BR1 traces at the fine face nodes (mortar_trace3d_kernel)
   double *d_bc = nullptr;
   double *d_S = nullptr;     // NS scratch: stress tensor + heat flux from the BR1 gradient, [e][d(d+1)/2 + d][node]
   double *d_T = nullptr;     // reacting scratch of eos_kernel: [e][2 + n_species][node] = p, a, omega_s
@@ -240,7 +241,7 @@ static cudaError_t run_compact(int np, const double *d_full, double *d_el, long 
 extern "C" void marut_mesh_destroy(marut_mesh *m) {
   if (!m) return;
   cudaDeviceSynchronize();
-  cudaFree(m->d_metric); cudaFree(m->d_fnorm); cudaFree(m->d_conn); cudaFree(m->d_mortar_fine); cudaFree(m->d_mortar_info); cudaFree(m->d_mflux); cudaFree(m->d_mortar_mat);
+  cudaFree(m->d_metric); cudaFree(m->d_fnorm); cudaFree(m->d_conn); cudaFree(m->d_mortar_fine); cudaFree(m->d_mortar_info); cudaFree(m->d_mflux); cudaFree(m->d_mW); cudaFree(m->d_mortar_mat);
   cudaFree(m->d_Vinv); cudaFree(m->d_araw); cudaFree(m->d_subn); cudaFree(m->d_bc); cudaFree(m->d_S); cudaFree(m->d_T); cudaFree(m->d_mech); cudaFree(m->d_red);
   cudaFree(m->d_red_next);
   if (m->h_red) cudaFreeHost(m->h_red);
@@ -258,8 +259,6 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   if (d->physics < 0 || d->physics > 2) return fail(MARUT_EINVAL, "unknown physics %d", d->physics);
   if (d->physics == MARUT_REACTING_EULER && (d->n_mortar || d->n_bface))
     return fail(MARUT_EINVAL, "REACTING_EULER supports conforming interior faces only");
-  if (d->physics == MARUT_NAVIER_STOKES && d->n_mortar && d->dim == 3)
-    return fail(MARUT_EINVAL, "NAVIER_STOKES: mortar faces are implemented in 2-D only");
   if (d->physics != MARUT_REACTING_EULER && !(d->gamma > 1.0)) return fail(MARUT_EINVAL, "gamma must be > 1");
   if (d->physics == MARUT_NAVIER_STOKES && (!(d->mu >= 0.0) || !(d->Pr > 0.0))) return fail(MARUT_EINVAL, "need mu >= 0, Pr > 0");
 
@@ -354,8 +353,8 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   }
   // mortar rows: 2-D [6] = eC,fC,eF_lo,eF_up,fF,orient; 3-D [8] = eC,fC,eF_00,eF_10,eF_01,eF_11,fF,orient (R21)
   const int nfine = (dim == 2) ? 2 : 4, mstride = nfine + 4;
-  if (dim == 3 && d->n_mortar > 0 && m->physics != MARUT_EULER)
-    return fail(MARUT_EINVAL, "3-D mortar faces are implemented for MARUT_EULER only");
+  if (dim == 3 && d->n_mortar > 0 && m->physics == MARUT_REACTING_EULER)
+    return fail(MARUT_EINVAL, "3-D mortar faces are implemented for MARUT_EULER and MARUT_NAVIER_STOKES");
   std::vector<int> mfine((size_t)std::max<long>(1, d->n_mortar) * nfine, 0), minfo((size_t)std::max<long>(1, d->n_mortar) * 3, 0);
   for (long i = 0; i < d->n_mortar; ++i) {
     const int *M = d->mortar + i * mstride;
@@ -395,6 +394,7 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
     CUDA_TRY(cudaMalloc(&m->d_mortar_info, minfo.size() * sizeof(int)));
     CUDA_TRY(cudaMemcpy(m->d_mortar_info, minfo.data(), minfo.size() * sizeof(int), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMalloc(&m->d_mflux, (size_t)d->n_mortar * 4 * np * np * m->nvar * sizeof(double)));
+    if (m->physics == MARUT_NAVIER_STOKES) CUDA_TRY(cudaMalloc(&m->d_mW, (size_t)d->n_mortar * 4 * np * np * m->nvar * sizeof(double)));
   }
   CUDA_TRY(cudaMalloc(&m->d_mortar_mat, mort.size() * sizeof(double)));
   CUDA_TRY(cudaMemcpy(m->d_mortar_mat, mort.data(), mort.size() * sizeof(double), cudaMemcpyHostToDevice));
@@ -515,7 +515,13 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
     G.u = u_in; G.S = m->d_S; G.metric = m->d_metric; G.conn = m->d_conn;
     G.gamma = m->gamma; G.inv_wb = 1.0 / m->w[0]; G.mu = m->mu; G.kappa = m->kappa; G.ne = m->ne; G.oriented = m->oriented ? 1 : 0;
     G.bc_state = m->d_bc; G.boundary = (m->n_bface > 0 || m->n_mortar > 0) ? 1 : 0;
-    G.mortar_fine = m->d_mortar_fine; G.mortar_mat = m->d_mortar_mat;
+    G.mortar_fine = m->d_mortar_fine; G.mortar_mat = m->d_mortar_mat; G.mW = m->d_mW;
+    if (m->dim == 3 && m->n_mortar > 0) {
+      cudaError_t et = launch_mortar_trace3d(m->np, u_in, m->d_mortar_info, m->d_mortar_fine, m->d_mortar_mat, m->gamma, m->d_mW,
+                                             m->n_mortar, st);
+      if (et != cudaSuccess) return fail(MARUT_ECUDA, "mortar trace kernel: %s", cudaGetErrorString(et));
+      m->launches++;
+    }
     memcpy(G.D, m->D, sizeof(G.D));
     cudaError_t e = launch_gradient(m->dim, m->np, m->affine, G, st);
     if (e != cudaSuccess) return fail(e == cudaErrorNotSupported ? MARUT_EINVAL : MARUT_ECUDA, "gradient kernel: %s", cudaGetErrorString(e));
@@ -540,8 +546,13 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.red_next = nullptr; P.dt_next = nullptr; P.cfl = 0.0; P.dx_min = m->dx_min; P.P2 = 2.0 * m->N + 1.0;
   memcpy(P.D, m->D, sizeof(P.D));
   P.mflux = m->d_mflux;
+  // Navier-Stokes with the strong form: the total flux F* - F_v* in one go; with the split form the hyperbolic flux for
+  // stage_split_kernel here and -F_v* for the viscous-only launch further down
+  const bool ns_total = m->physics == MARUT_NAVIER_STOKES && m->volume_form != MARUT_VOLUME_SPLIT_RANOCHA;
   if (m->dim == 3 && m->n_mortar > 0) {
-    cudaError_t em = launch_mortar_flux3d(m->np, u_in, m->d_metric, m->d_mortar_info, m->d_mortar_fine, m->d_mortar_mat, m->gamma,
+    cudaError_t em = ns_total ? launch_mortar_flux3d_ns(m->np, true, u_in, m->d_S, m->d_metric, m->d_mortar_info, m->d_mortar_fine,
+                                                        m->d_mortar_mat, m->gamma, m->d_mflux, m->n_mortar, st)
+                              : launch_mortar_flux3d(m->np, u_in, m->d_metric, m->d_mortar_info, m->d_mortar_fine, m->d_mortar_mat, m->gamma,
                                           m->d_mflux, m->n_mortar, st);
     if (em != cudaSuccess) return fail(MARUT_ECUDA, "mortar flux kernel: %s", cudaGetErrorString(em));
     m->launches++;
@@ -585,6 +596,12 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
         e = launch_stage_split(m->dim, m->np, m->affine, P, st);
         if (e != cudaSuccess) break;
         m->launches++;
+        if (m->dim == 3 && m->n_mortar > 0) {
+          e = launch_mortar_flux3d_ns(m->np, false, u_in, m->d_S, m->d_metric, m->d_mortar_info, m->d_mortar_fine, m->d_mortar_mat,
+                                      m->gamma, m->d_mflux, m->n_mortar, st);
+          if (e != cudaSuccess) break;
+          m->launches++;
+        }
         P.visc_only = 1;
         e = launch_stage_ns(m->dim, m->np, m->affine, P, st);
       } else e = launch_stage_ns(m->dim, m->np, m->affine, P, st);

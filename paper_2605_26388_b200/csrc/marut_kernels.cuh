@@ -81,6 +81,8 @@ struct GradParams {
   int boundary;                        // the mesh has boundary or mortar faces: launch the instantiation that knows them
   const int *__restrict__ mortar_fine; // 2-D mortars: [m][2] fine elements (lo, up)
   const double *__restrict__ mortar_mat; // [4][n*n]: Pf_lo, Pf_up, Pr_lo, Pr_up
+  const double *__restrict__ mW;       // 3-D mortars: the central trace What at the fine face nodes of every mortar,
+                                       //    [m][4][n*n][d+2] (mortar_trace3d_kernel, launched before this kernel); else NULL
 };
 
 // BR1 trace jump What - W at a boundary face node (reading R22).  kind: 0 prescribed state
@@ -192,6 +194,107 @@ __device__ __noinline__ void br1_mortar_jump_2d(const GradParams &P, long e, int
   }
 }
 
+// 3-D 4:1 mortars (readings R21 + R23): What = (W_F + (Pf[s0] x Pf[s1]) W_C)/2 at the 4 n^2 fine face nodes of every
+// mortar, evaluated once per mortar ahead of gradient_kernel (every coarse face node needs all of them).  One CTA per
+// mortar, one thread per (sub-face, fine face node); info[m] = (eC, fC, fF).
+template <int NP>
+__global__ void __launch_bounds__(4 * NP * NP) mortar_trace3d_kernel(const double *__restrict__ u, const int *__restrict__ info,
+                                                                     const int *__restrict__ mortar_fine,
+                                                                     const double *__restrict__ mortar_mat, double gamma,
+                                                                     double *__restrict__ mW) {
+  using G = Geo<3, NP>;
+  constexpr int NVAR = 5, NW = 5, NN = NP * NP * NP, NF = NP * NP;
+  __shared__ double WC[NF * NW], Pfs[2 * NP * NP];
+  const long m = blockIdx.x;
+  const int tid = threadIdx.x;
+  const int eC = info[m * 3], fC = info[m * 3 + 1], fF = info[m * 3 + 2];
+  if (tid < NF) {
+    double U[NVAR], W[NW];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) U[v] = __ldg(u + ((long)eC * NVAR + v) * NN + G::face_node(fC, tid % NP, tid / NP));
+    br1_vars<3>(U, gamma, W);
+#pragma unroll
+    for (int w = 0; w < NW; ++w) WC[tid * NW + w] = W[w];
+  }
+  for (int i = tid; i < 2 * NP * NP; i += 4 * NF) Pfs[i] = __ldg(&mortar_mat[i]);
+  __syncthreads();
+  const int s = tid / NF, b = tid - s * NF, b0 = b % NP, b1 = b / NP, s0 = s & 1, s1 = s >> 1;
+  const long eF = mortar_fine[m * 4 + s];
+  double UF[NVAR], WF[NW], Wi[NW];
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) UF[v] = __ldg(u + (eF * NVAR + v) * NN + G::face_node(fF, b0, b1));
+  br1_vars<3>(UF, gamma, WF);
+#pragma unroll
+  for (int w = 0; w < NW; ++w) Wi[w] = 0.0;
+  for (int j1 = 0; j1 < NP; ++j1) {
+    const double w1 = Pfs[(s1 * NP + b1) * NP + j1];
+    for (int j0 = 0; j0 < NP; ++j0) {
+      const double pw = Pfs[(s0 * NP + b0) * NP + j0] * w1;
+#pragma unroll
+      for (int w = 0; w < NW; ++w) Wi[w] += pw * WC[(j0 + NP * j1) * NW + w];
+    }
+  }
+#pragma unroll
+  for (int w = 0; w < NW; ++w) mW[((m * 4 + s) * NF + b) * NW + w] = 0.5 * (WF[w] + Wi[w]);
+}
+template <int NP>
+cudaError_t launch_mortar_trace3d_t(const double *u, const int *info, const int *fine, const double *mat, double gamma, double *mW,
+                                    long n_mortar, cudaStream_t st) {
+  mortar_trace3d_kernel<NP><<<(unsigned)n_mortar, 4 * NP * NP, 0, st>>>(u, info, fine, mat, gamma, mW);
+  return cudaGetLastError();
+}
+
+// BR1 surface term of the gradient at face node (a0, a1) of a 3-D mortar face (readings R21 + R23), from the stored
+// traces: fine side (What - W) n_c; coarse side  sum_s (Pr[s0] x Pr[s1]) (4 (-What_s n_F,s)) - W n_c.  Affine meshes
+// (the fine elements' normals are constant per face).  cn.x = mortar index, fR = the fine elements' face.
+template <int NP>
+__device__ __noinline__ void br1_mortar_jump_3d(const GradParams &P, int2 cn, int a0, int a1, const double *W, const double *nv,
+                                                double *add) {
+  constexpr int NW = 5, NF = NP * NP, MD = 10;
+  const int kind = cn.y & 3, fR = (cn.y >> 2) & 7, sub = (cn.y >> 8) & 3;
+  if (kind == FK_MORTAR_FINE) {
+    const double *Wh = P.mW + (((long)cn.x * 4 + sub) * NF + a0 + NP * a1) * NW;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+      const double jump = __ldg(Wh + w) - W[w];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) add[w * 3 + c] = jump * nv[c];
+    }
+  } else {
+    const double *Prv = P.mortar_mat + 2 * NP * NP;
+    double GC[NW * 3];
+#pragma unroll
+    for (int k = 0; k < NW * 3; ++k) GC[k] = 0.0;
+    const int lF = fR >> 1;
+    const double sF = (fR & 1) ? 1.0 : -1.0;
+    for (int m = 0; m < 4; ++m) {
+      const int s0 = m & 1, s1 = m >> 1;
+      const long eF = __ldg(&P.mortar_fine[cn.x * 4 + m]);
+      double nF[3];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) nF[c] = sF * __ldg(&P.metric[eF * MD + lF * 3 + c]);
+      const double *Wm = P.mW + ((long)cn.x * 4 + m) * NF * NW;
+      for (int b1 = 0; b1 < NP; ++b1) {
+        const double r1 = __ldg(&Prv[(s1 * NP + a1) * NP + b1]);
+        for (int b0 = 0; b0 < NP; ++b0) {
+          const double pr = __ldg(&Prv[(s0 * NP + a0) * NP + b0]) * r1;
+          const double *Wh = Wm + (b0 + NP * b1) * NW;
+#pragma unroll
+          for (int w = 0; w < NW; ++w) {
+            const double What = __ldg(Wh + w);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) GC[w * 3 + c] += pr * (4.0 * (-(What * nF[c])));
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int w = 0; w < NW; ++w)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) add[w * 3 + c] = GC[w * 3 + c] - W[w] * nv[c];
+  }
+}
+
 // ORIENT3: the instantiation for 3-D meshes with non-trivial face orientation codes (R20); the default one
 // keeps the identity pairing folded at compile time (the decode costs 12 registers here: 64 -> 76, one CTA less per SM)
 // BND: the instantiation for meshes with boundary faces (prescribed states, outflow, walls; reading R22) or 2-D mortars
@@ -273,6 +376,19 @@ gradient_kernel(const __grid_constant__ GradParams P) {
 #pragma unroll
           for (int c = 0; c < DIM; ++c) nv[c] = sgn * metric_at<DIM, NP, AFFINE>(P.metric, e, l * DIM + c, p);
           br1_mortar_jump_2d<NP, AFFINE>(P, e, f, q[1 - l], cn, W, Wsm + el * NN, TILE, nv, add);
+#pragma unroll
+          for (int k = 0; k < NW * DIM; ++k) Sg[k] += add[k] * P.inv_wb;
+          continue;
+        }
+      }
+      if constexpr (DIM == 3 && AFFINE) {
+        if ((cn.y & 3) != FK_CONFORMING) {          // 4:1 mortar face (readings R21 + R23)
+          double nv[DIM], add[NW * DIM];
+#pragma unroll
+          for (int c = 0; c < DIM; ++c) nv[c] = sgn * metric_at<DIM, NP, AFFINE>(P.metric, e, l * DIM + c, p);
+          int a0, a1;
+          G::face_coords(q, l, a0, a1);
+          br1_mortar_jump_3d<NP>(P, cn, a0, a1, W, nv, add);
 #pragma unroll
           for (int k = 0; k < NW * DIM; ++k) Sg[k] += add[k] * P.inv_wb;
           continue;

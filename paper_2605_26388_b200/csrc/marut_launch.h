@@ -14,5 +14,10 @@ cudaError_t launch_mortar_flux3d(int np, const double *u, const double *metric, 
 cudaError_t launch_stage_split(int dim, int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_stage_ns(int dim, int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_gradient(int dim, int np, bool affine, const GradParams &P, cudaStream_t st);
+cudaError_t launch_mortar_trace3d(int np, const double *u, const int *info, const int *fine, const double *mat, double gamma,
+                                  double *mW, long n_mortar, cudaStream_t st);
+cudaError_t launch_mortar_flux3d_ns(int np, bool hyp, const double *u, const double *S, const double *metric, const int *info,
+                                    const int *fine, const double *mat, double gamma, double *mflux, long n_mortar,
+                                    cudaStream_t st);
 cudaError_t launch_stage_react(int dim, int np, int nsp, bool affine, const StageParams &P, cudaStream_t st);
 }  // namespace marut

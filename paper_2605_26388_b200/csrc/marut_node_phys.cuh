@@ -108,6 +108,79 @@ __device__ __noinline__ void ns_mortar_viscous_2d(const StageParams &P, long e, 
   }
 }
 
+// Navier-Stokes across 3-D 4:1 mortars (readings R21 + R23): the TOTAL numerical flux T = F*_hyp - F_v* at the 4 n^2 fine
+// face nodes of every mortar (outward for the fine side, its normal), evaluated once per mortar ahead of the stage -- the
+// Rusanov flux of mortar_flux3d_kernel minus the central viscous flux (F_v(U_F, tau_F) + F_v(P U_C, P tau_C)).n_F / 2,
+// P = Pf[s0] x Pf[s1] applied to the coarse face's state and stored stress tensor / heat flux.  HYP = false: -F_v* alone
+// (the viscous-only launch after stage_split_kernel).  The stage then treats T exactly as the Euler kernels treat the
+// stored Rusanov flux (node_mortar_flux_3d).  One CTA per mortar, one thread per (sub-face, fine face node).  Affine.
+template <int NP, bool HYP>
+__global__ void __launch_bounds__(4 * NP * NP) mortar_flux3d_ns_kernel(const double *__restrict__ u, const double *__restrict__ S,
+                                                                       const double *__restrict__ metric, const int *__restrict__ info,
+                                                                       const int *__restrict__ mortar_fine,
+                                                                       const double *__restrict__ mortar_mat, double gamma,
+                                                                       double *__restrict__ mflux) {
+  using G = Geo<3, NP>;
+  constexpr int NVAR = 5, NN = NP * NP * NP, NF = NP * NP, MD = 10, NTAU = Tau<3>::NTAU, NC = NVAR + NTAU;
+  __shared__ double UC[NF * NC], Pfs[2 * NP * NP];      // coarse face: state and stored viscous tensor per face node
+  const long m = blockIdx.x;
+  const int tid = threadIdx.x;
+  const int eC = info[m * 3], fC = info[m * 3 + 1], fF = info[m * 3 + 2];
+  for (int i = tid; i < NF * NC; i += 4 * NF) {
+    const int j = i / NC, k = i - j * NC;
+    const int pC = G::face_node(fC, j % NP, j / NP);
+    UC[i] = (k < NVAR) ? __ldg(u + ((long)eC * NVAR + k) * NN + pC) : __ldg(S + ((long)eC * NTAU + (k - NVAR)) * NN + pC);
+  }
+  for (int i = tid; i < 2 * NP * NP; i += 4 * NF) Pfs[i] = __ldg(&mortar_mat[i]);
+  __syncthreads();
+  const int s = tid / NF, b = tid - s * NF, b0 = b % NP, b1 = b / NP, s0 = s & 1, s1 = s >> 1;
+  const long eF = mortar_fine[m * 4 + s];
+  const int pF = G::face_node(fF, b0, b1), lF = fF >> 1;
+  const double sF = (fF & 1) ? 1.0 : -1.0;
+  double UF[NVAR], tF[NTAU], Ci[NC], nF[3], T[NVAR];
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) UF[v] = __ldg(u + (eF * NVAR + v) * NN + pF);
+#pragma unroll
+  for (int k = 0; k < NTAU; ++k) tF[k] = __ldg(S + (eF * NTAU + k) * NN + pF);
+#pragma unroll
+  for (int k = 0; k < NC; ++k) Ci[k] = 0.0;
+  for (int j1 = 0; j1 < NP; ++j1) {
+    const double w1 = Pfs[(s1 * NP + b1) * NP + j1];
+    for (int j0 = 0; j0 < NP; ++j0) {
+      const double w = Pfs[(s0 * NP + b0) * NP + j0] * w1;
+#pragma unroll
+      for (int k = 0; k < NC; ++k) Ci[k] += w * UC[(j0 + NP * j1) * NC + k];
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) nF[c] = sF * __ldg(&metric[eF * MD + lF * 3 + c]);
+  const Prim<3> qF = prim_ideal<3, true>(UF, gamma);
+  const Prim<3> qC = prim_ideal<3, true>(Ci, gamma);
+  if constexpr (HYP) {
+    double FmF[NVAR];
+    flux_dot<3, 1>(UF, qF, nF, FmF);
+    rusanov<3, 1>(UF, qF, FmF, Ci, qC, nF, T);
+  } else {
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) T[v] = 0.0;
+  }
+  double FvF[NVAR], FvC[NVAR];
+  viscous_flux_dot_tau<3>(qF.v, tF, nF, FvF);
+  viscous_flux_dot_tau<3>(qC.v, Ci + NVAR, nF, FvC);
+#pragma unroll
+  for (int v = 1; v < NVAR; ++v) T[v] -= 0.5 * (FvF[v] + FvC[v]);
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) mflux[((m * 4 + s) * NF + b) * NVAR + v] = T[v];
+}
+template <int NP>
+cudaError_t launch_mortar_flux3d_ns_t(bool hyp, const double *u, const double *S, const double *metric, const int *info,
+                                      const int *fine, const double *mat, double gamma, double *mflux, long n_mortar,
+                                      cudaStream_t st) {
+  if (hyp) mortar_flux3d_ns_kernel<NP, true><<<(unsigned)n_mortar, 4 * NP * NP, 0, st>>>(u, S, metric, info, fine, mat, gamma, mflux);
+  else mortar_flux3d_ns_kernel<NP, false><<<(unsigned)n_mortar, 4 * NP * NP, 0, st>>>(u, S, metric, info, fine, mat, gamma, mflux);
+  return cudaGetLastError();
+}
+
 // BND (Navier-Stokes): the instantiation for meshes with boundary faces -- prescribed states, outflow, slip walls and the
 // no-slip adiabatic / isothermal walls of PAPER.md:223 (readings R18, R22); the default one carries no code
 // for them.
@@ -281,7 +354,7 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
       }
       nrm = sqrt(n2);
     }
-    const bool mort = BND && DIM == 2 && PHYS == PH_NS && (cn.y & 3) >= FK_MORTAR_FINE;   // 2-D 2:1 mortar face (reading R23)
+    const bool mort = BND && PHYS == PH_NS && (cn.y & 3) >= FK_MORTAR_FINE;   // 2:1 / 4:1 mortar face (readings R23, R21)
     if constexpr (BND) {
       if (mort) {
 #pragma unroll
@@ -350,6 +423,15 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
           ns_mortar_viscous_2d<NP>(P, ee, t.f, t.a0, cn, Fvm, nv, Fvs);
 #pragma unroll
           for (int v = 1; v < NVAR; ++v) lift[v] -= Fvs[v] - Fvm[v];
+        }
+      }
+      if constexpr (BND && DIM == 3 && AFFINE) {
+        if (mort) {
+          // the stored total flux T = F*_hyp - F_v* (mortar_flux3d_ns_kernel) against the own total normal flux
+          double Fs[NVAR];
+          node_mortar_flux_3d<NP>(P, t.a0, t.a1, cn, Fs);
+#pragma unroll
+          for (int v = 0; v < NVAR; ++v) lift[v] = Fs[v] - sgn * Fsm[((l * NVAR + v) * EB + t.el) * PS + sp];
         }
       }
       if (mort) {

@@ -61,8 +61,9 @@ def test_mortar3d_parity(N, axis, split):
 def test_mortar3d_is_rejected_where_it_is_not_built():
     import paper_2605_26388_b200 as mb
 
+    c = wl.make_case("c5", cells=2)                      # a reacting case: its mechanism on the half-refined box
     m = wl.octree_box_mesh(2, K=4)
-    m.physics, m.mu = wl.NAVIER_STOKES, 0.01
+    m.physics, m.mech = wl.REACTING_EULER, c.mesh.mech
     with pytest.raises(mb.MarutError):
         mb.MarutMesh(m)
 

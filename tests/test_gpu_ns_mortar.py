@@ -1,8 +1,9 @@
-"""GPU parity of the BR1 viscous terms across 2-D 2:1 mortars (DESIGN.md reading
-R23): the mortar branches of gradient_kernel (`br1_mortar_jump_2d`) and of stage_phys_kernel (`node_mortar_flux_2d` for
+"""GPU parity of the BR1 viscous terms across 2-D 2:1 mortars and 3-D 4:1 mortars (
+DESIGN.md readings R23, R21): the mortar branches of gradient_kernel (`br1_mortar_jump_2d`) and of stage_phys_kernel (`node_mortar_flux_2d` for
 the hyperbolic flux + `ns_mortar_viscous_2d`) against the oracle on the c4 band mesh run as a Navier-Stokes problem:
 N = 1..5, strong and split form, blended, all boundary kinds at the x boundaries; marut_rhs, marut_max_dt, a stage, steps,
-the shock-capturing composition; and the full c4 mesh size."""
+the shock-capturing composition; and the full c4 mesh size.  3-D: the half-refined periodic box (refinement along x, y,
+z), N = 1..5: the pre-kernels mortar_trace3d_kernel / mortar_flux3d_ns_kernel and the 3-D mortar branches."""
 import math
 
 import numpy as np
@@ -132,4 +133,71 @@ def test_full_c4_mesh_as_a_navier_stokes_problem():
     uc, tc, min_rho, min_p = om.run(u0, 3, cfl=CFL)
     assert min_rho > 0 and min_p > 0 and abs(tg - tc) <= 1e-12 * tc
     assert parity_error(ug, uc).max() <= RUN_TOL
+    gm.close()
+
+
+def _box3(N, axis, mu=0.02):
+    m = wl.octree_box_mesh(N, K=4, lo=(0.0,) * 3, hi=(2 * math.pi,) * 3, refine=lambda ix, iy, iz: (ix, iy, iz)[axis] < 2)
+    m.physics, m.mu, m.Pr = wl.NAVIER_STOKES, mu, 0.72
+    return m, wl.taylor_green(m, noise=1e-2)
+
+
+@pytest.mark.parametrize("N,axis", [(1, 0), (2, 1), (3, 2), (4, 0), (5, 1)])
+def test_navier_stokes_across_3d_mortars(N, axis):
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    m, u0 = _box3(N, axis)
+    assert len(m.mortar) == 32
+    om, gm = oracle.OracleMesh(m), mb.MarutMesh(m)
+    u = torch.from_numpy(u0).cuda()
+    du = torch.empty_like(u)
+    gm.rhs(u, du)
+    torch.cuda.synchronize()
+    assert parity_error(du.cpu().numpy(), om.rhs(u0)).max() <= RHS_TOL
+    dt = om.max_dt(u0, 0.3)
+    assert abs(gm.max_dt(u, 0.3) - dt) <= 1e-13 * dt
+    un_h = u0 * (1.0 + 1e-3)
+    un = torch.from_numpy(un_h).cuda()
+    gm.stage(2, dt, 0.0, un, u, un)
+    torch.cuda.synchronize()
+    assert parity_error(un.cpu().numpy(), om.ssprk_stage(2, dt, 0.0, un_h, u0)).max() <= RHS_TOL
+    ug, tg = gpu_run(gm, u0, 3, 0.3, torch)
+    uc, tc, min_rho, min_p = om.run(u0, 3, cfl=0.3)
+    assert min_rho > 0 and min_p > 0 and abs(tg - tc) <= 1e-12 * tc
+    assert parity_error(ug, uc).max() <= RUN_TOL
+    gm.close()
+
+
+@pytest.mark.parametrize("N,axis", [(2, 2), (3, 0), (4, 1)])
+def test_split_form_and_blend_across_3d_mortars(N, axis):
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    m, u0 = _box3(N, axis)
+    m.volume_form = 1
+    om, gm = oracle.OracleMesh(m), mb.MarutMesh(m)
+    u = torch.from_numpy(u0).cuda()
+    du = torch.empty_like(u)
+    alpha = np.random.default_rng(3).uniform(0, 1, m.n_elem)
+    alpha[::5] = 0.0
+    ad = torch.from_numpy(alpha).cuda()
+    for a in (None, alpha):
+        om.set_blend(a)
+        gm.set_blend(None if a is None else ad)
+        gm.rhs(u, du)
+        torch.cuda.synchronize()
+        assert parity_error(du.cpu().numpy(), om.rhs(u0)).max() <= RHS_TOL, a is not None
+    dt = om.max_dt(u0, 0.3)
+    ua, ub = torch.empty_like(u), torch.empty_like(u)
+    uh = u0
+    for _ in range(3):
+        uh = om.run(uh, 1, cfl=0.0, dt=dt)[0]
+        gm.step(u, ua, ub, dt)
+    torch.cuda.synchronize()
+    assert parity_error(u.cpu().numpy(), uh).max() <= RUN_TOL
     gm.close()
