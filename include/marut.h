@@ -166,6 +166,19 @@ marut_status marut_chem_implicit(marut_mesh *mesh, double *u, double dt, int *sw
 marut_status marut_shock_indicator(marut_mesh *mesh, const double *u, double s, double alpha_min, double alpha_max,
                                    int smooth, double *alpha, void *cuda_stream);
 
+/* marut_shock_indicator for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc).  marut_shock_indicator allocates on its first call per handle (V^-1; the unsmoothed alpha_e
+ * when smooth != 0); this variant runs the same kernels with that scratch in ONE fixed device array inside the library
+ * (8 MiB + 512 B per GPU that loads the library, held until exit) and calls no cudaMalloc / cudaFree / allocating
+ * routine.  Same arguments, same result (bit for bit).  Limit: n_elem <= marut_noalloc_max_elements() = 2^20, else
+ * EINVAL.  Every call on a device shares the array, which keeps the last call's contents; each call rewrites all it
+ * reads, so nothing needs clearing -- but two calls that OVERLAP on the GPU (different streams, same device) race: keep
+ * them on one stream or order them with events.  The first call per device looks up the array's device address
+ * (cudaGetSymbolAddress, no allocation); make that call outside a graph capture. */
+marut_status marut_shock_indicator_noalloc(marut_mesh *mesh, const double *u, double s, double alpha_min, double alpha_max,
+                                           int smooth, double *alpha, void *cuda_stream);
+long marut_noalloc_max_elements(void);
+
 /* Blended DG / sub-cell finite-volume volume residual (eq. 11, 655-672 eq. 42; DESIGN.md
  * reading R16):  R_i = (1 - alpha_e) R_i^(split) + alpha_e R_i^(FV), with the first-order finite-volume residual on the
  * LGL sub-cell grid

@@ -16,7 +16,7 @@ _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA"
 # every symbol include/marut.h declares
 SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt", "marut_max_dt_async", "marut_ssprk_stage_dev", "marut_rk_stage_dev",
            "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_rk_stage", "marut_lincomb", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count", "marut_debug_rcp_sqrt", "marut_debug_stage_kernel", "marut_ssprk33_step", "marut_ssprk33_step_cfl", "marut_ssprk54_step", "marut_strang_step",
-           "marut_last_error"]
+           "marut_shock_indicator_noalloc", "marut_noalloc_max_elements", "marut_last_error"]
 
 
 class MarutError(RuntimeError):
@@ -72,6 +72,10 @@ def lib():
         L.marut_chem_implicit.argtypes = [vp, vp, dbl, C.POINTER(C.c_int), vp]
         L.marut_shock_indicator.restype = C.c_int
         L.marut_shock_indicator.argtypes = [vp, vp, dbl, dbl, dbl, C.c_int, vp, vp]
+        L.marut_shock_indicator_noalloc.restype = C.c_int
+        L.marut_shock_indicator_noalloc.argtypes = [vp, vp, dbl, dbl, dbl, C.c_int, vp, vp]
+        L.marut_noalloc_max_elements.restype = C.c_long
+        L.marut_noalloc_max_elements.argtypes = []
         L.marut_rk_stage_dev.restype = C.c_int
         L.marut_rk_stage_dev.argtypes = [vp, dbl, dbl, dbl, vp, vp, vp, vp, vp]
         L.marut_rk_stage.restype = C.c_int
@@ -250,6 +254,15 @@ def marut_ssprk33_step(h, u, ua, ub, dt=0.0, dt_dev=None, stream=None):
 
 def marut_shock_indicator(h, u, alpha, s=9.21024, alpha_min=0.001, alpha_max=0.5, smooth=True, stream=None):
     _check(lib().marut_shock_indicator(h, _dev(u), s, alpha_min, alpha_max, int(bool(smooth)), _dev(alpha), _stream(stream)))
+
+
+def marut_shock_indicator_noalloc(h, u, alpha, s=9.21024, alpha_min=0.001, alpha_max=0.5, smooth=True, stream=None):
+    """marut_shock_indicator with its scratch in a fixed device array of the library: no allocation, n_elem <= 2^20"""
+    _check(lib().marut_shock_indicator_noalloc(h, _dev(u), s, alpha_min, alpha_max, int(bool(smooth)), _dev(alpha), _stream(stream)))
+
+
+def marut_noalloc_max_elements():
+    return int(lib().marut_noalloc_max_elements())
 
 
 def marut_set_boundary_kinds(h, kinds):

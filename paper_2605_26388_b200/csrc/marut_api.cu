@@ -1041,6 +1041,88 @@ extern "C" marut_status marut_shock_indicator(marut_mesh *m, const double *u, do
   return MARUT_OK;
 }
 
+// ------------------------------------------------------------------------------------ shock indicator without allocations
+// marut_shock_indicator allocates on its first call per handle (V^-1, and the unsmoothed alpha_e when smooth != 0).  Callers
+// that must not allocate -- code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc -- use
+// marut_shock_indicator_noalloc: the same two kernels with their scratch in ONE file-scope device array of fixed size,
+// [0, 64): V^-1 (n x n), [64, 64 + n_elem): the unsmoothed alpha_e.  8 MiB + 512 B per GPU that loads the library, held
+// until exit.  The array is shared by every call on the device and keeps the last call's contents: each call rewrites
+// all of what it reads (nothing has to start at zero), and two calls that overlap on the GPU (different streams) race.
+constexpr long NOALLOC_MAX_ELEM = 1L << 20;
+static __device__ __align__(256) double g_noalloc_scratch[64 + NOALLOC_MAX_ELEM];
+struct VinvArg { double v[MAX_NP * MAX_NP]; };
+__global__ void noalloc_set_vinv_kernel(VinvArg a, double *__restrict__ dst, int n) {
+  if ((int)threadIdx.x < n) dst[threadIdx.x] = a.v[threadIdx.x];
+}
+// device address of the scratch array: in host code its name is a host-side stand-in, not a device address.  Queried
+// once per device (with that device current), no allocation involved.
+static cudaError_t noalloc_scratch_ptr(double **out) {
+  static std::atomic<double *> ptr[64];
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  double *p = (dev >= 0 && dev < 64) ? ptr[dev].load(std::memory_order_acquire) : nullptr;
+  if (!p) {
+    e = cudaGetSymbolAddress((void **)&p, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < 64) ptr[dev].store(p, std::memory_order_release);
+  }
+  *out = p;
+  return cudaSuccess;
+}
+template <int DIM, int NP>
+static cudaError_t run_indicator_noalloc(const marut_mesh *m, const double *u, const double *Vinv, double s_over_T, double T,
+                                         double amin, double amax, double *out, cudaStream_t st) {
+  constexpr int NN = Geo<DIM, NP>::NN, EB = (NN >= 96) ? 1 : 128 / NN, NT = ((EB * NN + 31) / 32) * 32;
+  const unsigned grid = (unsigned)((m->ne + EB - 1) / EB);
+  indicator_kernel<DIM, NP, EB><<<grid, NT, 0, st>>>(u, Vinv, m->gamma, s_over_T, T, amin, amax, m->ne, out);
+  return cudaGetLastError();
+}
+extern "C" long marut_noalloc_max_elements(void) { return NOALLOC_MAX_ELEM; }
+extern "C" marut_status marut_shock_indicator_noalloc(marut_mesh *m, const double *u, double s, double alpha_min, double alpha_max,
+                                                      int smooth, double *alpha, void *stream) {
+  if (!m || !u || !alpha) return fail(MARUT_EINVAL, "NULL argument");
+  if (m->physics == MARUT_REACTING_EULER) return fail(MARUT_EINVAL, "marut_shock_indicator_noalloc: ideal-gas meshes only");
+  if (!(s > 0.0) || !(alpha_min >= 0.0) || !(alpha_max >= alpha_min) || !(alpha_max <= 1.0))
+    return fail(MARUT_EINVAL, "need s > 0 and 0 <= alpha_min <= alpha_max <= 1");
+  if (m->ne > NOALLOC_MAX_ELEM)
+    return fail(MARUT_EINVAL, "marut_shock_indicator_noalloc: %ld elements exceed the fixed scratch of %ld elements "
+                "(use marut_shock_indicator, which allocates)", m->ne, NOALLOC_MAX_ELEM);
+  cudaStream_t st = (cudaStream_t)stream;
+  double *scratch = nullptr;
+  cudaError_t e = noalloc_scratch_ptr(&scratch);
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "cudaGetSymbolAddress(scratch): %s", cudaGetErrorString(e));
+  VinvArg V;
+  {
+    double x[MAX_NP], w[MAX_NP], D[MAX_NP * MAX_NP];
+    build_operators(m->N, x, w, D);
+    for (int i = 0; i < MAX_NP * MAX_NP; ++i) V.v[i] = 0.0;
+    if (!build_modal_matrix(m->N, x, V.v)) return fail(MARUT_EINVAL, "singular Vandermonde matrix");
+  }
+  noalloc_set_vinv_kernel<<<1, 64, 0, st>>>(V, scratch, m->np * m->np);    // the matrix travels as a kernel argument
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "scratch set-up kernel: %s", cudaGetErrorString(e));
+  m->launches++;
+  const double T = 0.5 * std::pow(10.0, -1.8 * std::pow((double)(m->N + 1), 0.25));
+  double *raw = smooth ? scratch + 64 : alpha;
+  e = cudaErrorNotSupported;
+#define MARUT_IND(D_, NP_) if (m->dim == D_ && m->np == NP_) e = run_indicator_noalloc<D_, NP_>(m, u, scratch, s / T, T, alpha_min, alpha_max, raw, st);
+  MARUT_IND(2, 2) MARUT_IND(2, 3) MARUT_IND(2, 4) MARUT_IND(2, 5) MARUT_IND(2, 6) MARUT_IND(2, 7) MARUT_IND(2, 8)
+  MARUT_IND(3, 2) MARUT_IND(3, 3) MARUT_IND(3, 4) MARUT_IND(3, 5) MARUT_IND(3, 6) MARUT_IND(3, 7) MARUT_IND(3, 8)
+#undef MARUT_IND
+  if (e != cudaSuccess) return fail(MARUT_ECUDA, "indicator kernel: %s", cudaGetErrorString(e));
+  m->launches++;
+  if (smooth) {
+    const unsigned grid = (unsigned)((m->ne + 255) / 256);
+    if (m->dim == 2) indicator_smooth_kernel<2><<<grid, 256, 0, st>>>(raw, m->d_conn, m->d_mortar_fine, m->d_mortar_info, m->ne, alpha);
+    else indicator_smooth_kernel<3><<<grid, 256, 0, st>>>(raw, m->d_conn, m->d_mortar_fine, m->d_mortar_info, m->ne, alpha);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(MARUT_ECUDA, "indicator smoothing kernel: %s", cudaGetErrorString(e));
+    m->launches++;
+  }
+  return MARUT_OK;
+}
+
 // ------------------------------------------------------------------------------------ time step
 template <int DIM, int NSP, int PHYS>
 static cudaError_t launch_wave_speed(marut_mesh *m, const double *u, const MechDev *mech, cudaStream_t st) {
