@@ -307,6 +307,10 @@ gradient_kernel(const __grid_constant__ GradParams P) {
   extern __shared__ double smem[];
   double *Wsm = smem;                 // [NW][TILE]
   double *Dsm = smem + NW * TILE;     // [NP*NP]
+  // curved meshes: the node's own metric terms Ja^l_c go through shared memory, [DIM*DIM][TILE] -- one coalesced load
+  // per plane, in flight together with the state, instead of DIM * NP * DIM dependent loads inside the derivative loops
+  // (the kernel sat on them: long-scoreboard stalls 9.6 per issued instruction, profiles/r02_c3_stage.md)
+  double *Jsm = Dsm + ((NP * NP + 1) & ~1);
   const int tid = threadIdx.x;
   for (int i = tid; i < NP * NP; i += blockDim.x) Dsm[i] = P.D[i];
   const int el = tid / NN, p = tid - el * NN;
@@ -319,6 +323,13 @@ gradient_kernel(const __grid_constant__ GradParams P) {
     double U[NVAR];
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) U[v] = __ldg(P.u + (e * NVAR + v) * NN + p);
+    if constexpr (!AFFINE) {
+      double Jo[DIM * DIM];
+#pragma unroll
+      for (int k = 0; k < DIM * DIM; ++k) Jo[k] = __ldg(&P.metric[(e * MD + k) * NN + p]);
+#pragma unroll
+      for (int k = 0; k < DIM * DIM; ++k) Jsm[k * TILE + tid] = Jo[k];
+    }
     const Prim<DIM> pr = prim_ideal<DIM, false>(U, P.gamma);
     W[0] = pr.rho;
 #pragma unroll
@@ -339,7 +350,8 @@ gradient_kernel(const __grid_constant__ GradParams P) {
       const double d = Dsm[q[l] * NP + m];
       double Jm[DIM];
 #pragma unroll
-      for (int c = 0; c < DIM; ++c) Jm[c] = d * metric_at<DIM, NP, AFFINE>(P.metric, e, l * DIM + c, pbase + m * st);
+      for (int c = 0; c < DIM; ++c)
+        Jm[c] = d * (AFFINE ? metric_at<DIM, NP, AFFINE>(P.metric, e, l * DIM + c, pbase + m * st) : Jsm[(l * DIM + c) * TILE + base + m * st]);
 #pragma unroll
       for (int w = 0; w < NW; ++w) {
         const double Wm = Wsm[w * TILE + base + m * st];
@@ -444,7 +456,7 @@ __device__ __forceinline__ void load_mech(MechDev *dst_s, const MechDev *src_g) 
 // The stage kernel then needs no mechanism table, no exponentials and no Newton: it keeps the footprint of the Euler
 // stage (the chemistry is purely per node, "no inter-thread communication").
 template <int DIM, int NSP>
-__global__ void __launch_bounds__(256) eos_kernel(const double *__restrict__ u, double *__restrict__ aux,
+__global__ void __launch_bounds__(256, 3) eos_kernel(const double *__restrict__ u, double *__restrict__ aux,
                                                   const MechDev *__restrict__ mech_g, long ne, int nn, int with_source) {
   constexpr int NVAR = NSP + DIM + 1, NA = 2 + NSP;
   __shared__ MechDev mech;
@@ -936,7 +948,7 @@ cudaError_t launch_gradient_t(const GradParams &P, cudaStream_t st) {
   }
   constexpr int NN = Geo<DIM, NP>::NN, EB = elems_per_block<NN>();
   constexpr int threads = ((EB * NN + 31) / 32) * 32;
-  constexpr size_t smem = (size_t)((DIM + 2) * EB * NN + NP * NP) * sizeof(double);
+  constexpr size_t smem = (size_t)((DIM + 2) * EB * NN + ((NP * NP + 1) & ~1) + (AFFINE ? 0 : DIM * DIM * EB * NN)) * sizeof(double);
   auto k = gradient_kernel<DIM, NP, AFFINE, EB, ORIENT3, BND>;
   static std::atomic<unsigned long long> attr_done{0};
   if (cudaError_t err = set_smem_once((const void *)k, smem, attr_done); err != cudaSuccess) return err;

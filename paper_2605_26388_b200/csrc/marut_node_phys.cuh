@@ -28,7 +28,12 @@ struct PhysCfg {
   static constexpr int NFN = 2 * DIM * NF, NTASK = EB * NFN;
   static constexpr int NT = ((TILE + 31) / 32) * 32;
   static constexpr int NST = NVAR + 3;                       // stash planes: U, 1/rho, p, a
-  static constexpr int KS = NP * NP, PS = NN | 1;            // plane strides (odd plane stride)
+  // plane strides.  3-D, n = 4: lines of four doubles at row stride 4 / plane stride 16 put a half-warp's line tasks on 4
+  // of the 16 banks in the xi and eta passes (57 % of the kernel's shared-memory wavefronts were conflicts,
+  // profiles/r02_c3_stage.md); a k-plane stride of 17 and a variable-plane stride of 70 make the xi pass conflict-free and
+  // leave the eta pass at 1.6x the minimum (brute-force count over the strides, as for NodeLayout)
+  static constexpr bool PAD4 = (DIM == 3 && NP == 4);
+  static constexpr int KS = PAD4 ? 17 : NP * NP, PS = PAD4 ? 70 : (NN | 1);
   static constexpr int NFP = DIM * NVAR * EB;                // flux planes
   static constexpr int NRP = NVAR * EB;                      // result planes
   static constexpr int NSRC = 0;                             // (the chemistry source comes from eos_kernel's aux array)
