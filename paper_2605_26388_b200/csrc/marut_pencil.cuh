@@ -7,15 +7,16 @@
 //            issues the copy for the tile after next when the current tile is finished.  N = 4 in 3-D has 5000-byte
 //            elements: the 16-byte window the copy needs is obtained by starting one double early (`shift`).
 //            The tile's connectivity and metric terms come in by 8-byte cp.async one tile ahead; u_n of the tile is
-//            L2-prefetched (cp.async.bulk.prefetch.L2) after the first phase, two phases before it is read.
+//            L2-prefetched (cp.async.bulk.prefetch.L2) at the start of the tile, one phase before it is read.
 //   phase l (l = 0 .. d-1): the thread owns the line of direction l through (a0, a1): it reads the line's U from the
 //            tile, evaluates the contravariant flux Ftilde^l (eq. 9) at its n nodes, applies D along the line in
 //            registers, and -- because the line's two end nodes ARE the face nodes (a0, a1) of faces 2l and 2l+1 --
 //            evaluates both Rusanov lifts (eq. 12) from registers: no stash, no lift buffer, no divergence.
 //            Exterior traces: from the tile itself when the neighbour is one of the tile's elements, else gathered from
 //            global memory (L2); issued at the start of the phase, consumed at its end.
-//            The partial residual goes through one shared buffer R: phase 0 writes, phase 1 adds, the last phase
-//            adds, applies 1/J and the SSP-RK combination (eq. 45) and writes u_out (zeta lines: coalesced).
+//            The partial residual goes through one shared buffer R: phase 0 writes, phase 1 adds (and folds in the
+//            u_n term of eq. 45), the last phase adds, applies 1/J and the SSP-RK combination (eq. 45) and writes u_out
+//            (zeta lines: coalesced).
 //   Per node: 15 shared loads of U and 20 accesses of R, against ~115 shared accesses of the thread-per-node kernel;
 //   3 CTA barriers per tile; 1.0/x and sqrt(x) are evaluated by the branch-free sequences of marut_common.cuh.
 //
@@ -153,10 +154,10 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
   using C = PencilCfg<DIM, NP>;
   constexpr int NVAR = C::NVAR, NN = C::NN, NL = C::NL, ED = C::ED, MD = Geo<DIM, NP>::MD;
   constexpr bool FIRST = (L == 0), LAST = (L == DIM - 1);
-  // 3-D: the u_n term of eq. 45 enters the partial residual in the MIDDLE phase, R += g u_n with g = -ca J / cc, so that
-  // the last phase's  cb U + cc (0 - R / J)  already contains ca u_n: the loads run one variable ahead of their use in a
-  // phase that has the registers for it (in the last phase they stall the combination: 13 % of its issue slots)
-  constexpr bool FOLD3 = (DIM == 3), FOLD_HERE = FOLD3 && (L == 1);
+  // The u_n term of eq. 45 enters the partial residual in phase 1 (3-D: the middle phase, 2-D: the last one), R += g u_n
+  // with g = -ca J / cc, so that  cb U + cc (0 - R / J)  already contains ca u_n; its loads run one variable ahead of their
+  // use (loaded where the combination needs them they stalled it: 13 % of the last phase's issue slots in 3-D)
+  constexpr bool FOLD_HERE = (L == 1);
   constexpr int SM = (L == 0) ? 1 : ((L == 1) ? NP : NP * NP);
   if (t >= nel * NL) return;
   const int el = t / NL, r = t - el * NL;
@@ -178,7 +179,6 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
       for (int m = 0; m < NP; ++m) U[v][m] = ul[v * NN + m * SM];
     }
   }
-  const bool use_un = LAST && !FOLD3 && (P.ca != 0.0);
   const bool fold_un = FOLD_HERE && (P.ca != 0.0);
   const long gofs = e * ED + p0;
   const double *met = Md + C::NCN + el * MD;
@@ -213,13 +213,6 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
   double accE[NVAR][2];
 #pragma unroll
   for (int v = 0; v < NVAR; ++v) {
-    double un[NP];
-    if constexpr (LAST) {
-      if (use_un) {
-#pragma unroll
-        for (int m = 1; m < NP - 1; ++m) un[m] = __ldcs(P.u_n + gofs + v * NN + m * SM);
-      }
-    }
     if constexpr (FOLD_HERE) {
       if (fold_un && v + 1 < NVAR) {
 #pragma unroll
@@ -255,20 +248,9 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
     } else {
 #pragma unroll
       for (int m = 1; m < NP - 1; ++m) {
-        const double val = P.cb * U[v][m] + cc * (0.0 - invJ * acc[m]);
-        const double o = use_un ? (P.ca * un[m] + val) : val;
+        const double o = P.cb * U[v][m] + cc * (0.0 - invJ * acc[m]);
         P.u_out[gofs + v * NN + m * SM] = o;
         if constexpr (FUSE) U[v][m] = o;       // the node's new state replaces its old one (no longer needed)
-      }
-    }
-  }
-  double unE[NVAR][2];
-  if constexpr (LAST) {
-    if (use_un) {
-#pragma unroll
-      for (int v = 0; v < NVAR; ++v) {
-        unE[v][0] = __ldcs(P.u_n + gofs + v * NN);
-        unE[v][1] = __ldcs(P.u_n + gofs + v * NN + (NP - 1) * SM);
       }
     }
   }
@@ -321,8 +303,7 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
       rl[v * NN] = r0;
       rl[v * NN + (NP - 1) * SM] = r1;
     } else {
-      const double v0 = P.cb * U[v][0] + cc * (0.0 - invJ * r0), v1 = P.cb * U[v][NP - 1] + cc * (0.0 - invJ * r1);
-      const double o0 = use_un ? (P.ca * unE[v][0] + v0) : v0, o1 = use_un ? (P.ca * unE[v][1] + v1) : v1;
+      const double o0 = P.cb * U[v][0] + cc * (0.0 - invJ * r0), o1 = P.cb * U[v][NP - 1] + cc * (0.0 - invJ * r1);
       P.u_out[gofs + v * NN] = o0;
       P.u_out[gofs + v * NN + (NP - 1) * SM] = o1;
       if constexpr (FUSE) {
@@ -424,12 +405,10 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
       for (int i = tid; i < nel * ED; i += NT) dst[i] = __ldg(P.u_in + e0 * ED + i);
       __syncthreads();
     }
-    // u_n of this tile is read one phase (3-D: by the middle phase) or two phases (2-D) later: bring it into L2 now
-    // (earlier, and part of it is evicted again)
-    if (DIM == 3 && tid == 0 && use_un && by_tma) bulk_prefetch_l2(P.u_n + ws, (uint32_t)wl * 8u);
+    // u_n of this tile is read by phase 1: bring it into L2 one phase ahead (earlier, and part of it is evicted again)
+    if (tid == 0 && use_un && by_tma) bulk_prefetch_l2(P.u_n + ws, (uint32_t)wl * 8u);
     pencil_phase<DIM, NP, 0, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
     __syncthreads();
-    if (DIM == 2 && tid == 0 && use_un && by_tma) bulk_prefetch_l2(P.u_n + ws, (uint32_t)wl * 8u);
     if constexpr (DIM == 3) {
       pencil_phase<DIM, NP, 1, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
       __syncthreads();
