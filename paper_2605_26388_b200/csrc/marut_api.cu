@@ -41,6 +41,8 @@ struct marut_mesh {
   bool oriented = false;       // some 3-D interface has a non-trivial orientation code (R20)
   bool bc_kinds = false;       // some boundary id is an outflow / slip-wall face
   int pencil_reverse = 0;      // tile direction of the next launch of the persistent line kernel (alternates)
+  int *d_tiles_plain = nullptr, *d_tiles_mortar = nullptr;   // 2-D mortar meshes: the line kernel's tiles without / with mortar faces
+  long n_tiles_plain = 0, n_tiles_mortar = 0;
   double gamma = 1.4, mu = 0.0, Pr = 0.72, kappa = 0.0;
   bool affine = false;
   double dx_min = 0.0;
@@ -243,7 +245,7 @@ extern "C" void marut_mesh_destroy(marut_mesh *m) {
   cudaDeviceSynchronize();
   cudaFree(m->d_metric); cudaFree(m->d_fnorm); cudaFree(m->d_conn); cudaFree(m->d_mortar_fine); cudaFree(m->d_mortar_info); cudaFree(m->d_mflux); cudaFree(m->d_mW); cudaFree(m->d_mortar_mat);
   cudaFree(m->d_Vinv); cudaFree(m->d_araw); cudaFree(m->d_subn); cudaFree(m->d_bc); cudaFree(m->d_S); cudaFree(m->d_T); cudaFree(m->d_mech); cudaFree(m->d_red);
-  cudaFree(m->d_red_next);
+  cudaFree(m->d_red_next); cudaFree(m->d_tiles_plain); cudaFree(m->d_tiles_mortar);
   if (m->h_red) cudaFreeHost(m->h_red);
   delete m;
 }
@@ -388,6 +390,22 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   // ---- uploads
   CUDA_TRY(cudaMalloc(&m->d_conn, conn.size() * sizeof(int2)));
   CUDA_TRY(cudaMemcpy(m->d_conn, conn.data(), conn.size() * sizeof(int2), cudaMemcpyHostToDevice));
+  if (dim == 2 && d->n_mortar > 0) {
+    // tiles of the persistent line kernel (128 / n consecutive elements, csrc/marut_pencil.cuh) with and without mortar
+    // faces: the few with go to the kernel instantiation that carries the mortar path, the rest to the plain one
+    const long et = 128 / np, nt = (ne + et - 1) / et;
+    std::vector<int> plain, mort_t;
+    for (long t = 0; t < nt; ++t) {
+      bool has = false;
+      for (long i = t * et * nf2; i < std::min<long>((t + 1) * et, ne) * nf2 && !has; ++i) has = (conn[i].y & 3) >= FK_MORTAR_FINE;
+      (has ? mort_t : plain).push_back((int)t);
+    }
+    m->n_tiles_plain = (long)plain.size(); m->n_tiles_mortar = (long)mort_t.size();
+    CUDA_TRY(cudaMalloc(&m->d_tiles_plain, std::max<size_t>(1, plain.size()) * sizeof(int)));
+    CUDA_TRY(cudaMalloc(&m->d_tiles_mortar, std::max<size_t>(1, mort_t.size()) * sizeof(int)));
+    if (!plain.empty()) CUDA_TRY(cudaMemcpy(m->d_tiles_plain, plain.data(), plain.size() * sizeof(int), cudaMemcpyHostToDevice));
+    if (!mort_t.empty()) CUDA_TRY(cudaMemcpy(m->d_tiles_mortar, mort_t.data(), mort_t.size() * sizeof(int), cudaMemcpyHostToDevice));
+  }
   CUDA_TRY(cudaMalloc(&m->d_mortar_fine, mfine.size() * sizeof(int)));
   CUDA_TRY(cudaMemcpy(m->d_mortar_fine, mfine.data(), mfine.size() * sizeof(int), cudaMemcpyHostToDevice));
   if (dim == 3 && d->n_mortar > 0) {
@@ -542,7 +560,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.bc_state = m->d_bc; P.S = m->d_S; P.Taux = m->d_T; P.mech = m->d_mech;
   P.ca = ca; P.cb = cb; P.cc = cc; P.dt_dev = dt_dev;
   P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne; P.num_sms = m->num_sms;
-  P.visc_only = 0;
+  P.visc_only = 0; P.tile_list = nullptr; P.n_tile_list = 0; P.reverse = 0; P.zero = 0;
   P.red_next = nullptr; P.dt_next = nullptr; P.cfl = 0.0; P.dx_min = m->dx_min; P.P2 = 2.0 * m->N + 1.0;
   memcpy(P.D, m->D, sizeof(P.D));
   P.mflux = m->d_mflux;
@@ -580,7 +598,28 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
           // one in L2); the result does not depend on the direction
           P.zero = 0;
           P.reverse = m->pencil_reverse;
-          e = launch_stage_pencil(m->dim, m->np, m->n_mortar > 0, m->stage_kernel_pref == 2, P, st);
+          const bool force = m->stage_kernel_pref == 2;
+          if (m->n_mortar > 0) {
+            // two launches: the tiles without mortar faces through the plain instantiation (the one with the mortar
+            // path runs every tile 63 % slower: 168 registers, a stack frame), then the few tiles with mortar faces.
+            // The first contributes its maxima to the fused CFL reduction, the second finalizes it.
+            const long nres = 3L * m->num_sms;
+            if (m->n_tiles_plain + m->n_tiles_mortar < nres && !force) e = cudaErrorNotSupported;
+            else {
+              e = cudaSuccess;
+              if (m->n_tiles_plain > 0) {
+                StageParams Pa = P;
+                Pa.tile_list = m->d_tiles_plain; Pa.n_tile_list = m->n_tiles_plain; Pa.dt_next = nullptr;
+                e = launch_stage_pencil(m->dim, m->np, false, true, Pa, st);
+                if (e == cudaSuccess) m->launches++;
+              }
+              if (e == cudaSuccess) {
+                P.tile_list = m->d_tiles_mortar; P.n_tile_list = m->n_tiles_mortar;
+                e = launch_stage_pencil(m->dim, m->np, true, true, P, st);
+                P.tile_list = nullptr; P.n_tile_list = 0;
+              }
+            }
+          } else e = launch_stage_pencil(m->dim, m->np, false, force, P, st);
           if (e == cudaSuccess) m->pencil_reverse ^= 1;
           if (fuse) fuse->done = (e == cudaSuccess) && P.red_next != nullptr;
           P.red_next = nullptr;

@@ -21,7 +21,10 @@
 //   3 CTA barriers per tile; 1.0/x and sqrt(x) are evaluated by the branch-free sequences of marut_common.cuh.
 //
 // Selected for MARUT_EULER with the strong form on affine meshes without outflow / slip-wall faces and without 3-D
-// mortars (those run stage_node_kernel).  PAPER.md:179-204, 713-725; R4-R8, R10.
+// mortars (those run stage_node_kernel).  2-D meshes with 2:1 mortars run as TWO launches over tile lists built at
+// marut_mesh_create: the tiles without mortar faces through the plain instantiation, the few with mortar faces through
+// the MORTAR one (with the mortar path compiled into the kernel every tile ran 63 % slower: 168 registers and a stack
+// frame; dispatching per tile inside one kernel, inlined or out of line, did not recover it).  PAPER.md:179-204, 713-725; R4-R8, R10.
 // Product code; shares nothing with oracle/.
 #pragma once
 #include "marut_node.cuh"
@@ -338,7 +341,7 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
   double *Mds = Rs + TD;
   uint64_t *bars = reinterpret_cast<uint64_t *>(Mds + 2 * MW);
   const int tid = threadIdx.x;
-  const long ntile = (P.ne + ET - 1) / ET;
+  const long ntile = P.tile_list ? P.n_tile_list : (P.ne + ET - 1) / ET;
   const long total = P.ne * ED;
   const bool use_un = (P.ca != 0.0);
   auto window = [&](long tile, long &ws, int &wl, int &shift) -> bool {
@@ -351,7 +354,10 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
   };
   // P.reverse: the tiles are walked from the last to the first.  Consecutive stage launches alternate the direction, so
   // that a launch starts on the part of its input that the previous launch wrote or read last (still in L2).
-  auto phys = [&](long k) -> long { return P.reverse ? ntile - 1 - k : k; };
+  auto phys = [&](long k) -> long {
+    const long i = P.reverse ? ntile - 1 - k : k;
+    return P.tile_list ? (long)__ldg(&P.tile_list[i]) : i;
+  };
   auto issue = [&](long k, int buf) {
     const long tile = phys(k);
     long ws;
@@ -430,7 +436,7 @@ cudaError_t launch_stage_pencil_t(const StageParams &P, bool force, cudaStream_t
   auto k = stage_pencil_kernel<DIM, NP, MORTAR, FUSE>;
   static std::atomic<unsigned long long> attr_done{0};
   if (cudaError_t err = set_smem_once((const void *)k, C::smem_bytes, attr_done); err != cudaSuccess) return err;
-  const long ntile = (P.ne + C::ET - 1) / C::ET;
+  const long ntile = P.tile_list ? P.n_tile_list : (P.ne + C::ET - 1) / C::ET;
   const long nres = (long)C::MINB * P.num_sms;   // one resident wave
   // a mesh that cannot fill the GPU with tiles runs the thread-per-node kernel (its smaller CTAs spread it better),
   // unless the caller insists (marut_debug_stage_kernel: the parity tests of small meshes)
