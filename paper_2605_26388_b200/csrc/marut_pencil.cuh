@@ -265,8 +265,9 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
     const int late = __double2loint(accE[NVAR - 1][1]) & P.zero;
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) {
-      Up0[v] = __hiloint2double(__double2hiint(Up0[v]), __double2loint(Up0[v]) ^ late);
-      Up1[v] = __hiloint2double(__double2hiint(Up1[v]), __double2loint(Up1[v]) ^ late);
+      // (the HIGH word: the reciprocal's seed instruction, MUFU.RCP64H, reads nothing else)
+      Up0[v] = __hiloint2double(__double2hiint(Up0[v]) ^ late, __double2loint(Up0[v]));
+      Up1[v] = __hiloint2double(__double2hiint(Up1[v]) ^ late, __double2loint(Up1[v]));
     }
   }
   const PencilFace F0 = pencil_face<DIM>(Up0, Ja, nrm, P.gamma, vn[0], pr[0], rinv[0]);
