@@ -191,12 +191,14 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
   const double nrm = Md[C::NCN + C::NMT + el * DIM + L];
   double invJ = 0.0;
   if constexpr (LAST || FOLD_HERE) invJ = met[DIM * DIM];
-  double g = 0.0, unb[2][NP];      // u_n of variable v in unb[v & 1]: loaded while variable v - 1 is worked on
+  double g = 0.0, unb[3][NP];      // u_n of variable v in unb[v % 3]: loaded while variables v - 2, v - 1 are worked on
   if constexpr (FOLD_HERE) {
     if (fold_un) {
       g = (0.0 - P.ca) / (cc * invJ);
 #pragma unroll
       for (int m = 0; m < NP; ++m) unb[0][m] = __ldcs(P.u_n + gofs + m * SM);
+#pragma unroll
+      for (int m = 0; m < NP; ++m) unb[1][m] = __ldcs(P.u_n + gofs + NN + m * SM);
     }
   }
   double rinv[NP], pr[NP], vn[NP];
@@ -217,9 +219,9 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
 #pragma unroll
   for (int v = 0; v < NVAR; ++v) {
     if constexpr (FOLD_HERE) {
-      if (fold_un && v + 1 < NVAR) {
+      if (fold_un && v + 2 < NVAR) {
 #pragma unroll
-        for (int m = 0; m < NP; ++m) unb[(v + 1) & 1][m] = __ldcs(P.u_n + gofs + (v + 1) * NN + m * SM);
+        for (int m = 0; m < NP; ++m) unb[(v + 2) % 3][m] = __ldcs(P.u_n + gofs + (v + 2) * NN + m * SM);
       }
     }
     double f[NP], acc[NP];
@@ -240,7 +242,7 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
     if constexpr (FOLD_HERE) {
       if (fold_un) {
 #pragma unroll
-        for (int i = 0; i < NP; ++i) acc[i] = fma(g, unb[v & 1][i], acc[i]);
+        for (int i = 0; i < NP; ++i) acc[i] = fma(g, unb[v % 3][i], acc[i]);
       }
     }
     accE[v][0] = acc[0];
