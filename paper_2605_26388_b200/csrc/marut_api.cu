@@ -366,7 +366,11 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
     for (int k = 0; k < nfine; ++k) if (M[2 + k] < 0 || M[2 + k] >= ne) return fail(MARUT_ETOPOLOGY, "mortar %ld: element out of range", i);
     if (fC < 0 || fC >= nf2 || fF < 0 || fF >= nf2) return fail(MARUT_ETOPOLOGY, "mortar %ld: face out of range", i);
     bool ok = claim(M[0], fC, (int)i, pack_info(FK_MORTAR_COARSE, fF, 0, 0));
-    for (int k = 0; k < nfine && ok; ++k) ok = claim(M[2 + k], fF, (dim == 2) ? M[0] : (int)i, pack_info(FK_MORTAR_FINE, fC, 0, k));   // 3-D: the mortar index
+    // fine side: conn.x = the coarse element (2-D; the mortar index rides in conn.y bits 10.. for the stored-flux path of the
+    // line kernel) or the mortar index (3-D)
+    if (dim == 2 && i >= (1L << 21)) return fail(MARUT_EINVAL, "more than 2^21 mortar faces");
+    for (int k = 0; k < nfine && ok; ++k)
+      ok = claim(M[2 + k], fF, (dim == 2) ? M[0] : (int)i, pack_info(FK_MORTAR_FINE, fC, 0, k) | ((dim == 2) ? (int)(i << 10) : 0));
     if (!ok) return fail(MARUT_ETOPOLOGY, "mortar %ld: face listed twice", i);
     for (int k = 0; k < nfine; ++k) mfine[i * nfine + k] = M[2 + k];
     minfo[i * 3] = M[0]; minfo[i * 3 + 1] = fC; minfo[i * 3 + 2] = fF;
@@ -408,6 +412,12 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   }
   CUDA_TRY(cudaMalloc(&m->d_mortar_fine, mfine.size() * sizeof(int)));
   CUDA_TRY(cudaMemcpy(m->d_mortar_fine, mfine.data(), mfine.size() * sizeof(int), cudaMemcpyHostToDevice));
+  if (dim == 2 && d->n_mortar > 0 && m->physics == MARUT_EULER) {
+    // the line kernel's mortar path: fluxes at the fine face nodes of every mortar, stored by mortar_flux2d_kernel
+    CUDA_TRY(cudaMalloc(&m->d_mortar_info, minfo.size() * sizeof(int)));
+    CUDA_TRY(cudaMemcpy(m->d_mortar_info, minfo.data(), minfo.size() * sizeof(int), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMalloc(&m->d_mflux, (size_t)d->n_mortar * 2 * np * m->nvar * sizeof(double)));
+  }
   if (dim == 3 && d->n_mortar > 0) {
     CUDA_TRY(cudaMalloc(&m->d_mortar_info, minfo.size() * sizeof(int)));
     CUDA_TRY(cudaMemcpy(m->d_mortar_info, minfo.data(), minfo.size() * sizeof(int), cudaMemcpyHostToDevice));
@@ -606,7 +616,11 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
             const long nres = 3L * m->num_sms;
             if (m->n_tiles_plain + m->n_tiles_mortar < nres && !force) e = cudaErrorNotSupported;
             else {
-              e = cudaSuccess;
+              // the mortar fluxes, once per mortar, ahead of the stage
+              e = launch_mortar_flux2d(m->np, u_in, m->d_metric, 1, m->d_mortar_info, m->d_mortar_fine, m->d_mortar_mat, m->gamma,
+                                       m->d_mflux, m->n_mortar, st);
+              if (e == cudaSuccess) m->launches++;
+              else return fail(MARUT_ECUDA, "mortar flux kernel: %s", cudaGetErrorString(e));
               if (m->n_tiles_plain > 0) {
                 StageParams Pa = P;
                 Pa.tile_list = m->d_tiles_plain; Pa.n_tile_list = m->n_tiles_plain; Pa.dt_next = nullptr;

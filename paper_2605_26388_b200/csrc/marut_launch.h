@@ -11,6 +11,8 @@ cudaError_t launch_stage_node2d(int np, bool affine, const StageParams &P, cudaS
 cudaError_t launch_stage_node3d(int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_mortar_flux3d(int np, const double *u, const double *metric, const int *info, const int *fine, const double *mat,
                                  double gamma, double *mflux, long n_mortar, cudaStream_t st);
+cudaError_t launch_mortar_flux2d(int np, const double *u, const double *metric, int affine, const int *info, const int *fine,
+                                 const double *mat, double gamma, double *mflux, long n_mortar, cudaStream_t st);
 cudaError_t launch_stage_split(int dim, int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_stage_ns(int dim, int np, bool affine, const StageParams &P, cudaStream_t st);
 cudaError_t launch_gradient(int dim, int np, bool affine, const GradParams &P, cudaStream_t st);

@@ -124,6 +124,85 @@ __device__ __noinline__ void node_mortar_flux_2d(const StageParams &P, long e, i
 }
 
 
+// The 2-D mortar fluxes evaluated ONCE per mortar ahead of the stage (the line kernel's path; same arithmetic as
+// node_mortar_flux_2d, in the same order): F*(U_F, P_fwd^s U_C; n_F) at the 2 n fine face nodes of every mortar,
+// mflux[m][s][a][v], outward for the fine side.  One thread per (mortar, half s, fine face node a).  info[m] = (eC, fC, fF).
+// Evaluated inside the stage kernel, every coarse face node repeated all 2 n of them in a loop of dependent loads: a tile
+// with a mortar face took 26 us (profiles/r02_launches.md).
+template <int NP>
+__global__ void __launch_bounds__(128) mortar_flux2d_kernel(const double *__restrict__ u, const double *__restrict__ metric,
+                                                            int affine, const int *__restrict__ info,
+                                                            const int *__restrict__ mortar_fine,
+                                                            const double *__restrict__ mortar_mat, double gamma, long n_mortar,
+                                                            double *__restrict__ mflux) {
+  using G = Geo<2, NP>;
+  constexpr int NVAR = 4, NN = NP * NP;
+  const long g = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n_mortar * 2 * NP) return;
+  const long m = g / (2 * NP);
+  const int r = (int)(g - m * 2 * NP), s = r / NP, a = r - s * NP;
+  const int eC = __ldg(&info[m * 3]), fC = __ldg(&info[m * 3 + 1]), fF = __ldg(&info[m * 3 + 2]);
+  const long eF = __ldg(&mortar_fine[m * 2 + s]);
+  const int pF = G::face_node(fF, a, 0), lF = fF >> 1;
+  const double sF = (fF & 1) ? 1.0 : -1.0;
+  double UF[NVAR], UC[NVAR], nF[2], FmF[NVAR], Fs[NVAR];
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) {
+    UF[v] = __ldg(u + (eF * NVAR + v) * NN + pF);
+    UC[v] = 0.0;
+  }
+#pragma unroll
+  for (int j = 0; j < NP; ++j) {
+    const double w = __ldg(&mortar_mat[(s * NP + a) * NP + j]);
+    const double *uc = u + (long)eC * NVAR * NN + G::face_node(fC, j, 0);
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) UC[v] += w * __ldg(uc + v * NN);
+  }
+#pragma unroll
+  for (int c = 0; c < 2; ++c)
+    nF[c] = sF * (affine ? __ldg(&metric[eF * 5 + lF * 2 + c]) : __ldg(&metric[(eF * 5 + lF * 2 + c) * NN + pF]));
+  const Prim<2> qF = prim_ideal<2, true>(UF, gamma);
+  const Prim<2> qC = prim_ideal<2, true>(UC, gamma);
+  flux_dot<2, 1>(UF, qF, nF, FmF);
+  rusanov<2, 1>(UF, qF, FmF, UC, qC, nF, Fs);
+#pragma unroll
+  for (int v = 0; v < NVAR; ++v) mflux[g * NVAR + v] = Fs[v];
+}
+template <int NP>
+cudaError_t launch_mortar_flux2d_t(const double *u, const double *metric, int affine, const int *info, const int *fine,
+                                   const double *mat, double gamma, double *mflux, long n_mortar, cudaStream_t st) {
+  const long n = n_mortar * 2 * NP;
+  mortar_flux2d_kernel<NP><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(u, metric, affine, info, fine, mat, gamma, n_mortar, mflux);
+  return cudaGetLastError();
+}
+// numerical flux F* (outward, own normal) at face node a0 of a 2-D mortar face from the stored fluxes: fine side (mortar
+// index in conn.y bits 10..): its own; coarse side (conn.x = mortar index): projection sum_s P_rev^s (2 (-F*_s)) in the
+// order of node_mortar_flux_2d.  Cheap enough to sit inline in the line kernel.
+template <int NP>
+__device__ __forceinline__ void node_mortar_flux_2d_stored(const StageParams &P, int a0, int2 cn, double *Fs) {
+  constexpr int NVAR = 4;
+  const int kind = cn.y & 3, sub = (cn.y >> 8) & 1;
+  if (kind == FK_MORTAR_FINE) {
+    const double *F = P.mflux + (((long)(cn.y >> 10) * 2 + sub) * NP + a0) * NVAR;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Fs[v] = __ldg(F + v);
+  } else {
+    const double *Prv = P.mortar_mat + 2 * NP * NP;
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) Fs[v] = 0.0;
+#pragma unroll
+    for (int m = 0; m < 2; ++m) {
+#pragma unroll
+      for (int a = 0; a < NP; ++a) {
+        const double w2 = -2.0 * __ldg(&Prv[(m * NP + a0) * NP + a]);
+        const double *F = P.mflux + (((long)cn.x * 2 + m) * NP + a) * NVAR;
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) Fs[v] += w2 * __ldg(F + v);
+      }
+    }
+  }
+}
+
 // 3-D 4:1 mortar faces (R21): the tensor product of the 2-D construction.  The Riemann fluxes
 // F*(U_F, U_i; n_F) at the 4 n^2 fine face nodes of every mortar are evaluated once by mortar_flux3d_kernel before the
 // stage (every coarse face node needs all of them); cn.x = mortar index on both sides, sub = s0 + 2 s1 names the half

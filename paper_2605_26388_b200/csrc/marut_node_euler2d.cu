@@ -18,4 +18,18 @@ cudaError_t launch_stage_node2d(int np, bool affine, const StageParams &P, cudaS
   }
   return cudaErrorNotSupported;
 }
+// F* at the fine face nodes of every 2-D mortar, stored ahead of the line kernel (marut_node.cuh)
+cudaError_t launch_mortar_flux2d(int np, const double *u, const double *metric, int affine, const int *info, const int *fine,
+                                 const double *mat, double gamma, double *mflux, long n_mortar, cudaStream_t st) {
+  switch (np) {
+    case 2: return launch_mortar_flux2d_t<2>(u, metric, affine, info, fine, mat, gamma, mflux, n_mortar, st);
+    case 3: return launch_mortar_flux2d_t<3>(u, metric, affine, info, fine, mat, gamma, mflux, n_mortar, st);
+    case 4: return launch_mortar_flux2d_t<4>(u, metric, affine, info, fine, mat, gamma, mflux, n_mortar, st);
+    case 5: return launch_mortar_flux2d_t<5>(u, metric, affine, info, fine, mat, gamma, mflux, n_mortar, st);
+    case 6: return launch_mortar_flux2d_t<6>(u, metric, affine, info, fine, mat, gamma, mflux, n_mortar, st);
+    case 7: return launch_mortar_flux2d_t<7>(u, metric, affine, info, fine, mat, gamma, mflux, n_mortar, st);
+    case 8: return launch_mortar_flux2d_t<8>(u, metric, affine, info, fine, mat, gamma, mflux, n_mortar, st);
+  }
+  return cudaErrorNotSupported;
+}
 }  // namespace marut

@@ -274,24 +274,10 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
   }
   const PencilFace F0 = pencil_face<DIM>(Up0, Ja, nrm, P.gamma, vn[0], pr[0], rinv[0]);
   const PencilFace F1 = pencil_face<DIM>(Up1, Ja, nrm, P.gamma, vn[NP - 1], pr[NP - 1], rinv[NP - 1]);
-  double Fs0[NVAR], Fs1[NVAR];   // mortar faces only: F* (outward) from the mortar routine
+  double Fs0[NVAR], Fs1[NVAR];   // mortar faces only: F* (outward) from the fluxes mortar_flux2d_kernel stored
   if constexpr (MORTAR && DIM == 2) {
-    if (k0 >= FK_MORTAR_FINE) {
-      double Um[NVAR], nv[DIM];
-#pragma unroll
-      for (int v = 0; v < NVAR; ++v) Um[v] = U[v][0];
-#pragma unroll
-      for (int c = 0; c < DIM; ++c) nv[c] = 0.0 - Ja[c];
-      node_mortar_flux_2d<NP>(P, e, 2 * L, a0, c0, Um, nv, Fs0);
-    }
-    if (k1 >= FK_MORTAR_FINE) {
-      double Um[NVAR], nv[DIM];
-#pragma unroll
-      for (int v = 0; v < NVAR; ++v) Um[v] = U[v][NP - 1];
-#pragma unroll
-      for (int c = 0; c < DIM; ++c) nv[c] = Ja[c];
-      node_mortar_flux_2d<NP>(P, e, 2 * L + 1, a0, c1, Um, nv, Fs1);
-    }
+    if (k0 >= FK_MORTAR_FINE) node_mortar_flux_2d_stored<NP>(P, a0, c0, Fs0);
+    if (k1 >= FK_MORTAR_FINE) node_mortar_flux_2d_stored<NP>(P, a0, c1, Fs1);
   }
 #pragma unroll
   for (int v = 0; v < NVAR; ++v) {
@@ -362,10 +348,11 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
     return P.tile_list ? (long)__ldg(&P.tile_list[i]) : i;
   };
   auto issue = [&](long k, int buf) {
+    if (k >= ntile) return;                 // (before phys(k): the tile list ends at ntile)
     const long tile = phys(k);
     long ws;
     int wl, shift;
-    if (k < ntile && window(tile, ws, wl, shift)) {
+    if (window(tile, ws, wl, shift)) {
       mbar_expect_tx(&bars[buf], (uint32_t)wl * 8u);
       bulk_load(Ub + buf * UB, P.u_in + ws, (uint32_t)wl * 8u, &bars[buf]);
     }
