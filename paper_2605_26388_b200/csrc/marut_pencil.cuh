@@ -24,7 +24,8 @@
 // mortars (those run stage_node_kernel).  2-D meshes with 2:1 mortars run as TWO launches over tile lists built at
 // marut_mesh_create: the tiles without mortar faces through the plain instantiation, the few with mortar faces through
 // the MORTAR one (with the mortar path compiled into the kernel every tile ran 63 % slower: 168 registers and a stack
-// frame; dispatching per tile inside one kernel, inlined or out of line, did not recover it).  PAPER.md:179-204, 713-725; R4-R8, R10.
+// frame; dispatching per tile inside one kernel, inlined or out of line, did not recover it).  The mortar fluxes themselves
+// are evaluated once per mortar by mortar_flux2d_kernel ahead of the stage (marut_node.cuh) and read from there.  PAPER.md:179-204, 713-725; R4-R8, R10.
 // Product code; shares nothing with oracle/.
 #pragma once
 #include "marut_node.cuh"
@@ -110,7 +111,7 @@ __device__ __forceinline__ void pencil_gather(const StageParams &P, int2 cn, int
     for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(&P.bc_state[cn.x * NVAR + v]);
   } else {
 #pragma unroll
-    for (int v = 0; v < NVAR; ++v) Up[v] = 1.0;   // mortar faces: F* comes from node_mortar_flux_2d
+    for (int v = 0; v < NVAR; ++v) Up[v] = 1.0;   // mortar faces: F* comes from node_mortar_flux_2d_stored
   }
 }
 
