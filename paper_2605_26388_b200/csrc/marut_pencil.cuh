@@ -78,7 +78,13 @@ struct PencilCfg {
   // per-tile metadata, prefetched one tile ahead: conn[ET][2d] (int2), metric[ET][d*d+1], fnorm[ET][d]
   static constexpr int NCN = ET * 2 * DIM, NMT = ET * (DIM * DIM + 1), NFN = ET * DIM;
   static constexpr int MW = NCN + NMT + NFN;         // 8-byte words of one metadata slot
-  static constexpr size_t smem_bytes = (size_t)(2 * UB + TD + 2 * MW) * sizeof(double) + 2 * sizeof(uint64_t);
+  // partial-residual buffer R: element stride ER.  2-D: padded so that the xi and the eta lines of the 128 / n elements of
+  // a tile spread over the banks (with ER = ED every half-warp hit 4 of 16; pads by brute-force count over 0..16: 2.7x
+  // fewer wavefronts for n = 4).  3-D: unpadded (n = 5 fills the shared memory three CTAs per SM leave).
+  static constexpr int RPAD = (DIM != 2) ? 0 : (NP == 2 ? 2 : NP == 3 ? 5 : NP == 4 ? 3 : NP == 5 ? 5 : NP == 6 ? 7 : NP == 7 ? 4 : 1);
+  static constexpr int ER = ED + RPAD;
+  static constexpr int RD = (ET * ER + 1) & ~1;      // doubles of the R buffer
+  static constexpr size_t smem_bytes = (size_t)(2 * UB + RD + 2 * MW) * sizeof(double) + 2 * sizeof(uint64_t);
   static_assert(ET >= 1, "a direction's lines of one element must fit one CTA");
   // CTAs per SM the shared memory allows (228 KB per SM, 1 KB reserved per CTA), at most 3
   static constexpr int MINB = (233472 / (int)(smem_bytes + 1024)) >= 3 ? 3 : ((233472 / (int)(smem_bytes + 1024)) >= 2 ? 2 : 1);
@@ -215,7 +221,7 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
     pr[m] = (P.gamma - 1.0) * (U[DIM + 1][m] - 0.5 * ke);
     vn[m] = mn * rinv[m];
   }
-  double *rl = Rs + ofs;
+  double *rl = Rs + el * C::ER + p0;
   double accE[NVAR][2];
 #pragma unroll
   for (int v = 0; v < NVAR; ++v) {
@@ -328,7 +334,7 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
   extern __shared__ __align__(16) double smem[];
   double *Ub = smem;
   double *Rs = smem + 2 * UB;
-  double *Mds = Rs + TD;
+  double *Mds = Rs + C::RD;
   uint64_t *bars = reinterpret_cast<uint64_t *>(Mds + 2 * MW);
   const int tid = threadIdx.x;
   const long ntile = P.tile_list ? P.n_tile_list : (P.ne + ET - 1) / ET;
