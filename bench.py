@@ -280,6 +280,7 @@ def measured_peaks():
 
 
 KERNELS = {"euler": "stage_pencil_kernel (fused Euler stage: persistent TMA-fed line kernel)",
+           "euler_mortar2d": "mortar_flux2d_kernel + stage_pencil_kernel plain / mortar instantiations over tile lists (fused Euler stage, 2-D mortars)",
            "euler_node": "stage_node_kernel (fused Euler stage, thread per node)",
            "euler_mortar3d": "mortar_flux3d_kernel + stage_node_kernel (fused Euler stage, 3-D mortar instantiation)",
            "split": "stage_split_kernel (fused Euler stage, split-form volume integral)",
@@ -333,7 +334,15 @@ class Workload:
             return KERNELS["split_blend" if self.sc else "split"]
         if m.dim == 3 and len(m.mortar):
             return KERNELS["euler_mortar3d"]
-        return KERNELS["euler" if self.affine else "euler_node"]
+        # the library runs the line kernel only on meshes whose tiles (128 / n^(d-1) elements) fill the device: 3 CTAs per SM
+        lines = (m.N + 1) ** (m.dim - 1)
+        ntile = -(-m.n_elem // max(1, 128 // lines))
+        sms = self.torch.cuda.get_device_properties(self.u.device).multi_processor_count
+        if self.affine and ntile >= 3 * sms:
+            if m.dim == 2 and len(m.mortar):
+                return KERNELS["euler_mortar2d"]
+            return KERNELS["euler"]
+        return KERNELS["euler_node"]
 
     def _step(self, src, ev=None):
         torch, gm, sc, stream = self.torch, self.gm, self.sc, self.torch.cuda.current_stream()
