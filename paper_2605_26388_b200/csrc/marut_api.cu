@@ -324,6 +324,11 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
         h.nu_r[i][s] = (signed char)k->nu_r[r * h.ns + s];
         h.nu_p[i][s] = (signed char)k->nu_p[r * h.ns + s];
       }
+      h.dnu_sum[i] = 0.0;
+      for (int s = 0; s < MAX_SPEC; ++s) {
+        h.dnu[i][s] = (s < h.ns) ? (double)(k->nu_p[r * h.ns + s] - k->nu_r[r * h.ns + s]) : 0.0;
+        h.dnu_sum[i] += h.dnu[i][s];
+      }
     }
     m->nsp = h.ns;
     CUDA_TRY(cudaMalloc(&m->d_mech, sizeof(MechDev)));

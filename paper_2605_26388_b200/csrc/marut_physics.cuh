@@ -351,14 +351,9 @@ __device__ inline void production_rates_listed(const MechDev &m, double T, const
   for (int r = 0; r < m.nr; ++r) {
     if (m.new_group[r]) {
       double dG = 0.0;
-      int dnu = 0;
 #pragma unroll
-      for (int s = 0; s < NSP; ++s) {
-        const int d = m.nu_p[r][s] - m.nu_r[r][s];
-        dG += d * g[s];
-        dnu += d;
-      }
-      ikc = exp(dG - dnu * lnc0);
+      for (int s = 0; s < NSP; ++s) dG += m.dnu[r][s] * g[s];
+      ikc = exp(dG - m.dnu_sum[r] * lnc0);
     }
     double pf = 1.0, pb = 1.0;
 #pragma unroll
@@ -370,7 +365,7 @@ __device__ inline void production_rates_listed(const MechDev &m, double T, const
     const double kf = m.A[r] * exp(m.b[r] * lnT - m.Ea[r] * invT);
     const double Rr = kf * (pf - ikc * pb);
 #pragma unroll
-    for (int s = 0; s < NSP; ++s) omega[s] += (double)(m.nu_p[r][s] - m.nu_r[r][s]) * Rr;
+    for (int s = 0; s < NSP; ++s) omega[s] += m.dnu[r][s] * Rr;
   }
 #pragma unroll
   for (int s = 0; s < NSP; ++s) omega[s] = m.W[s] * omega[s] * 1.0e6;
