@@ -320,6 +320,12 @@ gradient_kernel(const __grid_constant__ GradParams P) {
   G::ijk(p, q);
   double W[NW];
   if (active) {
+    // 1/J (used last) and the connectivity entries of the node's faces (used right behind the barrier) are brought
+    // towards the SM now -- prefetches hold no registers across the barrier
+    if constexpr (!AFFINE) asm volatile("prefetch.global.L2 [%0];" ::"l"(&P.metric[(e * MD + DIM * DIM) * NN + p]));
+#pragma unroll
+    for (int l = 0; l < DIM; ++l)
+      if (q[l] == 0 || q[l] == NP - 1) asm volatile("prefetch.global.L2 [%0];" ::"l"(&P.conn[e * 2 * DIM + 2 * l + ((q[l] == 0) ? 0 : 1)]));
     double U[NVAR];
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) U[v] = __ldg(P.u + (e * NVAR + v) * NN + p);

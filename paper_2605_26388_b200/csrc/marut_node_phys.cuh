@@ -236,6 +236,12 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
     const double *up = P.u_in + e * NVAR * NN + p;
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
+    // what only the last pass reads -- 1/J of curved meshes, u_n -- is brought into L2 now (prefetches hold no registers)
+    if constexpr (!AFFINE) asm volatile("prefetch.global.L2 [%0];" ::"l"(&P.metric[(e * MD + DIM * DIM) * NN + p]));
+    if (!VONLY && P.ca != 0.0) {
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.u_n + (e * NVAR + v) * NN + p));
+    }
     if constexpr (PHYS == PH_REACT) {
       pA = __ldg(&P.Taux[e * NA * NN + p]);
       aA = __ldg(&P.Taux[(e * NA + 1) * NN + p]);
