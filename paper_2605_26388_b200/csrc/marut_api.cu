@@ -41,6 +41,7 @@ struct marut_mesh {
   bool oriented = false;       // some 3-D interface has a non-trivial orientation code (R20)
   bool bc_kinds = false;       // some boundary id is an outflow / slip-wall face
   int pencil_reverse = 0;      // tile direction of the next launch of the persistent line kernel (alternates)
+  unsigned int *d_tile_ctr = nullptr;   // the line kernel's tile counter (two words, zero between launches)
   int *d_tiles_plain = nullptr, *d_tiles_mortar = nullptr;   // 2-D mortar meshes: the line kernel's tiles without / with mortar faces
   long n_tiles_plain = 0, n_tiles_mortar = 0;
   double gamma = 1.4, mu = 0.0, Pr = 0.72, kappa = 0.0;
@@ -245,7 +246,7 @@ extern "C" void marut_mesh_destroy(marut_mesh *m) {
   cudaDeviceSynchronize();
   cudaFree(m->d_metric); cudaFree(m->d_fnorm); cudaFree(m->d_conn); cudaFree(m->d_mortar_fine); cudaFree(m->d_mortar_info); cudaFree(m->d_mflux); cudaFree(m->d_mW); cudaFree(m->d_mortar_mat);
   cudaFree(m->d_Vinv); cudaFree(m->d_araw); cudaFree(m->d_subn); cudaFree(m->d_bc); cudaFree(m->d_S); cudaFree(m->d_T); cudaFree(m->d_mech); cudaFree(m->d_red);
-  cudaFree(m->d_red_next); cudaFree(m->d_tiles_plain); cudaFree(m->d_tiles_mortar);
+  cudaFree(m->d_red_next); cudaFree(m->d_tiles_plain); cudaFree(m->d_tiles_mortar); cudaFree(m->d_tile_ctr);
   if (m->h_red) cudaFreeHost(m->h_red);
   delete m;
 }
@@ -439,6 +440,8 @@ static marut_status create_impl(const marut_mesh_desc *d, marut_mesh *m) {
   CUDA_TRY(cudaMalloc(&m->d_red, 5 * sizeof(unsigned long long)));   // [0..2] marut_max_dt, [3] marut_chem_implicit, [4] marut_positivity_floor
   CUDA_TRY(cudaMallocHost(&m->h_red, 5 * sizeof(unsigned long long)));
   CUDA_TRY(cudaMalloc(&m->d_red_next, 4 * sizeof(unsigned long long)));
+  CUDA_TRY(cudaMalloc(&m->d_tile_ctr, 2 * sizeof(unsigned int)));
+  CUDA_TRY(cudaMemset(m->d_tile_ctr, 0, 2 * sizeof(unsigned int)));
   CUDA_TRY(cudaMemset(m->d_red_next, 0, 4 * sizeof(unsigned long long)));
 
   // ---- metric terms on the device
@@ -575,7 +578,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   P.bc_state = m->d_bc; P.S = m->d_S; P.Taux = m->d_T; P.mech = m->d_mech;
   P.ca = ca; P.cb = cb; P.cc = cc; P.dt_dev = dt_dev;
   P.gamma = m->gamma; P.mu = m->mu; P.kappa = m->kappa; P.inv_wb = 1.0 / m->w[0]; P.ne = m->ne; P.num_sms = m->num_sms;
-  P.visc_only = 0; P.tile_list = nullptr; P.n_tile_list = 0; P.reverse = 0; P.zero = 0;
+  P.visc_only = 0; P.tile_list = nullptr; P.n_tile_list = 0; P.reverse = 0; P.zero = 0; P.tile_ctr = nullptr;
   P.red_next = nullptr; P.dt_next = nullptr; P.cfl = 0.0; P.dx_min = m->dx_min; P.P2 = 2.0 * m->N + 1.0;
   memcpy(P.D, m->D, sizeof(P.D));
   P.mflux = m->d_mflux;
@@ -613,6 +616,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
           // one in L2); the result does not depend on the direction
           P.zero = 0;
           P.reverse = m->pencil_reverse;
+          P.tile_ctr = (m->dim == 3) ? m->d_tile_ctr : nullptr;
           const bool force = m->stage_kernel_pref == 2;
           if (m->n_mortar > 0) {
             // two launches: the tiles without mortar faces through the plain instantiation (the one with the mortar
