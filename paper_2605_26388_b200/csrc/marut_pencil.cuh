@@ -374,6 +374,11 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
     for (int i = tid; i < nel * MD; i += NT) cp_async8(dst + C::NCN + i, P.metric + e0 * MD + i);
     for (int i = tid; i < nel * DIM; i += NT) cp_async8(dst + C::NCN + C::NMT + i, P.fnorm + e0 * DIM + i);
   };
+  // Programmatic dependent launch: the launch that follows on the stream may place its CTAs as soon as this one's leave
+  // (it does the same for its own successor), and runs its prologue -- barrier set-up, the first tile's connectivity and
+  // metric terms, which no kernel writes -- while the last CTAs of this launch finish; everything a predecessor writes
+  // (state, device-resident dt, mortar fluxes, the counter words) is touched only behind griddepcontrol.wait.
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   if (tid == 0) {
     mbar_init(&bars[0], 1);
     mbar_init(&bars[1], 1);
@@ -382,6 +387,7 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
   fetch_meta(blockIdx.x, 0);
   cp_async_wait_all();
   __syncthreads();
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   if (tid == 0) {
     issue(blockIdx.x, 0);
     issue((long)blockIdx.x + gridDim.x, 1);
@@ -461,8 +467,17 @@ cudaError_t launch_stage_pencil_t(const StageParams &P, bool force, cudaStream_t
   // unless the caller insists (marut_debug_stage_kernel: the parity tests of small meshes)
   if (ntile < nres && !force) return cudaErrorNotSupported;
   const long grid = ntile < nres ? ntile : nres;
-  k<<<(unsigned)grid, C::NT, C::smem_bytes, st>>>(P);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3(C::NT);
+  cfg.dynamicSmemBytes = C::smem_bytes;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, k, P);
 }
 
 }  // namespace marut
