@@ -371,6 +371,13 @@ class Workload:
         """step j of a cycle through marut_ssprk33_step_cfl: j = 0 restarts from u0 (copy + CFL reduction), then the two
         device doubles alternate as dt_in / dt_out"""
         gm, cfl, d = self.gm, self.case.cfl, self.dts
+        if self.mesh.physics == 2:
+            # reacting mixture: marut_ssprk33_step_dt -- the step's own CFL reduction rides on the first stage's
+            # thermochemistry pass (no separate wave-speed pass)
+            if j == 0:
+                self.u.copy_(self.u0_dev)
+            gm.ssprk33_step_dt(self.u, self.ua, self.ub, cfl, d[0:1])
+            return
         if j == 0:
             self.u.copy_(self.u0_dev)
             gm.max_dt_async(self.u, cfl, d[0:1])
@@ -591,7 +598,10 @@ def run_cuda(args):
         return {"workload": workload_name(w.case), "value": aggregate_value(n_dof, K, world, r["ms_block_median"]), "unit": UNIT,
                 "ms_per_step": r["ms_block_median"] / K, "ms_per_step_min": r["ms_blocks_min"] / K, "ms_per_step_max": r["ms_blocks_max"] / K,
                 "ms_per_step_eager": r["eager_ms_block"] / K, "repeats": r["repeats"], "timed_region_ms": r["timed_region_ms"],
-                "step_replayed_as_cuda_graph": r["graph"], "fused_cfl_step": bool(r["graph"] and w.fused_step), "cfl": w.case.cfl, "restart_from_u0_every_steps": w.case.steps,
+                "step_replayed_as_cuda_graph": r["graph"], "fused_cfl_step": bool(r["graph"] and w.fused_step),
+                "step_call": (("marut_ssprk33_step_dt (the CFL reduction rides on the first stage's thermochemistry pass)" if w.mesh.physics == 2
+                               else "marut_ssprk33_step_cfl") if (r["graph"] and w.fused_step) else "marut_max_dt_async + 3 x marut_ssprk_stage_dev"),
+                "cfl": w.case.cfl, "restart_from_u0_every_steps": w.case.steps,
                 "affine": bool(w.affine), "gpu_launches_per_step": r["launches_per_block"] / K,
                 "roofline": roofline_of(w, r, r["clocks"]), "clocks": r["clocks"]}
 
@@ -628,7 +638,10 @@ def run_cuda(args):
                 "config": {"workload": main_sum["workload"], "parallelism": "replicas only" if world > 1 else "1 GPU",
                            "l2": f"inputs larger than L2 ({3 * n_dof * 8 / 1e6:.0f} MB of state buffers vs 126 MB)"
                                  if 3 * n_dof * 8 > 126e6 else "state fits L2 (launch/latency-bound case; no flush)",
-                           "step": ("marut_ssprk33_step_cfl: three fused stages, the CFL reduction of the next step inside the last "
+                           "step": ("marut_ssprk33_step_dt: three fused stage calls, the step's CFL reduction inside the first stage's "
+                                    "thermochemistry pass (dt stays on the device; every restart from u0 adds a device copy)"
+                                    if (main_sum["fused_cfl_step"] and main_sum["step_call"].startswith("marut_ssprk33_step_dt")) else
+                                    "marut_ssprk33_step_cfl: three fused stages, the CFL reduction of the next step inside the last "
                                     "stage's kernel (dt stays on the device; every restart from u0 adds a device copy and one marut_max_dt_async)"
                                     if main_sum["fused_cfl_step"] else
                                     ("marut_max_dt" if args.sync_dt else "marut_max_dt_async (dt stays on the device)")

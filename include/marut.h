@@ -246,6 +246,15 @@ marut_status marut_ssprk33_step(marut_mesh *mesh, double *u, double *const *scra
  * A non-finite or non-positive wave speed poisons dt_out with NaN (as marut_max_dt_async).  Asynchronous. */
 marut_status marut_ssprk33_step_cfl(marut_mesh *mesh, double *u, double *const *scratch, double cfl, const double *dt_in,
                                     double *dt_out, void *cuda_stream);
+/* One SSP-RK33 step that takes its own time step: dt = cfl dx_min / ((2N+1) max(|v| + a)) of the state u it starts from
+ * (eq. 17-18; = marut_max_dt(u, cfl), bit for bit) is formed on the device, left in dt_out (DEVICE
+ * double) and used by the three stages -- the composition marut_max_dt_async + marut_ssprk33_step(dt_dev) in one call.
+ * REACTING_EULER: the reduction rides on the first stage's thermochemistry pass (eos_kernel has T and the frozen sound
+ * speed of every node of u), so no separate wave-speed pass (a Newton solve per node) runs.  Other physics: the
+ * separate reduction, then the stages.  A non-finite or non-positive wave speed poisons dt_out -- and through it the new
+ * state -- with NaN.  scratch: 2 DEVICE buffers like u.  Asynchronous. */
+marut_status marut_ssprk33_step_dt(marut_mesh *mesh, double *u, double *const *scratch, double cfl, double *dt_out,
+                                   void *cuda_stream);
 marut_status marut_ssprk54_step(marut_mesh *mesh, double *u, double *const *scratch, double dt, const double *dt_dev,
                                 void *cuda_stream);
 marut_status marut_strang_step(marut_mesh *mesh, double *u, double *const *scratch, double dt, int *sweeps_out,

@@ -16,7 +16,7 @@ _STATUS = {0: "MARUT_OK", 1: "MARUT_EINVAL", 2: "MARUT_ENOMEM", 3: "MARUT_ECUDA"
 # every symbol include/marut.h declares
 SYMBOLS = ["marut_mesh_create", "marut_mesh_destroy", "marut_rhs", "marut_ssprk_stage", "marut_max_dt", "marut_max_dt_async", "marut_ssprk_stage_dev", "marut_rk_stage_dev",
            "marut_chem_source", "marut_chem_implicit", "marut_shock_indicator", "marut_rk_stage", "marut_lincomb", "marut_set_blend", "marut_set_boundary_kinds", "marut_positivity_floor", "marut_set_explicit_source", "marut_set_volume_form", "marut_get_metrics", "marut_is_affine", "marut_dx_min", "marut_launch_count", "marut_debug_rcp_sqrt", "marut_debug_stage_kernel", "marut_ssprk33_step", "marut_ssprk33_step_cfl", "marut_ssprk54_step", "marut_strang_step",
-           "marut_shock_indicator_noalloc", "marut_noalloc_max_elements", "marut_last_error"]
+           "marut_shock_indicator_noalloc", "marut_noalloc_max_elements", "marut_ssprk33_step_dt", "marut_last_error"]
 
 
 class MarutError(RuntimeError):
@@ -104,6 +104,8 @@ def lib():
         L.marut_ssprk33_step.argtypes = [vp, vp, vp, dbl, vp, vp]
         L.marut_ssprk33_step_cfl.restype = C.c_int
         L.marut_ssprk33_step_cfl.argtypes = [vp, vp, vp, dbl, vp, vp, vp]
+        L.marut_ssprk33_step_dt.restype = C.c_int
+        L.marut_ssprk33_step_dt.argtypes = [vp, vp, vp, dbl, vp, vp]
         L.marut_ssprk54_step.restype = C.c_int
         L.marut_ssprk54_step.argtypes = [vp, vp, vp, dbl, vp, vp]
         L.marut_strang_step.restype = C.c_int
@@ -248,6 +250,11 @@ def marut_ssprk33_step_cfl(h, u, ua, ub, cfl, dt_in, dt_out, stream=None):
     _check(lib().marut_ssprk33_step_cfl(h, _dev(u), _bufs((ua, ub)), float(cfl), _dev(dt_in), _dev(dt_out), _stream(stream)))
 
 
+def marut_ssprk33_step_dt(h, u, ua, ub, cfl, dt_out, stream=None):
+    """one SSP-RK33 step with its own CFL time step (formed on the device from u, left in dt_out) = marut_ssprk33_step_dt"""
+    _check(lib().marut_ssprk33_step_dt(h, _dev(u), _bufs((ua, ub)), float(cfl), _dev(dt_out), _stream(stream)))
+
+
 def marut_ssprk33_step(h, u, ua, ub, dt=0.0, dt_dev=None, stream=None):
     _check(lib().marut_ssprk33_step(h, _dev(u), _bufs((ua, ub)), float(dt), None if dt_dev is None else _dev(dt_dev), _stream(stream)))
 
@@ -371,6 +378,9 @@ class MarutMesh:
 
     def ssprk33_step_cfl(self, u, ua, ub, cfl, dt_in, dt_out, stream=None):
         marut_ssprk33_step_cfl(self.h, u, ua, ub, cfl, dt_in, dt_out, stream)
+
+    def ssprk33_step_dt(self, u, ua, ub, cfl, dt_out, stream=None):
+        marut_ssprk33_step_dt(self.h, u, ua, ub, cfl, dt_out, stream)
 
     def ssprk33_step(self, u, ua, ub, dt=0.0, dt_dev=None, stream=None):
         marut_ssprk33_step(self.h, u, ua, ub, dt, dt_dev, stream)

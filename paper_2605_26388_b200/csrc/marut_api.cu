@@ -536,12 +536,18 @@ extern "C" marut_status marut_mesh_create(const marut_mesh_desc *desc, marut_mes
 // ------------------------------------------------------------------------------------ operator / stage
 static bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
+__global__ void dt_finalize_kernel(const unsigned long long *__restrict__ red, double cfl, double dx_min, double P2, double Pr,
+                                   int ns, double *__restrict__ dt_out);
+
 // fused CFL reduction of u_out in the stage kernel (marut_ssprk33_step_cfl): requested with cfl > 0 and dt_next; *done
 // tells the caller whether the kernel that ran took it (else the caller runs marut_max_dt_async on u_out)
 struct FuseCfl {
   double cfl = 0.0;
   double *dt_next = nullptr;
   bool done = false;
+  // marut_ssprk33_step_dt, reacting mixture: the time step of THIS stage's input state, reduced inside eos_kernel and
+  // finalized into dt_now before the stage kernel (which reads it as its device-resident dt) runs
+  double *dt_now = nullptr;
 };
 
 static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc, const double *u_n, const double *u_in,
@@ -566,11 +572,24 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   if (m->physics == MARUT_REACTING_EULER) {
     const long total = m->ne * m->nn;
     const unsigned grid = (unsigned)std::min<long>((total + 255) / 256, (long)m->num_sms * 16);
-    if (m->dim == 2) eos_kernel<2, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn, m->explicit_source);
-    else eos_kernel<3, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn, m->explicit_source);
+    const bool red = fuse && fuse->dt_now;
+    if (red) CUDA_TRY(cudaMemsetAsync(m->d_red, 0, 3 * sizeof(unsigned long long), st));
+    if (m->dim == 2) {
+      if (red) eos_kernel<2, 5, true><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn, m->explicit_source, m->d_red);
+      else eos_kernel<2, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn, m->explicit_source);
+    } else {
+      if (red) eos_kernel<3, 5, true><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn, m->explicit_source, m->d_red);
+      else eos_kernel<3, 5><<<grid, 256, 0, st>>>(u_in, m->d_T, m->d_mech, m->ne, m->nn, m->explicit_source);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(MARUT_ECUDA, "eos kernel: %s", cudaGetErrorString(e));
     m->launches++;
+    if (red) {
+      dt_finalize_kernel<<<1, 1, 0, st>>>(m->d_red, fuse->cfl, m->dx_min, 2.0 * m->N + 1.0, m->Pr, 0, fuse->dt_now);
+      e = cudaGetLastError();
+      if (e != cudaSuccess) return fail(MARUT_ECUDA, "dt kernel: %s", cudaGetErrorString(e));
+      m->launches++;
+    }
   }
   StageParams P;
   P.u_in = u_in; P.u_n = u_n; P.u_out = u_out;
@@ -930,6 +949,28 @@ extern "C" marut_status marut_ssprk33_step_cfl(marut_mesh *m, double *u, double 
   if ((s = run_operator(m, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, u, ub, u, st, dt_in, &f)) != MARUT_OK) return s;
   if (!f.done) return marut_max_dt_async(m, u, cfl, dt_out, stream);   // stage kernels without the fused reduction
   return MARUT_OK;
+}
+
+extern "C" marut_status marut_ssprk33_step_dt(marut_mesh *m, double *u, double *const *scratch, double cfl, double *dt_out,
+                                              void *stream) {
+  if (marut_status s = check_step_buffers(m, u, scratch, 2); s != MARUT_OK) return s;
+  if (!dt_out) return fail(MARUT_EINVAL, "NULL argument");
+  if (!(cfl > 0.0)) return fail(MARUT_EINVAL, "cfl must be positive");
+  cudaStream_t st = (cudaStream_t)stream;
+  double *ua = scratch[0], *ub = scratch[1];
+  marut_status s;
+  if (m->physics == MARUT_REACTING_EULER) {
+    // the first stage's thermochemistry pass has T and a of u: it reduces the wave speed on the way
+    FuseCfl f;
+    f.cfl = cfl;
+    f.dt_now = dt_out;
+    if ((s = run_operator(m, 0.0, 1.0, 1.0, u, u, ua, st, dt_out, &f)) != MARUT_OK) return s;
+  } else {
+    if ((s = marut_max_dt_async(m, u, cfl, dt_out, stream)) != MARUT_OK) return s;
+    if ((s = run_operator(m, 0.0, 1.0, 1.0, u, u, ua, st, dt_out)) != MARUT_OK) return s;
+  }
+  if ((s = run_operator(m, 0.75, 0.25, 0.25, u, ua, ub, st, dt_out)) != MARUT_OK) return s;
+  return run_operator(m, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0, u, ub, u, st, dt_out);
 }
 
 extern "C" marut_status marut_ssprk54_step(marut_mesh *m, double *u, double *const *scratch, double dt, const double *dt_dev,

@@ -461,13 +461,19 @@ __device__ __forceinline__ void load_mech(MechDev *dst_s, const MechDev *src_g) 
 // explicit source is on -- the production rates omega_s (eq. 21-22).  aux[e][2 + NSP][node] = p, a, omega_1..NSP.
 // The stage kernel then needs no mechanism table, no exponentials and no Newton: it keeps the footprint of the Euler
 // stage (the chemistry is purely per node, "no inter-thread communication").
-template <int DIM, int NSP>
+// RED (marut_ssprk33_step_dt): the kernel also reduces the wave speed |v| + a of the state it evaluates into red[0]
+// (and a bad-state count into red[2]) -- wave_speed_kernel's expressions on the same T and a, so the time step that
+// dt_finalize_kernel forms from them equals marut_max_dt's bit for bit, without another pass over the state.
+template <int DIM, int NSP, bool RED = false>
 __global__ void __launch_bounds__(256, 3) eos_kernel(const double *__restrict__ u, double *__restrict__ aux,
-                                                  const MechDev *__restrict__ mech_g, long ne, int nn, int with_source) {
+                                                  const MechDev *__restrict__ mech_g, long ne, int nn, int with_source,
+                                                  unsigned long long *__restrict__ red = nullptr) {
   constexpr int NVAR = NSP + DIM + 1, NA = 2 + NSP;
   __shared__ MechDev mech;
   __shared__ double Xs[NSP * 256];           // per-thread concentration columns of production_rates_listed
   load_mech(&mech, mech_g);
+  double lam = 0.0;
+  int bad = 0;
   const long total = ne * nn;
   for (long g = (long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
     const long e = g / nn;
@@ -480,11 +486,27 @@ __global__ void __launch_bounds__(256, 3) eos_kernel(const double *__restrict__ 
     double *a = aux + e * NA * nn + p;
     a[0] = q.p;
     a[nn] = q.a;
+    if constexpr (RED) {
+      double v2 = 0.0;
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) v2 += q.v[c] * q.v[c];
+      const double l = sqrt(v2) + q.a;
+      if (!(l > 0.0) || !isfinite(l)) bad = 1;
+      lam = fmax(lam, l);
+    }
     if (with_source) {
       double om[NSP];
       production_rates_listed<NSP>(mech, T, U, Xs + threadIdx.x, 256, om);
 #pragma unroll
       for (int s = 0; s < NSP; ++s) a[(2 + s) * nn] = om[s];
+    }
+  }
+  if constexpr (RED) {
+    lam = warp_max(lam);
+    bad = __any_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0) {
+      atomicMax(&red[0], (unsigned long long)__double_as_longlong(lam));
+      if (bad) atomicAdd(&red[2], 1ULL);
     }
   }
 }

@@ -182,3 +182,46 @@ def test_step_with_fused_cfl_reduction(name, cells, which):
     with pytest.raises(mb.MarutError):
         gm.ssprk33_step_cfl(u, ua, ub, c.cfl, dts[0:1], dts[0:1])       # dt_out aliases dt_in
     gm.close()
+
+
+@pytest.mark.parametrize("name,cells", [("c1", 8), ("c2", 3), ("c3", 3), ("c4", 32), ("c5", 4), ("c5", 7)])
+def test_step_with_its_own_time_step(name, cells):
+    """marut_ssprk33_step_dt: the step forms its CFL time step from the state it starts from (for the reacting mixture
+    inside the first stage's thermochemistry pass, without a separate wave-speed pass) -- dt and the new state equal
+    marut_max_dt + marut_ssprk33 step bit for bit, three steps in a row, and the run agrees with the oracle"""
+    import torch
+
+    import oracle
+    import paper_2605_26388_b200 as mb
+
+    c = wl.make_case(name, cells=cells)
+    om, gm = oracle.OracleMesh(c.mesh), mb.MarutMesh(c.mesh)
+    u = torch.from_numpy(c.u0).cuda()
+    v = u.clone()
+    ua, ub = torch.empty_like(u), torch.empty_like(u)
+    dt_dev = torch.zeros(1, dtype=torch.float64, device=u.device)
+    uh = c.u0
+    launches = []
+    for _ in range(3):
+        dt = gm.max_dt(u, c.cfl)
+        gm.step(u, ua, ub, dt)
+        n0 = gm.launch_count
+        gm.ssprk33_step_dt(v, ua, ub, c.cfl, dt_dev)
+        launches.append(gm.launch_count - n0)
+        torch.cuda.synchronize()
+        assert dt_dev.item() == dt
+        assert torch.equal(u, v)
+        uh = om.run(uh, 1, cfl=c.cfl)[0]
+    assert parity_error(v.cpu().numpy(), uh).max() <= RUN_TOL
+    if name == "c5":
+        assert launches[0] == 7          # 3 x (eos_kernel + stage) + dt_finalize: no wave-speed pass
+    # a bad state (negative density of an ideal gas) poisons dt and the new state
+    if name != "c5":
+        bad = torch.from_numpy(c.u0).cuda()
+        bad[0, 0, 0] = -1.0
+        gm.ssprk33_step_dt(bad, ua, ub, c.cfl, dt_dev)
+        torch.cuda.synchronize()
+        assert np.isnan(dt_dev.item())
+    with pytest.raises(mb.MarutError):
+        gm.ssprk33_step_dt(v, ua, ub, 0.0, dt_dev)
+    gm.close()
