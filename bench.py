@@ -500,6 +500,9 @@ def roofline_of(w, r, clocks):
             "peak_source": peak_src, "bytes_per_dof_stage": b_alg, "stage_ms_avg": stage_ms_avg,
             "stage_ms_by_stage": [sum(r["stage_ms"][k::3]) / len(r["stage_ms"][k::3]) for k in range(3)],
             "frac_of_8TBs_nominal": achieved / 8000.0}
+    if 3 * n_dof * 8 < 126e6 and stage_ms_avg < 0.03:
+        roof["note"] = ("the state fits L2 and a stage is one launch of a few microseconds: launch-latency bound, "
+                        "neither the HBM nor the FP64 roofline applies to this size")
     if mesh.physics == 1:
         roof["single_sweep_bytes_per_dof_stage"] = single_sweep_bytes_per_dof_stage(mesh, w.affine)
         roof["frac_vs_single_sweep_bytes"] = roof["single_sweep_bytes_per_dof_stage"] * n_dof / (stage_ms_avg * 1e-3) / 1e9 / peak
