@@ -84,7 +84,16 @@ struct PencilCfg {
   static constexpr int RPAD = (DIM != 2) ? 0 : (NP == 2 ? 2 : NP == 3 ? 5 : NP == 4 ? 3 : NP == 5 ? 5 : NP == 6 ? 7 : NP == 7 ? 4 : 1);
   static constexpr int ER = ED + RPAD;
   static constexpr int RD = (ET * ER + 1) & ~1;      // doubles of the R buffer
-  static constexpr size_t smem_bytes = (size_t)(2 * UB + RD + 2 * MW) * sizeof(double) + 4 * sizeof(uint64_t);
+  // 2-D: the tile's u_n block comes in by a bulk copy of its own (one slot, issued at the start of the tile, consumed in
+  // phase 1: phase 0 hides it) -- the 2-D kernels have the shared memory for it, and loading u_n through registers, even
+  // two variables ahead, left 15 % of the samples of stages 1 and 2 on the folds' operands.  3-D: no room (n = 5).
+  // (only where the slot does not cost a CTA per SM)
+  static constexpr size_t base_bytes = (size_t)(2 * UB + RD + 2 * MW) * sizeof(double) + 4 * sizeof(uint64_t);
+  static constexpr int UNB0 = (TD + 1) & ~1;
+  static constexpr int CTAS0 = (233472 / (int)(base_bytes + 1024)) >= 3 ? 3 : (233472 / (int)(base_bytes + 1024));
+  static constexpr bool UN_SMEM = (DIM == 2) && (233472 / (int)(base_bytes + UNB0 * sizeof(double) + 1024)) >= CTAS0;
+  static constexpr int UNB = UN_SMEM ? UNB0 : 0;
+  static constexpr size_t smem_bytes = base_bytes + (size_t)UNB * sizeof(double);
   static_assert(ET >= 1, "a direction's lines of one element must fit one CTA");
   // CTAs per SM the shared memory allows (228 KB per SM, 1 KB reserved per CTA), at most 3
   static constexpr int MINB = (233472 / (int)(smem_bytes + 1024)) >= 3 ? 3 : ((233472 / (int)(smem_bytes + 1024)) >= 2 ? 2 : 1);
@@ -160,7 +169,7 @@ __device__ __forceinline__ double pencil_flux_comp(int v, const double *Up, cons
 template <int DIM, int NP, int L, bool MORTAR, bool FUSE = false>
 __device__ __forceinline__ void pencil_phase(const StageParams &P, const double *__restrict__ Ut, double *__restrict__ Rs,
                                              const double *__restrict__ Md, long e0, int nel, int t, double cc, double &lam,
-                                             int &bad) {
+                                             int &bad, const double *Un = nullptr) {
   using C = PencilCfg<DIM, NP>;
   constexpr int NVAR = C::NVAR, NN = C::NN, NL = C::NL, ED = C::ED, MD = Geo<DIM, NP>::MD;
   constexpr bool FIRST = (L == 0), LAST = (L == DIM - 1);
@@ -203,9 +212,9 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
     if (fold_un) {
       g = (0.0 - P.ca) / (cc * invJ);
 #pragma unroll
-      for (int m = 0; m < NP; ++m) unb[0][m] = __ldcs(P.u_n + gofs + m * SM);
+      for (int m = 0; m < NP; ++m) unb[0][m] = C::UN_SMEM ? 0.0 : __ldcs(P.u_n + gofs + m * SM);
 #pragma unroll
-      for (int m = 0; m < NP; ++m) unb[1][m] = __ldcs(P.u_n + gofs + NN + m * SM);
+      for (int m = 0; m < NP; ++m) unb[1][m] = C::UN_SMEM ? 0.0 : __ldcs(P.u_n + gofs + NN + m * SM);
     }
   }
   double rinv[NP], pr[NP], vn[NP];
@@ -226,7 +235,7 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
 #pragma unroll
   for (int v = 0; v < NVAR; ++v) {
     if constexpr (FOLD_HERE) {
-      if (fold_un && v + 2 < NVAR) {
+      if (!C::UN_SMEM && fold_un && v + 2 < NVAR) {
 #pragma unroll
         for (int m = 0; m < NP; ++m) unb[(v + 2) % 3][m] = __ldcs(P.u_n + gofs + (v + 2) * NN + m * SM);
       }
@@ -249,7 +258,7 @@ __device__ __forceinline__ void pencil_phase(const StageParams &P, const double 
     if constexpr (FOLD_HERE) {
       if (fold_un) {
 #pragma unroll
-        for (int i = 0; i < NP; ++i) acc[i] = fma(g, unb[v % 3][i], acc[i]);
+        for (int i = 0; i < NP; ++i) acc[i] = fma(g, C::UN_SMEM ? Un[el * ED + p0 + v * NN + i * SM] : unb[v % 3][i], acc[i]);
       }
     }
     accE[v][0] = acc[0];
@@ -335,7 +344,8 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
   double *Ub = smem;
   double *Rs = smem + 2 * UB;
   double *Mds = Rs + C::RD;
-  uint64_t *bars = reinterpret_cast<uint64_t *>(Mds + 2 * MW);
+  double *Uns = Mds + 2 * MW;                 // 2-D: the tile's u_n block (C::UNB doubles)
+  uint64_t *bars = reinterpret_cast<uint64_t *>(Uns + C::UNB);   // [0], [1]: ring slots, [2]: tile queue word, [3]: u_n slot
   const int tid = threadIdx.x;
   const long ntile = P.tile_list ? P.n_tile_list : (P.ne + ET - 1) / ET;
   const long total = P.ne * ED;
@@ -382,6 +392,7 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
   if (tid == 0) {
     mbar_init(&bars[0], 1);
     mbar_init(&bars[1], 1);
+    mbar_init(&bars[3], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   fetch_meta(blockIdx.x, 0);
@@ -403,7 +414,7 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
   // c4w +4.6 %; drawing early and publishing a phase later held a register pair across the phase: worse for both.)
   volatile long *qs = reinterpret_cast<volatile long *>(bars + 2);
   long q0 = blockIdx.x, q1 = q0 + gridDim.x, q2 = q1 + gridDim.x;
-  int it = 0;
+  int it = 0, nun = 0;
   for (; q0 < ntile; ++it) {
     const long k = q0;
     if (tid == 0) *qs = P.tile_ctr ? 3L * gridDim.x + (long)atomicAdd(&P.tile_ctr[0], 1u) : q2 + gridDim.x;
@@ -424,15 +435,26 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
       for (int i = tid; i < nel * ED; i += NT) dst[i] = __ldg(P.u_in + e0 * ED + i);
       __syncthreads();
     }
-    // u_n of this tile is read by phase 1: bring it into L2 one phase ahead (earlier, and part of it is evicted again)
-    if (tid == 0 && use_un && by_tma) bulk_prefetch_l2(P.u_n + ws, (uint32_t)wl * 8u);
+    // u_n of this tile is read by phase 1.  3-D: bring it into L2 one phase ahead (earlier, and part of it is evicted
+    // again).  2-D: into its shared-memory slot (free since the barrier that ended the previous tile).
+    const bool un_smem = C::UN_SMEM && use_un && by_tma;
+    if (tid == 0 && use_un && by_tma) {
+      if constexpr (C::UN_SMEM) {
+        mbar_expect_tx(&bars[3], (uint32_t)wl * 8u);
+        bulk_load(Uns, P.u_n + ws, (uint32_t)wl * 8u, &bars[3]);
+      } else bulk_prefetch_l2(P.u_n + ws, (uint32_t)wl * 8u);
+    }
     pencil_phase<DIM, NP, 0, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
     __syncthreads();
     if constexpr (DIM == 3) {
       pencil_phase<DIM, NP, 1, MORTAR>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
       __syncthreads();
     }
-    pencil_phase<DIM, NP, DIM - 1, MORTAR, FUSE>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad);
+    if constexpr (C::UN_SMEM) {
+      if (un_smem) mbar_wait(&bars[3], (uint32_t)(nun & 1));
+    }
+    pencil_phase<DIM, NP, DIM - 1, MORTAR, FUSE>(P, Ut, Rs, Md, e0, nel, tid, cc, lam, bad, Uns);
+    if (un_smem) ++nun;
     cp_async_wait_all();
     const long qn = *qs;                    // (written by thread 0 at the top of the iteration, barriers in between)
     __syncthreads();
