@@ -119,7 +119,7 @@ __device__ __forceinline__ void pencil_gather(const StageParams &P, int2 cn, int
     } else {
       const double *un = P.u_in + (long)cn.x * NVAR * NN + node;
 #pragma unroll
-      for (int v = 0; v < NVAR; ++v) Up[v] = __ldg(un + v * NN);
+      for (int v = 0; v < NVAR; ++v) Up[v] = __ldcg(un + v * NN);
     }
   } else if (kind == FK_BOUNDARY) {
 #pragma unroll
