@@ -7,7 +7,10 @@
 //            issues the copy for the tile after next when the current tile is finished.  N = 4 in 3-D has 5000-byte
 //            elements: the 16-byte window the copy needs is obtained by starting one double early (`shift`).
 //            The tile's connectivity and metric terms come in by 8-byte cp.async one tile ahead; u_n of the tile is
-//            L2-prefetched (cp.async.bulk.prefetch.L2) at the start of the tile, one phase before it is read.
+//            L2-prefetched (cp.async.bulk.prefetch.L2) at the start of the tile, one phase before it is read (3-D), or
+//            brought into a shared-memory slot of its own by a second bulk copy (2-D, which has the room).
+//            Tiles: the first three of a CTA round-robin, then (3-D) drawn from a device-wide counter.  Launches are
+//            programmatic dependents of their stream predecessor (the prologue overlaps its tail).
 //   phase l (l = 0 .. d-1): the thread owns the line of direction l through (a0, a1): it reads the line's U from the
 //            tile, evaluates the contravariant flux Ftilde^l (eq. 9) at its n nodes, applies D along the line in
 //            registers, and -- because the line's two end nodes ARE the face nodes (a0, a1) of faces 2l and 2l+1 --
@@ -25,7 +28,8 @@
 // marut_mesh_create: the tiles without mortar faces through the plain instantiation, the few with mortar faces through
 // the MORTAR one (with the mortar path compiled into the kernel every tile ran 63 % slower: 168 registers and a stack
 // frame; dispatching per tile inside one kernel, inlined or out of line, did not recover it).  The mortar fluxes themselves
-// are evaluated once per mortar by mortar_flux2d_kernel ahead of the stage (marut_node.cuh) and read from there.  PAPER.md:179-204, 713-725; R4-R8, R10.
+// are evaluated once per mortar by mortar_flux2d_kernel ahead of the stage (marut_node.cuh) and read from there.
+// PAPER.md:179-204, 713-725; R4-R8, R10.
 // Product code; shares nothing with oracle/.
 #pragma once
 #include "marut_node.cuh"
