@@ -225,3 +225,48 @@ def test_step_with_its_own_time_step(name, cells):
     with pytest.raises(mb.MarutError):
         gm.ssprk33_step_dt(v, ua, ub, 0.0, dt_dev)
     gm.close()
+
+
+@pytest.mark.parametrize("name,cells,steps_fn", [("c2", 6, "cfl"), ("c4", 32, "cfl"), ("c1", 16, "cfl"), ("c5", 4, "dt")])
+def test_library_steps_of_the_line_kernel_in_a_cuda_graph(name, cells, steps_fn):
+    """the whole-step entry points captured in a CUDA graph with the persistent line kernel forced (its launches are
+    programmatic dependents of their stream predecessor, its tiles come from tile lists on 2-D mortar meshes, and the
+    fused CFL reduction is finalised by the last launch): replayed, they advance the solution exactly as the eager calls"""
+    import torch
+
+    import paper_2605_26388_b200 as mb
+
+    c = wl.make_case(name, cells=cells)
+    gm = mb.MarutMesh(c.mesh)
+    if c.mesh.physics == wl.EULER:
+        gm.debug_stage_kernel(2)
+    u = torch.from_numpy(c.u0).cuda()
+    v = u.clone()
+    ua, ub = torch.empty_like(u), torch.empty_like(u)
+    d = torch.zeros(2, dtype=torch.float64, device=u.device)
+
+    def two_steps(w):
+        if steps_fn == "cfl":
+            gm.ssprk33_step_cfl(w, ua, ub, c.cfl, d[0:1], d[1:2])
+            gm.ssprk33_step_cfl(w, ua, ub, c.cfl, d[1:2], d[0:1])
+        else:
+            gm.ssprk33_step_dt(w, ua, ub, c.cfl, d[0:1])
+            gm.ssprk33_step_dt(w, ua, ub, c.cfl, d[1:2])
+
+    gm.max_dt_async(u, c.cfl, d[0:1])
+    for _ in range(3):
+        two_steps(u)
+    torch.cuda.synchronize()
+    dt_eager = d.clone()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        two_steps(v)
+    v.copy_(torch.from_numpy(c.u0))
+    gm.max_dt_async(v, c.cfl, d[0:1])
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(u, v) and torch.equal(d, dt_eager)
+    assert torch.isfinite(d).all() and (d > 0).all()
+    del graph
+    gm.close()
