@@ -44,6 +44,9 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   uint32_t ok;
   do {
@@ -435,6 +438,10 @@ __global__ void __launch_bounds__(PencilCfg<DIM, NP>::NT, PencilCfg<DIM, NP>::MI
     if (by_tma) {
       mbar_wait(&bars[buf], (uint32_t)((it >> 1) & 1));
     } else {
+      // A tile that comes in without TMA (the last one of an odd-sized array, which a reversed or counter-drawn walk
+      // meets early) still completes one phase of its slot's barrier, so that the parity of the slot's later waits
+      // follows from `it` alone (the next wait on this slot lies two iterations, several barriers, ahead).
+      if (tid == 0) mbar_arrive(&bars[buf]);
       double *dst = Ub + buf * UB + shift;
       for (int i = tid; i < nel * ED; i += NT) dst[i] = __ldg(P.u_in + e0 * ED + i);
       __syncthreads();

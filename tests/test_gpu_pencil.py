@@ -64,6 +64,16 @@ def test_ring_wraps_and_ragged_tail_3d_n4():
     _compare(m, wl.taylor_green(m, noise=1e-3), steps=2)
 
 
+@pytest.mark.parametrize("N,cells", [(4, 19), (2, 27)])
+def test_tiles_drawn_from_the_device_counter_3d(N, cells):
+    # more than three tiles per resident CTA (444 CTAs): beyond its first three tiles a CTA draws the rest from the
+    # device-wide counter, which the last CTA to finish resets (N = 4: 19^3 = 6859 elements = 1372 tiles, odd-sized
+    # array: the last tile without TMA; N = 2: 27^3 = 19683 elements = 1406 tiles of 14); RHS, the three stage kinds and
+    # two steps run back to back on one handle, so every launch relies on the reset of the one before
+    m = wl.cartesian_mesh(3, N, (cells,) * 3, (0.0,) * 3, (2 * math.pi,) * 3)
+    _compare(m, wl.taylor_green(m, noise=1e-3), steps=2)
+
+
 def test_odd_sized_array_last_tile_without_tma_3d_n4():
     # 11^3 = 1331 elements: 1331 * 625 doubles is odd: the last tile's 16-byte window would leave the array
     m = wl.cartesian_mesh(3, 4, (11,) * 3, (0.0,) * 3, (2 * math.pi,) * 3)
