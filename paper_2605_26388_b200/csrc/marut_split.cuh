@@ -50,6 +50,14 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
   const long e0 = (long)blockIdx.x * EB;
   const int nel = (int)((P.ne - e0 < EB) ? (P.ne - e0) : EB);
   const int ntask = nel * NFN;
+  // L2 prefetch of the state (curved: and metric) planes of the block about half a wave ahead, as in stage_phys_kernel
+  if (tid == 0) {
+    const long ep = e0 + (long)(74 * MINB) * EB;
+    if (ep + EB < P.ne) {
+      l2_prefetch(P.u_in + ep * NVAR * NN, (size_t)EB * NVAR * NN * sizeof(double));
+      if constexpr (!AFFINE) l2_prefetch(P.metric + ep * MD * NN, (size_t)EB * MD * NN * sizeof(double));
+    }
+  }
   const bool has0 = tid < ntask;
   const FaceTask t0 = decode_task<DIM, NP>(has0 ? tid : 0);
   int2 cn0 = make_int2(0, FK_BOUNDARY);
