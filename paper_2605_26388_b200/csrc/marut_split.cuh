@@ -79,6 +79,12 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
     const double *up = P.u_in + e * NVAR * NN + p;
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) U[v] = __ldg(up + v * NN);
+    // u_n, read by the combination at the kernel's end, and 1/J of a curved mesh: into L2 now (no registers held)
+    if (P.ca != 0.0) {
+#pragma unroll
+      for (int v = 0; v < NVAR; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.u_n + (e * NVAR + v) * NN + p));
+    }
+    if constexpr (!AFFINE) asm volatile("prefetch.global.L2 [%0];" ::"l"(&P.metric[(e * MD + DIM * DIM) * NN + p]));
     const Prim<DIM> pr = prim_ideal<DIM, true>(U, P.gamma);
 #pragma unroll
     for (int c = 0; c < DIM; ++c) vi[c] = pr.v[c];
