@@ -40,7 +40,7 @@ struct marut_mesh {
   int n_bc = 0;
   bool oriented = false;       // some 3-D interface has a non-trivial orientation code (R20)
   bool bc_kinds = false;       // some boundary id is an outflow / slip-wall face
-  int pencil_reverse = 0;      // tile direction of the next launch of the persistent line kernel (alternates)
+  int pencil_reverse = 0;      // tile / block direction of the next launch of the line kernel or the split-form kernel (alternates)
   unsigned int *d_tile_ctr = nullptr;   // the line kernel's tile counter (two words, zero between launches)
   int *d_tiles_plain = nullptr, *d_tiles_mortar = nullptr;   // 2-D mortar meshes: the line kernel's tiles without / with mortar faces
   long n_tiles_plain = 0, n_tiles_mortar = 0;
@@ -624,7 +624,13 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
   cudaError_t e;
   switch (m->physics) {
     case MARUT_EULER:
-      if (m->volume_form == MARUT_VOLUME_SPLIT_RANOCHA) e = launch_stage_split(m->dim, m->np, m->affine, P, st);
+      if (m->volume_form == MARUT_VOLUME_SPLIT_RANOCHA) {
+        // consecutive launches walk the element blocks in opposite directions, like the line kernel's tiles: a stage
+        // starts on the end of the state its predecessor wrote last
+        P.reverse = m->pencil_reverse;
+        e = launch_stage_split(m->dim, m->np, m->affine, P, st);
+        if (e == cudaSuccess) m->pencil_reverse ^= 1;
+      }
       else {
         // affine meshes with conforming / prescribed-state / 2-D mortar faces: the persistent TMA-fed line kernel;
         // curved meshes, outflow / slip-wall faces and 3-D mortars: the thread-per-node kernel
@@ -674,6 +680,7 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
       }
       break;
     case MARUT_NAVIER_STOKES:
+      P.reverse = 1;              // stage_phys_kernel walks against the gradient sweep (L2 reuse at both ends)
       if (m->volume_form == MARUT_VOLUME_SPLIT_RANOCHA) {
         // hyperbolic part with the split-form (and blended) volume integral, then the parabolic part added to u_out
         // (the two pipelines add their contributions into one residual)
@@ -690,7 +697,10 @@ static marut_status run_operator(marut_mesh *m, double ca, double cb, double cc,
         e = launch_stage_ns(m->dim, m->np, m->affine, P, st);
       } else e = launch_stage_ns(m->dim, m->np, m->affine, P, st);
       break;
-    default: e = launch_stage_react(m->dim, m->np, m->nsp, m->affine, P, st); break;
+    default:
+      P.reverse = 1;              // against eos_kernel's sweep over the nodes
+      e = launch_stage_react(m->dim, m->np, m->nsp, m->affine, P, st);
+      break;
   }
   if (e == cudaErrorNotSupported) return fail(MARUT_EINVAL, "no kernel instantiated for dim=%d N=%d physics=%d", m->dim, m->N, m->physics);
   if (e != cudaSuccess) return fail(MARUT_ECUDA, "stage kernel: %s", cudaGetErrorString(e));

@@ -211,7 +211,10 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   double *Msm = Lft + NVAR * NTASK;                // affine: [EB][MDP] Ja, 1/J, |Ja^l|
 
   const int tid = threadIdx.x;
-  const long e0 = (long)blockIdx.x * EB;
+  // P.reverse (Navier-Stokes: set by the library): the blocks are walked from the last element to the first, against the
+  // direction of the gradient sweep ahead of this launch -- it starts on the stress planes that sweep wrote last (still
+  // in L2) and ends where the next stage's gradient sweep starts reading u_out
+  const long e0 = (P.reverse ? (long)gridDim.x - 1 - (long)blockIdx.x : (long)blockIdx.x) * EB;
   const int nel = (int)((P.ne - e0 < EB) ? (P.ne - e0) : EB);
   const int ntask = nel * NFN, nline = nel * NLT;
 
@@ -220,8 +223,8 @@ stage_phys_kernel(const __grid_constant__ StageParams P) {
   // Measured (c5, ms per step): none 1.751, 148 * MINB blocks ahead 1.682, 74 * MINB 1.678, 296 * MINB 1.712, with u_n
   // as well 1.687; c3 (power-capped, DRAM-side) does not move with any of them.
   if (tid == 0) {
-    const long ep = e0 + (long)(74 * MINB) * EB;
-    if (ep + EB < P.ne) {
+    const long ep = e0 + (P.reverse ? -1L : 1L) * (74 * MINB) * EB;
+    if (ep >= 0 && ep + EB < P.ne) {
       l2_prefetch(P.u_in + ep * NVAR * NN, (size_t)EB * NVAR * NN * sizeof(double));
       if constexpr (PHYS == PH_NS) l2_prefetch(P.S + ep * Tau<DIM>::NTAU * NN, (size_t)EB * Tau<DIM>::NTAU * NN * sizeof(double));
       if constexpr (!AFFINE) l2_prefetch(P.metric + ep * MD * NN, (size_t)EB * MD * NN * sizeof(double));

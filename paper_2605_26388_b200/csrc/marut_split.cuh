@@ -47,13 +47,13 @@ stage_split_kernel(const __grid_constant__ StageParams P) {
   double *Msm = Lft + NVAR * C::LFS;        // affine: [EB][MDP] Ja, 1/J, |Ja^l|
 
   const int tid = threadIdx.x;
-  const long e0 = (long)blockIdx.x * EB;
+  const long e0 = (P.reverse ? (long)gridDim.x - 1 - (long)blockIdx.x : (long)blockIdx.x) * EB;   // (see stage_phys_kernel)
   const int nel = (int)((P.ne - e0 < EB) ? (P.ne - e0) : EB);
   const int ntask = nel * NFN;
   // L2 prefetch of the state (curved: and metric) planes of the block about half a wave ahead, as in stage_phys_kernel
   if (tid == 0) {
-    const long ep = e0 + (long)(74 * MINB) * EB;
-    if (ep + EB < P.ne) {
+    const long ep = e0 + (P.reverse ? -1L : 1L) * (74 * MINB) * EB;
+    if (ep >= 0 && ep + EB < P.ne) {
       l2_prefetch(P.u_in + ep * NVAR * NN, (size_t)EB * NVAR * NN * sizeof(double));
       if constexpr (!AFFINE) l2_prefetch(P.metric + ep * MD * NN, (size_t)EB * MD * NN * sizeof(double));
     }
